@@ -1,0 +1,553 @@
+// oracle/tso.cpp -- CPU ORACLE (test infrastructure, NOT the product; see oracle/tso.h).
+//
+// Plain, slow, single-threaded restatement of the Triangle Splatting SLAM rasteriser:
+//   Eq. 1   v_I = pi(T_CW v_W)                         -> project()
+//   Eq. 2   phi(p) = max_i L_i(p), outward unit normals -> face_setup(), eval()
+//   Eq. 3   I(p) = ReLU(phi(p)/phi(s))^sigma            -> eval()
+//   :82                      barycentric vertex colour, mean vertex opacity
+//   Eq. 4 front-to-back compositing in depth order    -> render_fwd()
+//   Eq. 5-7 analytic se(3) pose Jacobian              -> project_bwd()
+// Step names F1..F8 / B1..B9 and readings S1..S24 / N1..N5 refer to DESIGN.md section 3.
+// Build: g++ -std=c++17 -O2 -ffp-contract=off (no implicit FMA contraction; the float32
+// projection uses explicit std::fma where N1..N3 say so).
+#include "tso.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+template <class T>
+struct Cam {
+    int W, H;
+    T fx, fy, cx, cy, znear;
+    explicit Cam(const tso_camera* c)
+        : W(c->width), H(c->height), fx((T)c->fx), fy((T)c->fy), cx((T)c->cx), cy((T)c->cy), znear((T)c->znear) {}
+};
+
+inline int vid(const int32_t* faces, int m, int k) { return faces ? faces[3 * m + k] : 3 * m + k; }
+
+template <class T> inline T third();
+template <> inline float third<float>() { return 1.0f / 3.0f; }
+template <> inline double third<double>() { return 1.0 / 3.0; }
+
+// N3: signed doubled area of the screen triangle, S = fma(a, b, -(c*d)).
+template <class T>
+inline T signed_area(const T u[3], const T v[3]) {
+    T a = u[1] - u[0], b = v[2] - v[0], c = v[1] - v[0], d = u[2] - u[0];
+    T cd = c * d;
+    return std::fma(a, b, -cd);
+}
+
+// ---------------------------------------------------------------------------------- F1..F6
+template <class T>
+int64_t project(const T* pos, const int32_t* faces, int32_t M, const T* Tcw, const tso_camera* cam_,
+                const tso_params* prm, uint8_t* visible, int16_t* rect, uint32_t* depth_key,
+                uint32_t* tiles_touched, T* scr, T* Q, T* zbar) {
+    const Cam<T> cam(cam_);
+    const T eps_area = (T)prm->eps_area;
+    const T area_max = (T)1e10;
+    int64_t nvis = 0;
+    for (int m = 0; m < M; ++m) {
+        visible[m] = 0;
+        tiles_touched[m] = 0;
+        depth_key[m] = 0;
+        zbar[m] = 0;
+        for (int j = 0; j < 4; ++j) rect[4 * m + j] = 0;
+        for (int j = 0; j < 9; ++j) scr[9 * m + j] = 0, Q[9 * m + j] = 0;
+        T X[3], Y[3], Z[3], u[3], v[3], w[3];
+        for (int k = 0; k < 3; ++k) {
+            const T* p = pos + 3 * (int64_t)vid(faces, m, k);
+            // F1 / N1: Q = R p + t, innermost term first.
+            X[k] = std::fma(Tcw[0], p[0], std::fma(Tcw[1], p[1], std::fma(Tcw[2], p[2], Tcw[3])));
+            Y[k] = std::fma(Tcw[4], p[0], std::fma(Tcw[5], p[1], std::fma(Tcw[6], p[2], Tcw[7])));
+            Z[k] = std::fma(Tcw[8], p[0], std::fma(Tcw[9], p[1], std::fma(Tcw[10], p[2], Tcw[11])));
+        }
+        // F2: near cull, written so NaN culls.
+        if (!(Z[0] > cam.znear) || !(Z[1] > cam.znear) || !(Z[2] > cam.znear)) continue;
+        for (int k = 0; k < 3; ++k) {
+            // F3 / N2: w = 1/Z (IEEE), X*w rounded separately, then one fma.
+            w[k] = (T)1 / Z[k];
+            T xw = X[k] * w[k], yw = Y[k] * w[k];
+            u[k] = std::fma(cam.fx, xw, cam.cx);
+            v[k] = std::fma(cam.fy, yw, cam.cy);
+        }
+        // F4 / N3: degenerate cull.
+        T S = signed_area(u, v);
+        T aS = std::fabs(S);
+        if (!(aS > eps_area) || !(aS < area_max)) continue;
+        // F5 / N4: integer pixel centres inside the vertex AABB, clipped to the image.
+        T umin = std::fmin(u[0], std::fmin(u[1], u[2])), umax = std::fmax(u[0], std::fmax(u[1], u[2]));
+        T vmin = std::fmin(v[0], std::fmin(v[1], v[2])), vmax = std::fmax(v[0], std::fmax(v[1], v[2]));
+        int x0 = (int)std::fmin(std::fmax(std::ceil(umin), (T)0), (T)cam.W);
+        int x1 = (int)std::fmin(std::fmax(std::floor(umax), (T)-1), (T)(cam.W - 1));
+        int y0 = (int)std::fmin(std::fmax(std::ceil(vmin), (T)0), (T)cam.H);
+        int y1 = (int)std::fmin(std::fmax(std::floor(vmax), (T)-1), (T)(cam.H - 1));
+        if (x0 > x1 || y0 > y1) continue;
+        // F6 / N5: depth key = bits of the float32 mean camera depth.
+        T zb = ((Z[0] + Z[1]) + Z[2]) * third<T>();
+        float zf = (float)zb;
+        uint32_t bits;
+        std::memcpy(&bits, &zf, 4);
+        visible[m] = 1;
+        rect[4 * m + 0] = (int16_t)x0, rect[4 * m + 1] = (int16_t)y0;
+        rect[4 * m + 2] = (int16_t)x1, rect[4 * m + 3] = (int16_t)y1;
+        depth_key[m] = bits;
+        zbar[m] = zb;
+        tiles_touched[m] = (uint32_t)(((x1 >> 4) - (x0 >> 4) + 1) * ((y1 >> 4) - (y0 >> 4) + 1));
+        for (int k = 0; k < 3; ++k) {
+            scr[9 * m + 3 * k + 0] = u[k], scr[9 * m + 3 * k + 1] = v[k], scr[9 * m + 3 * k + 2] = w[k];
+            Q[9 * m + 3 * k + 0] = X[k], Q[9 * m + 3 * k + 1] = Y[k], Q[9 * m + 3 * k + 2] = Z[k];
+        }
+        ++nvis;
+    }
+    return nvis;
+}
+
+// ---------------------------------------------------------------------------------- F7
+template <class T>
+struct Face {
+    T qx[3], qy[3], w[3];   // screen vertices and inverse depths
+    T nx[3], ny[3];         // outward unit normal of edge k (opposite vertex k)
+    T ell[3], h[3];         // edge length, altitude of vertex k
+    T r, absS, sumell;      // inradius = -phi(s), |S|, perimeter
+    T obar;                 // face opacity = mean of vertex opacities (:82)
+    T col[3][3];            // vertex colours
+    int x0, y0, x1, y1;
+};
+
+template <class T>
+void face_setup(Face<T>& f, const T* scr9, const int16_t* rc, const T* color, const T* opacity, const int32_t* faces,
+                int m) {
+    for (int k = 0; k < 3; ++k) f.qx[k] = scr9[3 * k], f.qy[k] = scr9[3 * k + 1], f.w[k] = scr9[3 * k + 2];
+    T S = signed_area(f.qx, f.qy);
+    T s = S > 0 ? (T)1 : (T)-1;
+    f.absS = std::fabs(S);
+    f.sumell = 0;
+    for (int k = 0; k < 3; ++k) {
+        int a = (k + 1) % 3, b = (k + 2) % 3;   // edge k runs from q_{k+1} to q_{k+2}
+        T ex = f.qx[b] - f.qx[a], ey = f.qy[b] - f.qy[a];
+        f.ell[k] = std::sqrt(ex * ex + ey * ey);
+        f.nx[k] = s * ey / f.ell[k];
+        f.ny[k] = -s * ex / f.ell[k];
+        f.h[k] = f.absS / f.ell[k];
+        f.sumell += f.ell[k];
+    }
+    f.r = f.absS / f.sumell;
+    T osum = 0;
+    for (int k = 0; k < 3; ++k) {
+        int v = vid(faces, m, k);
+        osum += opacity[v];
+        for (int c = 0; c < 3; ++c) f.col[k][c] = color[3 * (int64_t)v + c];
+    }
+    f.obar = osum / (T)3;
+    f.x0 = rc[0], f.y0 = rc[1], f.x1 = rc[2], f.y1 = rc[3];
+}
+
+// ---------------------------------------------------------------------------------- F8.1-4
+template <class T>
+struct Hit {
+    T L[3], x, I, alpha, b[3], om[3], Om, lam[3], z, c[3];
+    int kstar;
+};
+
+// returns 0 = no contribution, 1 = contributes.  *amb set if the alpha_min decision is within amb_tol.
+template <class T>
+inline int eval(const Face<T>& f, T px, T py, T sigma, T alpha_min, T amb_tol, Hit<T>& h, bool* amb) {
+    for (int k = 0; k < 3; ++k) {
+        int a = (k + 1) % 3;
+        h.L[k] = f.nx[k] * (px - f.qx[a]) + f.ny[k] * (py - f.qy[a]);   // Eq. 2, relative to a vertex (S6)
+    }
+    h.kstar = 0;
+    T phi = h.L[0];
+    for (int k = 1; k < 3; ++k)
+        if (h.L[k] > phi) phi = h.L[k], h.kstar = k;
+    h.x = -phi / f.r;                       // phi(p)/phi(s), phi(s) = -r
+    if (!(h.x > 0)) return 0;               // ReLU (Eq. 3)
+    h.I = std::pow(h.x, sigma);
+    h.alpha = f.obar * h.I;
+    if (amb && amb_tol > 0 && alpha_min > 0 && std::fabs(h.alpha - alpha_min) <= amb_tol * alpha_min) *amb = true;
+    if (h.alpha < alpha_min) return 0;      // S7
+    for (int k = 0; k < 3; ++k) {
+        h.b[k] = -h.L[k] / f.h[k];          // screen-space barycentrics
+        h.om[k] = h.b[k] * f.w[k];          // perspective correction (S10)
+    }
+    h.Om = (h.om[0] + h.om[1]) + h.om[2];
+    h.z = (T)1 / h.Om;
+    for (int k = 0; k < 3; ++k) h.lam[k] = h.om[k] / h.Om;
+    for (int c = 0; c < 3; ++c) h.c[c] = h.lam[0] * f.col[0][c] + h.lam[1] * f.col[1][c] + h.lam[2] * f.col[2][c];
+    return 1;
+}
+
+template <class T>
+struct Lists {
+    const uint32_t* list;
+    int64_t n_list;
+    const uint32_t* ranges;   // NULL = brute
+    int tiles_x;
+    inline void span(int x, int y, int64_t& b, int64_t& e) const {
+        if (!ranges) { b = 0, e = n_list; return; }
+        int t = (y >> 4) * tiles_x + (x >> 4);
+        b = ranges[2 * t], e = ranges[2 * t + 1];
+    }
+};
+
+// set-up every visible face once (the per-face constants do not depend on the pixel)
+template <class T>
+std::vector<Face<T>> setup_all(const T* color, const T* opacity, const int32_t* faces, int32_t M,
+                               const uint8_t* visible, const int16_t* rect, const T* scr) {
+    std::vector<Face<T>> F((size_t)M);
+    for (int m = 0; m < M; ++m)
+        if (visible[m]) face_setup(F[m], scr + 9 * (int64_t)m, rect + 4 * (int64_t)m, color, opacity, faces, m);
+    return F;
+}
+
+// ---------------------------------------------------------------------------------- F8.5-6
+template <class T>
+void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t M, const tso_camera* cam_,
+                const tso_params* prm, const uint8_t* visible, const int16_t* rect, const T* scr,
+                const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, T* oc, T* od, T* oa,
+                uint32_t* n_contrib, uint8_t* ambig, uint64_t* sig, uint64_t* counters) {
+    const Cam<T> cam(cam_);
+    const int W = cam.W, H = cam.H;
+    const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min, atol = (T)prm->amb_tol;
+    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr);
+    Lists<T> LS{list, n_list, tile_ranges, (W + 15) / 16};
+    uint64_t n_visit = 0, n_rect = 0, n_hit = 0;
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            int64_t b, e;
+            LS.span(x, y, b, e);
+            T Tr = 1, C[3] = {0, 0, 0}, D = 0;
+            uint32_t last = 0;
+            bool amb = false;
+            uint64_t sg = 1469598103934665603ull;
+            for (int64_t i = b; i < e; ++i) {
+                const Face<T>& f = F[list[i]];
+                ++n_visit;
+                if (x < f.x0 || x > f.x1 || y < f.y0 || y > f.y1) continue;   // rect is part of the hit rule (S5)
+                ++n_rect;
+                Hit<T> h;
+                if (!eval(f, (T)x, (T)y, sigma, amin, atol, h, &amb)) continue;
+                ++n_hit;
+                T wgt = Tr * h.alpha;                                          // Eq. 4
+                for (int c = 0; c < 3; ++c) C[c] += wgt * h.c[c];
+                D += wgt * h.z;                                                // S11
+                Tr = Tr * ((T)1 - h.alpha);
+                last = (uint32_t)(i - b + 1);
+                sg = (sg ^ (uint64_t)(list[i] + 1)) * 1099511628211ull;
+                if (atol > 0 && tmin > 0 && std::fabs(Tr - tmin) <= atol * tmin) amb = true;
+                if (Tr <= tmin) break;                                         // S12: include, then test
+            }
+            int64_t p = (int64_t)y * W + x;
+            for (int c = 0; c < 3; ++c) oc[(int64_t)c * W * H + p] = C[c];
+            od[p] = D;
+            oa[p] = (T)1 - Tr;
+            if (n_contrib) n_contrib[p] = last;
+            if (ambig) ambig[p] = amb ? 1 : 0;
+            if (sig) sig[p] = sg;
+        }
+    if (counters) counters[0] = n_visit, counters[1] = n_rect, counters[2] = n_hit, counters[3] = 0;
+}
+
+// ---------------------------------------------------------------------------------- B1..B6
+template <class T>
+void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t M, const tso_camera* cam_,
+                const tso_params* prm, const uint8_t* visible, const int16_t* rect, const T* scr,
+                const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, const T* gCi, const T* gDi,
+                const T* gAi, T* grad_color, T* grad_opacity, T* g_scr) {
+    const Cam<T> cam(cam_);
+    const int W = cam.W, H = cam.H;
+    const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min;
+    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr);
+    Lists<T> LS{list, n_list, tile_ranges, (W + 15) / 16};
+    struct Rec { uint32_t m; T Tn; };
+    std::vector<Rec> hits;
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            int64_t p = (int64_t)y * W + x;
+            T gC[3] = {0, 0, 0}, gD = 0, gA = 0;
+            if (gCi) for (int c = 0; c < 3; ++c) gC[c] = gCi[(int64_t)c * W * H + p];
+            if (gDi) gD = gDi[p];
+            if (gAi) gA = gAi[p];
+            // forward walk, remembering the transmittance in front of every contributing face
+            int64_t b, e;
+            LS.span(x, y, b, e);
+            hits.clear();
+            T Tr = 1;
+            Hit<T> h;
+            for (int64_t i = b; i < e; ++i) {
+                const Face<T>& f = F[list[i]];
+                if (x < f.x0 || x > f.x1 || y < f.y0 || y > f.y1) continue;
+                if (!eval(f, (T)x, (T)y, sigma, amin, (T)0, h, nullptr)) continue;
+                hits.push_back({list[i], Tr});
+                Tr = Tr * ((T)1 - h.alpha);
+                if (Tr <= tmin) break;
+            }
+            // reverse walk; R* = what is composited BEHIND the current face with unit transmittance
+            T Rc[3] = {0, 0, 0}, Rd = 0, Ra = 0;
+            for (int64_t j = (int64_t)hits.size() - 1; j >= 0; --j) {
+                const uint32_t m = hits[j].m;
+                const Face<T>& f = F[m];
+                const T Tn = hits[j].Tn;
+                eval(f, (T)x, (T)y, sigma, amin, (T)0, h, nullptr);
+                const T wgt = Tn * h.alpha;
+                // B1: vertex colours
+                if (grad_color)
+                    for (int k = 0; k < 3; ++k)
+                        for (int c = 0; c < 3; ++c)
+                            grad_color[3 * (int64_t)vid(faces, m, k) + c] += h.lam[k] * wgt * gC[c];
+                // B2: dL/dalpha_n
+                T ga = 0;
+                for (int c = 0; c < 3; ++c) ga += (h.c[c] - Rc[c]) * gC[c];
+                ga += (h.z - Rd) * gD + ((T)1 - Ra) * gA;
+                ga *= Tn;
+                // B3: push this face onto the "behind" accumulators
+                for (int c = 0; c < 3; ++c) Rc[c] = h.alpha * h.c[c] + ((T)1 - h.alpha) * Rc[c];
+                Rd = h.alpha * h.z + ((T)1 - h.alpha) * Rd;
+                Ra = h.alpha + ((T)1 - h.alpha) * Ra;
+                // B4: opacity (mean -> 1/3 each, :82) and window
+                if (grad_opacity)
+                    for (int k = 0; k < 3; ++k) grad_opacity[vid(faces, m, k)] += (h.I / (T)3) * ga;
+                const T gI = f.obar * ga;
+                const T gx = gI * sigma * h.I / h.x;
+                // B5: interpolation
+                T gom[3], gb[3], gw[3];
+                for (int k = 0; k < 3; ++k) {
+                    T d = 0;
+                    for (int c = 0; c < 3; ++c) d += (f.col[k][c] - h.c[c]) * gC[c];
+                    gom[k] = (wgt / h.Om) * (d - h.z * gD);
+                    gb[k] = f.w[k] * gom[k];
+                    gw[k] = h.b[k] * gom[k];
+                }
+                // B6: screen-space vertex gradients
+                T gqx[3] = {0, 0, 0}, gqy[3] = {0, 0, 0};
+                // (i) barycentric path: db_k/dq_j = -b_j grad_p b_k, grad_p b_k = -n_k/h_k
+                T Gx = 0, Gy = 0;
+                for (int k = 0; k < 3; ++k) Gx += gb[k] * (-f.nx[k] / f.h[k]), Gy += gb[k] * (-f.ny[k] / f.h[k]);
+                for (int j2 = 0; j2 < 3; ++j2) gqx[j2] += -h.b[j2] * Gx, gqy[j2] += -h.b[j2] * Gy;
+                // (ii) window numerator x = -L_{k*}/r
+                {
+                    const int ks = h.kstar, a = (ks + 1) % 3, bb = (ks + 2) % 3;
+                    const T gL = -gx / f.r;
+                    const T ex = f.qx[bb] - f.qx[a], ey = f.qy[bb] - f.qy[a];
+                    const T t = (((T)x - f.qx[a]) * ex + ((T)y - f.qy[a]) * ey) / (f.ell[ks] * f.ell[ks]);
+                    gqx[a] += -((T)1 - t) * f.nx[ks] * gL, gqy[a] += -((T)1 - t) * f.ny[ks] * gL;
+                    gqx[bb] += -t * f.nx[ks] * gL, gqy[bb] += -t * f.ny[ks] * gL;
+                }
+                // (iii) window denominator r = |S| / sum(ell)
+                {
+                    const T gr = -(h.x / f.r) * gx;
+                    for (int j2 = 0; j2 < 3; ++j2) {
+                        const int i1 = (j2 + 1) % 3, i2 = (j2 + 2) % 3;
+                        // |q_j - q_{j+1}| is edge (j+2); |q_j - q_{j+2}| is edge (j+1)
+                        const T u1x = (f.qx[j2] - f.qx[i1]) / f.ell[i2], u1y = (f.qy[j2] - f.qy[i1]) / f.ell[i2];
+                        const T u2x = (f.qx[j2] - f.qx[i2]) / f.ell[i1], u2y = (f.qy[j2] - f.qy[i2]) / f.ell[i1];
+                        const T drx = (-f.ell[j2] * f.nx[j2]) / f.sumell - (f.absS / (f.sumell * f.sumell)) * (u1x + u2x);
+                        const T dry = (-f.ell[j2] * f.ny[j2]) / f.sumell - (f.absS / (f.sumell * f.sumell)) * (u1y + u2y);
+                        gqx[j2] += gr * drx, gqy[j2] += gr * dry;
+                    }
+                }
+                T* gs = g_scr + 9 * (int64_t)m;
+                for (int k = 0; k < 3; ++k) gs[3 * k] += gqx[k], gs[3 * k + 1] += gqy[k], gs[3 * k + 2] += gw[k];
+            }
+        }
+}
+
+// ---------------------------------------------------------------------------------- B7..B9
+template <class T>
+void project_bwd(const int32_t* faces, int32_t M, const T* Tcw, const tso_camera* cam_, const uint8_t* visible,
+                 const T* Q, const T* g_scr, T* grad_pos, T* dL_dtau) {
+    const Cam<T> cam(cam_);
+    T tau[6] = {0, 0, 0, 0, 0, 0};
+    for (int m = 0; m < M; ++m) {
+        if (!visible[m]) continue;
+        for (int k = 0; k < 3; ++k) {
+            const T X = Q[9 * (int64_t)m + 3 * k], Y = Q[9 * (int64_t)m + 3 * k + 1], Z = Q[9 * (int64_t)m + 3 * k + 2];
+            const T gu = g_scr[9 * (int64_t)m + 3 * k], gv = g_scr[9 * (int64_t)m + 3 * k + 1],
+                    gw = g_scr[9 * (int64_t)m + 3 * k + 2];
+            // B7: d(u,v,w)/d(X,Y,Z) of Eq. 1 -- the dv_I/dv_C factor of Eq. 5
+            const T g[3] = {cam.fx / Z * gu, cam.fy / Z * gv,
+                            -cam.fx * X / (Z * Z) * gu - cam.fy * Y / (Z * Z) * gv - gw / (Z * Z)};
+            // B8: world, dQ/dP = R
+            if (grad_pos) {
+                T* gp = grad_pos + 3 * (int64_t)vid(faces, m, k);
+                for (int a = 0; a < 3; ++a) gp[a] += Tcw[a] * g[0] + Tcw[4 + a] * g[1] + Tcw[8 + a] * g[2];
+            }
+            // B9: Eq. 7, Dv_C/DT = [I3, -[v_C]x]  ->  dL/dtau = [g ; Q x g]
+            tau[0] += g[0], tau[1] += g[1], tau[2] += g[2];
+            tau[3] += Y * g[2] - Z * g[1];
+            tau[4] += Z * g[0] - X * g[2];
+            tau[5] += X * g[1] - Y * g[0];
+        }
+    }
+    if (dL_dtau) for (int i = 0; i < 6; ++i) dL_dtau[i] = tau[i];
+}
+
+template <class T>
+double l1_loss(int32_t W, int32_t H, const T* C, const T* D, const T* Ch, const T* Dh, double lambda_dep, T* gC,
+               T* gD) {
+    const int64_t n = (int64_t)W * H;
+    const T wc = (T)(1.0 / (3.0 * (double)n)), wd = (T)(lambda_dep / (double)n);
+    double L = 0;
+    for (int64_t i = 0; i < 3 * n; ++i) {
+        T d = C[i] - Ch[i];
+        L += (double)wc * std::fabs((double)d);
+        gC[i] = d > 0 ? wc : (d < 0 ? -wc : (T)0);
+    }
+    for (int64_t i = 0; i < n; ++i) {
+        if (!(Dh[i] > 0)) { gD[i] = 0; continue; }
+        T d = D[i] - Dh[i];
+        L += (double)wd * std::fabs((double)d);
+        gD[i] = d > 0 ? wd : (d < 0 ? -wd : (T)0);
+    }
+    return L;
+}
+
+// SE(3) exponential, tau = (rho, theta).  out = Exp(tau) o T.
+template <class T>
+void left_perturb(const T* Tcw, const T* tau, T* out) {
+    const T rx = tau[0], ry = tau[1], rz = tau[2], wx = tau[3], wy = tau[4], wz = tau[5];
+    const T th2 = wx * wx + wy * wy + wz * wz, th = std::sqrt(th2);
+    T A, B, Cc;   // sin/th, (1-cos)/th^2, (th-sin)/th^3
+    if (th < (T)1e-4) {
+        A = (T)1 - th2 / (T)6, B = (T)0.5 - th2 / (T)24, Cc = (T)1 / (T)6 - th2 / (T)120;
+    } else {
+        A = std::sin(th) / th, B = ((T)1 - std::cos(th)) / th2, Cc = (th - std::sin(th)) / (th2 * th);
+    }
+    const T K[9] = {0, -wz, wy, wz, 0, -wx, -wy, wx, 0};
+    T K2[9];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) K2[3 * i + j] = K[3 * i] * K[j] + K[3 * i + 1] * K[3 + j] + K[3 * i + 2] * K[6 + j];
+    T R[9], Vm[9];
+    for (int i = 0; i < 9; ++i) {
+        T I = (i % 4 == 0) ? (T)1 : (T)0;
+        R[i] = I + A * K[i] + B * K2[i];
+        Vm[i] = I + B * K[i] + Cc * K2[i];
+    }
+    const T tt[3] = {Vm[0] * rx + Vm[1] * ry + Vm[2] * rz, Vm[3] * rx + Vm[4] * ry + Vm[5] * rz,
+                     Vm[6] * rx + Vm[7] * ry + Vm[8] * rz};
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 4; ++j) {
+            T acc = R[3 * i] * Tcw[j] + R[3 * i + 1] * Tcw[4 + j] + R[3 * i + 2] * Tcw[8 + j];
+            out[4 * i + j] = acc + (j == 3 ? tt[i] : (T)0);
+        }
+    }
+}
+
+}  // namespace
+
+// ====================================================================================== C ABI
+extern "C" {
+
+int64_t tso_project_f32(const float* pos, const int32_t* faces, int32_t, int32_t M, const float* T_cw,
+                        const tso_camera* cam, const tso_params* prm, uint8_t* visible, int16_t* rect,
+                        uint32_t* depth_key, uint32_t* tiles_touched, float* scr, float* Q, float* zbar) {
+    return project<float>(pos, faces, M, T_cw, cam, prm, visible, rect, depth_key, tiles_touched, scr, Q, zbar);
+}
+int64_t tso_project_f64(const double* pos, const int32_t* faces, int32_t, int32_t M, const double* T_cw,
+                        const tso_camera* cam, const tso_params* prm, uint8_t* visible, int16_t* rect,
+                        uint32_t* depth_key, uint32_t* tiles_touched, double* scr, double* Q, double* zbar) {
+    return project<double>(pos, faces, M, T_cw, cam, prm, visible, rect, depth_key, tiles_touched, scr, Q, zbar);
+}
+
+int64_t tso_bin_sort(int32_t M, int32_t W, int32_t H, const uint8_t* visible, const int16_t* rect,
+                     const uint32_t* depth_key, const uint32_t* tiles_touched, uint64_t* keys, uint32_t* vals,
+                     uint32_t* ranges) {
+    (void)tiles_touched;
+    const int tiles_x = (W + 15) / 16, tiles_y = (H + 15) / 16, NT = tiles_x * tiles_y;
+    struct KV { uint64_t k; uint32_t v; };
+    std::vector<KV> pairs;
+    for (int m = 0; m < M; ++m) {
+        if (!visible[m]) continue;
+        const int16_t* rc = rect + 4 * (int64_t)m;
+        for (int ty = rc[1] >> 4; ty <= (rc[3] >> 4); ++ty)
+            for (int tx = rc[0] >> 4; tx <= (rc[2] >> 4); ++tx)
+                pairs.push_back({((uint64_t)(ty * tiles_x + tx) << 32) | depth_key[m], (uint32_t)m});
+    }
+    std::stable_sort(pairs.begin(), pairs.end(), [](const KV& a, const KV& b) { return a.k < b.k; });
+    for (int t = 0; t < 2 * NT; ++t) ranges[t] = 0;
+    const int64_t P = (int64_t)pairs.size();
+    for (int64_t i = 0; i < P; ++i) {
+        keys[i] = pairs[i].k, vals[i] = pairs[i].v;
+        uint32_t t = (uint32_t)(pairs[i].k >> 32);
+        if (i == 0 || (uint32_t)(pairs[i - 1].k >> 32) != t) ranges[2 * t] = (uint32_t)i;
+        ranges[2 * t + 1] = (uint32_t)(i + 1);
+    }
+    return P;
+}
+
+#define TSO_FWD_ARGS color, opacity, faces, M, cam, prm, visible, rect, scr, list, n_list, tile_ranges
+void tso_render_fwd_f32(const float* color, const float* opacity, const int32_t* faces, int32_t M,
+                        const tso_camera* cam, const tso_params* prm, const uint8_t* visible, const int16_t* rect,
+                        const float* scr, const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges,
+                        float* out_color, float* out_depth, float* out_alpha, uint32_t* n_contrib, uint8_t* ambig,
+                        uint64_t* sig, uint64_t* counters) {
+    render_fwd<float>(TSO_FWD_ARGS, out_color, out_depth, out_alpha, n_contrib, ambig, sig, counters);
+}
+void tso_render_fwd_f64(const double* color, const double* opacity, const int32_t* faces, int32_t M,
+                        const tso_camera* cam, const tso_params* prm, const uint8_t* visible, const int16_t* rect,
+                        const double* scr, const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges,
+                        double* out_color, double* out_depth, double* out_alpha, uint32_t* n_contrib,
+                        uint8_t* ambig, uint64_t* sig, uint64_t* counters) {
+    render_fwd<double>(TSO_FWD_ARGS, out_color, out_depth, out_alpha, n_contrib, ambig, sig, counters);
+}
+void tso_render_bwd_f32(const float* color, const float* opacity, const int32_t* faces, int32_t M,
+                        const tso_camera* cam, const tso_params* prm, const uint8_t* visible, const int16_t* rect,
+                        const float* scr, const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges,
+                        const float* dL_dcolor, const float* dL_ddepth, const float* dL_dalpha, float* grad_color,
+                        float* grad_opacity, float* g_scr) {
+    render_bwd<float>(TSO_FWD_ARGS, dL_dcolor, dL_ddepth, dL_dalpha, grad_color, grad_opacity, g_scr);
+}
+void tso_render_bwd_f64(const double* color, const double* opacity, const int32_t* faces, int32_t M,
+                        const tso_camera* cam, const tso_params* prm, const uint8_t* visible, const int16_t* rect,
+                        const double* scr, const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges,
+                        const double* dL_dcolor, const double* dL_ddepth, const double* dL_dalpha,
+                        double* grad_color, double* grad_opacity, double* g_scr) {
+    render_bwd<double>(TSO_FWD_ARGS, dL_dcolor, dL_ddepth, dL_dalpha, grad_color, grad_opacity, g_scr);
+}
+
+void tso_project_bwd_f32(const int32_t* faces, int32_t M, const float* T_cw, const tso_camera* cam,
+                         const uint8_t* visible, const float* Q, const float* g_scr, float* grad_pos,
+                         float* dL_dtau) {
+    project_bwd<float>(faces, M, T_cw, cam, visible, Q, g_scr, grad_pos, dL_dtau);
+}
+void tso_project_bwd_f64(const int32_t* faces, int32_t M, const double* T_cw, const tso_camera* cam,
+                         const uint8_t* visible, const double* Q, const double* g_scr, double* grad_pos,
+                         double* dL_dtau) {
+    project_bwd<double>(faces, M, T_cw, cam, visible, Q, g_scr, grad_pos, dL_dtau);
+}
+
+double tso_l1_loss_f32(int32_t W, int32_t H, const float* C, const float* D, const float* Chat, const float* Dhat,
+                       double lambda_dep, float* gC, float* gD) {
+    return l1_loss<float>(W, H, C, D, Chat, Dhat, lambda_dep, gC, gD);
+}
+double tso_l1_loss_f64(int32_t W, int32_t H, const double* C, const double* D, const double* Chat,
+                       const double* Dhat, double lambda_dep, double* gC, double* gD) {
+    return l1_loss<double>(W, H, C, D, Chat, Dhat, lambda_dep, gC, gD);
+}
+
+void tso_pose_step_f32(float* T_cw, const float* g, float* state, const float* lr, float beta1, float beta2,
+                       float eps) {
+    float* m = state;
+    float* v = state + 6;
+    state[12] += 1.0f;
+    const float t = state[12];
+    const float c1 = 1.0f - std::pow(beta1, t), c2 = 1.0f - std::pow(beta2, t);
+    float delta[6];
+    for (int i = 0; i < 6; ++i) {
+        m[i] = beta1 * m[i] + (1.0f - beta1) * g[i];
+        v[i] = beta2 * v[i] + (1.0f - beta2) * g[i] * g[i];
+        const float mh = m[i] / c1, vh = v[i] / c2;
+        delta[i] = -lr[i] * mh / (std::sqrt(vh) + eps);
+    }
+    float T4[12];
+    left_perturb<float>(T_cw, delta, T4);
+    for (int i = 0; i < 12; ++i) T_cw[i] = T4[i];
+}
+
+void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out) { left_perturb<double>(T_cw, tau, out); }
+
+}  // extern "C"

@@ -1,0 +1,202 @@
+"""ctypes binding of the CPU oracle (oracle/tso.cpp).
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only tests/, __graft_entry__.smoke() and the
+cpu_baseline / --impl reference legs of bench.py may import this module.  It shares no code
+with the CUDA path (paper_2605_31419_b200/csrc) and does not import it.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from types import SimpleNamespace
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libtso.so")
+_SRC = [os.path.join(_HERE, "tso.cpp"), os.path.join(_HERE, "tso.h")]
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off: no implicit FMA contraction, the float32 path uses explicit fma."""
+    if not force and os.path.exists(_SO) and all(os.path.getmtime(_SO) >= os.path.getmtime(s) for s in _SRC):
+        return _SO
+    cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
+           "-o", _SO, _SRC[0]]
+    subprocess.check_call(cmd)
+    return _SO
+
+
+class _Cam(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_double), ("fy", C.c_double),
+                ("cx", C.c_double), ("cy", C.c_double), ("znear", C.c_double)]
+
+
+class _Prm(C.Structure):
+    _fields_ = [("sigma", C.c_double), ("alpha_min", C.c_double), ("t_min", C.c_double),
+                ("eps_area", C.c_double), ("amb_tol", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.tso_project_f32.restype = C.c_int64
+        _lib.tso_project_f64.restype = C.c_int64
+        _lib.tso_bin_sort.restype = C.c_int64
+        _lib.tso_l1_loss_f32.restype = C.c_double
+        _lib.tso_l1_loss_f64.restype = C.c_double
+    return _lib
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+def _q(prec, x):
+    """Quantise python scalars to float32-representable doubles for the f32 oracle."""
+    return float(np.float32(x)) if prec == "f32" else float(x)
+
+
+class Oracle:
+    """One view of one scene.  prec = 'f32' (parity) or 'f64' (finite differences / accuracy reference)."""
+
+    def __init__(self, pos, color, opacity, faces, T_cw, cam, params, prec="f32", amb_tol=0.0):
+        self.prec = prec
+        self.dt = np.float32 if prec == "f32" else np.float64
+        self.sfx = "_" + prec
+        self.pos = np.ascontiguousarray(pos, dtype=self.dt).reshape(-1, 3)
+        self.color = np.ascontiguousarray(color, dtype=self.dt).reshape(-1, 3)
+        self.opacity = np.ascontiguousarray(opacity, dtype=self.dt).reshape(-1)
+        self.faces = None if faces is None else np.ascontiguousarray(faces, dtype=np.int32).reshape(-1, 3)
+        self.V = self.pos.shape[0]
+        self.M = self.V // 3 if self.faces is None else self.faces.shape[0]
+        self.T_cw = np.ascontiguousarray(np.asarray(T_cw)[:3, :4], dtype=self.dt)
+        self.W, self.H = int(cam.width), int(cam.height)
+        self.cam = _Cam(self.W, self.H, _q(prec, cam.fx), _q(prec, cam.fy), _q(prec, cam.cx), _q(prec, cam.cy),
+                        _q(prec, cam.znear))
+        self.prm = _Prm(_q(prec, params.sigma), _q(prec, params.alpha_min), _q(prec, params.t_min),
+                        _q(prec, params.eps_area), float(amb_tol))
+        self.tiles_x, self.tiles_y = (self.W + 15) // 16, (self.H + 15) // 16
+        self.NT = self.tiles_x * self.tiles_y
+        self._proj = None
+        self._bins = None
+
+    def _fn(self, name):
+        return getattr(lib(), name + self.sfx)
+
+    # ------------------------------------------------------------------ F1-F6
+    def project(self):
+        if self._proj is None:
+            M = self.M
+            o = SimpleNamespace(
+                visible=np.zeros(M, np.uint8), rect=np.zeros((M, 4), np.int16), depth_key=np.zeros(M, np.uint32),
+                tiles_touched=np.zeros(M, np.uint32), scr=np.zeros((M, 9), self.dt), Q=np.zeros((M, 9), self.dt),
+                zbar=np.zeros(M, self.dt))
+            o.n_visible = self._fn("tso_project")(
+                _p(self.pos), _p(self.faces), C.c_int32(self.V), C.c_int32(M), _p(self.T_cw), C.byref(self.cam),
+                C.byref(self.prm), _p(o.visible), _p(o.rect), _p(o.depth_key), _p(o.tiles_touched), _p(o.scr),
+                _p(o.Q), _p(o.zbar))
+            self._proj = o
+        return self._proj
+
+    def bin_sort(self):
+        """Tiled mode lists.  f32: std::stable_sort on (tile<<32 | float bits).  f64: same tiles, order by the
+        double mean depth (then face index) so that finite differences see a consistent order."""
+        if self._bins is None:
+            pr = self.project()
+            P = int(pr.tiles_touched.sum(dtype=np.int64))
+            keys = np.zeros(max(P, 1), np.uint64)
+            vals = np.zeros(max(P, 1), np.uint32)
+            ranges = np.zeros((self.NT, 2), np.uint32)
+            Pn = lib().tso_bin_sort(C.c_int32(self.M), C.c_int32(self.W), C.c_int32(self.H), _p(pr.visible),
+                                    _p(pr.rect), _p(pr.depth_key), _p(pr.tiles_touched), _p(keys), _p(vals),
+                                    _p(ranges))
+            assert Pn == P
+            keys, vals = keys[:P], vals[:P]
+            if self.prec == "f64" and P > 0:
+                tile = (keys >> np.uint64(32)).astype(np.int64)
+                order = np.lexsort((vals, pr.zbar[vals], tile))
+                keys, vals = keys[order], vals[order]
+            self._bins = SimpleNamespace(P=P, keys=keys, vals=np.ascontiguousarray(vals), ranges=ranges)
+        return self._bins
+
+    def global_order(self):
+        """Brute mode list: all visible faces in ascending (depth, face index)."""
+        pr = self.project()
+        ids = np.nonzero(pr.visible)[0].astype(np.uint32)
+        k = pr.depth_key[ids] if self.prec == "f32" else pr.zbar[ids]
+        return np.ascontiguousarray(ids[np.lexsort((ids, k))])
+
+    def _lists(self, mode):
+        if mode == "brute":
+            lst = self.global_order()
+            return lst, None
+        b = self.bin_sort()
+        return b.vals, b.ranges
+
+    # ------------------------------------------------------------------ F7-F8
+    def forward(self, mode="tiled", color=None, opacity=None):
+        pr = self.project()
+        lst, ranges = self._lists(mode)
+        H, W = self.H, self.W
+        o = SimpleNamespace(color=np.zeros((3, H, W), self.dt), depth=np.zeros((H, W), self.dt),
+                            alpha=np.zeros((H, W), self.dt), n_contrib=np.zeros((H, W), np.uint32),
+                            ambig=np.zeros((H, W), np.uint8), sig=np.zeros((H, W), np.uint64),
+                            counters=np.zeros(4, np.uint64))
+        col = self.color if color is None else np.ascontiguousarray(color, self.dt)
+        opa = self.opacity if opacity is None else np.ascontiguousarray(opacity, self.dt)
+        self._fn("tso_render_fwd")(
+            _p(col), _p(opa), _p(self.faces), C.c_int32(self.M), C.byref(self.cam), C.byref(self.prm),
+            _p(pr.visible), _p(pr.rect), _p(pr.scr), _p(lst), C.c_int64(lst.shape[0]), _p(ranges), _p(o.color),
+            _p(o.depth), _p(o.alpha), _p(o.n_contrib), _p(o.ambig), _p(o.sig), _p(o.counters))
+        return o
+
+    # ------------------------------------------------------------------ B1-B9
+    def backward(self, gC=None, gD=None, gA=None, mode="tiled", want=("pos", "color", "opacity", "pose")):
+        pr = self.project()
+        lst, ranges = self._lists(mode)
+        cv = lambda a: None if a is None else np.ascontiguousarray(a, self.dt)
+        gC, gD, gA = cv(gC), cv(gD), cv(gA)
+        o = SimpleNamespace()
+        o.grad_color = np.zeros_like(self.color) if "color" in want else None
+        o.grad_opacity = np.zeros_like(self.opacity) if "opacity" in want else None
+        o.g_scr = np.zeros((self.M, 9), self.dt)
+        self._fn("tso_render_bwd")(
+            _p(self.color), _p(self.opacity), _p(self.faces), C.c_int32(self.M), C.byref(self.cam),
+            C.byref(self.prm), _p(pr.visible), _p(pr.rect), _p(pr.scr), _p(lst), C.c_int64(lst.shape[0]),
+            _p(ranges), _p(gC), _p(gD), _p(gA), _p(o.grad_color), _p(o.grad_opacity), _p(o.g_scr))
+        o.grad_pos = np.zeros_like(self.pos) if "pos" in want else None
+        o.dL_dtau = np.zeros(6, self.dt)
+        self._fn("tso_project_bwd")(_p(self.faces), C.c_int32(self.M), _p(self.T_cw), C.byref(self.cam),
+                                    _p(pr.visible), _p(pr.Q), _p(o.g_scr), _p(o.grad_pos), _p(o.dL_dtau))
+        return o
+
+    def l1_loss(self, Cimg, Dimg, Chat, Dhat, lambda_dep):
+        cv = lambda a: np.ascontiguousarray(a, self.dt)
+        Cimg, Dimg, Chat, Dhat = cv(Cimg), cv(Dimg), cv(Chat), cv(Dhat)
+        gC, gD = np.zeros_like(Cimg), np.zeros_like(Dimg)
+        L = self._fn("tso_l1_loss")(C.c_int32(self.W), C.c_int32(self.H), _p(Cimg), _p(Dimg), _p(Chat), _p(Dhat),
+                                    C.c_double(lambda_dep), _p(gC), _p(gD))
+        return L, gC, gD
+
+
+def left_perturb(T_cw, tau):
+    T = np.ascontiguousarray(np.asarray(T_cw)[:3, :4], np.float64)
+    tau = np.ascontiguousarray(tau, np.float64)
+    out = np.zeros((3, 4), np.float64)
+    lib().tso_left_perturb_f64(_p(T), _p(tau), _p(out))
+    return out
+
+
+def pose_step_f32(T_cw, g, state, lr, beta1=0.9, beta2=0.999, eps=1e-8):
+    T = np.ascontiguousarray(T_cw, np.float32).copy()
+    st = np.ascontiguousarray(state, np.float32).copy()
+    lib().tso_pose_step_f32(_p(T), _p(np.ascontiguousarray(g, np.float32)), _p(st),
+                            _p(np.ascontiguousarray(lr, np.float32)), C.c_float(beta1), C.c_float(beta2),
+                            C.c_float(eps))
+    return T, st
