@@ -1,0 +1,136 @@
+/* include/ts.h -- C ABI of libts: the B200 (sm_100a) differentiable triangle-soup rasteriser,
+ * i.e. the hot path of Triangle Splatting SLAM (arxiv/paper_2605_31419).
+ *
+ * Conventions (all exports):
+ *  - Return value: int32 status (TS_OK = 0, negative = error).  No exceptions, no aborts, no stdout.
+ *    Argument errors are detected on the host before any launch.  Data-dependent overflow of the
+ *    caller-sized buffers is reported asynchronously through ts_frame_status (flags & TS_FLAG_OVERFLOW);
+ *    outputs of an overflowed frame are unspecified (never out-of-bounds) and the caller re-binds a larger
+ *    workspace and repeats.
+ *  - Ownership: every DEVICE buffer is owned by the caller (e.g. torch tensors' data_ptr()), including the
+ *    frame workspace.  The library allocates no device memory after ts_create, never frees caller memory and
+ *    keeps no caller pointer beyond the call, except inside the caller-provided workspace of a ts_frame.
+ *  - Streams: `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is enqueued
+ *    on it.  No export synchronises except ts_frame_status and ts_frame_view.  All exports may be captured
+ *    into a CUDA graph (launch geometry never depends on device-side counts).
+ *  - Layout: float32, row-major, contiguous.  pos[V][3], color[V][3], opacity[V] (already activated, in
+ *    [0,1]); faces[M][3] int32 vertex indices, or NULL = soup (V == 3M, face m = (3m,3m+1,3m+2), the map
+ *    layout the paper uses during SLAM).  Pose T_cw[12] = row-major 3x4 [R|t] IN DEVICE MEMORY
+ *    (a tracking loop updates it without the host).  Images are planar: color[3][H][W], depth[H][W],
+ *    alpha[H][W].  Pixel (x,y) is sampled at exactly (x,y).
+ *  - Gradient outputs ACCUMULATE (+=); the caller zeroes them.  dL_dtau[6] is overwritten, order
+ *    (rho_x,rho_y,rho_z,theta_x,theta_y,theta_z), left perturbation T <- Exp(tau) o T (Eq. 6-7).
+ */
+#ifndef TS_H
+#define TS_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ts_ctx ts_ctx;      /* opaque: device properties, one per device */
+typedef struct ts_frame ts_frame;  /* opaque: one view's intermediate state inside caller memory */
+
+typedef struct { int32_t width, height; float fx, fy, cx, cy, znear; } ts_camera;
+/* sigma: window smoothness (Eq. 3, global constant; 0.5 in the paper).
+ * alpha_min: pairs with alpha < alpha_min contribute nothing (0 = literal Eq. 4).  t_min: stop a pixel's walk
+ * once its transmittance is <= t_min (the face that crossed IS included; 0 = literal Eq. 4).
+ * eps_area: faces with |doubled screen area| <= eps_area are culled. */
+typedef struct { float sigma, alpha_min, t_min, eps_area; uint32_t flags; } ts_params;
+typedef struct { const float *pos, *color, *opacity; const int32_t *faces; int32_t V, M; } ts_scene; /* device ptrs */
+
+enum { TS_OK = 0, TS_ERR_INVALID_ARG = -1, TS_ERR_WORKSPACE = -2, TS_ERR_CAPACITY = -3, TS_ERR_CUDA = -4,
+       TS_ERR_STATE = -5 };
+enum { TS_GRAD_POS = 1, TS_GRAD_COLOR = 2, TS_GRAD_OPACITY = 4, TS_GRAD_POSE = 8 };
+enum { TS_FLAG_OVERFLOW_PAIRS = 1, TS_FLAG_OVERFLOW_VISIBLE = 2 };
+/* ts_params.flags */
+enum { TS_SORT_ONESWEEP = 0,   /* global LSD onesweep radix sort on the (tile, depth) key (default) */
+       TS_SORT_HYBRID = 1 };   /* one MSD counting pass on the tile digit + per-tile depth sort in shared memory */
+
+const char* ts_strerror(int32_t status);
+
+/* ---- lifecycle ------------------------------------------------------------------------------------------ */
+int32_t ts_create(int32_t device, ts_ctx** out);
+int32_t ts_destroy(ts_ctx* ctx);
+
+/* Bytes of device workspace a frame needs for M faces, a WxH image, at most `pair_capacity` (tile, face)
+ * pairs and at most `visible_capacity` faces surviving the cull (0 = M).  Returns 0 on invalid arguments. */
+size_t ts_frame_bytes(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pair_capacity,
+                      uint64_t visible_capacity);
+/* Carves `dev_ws` (device memory, >= ts_frame_bytes, 256-byte aligned) into the frame's arrays; allocates
+ * only the small host-side handle.  Enqueues a one-time clear of the workspace control block on `stream`. */
+int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_t W, int32_t H,
+                      uint64_t pair_capacity, uint64_t visible_capacity, void* stream, ts_frame** out);
+int32_t ts_frame_release(ts_frame* frame);   /* frees the host handle only */
+/* Synchronises `stream`, then reports the counters of the last ts_project/ts_bin_sort on this frame. */
+int32_t ts_frame_status(ts_ctx* ctx, ts_frame* frame, uint32_t* flags, uint32_t* n_visible, uint64_t* n_pairs,
+                        void* stream);
+
+/* ---- the five hot-path calls ----------------------------------------------------------------------------- */
+
+/* a1: Eq. 1.  Per face: Q_k = R P_k + t; cull unless all Z_k > znear; u = fx X/Z + cx,
+ * v = fy Y/Z + cy; cull degenerate screen area; pixel rect = integer pixel centres inside the vertex AABB,
+ * clipped to the image, cull if empty; depth key = float32 bits of the mean camera depth.  Surviving faces get
+ * consecutive slots in face order (single-pass chained scan), their screen record (u,v,1/Z)x3 + mean opacity
+ * (PAPER.md:82), and one (tile<<32 | depth_key, slot) pair per touched 16x16 tile, emitted in face order,
+ * ty-major then tx.  float32 with a fixed operation order: bit-identical to the oracle (N1-N5).
+ * scene->color may be NULL here; scene->opacity must be valid. */
+int32_t ts_project(ts_ctx* ctx, const ts_scene* scene, const ts_camera* cam, const ts_params* prm,
+                   const float* T_cw_dev, ts_frame* frame, void* stream);
+
+/* a2: "faces are sorted in depth order".  Stable sort of the emitted pairs by the
+ * 32+ceil(log2 NT)-bit key, then tile_ranges[NT] = (begin,end) into the sorted list.  Ties keep ascending
+ * face index.  Requires ts_project on the same frame and stream order. */
+int32_t ts_bin_sort(ts_ctx* ctx, ts_frame* frame, void* stream);
+
+/* a3: Eq. 2-4.  Per pixel walk its tile's list front to back: phi = max_k L_k,
+ * I = ReLU(phi(p)/phi(s))^sigma, alpha = mean-opacity * I, perspective-correct barycentric colour and depth,
+ * C += T alpha c, D += T alpha z, T *= (1-alpha); A = 1 - T.  Any output pointer may be NULL. */
+int32_t ts_render_fwd(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
+                      float* out_alpha, void* stream);
+
+/* a5+a6: reverse walk of the same lists (B1-B8), gradients of L given dL/dC, dL/dD, dL/dA
+ * (same layouts as the outputs; any may be NULL = 0).  grad_mask selects TS_GRAD_*.  With TS_GRAD_POSE alone
+ * ("pose-only", the tracking mode) no per-vertex buffer is touched: per-thread se(3) terms are tree-reduced
+ * in-kernel to one 6-vector per tile.  Otherwise per-face screen-space gradients are warp-reduced, added with
+ * global float atomics and pushed through the projection (B7-B8) into grad_pos; colour / opacity gradients are
+ * added to grad_color / grad_opacity.  Requires ts_render_fwd on the same frame. */
+int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, const float* dL_dcolor,
+                      const float* dL_ddepth, const float* dL_dalpha, float* grad_pos, float* grad_color,
+                      float* grad_opacity, uint32_t grad_mask, void* stream);
+
+/* a7: Eq. 5-7: dL/dtau = sum_{face vertices} [g_C ; Q x g_C] from the partial sums the
+ * last ts_render_bwd (with TS_GRAD_POSE) left in the frame; fixed-order tree reduction (deterministic). */
+int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* frame, float* dL_dtau_dev, void* stream);
+
+/* ---- harness helpers (not part of the five; rows a4 / a8 of DESIGN.md) ------------------------------------ */
+
+/* a4: L = 1/(3HW) sum|C-Chat| + lambda_dep/(HW) sum_{Dhat>0}|D-Dhat| (Eq. 8-10 without D-SSIM); writes the
+ * cotangent images gC[3][H][W], gD[H][W] and, if loss_dev != NULL, adds L to *loss_dev (caller zeroes). */
+int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* D, const float* Chat,
+                        const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev, void* stream);
+/* a8: one Adam step on tau, then T_cw <- Exp(-delta) o T_cw, all on the device.
+ * state_dev[13] = m[6], v[6], step; lr[6] passed by value (rho then theta). */
+int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev, const float* lr6,
+                     float beta1, float beta2, float eps, void* stream);
+
+/* ---- read-only debug accessors (bit-exact tests) ---------------------------------------------------------- */
+enum { TS_VIEW_VIS_FACE = 0,     /* u32[n_visible]   face index of each visible slot (ascending)            */
+       TS_VIEW_RECT = 1,         /* i16[n_visible][4] x0,y0,x1,y1                                           */
+       TS_VIEW_DEPTH_KEY = 2,    /* u32[n_visible]                                                          */
+       TS_VIEW_TILES_TOUCHED = 3,/* u32[n_visible]                                                          */
+       TS_VIEW_SCR = 4,          /* f32[n_visible][12] (u,v,w)x3, mean opacity, pad                         */
+       TS_VIEW_KEYS = 5,         /* u64[n_pairs] sorted keys                                                */
+       TS_VIEW_VALS = 6,         /* u32[n_pairs] sorted slots (face = VIS_FACE[slot])                       */
+       TS_VIEW_TILE_RANGES = 7,  /* u32[NT][2]                                                              */
+       TS_VIEW_N_CONTRIB = 8,    /* u32[H][W]                                                               */
+       TS_VIEW_COUNTERS = 9 };   /* u64[8]: n_visit(warp-level), n_rect, n_hit, ... (debug builds only)     */
+/* Synchronises `stream`; returns the device pointer and element count of an internal array. */
+int32_t ts_frame_view(ts_ctx* ctx, ts_frame* frame, int32_t which, const void** dev_ptr, size_t* count,
+                      void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

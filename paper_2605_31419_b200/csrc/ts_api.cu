@@ -1,0 +1,248 @@
+// ts_api.cu -- the C-ABI boundary (include/ts.h): context, frame workspace carving, status / debug views and
+// host-side argument validation for the five hot-path calls.  No device memory is allocated here: the frame lives
+// entirely inside caller-provided memory.
+#include <new>
+
+#include "ts_internal.cuh"
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+struct Layout {
+    size_t ctrl, scan_state, vis_face, rect, depth_key, tiles_touched, scr, gscr, keys0, keys1, vals0, vals1, hist,
+        sort_state, tile_ranges, n_contrib, t_last, pose_partials, total;
+    int32_t tiles_x, tiles_y, NT, key_bits, n_passes;
+    uint32_t n_proj_tiles, n_sort_tiles_cap, n_partials_cap;
+};
+
+bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pair_cap, uint64_t vis_cap, Layout& L) {
+    if (!ctx || M <= 0 || W <= 0 || H <= 0 || W > 32767 || H > 32767 || pair_cap == 0 || pair_cap >= (1ull << 30) ||
+        vis_cap == 0 || vis_cap >= (1ull << 28) || (uint64_t)M >= (1ull << 28))
+        return false;
+    L.tiles_x = (W + TS_TILE - 1) / TS_TILE, L.tiles_y = (H + TS_TILE - 1) / TS_TILE, L.NT = L.tiles_x * L.tiles_y;
+    int tb = 0;
+    while ((1 << tb) < L.NT) ++tb;
+    L.key_bits = 32 + tb;
+    L.n_passes = (L.key_bits + TS_RADIX_BITS - 1) / TS_RADIX_BITS;
+    L.n_proj_tiles = (uint32_t)((M + TS_PROJ_THREADS - 1) / TS_PROJ_THREADS);
+    L.n_sort_tiles_cap = (uint32_t)((pair_cap + TS_SORT_TILE - 1) / TS_SORT_TILE);
+    L.n_partials_cap = (uint32_t)ctx->num_sms * 4u;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
+    L.ctrl = take(sizeof(TsCtrl));
+    L.scan_state = take(8ull * L.n_proj_tiles);
+    L.vis_face = take(4ull * vis_cap);
+    L.rect = take(8ull * vis_cap);
+    L.depth_key = take(4ull * vis_cap);
+    L.tiles_touched = take(4ull * vis_cap);
+    L.scr = take(48ull * vis_cap);
+    L.gscr = take(36ull * vis_cap);
+    L.keys0 = take(8ull * pair_cap);
+    L.keys1 = take(8ull * pair_cap);
+    L.vals0 = take(4ull * pair_cap);
+    L.vals1 = take(4ull * pair_cap);
+    L.hist = take(4ull * TS_MAX_PASSES * TS_RADIX);
+    L.sort_state = take(4ull * L.n_passes * L.n_sort_tiles_cap * TS_RADIX);
+    L.tile_ranges = take(8ull * L.NT);
+    L.n_contrib = take(4ull * W * H);
+    L.t_last = take(4ull * W * H);
+    L.pose_partials = take(24ull * L.n_partials_cap);
+    L.total = o;
+    return true;
+}
+
+__global__ void frame_init_kernel(TsCtrl* c) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) c->epoch = 1;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ts_strerror(int32_t s) {
+    switch (s) {
+        case TS_OK: return "ok";
+        case TS_ERR_INVALID_ARG: return "invalid argument";
+        case TS_ERR_WORKSPACE: return "workspace too small or misaligned";
+        case TS_ERR_CAPACITY: return "pair / visible-face capacity exceeded";
+        case TS_ERR_CUDA: return "CUDA error";
+        case TS_ERR_STATE: return "call out of order for this frame";
+        default: return "unknown status";
+    }
+}
+
+int32_t ts_create(int32_t device, ts_ctx** out) {
+    if (!out) return TS_ERR_INVALID_ARG;
+    int n = 0;
+    if (cudaGetDeviceCount(&n) != cudaSuccess || device < 0 || device >= n) return TS_ERR_CUDA;
+    cudaDeviceProp p;
+    if (cudaGetDeviceProperties(&p, device) != cudaSuccess) return TS_ERR_CUDA;
+    ts_ctx* c = new (std::nothrow) ts_ctx;
+    if (!c) return TS_ERR_CUDA;
+    c->device = device, c->num_sms = p.multiProcessorCount, c->max_smem_optin = (int)p.sharedMemPerBlockOptin;
+    *out = c;
+    return TS_OK;
+}
+
+int32_t ts_destroy(ts_ctx* ctx) {
+    delete ctx;
+    return TS_OK;
+}
+
+size_t ts_frame_bytes(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pair_capacity,
+                      uint64_t visible_capacity) {
+    Layout L;
+    if (visible_capacity == 0) visible_capacity = (uint64_t)(M > 0 ? M : 0);
+    if (!make_layout(ctx, M, W, H, pair_capacity, visible_capacity, L)) return 0;
+    return L.total;
+}
+
+int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_t W, int32_t H, uint64_t pair_capacity,
+                      uint64_t visible_capacity, void* stream, ts_frame** out) {
+    if (!out || !dev_ws) return TS_ERR_INVALID_ARG;
+    Layout L;
+    if (visible_capacity == 0) visible_capacity = (uint64_t)(M > 0 ? M : 0);
+    if (!make_layout(ctx, M, W, H, pair_capacity, visible_capacity, L)) return TS_ERR_INVALID_ARG;
+    if (bytes < L.total || (reinterpret_cast<uintptr_t>(dev_ws) & 255u)) return TS_ERR_WORKSPACE;
+    ts_frame* fr = new (std::nothrow) ts_frame();
+    if (!fr) return TS_ERR_CUDA;
+    char* b = static_cast<char*>(dev_ws);
+    TsFrameDev& d = fr->d;
+    d.M = M, d.W = W, d.H = H, d.tiles_x = L.tiles_x, d.tiles_y = L.tiles_y, d.NT = L.NT;
+    d.pair_cap = (uint32_t)pair_capacity, d.vis_cap = (uint32_t)visible_capacity;
+    d.key_bits = L.key_bits, d.n_passes = L.n_passes;
+    d.n_proj_tiles = L.n_proj_tiles, d.n_sort_tiles_cap = L.n_sort_tiles_cap, d.n_partials_cap = L.n_partials_cap;
+    d.ctrl = reinterpret_cast<TsCtrl*>(b + L.ctrl);
+    d.scan_state = reinterpret_cast<unsigned long long*>(b + L.scan_state);
+    d.vis_face = reinterpret_cast<uint32_t*>(b + L.vis_face);
+    d.rect = reinterpret_cast<int2*>(b + L.rect);
+    d.depth_key = reinterpret_cast<uint32_t*>(b + L.depth_key);
+    d.tiles_touched = reinterpret_cast<uint32_t*>(b + L.tiles_touched);
+    d.scr = reinterpret_cast<float4*>(b + L.scr);
+    d.gscr = reinterpret_cast<float*>(b + L.gscr);
+    d.keys[0] = reinterpret_cast<unsigned long long*>(b + L.keys0);
+    d.keys[1] = reinterpret_cast<unsigned long long*>(b + L.keys1);
+    d.vals[0] = reinterpret_cast<uint32_t*>(b + L.vals0);
+    d.vals[1] = reinterpret_cast<uint32_t*>(b + L.vals1);
+    d.hist = reinterpret_cast<uint32_t*>(b + L.hist);
+    d.sort_state = reinterpret_cast<uint32_t*>(b + L.sort_state);
+    d.tile_ranges = reinterpret_cast<uint2*>(b + L.tile_ranges);
+    d.n_contrib = reinterpret_cast<uint32_t*>(b + L.n_contrib);
+    d.t_last = reinterpret_cast<float*>(b + L.t_last);
+    d.pose_partials = reinterpret_cast<float*>(b + L.pose_partials);
+    fr->bytes = L.total, fr->base = dev_ws;
+    cudaStream_t st = (cudaStream_t)stream;
+    // one-time clears: control block, chained-scan states, the always-zero screen-gradient accumulator
+    if (cudaMemsetAsync(b + L.ctrl, 0, L.vis_face - L.ctrl, st) != cudaSuccess ||
+        cudaMemsetAsync(b + L.gscr, 0, 36ull * visible_capacity, st) != cudaSuccess ||
+        cudaMemsetAsync(b + L.tile_ranges, 0, 8ull * L.NT, st) != cudaSuccess) {
+        delete fr;
+        return TS_ERR_CUDA;
+    }
+    frame_init_kernel<<<1, 32, 0, st>>>(d.ctrl);
+    if (cudaGetLastError() != cudaSuccess) {
+        delete fr;
+        return TS_ERR_CUDA;
+    }
+    *out = fr;
+    return TS_OK;
+}
+
+int32_t ts_frame_release(ts_frame* frame) {
+    delete frame;
+    return TS_OK;
+}
+
+int32_t ts_frame_status(ts_ctx* ctx, ts_frame* fr, uint32_t* flags, uint32_t* n_visible, uint64_t* n_pairs, void* stream) {
+    if (!ctx || !fr) return TS_ERR_INVALID_ARG;
+    TsCtrl h;
+    if (cudaMemcpyAsync(&h, fr->d.ctrl, sizeof(TsCtrl), cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess ||
+        cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess)
+        return TS_ERR_CUDA;
+    if (flags) *flags = h.flags;
+    if (n_visible) *n_visible = h.n_visible;
+    if (n_pairs) *n_pairs = h.n_pairs;
+    return h.flags ? TS_ERR_CAPACITY : TS_OK;
+}
+
+int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const ts_params* prm, const float* T_cw_dev,
+                   ts_frame* fr, void* stream) {
+    if (!ctx || !sc || !cam || !prm || !T_cw_dev || !fr || !sc->pos || !sc->opacity) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M || cam->width != fr->d.W || cam->height != fr->d.H) return TS_ERR_INVALID_ARG;
+    if (sc->faces == nullptr && sc->V != 3 * sc->M) return TS_ERR_INVALID_ARG;
+    if (!(prm->sigma > 0.0f) || !(prm->alpha_min >= 0.0f) || !(prm->t_min >= 0.0f) || !(prm->eps_area >= 0.0f) ||
+        !(cam->znear > 0.0f))
+        return TS_ERR_INVALID_ARG;
+    fr->cam = TsCamDev{cam->width, cam->height, cam->fx, cam->fy, cam->cx, cam->cy, cam->znear};
+    fr->prm = TsPrmDev{prm->sigma, prm->alpha_min, prm->t_min, prm->eps_area, prm->flags};
+    fr->T_cw = T_cw_dev;
+    fr->have_sort = fr->have_fwd = 0;
+    fr->pose_src = 0;
+    const int32_t s = ts_launch_project(ctx, fr, sc, (cudaStream_t)stream);
+    fr->have_project = (s == TS_OK);
+    return s;
+}
+
+int32_t ts_bin_sort(ts_ctx* ctx, ts_frame* fr, void* stream) {
+    if (!ctx || !fr) return TS_ERR_INVALID_ARG;
+    if (!fr->have_project) return TS_ERR_STATE;
+    const int32_t s = ts_launch_sort(ctx, fr, (cudaStream_t)stream);
+    fr->have_sort = (s == TS_OK);
+    return s;
+}
+
+int32_t ts_render_fwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
+                      float* out_alpha, void* stream) {
+    if (!ctx || !sc || !fr || !sc->color) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if (!fr->have_sort) return TS_ERR_STATE;
+    const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, (cudaStream_t)stream);
+    fr->have_fwd = (s == TS_OK);
+    return s;
+}
+
+int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
+                      const float* dL_dalpha, float* grad_pos, float* grad_color, float* grad_opacity,
+                      uint32_t grad_mask, void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !sc->pos) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_POS) && !grad_pos) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_COLOR) && !grad_color) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_OPACITY) && !grad_opacity) return TS_ERR_INVALID_ARG;
+    if (grad_mask & ~(uint32_t)(TS_GRAD_POS | TS_GRAD_COLOR | TS_GRAD_OPACITY | TS_GRAD_POSE)) return TS_ERR_INVALID_ARG;
+    if (!fr->have_fwd) return TS_ERR_STATE;
+    return ts_launch_render_bwd(ctx, fr, sc, dL_dcolor, dL_ddepth, dL_dalpha, grad_pos, grad_color, grad_opacity,
+                                grad_mask, (cudaStream_t)stream);
+}
+
+int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, void* stream) {
+    if (!ctx || !fr || !dL_dtau_dev) return TS_ERR_INVALID_ARG;
+    return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, (cudaStream_t)stream);
+}
+
+int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev_ptr, size_t* count, void* stream) {
+    if (!ctx || !fr || !dev_ptr || !count) return TS_ERR_INVALID_ARG;
+    TsCtrl h;
+    if (cudaMemcpyAsync(&h, fr->d.ctrl, sizeof(TsCtrl), cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess ||
+        cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess)
+        return TS_ERR_CUDA;
+    const size_t nv = h.flags ? 0 : h.n_visible, np = h.flags ? 0 : h.n_pairs;
+    const TsFrameDev& d = fr->d;
+    switch (which) {
+        case TS_VIEW_VIS_FACE: *dev_ptr = d.vis_face, *count = nv; break;
+        case TS_VIEW_RECT: *dev_ptr = d.rect, *count = 4 * nv; break;
+        case TS_VIEW_DEPTH_KEY: *dev_ptr = d.depth_key, *count = nv; break;
+        case TS_VIEW_TILES_TOUCHED: *dev_ptr = d.tiles_touched, *count = nv; break;
+        case TS_VIEW_SCR: *dev_ptr = d.scr, *count = 12 * nv; break;
+        case TS_VIEW_KEYS: *dev_ptr = d.keys[fr->sorted_buf], *count = np; break;
+        case TS_VIEW_VALS: *dev_ptr = d.vals[fr->sorted_buf], *count = np; break;
+        case TS_VIEW_TILE_RANGES: *dev_ptr = d.tile_ranges, *count = 2 * (size_t)d.NT; break;
+        case TS_VIEW_N_CONTRIB: *dev_ptr = d.n_contrib, *count = (size_t)d.W * d.H; break;
+        case TS_VIEW_COUNTERS: *dev_ptr = &d.ctrl->counters[0], *count = 8; break;
+        default: return TS_ERR_INVALID_ARG;
+    }
+    return TS_OK;
+}
+
+}  // extern "C"

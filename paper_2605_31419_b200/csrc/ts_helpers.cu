@@ -1,0 +1,109 @@
+// ts_helpers.cu -- harness helpers a4 (L1 colour+depth loss gradient, Eq. 8-10 without D-SSIM) and a8 (on-device
+// Adam step on tau followed by T <- Exp(-delta) o T).  Elementwise / tiny; they exist so that a whole tracking
+// iteration stays on the device and can be captured into one CUDA graph.
+#include "ts_internal.cuh"
+
+namespace {
+
+__global__ void __launch_bounds__(256)
+l1_loss_grad_kernel(size_t n, const float* __restrict__ C, const float* __restrict__ D, const float* __restrict__ Ch,
+                    const float* __restrict__ Dh, float wc, float wd, float* __restrict__ gC, float* __restrict__ gD,
+                    float* __restrict__ loss) {
+    float acc = 0.f;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float d = C[c * n + i] - Ch[c * n + i];
+            gC[c * n + i] = d > 0.f ? wc : (d < 0.f ? -wc : 0.f);
+            acc += wc * fabsf(d);
+        }
+        const float dh = Dh[i];
+        float g = 0.f;
+        if (dh > 0.f) {
+            const float d = D[i] - dh;
+            g = d > 0.f ? wd : (d < 0.f ? -wd : 0.f);
+            acc += wd * fabsf(d);
+        }
+        gD[i] = g;
+    }
+    if (loss) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+        __shared__ float s[8];
+        if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = acc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            float t = 0.f;
+            for (int w = 0; w < 8; ++w) t += s[w];
+            atomicAdd(loss, t);
+        }
+    }
+}
+
+struct Lr6 { float v[6]; };
+
+__global__ void pose_step_kernel(float* __restrict__ T, const float* __restrict__ g, float* __restrict__ state, Lr6 lr,
+                                 float beta1, float beta2, float eps) {
+    if (threadIdx.x != 0) return;
+    float* m = state;
+    float* v = state + 6;
+    const float t = state[12] + 1.0f;
+    state[12] = t;
+    const float c1 = 1.0f - powf(beta1, t), c2 = 1.0f - powf(beta2, t);
+    float d[6];
+    for (int i = 0; i < 6; ++i) {
+        const float gi = g[i];
+        m[i] = beta1 * m[i] + (1.0f - beta1) * gi;
+        v[i] = beta2 * v[i] + (1.0f - beta2) * gi * gi;
+        d[i] = -lr.v[i] * (m[i] / c1) / (sqrtf(v[i] / c2) + eps);
+    }
+    // Exp(d): rotation by Rodrigues, translation V(theta) rho
+    const float wx = d[3], wy = d[4], wz = d[5];
+    const float th2 = wx * wx + wy * wy + wz * wz, th = sqrtf(th2);
+    float A, B, Cc;
+    if (th < 1e-4f) {
+        A = 1.0f - th2 / 6.0f, B = 0.5f - th2 / 24.0f, Cc = 1.0f / 6.0f - th2 / 120.0f;
+    } else {
+        A = sinf(th) / th, B = (1.0f - cosf(th)) / th2, Cc = (th - sinf(th)) / (th2 * th);
+    }
+    const float K[9] = {0.f, -wz, wy, wz, 0.f, -wx, -wy, wx, 0.f};
+    float K2[9], R[9], V[9];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) K2[3 * i + j] = K[3 * i] * K[j] + K[3 * i + 1] * K[3 + j] + K[3 * i + 2] * K[6 + j];
+    for (int i = 0; i < 9; ++i) {
+        const float I = (i % 4 == 0) ? 1.0f : 0.0f;
+        R[i] = I + A * K[i] + B * K2[i];
+        V[i] = I + B * K[i] + Cc * K2[i];
+    }
+    const float tt[3] = {V[0] * d[0] + V[1] * d[1] + V[2] * d[2], V[3] * d[0] + V[4] * d[1] + V[5] * d[2],
+                         V[6] * d[0] + V[7] * d[1] + V[8] * d[2]};
+    float o[12];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 4; ++j)
+            o[4 * i + j] = R[3 * i] * T[j] + R[3 * i + 1] * T[4 + j] + R[3 * i + 2] * T[8 + j] + (j == 3 ? tt[i] : 0.0f);
+    for (int i = 0; i < 12; ++i) T[i] = o[i];
+}
+
+}  // namespace
+
+extern "C" int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* D, const float* Chat,
+                                   const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
+                                   void* stream) {
+    if (!ctx || W <= 0 || H <= 0 || !C || !D || !Chat || !Dhat || !gC || !gD) return TS_ERR_INVALID_ARG;
+    const size_t n = (size_t)W * H;
+    const float wc = (float)(1.0 / (3.0 * (double)n)), wd = (float)((double)lambda_dep / (double)n);
+    const int grid = (int)((n + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n + 255) / 256 : (size_t)ctx->num_sms * 8);
+    l1_loss_grad_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(n, C, D, Chat, Dhat, wc, wd, gC, gD, loss_dev);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
+
+extern "C" int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev,
+                                const float* lr6, float beta1, float beta2, float eps, void* stream) {
+    if (!ctx || !T_cw_dev || !dL_dtau_dev || !state_dev || !lr6) return TS_ERR_INVALID_ARG;
+    Lr6 lr;
+    for (int i = 0; i < 6; ++i) lr.v[i] = lr6[i];
+    pose_step_kernel<<<1, 32, 0, (cudaStream_t)stream>>>(T_cw_dev, dL_dtau_dev, state_dev, lr, beta1, beta2, eps);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}

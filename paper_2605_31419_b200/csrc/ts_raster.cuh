@@ -1,0 +1,123 @@
+// ts_raster.cuh -- per-face setup (F7) and per-(pixel, face) window evaluation (F8.1-3) shared by the forward and
+// backward compositing kernels.  Every operation that decides alpha is written with explicit round-to-nearest
+// intrinsics so that the backward kernel recomputes bit-identical alpha / transmittance values (no freedom for
+// the compiler to contract differently in the two kernels).
+//
+// Formulation: with the incentre-normalised edge functions
+//     lhat_k(p) = L_k(p) / r = m_k . (p - ref) + c_k,   m_k = n_k / r,   c_k = n_k . (ref - q_{k+1}) / r
+// (ref = the float-rounded incentre, so |lhat_k| <= ~1 inside the face and c_k ~ -1), Eq. 2-3 become
+//     phi(p)/phi(s) = -max_k lhat_k(p) =: x,     I = x^sigma  (x > 0).
+// Screen barycentrics are b_k = -lhat_k * rho_k with rho_k = r/h_k = ell_k / sum(ell), and the perspective
+// weights are omega_k = lhat_k * kappa_k with kappa_k = -rho_k w_k.
+#pragma once
+#include "ts_internal.cuh"
+
+struct TsGeom {
+    float qx[3], qy[3], w[3];
+    float nx[3], ny[3], ell[3], inv_ell[3];
+    float absS, sgn, sumell, inv_sumell, r, inv_r;
+    float refx, refy, mx[3], my[3], c[3], rho[3], kap[3];
+    float obar;
+    int x0, y0, x1, y1;
+};
+
+__device__ __forceinline__ float ts_sqrt_approx(float x) {
+    float y;
+    asm("sqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+__device__ __forceinline__ void ts_face_geom(const float4 s0, const float4 s1, const float4 s2, TsGeom& g) {
+    g.qx[0] = s0.x, g.qy[0] = s0.y, g.w[0] = s0.z;
+    g.qx[1] = s0.w, g.qy[1] = s1.x, g.w[1] = s1.y;
+    g.qx[2] = s1.z, g.qy[2] = s1.w, g.w[2] = s2.x;
+    g.obar = s2.y;
+    const int rlo = __float_as_int(s2.z), rhi = __float_as_int(s2.w);
+    g.x0 = (int)(short)(rlo & 0xffff), g.y0 = rlo >> 16, g.x1 = (int)(short)(rhi & 0xffff), g.y1 = rhi >> 16;
+    // signed doubled area with the same operation order as the projection (N3): same sign on both sides
+    const float a = __fsub_rn(g.qx[1], g.qx[0]), b = __fsub_rn(g.qy[2], g.qy[0]);
+    const float c = __fsub_rn(g.qy[1], g.qy[0]), d = __fsub_rn(g.qx[2], g.qx[0]);
+    const float S = __fmaf_rn(a, b, -__fmul_rn(c, d));
+    g.sgn = S > 0.0f ? 1.0f : -1.0f;
+    g.absS = fabsf(S);
+    float sum = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int ia = (k + 1) % 3, ib = (k + 2) % 3;
+        const float ex = __fsub_rn(g.qx[ib], g.qx[ia]), ey = __fsub_rn(g.qy[ib], g.qy[ia]);
+        g.ell[k] = __fsqrt_rn(__fmaf_rn(ex, ex, __fmul_rn(ey, ey)));
+        g.inv_ell[k] = __frcp_rn(g.ell[k]);
+        g.nx[k] = __fmul_rn(__fmul_rn(g.sgn, ey), g.inv_ell[k]);
+        g.ny[k] = -__fmul_rn(__fmul_rn(g.sgn, ex), g.inv_ell[k]);
+        sum = __fadd_rn(sum, g.ell[k]);
+    }
+    g.sumell = sum;
+    g.inv_sumell = __frcp_rn(sum);
+    g.r = __fmul_rn(g.absS, g.inv_sumell);
+    g.inv_r = __fdiv_rn(sum, g.absS);
+    // reference point: incentre = sum(ell_k q_k) / sum(ell) (ell_k is the edge opposite vertex k), float-rounded
+    g.refx = __fmul_rn(__fmaf_rn(g.ell[0], g.qx[0], __fmaf_rn(g.ell[1], g.qx[1], __fmul_rn(g.ell[2], g.qx[2]))), g.inv_sumell);
+    g.refy = __fmul_rn(__fmaf_rn(g.ell[0], g.qy[0], __fmaf_rn(g.ell[1], g.qy[1], __fmul_rn(g.ell[2], g.qy[2]))), g.inv_sumell);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int ia = (k + 1) % 3;
+        g.mx[k] = __fmul_rn(g.nx[k], g.inv_r);
+        g.my[k] = __fmul_rn(g.ny[k], g.inv_r);
+        const float dx = __fsub_rn(g.refx, g.qx[ia]), dy = __fsub_rn(g.refy, g.qy[ia]);
+        g.c[k] = __fmul_rn(__fmaf_rn(g.nx[k], dx, __fmul_rn(g.ny[k], dy)), g.inv_r);
+        g.rho[k] = __fmul_rn(g.ell[k], g.inv_sumell);
+        g.kap[k] = -__fmul_rn(g.rho[k], g.w[k]);
+    }
+}
+
+// sigma dispatch: 0 = generic exp2(sigma log2 x), 1 = sigma 1, 2 = sigma 0.5, 3 = sigma 2
+template <int SM>
+__device__ __forceinline__ float ts_window_pow(float x, float sigma) {
+    if (SM == 1) return x;
+    if (SM == 2) return ts_sqrt_approx(x);
+    if (SM == 3) return __fmul_rn(x, x);
+    return __powf(x, sigma);
+}
+__host__ __device__ inline int ts_sigma_mode(float sigma) {
+    return sigma == 1.0f ? 1 : (sigma == 0.5f ? 2 : (sigma == 2.0f ? 3 : 0));
+}
+
+// F8.1-3.  Returns true if the face contributes at (px,py); l[] = lhat_k, x, I, alpha are outputs.
+template <int SM>
+__device__ __forceinline__ bool ts_eval_alpha(float refx, float refy, float m0x, float m0y, float m1x, float m1y,
+                                              float m2x, float m2y, float c0, float c1, float c2, float obar, float px,
+                                              float py, float sigma, float alpha_min, float l[3], float& x, float& I,
+                                              float& alpha) {
+    const float dx = __fsub_rn(px, refx), dy = __fsub_rn(py, refy);
+    l[0] = __fmaf_rn(m0x, dx, __fmaf_rn(m0y, dy, c0));
+    l[1] = __fmaf_rn(m1x, dx, __fmaf_rn(m1y, dy, c1));
+    l[2] = __fmaf_rn(m2x, dx, __fmaf_rn(m2y, dy, c2));
+    x = -fmaxf(l[0], fmaxf(l[1], l[2]));
+    if (!(x > 0.0f)) return false;
+    I = ts_window_pow<SM>(x, sigma);
+    alpha = __fmul_rn(obar, I);
+    return alpha >= alpha_min;
+}
+
+// thread -> pixel mapping inside a 16x16 tile: warp w owns the 8x4 block at (8*(w&1), 4*(w>>1)); keeping a warp's
+// pixels compact lets whole warps skip faces whose pixel rect misses their block.
+__device__ __forceinline__ void ts_thread_pixel(int tid, int& lx, int& ly) {
+    const int w = tid >> 5, l = tid & 31;
+    lx = ((w & 1) << 3) + (l & 7);
+    ly = ((w >> 1) << 2) + (l >> 3);
+}
+
+// 8-bit mask of the warp blocks a pixel rect (tile-relative, clamped to 0..15) overlaps
+__device__ __forceinline__ uint32_t ts_subtile_mask(int rx0, int ry0, int rx1, int ry1) {
+    uint32_t colm = 0, rowm = 0;
+    if (rx0 <= 7) colm |= 1u;
+    if (rx1 >= 8) colm |= 2u;
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+        if (ry0 <= 4 * j + 3 && ry1 >= 4 * j) rowm |= (1u << j);
+    uint32_t m = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+        if (rowm & (1u << j)) m |= colm << (2 * j);
+    return m;
+}

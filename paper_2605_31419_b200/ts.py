@@ -1,0 +1,210 @@
+"""Thin ctypes binding of libts.so (include/ts.h).  Argument marshalling only: every step of the hot path runs in
+the CUDA kernels of paper_2605_31419_b200/csrc.  PyTorch is used for device memory and streams, nothing else.
+
+There is NO CPU fallback: importing this module without a built libts.so raises, and every call on a machine
+without a CUDA device fails with TsError.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libts.so")
+
+OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4, -5
+GRAD_POS, GRAD_COLOR, GRAD_OPACITY, GRAD_POSE = 1, 2, 4, 8
+GRAD_ALL = 15
+FLAG_OVERFLOW_PAIRS, FLAG_OVERFLOW_VISIBLE = 1, 2
+PARAM_COUNTERS = 0x100   # ts_params.flags: count visits / rect tests / hits (debug instantiation)
+(VIEW_VIS_FACE, VIEW_RECT, VIEW_DEPTH_KEY, VIEW_TILES_TOUCHED, VIEW_SCR, VIEW_KEYS, VIEW_VALS, VIEW_TILE_RANGES,
+ VIEW_N_CONTRIB, VIEW_COUNTERS) = range(10)
+_VIEW_DTYPES = {VIEW_VIS_FACE: torch.int32, VIEW_RECT: torch.int16, VIEW_DEPTH_KEY: torch.int32,
+                VIEW_TILES_TOUCHED: torch.int32, VIEW_SCR: torch.float32, VIEW_KEYS: torch.int64,
+                VIEW_VALS: torch.int32, VIEW_TILE_RANGES: torch.int32, VIEW_N_CONTRIB: torch.int32,
+                VIEW_COUNTERS: torch.int64}
+
+EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
+           "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_bwd",
+           "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_pose_step", "ts_frame_view"]
+
+
+class TsError(RuntimeError):
+    pass
+
+
+class ts_camera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("znear", C.c_float)]
+
+
+class ts_params(C.Structure):
+    _fields_ = [("sigma", C.c_float), ("alpha_min", C.c_float), ("t_min", C.c_float), ("eps_area", C.c_float),
+                ("flags", C.c_uint32)]
+
+
+class ts_scene(C.Structure):
+    _fields_ = [("pos", C.c_void_p), ("color", C.c_void_p), ("opacity", C.c_void_p), ("faces", C.c_void_p),
+                ("V", C.c_int32), ("M", C.c_int32)]
+
+
+def _load():
+    if not os.path.exists(_SO):
+        raise ImportError(f"{_SO} is missing: build it with `python -m paper_2605_31419_b200.build` "
+                          "(nvcc, sm_100a).  There is no CPU fallback.")
+    lib = C.CDLL(_SO)
+    for name in EXPORTS:
+        getattr(lib, name)          # fail loudly on a stale library
+    lib.ts_strerror.restype = C.c_char_p
+    lib.ts_frame_bytes.restype = C.c_size_t
+    lib.ts_frame_bytes.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32, C.c_uint64, C.c_uint64]
+    lib.ts_frame_bind.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int32, C.c_int32, C.c_int32, C.c_uint64,
+                                  C.c_uint64, C.c_void_p, C.POINTER(C.c_void_p)]
+    lib.ts_project.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.POINTER(ts_camera), C.POINTER(ts_params),
+                               C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_bin_sort.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_render_fwd.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                  C.c_void_p]
+    lib.ts_render_bwd.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    lib.ts_pose_jacobian_reduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_l1_loss_grad.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
+                                    C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_pose_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_float), C.c_float,
+                                 C.c_float, C.c_float, C.c_void_p]
+    lib.ts_frame_status.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_uint32),
+                                    C.POINTER(C.c_uint64), C.c_void_p]
+    lib.ts_frame_view.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t),
+                                  C.c_void_p]
+    lib.ts_frame_release.argtypes = [C.c_void_p]
+    lib.ts_destroy.argtypes = [C.c_void_p]
+    lib.ts_create.argtypes = [C.c_int32, C.POINTER(C.c_void_p)]
+    return lib
+
+
+lib = _load()
+
+
+def _check(status):
+    if status != OK:
+        raise TsError(f"libts: {lib.ts_strerror(status).decode()} ({status})")
+
+
+def _ptr(t, dtype=torch.float32):
+    if t is None:
+        return None
+    if not (t.is_cuda and t.is_contiguous() and t.dtype == dtype):
+        raise TsError(f"expected a contiguous CUDA tensor of {dtype}, got {t.dtype} on {t.device}")
+    return t.data_ptr()
+
+
+def _stream(stream=None):
+    return (stream if stream is not None else torch.cuda.current_stream()).cuda_stream
+
+
+class Context:
+    def __init__(self, device=0):
+        h = C.c_void_p()
+        _check(lib.ts_create(int(device), C.byref(h)))
+        self.h, self.device = h, int(device)
+
+    def close(self):
+        if self.h:
+            lib.ts_destroy(self.h)
+            self.h = None
+
+
+class Scene:
+    """Device-resident map (V, F): pos[V,3], color[V,3], opacity[V] float32; faces[M,3] int32 or None (soup)."""
+
+    def __init__(self, pos, color, opacity, faces=None):
+        self.pos, self.color, self.opacity, self.faces = pos, color, opacity, faces
+        self.V = int(pos.shape[0])
+        self.M = self.V // 3 if faces is None else int(faces.shape[0])
+        self.c = ts_scene(_ptr(pos), _ptr(color), _ptr(opacity), _ptr(faces, torch.int32), self.V, self.M)
+
+
+class Frame:
+    """One view's intermediate state; the workspace is a torch uint8 tensor owned here (caller memory for libts)."""
+
+    def __init__(self, ctx, M, W, H, pair_capacity, visible_capacity=0, stream=None):
+        self.ctx, self.M, self.W, self.H = ctx, int(M), int(W), int(H)
+        n = lib.ts_frame_bytes(ctx.h, self.M, self.W, self.H, int(pair_capacity), int(visible_capacity))
+        if n == 0:
+            raise TsError("ts_frame_bytes: invalid arguments")
+        self.ws = torch.empty(n + 256, dtype=torch.uint8, device=f"cuda:{ctx.device}")
+        off = (-self.ws.data_ptr()) % 256
+        self.ws_ptr = self.ws.data_ptr() + off
+        self.ws_off = off
+        h = C.c_void_p()
+        _check(lib.ts_frame_bind(ctx.h, self.ws_ptr, n, self.M, self.W, self.H, int(pair_capacity),
+                                 int(visible_capacity), _stream(stream), C.byref(h)))
+        self.h, self.bytes = h, n
+
+    def release(self):
+        if self.h:
+            lib.ts_frame_release(self.h)
+            self.h = None
+
+
+def make_camera(cam):
+    return ts_camera(int(cam.width), int(cam.height), cam.fx, cam.fy, cam.cx, cam.cy, cam.znear)
+
+
+def make_params(p, flags=0):
+    return ts_params(p.sigma, p.alpha_min, p.t_min, p.eps_area, flags)
+
+
+def ts_project(ctx, scene, cam, prm, T_cw, frame, stream=None):
+    _check(lib.ts_project(ctx.h, C.byref(scene.c), C.byref(cam), C.byref(prm), _ptr(T_cw), frame.h, _stream(stream)))
+
+
+def ts_bin_sort(ctx, frame, stream=None):
+    _check(lib.ts_bin_sort(ctx.h, frame.h, _stream(stream)))
+
+
+def ts_render_fwd(ctx, scene, frame, out_color, out_depth, out_alpha, stream=None):
+    _check(lib.ts_render_fwd(ctx.h, C.byref(scene.c), frame.h, _ptr(out_color), _ptr(out_depth), _ptr(out_alpha),
+                             _stream(stream)))
+
+
+def ts_render_bwd(ctx, scene, frame, dL_dcolor, dL_ddepth, dL_dalpha, grad_pos, grad_color, grad_opacity, grad_mask,
+                  stream=None):
+    _check(lib.ts_render_bwd(ctx.h, C.byref(scene.c), frame.h, _ptr(dL_dcolor), _ptr(dL_ddepth), _ptr(dL_dalpha),
+                             _ptr(grad_pos), _ptr(grad_color), _ptr(grad_opacity), int(grad_mask), _stream(stream)))
+
+
+def ts_pose_jacobian_reduce(ctx, frame, dL_dtau, stream=None):
+    _check(lib.ts_pose_jacobian_reduce(ctx.h, frame.h, _ptr(dL_dtau), _stream(stream)))
+
+
+def ts_l1_loss_grad(ctx, W, H, Cimg, Dimg, Chat, Dhat, lambda_dep, gC, gD, loss=None, stream=None):
+    _check(lib.ts_l1_loss_grad(ctx.h, int(W), int(H), _ptr(Cimg), _ptr(Dimg), _ptr(Chat), _ptr(Dhat),
+                               float(lambda_dep), _ptr(gC), _ptr(gD), _ptr(loss), _stream(stream)))
+
+
+def ts_pose_step(ctx, T_cw, dL_dtau, state, lr6, beta1=0.9, beta2=0.999, eps=1e-8, stream=None):
+    lr = (C.c_float * 6)(*[float(x) for x in lr6])
+    _check(lib.ts_pose_step(ctx.h, _ptr(T_cw), _ptr(dL_dtau), _ptr(state), lr, beta1, beta2, eps, _stream(stream)))
+
+
+def ts_frame_status(ctx, frame, stream=None, check=True):
+    fl, nv, npairs = C.c_uint32(), C.c_uint32(), C.c_uint64()
+    st = lib.ts_frame_status(ctx.h, frame.h, C.byref(fl), C.byref(nv), C.byref(npairs), _stream(stream))
+    if check:
+        _check(st)
+    return fl.value, nv.value, npairs.value
+
+
+def ts_frame_view(ctx, frame, which, stream=None):
+    """Copy of an internal array as a torch tensor (debug / bit-exact tests)."""
+    p, n = C.c_void_p(), C.c_size_t()
+    _check(lib.ts_frame_view(ctx.h, frame.h, int(which), C.byref(p), C.byref(n), _stream(stream)))
+    dt = _VIEW_DTYPES[which]
+    nbytes = n.value * torch.empty((), dtype=dt).element_size()
+    off = (p.value or 0) - frame.ws.data_ptr()
+    if nbytes == 0:
+        return torch.empty(0, dtype=dt, device=frame.ws.device)
+    return frame.ws[off:off + nbytes].view(dt).clone()

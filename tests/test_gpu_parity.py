@@ -1,0 +1,170 @@
+"""-m gpu parity tests: the CUDA path (through the C ABI) against the float32 oracle on the same seeded inputs.
+Integer work (cull set, rects, depth keys, tile counts, sorted keys/vals, tile ranges) must be bit-exact;
+images to 1e-4, gradients to 1e-3."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2605_31419_b200 import scenes
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    from paper_2605_31419_b200 import ts
+    c = ts.Context(0)
+    yield c
+    c.close()
+
+
+def small_cfg(i):
+    """Sizes the oracle finishes in seconds that still span many tiles, several batches and ragged tails."""
+    if i == 0:
+        return scenes.config0()
+    if i == 1:
+        return scenes.config1(n_faces=100_000)
+    if i == 2:
+        return scenes.config2(n_faces=120_000)
+    if i == 3:
+        return scenes.config3(n_faces=150_000, n_views=2)
+    return scenes.config4(n_faces=200_000)
+
+
+def both(ctx, oracle_mod, sc, view=0, params=None, faces=None, T=None, **kw):
+    from gpu_util import GpuView
+    prm = params or sc.params
+    T = sc.T_start[view] if T is None else T
+    o = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, faces, T, sc.cam, prm, "f32", amb_tol=5e-3)
+    g = GpuView(ctx, sc.pos, sc.color, sc.opacity, faces, T, sc.cam, prm, **kw)
+    return o, g
+
+
+def check_project_and_sort(o, g, M):
+    from gpu_util import scatter_per_face
+    from paper_2605_31419_b200 import ts
+    g.sort()
+    flags, nvis, npairs = g.status()
+    pr, b = o.project(), o.bin_sort()
+    assert flags == 0 and nvis == pr.n_visible and npairs == b.P
+    vf = g.view(ts.VIEW_VIS_FACE).astype(np.int64)
+    assert np.array_equal(vf, np.nonzero(pr.visible)[0])                       # same cull set, ascending slots
+    assert np.array_equal(scatter_per_face(M, vf, g.view(ts.VIEW_RECT).reshape(-1, 4)), pr.rect)
+    assert np.array_equal(scatter_per_face(M, vf, g.view(ts.VIEW_DEPTH_KEY).view(np.uint32)), pr.depth_key)
+    assert np.array_equal(scatter_per_face(M, vf, g.view(ts.VIEW_TILES_TOUCHED).view(np.uint32)), pr.tiles_touched)
+    scr = g.view(ts.VIEW_SCR).reshape(-1, 12)
+    assert np.array_equal(scr[:, :9].view(np.uint32), pr.scr[vf].view(np.uint32))   # (u,v,w) bit for bit
+    assert np.array_equal(g.view(ts.VIEW_KEYS).view(np.uint64), b.keys)
+    assert np.array_equal(vf[g.view(ts.VIEW_VALS).astype(np.int64)], b.vals.astype(np.int64))
+    assert np.array_equal(g.view(ts.VIEW_TILE_RANGES).reshape(-1, 2).view(np.uint32), b.ranges)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_project_and_sort_bit_exact(ctx, oracle_mod, cfg):
+    sc = small_cfg(cfg)
+    o, g = both(ctx, oracle_mod, sc)
+    check_project_and_sort(o, g, sc.M)
+    g.close()
+
+
+def check_forward(o, g):
+    from gpu_util import assert_images_close
+    f = o.forward("tiled")
+    C, D, A = g.forward()
+    ok = f.ambig == 0
+    assert (~ok).mean() < 1e-4, "too many ambiguous pixels"
+    assert_images_close("color", C, f.color, ok[None])
+    assert_images_close("alpha", A, f.alpha, ok)
+    assert_images_close("depth", D, f.depth, ok, scale=float(np.abs(f.depth).max()))
+    return f, ok
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_forward_parity(ctx, oracle_mod, cfg):
+    sc = small_cfg(cfg)
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    assert f.alpha.max() > 0.5
+    g.close()
+
+
+def check_backward(o, g, ok, seed, mask_sets):
+    from gpu_util import assert_grad_close
+    from paper_2605_31419_b200 import ts
+    rng = np.random.default_rng(seed)
+    H, W = ok.shape
+    gC = (rng.normal(size=(3, H, W)) * ok[None]).astype(np.float32)
+    gD = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+    gA = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+    ref = o.backward(gC, gD, gA)
+    for mask in mask_sets:
+        gp, gc, go, tau = g.backward(gC, gD, gA, mask)
+        if mask & ts.GRAD_POS:
+            assert_grad_close("grad_pos", gp, ref.grad_pos)
+        if mask & ts.GRAD_COLOR:
+            assert_grad_close("grad_color", gc, ref.grad_color)
+        if mask & ts.GRAD_OPACITY:
+            assert_grad_close("grad_opacity", go, ref.grad_opacity)
+        if mask & ts.GRAD_POSE:
+            assert np.abs(tau - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max(), (tau, ref.dL_dtau)
+    return ref
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
+def test_backward_parity(ctx, oracle_mod, cfg):
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(cfg)
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    check_backward(o, g, ok, 100 + cfg, [ts.GRAD_ALL, ts.GRAD_POSE, ts.GRAD_COLOR | ts.GRAD_OPACITY, ts.GRAD_POS])
+    g.close()
+
+
+@pytest.mark.parametrize("sigma,amin,tmin", [(1.0, 0.0, 0.0), (0.5, 0.0, 0.0), (2.0, 1 / 255, 1e-4), (0.7, 1 / 255, 1e-4)])
+def test_sigma_and_threshold_variants(ctx, oracle_mod, sigma, amin, tmin):
+    from paper_2605_31419_b200 import ts
+    sc = scenes.config0()
+    prm = scenes.Params(sigma=sigma, alpha_min=amin, t_min=tmin)
+    o, g = both(ctx, oracle_mod, sc, params=prm)
+    f, ok = check_forward(o, g)
+    check_backward(o, g, ok, 7, [ts.GRAD_ALL])
+    g.close()
+
+
+def test_l1_loss_and_tracking_gradient(ctx, oracle_mod):
+    """Config-0 recipe: L1 colour+depth loss against a render of the jittered copy, gradients wrt everything."""
+    from gpu_util import assert_grad_close, dev
+    from paper_2605_31419_b200 import ts
+    sc = scenes.config0()
+    tgt = oracle_mod.Oracle(sc.pos_target, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward()
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    L, gC, gD = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, sc.params.lambda_dep)
+    gCd, gDd, loss = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
+    ts.ts_l1_loss_grad(ctx, g.W, g.H, dev(f.color), dev(f.depth), dev(tgt.color), dev(tgt.depth), sc.params.lambda_dep,
+                       gCd, gDd, loss)
+    assert np.array_equal(gCd.cpu().numpy(), gC) and np.array_equal(gDd.cpu().numpy(), gD)
+    assert abs(loss.item() - L) <= 1e-5 * L
+    ref = o.backward(gC, gD, None)
+    gp, gc, go, tau = g.backward(gC, gD, None, ts.GRAD_ALL)
+    assert_grad_close("grad_pos", gp, ref.grad_pos)
+    assert_grad_close("grad_color", gc, ref.grad_color)
+    assert_grad_close("grad_opacity", go, ref.grad_opacity)
+    assert np.abs(tau - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max()
+    g.close()
+
+
+def test_pose_step_matches_oracle(ctx, oracle_mod):
+    from gpu_util import dev
+    from paper_2605_31419_b200 import ts
+    rng = np.random.default_rng(3)
+    T = scenes.look_level((0.3, -0.2, 0.0), 0.6).astype(np.float32)
+    state = np.zeros(13, np.float32)
+    lr = [1e-3] * 3 + [3e-3] * 3
+    Td, sd = dev(T.reshape(-1)), dev(state)
+    for it in range(5):
+        gvec = rng.normal(size=6).astype(np.float32)
+        T, state = oracle_mod.pose_step_f32(T, gvec, state, lr)
+        ts.ts_pose_step(ctx, Td, dev(gvec), sd, lr)
+        assert np.allclose(Td.cpu().numpy().reshape(3, 4), T, atol=2e-6)
+        assert np.allclose(sd.cpu().numpy(), state, rtol=1e-5, atol=1e-7)
