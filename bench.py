@@ -1,0 +1,396 @@
+#!/usr/bin/env python
+"""bench.py -- fwd+bwd render throughput of the triangle-splatting rasteriser hot path (BASELINE.json metric:
+"fwd+bwd render Mpix/s @1200x680, 500k tris; tracking iters/s; % of roofline").
+
+A step = ONE tracking iteration on BASELINE.json configs[2] (Replica-shaped, 1200x680, 500k faces, seed 2):
+ts_project -> ts_bin_sort -> ts_render_fwd -> ts_l1_loss_grad -> ts_render_bwd(pose-only) ->
+ts_pose_jacobian_reduce -> ts_pose_step, i.e. every row a1..a8 of DESIGN.md section 2, on synthetic data.
+L2 is flushed between timed steps (the 18 MB map would otherwise stay L2-resident across iterations); the extra
+"tracking_iters_per_s" figure is the 100-iteration block of one frame WITHOUT flushes (the real tracking loop).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+FP32_LANES_PER_SM = 128
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"hbm_gbs": d["hbm_gbs"], "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm = [float(r[0]) for r in self.rows if len(r) >= 7 and r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if len(r) >= 7 and r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(len(r) >= 7 and r[3 + i].lower().startswith("active") for r in self.rows)]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def algorithmic_work(cnt, HW, NT, M, p_sort, mode="pose"):
+    """algorithmic bytes / FP32 flops per step from the measured counters."""
+    nv, P, nr, nh = cnt["n_visible"], cnt["n_pairs"], cnt["n_rect"], cnt["n_hit"]
+    B = {"project": 36 * M + 4 * nv + 48 * nv,
+         "bin_sort": 12 * nv + P * (12 + 8 + 24 * p_sort + 4) + 8 * NT,
+         "render_fwd": 84 * nv + 24 * HW,
+         "loss": 36 * HW,
+         "render_bwd": 84 * nv + 28 * HW + (24 * NT if mode == "pose" else 168 * nv) + (0 if mode == "pose" else 144 * nv),
+         "pose_reduce": 24 * NT}
+    F = {"project": 130 * M, "bin_sort": 0, "render_fwd": 100 * P + 15 * nr + 40 * nh, "loss": 8 * HW,
+         "render_bwd": 100 * P + 15 * nr + (170 if mode == "pose" else 190) * nh + 60 * nv, "pose_reduce": 60 * nv}
+    return B, F
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle, as it stands, on the same config / metric (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from oracle import tso
+    from paper_2605_31419_b200 import scenes
+    sc = scenes.make_config(args.config)
+    HW = sc.cam.width * sc.cam.height
+    tgt_o = tso.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+    T = sc.T_start[0].copy()
+    state = np.zeros(13, np.float32)
+    lr = [1e-3] * 3 + [3e-3] * 3
+
+    def step(T, state):
+        o = tso.Oracle(sc.pos, sc.color, sc.opacity, None, T, sc.cam, sc.params, "f32")
+        f = o.forward("tiled")
+        L, gC, gD = o.l1_loss(f.color, f.depth, tgt_o.color, tgt_o.depth, sc.params.lambda_dep)
+        g = o.backward(gC, gD, None, want=("pose",))
+        return tso.pose_step_f32(T, g.dL_dtau, state, lr)
+
+    for _ in range(args.warmup):
+        T, state = step(T, state)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        T, state = step(T, state)
+    dt = (time.perf_counter() - t0) / max(1, args.steps)
+    val = HW / dt / 1e6
+    cpu = {"value": val, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
+           "sample": f"{args.steps} full tracking iterations of {sc.name} (float32 tiled oracle, single thread)"}
+    print(json.dumps({"impl": "reference", "metric": "fwd+bwd render Mpix/s", "value": val, "unit": "Mpix/s",
+                      "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+                      "data": "synthetic", "config": {"workload": sc.name, "faces": sc.M, "image": [sc.cam.width, sc.cam.height]},
+                      "cpu_baseline": cpu,
+                      "e2e": {"value": val, "unit": "Mpix/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+class Tracker:
+    """Device state of one tracking problem + the call sequence of one iteration (argument marshalling only)."""
+
+    def __init__(self, sc, device, count_flags=0):
+        import torch
+        from paper_2605_31419_b200 import ts
+        self.torch, self.ts, self.sc = torch, ts, sc
+        self.ctx = ts.Context(device)
+        d = lambda a, dt=torch.float32: torch.as_tensor(np.ascontiguousarray(a), dtype=dt).cuda()
+        self.scene = ts.Scene(d(sc.pos), d(sc.color), d(sc.opacity))
+        self.cam, self.prm = ts.make_camera(sc.cam), ts.make_params(sc.params, count_flags)
+        self.W, self.H = sc.cam.width, sc.cam.height
+        self.frame = ts.Frame(self.ctx, self.scene.M, self.W, self.H, pair_capacity=max(2 * self.scene.M, 1 << 16))
+        H, W = self.H, self.W
+        z = lambda *s: torch.zeros(*s, device="cuda")
+        self.C, self.D, self.A = z(3, H, W), z(H, W), z(H, W)
+        self.Chat, self.Dhat = z(3, H, W), z(H, W)
+        self.gC, self.gD = z(3, H, W), z(H, W)
+        self.T, self.tau, self.state, self.loss = d(sc.T_start[0].reshape(-1)), z(6), z(13), z(1)
+        self.T0 = self.T.clone()
+        self.lr = [1e-3] * 3 + [3e-3] * 3          # PAPER.md:440-441 (trans 0.001, rot 0.003)
+        # target RGB-D frame = our own render at the ground-truth pose (synthetic stand-in for the dataset frame)
+        Tgt = d(sc.T_gt[0].reshape(-1))
+        ts.ts_project(self.ctx, self.scene, self.cam, self.prm, Tgt, self.frame)
+        ts.ts_bin_sort(self.ctx, self.frame)
+        ts.ts_render_fwd(self.ctx, self.scene, self.frame, self.Chat, self.Dhat, None)
+        torch.cuda.synchronize()
+
+    launches_per_iter = 1 + 9 + 1 + 1 + 2 + 1 + 1
+
+    def forward(self):
+        ts = self.ts
+        ts.ts_project(self.ctx, self.scene, self.cam, self.prm, self.T, self.frame)
+        ts.ts_bin_sort(self.ctx, self.frame)
+        ts.ts_render_fwd(self.ctx, self.scene, self.frame, self.C, self.D, self.A)
+
+    def backward(self):
+        ts = self.ts
+        ts.ts_l1_loss_grad(self.ctx, self.W, self.H, self.C, self.D, self.Chat, self.Dhat, self.sc.params.lambda_dep,
+                           self.gC, self.gD, self.loss)
+        ts.ts_render_bwd(self.ctx, self.scene, self.frame, self.gC, self.gD, None, None, None, None, ts.GRAD_POSE)
+        ts.ts_pose_jacobian_reduce(self.ctx, self.frame, self.tau)
+        ts.ts_pose_step(self.ctx, self.T, self.tau, self.state, self.lr)
+
+    def iteration(self):
+        self.forward()
+        self.backward()
+
+    def reset(self):
+        self.T.copy_(self.T0)
+        self.state.zero_()
+        self.loss.zero_()
+
+    def stages(self):
+        ts = self.ts
+        return [("project", lambda: ts.ts_project(self.ctx, self.scene, self.cam, self.prm, self.T, self.frame)),
+                ("bin_sort", lambda: ts.ts_bin_sort(self.ctx, self.frame)),
+                ("render_fwd", lambda: ts.ts_render_fwd(self.ctx, self.scene, self.frame, self.C, self.D, self.A)),
+                ("loss", lambda: ts.ts_l1_loss_grad(self.ctx, self.W, self.H, self.C, self.D, self.Chat, self.Dhat,
+                                                    self.sc.params.lambda_dep, self.gC, self.gD, self.loss)),
+                ("render_bwd", lambda: ts.ts_render_bwd(self.ctx, self.scene, self.frame, self.gC, self.gD, None, None,
+                                                        None, None, ts.GRAD_POSE)),
+                ("pose_reduce", lambda: ts.ts_pose_jacobian_reduce(self.ctx, self.frame, self.tau)),
+                ("pose_step", lambda: ts.ts_pose_step(self.ctx, self.T, self.tau, self.state, self.lr))]
+
+
+def cpu_baseline(sc, budget_iters=3):
+    """The oracle as it stands, single thread, on the same frame (bounded: a few full iterations)."""
+    from oracle import tso
+    tgt = tso.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+    t0 = time.perf_counter()
+    for _ in range(budget_iters):
+        o = tso.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params, "f32")
+        f = o.forward("tiled")
+        L, gC, gD = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, sc.params.lambda_dep)
+        o.backward(gC, gD, None, want=("pose",))
+    dt = (time.perf_counter() - t0) / budget_iters
+    return {"value": sc.cam.width * sc.cam.height / dt / 1e6, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
+            "sample": f"{budget_iters} full fwd+bwd tracking iterations of {sc.name}, float32 tiled oracle, 1 thread",
+            "ms_per_step": dt * 1e3}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--skip-extras", action="store_true", help="only the timed region (for ncu launch lists)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2605_31419_b200 import scenes, ts
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peaks = load_peaks()
+    # replicas / weak scaling: every rank tracks its own frame of the same scene family (seed offset by rank)
+    sc = scenes.make_config(args.config, seed=args.config + 100 * rank) if rank else scenes.make_config(args.config)
+    HW, M = sc.cam.width * sc.cam.height, sc.M
+
+    # counters (debug instantiation, outside the timed region)
+    trc = Tracker(sc, local, count_flags=ts.PARAM_COUNTERS)
+    trc.forward()
+    fl, nvis, npairs = ts.ts_frame_status(trc.ctx, trc.frame)
+    cn = ts.ts_frame_view(trc.ctx, trc.frame, ts.VIEW_COUNTERS).cpu().numpy()
+    # the target render in Tracker.__init__ also counted: two forwards ran with counters on
+    cnt = {"n_visible": int(nvis), "n_pairs": int(npairs), "n_warp_visits": int(cn[0]), "n_rect": int(cn[1]), "n_hit": int(cn[2]),
+           "note": "n_rect/n_hit/n_warp_visits summed over the target render and the start-pose render"}
+    del trc
+    torch.cuda.empty_cache()
+
+    tr = Tracker(sc, local)
+    NT = tr.frame_nt = ((sc.cam.width + 15) // 16) * ((sc.cam.height + 15) // 16)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.Stream()
+    graph = None
+    with torch.cuda.stream(stream):
+        for _ in range(3):
+            tr.iteration()
+        stream.synchronize()
+        if not args.no_graph:
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph, stream=stream):
+                tr.iteration()
+    run = (lambda: graph.replay()) if graph is not None else tr.iteration
+
+    def timed(k, do_flush=True):
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+        with torch.cuda.stream(stream):
+            for a, b in ev:
+                if do_flush:
+                    flush.fill_(1)
+                a.record(stream)
+                run()
+                b.record(stream)
+        stream.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    tr.reset()
+    timed(args.warmup)
+    tr.reset()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clk = ClockSampler(local)
+    clk.start()
+    t_wall0 = time.perf_counter()
+    ms = timed(args.steps)
+    torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    total_ms = float(sum(ms))
+    if dist is not None:
+        t = torch.tensor([total_ms], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        dist.barrier()
+    ms_per_step = total_ms / args.steps
+
+    if args.skip_extras:
+        if rank == 0:
+            print(json.dumps({"metric": "fwd+bwd render Mpix/s", "value": world * HW / (ms_per_step * 1e-3) / 1e6,
+                              "unit": "Mpix/s", "ms_per_step": ms_per_step, "steps": args.steps, "partial": True}))
+        return
+    # one frame = 100 tracking iterations back to back, no flush
+    tr.reset()
+    with torch.cuda.stream(stream):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        for _ in range(100):
+            run()
+        b.record(stream)
+    stream.synchronize()
+    frame_ms = a.elapsed_time(b)
+    loss_after = None
+
+    # per-stage device times (eager launches, events between the calls; flush between steps)
+    tr.reset()
+    stage_ms = {}
+    with torch.cuda.stream(stream):
+        for it in range(args.steps):
+            flush.fill_(1)
+            for name, fn in tr.stages():
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                fn()
+                e1.record(stream)
+                stage_ms.setdefault(name, []).append((e0, e1))
+    stream.synchronize()
+    stage_ms = {k: float(np.mean([a.elapsed_time(b) for a, b in v])) for k, v in stage_ms.items()}
+    clocks = clk.stop()
+
+    # e2e: same iteration through the C ABI with HOST buffers: the frame's target RGB-D (pinned) and the pose go
+    # up, dL/dtau and the loss come back, every step, inside the timed region
+    hC, hD = tr.Chat.cpu().pin_memory(), tr.Dhat.cpu().pin_memory()
+    hT = tr.T0.cpu().pin_memory()
+    h_out = torch.empty(7).pin_memory()
+    tr.reset()
+    e2e_ms = []
+    for it in range(args.warmup + args.steps):
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        with torch.cuda.stream(stream):
+            tr.Chat.copy_(hC, non_blocking=True)
+            tr.Dhat.copy_(hD, non_blocking=True)
+            tr.T.copy_(hT, non_blocking=True)
+            run()
+            h_out[:6].copy_(tr.tau, non_blocking=True)
+            h_out[6:].copy_(tr.loss, non_blocking=True)
+        stream.synchronize()
+        if it >= args.warmup:
+            e2e_ms.append((time.perf_counter() - t0) * 1e3)
+    e2e_step = float(np.mean(e2e_ms))
+    if dist is not None:
+        t = torch.tensor([e2e_step], device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_step = float(t.item())
+
+    value = world * HW / (ms_per_step * 1e-3) / 1e6
+    p_sort = (32 + max(0, (NT - 1).bit_length()) + 7) // 8
+    half = {k: (v // 2 if k in ("n_rect", "n_hit", "n_warp_visits") else v) for k, v in cnt.items() if k != "note"}
+    B, F = algorithmic_work(half, HW, NT, M, p_sort, "pose")
+    p_fp32 = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12        # TFLOP/s, nominal
+    t_hbm = sum(B.values()) / (peaks["hbm_gbs"] * 1e9)
+    t_alu = sum(F.values()) / (p_fp32 * 1e12)
+    t_roof = max(t_hbm, t_alu)
+    dom = max((k for k in stage_ms if k in B), key=lambda k: stage_ms[k])
+    dom_t = stage_ms[dom] * 1e-3
+    if F[dom] / (p_fp32 * 1e12) > B[dom] / (peaks["hbm_gbs"] * 1e9):
+        roof = {"bound": "alu", "kernel": dom, "achieved": F[dom] / dom_t / 1e12, "peak": p_fp32, "unit": "TFLOP/s",
+                "peak_source": "nominal 148 SM x 128 FP32 lanes x 2 x sm_max_mhz (DESIGN.md section 8)"}
+    else:
+        roof = {"bound": "hbm", "kernel": dom, "achieved": B[dom] / dom_t / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "peak_source": peaks["src"]}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["algorithmic_bytes"] = B[dom]
+    roof["algorithmic_flops"] = F[dom]
+    roof["launch_ms"] = stage_ms[dom]
+
+    out = {"metric": "fwd+bwd render Mpix/s", "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": sc.name, "faces": M, "image": [sc.cam.width, sc.cam.height], "sigma": sc.params.sigma,
+                      "mode": "tracking iteration, pose-only gradients", "l2": "flushed between timed steps (256 MiB write)",
+                      "cuda_graph": graph is not None},
+           "clocks": clocks, "gpu_launches": Tracker.launches_per_iter * args.steps,
+           "e2e": {"value": world * HW / (e2e_step * 1e-3) / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": 16 * HW + 48,
+                   "d2h_bytes_per_step": 28, "ms_per_step": e2e_step},
+           "roofline": roof,
+           "step_roofline": {"t_hbm_us": t_hbm * 1e6, "t_alu_us": t_alu * 1e6, "t_roof_us": t_roof * 1e6,
+                             "frac": t_roof / (ms_per_step * 1e-3), "algorithmic_bytes": sum(B.values()),
+                             "algorithmic_flops": sum(F.values()), "hbm_peak_gbs": peaks["hbm_gbs"], "fp32_peak_tflops": p_fp32},
+           "tracking_iters_per_s": world * 100.0 / (frame_ms * 1e-3), "frame_100_iters_ms": frame_ms,
+           "stage_ms": stage_ms, "counters": cnt, "wall_s_timed_region": t_wall}
+    if rank == 0:
+        if not args.no_cpu_baseline and world >= 1:
+            out["cpu_baseline"] = cpu_baseline(sc)
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

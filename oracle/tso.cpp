@@ -112,7 +112,7 @@ struct Face {
     T qx[3], qy[3], w[3];   // screen vertices and inverse depths
     T nx[3], ny[3];         // outward unit normal of edge k (opposite vertex k)
     T ell[3], h[3];         // edge length, altitude of vertex k
-    T r, absS, sumell;      // inradius = -phi(s), |S|, perimeter
+    T r, absS, sumell, s;   // inradius = -phi(s), |S|, perimeter, sign of S
     T obar;                 // face opacity = mean of vertex opacities (:82)
     T col[3][3];            // vertex colours
     int x0, y0, x1, y1;
@@ -124,6 +124,7 @@ void face_setup(Face<T>& f, const T* scr9, const int16_t* rc, const T* color, co
     for (int k = 0; k < 3; ++k) f.qx[k] = scr9[3 * k], f.qy[k] = scr9[3 * k + 1], f.w[k] = scr9[3 * k + 2];
     T S = signed_area(f.qx, f.qy);
     T s = S > 0 ? (T)1 : (T)-1;
+    f.s = s;
     f.absS = std::fabs(S);
     f.sumell = 0;
     for (int k = 0; k < 3; ++k) {
@@ -157,8 +158,14 @@ struct Hit {
 template <class T>
 inline int eval(const Face<T>& f, T px, T py, T sigma, T alpha_min, T amb_tol, Hit<T>& h, bool* amb) {
     for (int k = 0; k < 3; ++k) {
-        int a = (k + 1) % 3;
-        h.L[k] = f.nx[k] * (px - f.qx[a]) + f.ny[k] * (py - f.qy[a]);   // Eq. 2, relative to a vertex (S6)
+        // Eq. 2: L_k(p) = n_k . (p - q_{k+1}) = -s * cross(e_k, p - q_{k+1}) / ell_k, evaluated relative to a vertex
+        // (S6).  The cross product is formed with the compensated 2x2 determinant (one fma recovers the rounding
+        // error of the first product), so L_k keeps its RELATIVE accuracy next to the edge, where sigma < 1 makes
+        // dI/dx = sigma x^(sigma-1) large (N6).
+        int a = (k + 1) % 3, b = (k + 2) % 3;
+        const T ex = f.qx[b] - f.qx[a], ey = f.qy[b] - f.qy[a], dx = px - f.qx[a], dy = py - f.qy[a];
+        const T w = ey * dx, e = std::fma(ey, dx, -w), g = std::fma(ex, dy, -w);
+        h.L[k] = -f.s * (g - e) / f.ell[k];
     }
     h.kstar = 0;
     T phi = h.L[0];

@@ -82,17 +82,54 @@ __host__ __device__ inline int ts_sigma_mode(float sigma) {
     return sigma == 1.0f ? 1 : (sigma == 0.5f ? 2 : (sigma == 2.0f ? 3 : 0));
 }
 
+// Near an edge (|x| below this band) the fast affine form above loses RELATIVE accuracy in x (its absolute error is
+// ~2e-7), and for sigma < 1 dI/dx = sigma x^(sigma-1) amplifies that beyond the gradient tolerance.  There -- for
+// well under 1 % of the visited lanes -- x and lhat_k are recomputed from the raw screen vertices with the
+// compensated 2x2 determinant (N6), which is accurate to a few ulp relative, like the oracle's.
+#define TS_REFINE_BAND 4e-3f
+
+static __device__ __noinline__ float3 ts_refine_lhat(const float4* __restrict__ s4, float px, float py) {
+    const float4 s0 = __ldg(s4), s1 = __ldg(s4 + 1);
+    const float qx[3] = {s0.x, s0.w, s1.z}, qy[3] = {s0.y, s1.x, s1.w};
+    const float a = __fsub_rn(qx[1], qx[0]), b = __fsub_rn(qy[2], qy[0]);
+    const float c = __fsub_rn(qy[1], qy[0]), d = __fsub_rn(qx[2], qx[0]);
+    const float S = __fmaf_rn(a, b, -__fmul_rn(c, d));
+    const float sgn = S > 0.0f ? 1.0f : -1.0f;
+    float ell[3], cr[3], sum = 0.0f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int ia = (k + 1) % 3, ib = (k + 2) % 3;
+        const float ex = __fsub_rn(qx[ib], qx[ia]), ey = __fsub_rn(qy[ib], qy[ia]);
+        const float dx = __fsub_rn(px, qx[ia]), dy = __fsub_rn(py, qy[ia]);
+        ell[k] = __fsqrt_rn(__fmaf_rn(ex, ex, __fmul_rn(ey, ey)));
+        sum = __fadd_rn(sum, ell[k]);
+        const float w = __fmul_rn(ey, dx), e = __fmaf_rn(ey, dx, -w), g = __fmaf_rn(ex, dy, -w);
+        cr[k] = __fsub_rn(g, e);                       // cross(e_k, p - q_{k+1}), compensated
+    }
+    const float inv_r = __fdiv_rn(sum, fabsf(S));
+    float l[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) l[k] = __fmul_rn(__fdiv_rn(-__fmul_rn(sgn, cr[k]), ell[k]), inv_r);   // L_k / r
+    return make_float3(l[0], l[1], l[2]);
+}
+
 // F8.1-3.  Returns true if the face contributes at (px,py); l[] = lhat_k, x, I, alpha are outputs.
+// `s4` points at the face's raw screen record (only read inside the refinement band).
 template <int SM>
 __device__ __forceinline__ bool ts_eval_alpha(float refx, float refy, float m0x, float m0y, float m1x, float m1y,
                                               float m2x, float m2y, float c0, float c1, float c2, float obar, float px,
-                                              float py, float sigma, float alpha_min, float l[3], float& x, float& I,
-                                              float& alpha) {
+                                              float py, float sigma, float alpha_min, const float4* __restrict__ s4,
+                                              float l[3], float& x, float& I, float& alpha) {
     const float dx = __fsub_rn(px, refx), dy = __fsub_rn(py, refy);
     l[0] = __fmaf_rn(m0x, dx, __fmaf_rn(m0y, dy, c0));
     l[1] = __fmaf_rn(m1x, dx, __fmaf_rn(m1y, dy, c1));
     l[2] = __fmaf_rn(m2x, dx, __fmaf_rn(m2y, dy, c2));
     x = -fmaxf(l[0], fmaxf(l[1], l[2]));
+    if (fabsf(x) < TS_REFINE_BAND) {
+        const float3 lr = ts_refine_lhat(s4, px, py);
+        l[0] = lr.x, l[1] = lr.y, l[2] = lr.z;
+        x = -fmaxf(l[0], fmaxf(l[1], l[2]));
+    }
     if (!(x > 0.0f)) return false;
     I = ts_window_pow<SM>(x, sigma);
     alpha = __fmul_rn(obar, I);

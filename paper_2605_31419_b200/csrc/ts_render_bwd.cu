@@ -140,9 +140,10 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, const uint32_t* __restrict__ vals, 
                                          py >= (rlo >> 16) && py <= (rhi >> 16);
                     if (!__any_sync(0xffffffffu, in_rect)) continue;
                     const float4 r1 = R.r[1], r2 = R.r[2], r3 = R.r[3];
+                    const float4* s4 = f.scr + 3 * (size_t)__float_as_uint(R.r[11].w);
                     float l[3], x, I, alpha;
                     const bool hit = in_rect && ts_eval_alpha<SM>(r0.x, r0.y, r1.x, r1.y, r1.z, r1.w, r2.x, r2.y, r2.z,
-                                                                  r2.w, r3.x, r3.y, fpx, fpy, sigma, alpha_min, l, x, I, alpha);
+                                                                  r2.w, r3.x, r3.y, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
                     const uint32_t hm = __ballot_sync(0xffffffffu, hit);
                     if (!hm) continue;
                     const float4 r4 = R.r[4], r5 = R.r[5], r6 = R.r[6];

@@ -36,7 +36,7 @@ __device__ __forceinline__ void stage_face(const TsFrameDev& f, const ts_scene& 
     out.r[3] = make_float4(g.c[2], g.obar, g.kap[0], g.kap[1]);
     out.r[4] = make_float4(g.kap[2], col[0], col[1], col[2]);
     out.r[5] = make_float4(col[3], col[4], col[5], col[6]);
-    out.r[6] = make_float4(col[7], col[8], 0.0f, 0.0f);
+    out.r[6] = make_float4(col[7], col[8], __uint_as_float(slot), 0.0f);
     x0 = g.x0, y0 = g.y0, x1 = g.x1, y1 = g.y1;
 }
 
@@ -92,9 +92,10 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, const uint32_t* __restrict__ vals, 
                 if (COUNT) n_visit += 1, n_rect += in_rect ? 1 : 0;
                 if (!__any_sync(0xffffffffu, in_rect)) continue;
                 const float4 r1 = R.r[1], r2 = R.r[2], r3 = R.r[3];
+                const float4* s4 = f.scr + 3 * (size_t)__float_as_uint(R.r[6].z);
                 float l[3], x, I, alpha;
                 const bool hit = in_rect && ts_eval_alpha<SM>(r0.x, r0.y, r1.x, r1.y, r1.z, r1.w, r2.x, r2.y, r2.z, r2.w,
-                                                              r3.x, r3.y, fpx, fpy, sigma, alpha_min, l, x, I, alpha);
+                                                              r3.x, r3.y, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
                 if (!__any_sync(0xffffffffu, hit)) continue;
                 const float4 r4 = R.r[4], r5 = R.r[5], r6 = R.r[6];
                 if (hit) {
