@@ -146,7 +146,7 @@ class Tracker:
         ts.ts_render_fwd(self.ctx, self.scene, self.frame, self.Chat, self.Dhat, None)
         torch.cuda.synchronize()
 
-    launches_per_iter = 1 + 9 + 1 + 1 + 2 + 1 + 1
+    launches_per_iter = 1 + 2 + 1 + 1 + 1 + 1 + 1   # project, bin+sort, fwd, loss, bwd, reduce, step
 
     def forward(self):
         ts = self.ts

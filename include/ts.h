@@ -45,8 +45,7 @@ enum { TS_OK = 0, TS_ERR_INVALID_ARG = -1, TS_ERR_WORKSPACE = -2, TS_ERR_CAPACIT
 enum { TS_GRAD_POS = 1, TS_GRAD_COLOR = 2, TS_GRAD_OPACITY = 4, TS_GRAD_POSE = 8 };
 enum { TS_FLAG_OVERFLOW_PAIRS = 1, TS_FLAG_OVERFLOW_VISIBLE = 2 };
 /* ts_params.flags */
-enum { TS_SORT_ONESWEEP = 0,   /* global LSD onesweep radix sort on the (tile, depth) key (default) */
-       TS_SORT_HYBRID = 1 };   /* one MSD counting pass on the tile digit + per-tile depth sort in shared memory */
+enum { TS_PARAM_COUNTERS = 0x100 };   /* count visits / rect tests / hits into the frame's debug counters */
 
 const char* ts_strerror(int32_t status);
 
@@ -71,17 +70,21 @@ int32_t ts_frame_status(ts_ctx* ctx, ts_frame* frame, uint32_t* flags, uint32_t*
 
 /* a1: Eq. 1.  Per face: Q_k = R P_k + t; cull unless all Z_k > znear; u = fx X/Z + cx,
  * v = fy Y/Z + cy; cull degenerate screen area; pixel rect = integer pixel centres inside the vertex AABB,
- * clipped to the image, cull if empty; depth key = float32 bits of the mean camera depth.  Surviving faces get
- * consecutive slots in face order (single-pass chained scan), their screen record (u,v,1/Z)x3 + mean opacity
- * (PAPER.md:82), and one (tile<<32 | depth_key, slot) pair per touched 16x16 tile, emitted in face order,
- * ty-major then tx.  float32 with a fixed operation order: bit-identical to the oracle (N1-N5).
+ * clipped to the image, cull if empty; depth key = float32 bits of the mean camera depth.  Surviving faces get a
+ * slot (allocation order, not face order), their screen record (u,v,1/Z)x3 + mean opacity + rect +
+ * depth key, and are counted into every 16x16 tile they touch; the per-tile counts are scanned into
+ * tile_ranges[NT] = (begin,end).  float32 with a fixed operation order: cull set, rects, depth keys and tile
+ * counts are bit-identical to the oracle (N1-N5).  One kernel, one pass over the map.
  * scene->color may be NULL here; scene->opacity must be valid. */
 int32_t ts_project(ts_ctx* ctx, const ts_scene* scene, const ts_camera* cam, const ts_params* prm,
                    const float* T_cw_dev, ts_frame* frame, void* stream);
 
-/* a2: "faces are sorted in depth order".  Stable sort of the emitted pairs by the
- * 32+ceil(log2 NT)-bit key, then tile_ranges[NT] = (begin,end) into the sorted list.  Ties keep ascending
- * face index.  Requires ts_project on the same frame and stream order. */
+/* a2: "faces are sorted in depth order".  MSD-first radix sort of the (tile, depth) key: the
+ * tile digit is a counting sort (scatter of every (tile, face) pair into its tile's segment, fused with the
+ * per-face set-up of Eq. 2-3: unit normals, inradius, incentre), then every segment is sorted by
+ * (depth_key, face index) in shared memory.  The result equals the stable sort of (tile << 32 | depth_key) with
+ * pairs emitted in face order: ties keep ascending face index.  Requires ts_project on the same frame and stream
+ * order. */
 int32_t ts_bin_sort(ts_ctx* ctx, ts_frame* frame, void* stream);
 
 /* a3: Eq. 2-4.  Per pixel walk its tile's list front to back: phi = max_k L_k,
@@ -116,16 +119,14 @@ int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, flo
                      float beta1, float beta2, float eps, void* stream);
 
 /* ---- read-only debug accessors (bit-exact tests) ---------------------------------------------------------- */
-enum { TS_VIEW_VIS_FACE = 0,     /* u32[n_visible]   face index of each visible slot (ascending)            */
-       TS_VIEW_RECT = 1,         /* i16[n_visible][4] x0,y0,x1,y1                                           */
-       TS_VIEW_DEPTH_KEY = 2,    /* u32[n_visible]                                                          */
-       TS_VIEW_TILES_TOUCHED = 3,/* u32[n_visible]                                                          */
-       TS_VIEW_SCR = 4,          /* f32[n_visible][12] (u,v,w)x3, mean opacity, pad                         */
-       TS_VIEW_KEYS = 5,         /* u64[n_pairs] sorted keys                                                */
-       TS_VIEW_VALS = 6,         /* u32[n_pairs] sorted slots (face = VIS_FACE[slot])                       */
-       TS_VIEW_TILE_RANGES = 7,  /* u32[NT][2]                                                              */
-       TS_VIEW_N_CONTRIB = 8,    /* u32[H][W]                                                               */
-       TS_VIEW_COUNTERS = 9 };   /* u64[8]: n_visit(warp-level), n_rect, n_hit, ... (debug builds only)     */
+enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slot order (slots are NOT in face order):
+                                    f32 (u,v,w)x3, f32 mean opacity, i16 x0,y0,x1,y1, u32 face, u32 depth_key,
+                                    u32 tiles_touched, u32 0                                                  */
+       TS_VIEW_KEYS = 1,         /* u64[n_pairs] sorted keys (tile << 32 | depth_key)                        */
+       TS_VIEW_VALS = 2,         /* u32[n_pairs][2] sorted (slot, face) pairs                                */
+       TS_VIEW_TILE_RANGES = 3,  /* u32[NT][2]                                                               */
+       TS_VIEW_N_CONTRIB = 4,    /* u32[H][W]                                                                */
+       TS_VIEW_COUNTERS = 5 };   /* u64[8]: n_visit(warp-level), n_rect, n_hit, ... (TS_PARAM_COUNTERS only)  */
 /* Synchronises `stream`; returns the device pointer and element count of an internal array. */
 int32_t ts_frame_view(ts_ctx* ctx, ts_frame* frame, int32_t which, const void** dev_ptr, size_t* count,
                       void* stream);

@@ -10,10 +10,10 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t ctrl, scan_state, vis_face, rect, depth_key, tiles_touched, scr, gscr, keys0, keys1, vals0, vals1, hist,
-        sort_state, tile_ranges, n_contrib, t_last, pose_partials, total;
-    int32_t tiles_x, tiles_y, NT, key_bits, n_passes;
-    uint32_t n_proj_tiles, n_sort_tiles_cap, n_partials_cap;
+    size_t ctrl, tile_count, tile_cursor, tile_ranges, scr, rec, gscr, pkey, pslot, skey, sorted, n_contrib, t_last,
+        pose_partials, total;
+    int32_t tiles_x, tiles_y, NT;
+    uint32_t n_partials_cap;
 };
 
 bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pair_cap, uint64_t vis_cap, Layout& L) {
@@ -21,39 +21,25 @@ bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pa
         vis_cap == 0 || vis_cap >= (1ull << 28) || (uint64_t)M >= (1ull << 28))
         return false;
     L.tiles_x = (W + TS_TILE - 1) / TS_TILE, L.tiles_y = (H + TS_TILE - 1) / TS_TILE, L.NT = L.tiles_x * L.tiles_y;
-    int tb = 0;
-    while ((1 << tb) < L.NT) ++tb;
-    L.key_bits = 32 + tb;
-    L.n_passes = (L.key_bits + TS_RADIX_BITS - 1) / TS_RADIX_BITS;
-    L.n_proj_tiles = (uint32_t)((M + TS_PROJ_THREADS - 1) / TS_PROJ_THREADS);
-    L.n_sort_tiles_cap = (uint32_t)((pair_cap + TS_SORT_TILE - 1) / TS_SORT_TILE);
-    L.n_partials_cap = (uint32_t)ctx->num_sms * 4u;
+    L.n_partials_cap = (uint32_t)L.NT > (uint32_t)ctx->num_sms * 4u ? (uint32_t)L.NT : (uint32_t)ctx->num_sms * 4u;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
     L.ctrl = take(sizeof(TsCtrl));
-    L.scan_state = take(8ull * L.n_proj_tiles);
-    L.vis_face = take(4ull * vis_cap);
-    L.rect = take(8ull * vis_cap);
-    L.depth_key = take(4ull * vis_cap);
-    L.tiles_touched = take(4ull * vis_cap);
-    L.scr = take(48ull * vis_cap);
-    L.gscr = take(36ull * vis_cap);
-    L.keys0 = take(8ull * pair_cap);
-    L.keys1 = take(8ull * pair_cap);
-    L.vals0 = take(4ull * pair_cap);
-    L.vals1 = take(4ull * pair_cap);
-    L.hist = take(4ull * TS_MAX_PASSES * TS_RADIX);
-    L.sort_state = take(4ull * L.n_passes * L.n_sort_tiles_cap * TS_RADIX);
+    L.tile_count = take(4ull * L.NT);
+    L.tile_cursor = take(4ull * L.NT);
     L.tile_ranges = take(8ull * L.NT);
+    L.scr = take(16ull * TS_SCR_F4 * vis_cap);
+    L.rec = take(16ull * TS_REC_F4 * vis_cap);
+    L.gscr = take(36ull * vis_cap);
+    L.pkey = take(8ull * pair_cap);
+    L.pslot = take(4ull * pair_cap);
+    L.skey = take(8ull * pair_cap);
+    L.sorted = take(8ull * pair_cap);
     L.n_contrib = take(4ull * W * H);
     L.t_last = take(4ull * W * H);
     L.pose_partials = take(24ull * L.n_partials_cap);
     L.total = o;
     return true;
-}
-
-__global__ void frame_init_kernel(TsCtrl* c) {
-    if (threadIdx.x == 0 && blockIdx.x == 0) c->epoch = 1;
 }
 
 }  // namespace
@@ -111,37 +97,27 @@ int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_
     TsFrameDev& d = fr->d;
     d.M = M, d.W = W, d.H = H, d.tiles_x = L.tiles_x, d.tiles_y = L.tiles_y, d.NT = L.NT;
     d.pair_cap = (uint32_t)pair_capacity, d.vis_cap = (uint32_t)visible_capacity;
-    d.key_bits = L.key_bits, d.n_passes = L.n_passes;
-    d.n_proj_tiles = L.n_proj_tiles, d.n_sort_tiles_cap = L.n_sort_tiles_cap, d.n_partials_cap = L.n_partials_cap;
+    d.n_partials_cap = L.n_partials_cap;
     d.ctrl = reinterpret_cast<TsCtrl*>(b + L.ctrl);
-    d.scan_state = reinterpret_cast<unsigned long long*>(b + L.scan_state);
-    d.vis_face = reinterpret_cast<uint32_t*>(b + L.vis_face);
-    d.rect = reinterpret_cast<int2*>(b + L.rect);
-    d.depth_key = reinterpret_cast<uint32_t*>(b + L.depth_key);
-    d.tiles_touched = reinterpret_cast<uint32_t*>(b + L.tiles_touched);
-    d.scr = reinterpret_cast<float4*>(b + L.scr);
-    d.gscr = reinterpret_cast<float*>(b + L.gscr);
-    d.keys[0] = reinterpret_cast<unsigned long long*>(b + L.keys0);
-    d.keys[1] = reinterpret_cast<unsigned long long*>(b + L.keys1);
-    d.vals[0] = reinterpret_cast<uint32_t*>(b + L.vals0);
-    d.vals[1] = reinterpret_cast<uint32_t*>(b + L.vals1);
-    d.hist = reinterpret_cast<uint32_t*>(b + L.hist);
-    d.sort_state = reinterpret_cast<uint32_t*>(b + L.sort_state);
+    d.tile_count = reinterpret_cast<uint32_t*>(b + L.tile_count);
+    d.tile_cursor = reinterpret_cast<uint32_t*>(b + L.tile_cursor);
     d.tile_ranges = reinterpret_cast<uint2*>(b + L.tile_ranges);
+    d.scr = reinterpret_cast<float4*>(b + L.scr);
+    d.rec = reinterpret_cast<float4*>(b + L.rec);
+    d.gscr = reinterpret_cast<float*>(b + L.gscr);
+    d.pkey = reinterpret_cast<unsigned long long*>(b + L.pkey);
+    d.pslot = reinterpret_cast<uint32_t*>(b + L.pslot);
+    d.skey = reinterpret_cast<unsigned long long*>(b + L.skey);
+    d.sorted = reinterpret_cast<uint2*>(b + L.sorted);
     d.n_contrib = reinterpret_cast<uint32_t*>(b + L.n_contrib);
     d.t_last = reinterpret_cast<float*>(b + L.t_last);
     d.pose_partials = reinterpret_cast<float*>(b + L.pose_partials);
     fr->bytes = L.total, fr->base = dev_ws;
     cudaStream_t st = (cudaStream_t)stream;
-    // one-time clears: control block, chained-scan states, the always-zero screen-gradient accumulator
-    if (cudaMemsetAsync(b + L.ctrl, 0, L.vis_face - L.ctrl, st) != cudaSuccess ||
-        cudaMemsetAsync(b + L.gscr, 0, 36ull * visible_capacity, st) != cudaSuccess ||
-        cudaMemsetAsync(b + L.tile_ranges, 0, 8ull * L.NT, st) != cudaSuccess) {
-        delete fr;
-        return TS_ERR_CUDA;
-    }
-    frame_init_kernel<<<1, 32, 0, st>>>(d.ctrl);
-    if (cudaGetLastError() != cudaSuccess) {
+    // one-time clears: control block, tile counters / cursors / ranges (contiguous), the zero-at-rest screen-gradient
+    // accumulator
+    if (cudaMemsetAsync(b + L.ctrl, 0, L.scr - L.ctrl, st) != cudaSuccess ||
+        cudaMemsetAsync(b + L.gscr, 0, 36ull * visible_capacity, st) != cudaSuccess) {
         delete fr;
         return TS_ERR_CUDA;
     }
@@ -230,13 +206,9 @@ int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev
     const size_t nv = h.flags ? 0 : h.n_visible, np = h.flags ? 0 : h.n_pairs;
     const TsFrameDev& d = fr->d;
     switch (which) {
-        case TS_VIEW_VIS_FACE: *dev_ptr = d.vis_face, *count = nv; break;
-        case TS_VIEW_RECT: *dev_ptr = d.rect, *count = 4 * nv; break;
-        case TS_VIEW_DEPTH_KEY: *dev_ptr = d.depth_key, *count = nv; break;
-        case TS_VIEW_TILES_TOUCHED: *dev_ptr = d.tiles_touched, *count = nv; break;
-        case TS_VIEW_SCR: *dev_ptr = d.scr, *count = 12 * nv; break;
-        case TS_VIEW_KEYS: *dev_ptr = d.keys[fr->sorted_buf], *count = np; break;
-        case TS_VIEW_VALS: *dev_ptr = d.vals[fr->sorted_buf], *count = np; break;
+        case TS_VIEW_VIS: *dev_ptr = d.scr, *count = 16 * nv; break;
+        case TS_VIEW_KEYS: *dev_ptr = d.skey, *count = np; break;
+        case TS_VIEW_VALS: *dev_ptr = d.sorted, *count = 2 * np; break;
         case TS_VIEW_TILE_RANGES: *dev_ptr = d.tile_ranges, *count = 2 * (size_t)d.NT; break;
         case TS_VIEW_N_CONTRIB: *dev_ptr = d.n_contrib, *count = (size_t)d.W * d.H; break;
         case TS_VIEW_COUNTERS: *dev_ptr = &d.ctrl->counters[0], *count = 8; break;

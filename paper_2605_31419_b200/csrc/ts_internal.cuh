@@ -7,48 +7,44 @@
 #include "../../include/ts.h"
 
 #define TS_TILE 16
-#define TS_PROJ_THREADS 256          // faces per project tile
+#define TS_PROJ_THREADS 256          // faces per project CTA
+#define TS_BIN_THREADS 128           // visible slots per bin/setup CTA iteration
 #define TS_SORT_THREADS 256
-#define TS_SORT_ITEMS 8              // keys per thread per onesweep tile
-#define TS_SORT_TILE (TS_SORT_THREADS * TS_SORT_ITEMS)
-#define TS_RADIX_BITS 8
-#define TS_RADIX 256
-#define TS_MAX_PASSES 8
-#define TS_BATCH 128                 // list entries staged per batch in the render kernels
+#define TS_SORT_SMEM 2048            // tile lists up to this length are sorted in shared memory
+#define TS_BATCH 128                 // list entries staged per batch in the forward kernel
+#define TS_BATCH_BWD 64              // ... in the backward kernel (records are twice as large)
+#define TS_REC_F4 10                 // float4 per face record (160 B)
+#define TS_SCR_F4 4                  // float4 per raw projected record (64 B)
 
-// Device control block (one per frame, lives at the start of the workspace).
+// Device control block (one per frame, lives at the start of the workspace).  Every field that a kernel
+// accumulates into is back at zero when that kernel's grid has finished ("zero at rest"), so a frame can be
+// re-used by graph replays without host-side clears.
 struct TsCtrl {
     uint32_t n_visible;      // faces surviving the cull (may exceed vis_cap on overflow)
-    uint32_t n_pairs;        // (tile, face) pairs emitted (may exceed pair_cap on overflow)
+    uint32_t n_pairs;        // (tile, face) pairs (may exceed pair_cap on overflow)
     uint32_t flags;          // TS_FLAG_*
-    uint32_t epoch;          // chained-scan epoch (1..15), advanced by the last project block
-    uint32_t proj_ticket;    // dynamic tile id of the project kernel
-    uint32_t proj_done;      // blocks finished
-    uint32_t sort_ticket[TS_MAX_PASSES];
-    uint32_t max_list;       // longest tile list (hybrid path)
-    uint32_t pad[1];
-    unsigned long long counters[8];   // debug counters
+    uint32_t max_list;       // longest tile list of the last ts_project
+    uint32_t vis_counter;    // slot allocator of the project kernel (zero at rest)
+    uint32_t proj_done;      // project CTAs finished (zero at rest)
+    uint32_t pad[2];
+    unsigned long long counters[8];   // debug counters (TS_PARAM_COUNTERS)
 };
 
 // Everything a kernel needs to know about a frame; passed by value.
 struct TsFrameDev {
     int32_t M, W, H, tiles_x, tiles_y, NT;
     uint32_t pair_cap, vis_cap;
-    int32_t key_bits, n_passes;
-    uint32_t n_proj_tiles, n_sort_tiles_cap;
     TsCtrl* ctrl;
-    unsigned long long* scan_state;   // [n_proj_tiles]
-    uint32_t* vis_face;               // [vis_cap]
-    int2* rect;                       // [vis_cap]  (x0 | y0<<16, x1 | y1<<16) as int16 pairs
-    uint32_t* depth_key;              // [vis_cap]
-    uint32_t* tiles_touched;          // [vis_cap]
-    float4* scr;                      // [vis_cap][3]: (u0,v0,w0,u1) (v1,w1,u2,v2) (w2, obar, rect_lo, rect_hi)
-    float* gscr;                      // [vis_cap][9]: dL/d(u,v,w) per face vertex (full-gradient mode), kept zero
-    unsigned long long* keys[2];      // [pair_cap] ping-pong
-    uint32_t* vals[2];                // [pair_cap]
-    uint32_t* hist;                   // [TS_MAX_PASSES][256]
-    uint32_t* sort_state;             // [n_passes][n_sort_tiles_cap][256]
-    uint2* tile_ranges;               // [NT]
+    uint32_t* tile_count;             // [NT] pairs per tile, counted by the project kernel (zero at rest)
+    uint32_t* tile_cursor;            // [NT] write cursor of the binning pass (absolute positions)
+    uint2* tile_ranges;               // [NT] (begin, end) into the pair arrays
+    float4* scr;                      // [vis_cap][4]: (u0,v0,w0,u1) (v1,w1,u2,v2) (w2,obar,rect_lo,rect_hi) (face,key,tiles,0)
+    float4* rec;                      // [vis_cap][10]: per-face render record, see ts_raster.cuh
+    float* gscr;                      // [vis_cap][9]: dL/d(u,v,w) per face vertex (full-gradient mode), zero at rest
+    unsigned long long* pkey;         // [pair_cap] binned, unsorted: depth_key << 32 | face
+    uint32_t* pslot;                  // [pair_cap] binned, unsorted: slot
+    unsigned long long* skey;         // [pair_cap] sorted: tile << 32 | depth_key
+    uint2* sorted;                    // [pair_cap] sorted: (slot, face)
     uint32_t* n_contrib;              // [H*W]
     float* t_last;                    // [H*W] transmittance in front of the last contributing face
     float* pose_partials;             // [n_partials_cap][6]
@@ -68,10 +64,9 @@ struct ts_frame {
     TsFrameDev d;
     TsCamDev cam;
     TsPrmDev prm;
-    const float* T_cw;       // device pointer given to the last ts_project
-    int sorted_buf;          // which ping-pong buffer holds the sorted pairs
+    const float* T_cw;       // device pointer given to the last ts_project (read again by the projection backward)
     int have_project, have_sort, have_fwd;
-    uint32_t pose_src;       // 0 = none, 1 = per-tile partials (pose-only), 2 = per-block partials (epilogue)
+    uint32_t pose_src;       // 0 = none, 1 = per-tile partials (pose-only), 2 = per-block partials (projection backward)
     uint32_t n_pose_partials;
     size_t bytes;
     void* base;

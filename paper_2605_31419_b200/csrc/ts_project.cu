@@ -1,23 +1,16 @@
-// ts_project.cu -- a1: project + cull + bounds (Eq. 1), fused with the single-pass chained
-// scan that gives every surviving face its slot and pair offset, and with the emission of the unsorted
-// (tile<<32 | depth, slot) pairs.  One kernel, one pass over the map: 36 B read per face (soup), float4 loads.
+// ts_project.cu -- a1: project + cull + bounds (Eq. 1) in ONE streaming pass over the map:
+// 36 B read per face (soup), float4 loads staged through shared memory, no inter-CTA dependency.  Surviving
+// faces get a slot from a per-CTA-aggregated atomic counter (slots are NOT in face order: every later stage
+// orders by face index explicitly), write their 64 B raw screen record and count themselves into the tiles they
+// touch (RED.ADD on tile_count).  The last CTA to finish turns the counts into tile ranges and write cursors
+// (exclusive scan over the NT tiles), publishes n_visible / n_pairs / overflow flags and leaves every counter
+// it used at zero for the next call, so the launch sequence can be replayed from a CUDA graph unchanged.
 //
 // Arithmetic follows the fixed operation order N1-N5 of DESIGN.md with explicit round-to-nearest intrinsics,
 // so cull decisions, pixel rects, tile counts and depth keys are bit-identical to the float32 oracle.
 #include "ts_internal.cuh"
 
 namespace {
-
-// chained-scan state: flag(2) | pairs(30) | epoch(4) | visible(28)
-constexpr unsigned long long ST_AGG = 1ull << 62, ST_PREFIX = 2ull << 62, ST_FLAGS = 3ull << 62;
-__device__ __forceinline__ unsigned long long st_pack(unsigned long long flag, uint32_t vis, uint32_t pairs,
-                                                      uint32_t epoch) {
-    return flag | ((unsigned long long)(pairs & 0x3FFFFFFFu) << 32) | ((unsigned long long)(epoch & 0xFu) << 28) |
-           (unsigned long long)(vis & 0x0FFFFFFFu);
-}
-__device__ __forceinline__ uint32_t st_vis(unsigned long long s) { return (uint32_t)(s & 0x0FFFFFFFull); }
-__device__ __forceinline__ uint32_t st_pairs(unsigned long long s) { return (uint32_t)((s >> 32) & 0x3FFFFFFFull); }
-__device__ __forceinline__ uint32_t st_epoch(unsigned long long s) { return (uint32_t)((s >> 28) & 0xFull); }
 
 struct FaceOut {
     float u[3], v[3], w[3];
@@ -71,19 +64,11 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
                int pos_aligned) {
     __shared__ __align__(16) float sp[TS_PROJ_THREADS * 9];
     __shared__ float sT[12];
-    __shared__ uint32_t s_tile, s_epoch;
-    __shared__ uint32_t s_wv[8], s_wp[8];
-    __shared__ uint32_t s_excl_vis, s_excl_pairs;
+    __shared__ uint32_t s_w[TS_PROJ_THREADS / 32];
+    __shared__ uint32_t s_base, s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    volatile TsCtrl* ctrl = f.ctrl;
-    if (tid == 0) {
-        s_tile = atomicAdd((uint32_t*)&f.ctrl->proj_ticket, 1u);   // ticket order => look-back always progresses
-        s_epoch = ctrl->epoch;
-    }
     if (tid < 12) sT[tid] = __ldg(Tcw + tid);
-    __syncthreads();
-    const uint32_t tile = s_tile, epoch = s_epoch;
-    const int64_t face0 = (int64_t)tile * TS_PROJ_THREADS;
+    const int64_t face0 = (int64_t)blockIdx.x * TS_PROJ_THREADS;
     const int n_here = (int)min((int64_t)TS_PROJ_THREADS, (int64_t)f.M - face0);
     float p[9];
     if (SOUP) {
@@ -103,82 +88,38 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
 #pragma unroll
             for (int j = 0; j < 9; ++j) p[j] = sp[tid * 9 + j];
         }
-    } else if (tid < n_here) {
+    } else {
+        if (tid < n_here) {
 #pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const int v = __ldg(faces + (face0 + tid) * 3 + k);
-            p[3 * k] = __ldg(pos + 3 * (int64_t)v), p[3 * k + 1] = __ldg(pos + 3 * (int64_t)v + 1),
-            p[3 * k + 2] = __ldg(pos + 3 * (int64_t)v + 2);
+            for (int k = 0; k < 3; ++k) {
+                const int v = __ldg(faces + (face0 + tid) * 3 + k);
+                p[3 * k] = __ldg(pos + 3 * (int64_t)v), p[3 * k + 1] = __ldg(pos + 3 * (int64_t)v + 1),
+                p[3 * k + 2] = __ldg(pos + 3 * (int64_t)v + 2);
+            }
         }
+        __syncthreads();   // sT
     }
     FaceOut o;
     o.vis = false, o.tiles = 0;
     if (tid < n_here) project_face(p, sT, cam, eps_area, o);
 
-    // block-wide exclusive scan of (visible, tiles)
-    uint32_t iv = o.vis ? 1u : 0u, ip = o.tiles;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t tv = __shfl_up_sync(0xffffffffu, iv, d), tp = __shfl_up_sync(0xffffffffu, ip, d);
-        if (lane >= d) iv += tv, ip += tp;
-    }
-    if (lane == 31) s_wv[warp] = iv, s_wp[warp] = ip;
+    // slot allocation: warp ballot -> CTA total -> one global atomic per CTA
+    const uint32_t bal = __ballot_sync(0xffffffffu, o.vis);
+    if (lane == 0) s_w[warp] = __popc(bal);
     __syncthreads();
-    if (warp == 0) {
-        uint32_t wv = lane < 8 ? s_wv[lane] : 0u, wp = lane < 8 ? s_wp[lane] : 0u;
-        uint32_t cv = wv, cp = wp;
+    if (tid == 0) {
+        uint32_t tot = 0;
 #pragma unroll
-        for (int d = 1; d < 8; d <<= 1) {
-            const uint32_t tv = __shfl_up_sync(0xffffffffu, cv, d), tp = __shfl_up_sync(0xffffffffu, cp, d);
-            if (lane >= d) cv += tv, cp += tp;
+        for (int w = 0; w < TS_PROJ_THREADS / 32; ++w) {
+            const uint32_t c = s_w[w];
+            s_w[w] = tot;
+            tot += c;
         }
-        const uint32_t tot_v = __shfl_sync(0xffffffffu, cv, 7), tot_p = __shfl_sync(0xffffffffu, cp, 7);
-        if (lane < 8) s_wv[lane] = cv - wv, s_wp[lane] = cp - wp;
-        // decoupled look-back (warp-parallel window of 32 predecessors)
-        volatile unsigned long long* st = f.scan_state;
-        if (lane == 0) st[tile] = st_pack(tile == 0 ? ST_PREFIX : ST_AGG, tot_v, tot_p, epoch);
-        uint32_t ex_v = 0, ex_p = 0;
-        int64_t look = (int64_t)tile - 1;
-        while (look >= 0) {
-            const int64_t t = look - lane;
-            unsigned long long s = 0;
-            bool ready = (t < 0);
-            while (!__all_sync(0xffffffffu, ready)) {
-                if (!ready) {
-                    s = st[t];
-                    ready = ((s & ST_FLAGS) != 0) && st_epoch(s) == epoch;
-                }
-            }
-            const bool is_prefix = (t >= 0) && ((s & ST_FLAGS) == ST_PREFIX);
-            const uint32_t pm = __ballot_sync(0xffffffffu, is_prefix);
-            const int stop = pm ? (__ffs(pm) - 1) : 31;         // nearest predecessor holding an inclusive prefix
-            uint32_t cv2 = (t >= 0 && lane <= stop) ? st_vis(s) : 0u, cp2 = (t >= 0 && lane <= stop) ? st_pairs(s) : 0u;
-#pragma unroll
-            for (int d = 16; d > 0; d >>= 1) {
-                cv2 += __shfl_xor_sync(0xffffffffu, cv2, d);
-                cp2 += __shfl_xor_sync(0xffffffffu, cp2, d);
-            }
-            ex_v += cv2, ex_p += cp2;
-            if (pm) break;
-            look -= 32;
-        }
-        if (lane == 0) {
-            if (tile != 0) st[tile] = st_pack(ST_PREFIX, ex_v + tot_v, ex_p + tot_p, epoch);
-            s_excl_vis = ex_v, s_excl_pairs = ex_p;
-            if (tile == f.n_proj_tiles - 1) {
-                const uint32_t nv = ex_v + tot_v, np = ex_p + tot_p;
-                ctrl->n_visible = nv, ctrl->n_pairs = np;
-                uint32_t fl = 0;
-                if (np > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
-                if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
-                ctrl->flags = fl;
-            }
-        }
+        s_base = tot ? atomicAdd(&f.ctrl->vis_counter, tot) : 0u;
     }
     __syncthreads();
     if (o.vis) {
-        const uint32_t slot = s_excl_vis + s_wv[warp] + iv - 1u;
-        uint32_t poff = s_excl_pairs + s_wp[warp] + ip - o.tiles;
+        const uint32_t slot = s_base + s_w[warp] + __popc(bal & ((1u << lane) - 1u));
         if (slot < f.vis_cap) {
             const uint32_t m = (uint32_t)(face0 + tid);
             float ob;
@@ -190,36 +131,69 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
                       __ldg(opacity + __ldg(faces + 3 * (int64_t)m + 2))) * (1.0f / 3.0f);
             }
             const int rlo = (o.x0 & 0xffff) | (o.y0 << 16), rhi = (o.x1 & 0xffff) | (o.y1 << 16);
-            f.vis_face[slot] = m;
-            f.rect[slot] = make_int2(rlo, rhi);
-            f.depth_key[slot] = o.key;
-            f.tiles_touched[slot] = o.tiles;
-            float4* s4 = f.scr + 3 * (int64_t)slot;
+            float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
             s4[0] = make_float4(o.u[0], o.v[0], o.w[0], o.u[1]);
             s4[1] = make_float4(o.v[1], o.w[1], o.u[2], o.v[2]);
             s4[2] = make_float4(o.w[2], ob, __int_as_float(rlo), __int_as_float(rhi));
-            // F6 emission: ty-major then tx, face order is the scan order
+            s4[3] = make_float4(__uint_as_float(m), __uint_as_float(o.key), __uint_as_float(o.tiles), 0.0f);
             for (int ty = o.y0 >> 4; ty <= (o.y1 >> 4); ++ty)
-                for (int tx = o.x0 >> 4; tx <= (o.x1 >> 4); ++tx) {
-                    if (poff < f.pair_cap) {
-                        f.keys[0][poff] = ((unsigned long long)(uint32_t)(ty * f.tiles_x + tx) << 32) | o.key;
-                        f.vals[0][poff] = slot;
-                    }
-                    ++poff;
-                }
+                for (int tx = o.x0 >> 4; tx <= (o.x1 >> 4); ++tx) atomicAdd(f.tile_count + ty * f.tiles_x + tx, 1u);
         }
     }
-    // the last block to finish re-arms the tickets and advances the epoch for the next call
+
+    // ---- last CTA: tile counts -> ranges / cursors, publish the frame counters, re-arm ----
     __syncthreads();
     if (tid == 0) {
         __threadfence();
-        const uint32_t done = atomicAdd((uint32_t*)&f.ctrl->proj_done, 1u);
-        if (done == gridDim.x - 1) {
-            ctrl->proj_done = 0;
-            ctrl->proj_ticket = 0;
-            ctrl->epoch = (epoch % 15u) + 1u;
-            __threadfence();
-        }
+        s_last = (atomicAdd(&f.ctrl->proj_done, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    volatile TsCtrl* ctrl = f.ctrl;
+    const uint32_t nv = ctrl->vis_counter;
+    const int per = (f.NT + TS_PROJ_THREADS - 1) / TS_PROJ_THREADS;
+    const int t0 = tid * per, t1 = min(f.NT, t0 + per);
+    uint32_t sum = 0, mx = 0;
+#pragma unroll 8
+    for (int t = t0; t < t1; ++t) {
+        const uint32_t c = __ldcg(f.tile_count + t);
+        sum += c;
+        mx = max(mx, c);
+    }
+    // block exclusive scan of the per-thread sums
+    uint32_t incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+    }
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    __shared__ uint32_t s_ws[TS_PROJ_THREADS / 32], s_wm[TS_PROJ_THREADS / 32];
+    if (lane == 31) s_ws[warp] = incl;
+    if (lane == 0) s_wm[warp] = mx;
+    __syncthreads();
+    uint32_t woff = 0, total = 0, gmax = 0;
+#pragma unroll
+    for (int w = 0; w < TS_PROJ_THREADS / 32; ++w) {
+        if (w < warp) woff += s_ws[w];
+        total += s_ws[w];
+        gmax = max(gmax, s_wm[w]);
+    }
+    uint32_t fl = 0;
+    if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
+    if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
+    uint32_t run = woff + incl - sum;
+    for (int t = t0; t < t1; ++t) {
+        const uint32_t c = __ldcg(f.tile_count + t);
+        f.tile_ranges[t] = (fl || c == 0u) ? make_uint2(0u, 0u) : make_uint2(run, run + c);   // empty tile = (0,0)
+        f.tile_cursor[t] = run;
+        f.tile_count[t] = 0u;
+        run += c;
+    }
+    if (tid == 0) {
+        ctrl->n_visible = nv, ctrl->n_pairs = total, ctrl->flags = fl, ctrl->max_list = gmax;
+        ctrl->vis_counter = 0u, ctrl->proj_done = 0u;
     }
 }
 
@@ -229,12 +203,13 @@ int32_t ts_launch_project(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, c
     (void)ctx;
     const TsFrameDev& f = fr->d;
     const int aligned = ((reinterpret_cast<uintptr_t>(sc->pos) & 15u) == 0) ? 1 : 0;
+    const uint32_t grid = (uint32_t)((f.M + TS_PROJ_THREADS - 1) / TS_PROJ_THREADS);
     if (sc->faces == nullptr)
-        project_kernel<true><<<f.n_proj_tiles, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, nullptr, sc->opacity, fr->T_cw,
-                                                                             fr->cam, fr->prm.eps_area, aligned);
+        project_kernel<true><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, nullptr, sc->opacity, fr->T_cw, fr->cam,
+                                                                   fr->prm.eps_area, aligned);
     else
-        project_kernel<false><<<f.n_proj_tiles, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, sc->faces, sc->opacity,
-                                                                              fr->T_cw, fr->cam, fr->prm.eps_area, aligned);
+        project_kernel<false><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, sc->faces, sc->opacity, fr->T_cw,
+                                                                    fr->cam, fr->prm.eps_area, aligned);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

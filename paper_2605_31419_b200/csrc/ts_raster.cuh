@@ -1,7 +1,8 @@
-// ts_raster.cuh -- per-face setup (F7) and per-(pixel, face) window evaluation (F8.1-3) shared by the forward and
-// backward compositing kernels.  Every operation that decides alpha is written with explicit round-to-nearest
-// intrinsics so that the backward kernel recomputes bit-identical alpha / transmittance values (no freedom for
-// the compiler to contract differently in the two kernels).
+// ts_raster.cuh -- the per-face render record (F7), written once per visible face by the binning kernel, and the
+// per-(pixel, face) window evaluation (F8.1-3) shared by the forward and backward compositing kernels.  Every
+// operation that decides alpha is written with explicit round-to-nearest intrinsics so that the backward kernel
+// recomputes bit-identical alpha / transmittance values (no freedom for the compiler to contract differently in
+// the two kernels).
 //
 // Formulation: with the incentre-normalised edge functions
 //     lhat_k(p) = L_k(p) / r = m_k . (p - ref) + c_k,   m_k = n_k / r,   c_k = n_k . (ref - q_{k+1}) / r
@@ -9,6 +10,16 @@
 //     phi(p)/phi(s) = -max_k lhat_k(p) =: x,     I = x^sigma  (x > 0).
 // Screen barycentrics are b_k = -lhat_k * rho_k with rho_k = r/h_k = ell_k / sum(ell), and the perspective
 // weights are omega_k = lhat_k * kappa_k with kappa_k = -rho_k w_k.
+//
+// Record layout, 10 float4 = 160 B per visible face (global memory, f.rec + 10 * slot):
+//   R0  refx  refy  m0x   m0y        R5  w0     w1     w2     tau0
+//   R1  m1x   m1y   m2x   m2y        R6  tau1   tau2   drr0x  drr0y
+//   R2  c0    c1    c2    obar       R7  drr1x  drr1y  drr2x  drr2y
+//   R3  kap0  kap1  kap2  rect_lo    R8  xn0    yn0    xn1    yn1
+//   R4  rho0  rho1  rho2  rect_hi    R9  xn2    yn2    -      -
+// R0-R2 decide alpha (forward and backward), R3 interpolates, R4-R7 are the backward-only geometry terms
+// (tau_k = foot of vertex k on its opposite edge, drr_j = -(1/r) dr/dq_j), R8-R9 the normalised camera
+// coordinates (X/Z, Y/Z) of the vertices for the in-kernel se(3) terms.
 #pragma once
 #include "ts_internal.cuh"
 
@@ -18,7 +29,6 @@ struct TsGeom {
     float absS, sgn, sumell, inv_sumell, r, inv_r;
     float refx, refy, mx[3], my[3], c[3], rho[3], kap[3];
     float obar;
-    int x0, y0, x1, y1;
 };
 
 __device__ __forceinline__ float ts_sqrt_approx(float x) {
@@ -32,8 +42,6 @@ __device__ __forceinline__ void ts_face_geom(const float4 s0, const float4 s1, c
     g.qx[1] = s0.w, g.qy[1] = s1.x, g.w[1] = s1.y;
     g.qx[2] = s1.z, g.qy[2] = s1.w, g.w[2] = s2.x;
     g.obar = s2.y;
-    const int rlo = __float_as_int(s2.z), rhi = __float_as_int(s2.w);
-    g.x0 = (int)(short)(rlo & 0xffff), g.y0 = rlo >> 16, g.x1 = (int)(short)(rhi & 0xffff), g.y1 = rhi >> 16;
     // signed doubled area with the same operation order as the projection (N3): same sign on both sides
     const float a = __fsub_rn(g.qx[1], g.qx[0]), b = __fsub_rn(g.qy[2], g.qy[0]);
     const float c = __fsub_rn(g.qy[1], g.qy[0]), d = __fsub_rn(g.qx[2], g.qx[0]);
@@ -68,6 +76,40 @@ __device__ __forceinline__ void ts_face_geom(const float4 s0, const float4 s1, c
         g.rho[k] = __fmul_rn(g.ell[k], g.inv_sumell);
         g.kap[k] = -__fmul_rn(g.rho[k], g.w[k]);
     }
+}
+
+// F7 + the backward-only per-face terms -> the 10-float4 record.  s0..s2 = raw screen record, cam for (xn, yn).
+__device__ __forceinline__ void ts_build_record(const float4 s0, const float4 s1, const float4 s2, const TsCamDev& cam,
+                                                float4* __restrict__ out) {
+    TsGeom g;
+    ts_face_geom(s0, s1, s2, g);
+    // d r / d q_j = -rho_j n_j - (r / sum ell) (u_{j,j+1} + u_{j,j+2}),  u_{j,i} = (q_j - q_i)/|q_j - q_i|;
+    // stored as drr_j = -(1/r) dr/dq_j so that gq_j += (x * gx) * drr_j  (B6 iii)
+    float drrx[3], drry[3], tau[3], xn[3], yn[3];
+    const float rs = g.r * g.inv_sumell;
+    const float ifx = 1.0f / cam.fx, ify = 1.0f / cam.fy;
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+        const int i1 = (j + 1) % 3, i2 = (j + 2) % 3;
+        const float u1x = (g.qx[j] - g.qx[i1]) * g.inv_ell[i2], u1y = (g.qy[j] - g.qy[i1]) * g.inv_ell[i2];
+        const float u2x = (g.qx[j] - g.qx[i2]) * g.inv_ell[i1], u2y = (g.qy[j] - g.qy[i2]) * g.inv_ell[i1];
+        const float drx = -g.rho[j] * g.nx[j] - rs * (u1x + u2x), dry = -g.rho[j] * g.ny[j] - rs * (u1y + u2y);
+        drrx[j] = -drx * g.inv_r, drry[j] = -dry * g.inv_r;
+        // edge j runs from a = q_{j+1} to b = q_{j+2}; tau_j = ((q_j - a) . e) / |e|^2  (B6 ii)
+        const float ex = g.qx[i2] - g.qx[i1], ey = g.qy[i2] - g.qy[i1];
+        tau[j] = ((g.qx[j] - g.qx[i1]) * ex + (g.qy[j] - g.qy[i1]) * ey) * (g.inv_ell[j] * g.inv_ell[j]);
+        xn[j] = (g.qx[j] - cam.cx) * ifx, yn[j] = (g.qy[j] - cam.cy) * ify;
+    }
+    out[0] = make_float4(g.refx, g.refy, g.mx[0], g.my[0]);
+    out[1] = make_float4(g.mx[1], g.my[1], g.mx[2], g.my[2]);
+    out[2] = make_float4(g.c[0], g.c[1], g.c[2], g.obar);
+    out[3] = make_float4(g.kap[0], g.kap[1], g.kap[2], s2.z);
+    out[4] = make_float4(g.rho[0], g.rho[1], g.rho[2], s2.w);
+    out[5] = make_float4(g.w[0], g.w[1], g.w[2], tau[0]);
+    out[6] = make_float4(tau[1], tau[2], drrx[0], drry[0]);
+    out[7] = make_float4(drrx[1], drry[1], drrx[2], drry[2]);
+    out[8] = make_float4(xn[0], yn[0], xn[1], yn[1]);
+    out[9] = make_float4(xn[2], yn[2], 0.0f, 0.0f);
 }
 
 // sigma dispatch: 0 = generic exp2(sigma log2 x), 1 = sigma 1, 2 = sigma 0.5, 3 = sigma 2
@@ -114,16 +156,15 @@ static __device__ __noinline__ float3 ts_refine_lhat(const float4* __restrict__ 
 }
 
 // F8.1-3.  Returns true if the face contributes at (px,py); l[] = lhat_k, x, I, alpha are outputs.
-// `s4` points at the face's raw screen record (only read inside the refinement band).
+// r0..r2 = record rows R0-R2; `s4` points at the face's raw screen record (only read inside the refinement band).
 template <int SM>
-__device__ __forceinline__ bool ts_eval_alpha(float refx, float refy, float m0x, float m0y, float m1x, float m1y,
-                                              float m2x, float m2y, float c0, float c1, float c2, float obar, float px,
-                                              float py, float sigma, float alpha_min, const float4* __restrict__ s4,
-                                              float l[3], float& x, float& I, float& alpha) {
-    const float dx = __fsub_rn(px, refx), dy = __fsub_rn(py, refy);
-    l[0] = __fmaf_rn(m0x, dx, __fmaf_rn(m0y, dy, c0));
-    l[1] = __fmaf_rn(m1x, dx, __fmaf_rn(m1y, dy, c1));
-    l[2] = __fmaf_rn(m2x, dx, __fmaf_rn(m2y, dy, c2));
+__device__ __forceinline__ bool ts_eval_alpha(const float4 r0, const float4 r1, const float4 r2, float px, float py,
+                                              float sigma, float alpha_min, const float4* __restrict__ s4, float l[3],
+                                              float& x, float& I, float& alpha) {
+    const float dx = __fsub_rn(px, r0.x), dy = __fsub_rn(py, r0.y);
+    l[0] = __fmaf_rn(r0.z, dx, __fmaf_rn(r0.w, dy, r2.x));
+    l[1] = __fmaf_rn(r1.x, dx, __fmaf_rn(r1.y, dy, r2.y));
+    l[2] = __fmaf_rn(r1.z, dx, __fmaf_rn(r1.w, dy, r2.z));
     x = -fmaxf(l[0], fmaxf(l[1], l[2]));
     if (fabsf(x) < TS_REFINE_BAND) {
         const float3 lr = ts_refine_lhat(s4, px, py);
@@ -132,29 +173,26 @@ __device__ __forceinline__ bool ts_eval_alpha(float refx, float refy, float m0x,
     }
     if (!(x > 0.0f)) return false;
     I = ts_window_pow<SM>(x, sigma);
-    alpha = __fmul_rn(obar, I);
+    alpha = __fmul_rn(r2.w, I);
     return alpha >= alpha_min;
 }
 
-// thread -> pixel mapping inside a 16x16 tile: warp w owns the 8x4 block at (8*(w&1), 4*(w>>1)); keeping a warp's
-// pixels compact lets whole warps skip faces whose pixel rect misses their block.
+// thread -> pixel mapping inside a 16x16 tile: warp w owns the 8x4 block at (8*(w&1), 4*(w>>1)), lane l the pixel
+// (l & 7, l >> 3) of it; keeping a warp's pixels compact lets whole warps skip faces whose rect misses their block.
 __device__ __forceinline__ void ts_thread_pixel(int tid, int& lx, int& ly) {
     const int w = tid >> 5, l = tid & 31;
     lx = ((w & 1) << 3) + (l & 7);
     ly = ((w >> 1) << 2) + (l >> 3);
 }
 
-// 8-bit mask of the warp blocks a pixel rect (tile-relative, clamped to 0..15) overlaps
-__device__ __forceinline__ uint32_t ts_subtile_mask(int rx0, int ry0, int rx1, int ry1) {
-    uint32_t colm = 0, rowm = 0;
-    if (rx0 <= 7) colm |= 1u;
-    if (rx1 >= 8) colm |= 2u;
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-        if (ry0 <= 4 * j + 3 && ry1 >= 4 * j) rowm |= (1u << j);
-    uint32_t m = 0;
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-        if (rowm & (1u << j)) m |= colm << (2 * j);
-    return m;
+// 32-bit lane mask of warp block `w`: bit l set iff lane l's pixel lies inside the tile-relative rect
+// [rx0,rx1] x [ry0,ry1] (already clamped to 0..15).
+__device__ __forceinline__ uint32_t ts_lane_mask(int w, int rx0, int ry0, int rx1, int ry1) {
+    const int bx = (w & 1) << 3, by = (w >> 1) << 2;
+    const int cx0 = max(rx0 - bx, 0), cx1 = min(rx1 - bx, 7);
+    const int cy0 = max(ry0 - by, 0), cy1 = min(ry1 - by, 3);
+    if (cx0 > cx1 || cy0 > cy1) return 0u;
+    const uint32_t col = ((2u << cx1) - (1u << cx0)) & 0xffu;
+    const uint32_t rows = (0xffffffffu >> (8 * (3 - cy1))) & (0xffffffffu << (8 * cy0));
+    return (col * 0x01010101u) & rows;
 }

@@ -1,65 +1,30 @@
 // ts_render_bwd.cu -- a5/a6/a7: reverse-order backward of the compositing (B1-B9).
 //   render_bwd_kernel : one CTA per tile, one thread per pixel, walks the tile list BACK from the last
 //       contributing entry; recomputes alpha bit-identically to the forward kernel (ts_raster.cuh), recovers the
-//       transmittance in front of each face by T_n = T_{n+1}/(1-alpha_n), keeps the "behind" accumulators
-//       R^c, R^d, R^a (no division by T), and forms the per-hit gradients wrt the face's screen vertices
-//       (u,v,w) x 3, its vertex colours and its opacity.  Per face these are reduced across the warp with
-//       shuffles BEFORE any global atomic (one lane issues the RED.ADD.F32s).
-//   proj_bwd_kernel   : per visible face, screen -> camera -> world (B7-B8) and the se(3) terms
-//       [g_C ; Q x g_C] of Eq. 5-7, tree-reduced per CTA into fixed-order partials.
+//       transmittance in front of each face by T_n = T_{n+1}/(1-alpha_n), keeps ONE scalar "behind" accumulator
+//       R = R^c.gC + R^d gD + R^a gA (no division by T), and forms the per-hit gradients wrt the face's screen
+//       vertices (u,v,w) x 3, its vertex colours and its opacity.
+//       POSE-ONLY mode (tracking): every hit's nine screen terms are pushed straight through d(u,v,w)/dtau
+//       (Eq. 5-7) into six per-thread accumulators -- no shuffle, no atomic, no per-face
+//       buffer -- which are tree-reduced once per CTA into a per-tile partial (deterministic).
+//       FULL mode (mapping): per face the terms are reduced across the warp with shuffles BEFORE any global
+//       atomic (lane j issues the RED.ADD.F32 of term j).
+//   proj_bwd_kernel   : full mode only; per visible face, screen -> camera -> world (B7-B8) and the se(3) terms
+//       [g_C ; Q x g_C], tree-reduced per CTA into fixed-order partials.
 //   pose_reduce_kernel: fixed-order final reduction of the partials to dL/dtau[6].
 #include "ts_raster.cuh"
 
 namespace {
 
-struct BwdRec { float4 r[12]; };   // 192 B, see stage_face_bwd()
-
-__device__ __forceinline__ void stage_face_bwd(const TsFrameDev& f, const ts_scene& sc, uint32_t slot, BwdRec& out,
-                                               uint32_t& face, int& x0, int& y0, int& x1, int& y1) {
-    const float4* s4 = f.scr + 3 * (size_t)slot;
-    const float4 s0 = __ldg(s4), s1 = __ldg(s4 + 1), s2 = __ldg(s4 + 2);
-    TsGeom g;
-    ts_face_geom(s0, s1, s2, g);
-    const uint32_t m = __ldg(f.vis_face + slot);
-    face = m;
-    float col[9];
-    if (sc.faces == nullptr) {
-        const float* cp = sc.color + 9 * (size_t)m;
-#pragma unroll
-        for (int j = 0; j < 9; ++j) col[j] = __ldg(cp + j);
-    } else {
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            const float* cp = sc.color + 3 * (size_t)__ldg(sc.faces + 3 * (size_t)m + k);
-            col[3 * k] = __ldg(cp), col[3 * k + 1] = __ldg(cp + 1), col[3 * k + 2] = __ldg(cp + 2);
-        }
-    }
-    // d r / d q_j = -rho_j n_j - (r / sum ell) (u_{j,j+1} + u_{j,j+2}),  u_{j,i} = (q_j - q_i)/|q_j - q_i|;
-    // stored as drr_j = -(1/r) dr/dq_j so that gq_j += (x * gx) * drr_j  (B6 iii)
-    float drrx[3], drry[3];
-    const float rs = g.r * g.inv_sumell;
-#pragma unroll
-    for (int j = 0; j < 3; ++j) {
-        const int i1 = (j + 1) % 3, i2 = (j + 2) % 3;
-        const float u1x = (g.qx[j] - g.qx[i1]) * g.inv_ell[i2], u1y = (g.qy[j] - g.qy[i1]) * g.inv_ell[i2];
-        const float u2x = (g.qx[j] - g.qx[i2]) * g.inv_ell[i1], u2y = (g.qy[j] - g.qy[i2]) * g.inv_ell[i1];
-        const float drx = -g.rho[j] * g.nx[j] - rs * (u1x + u2x), dry = -g.rho[j] * g.ny[j] - rs * (u1y + u2y);
-        drrx[j] = -drx * g.inv_r, drry[j] = -dry * g.inv_r;
-    }
-    out.r[0] = make_float4(g.refx, g.refy, s2.z, s2.w);
-    out.r[1] = make_float4(g.mx[0], g.my[0], g.mx[1], g.my[1]);
-    out.r[2] = make_float4(g.mx[2], g.my[2], g.c[0], g.c[1]);
-    out.r[3] = make_float4(g.c[2], g.obar, g.kap[0], g.kap[1]);
-    out.r[4] = make_float4(g.kap[2], col[0], col[1], col[2]);
-    out.r[5] = make_float4(col[3], col[4], col[5], col[6]);
-    out.r[6] = make_float4(col[7], col[8], g.rho[0], g.rho[1]);
-    out.r[7] = make_float4(g.rho[2], g.w[0], g.w[1], g.w[2]);
-    out.r[8] = make_float4(g.qx[0] - g.refx, g.qy[0] - g.refy, g.qx[1] - g.refx, g.qy[1] - g.refy);
-    out.r[9] = make_float4(g.qx[2] - g.refx, g.qy[2] - g.refy, g.inv_ell[0] * g.inv_ell[0], g.inv_ell[1] * g.inv_ell[1]);
-    out.r[10] = make_float4(g.inv_ell[2] * g.inv_ell[2], drrx[0], drry[0], drrx[1]);
-    out.r[11] = make_float4(drry[1], drrx[2], drry[2], __uint_as_float(slot));
-    x0 = g.x0, y0 = g.y0, x1 = g.x1, y1 = g.y1;
-}
+struct BwdSmem {
+    float4 r[TS_BATCH_BWD][12];       // R0 R1 R2 | kap,c00 | colours | colours | R4 R5 R6 R7 | R8 R9
+    uint32_t lm[8][TS_BATCH_BWD];
+    uint32_t slot[TS_BATCH_BWD];
+    uint32_t face[TS_BATCH_BWD];
+    uint32_t masks[8][TS_BATCH_BWD / 32];
+    uint32_t s_max;
+    float red[8][6];
+};
 
 __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll
@@ -67,16 +32,14 @@ __device__ __forceinline__ float warp_sum(float v) {
     return v;
 }
 
-// ATTR: also colour / opacity gradients (B1, B4).  GEOM: screen-space vertex gradients (B5-B6).
-template <int SM, bool ATTR, bool GEOM>
+// ATTR: colour / opacity gradients (B1, B4).  GEOM: screen-space vertex gradients into gscr (B5-B6).
+// POSE: screen-space vertex gradients pushed through Eq. 5-7 into per-thread se(3) accumulators (pose-only).
+template <int SM, bool ATTR, bool GEOM, bool POSE>
 __global__ void __launch_bounds__(256)
-render_bwd_kernel(TsFrameDev f, ts_scene sc, const uint32_t* __restrict__ vals, float sigma, float alpha_min,
+render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float fx, float fy,
                   const float* __restrict__ gCi, const float* __restrict__ gDi, const float* __restrict__ gAi,
                   float* __restrict__ grad_color, float* __restrict__ grad_opacity) {
-    __shared__ BwdRec recs[TS_BATCH];
-    __shared__ uint32_t faces_s[TS_BATCH];
-    __shared__ uint32_t masks[8][TS_BATCH / 32];
-    __shared__ uint32_t s_max;
+    __shared__ BwdSmem sm;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x, tx0 = (tile % f.tiles_x) * TS_TILE, ty0 = (tile / f.tiles_x) * TS_TILE;
     int lx, ly;
@@ -84,8 +47,7 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, const uint32_t* __restrict__ vals, 
     const int px = tx0 + lx, py = ty0 + ly;
     const bool inside = px < f.W && py < f.H;
     const float fpx = (float)px, fpy = (float)py;
-    uint2 range = f.tile_ranges[tile];
-    if (ts_eff_pairs(f) == 0) range = make_uint2(0u, 0u);
+    const uint2 range = f.tile_ranges[tile];
     const size_t p = (size_t)py * f.W + px, hw = (size_t)f.W * f.H;
     uint32_t ncon = 0;
     float Tcur = 1.0f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f;
@@ -96,78 +58,105 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, const uint32_t* __restrict__ vals, 
         if (gDi) gD = gDi[p];
         if (gAi) gA = gAi[p];
     }
-    if (tid == 0) s_max = 0;
+    if (tid == 0) sm.s_max = 0;
     __syncthreads();
     const uint32_t wmax = __reduce_max_sync(0xffffffffu, ncon);
-    if (lane == 0 && wmax) atomicMax(&s_max, wmax);
+    if (lane == 0 && wmax) atomicMax(&sm.s_max, wmax);
     __syncthreads();
-    const uint32_t n_walk = min(s_max, range.y - range.x);
-    float Rc0 = 0.f, Rc1 = 0.f, Rc2 = 0.f, Rd = 0.f, Ra = 0.f;
+    const uint32_t n_walk = min(sm.s_max, range.y - range.x);
+    float Rs = 0.f;                    // R^c.gC + R^d gD + R^a gA behind the current face
+    float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     bool first = true;
 
     for (uint32_t hi = n_walk; hi > 0;) {
-        const uint32_t lo = hi > TS_BATCH ? hi - TS_BATCH : 0u;
+        const uint32_t lo = hi > TS_BATCH_BWD ? hi - TS_BATCH_BWD : 0u;
         const int nb = (int)(hi - lo);
         __syncthreads();
-        if (tid < TS_BATCH) {
-            uint32_t sub = 0;
+        if (tid < TS_BATCH_BWD) {
+            uint32_t lmask[8];
+#pragma unroll
+            for (int w = 0; w < 8; ++w) lmask[w] = 0u;
             if (tid < nb) {
-                int x0, y0, x1, y1;
-                uint32_t face;
-                stage_face_bwd(f, sc, __ldg(vals + range.x + lo + tid), recs[tid], face, x0, y0, x1, y1);
-                faces_s[tid] = face;
-                sub = ts_subtile_mask(max(x0 - tx0, 0), max(y0 - ty0, 0), min(x1 - tx0, 15), min(y1 - ty0, 15));
+                const uint2 sf = f.sorted[range.x + lo + tid];   // (slot, face)
+                const float4* rp = f.rec + TS_REC_F4 * (size_t)sf.x;
+                float4 r[TS_REC_F4];
+#pragma unroll
+                for (int i = 0; i < (POSE ? 10 : 8); ++i) r[i] = __ldg(rp + i);
+                float col[9];
+                if (sc.faces == nullptr) {
+                    const float* cp = sc.color + 9 * (size_t)sf.y;
+#pragma unroll
+                    for (int j = 0; j < 9; ++j) col[j] = __ldg(cp + j);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        const float* cp = sc.color + 3 * (size_t)__ldg(sc.faces + 3 * (size_t)sf.y + k);
+                        col[3 * k] = __ldg(cp), col[3 * k + 1] = __ldg(cp + 1), col[3 * k + 2] = __ldg(cp + 2);
+                    }
+                }
+                float4* d = sm.r[tid];
+                d[0] = r[0], d[1] = r[1], d[2] = r[2];
+                d[3] = make_float4(r[3].x, r[3].y, r[3].z, col[0]);
+                d[4] = make_float4(col[1], col[2], col[3], col[4]);
+                d[5] = make_float4(col[5], col[6], col[7], col[8]);
+                d[6] = r[4], d[7] = r[5], d[8] = r[6], d[9] = r[7];
+                if (POSE) d[10] = r[8], d[11] = r[9];
+                sm.slot[tid] = sf.x, sm.face[tid] = sf.y;
+                const int rlo = __float_as_int(r[3].w), rhi = __float_as_int(r[4].w);
+                const int rx0 = max((int)(short)(rlo & 0xffff) - tx0, 0), ry0 = max((rlo >> 16) - ty0, 0);
+                const int rx1 = min((int)(short)(rhi & 0xffff) - tx0, 15), ry1 = min((rhi >> 16) - ty0, 15);
+#pragma unroll
+                for (int w = 0; w < 8; ++w) lmask[w] = ts_lane_mask(w, rx0, ry0, rx1, ry1);
             }
 #pragma unroll
             for (int w = 0; w < 8; ++w) {
-                const uint32_t bal = __ballot_sync(0xffffffffu, (sub >> w) & 1u);
-                if (lane == 0) masks[w][warp] = bal;
+                sm.lm[w][tid] = lmask[w];
+                const uint32_t bal = __ballot_sync(0xffffffffu, lmask[w] != 0u);
+                if (lane == 0) sm.masks[w][warp] = bal;
             }
         }
         __syncthreads();
         if (wmax > lo) {
             for (int g = (nb - 1) >> 5; g >= 0; --g) {
-                uint32_t mk = masks[warp][g];
+                uint32_t mk = sm.masks[warp][g];
                 while (mk) {
                     const int bit = 31 - __clz(mk);
                     mk &= ~(1u << bit);
                     const int e = (g << 5) + bit;
                     const uint32_t idx = lo + (uint32_t)e;          // list position relative to range.x
-                    const BwdRec& R = recs[e];
-                    const float4 r0 = R.r[0];
-                    const int rlo = __float_as_int(r0.z), rhi = __float_as_int(r0.w);
-                    const bool in_rect = idx < ncon && px >= (int)(short)(rlo & 0xffff) && px <= (int)(short)(rhi & 0xffff) &&
-                                         py >= (rlo >> 16) && py <= (rhi >> 16);
+                    const bool in_rect = idx < ncon && ((sm.lm[warp][e] >> lane) & 1u);
                     if (!__any_sync(0xffffffffu, in_rect)) continue;
-                    const float4 r1 = R.r[1], r2 = R.r[2], r3 = R.r[3];
-                    const float4* s4 = f.scr + 3 * (size_t)__float_as_uint(R.r[11].w);
+                    const float4* R = sm.r[e];
+                    const float4 r0 = R[0], r1 = R[1], r2 = R[2];
+                    const float4* s4 = f.scr + TS_SCR_F4 * (size_t)sm.slot[e];
                     float l[3], x, I, alpha;
-                    const bool hit = in_rect && ts_eval_alpha<SM>(r0.x, r0.y, r1.x, r1.y, r1.z, r1.w, r2.x, r2.y, r2.z,
-                                                                  r2.w, r3.x, r3.y, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
+                    const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
                     const uint32_t hm = __ballot_sync(0xffffffffu, hit);
                     if (!hm) continue;
-                    const float4 r4 = R.r[4], r5 = R.r[5], r6 = R.r[6];
                     float acc[19];
+                    if (!POSE) {
 #pragma unroll
-                    for (int j = 0; j < 19; ++j) acc[j] = 0.f;
+                        for (int j = 0; j < 19; ++j) acc[j] = 0.f;
+                    }
                     if (hit) {
+                        const float4 r3 = R[3], r4 = R[4], r5 = R[5];
                         // transmittance in front of this face
                         const float one_m = __fsub_rn(1.0f, alpha);
-                        const float Tn = first ? Tcur : __fdiv_rn(Tcur, one_m);
+                        const float Tn = first ? Tcur : __fdividef(Tcur, one_m);
                         Tcur = Tn, first = false;
-                        const float o0 = l[0] * r3.z, o1 = l[1] * r3.w, o2 = l[2] * r4.x;
+                        const float o0 = l[0] * r3.x, o1 = l[1] * r3.y, o2 = l[2] * r3.z;
                         const float Om = (o0 + o1) + o2, z = __fdividef(1.0f, Om);
                         const float lam0 = o0 * z, lam1 = o1 * z, lam2 = o2 * z;
-                        const float c0 = lam0 * r4.y + lam1 * r5.x + lam2 * r5.w;
-                        const float c1 = lam0 * r4.z + lam1 * r5.y + lam2 * r6.x;
-                        const float c2 = lam0 * r4.w + lam1 * r5.z + lam2 * r6.y;
+                        // d_k = c_k . gC
+                        const float d0 = r3.w * gC0 + r4.x * gC1 + r4.y * gC2;
+                        const float d1 = r4.z * gC0 + r4.w * gC1 + r5.x * gC2;
+                        const float d2 = r5.y * gC0 + r5.z * gC1 + r5.w * gC2;
+                        const float cg = lam0 * d0 + lam1 * d1 + lam2 * d2;       // c . gC
+                        const float zgd = z * gD;
+                        const float S = cg + zgd + gA;
                         const float wgt = Tn * alpha;
-                        // B2
-                        const float ga = Tn * ((c0 - Rc0) * gC0 + (c1 - Rc1) * gC1 + (c2 - Rc2) * gC2 + (z - Rd) * gD +
-                                               (1.0f - Ra) * gA);
-                        // B3
-                        Rc0 = alpha * c0 + one_m * Rc0, Rc1 = alpha * c1 + one_m * Rc1, Rc2 = alpha * c2 + one_m * Rc2;
-                        Rd = alpha * z + one_m * Rd, Ra = alpha + one_m * Ra;
+                        const float ga = Tn * (S - Rs);                           // B2
+                        Rs = alpha * S + one_m * Rs;                              // B3
                         if (ATTR) {
                             // B1 colours, B4 opacity (one value per face; /3 applied when written)
                             const float w0 = lam0 * wgt, w1 = lam1 * wgt, w2 = lam2 * wgt;
@@ -176,83 +165,101 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, const uint32_t* __restrict__ vals, 
                             acc[15] = w2 * gC0, acc[16] = w2 * gC1, acc[17] = w2 * gC2;
                             acc[18] = I * ga;
                         }
-                        if (GEOM) {
-                            const float4 r7 = R.r[7], r8 = R.r[8], r9 = R.r[9], r10 = R.r[10], r11 = R.r[11];
+                        if (GEOM || POSE) {
+                            const float4 q4 = R[6], q5 = R[7], q6 = R[8], q7 = R[9];   // record rows R4..R7
                             // B4 window: gx = dL/dx
-                            const float gI = r3.y * ga;
+                            const float gI = r2.w * ga;
                             float gx;
                             if (SM == 1) gx = gI;
                             else if (SM == 2) gx = 0.5f * gI * __fdividef(1.0f, I);
                             else if (SM == 3) gx = 2.0f * gI * x;
                             else gx = gI * sigma * I * __fdividef(1.0f, x);
                             // B5 interpolation
-                            const float cg = c0 * gC0 + c1 * gC1 + c2 * gC2;
-                            const float wz = wgt * z, zgd = z * gD;
-                            const float go0 = wz * ((r4.y * gC0 + r4.z * gC1 + r4.w * gC2) - cg - zgd);
-                            const float go1 = wz * ((r5.x * gC0 + r5.y * gC1 + r5.z * gC2) - cg - zgd);
-                            const float go2 = wz * ((r5.w * gC0 + r6.x * gC1 + r6.y * gC2) - cg - zgd);
-                            const float b0 = -l[0] * r6.z, b1 = -l[1] * r6.w, b2 = -l[2] * r7.x;      // b_k = -lhat_k rho_k
-                            const float gb0 = r7.y * go0, gb1 = r7.z * go1, gb2 = r7.w * go2;         // w_k * gomega_k
-                            acc[2] = b0 * go0, acc[5] = b1 * go1, acc[8] = b2 * go2;                 // dL/dw_k
-                            // B6 (i): G = sum_k gb_k grad_p b_k,  grad_p b_k = -rho_k m_k
-                            const float t0 = gb0 * r6.z, t1 = gb1 * r6.w, t2 = gb2 * r7.x;
-                            const float Gx = -(t0 * r1.x + t1 * r1.z + t2 * r2.x), Gy = -(t0 * r1.y + t1 * r1.w + t2 * r2.y);
+                            const float wz = wgt * z, base = cg + zgd;
+                            const float go0 = wz * (d0 - base), go1 = wz * (d1 - base), go2 = wz * (d2 - base);
+                            const float b0 = -l[0] * q4.x, b1 = -l[1] * q4.y, b2 = -l[2] * q4.z;      // b_k = -lhat_k rho_k
+                            const float gw0 = b0 * go0, gw1 = b1 * go1, gw2 = b2 * go2;               // dL/dw_k
+                            // B6 (i): G = sum_k (w_k go_k) grad_p b_k,  grad_p b_k = -rho_k m_k
+                            const float t0 = q5.x * go0 * q4.x, t1 = q5.y * go1 * q4.y, t2 = q5.z * go2 * q4.z;
+                            const float Gx = -(t0 * r0.z + t1 * r1.x + t2 * r1.z), Gy = -(t0 * r0.w + t1 * r1.y + t2 * r1.w);
                             float q0x = -b0 * Gx, q0y = -b0 * Gy, q1x = -b1 * Gx, q1y = -b1 * Gy, q2x = -b2 * Gx, q2y = -b2 * Gy;
-                            // B6 (ii): x = -lhat_{k*}; edge k* runs from a = q_{k*+1} to b = q_{k*+2}
-                            const int ks = (l[0] >= l[1] && l[0] >= l[2]) ? 0 : (l[1] >= l[2] ? 1 : 2);
-                            const float dx = fpx - r0.x, dy = fpy - r0.y;
-                            float ax, ay, bx, by, mkx, mky, il2;
-                            if (ks == 0) ax = r8.z, ay = r8.w, bx = r9.x, by = r9.y, mkx = r1.x, mky = r1.y, il2 = r9.z;
-                            else if (ks == 1) ax = r9.x, ay = r9.y, bx = r8.x, by = r8.y, mkx = r1.z, mky = r1.w, il2 = r9.w;
-                            else ax = r8.x, ay = r8.y, bx = r8.z, by = r8.w, mkx = r2.x, mky = r2.y, il2 = r10.x;
-                            const float ex = bx - ax, ey = by - ay;
-                            const float t = ((dx - ax) * ex + (dy - ay) * ey) * il2;
-                            const float vax = (1.0f - t) * mkx * gx, vay = (1.0f - t) * mky * gx;
-                            const float vbx = t * mkx * gx, vby = t * mky * gx;
-                            if (ks == 0) q1x += vax, q1y += vay, q2x += vbx, q2y += vby;
-                            else if (ks == 1) q2x += vax, q2y += vay, q0x += vbx, q0y += vby;
-                            else q0x += vax, q0y += vay, q1x += vbx, q1y += vby;
+                            // B6 (ii): x = -lhat_{k*}; edge k* runs from a = q_{k*+1} to b = q_{k*+2};
+                            // t = b_{k*+2} + b_{k*} tau_{k*}
+                            if (l[0] >= l[1] && l[0] >= l[2]) {
+                                const float t = b2 + b0 * q5.w, mgx = r0.z * gx, mgy = r0.w * gx;
+                                q1x += (1.0f - t) * mgx, q1y += (1.0f - t) * mgy, q2x += t * mgx, q2y += t * mgy;
+                            } else if (l[1] >= l[2]) {
+                                const float t = b0 + b1 * q6.x, mgx = r1.x * gx, mgy = r1.y * gx;
+                                q2x += (1.0f - t) * mgx, q2y += (1.0f - t) * mgy, q0x += t * mgx, q0y += t * mgy;
+                            } else {
+                                const float t = b1 + b2 * q6.y, mgx = r1.z * gx, mgy = r1.w * gx;
+                                q0x += (1.0f - t) * mgx, q0y += (1.0f - t) * mgy, q1x += t * mgx, q1y += t * mgy;
+                            }
                             // B6 (iii): through the inradius
                             const float xg = x * gx;
-                            q0x += xg * r10.y, q0y += xg * r10.z, q1x += xg * r10.w, q1y += xg * r11.x;
-                            q2x += xg * r11.y, q2y += xg * r11.z;
-                            acc[0] = q0x, acc[1] = q0y, acc[3] = q1x, acc[4] = q1y, acc[6] = q2x, acc[7] = q2y;
-                        }
-                    }
-                    // reduce across the warp, then one lane issues the atomics
-                    const bool single = (hm & (hm - 1)) == 0;
-                    const int src = __ffs(hm) - 1;
-                    if (!single) {
-                        if (GEOM) {
-#pragma unroll
-                            for (int j = 0; j < 9; ++j) acc[j] = warp_sum(acc[j]);
-                        }
-                        if (ATTR) {
-#pragma unroll
-                            for (int j = 9; j < 19; ++j) acc[j] = warp_sum(acc[j]);
-                        }
-                    }
-                    if (lane == src) {
-                        if (GEOM) {
-                            float* gs = f.gscr + 9 * (size_t)__float_as_uint(R.r[11].w);
-#pragma unroll
-                            for (int j = 0; j < 9; ++j) atomicAdd(gs + j, acc[j]);
-                        }
-                        if (ATTR) {
-                            const uint32_t m = faces_s[e];
-                            uint32_t v[3];
-#pragma unroll
-                            for (int k = 0; k < 3; ++k) v[k] = sc.faces ? (uint32_t)__ldg(sc.faces + 3 * (size_t)m + k) : 3u * m + k;
-                            if (grad_color) {
-#pragma unroll
-                                for (int k = 0; k < 3; ++k)
-#pragma unroll
-                                    for (int ch = 0; ch < 3; ++ch) atomicAdd(grad_color + 3 * (size_t)v[k] + ch, acc[9 + 3 * k + ch]);
+                            q0x += xg * q6.z, q0y += xg * q6.w, q1x += xg * q7.x, q1y += xg * q7.y;
+                            q2x += xg * q7.z, q2y += xg * q7.w;
+                            if (POSE) {
+                                // B7 + B9 per vertex, with Q = (xn, yn, 1)/w:  Z g_C = (a, b, c),
+                                // a = fx gu, b = fy gv, c = -(xn a + yn b) - w gw;  rho += w (a,b,c);  theta += Q x g_C
+                                const float4 n0 = R[10], n1 = R[11];
+                                {
+                                    const float a = fx * q0x, b = fy * q0y, c = -(n0.x * a + n0.y * b) - q5.x * gw0;
+                                    tau[0] += q5.x * a, tau[1] += q5.x * b, tau[2] += q5.x * c;
+                                    tau[3] += n0.y * c - b, tau[4] += a - n0.x * c, tau[5] += n0.x * b - n0.y * a;
+                                }
+                                {
+                                    const float a = fx * q1x, b = fy * q1y, c = -(n0.z * a + n0.w * b) - q5.y * gw1;
+                                    tau[0] += q5.y * a, tau[1] += q5.y * b, tau[2] += q5.y * c;
+                                    tau[3] += n0.w * c - b, tau[4] += a - n0.z * c, tau[5] += n0.z * b - n0.w * a;
+                                }
+                                {
+                                    const float a = fx * q2x, b = fy * q2y, c = -(n1.x * a + n1.y * b) - q5.z * gw2;
+                                    tau[0] += q5.z * a, tau[1] += q5.z * b, tau[2] += q5.z * c;
+                                    tau[3] += n1.y * c - b, tau[4] += a - n1.x * c, tau[5] += n1.x * b - n1.y * a;
+                                }
+                            } else {
+                                acc[0] = q0x, acc[1] = q0y, acc[2] = gw0, acc[3] = q1x, acc[4] = q1y, acc[5] = gw1;
+                                acc[6] = q2x, acc[7] = q2y, acc[8] = gw2;
                             }
-                            if (grad_opacity) {
-                                const float go = acc[18] * (1.0f / 3.0f);
+                        }
+                    }
+                    if (!POSE) {
+                        // reduce across the warp, then lane j issues the atomic of term j
+                        const bool single = (hm & (hm - 1)) == 0;
+                        const int src = __ffs(hm) - 1;
+                        if (!single) {
+                            if (GEOM) {
 #pragma unroll
-                                for (int k = 0; k < 3; ++k) atomicAdd(grad_opacity + v[k], go);
+                                for (int j = 0; j < 9; ++j) acc[j] = warp_sum(acc[j]);
+                            }
+                            if (ATTR) {
+#pragma unroll
+                                for (int j = 9; j < 19; ++j) acc[j] = warp_sum(acc[j]);
+                            }
+                        }
+                        if (lane == src) {
+                            if (GEOM) {
+                                float* gs = f.gscr + 9 * (size_t)sm.slot[e];
+#pragma unroll
+                                for (int j = 0; j < 9; ++j) atomicAdd(gs + j, acc[j]);
+                            }
+                            if (ATTR) {
+                                const uint32_t m = sm.face[e];
+                                uint32_t v[3];
+#pragma unroll
+                                for (int k = 0; k < 3; ++k) v[k] = sc.faces ? (uint32_t)__ldg(sc.faces + 3 * (size_t)m + k) : 3u * m + k;
+                                if (grad_color) {
+#pragma unroll
+                                    for (int k = 0; k < 3; ++k)
+#pragma unroll
+                                        for (int ch = 0; ch < 3; ++ch) atomicAdd(grad_color + 3 * (size_t)v[k] + ch, acc[9 + 3 * k + ch]);
+                                }
+                                if (grad_opacity) {
+                                    const float go = acc[18] * (1.0f / 3.0f);
+#pragma unroll
+                                    for (int k = 0; k < 3; ++k) atomicAdd(grad_opacity + v[k], go);
+                                }
                             }
                         }
                     }
@@ -260,6 +267,21 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, const uint32_t* __restrict__ vals, 
             }
         }
         hi = lo;
+    }
+    if (POSE) {
+        // per-thread -> per-warp (shuffles) -> per-CTA (shared memory, fixed order) -> per-tile partial
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            const float s = warp_sum(tau[j]);
+            if (lane == 0) sm.red[warp][j] = s;
+        }
+        __syncthreads();
+        if (tid < 6) {
+            float s = 0.f;
+#pragma unroll
+            for (int w = 0; w < 8; ++w) s += sm.red[w][tid];
+            f.pose_partials[6 * (size_t)tile + tid] = s;
+        }
     }
 }
 
@@ -269,7 +291,8 @@ namespace {
 
 constexpr int PB_THREADS = 256;
 
-// a6 + the per-vertex terms of a7.  Persistent grid-stride over visible slots; consumes and re-zeroes gscr.
+// a6 + the per-vertex terms of a7 (full-gradient mode).  Persistent grid-stride over visible slots; consumes and
+// re-zeroes gscr.
 template <bool SOUP>
 __global__ void __launch_bounds__(PB_THREADS)
 proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __restrict__ faces,
@@ -293,7 +316,7 @@ proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __re
         if (!any) continue;
 #pragma unroll
         for (int j = 0; j < 9; ++j) gs[j] = 0.0f;
-        const uint32_t m = f.vis_face[slot];
+        const uint32_t m = __float_as_uint(f.scr[TS_SCR_F4 * (size_t)slot + 3].x);
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
             const size_t v = SOUP ? (size_t)3 * m + k : (size_t)__ldg(faces + 3 * (size_t)m + k);
@@ -353,13 +376,14 @@ __global__ void __launch_bounds__(256) pose_reduce_kernel(const float* __restric
 }
 
 template <int SM>
-void launch_bwd_sm(const ts_frame* fr, const ts_scene& sc, const uint32_t* vals, const float* gC, const float* gD,
-                   const float* gA, float* gcol, float* gopa, bool attr, bool geom, cudaStream_t st) {
+void launch_bwd_sm(const ts_frame* fr, const ts_scene& sc, const float* gC, const float* gD, const float* gA,
+                   float* gcol, float* gopa, bool attr, bool geom, bool pose_only, cudaStream_t st) {
     const TsFrameDev& f = fr->d;
-    const float sg = fr->prm.sigma, am = fr->prm.alpha_min;
-    if (attr && geom) render_bwd_kernel<SM, true, true><<<f.NT, 256, 0, st>>>(f, sc, vals, sg, am, gC, gD, gA, gcol, gopa);
-    else if (geom) render_bwd_kernel<SM, false, true><<<f.NT, 256, 0, st>>>(f, sc, vals, sg, am, gC, gD, gA, gcol, gopa);
-    else render_bwd_kernel<SM, true, false><<<f.NT, 256, 0, st>>>(f, sc, vals, sg, am, gC, gD, gA, gcol, gopa);
+    const float sg = fr->prm.sigma, am = fr->prm.alpha_min, fx = fr->cam.fx, fy = fr->cam.fy;
+    if (pose_only) render_bwd_kernel<SM, false, false, true><<<f.NT, 256, 0, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa);
+    else if (attr && geom) render_bwd_kernel<SM, true, true, false><<<f.NT, 256, 0, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa);
+    else if (geom) render_bwd_kernel<SM, false, true, false><<<f.NT, 256, 0, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa);
+    else render_bwd_kernel<SM, true, false, false><<<f.NT, 256, 0, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa);
 }
 
 }  // namespace
@@ -369,19 +393,21 @@ int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
                              cudaStream_t st) {
     const bool attr = (mask & (TS_GRAD_COLOR | TS_GRAD_OPACITY)) != 0;
     const bool geom = (mask & (TS_GRAD_POS | TS_GRAD_POSE)) != 0;
+    const bool pose_only = (mask == TS_GRAD_POSE);
     if (!attr && !geom) return TS_OK;
     float* gcol = (mask & TS_GRAD_COLOR) ? grad_color : nullptr;
     float* gopa = (mask & TS_GRAD_OPACITY) ? grad_opacity : nullptr;
-    const uint32_t* vals = fr->d.vals[fr->sorted_buf];
     switch (ts_sigma_mode(fr->prm.sigma)) {
-        case 1: launch_bwd_sm<1>(fr, *sc, vals, gC, gD, gA, gcol, gopa, attr, geom, st); break;
-        case 2: launch_bwd_sm<2>(fr, *sc, vals, gC, gD, gA, gcol, gopa, attr, geom, st); break;
-        case 3: launch_bwd_sm<3>(fr, *sc, vals, gC, gD, gA, gcol, gopa, attr, geom, st); break;
-        default: launch_bwd_sm<0>(fr, *sc, vals, gC, gD, gA, gcol, gopa, attr, geom, st); break;
+        case 1: launch_bwd_sm<1>(fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
+        case 2: launch_bwd_sm<2>(fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
+        case 3: launch_bwd_sm<3>(fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
+        default: launch_bwd_sm<0>(fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
     }
     fr->pose_src = 0;
-    if (geom) {
-        const int grid = (int)fr->d.n_partials_cap;
+    if (pose_only) {
+        fr->pose_src = 1, fr->n_pose_partials = (uint32_t)fr->d.NT;
+    } else if (geom) {
+        const int grid = (int)min((uint32_t)(ctx->num_sms * 4), fr->d.n_partials_cap);
         const int want_pose = (mask & TS_GRAD_POSE) ? 1 : 0;
         float* gp = (mask & TS_GRAD_POS) ? grad_pos : nullptr;
         if (sc->faces == nullptr)
@@ -390,7 +416,6 @@ int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
             proj_bwd_kernel<false><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, sc->faces, fr->T_cw, fr->cam, gp, want_pose);
         if (want_pose) fr->pose_src = 2, fr->n_pose_partials = (uint32_t)grid;
     }
-    (void)ctx;
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

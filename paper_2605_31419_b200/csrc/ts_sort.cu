@@ -1,146 +1,149 @@
-// ts_sort.cu -- a2: stable LSD radix sort of the (tile<<32 | depth) keys ("faces are sorted in depth order",
-// PAPER.md:103) as a hand-written onesweep: one upfront histogram of every digit, then ONE kernel per 8-bit
-// digit that ranks, resolves its global offsets by decoupled look-back and scatters -- each key is read and
-// written once per digit.  Launch geometry never depends on the (device-side) pair count: persistent CTAs pull
-// tile indices from a ticket counter, which also guarantees look-back progress.  Integer only; bit-exact.
-#include "ts_internal.cuh"
+// ts_sort.cu -- a2: bin + sort ("faces are sorted in depth order") as an MSD-first radix sort of
+// the (tile, depth) key, shaped for P ~ 1e5..1e6 pairs where a global LSD sort is pure launch latency:
+//   bin_setup_kernel : the most-significant digit IS the tile id, and its histogram and exclusive scan already
+//       exist (tile_count -> tile_ranges / tile_cursor, made by the project kernel), so the MSD pass is one
+//       scatter: every visible face writes (depth_key << 32 | face, slot) into the segment of each tile it
+//       touches (cursor atomics; faces that touch many tiles are spread over the warp).  The same pass builds
+//       the face's 160 B render record once (F7), instead of once per (tile, face) pair inside the renderers.
+//   tile_sort_kernel : one CTA per tile sorts its segment by the remaining 60 key bits (depth, then face index:
+//       the result is exactly the stable sort of (tile << 32 | depth) with faces emitted in index order, F6) in
+//       shared memory -- rank sort for short lists, bitonic network above -- and writes the sorted (slot, face)
+//       list the renderers walk plus the sorted 64-bit keys.  Segments longer than TS_SORT_SMEM run the same
+//       network in global memory (slow, correct, rare).
+// Integer only; bit-exact against the oracle's std::stable_sort.
+#include "ts_raster.cuh"
 
 namespace {
 
-constexpr uint32_t SS_AGG = 1u << 30, SS_PREFIX = 2u << 30, SS_FLAGS = 3u << 30, SS_VAL = (1u << 30) - 1u;
-
-// zero what this sort will use: digit histograms, look-back states of the tiles in play, tickets, tile ranges
-__global__ void sort_prep_kernel(TsFrameDev f) {
-    const uint32_t n = ts_eff_pairs(f);
-    const uint32_t n_tiles = (n + TS_SORT_TILE - 1) / TS_SORT_TILE;
-    const size_t stride = (size_t)gridDim.x * blockDim.x, gid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (size_t i = gid; i < (size_t)TS_MAX_PASSES * TS_RADIX; i += stride) f.hist[i] = 0;
-    for (int p = 0; p < f.n_passes; ++p) {
-        uint32_t* st = f.sort_state + (size_t)p * f.n_sort_tiles_cap * TS_RADIX;
-        for (size_t i = gid; i < (size_t)n_tiles * TS_RADIX; i += stride) st[i] = 0;
-    }
-    for (size_t i = gid; i < (size_t)f.NT; i += stride) f.tile_ranges[i] = make_uint2(0u, 0u);
-    if (gid < TS_MAX_PASSES) f.ctrl->sort_ticket[gid] = 0;
-}
-
-// all digit histograms in one read of the keys
-__global__ void __launch_bounds__(256) sort_hist_kernel(TsFrameDev f) {
-    __shared__ uint32_t sh[TS_MAX_PASSES * TS_RADIX];
-    const uint32_t n = ts_eff_pairs(f);
-    for (int i = threadIdx.x; i < f.n_passes * TS_RADIX; i += blockDim.x) sh[i] = 0;
-    __syncthreads();
-    const unsigned long long* keys = f.keys[0];
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const unsigned long long k = keys[i];
-        for (int p = 0; p < f.n_passes; ++p) atomicAdd(&sh[p * TS_RADIX + (uint32_t)((k >> (8 * p)) & 0xffu)], 1u);
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < f.n_passes * TS_RADIX; i += blockDim.x)
-        if (sh[i]) atomicAdd(&f.hist[i], sh[i]);
-}
-
-// one digit: rank (warp match), look back, scatter.  Stable: keys keep their input order within a digit.
-__global__ void __launch_bounds__(TS_SORT_THREADS)
-onesweep_pass_kernel(TsFrameDev f, int pass, const unsigned long long* __restrict__ kin,
-                     const uint32_t* __restrict__ vin, unsigned long long* __restrict__ kout,
-                     uint32_t* __restrict__ vout) {
-    __shared__ uint32_t wh[TS_SORT_THREADS / 32][TS_RADIX];   // per-warp digit counts -> exclusive warp prefixes
-    __shared__ uint32_t base[TS_RADIX];                        // global position of this tile's first key per digit
-    __shared__ uint32_t gofs[TS_RADIX];                        // exclusive scan of the global digit histogram
-    __shared__ uint32_t s_tile;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t n = ts_eff_pairs(f);
-    const uint32_t n_tiles = (n + TS_SORT_TILE - 1) / TS_SORT_TILE;
-    const int shift = 8 * pass;
-    uint32_t* state = f.sort_state + (size_t)pass * f.n_sort_tiles_cap * TS_RADIX;
-    // exclusive scan of hist[pass] (256 entries, redone by every CTA: cheaper than a launch)
-    {
-        const uint32_t h = f.hist[pass * TS_RADIX + tid];
-        uint32_t incl = h;
+__global__ void __launch_bounds__(TS_BIN_THREADS)
+bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t nvis = min(ts_eff_visible(f), f.vis_cap);
+    const uint32_t n_round = (nvis + TS_BIN_THREADS - 1) / TS_BIN_THREADS * TS_BIN_THREADS;
+    for (uint32_t slot = blockIdx.x * TS_BIN_THREADS + threadIdx.x; slot < n_round; slot += gridDim.x * TS_BIN_THREADS) {
+        const bool live = slot < nvis;
+        int tx0 = 0, ty0 = 0, ntx = 0, nty = 0;
+        unsigned long long key = 0;
+        if (live) {
+            const float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
+            const float4 s0 = s4[0], s1 = s4[1], s2 = s4[2], s3 = s4[3];
+            float4 rec[TS_REC_F4];
+            ts_build_record(s0, s1, s2, cam, rec);
+            float4* out = f.rec + TS_REC_F4 * (size_t)slot;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += t;
+            for (int i = 0; i < TS_REC_F4; ++i) out[i] = rec[i];
+            const int rlo = __float_as_int(s2.z), rhi = __float_as_int(s2.w);
+            const int x0 = (int)(short)(rlo & 0xffff), y0 = rlo >> 16, x1 = (int)(short)(rhi & 0xffff), y1 = rhi >> 16;
+            tx0 = x0 >> 4, ty0 = y0 >> 4, ntx = (x1 >> 4) - tx0 + 1, nty = (y1 >> 4) - ty0 + 1;
+            key = ((unsigned long long)__float_as_uint(s3.y) << 32) | __float_as_uint(s3.x);
         }
-        if (lane == 31) base[warp] = incl;
-        __syncthreads();
-        uint32_t woff = 0;
-        for (int w = 0; w < warp; ++w) woff += base[w];
-        __syncthreads();
-        gofs[tid] = woff + incl - h;
-    }
-    for (;;) {
-        __syncthreads();
-        if (tid == 0) s_tile = atomicAdd(&f.ctrl->sort_ticket[pass], 1u);
-        for (int i = tid; i < (TS_SORT_THREADS / 32) * TS_RADIX; i += TS_SORT_THREADS) (&wh[0][0])[i] = 0;
-        __syncthreads();
-        const uint32_t tile = s_tile;
-        if (tile >= n_tiles) break;
-        const uint32_t wbase = tile * TS_SORT_TILE + warp * (TS_SORT_ITEMS * 32);
-        unsigned long long key[TS_SORT_ITEMS];
-        uint32_t val[TS_SORT_ITEMS], ofs[TS_SORT_ITEMS], dig[TS_SORT_ITEMS];
-#pragma unroll
-        for (int i = 0; i < TS_SORT_ITEMS; ++i) {
-            const uint32_t idx = wbase + i * 32 + lane;
-            const bool ok = idx < n;
-            key[i] = ok ? kin[idx] : 0ull;
-            val[i] = ok ? vin[idx] : 0u;
-            dig[i] = ok ? (uint32_t)((key[i] >> shift) & 0xffu) : (0x100u | lane);   // invalid lanes match nobody
-        }
-#pragma unroll
-        for (int i = 0; i < TS_SORT_ITEMS; ++i) {
-            const uint32_t peers = __match_any_sync(0xffffffffu, dig[i]);
-            const int leader = __ffs(peers) - 1;
-            uint32_t old = 0;
-            if (lane == leader && dig[i] < 0x100u) {
-                old = wh[warp][dig[i]];
-                wh[warp][dig[i]] = old + __popc(peers);
+        const int nt = ntx * nty;
+        // narrow faces (the common case): the owning lane scatters its <= 4 pairs itself
+        if (nt <= 4) {
+            for (int i = 0; i < nt; ++i) {
+                const int ty = ty0 + i / ntx, tx = tx0 + i % ntx;
+                const uint32_t pos = atomicAdd(f.tile_cursor + ty * f.tiles_x + tx, 1u);
+                if (pos < f.pair_cap) f.pkey[pos] = key, f.pslot[pos] = slot;
             }
-            old = __shfl_sync(0xffffffffu, old, leader);
-            ofs[i] = old + __popc(peers & ((1u << lane) - 1u));
-            __syncwarp();
         }
-        __syncthreads();
-        // per digit: warp counts -> exclusive warp prefixes, tile count
-        uint32_t cnt = 0;
-#pragma unroll
-        for (int w = 0; w < TS_SORT_THREADS / 32; ++w) {
-            const uint32_t t = wh[w][tid];
-            wh[w][tid] = cnt;
-            cnt += t;
-        }
-        // decoupled look-back for digit `tid`
-        volatile uint32_t* st = state;
-        st[(size_t)tile * TS_RADIX + tid] = (tile == 0 ? SS_PREFIX : SS_AGG) | cnt;
-        uint32_t excl = 0;
-        for (int64_t t = (int64_t)tile - 1; t >= 0; --t) {
-            uint32_t s;
-            do { s = st[(size_t)t * TS_RADIX + tid]; } while ((s & SS_FLAGS) == 0);
-            excl += s & SS_VAL;
-            if ((s & SS_FLAGS) == SS_PREFIX) break;
-        }
-        if (tile != 0) st[(size_t)tile * TS_RADIX + tid] = SS_PREFIX | (excl + cnt);
-        base[tid] = gofs[tid] + excl;
-        __syncthreads();
-#pragma unroll
-        for (int i = 0; i < TS_SORT_ITEMS; ++i) {
-            if (dig[i] < 0x100u) {
-                const uint32_t dst = base[dig[i]] + wh[warp][dig[i]] + ofs[i];
-                kout[dst] = key[i];
-                vout[dst] = val[i];
+        // wide faces: the whole warp scatters one face's tiles together
+        uint32_t wide = __ballot_sync(0xffffffffu, nt > 4);
+        while (wide) {
+            const int src = __ffs(wide) - 1;
+            wide &= wide - 1;
+            const int btx0 = __shfl_sync(0xffffffffu, tx0, src), bty0 = __shfl_sync(0xffffffffu, ty0, src);
+            const int bntx = __shfl_sync(0xffffffffu, ntx, src), bnt = __shfl_sync(0xffffffffu, nt, src);
+            const unsigned long long bkey = __shfl_sync(0xffffffffu, key, src);
+            const uint32_t bslot = __shfl_sync(0xffffffffu, slot, src);
+            for (int i = lane; i < bnt; i += 32) {
+                const int ty = bty0 + i / bntx, tx = btx0 + i % bntx;
+                const uint32_t pos = atomicAdd(f.tile_cursor + ty * f.tiles_x + tx, 1u);
+                if (pos < f.pair_cap) f.pkey[pos] = bkey, f.pslot[pos] = bslot;
             }
         }
     }
 }
 
-// tile_ranges from the sorted keys
-__global__ void tile_ranges_kernel(TsFrameDev f, const unsigned long long* __restrict__ keys) {
-    const uint32_t n = ts_eff_pairs(f);
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const uint32_t t = (uint32_t)(keys[i] >> 32);
-        if (t >= (uint32_t)f.NT) continue;
-        if (i == 0 || (uint32_t)(keys[i - 1] >> 32) != t) f.tile_ranges[t].x = (uint32_t)i;
-        if (i + 1 == n || (uint32_t)(keys[i + 1] >> 32) != t) f.tile_ranges[t].y = (uint32_t)(i + 1);
+// ascending compare-exchange network for arbitrary n (indices >= n behave as +inf and never move): bitonic sort in
+// the "mirror first step" form, in which every exchange puts the smaller key at the lower index.
+template <typename KP, typename VP>
+__device__ __forceinline__ void cta_sort_network(KP k, VP v, uint32_t n) {
+    uint32_t N = 1;
+    while (N < n) N <<= 1;
+    const uint32_t half = N >> 1;
+    for (uint32_t size = 2; size <= N; size <<= 1) {
+        const uint32_t hs = size >> 1;
+        for (uint32_t t = threadIdx.x; t < half; t += blockDim.x) {
+            const uint32_t blk = t / hs, off = t - blk * hs;
+            const uint32_t lo = blk * size + off, hi = blk * size + size - 1 - off;
+            if (hi < n) {
+                const unsigned long long a = k[lo], b = k[hi];
+                if (b < a) {
+                    k[lo] = b, k[hi] = a;
+                    const uint32_t va = v[lo];
+                    v[lo] = v[hi], v[hi] = va;
+                }
+            }
+        }
+        __syncthreads();
+        for (uint32_t stride = hs >> 1; stride > 0; stride >>= 1) {
+            for (uint32_t t = threadIdx.x; t < half; t += blockDim.x) {
+                const uint32_t lo = 2 * stride * (t / stride) + (t % stride), hi = lo + stride;
+                if (hi < n) {
+                    const unsigned long long a = k[lo], b = k[hi];
+                    if (b < a) {
+                        k[lo] = b, k[hi] = a;
+                        const uint32_t va = v[lo];
+                        v[lo] = v[hi], v[hi] = va;
+                    }
+                }
+            }
+            __syncthreads();
+        }
+    }
+}
+
+__global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f) {
+    __shared__ unsigned long long sk[TS_SORT_SMEM];
+    __shared__ uint32_t sv[TS_SORT_SMEM];
+    const uint32_t tile = blockIdx.x;
+    const uint2 range = f.tile_ranges[tile];
+    const uint32_t n = range.y - range.x;
+    if (n == 0) return;
+    const unsigned long long thi = (unsigned long long)tile << 32;
+    unsigned long long* gk = f.pkey + range.x;
+    uint32_t* gv = f.pslot + range.x;
+    if (n <= TS_SORT_THREADS) {
+        // rank sort: keys are unique (the face index is part of the key), so ranks are a permutation
+        unsigned long long mine = 0;
+        uint32_t mv = 0;
+        if (threadIdx.x < n) mine = gk[threadIdx.x], mv = gv[threadIdx.x], sk[threadIdx.x] = mine;
+        __syncthreads();
+        if (threadIdx.x < n) {
+            uint32_t rank = 0;
+            for (uint32_t j = 0; j < n; ++j) rank += (sk[j] < mine) ? 1u : 0u;
+            f.sorted[range.x + rank] = make_uint2(mv, (uint32_t)mine);
+            f.skey[range.x + rank] = thi | (mine >> 32);
+        }
+        return;
+    }
+    if (n <= TS_SORT_SMEM) {
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) sk[i] = gk[i], sv[i] = gv[i];
+        __syncthreads();
+        cta_sort_network(sk, sv, n);
+        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+            const unsigned long long kk = sk[i];
+            f.sorted[range.x + i] = make_uint2(sv[i], (uint32_t)kk);
+            f.skey[range.x + i] = thi | (kk >> 32);
+        }
+        return;
+    }
+    // oversize segment: same network, in place in global memory (volatile: exchanged across threads between barriers)
+    cta_sort_network((volatile unsigned long long*)gk, (volatile uint32_t*)gv, n);
+    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+        const unsigned long long kk = gk[i];
+        f.sorted[range.x + i] = make_uint2(gv[i], (uint32_t)kk);
+        f.skey[range.x + i] = thi | (kk >> 32);
     }
 }
 
@@ -148,18 +151,10 @@ __global__ void tile_ranges_kernel(TsFrameDev f, const unsigned long long* __res
 
 int32_t ts_launch_sort(const ts_ctx* ctx, ts_frame* fr, cudaStream_t stream) {
     const TsFrameDev& f = fr->d;
-    const int grid_small = ctx->num_sms * 2;
-    sort_prep_kernel<<<grid_small, 256, 0, stream>>>(f);
-    sort_hist_kernel<<<grid_small, 256, 0, stream>>>(f);
-    const uint32_t grid_pass = (uint32_t)min((uint64_t)f.n_sort_tiles_cap, (uint64_t)ctx->num_sms * 4u);
-    int cur = 0;
-    for (int p = 0; p < f.n_passes; ++p) {
-        onesweep_pass_kernel<<<grid_pass, TS_SORT_THREADS, 0, stream>>>(f, p, f.keys[cur], f.vals[cur], f.keys[cur ^ 1],
-                                                                        f.vals[cur ^ 1]);
-        cur ^= 1;
-    }
-    fr->sorted_buf = cur;
-    tile_ranges_kernel<<<grid_small, 256, 0, stream>>>(f, f.keys[cur]);
+    const uint32_t grid_bin = (uint32_t)min((uint64_t)(f.vis_cap + TS_BIN_THREADS - 1) / TS_BIN_THREADS,
+                                            (uint64_t)ctx->num_sms * 16u);
+    bin_setup_kernel<<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam);
+    tile_sort_kernel<<<f.NT, TS_SORT_THREADS, 0, stream>>>(f);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

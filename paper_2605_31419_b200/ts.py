@@ -19,12 +19,9 @@ GRAD_POS, GRAD_COLOR, GRAD_OPACITY, GRAD_POSE = 1, 2, 4, 8
 GRAD_ALL = 15
 FLAG_OVERFLOW_PAIRS, FLAG_OVERFLOW_VISIBLE = 1, 2
 PARAM_COUNTERS = 0x100   # ts_params.flags: count visits / rect tests / hits (debug instantiation)
-(VIEW_VIS_FACE, VIEW_RECT, VIEW_DEPTH_KEY, VIEW_TILES_TOUCHED, VIEW_SCR, VIEW_KEYS, VIEW_VALS, VIEW_TILE_RANGES,
- VIEW_N_CONTRIB, VIEW_COUNTERS) = range(10)
-_VIEW_DTYPES = {VIEW_VIS_FACE: torch.int32, VIEW_RECT: torch.int16, VIEW_DEPTH_KEY: torch.int32,
-                VIEW_TILES_TOUCHED: torch.int32, VIEW_SCR: torch.float32, VIEW_KEYS: torch.int64,
-                VIEW_VALS: torch.int32, VIEW_TILE_RANGES: torch.int32, VIEW_N_CONTRIB: torch.int32,
-                VIEW_COUNTERS: torch.int64}
+VIEW_VIS, VIEW_KEYS, VIEW_VALS, VIEW_TILE_RANGES, VIEW_N_CONTRIB, VIEW_COUNTERS = range(6)
+_VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.int32,
+                VIEW_TILE_RANGES: torch.int32, VIEW_N_CONTRIB: torch.int32, VIEW_COUNTERS: torch.int64}
 
 EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_bwd",

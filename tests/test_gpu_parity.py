@@ -47,15 +47,18 @@ def check_project_and_sort(o, g, M):
     flags, nvis, npairs = g.status()
     pr, b = o.project(), o.bin_sort()
     assert flags == 0 and nvis == pr.n_visible and npairs == b.P
-    vf = g.view(ts.VIEW_VIS_FACE).astype(np.int64)
-    assert np.array_equal(vf, np.nonzero(pr.visible)[0])                       # same cull set, ascending slots
-    assert np.array_equal(scatter_per_face(M, vf, g.view(ts.VIEW_RECT).reshape(-1, 4)), pr.rect)
-    assert np.array_equal(scatter_per_face(M, vf, g.view(ts.VIEW_DEPTH_KEY).view(np.uint32)), pr.depth_key)
-    assert np.array_equal(scatter_per_face(M, vf, g.view(ts.VIEW_TILES_TOUCHED).view(np.uint32)), pr.tiles_touched)
-    scr = g.view(ts.VIEW_SCR).reshape(-1, 12)
-    assert np.array_equal(scr[:, :9].view(np.uint32), pr.scr[vf].view(np.uint32))   # (u,v,w) bit for bit
+    vis = g.view(ts.VIEW_VIS).reshape(-1, 16)                                  # one 64 B record per slot
+    vf = vis[:, 12].view(np.uint32).astype(np.int64)                           # slot -> face (allocation order)
+    assert np.array_equal(np.sort(vf), np.nonzero(pr.visible)[0])              # same cull set
+    rect = np.ascontiguousarray(vis[:, 10:12]).view(np.int16).reshape(-1, 4)   # x0,y0,x1,y1
+    assert np.array_equal(scatter_per_face(M, vf, rect), pr.rect)
+    assert np.array_equal(scatter_per_face(M, vf, vis[:, 13].view(np.uint32)), pr.depth_key)
+    assert np.array_equal(scatter_per_face(M, vf, vis[:, 14].view(np.uint32)), pr.tiles_touched)
+    assert np.array_equal(vis[:, :9].view(np.uint32), pr.scr[vf].view(np.uint32))   # (u,v,w) bit for bit
     assert np.array_equal(g.view(ts.VIEW_KEYS).view(np.uint64), b.keys)
-    assert np.array_equal(vf[g.view(ts.VIEW_VALS).astype(np.int64)], b.vals.astype(np.int64))
+    sv = g.view(ts.VIEW_VALS).reshape(-1, 2).astype(np.int64)                  # sorted (slot, face)
+    assert np.array_equal(sv[:, 1], b.vals.astype(np.int64))
+    assert np.array_equal(vf[sv[:, 0]], sv[:, 1])
     assert np.array_equal(g.view(ts.VIEW_TILE_RANGES).reshape(-1, 2).view(np.uint32), b.ranges)
 
 
