@@ -9,7 +9,9 @@
  *    workspace and repeats.
  *  - Ownership: every DEVICE buffer is owned by the caller (e.g. torch tensors' data_ptr()), including the
  *    frame workspace.  The library allocates no device memory after ts_create, never frees caller memory and
- *    keeps no caller pointer beyond the call, except inside the caller-provided workspace of a ts_frame.
+ *    keeps no caller pointer beyond the call, with one exception: a ts_frame remembers the scene and pose pointers
+ *    given to ts_project until the next ts_project on it (ts_bin_sort reads scene->opacity, ts_render_bwd reads the
+ *    pose), so they must stay valid and unchanged until the frame's backward pass has been enqueued.
  *  - Streams: `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is enqueued
  *    on it.  No export synchronises except ts_frame_status and ts_frame_view.  All exports may be captured
  *    into a CUDA graph (launch geometry never depends on device-side counts).
@@ -123,7 +125,7 @@ enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slo
                                     f32 (u,v,w)x3, f32 mean opacity, i16 x0,y0,x1,y1, u32 face, u32 depth_key,
                                     u32 tiles_touched, u32 0                                                  */
        TS_VIEW_KEYS = 1,         /* u64[n_pairs] sorted keys (tile << 32 | depth_key)                        */
-       TS_VIEW_VALS = 2,         /* u32[n_pairs][2] sorted (slot, face) pairs                                */
+       TS_VIEW_VALS = 2,         /* u32[n_pairs][4] sorted (slot, face, rect_lo, rect_hi) entries            */
        TS_VIEW_TILE_RANGES = 3,  /* u32[NT][2]                                                               */
        TS_VIEW_N_CONTRIB = 4,    /* u32[H][W]                                                                */
        TS_VIEW_COUNTERS = 5 };   /* u64[8]: n_visit(warp-level), n_rect, n_hit, ... (TS_PARAM_COUNTERS only)  */

@@ -10,7 +10,8 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t ctrl, tile_count, tile_cursor, tile_ranges, scr, rec, gscr, pkey, pslot, skey, sorted, n_contrib, t_last,
+    size_t ctrl, tile_count, tile_cursor, tile_offset, tile_order, tile_ranges, scr, rec, gscr, pair_a, pair_b, big_key, big_idx, skey, sorted,
+        n_contrib, t_last,
         pose_partials, total;
     int32_t tiles_x, tiles_y, NT;
     uint32_t n_partials_cap;
@@ -21,20 +22,24 @@ bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pa
         vis_cap == 0 || vis_cap >= (1ull << 28) || (uint64_t)M >= (1ull << 28))
         return false;
     L.tiles_x = (W + TS_TILE - 1) / TS_TILE, L.tiles_y = (H + TS_TILE - 1) / TS_TILE, L.NT = L.tiles_x * L.tiles_y;
-    L.n_partials_cap = (uint32_t)L.NT > (uint32_t)ctx->num_sms * 4u ? (uint32_t)L.NT : (uint32_t)ctx->num_sms * 4u;
+    L.n_partials_cap = (uint32_t)L.NT * 8u > (uint32_t)ctx->num_sms * 4u ? (uint32_t)L.NT * 8u : (uint32_t)ctx->num_sms * 4u;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t r = o; o = align_up(o + bytes); return r; };
     L.ctrl = take(sizeof(TsCtrl));
     L.tile_count = take(4ull * L.NT);
     L.tile_cursor = take(4ull * L.NT);
+    L.tile_offset = take(4ull * L.NT);
+    L.tile_order = take(4ull * L.NT);
     L.tile_ranges = take(8ull * L.NT);
     L.scr = take(16ull * TS_SCR_F4 * vis_cap);
     L.rec = take(16ull * TS_REC_F4 * vis_cap);
     L.gscr = take(36ull * vis_cap);
-    L.pkey = take(8ull * pair_cap);
-    L.pslot = take(4ull * pair_cap);
+    L.pair_a = take(16ull * pair_cap);
+    L.pair_b = take(4ull * pair_cap);
+    L.big_key = take(8ull * pair_cap);
+    L.big_idx = take(4ull * pair_cap);
     L.skey = take(8ull * pair_cap);
-    L.sorted = take(8ull * pair_cap);
+    L.sorted = take(16ull * pair_cap);
     L.n_contrib = take(4ull * W * H);
     L.t_last = take(4ull * W * H);
     L.pose_partials = take(24ull * L.n_partials_cap);
@@ -101,14 +106,18 @@ int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_
     d.ctrl = reinterpret_cast<TsCtrl*>(b + L.ctrl);
     d.tile_count = reinterpret_cast<uint32_t*>(b + L.tile_count);
     d.tile_cursor = reinterpret_cast<uint32_t*>(b + L.tile_cursor);
+    d.tile_offset = reinterpret_cast<uint32_t*>(b + L.tile_offset);
+    d.tile_order = reinterpret_cast<uint32_t*>(b + L.tile_order);
     d.tile_ranges = reinterpret_cast<uint2*>(b + L.tile_ranges);
     d.scr = reinterpret_cast<float4*>(b + L.scr);
     d.rec = reinterpret_cast<float4*>(b + L.rec);
     d.gscr = reinterpret_cast<float*>(b + L.gscr);
-    d.pkey = reinterpret_cast<unsigned long long*>(b + L.pkey);
-    d.pslot = reinterpret_cast<uint32_t*>(b + L.pslot);
+    d.pair_a = reinterpret_cast<uint4*>(b + L.pair_a);
+    d.pair_b = reinterpret_cast<uint32_t*>(b + L.pair_b);
+    d.big_key = reinterpret_cast<unsigned long long*>(b + L.big_key);
+    d.big_idx = reinterpret_cast<uint32_t*>(b + L.big_idx);
     d.skey = reinterpret_cast<unsigned long long*>(b + L.skey);
-    d.sorted = reinterpret_cast<uint2*>(b + L.sorted);
+    d.sorted = reinterpret_cast<uint4*>(b + L.sorted);
     d.n_contrib = reinterpret_cast<uint32_t*>(b + L.n_contrib);
     d.t_last = reinterpret_cast<float*>(b + L.t_last);
     d.pose_partials = reinterpret_cast<float*>(b + L.pose_partials);
@@ -153,18 +162,28 @@ int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const 
     fr->cam = TsCamDev{cam->width, cam->height, cam->fx, cam->fy, cam->cx, cam->cy, cam->znear};
     fr->prm = TsPrmDev{prm->sigma, prm->alpha_min, prm->t_min, prm->eps_area, prm->flags};
     fr->T_cw = T_cw_dev;
+    fr->scene = *sc;
     fr->have_sort = fr->have_fwd = 0;
     fr->pose_src = 0;
+    if (fr->counters_dirty) {
+        // the previous ts_project was never followed by ts_bin_sort: its slot / tile counters are still live
+        char* b = static_cast<char*>(fr->base);
+        if (cudaMemsetAsync(b, 0, reinterpret_cast<char*>(fr->d.tile_offset) - b, (cudaStream_t)stream) != cudaSuccess)
+            return TS_ERR_CUDA;
+    }
     const int32_t s = ts_launch_project(ctx, fr, sc, (cudaStream_t)stream);
     fr->have_project = (s == TS_OK);
+    fr->counters_dirty = 1;
     return s;
 }
 
 int32_t ts_bin_sort(ts_ctx* ctx, ts_frame* fr, void* stream) {
     if (!ctx || !fr) return TS_ERR_INVALID_ARG;
     if (!fr->have_project) return TS_ERR_STATE;
+    if (!fr->counters_dirty) return TS_ERR_STATE;          // one ts_bin_sort per ts_project
     const int32_t s = ts_launch_sort(ctx, fr, (cudaStream_t)stream);
     fr->have_sort = (s == TS_OK);
+    fr->counters_dirty = 0;
     return s;
 }
 
@@ -208,7 +227,7 @@ int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev
     switch (which) {
         case TS_VIEW_VIS: *dev_ptr = d.scr, *count = 16 * nv; break;
         case TS_VIEW_KEYS: *dev_ptr = d.skey, *count = np; break;
-        case TS_VIEW_VALS: *dev_ptr = d.sorted, *count = 2 * np; break;
+        case TS_VIEW_VALS: *dev_ptr = d.sorted, *count = 4 * np; break;
         case TS_VIEW_TILE_RANGES: *dev_ptr = d.tile_ranges, *count = 2 * (size_t)d.NT; break;
         case TS_VIEW_N_CONTRIB: *dev_ptr = d.n_contrib, *count = (size_t)d.W * d.H; break;
         case TS_VIEW_COUNTERS: *dev_ptr = &d.ctrl->counters[0], *count = 8; break;

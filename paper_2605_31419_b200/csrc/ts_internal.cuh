@@ -8,8 +8,9 @@
 
 #define TS_TILE 16
 #define TS_PROJ_THREADS 256          // faces per project CTA
-#define TS_BIN_THREADS 128           // visible slots per bin/setup CTA iteration
-#define TS_SORT_THREADS 256
+#define TS_BIN_THREADS 256           // visible slots per bin/setup CTA iteration
+#define TS_SCAN_LOCAL_MAX 4096       // up to this many tiles every binning CTA scans the tile counts itself (smem)
+#define TS_SORT_THREADS 128
 #define TS_SORT_SMEM 2048            // tile lists up to this length are sorted in shared memory
 #define TS_BATCH 128                 // list entries staged per batch in the forward kernel
 #define TS_BATCH_BWD 64              // ... in the backward kernel (records are twice as large)
@@ -24,9 +25,10 @@ struct TsCtrl {
     uint32_t n_pairs;        // (tile, face) pairs (may exceed pair_cap on overflow)
     uint32_t flags;          // TS_FLAG_*
     uint32_t max_list;       // longest tile list of the last ts_project
-    uint32_t vis_counter;    // slot allocator of the project kernel (zero at rest)
-    uint32_t proj_done;      // project CTAs finished (zero at rest)
-    uint32_t pad[2];
+    uint32_t vis_counter;    // slot allocator of the project kernel (zeroed by the sort kernel)
+    uint32_t job_ticket[2];  // work queues of the forward / backward render kernels (zero at rest)
+    uint32_t job_done[2];    // warps finished, per render kernel (zero at rest)
+    uint32_t pad[3];
     unsigned long long counters[8];   // debug counters (TS_PARAM_COUNTERS)
 };
 
@@ -35,16 +37,20 @@ struct TsFrameDev {
     int32_t M, W, H, tiles_x, tiles_y, NT;
     uint32_t pair_cap, vis_cap;
     TsCtrl* ctrl;
-    uint32_t* tile_count;             // [NT] pairs per tile, counted by the project kernel (zero at rest)
-    uint32_t* tile_cursor;            // [NT] write cursor of the binning pass (absolute positions)
+    uint32_t* tile_count;             // [NT] pairs per tile, counted by the project kernel (zeroed by the sort kernel)
+    uint32_t* tile_cursor;            // [NT] write cursor of the binning pass, relative to the tile's begin (zero at rest)
+    uint32_t* tile_offset;            // [NT] exclusive scan of tile_count (only used when NT > TS_SCAN_LOCAL_MAX)
+    uint32_t* tile_order;             // [NT] tiles by descending list length (render work queues)
     uint2* tile_ranges;               // [NT] (begin, end) into the pair arrays
     float4* scr;                      // [vis_cap][4]: (u0,v0,w0,u1) (v1,w1,u2,v2) (w2,obar,rect_lo,rect_hi) (face,key,tiles,0)
     float4* rec;                      // [vis_cap][10]: per-face render record, see ts_raster.cuh
     float* gscr;                      // [vis_cap][9]: dL/d(u,v,w) per face vertex (full-gradient mode), zero at rest
-    unsigned long long* pkey;         // [pair_cap] binned, unsorted: depth_key << 32 | face
-    uint32_t* pslot;                  // [pair_cap] binned, unsorted: slot
+    uint4* pair_a;                    // [pair_cap] binned, unsorted: (depth_key, face, slot, rect_lo)
+    uint32_t* pair_b;                 // [pair_cap] binned, unsorted: rect_hi
+    unsigned long long* big_key;      // [pair_cap] scratch of the oversize-segment sort
+    uint32_t* big_idx;                // [pair_cap] scratch of the oversize-segment sort
     unsigned long long* skey;         // [pair_cap] sorted: tile << 32 | depth_key
-    uint2* sorted;                    // [pair_cap] sorted: (slot, face)
+    uint4* sorted;                    // [pair_cap] sorted: (slot, face, rect_lo, rect_hi)
     uint32_t* n_contrib;              // [H*W]
     float* t_last;                    // [H*W] transmittance in front of the last contributing face
     float* pose_partials;             // [n_partials_cap][6]
@@ -65,7 +71,9 @@ struct ts_frame {
     TsCamDev cam;
     TsPrmDev prm;
     const float* T_cw;       // device pointer given to the last ts_project (read again by the projection backward)
+    ts_scene scene;          // scene given to the last ts_project (opacity is read by the binning kernel)
     int have_project, have_sort, have_fwd;
+    int counters_dirty;      // ts_project ran but ts_bin_sort has not consumed (and re-zeroed) its counters yet
     uint32_t pose_src;       // 0 = none, 1 = per-tile partials (pose-only), 2 = per-block partials (projection backward)
     uint32_t n_pose_partials;
     size_t bytes;

@@ -1,10 +1,8 @@
 // ts_project.cu -- a1: project + cull + bounds (Eq. 1) in ONE streaming pass over the map:
-// 36 B read per face (soup), float4 loads staged through shared memory, no inter-CTA dependency.  Surviving
-// faces get a slot from a per-CTA-aggregated atomic counter (slots are NOT in face order: every later stage
-// orders by face index explicitly), write their 64 B raw screen record and count themselves into the tiles they
-// touch (RED.ADD on tile_count).  The last CTA to finish turns the counts into tile ranges and write cursors
-// (exclusive scan over the NT tiles), publishes n_visible / n_pairs / overflow flags and leaves every counter
-// it used at zero for the next call, so the launch sequence can be replayed from a CUDA graph unchanged.
+// 36 B read per face (soup), float4 loads staged through shared memory, no inter-CTA dependency and no tail.
+// Surviving faces get a slot from a per-CTA-aggregated atomic counter (slots are NOT in face order: every later
+// stage orders by face index explicitly), write their 64 B raw screen record and count themselves into the tiles
+// they touch (RED.ADD on tile_count).  The scan of the tile counts is done by the binning kernel (ts_sort.cu).
 //
 // Arithmetic follows the fixed operation order N1-N5 of DESIGN.md with explicit round-to-nearest intrinsics,
 // so cull decisions, pixel rects, tile counts and depth keys are bit-identical to the float32 oracle.
@@ -60,12 +58,11 @@ __device__ __forceinline__ void project_face(const float* p, const float* T, con
 template <bool SOUP>
 __global__ void __launch_bounds__(TS_PROJ_THREADS)
 project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __restrict__ faces,
-               const float* __restrict__ opacity, const float* __restrict__ Tcw, TsCamDev cam, float eps_area,
-               int pos_aligned) {
+               const float* __restrict__ Tcw, TsCamDev cam, float eps_area, int pos_aligned) {
     __shared__ __align__(16) float sp[TS_PROJ_THREADS * 9];
     __shared__ float sT[12];
     __shared__ uint32_t s_w[TS_PROJ_THREADS / 32];
-    __shared__ uint32_t s_base, s_last;
+    __shared__ uint32_t s_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid < 12) sT[tid] = __ldg(Tcw + tid);
     const int64_t face0 = (int64_t)blockIdx.x * TS_PROJ_THREADS;
@@ -122,79 +119,17 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
         const uint32_t slot = s_base + s_w[warp] + __popc(bal & ((1u << lane) - 1u));
         if (slot < f.vis_cap) {
             const uint32_t m = (uint32_t)(face0 + tid);
-            float ob;
-            if (SOUP) {
-                ob = (__ldg(opacity + 3 * (int64_t)m) + __ldg(opacity + 3 * (int64_t)m + 1) +
-                      __ldg(opacity + 3 * (int64_t)m + 2)) * (1.0f / 3.0f);
-            } else {
-                ob = (__ldg(opacity + __ldg(faces + 3 * (int64_t)m)) + __ldg(opacity + __ldg(faces + 3 * (int64_t)m + 1)) +
-                      __ldg(opacity + __ldg(faces + 3 * (int64_t)m + 2))) * (1.0f / 3.0f);
-            }
             const int rlo = (o.x0 & 0xffff) | (o.y0 << 16), rhi = (o.x1 & 0xffff) | (o.y1 << 16);
             float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
             s4[0] = make_float4(o.u[0], o.v[0], o.w[0], o.u[1]);
             s4[1] = make_float4(o.v[1], o.w[1], o.u[2], o.v[2]);
-            s4[2] = make_float4(o.w[2], ob, __int_as_float(rlo), __int_as_float(rhi));
+            s4[2] = make_float4(o.w[2], 0.0f, __int_as_float(rlo), __int_as_float(rhi));   // .y = mean opacity, set by the binning kernel
             s4[3] = make_float4(__uint_as_float(m), __uint_as_float(o.key), __uint_as_float(o.tiles), 0.0f);
             for (int ty = o.y0 >> 4; ty <= (o.y1 >> 4); ++ty)
                 for (int tx = o.x0 >> 4; tx <= (o.x1 >> 4); ++tx) atomicAdd(f.tile_count + ty * f.tiles_x + tx, 1u);
         }
     }
 
-    // ---- last CTA: tile counts -> ranges / cursors, publish the frame counters, re-arm ----
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        s_last = (atomicAdd(&f.ctrl->proj_done, 1u) == gridDim.x - 1) ? 1u : 0u;
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    volatile TsCtrl* ctrl = f.ctrl;
-    const uint32_t nv = ctrl->vis_counter;
-    const int per = (f.NT + TS_PROJ_THREADS - 1) / TS_PROJ_THREADS;
-    const int t0 = tid * per, t1 = min(f.NT, t0 + per);
-    uint32_t sum = 0, mx = 0;
-#pragma unroll 8
-    for (int t = t0; t < t1; ++t) {
-        const uint32_t c = __ldcg(f.tile_count + t);
-        sum += c;
-        mx = max(mx, c);
-    }
-    // block exclusive scan of the per-thread sums
-    uint32_t incl = sum;
-#pragma unroll
-    for (int d = 1; d < 32; d <<= 1) {
-        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
-        if (lane >= d) incl += t;
-    }
-    mx = __reduce_max_sync(0xffffffffu, mx);
-    __shared__ uint32_t s_ws[TS_PROJ_THREADS / 32], s_wm[TS_PROJ_THREADS / 32];
-    if (lane == 31) s_ws[warp] = incl;
-    if (lane == 0) s_wm[warp] = mx;
-    __syncthreads();
-    uint32_t woff = 0, total = 0, gmax = 0;
-#pragma unroll
-    for (int w = 0; w < TS_PROJ_THREADS / 32; ++w) {
-        if (w < warp) woff += s_ws[w];
-        total += s_ws[w];
-        gmax = max(gmax, s_wm[w]);
-    }
-    uint32_t fl = 0;
-    if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
-    if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
-    uint32_t run = woff + incl - sum;
-    for (int t = t0; t < t1; ++t) {
-        const uint32_t c = __ldcg(f.tile_count + t);
-        f.tile_ranges[t] = (fl || c == 0u) ? make_uint2(0u, 0u) : make_uint2(run, run + c);   // empty tile = (0,0)
-        f.tile_cursor[t] = run;
-        f.tile_count[t] = 0u;
-        run += c;
-    }
-    if (tid == 0) {
-        ctrl->n_visible = nv, ctrl->n_pairs = total, ctrl->flags = fl, ctrl->max_list = gmax;
-        ctrl->vis_counter = 0u, ctrl->proj_done = 0u;
-    }
 }
 
 }  // namespace
@@ -205,11 +140,11 @@ int32_t ts_launch_project(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, c
     const int aligned = ((reinterpret_cast<uintptr_t>(sc->pos) & 15u) == 0) ? 1 : 0;
     const uint32_t grid = (uint32_t)((f.M + TS_PROJ_THREADS - 1) / TS_PROJ_THREADS);
     if (sc->faces == nullptr)
-        project_kernel<true><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, nullptr, sc->opacity, fr->T_cw, fr->cam,
-                                                                   fr->prm.eps_area, aligned);
+        project_kernel<true><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, nullptr, fr->T_cw, fr->cam, fr->prm.eps_area,
+                                                                   aligned);
     else
-        project_kernel<false><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, sc->faces, sc->opacity, fr->T_cw,
-                                                                    fr->cam, fr->prm.eps_area, aligned);
+        project_kernel<false><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, sc->faces, fr->T_cw, fr->cam,
+                                                                    fr->prm.eps_area, aligned);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

@@ -33,15 +33,20 @@ struct TsGeom {
 
 __device__ __forceinline__ float ts_sqrt_approx(float x) {
     float y;
-    asm("sqrt.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float ts_rcp_approx(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
 
-__device__ __forceinline__ void ts_face_geom(const float4 s0, const float4 s1, const float4 s2, TsGeom& g) {
+__device__ __forceinline__ void ts_face_geom(const float4 s0, const float4 s1, const float4 s2, float obar, TsGeom& g) {
     g.qx[0] = s0.x, g.qy[0] = s0.y, g.w[0] = s0.z;
     g.qx[1] = s0.w, g.qy[1] = s1.x, g.w[1] = s1.y;
     g.qx[2] = s1.z, g.qy[2] = s1.w, g.w[2] = s2.x;
-    g.obar = s2.y;
+    g.obar = obar;
     // signed doubled area with the same operation order as the projection (N3): same sign on both sides
     const float a = __fsub_rn(g.qx[1], g.qx[0]), b = __fsub_rn(g.qy[2], g.qy[0]);
     const float c = __fsub_rn(g.qy[1], g.qy[0]), d = __fsub_rn(g.qx[2], g.qx[0]);
@@ -78,11 +83,12 @@ __device__ __forceinline__ void ts_face_geom(const float4 s0, const float4 s1, c
     }
 }
 
-// F7 + the backward-only per-face terms -> the 10-float4 record.  s0..s2 = raw screen record, cam for (xn, yn).
-__device__ __forceinline__ void ts_build_record(const float4 s0, const float4 s1, const float4 s2, const TsCamDev& cam,
-                                                float4* __restrict__ out) {
+// F7 + the backward-only per-face terms -> the 10-float4 record.  s0..s2 = raw screen record, obar = mean vertex
+// opacity, cam for (xn, yn).
+__device__ __forceinline__ void ts_build_record(const float4 s0, const float4 s1, const float4 s2, float obar,
+                                                const TsCamDev& cam, float4* __restrict__ out) {
     TsGeom g;
-    ts_face_geom(s0, s1, s2, g);
+    ts_face_geom(s0, s1, s2, obar, g);
     // d r / d q_j = -rho_j n_j - (r / sum ell) (u_{j,j+1} + u_{j,j+2}),  u_{j,i} = (q_j - q_i)/|q_j - q_i|;
     // stored as drr_j = -(1/r) dr/dq_j so that gq_j += (x * gx) * drr_j  (B6 iii)
     float drrx[3], drry[3], tau[3], xn[3], yn[3];

@@ -1,29 +1,28 @@
 // ts_render_bwd.cu -- a5/a6/a7: reverse-order backward of the compositing (B1-B9).
-//   render_bwd_kernel : one CTA per tile, one thread per pixel, walks the tile list BACK from the last
-//       contributing entry; recomputes alpha bit-identically to the forward kernel (ts_raster.cuh), recovers the
-//       transmittance in front of each face by T_n = T_{n+1}/(1-alpha_n), keeps ONE scalar "behind" accumulator
-//       R = R^c.gC + R^d gD + R^a gA (no division by T), and forms the per-hit gradients wrt the face's screen
-//       vertices (u,v,w) x 3, its vertex colours and its opacity.
+//   render_bwd_kernel : persistent warps, one 8x4-pixel block per job (ts_jobs.cuh), one pixel per lane; walks the
+//       tile list BACK from the block's last contributing entry, 32 entries at a time; recomputes alpha
+//       bit-identically to the forward kernel (ts_raster.cuh), recovers the transmittance in front of each face by
+//       T_n = T_{n+1}/(1-alpha_n), keeps ONE scalar "behind" accumulator R = R^c.gC + R^d gD + R^a gA (no division
+//       by T), and forms the per-hit gradients wrt the face's screen vertices (u,v,w) x 3, its vertex colours and
+//       its opacity.
 //       POSE-ONLY mode (tracking): every hit's nine screen terms are pushed straight through d(u,v,w)/dtau
 //       (Eq. 5-7) into six per-thread accumulators -- no shuffle, no atomic, no per-face
-//       buffer -- which are tree-reduced once per CTA into a per-tile partial (deterministic).
+//       buffer -- which are tree-reduced once per job into a per-job partial (fixed order: deterministic).
 //       FULL mode (mapping): per face the terms are reduced across the warp with shuffles BEFORE any global
-//       atomic (lane j issues the RED.ADD.F32 of term j).
+//       atomic (one lane issues the RED.ADD.F32s).
 //   proj_bwd_kernel   : full mode only; per visible face, screen -> camera -> world (B7-B8) and the se(3) terms
 //       [g_C ; Q x g_C], tree-reduced per CTA into fixed-order partials.
 //   pose_reduce_kernel: fixed-order final reduction of the partials to dL/dtau[6].
-#include "ts_raster.cuh"
+#include "ts_jobs.cuh"
 
 namespace {
 
-struct BwdSmem {
-    float4 r[TS_BATCH_BWD][12];       // R0 R1 R2 | kap,c00 | colours | colours | R4 R5 R6 R7 | R8 R9
-    uint32_t lm[8][TS_BATCH_BWD];
-    uint32_t slot[TS_BATCH_BWD];
-    uint32_t face[TS_BATCH_BWD];
-    uint32_t masks[8][TS_BATCH_BWD / 32];
-    uint32_t s_max;
-    float red[8][6];
+struct BwdWarpSmem {
+    float4 r[32][12];                 // R0 R1 R2 | kap,c00 | colours | colours | R4 R5 R6 R7 | R8 R9
+    uint32_t lm[32];
+    uint32_t slot[32];
+    uint32_t face[32];
+    uint32_t pos[32];                 // position of the entry in the tile list (0-based)
 };
 
 __device__ __forceinline__ float warp_sum(float v) {
@@ -35,254 +34,224 @@ __device__ __forceinline__ float warp_sum(float v) {
 // ATTR: colour / opacity gradients (B1, B4).  GEOM: screen-space vertex gradients into gscr (B5-B6).
 // POSE: screen-space vertex gradients pushed through Eq. 5-7 into per-thread se(3) accumulators (pose-only).
 template <int SM, bool ATTR, bool GEOM, bool POSE>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(TS_JOB_WARPS * 32)
 render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float fx, float fy,
                   const float* __restrict__ gCi, const float* __restrict__ gDi, const float* __restrict__ gAi,
                   float* __restrict__ grad_color, float* __restrict__ grad_opacity) {
-    __shared__ BwdSmem sm;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tile = blockIdx.x, tx0 = (tile % f.tiles_x) * TS_TILE, ty0 = (tile / f.tiles_x) * TS_TILE;
-    int lx, ly;
-    ts_thread_pixel(tid, lx, ly);
-    const int px = tx0 + lx, py = ty0 + ly;
-    const bool inside = px < f.W && py < f.H;
-    const float fpx = (float)px, fpy = (float)py;
-    const uint2 range = f.tile_ranges[tile];
-    const size_t p = (size_t)py * f.W + px, hw = (size_t)f.W * f.H;
-    uint32_t ncon = 0;
-    float Tcur = 1.0f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f;
-    if (inside && range.y > range.x) {
-        ncon = f.n_contrib[p];
-        Tcur = f.t_last[p];
-        if (gCi) gC0 = gCi[p], gC1 = gCi[hw + p], gC2 = gCi[2 * hw + p];
-        if (gDi) gD = gDi[p];
-        if (gAi) gA = gAi[p];
-    }
-    if (tid == 0) sm.s_max = 0;
-    __syncthreads();
-    const uint32_t wmax = __reduce_max_sync(0xffffffffu, ncon);
-    if (lane == 0 && wmax) atomicMax(&sm.s_max, wmax);
-    __syncthreads();
-    const uint32_t n_walk = min(sm.s_max, range.y - range.x);
-    float Rs = 0.f;                    // R^c.gC + R^d gD + R^a gA behind the current face
-    float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    bool first = true;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31;
+    BwdWarpSmem& sm = reinterpret_cast<BwdWarpSmem*>(smem_raw)[threadIdx.x >> 5];
+    const uint32_t n_jobs = (uint32_t)f.NT * TS_BLOCKS_PER_TILE;
+    const uint32_t lt = (1u << lane) - 1u;
+    const size_t hw = (size_t)f.W * f.H;
 
-    for (uint32_t hi = n_walk; hi > 0;) {
-        const uint32_t lo = hi > TS_BATCH_BWD ? hi - TS_BATCH_BWD : 0u;
-        const int nb = (int)(hi - lo);
-        __syncthreads();
-        if (tid < TS_BATCH_BWD) {
-            uint32_t lmask[8];
-#pragma unroll
-            for (int w = 0; w < 8; ++w) lmask[w] = 0u;
-            if (tid < nb) {
-                const uint2 sf = f.sorted[range.x + lo + tid];   // (slot, face)
-                const float4* rp = f.rec + TS_REC_F4 * (size_t)sf.x;
+    uint32_t j = ts_job_take(f, 1, lane);
+    while (j < n_jobs) {
+        TsJob job;
+        ts_job_decode(f, j, lane, job);
+        const uint32_t this_job = j;
+        j = ts_job_take(f, 1, lane);
+        const float fpx = (float)job.px, fpy = (float)job.py;
+        const size_t p = (size_t)job.py * f.W + job.px;
+        uint32_t ncon = 0;
+        float Tcur = 1.0f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f;
+        if (job.inside && job.range.y > job.range.x) {
+            ncon = f.n_contrib[p];
+            Tcur = f.t_last[p];
+            if (gCi) gC0 = gCi[p], gC1 = gCi[hw + p], gC2 = gCi[2 * hw + p];
+            if (gDi) gD = gDi[p];
+            if (gAi) gA = gAi[p];
+        }
+        const uint32_t n_walk = min(__reduce_max_sync(0xffffffffu, ncon), job.range.y - job.range.x);
+        float Rs = 0.f;                    // R^c.gC + R^d gD + R^a gA behind the current face
+        float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        bool first = true;
+
+        for (uint32_t hi = n_walk; hi > 0;) {
+            const uint32_t lo = hi > 32u ? hi - 32u : 0u;
+            const uint32_t n = hi - lo;
+            uint4 cur = make_uint4(0u, 0u, 0u, 0u);
+            if ((uint32_t)lane < n) cur = f.sorted[job.range.x + lo + lane];
+            const uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
+            const uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);
+            hi = lo;
+            if (ov == 0u) continue;
+            __syncwarp();
+            if (lmask) {
+                const int idx = __popc(ov & lt);
+                const float4* rp = f.rec + TS_REC_F4 * (size_t)cur.x;
                 float4 r[TS_REC_F4];
 #pragma unroll
                 for (int i = 0; i < (POSE ? 10 : 8); ++i) r[i] = __ldg(rp + i);
                 float col[9];
-                if (sc.faces == nullptr) {
-                    const float* cp = sc.color + 9 * (size_t)sf.y;
-#pragma unroll
-                    for (int j = 0; j < 9; ++j) col[j] = __ldg(cp + j);
-                } else {
-#pragma unroll
-                    for (int k = 0; k < 3; ++k) {
-                        const float* cp = sc.color + 3 * (size_t)__ldg(sc.faces + 3 * (size_t)sf.y + k);
-                        col[3 * k] = __ldg(cp), col[3 * k + 1] = __ldg(cp + 1), col[3 * k + 2] = __ldg(cp + 2);
-                    }
-                }
-                float4* d = sm.r[tid];
+                ts_load_colors(sc, cur.y, col);
+                float4* d = sm.r[idx];
                 d[0] = r[0], d[1] = r[1], d[2] = r[2];
                 d[3] = make_float4(r[3].x, r[3].y, r[3].z, col[0]);
                 d[4] = make_float4(col[1], col[2], col[3], col[4]);
                 d[5] = make_float4(col[5], col[6], col[7], col[8]);
                 d[6] = r[4], d[7] = r[5], d[8] = r[6], d[9] = r[7];
                 if (POSE) d[10] = r[8], d[11] = r[9];
-                sm.slot[tid] = sf.x, sm.face[tid] = sf.y;
-                const int rlo = __float_as_int(r[3].w), rhi = __float_as_int(r[4].w);
-                const int rx0 = max((int)(short)(rlo & 0xffff) - tx0, 0), ry0 = max((rlo >> 16) - ty0, 0);
-                const int rx1 = min((int)(short)(rhi & 0xffff) - tx0, 15), ry1 = min((rhi >> 16) - ty0, 15);
-#pragma unroll
-                for (int w = 0; w < 8; ++w) lmask[w] = ts_lane_mask(w, rx0, ry0, rx1, ry1);
+                sm.lm[idx] = lmask, sm.slot[idx] = cur.x, sm.face[idx] = cur.y, sm.pos[idx] = lo + (uint32_t)lane;
             }
+            __syncwarp();
+            for (int e = __popc(ov) - 1; e >= 0; --e) {
+                const bool in_rect = sm.pos[e] < ncon && ((sm.lm[e] >> lane) & 1u);
+                if (!__any_sync(0xffffffffu, in_rect)) continue;
+                const float4* R = sm.r[e];
+                const float4 r0 = R[0], r1 = R[1], r2 = R[2];
+                const float4* s4 = f.scr + TS_SCR_F4 * (size_t)sm.slot[e];
+                float l[3], x, I, alpha;
+                const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
+                const uint32_t hm = __ballot_sync(0xffffffffu, hit);
+                if (!hm) continue;
+                float acc[19];
+                if (!POSE) {
 #pragma unroll
-            for (int w = 0; w < 8; ++w) {
-                sm.lm[w][tid] = lmask[w];
-                const uint32_t bal = __ballot_sync(0xffffffffu, lmask[w] != 0u);
-                if (lane == 0) sm.masks[w][warp] = bal;
-            }
-        }
-        __syncthreads();
-        if (wmax > lo) {
-            for (int g = (nb - 1) >> 5; g >= 0; --g) {
-                uint32_t mk = sm.masks[warp][g];
-                while (mk) {
-                    const int bit = 31 - __clz(mk);
-                    mk &= ~(1u << bit);
-                    const int e = (g << 5) + bit;
-                    const uint32_t idx = lo + (uint32_t)e;          // list position relative to range.x
-                    const bool in_rect = idx < ncon && ((sm.lm[warp][e] >> lane) & 1u);
-                    if (!__any_sync(0xffffffffu, in_rect)) continue;
-                    const float4* R = sm.r[e];
-                    const float4 r0 = R[0], r1 = R[1], r2 = R[2];
-                    const float4* s4 = f.scr + TS_SCR_F4 * (size_t)sm.slot[e];
-                    float l[3], x, I, alpha;
-                    const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
-                    const uint32_t hm = __ballot_sync(0xffffffffu, hit);
-                    if (!hm) continue;
-                    float acc[19];
-                    if (!POSE) {
-#pragma unroll
-                        for (int j = 0; j < 19; ++j) acc[j] = 0.f;
+                    for (int jj = 0; jj < 19; ++jj) acc[jj] = 0.f;
+                }
+                if (hit) {
+                    const float4 r3 = R[3], r4 = R[4], r5 = R[5];
+                    // transmittance in front of this face
+                    const float one_m = __fsub_rn(1.0f, alpha);
+                    const float Tn = first ? Tcur : Tcur * ts_rcp_approx(one_m);
+                    Tcur = Tn, first = false;
+                    const float o0 = l[0] * r3.x, o1 = l[1] * r3.y, o2 = l[2] * r3.z;
+                    const float Om = (o0 + o1) + o2, z = ts_rcp_approx(Om);
+                    const float lam0 = o0 * z, lam1 = o1 * z, lam2 = o2 * z;
+                    // d_k = c_k . gC
+                    const float d0 = r3.w * gC0 + r4.x * gC1 + r4.y * gC2;
+                    const float d1 = r4.z * gC0 + r4.w * gC1 + r5.x * gC2;
+                    const float d2 = r5.y * gC0 + r5.z * gC1 + r5.w * gC2;
+                    const float cg = lam0 * d0 + lam1 * d1 + lam2 * d2;       // c . gC
+                    const float zgd = z * gD;
+                    const float S = cg + zgd + gA;
+                    const float wgt = Tn * alpha;
+                    const float ga = Tn * (S - Rs);                           // B2
+                    Rs = alpha * S + one_m * Rs;                              // B3
+                    if (ATTR) {
+                        // B1 colours, B4 opacity (one value per face; /3 applied when written)
+                        const float w0 = lam0 * wgt, w1 = lam1 * wgt, w2 = lam2 * wgt;
+                        acc[9] = w0 * gC0, acc[10] = w0 * gC1, acc[11] = w0 * gC2;
+                        acc[12] = w1 * gC0, acc[13] = w1 * gC1, acc[14] = w1 * gC2;
+                        acc[15] = w2 * gC0, acc[16] = w2 * gC1, acc[17] = w2 * gC2;
+                        acc[18] = I * ga;
                     }
-                    if (hit) {
-                        const float4 r3 = R[3], r4 = R[4], r5 = R[5];
-                        // transmittance in front of this face
-                        const float one_m = __fsub_rn(1.0f, alpha);
-                        const float Tn = first ? Tcur : __fdividef(Tcur, one_m);
-                        Tcur = Tn, first = false;
-                        const float o0 = l[0] * r3.x, o1 = l[1] * r3.y, o2 = l[2] * r3.z;
-                        const float Om = (o0 + o1) + o2, z = __fdividef(1.0f, Om);
-                        const float lam0 = o0 * z, lam1 = o1 * z, lam2 = o2 * z;
-                        // d_k = c_k . gC
-                        const float d0 = r3.w * gC0 + r4.x * gC1 + r4.y * gC2;
-                        const float d1 = r4.z * gC0 + r4.w * gC1 + r5.x * gC2;
-                        const float d2 = r5.y * gC0 + r5.z * gC1 + r5.w * gC2;
-                        const float cg = lam0 * d0 + lam1 * d1 + lam2 * d2;       // c . gC
-                        const float zgd = z * gD;
-                        const float S = cg + zgd + gA;
-                        const float wgt = Tn * alpha;
-                        const float ga = Tn * (S - Rs);                           // B2
-                        Rs = alpha * S + one_m * Rs;                              // B3
+                    if (GEOM || POSE) {
+                        const float4 q4 = R[6], q5 = R[7], q6 = R[8], q7 = R[9];   // record rows R4..R7
+                        // B4 window: gx = dL/dx
+                        const float gI = r2.w * ga;
+                        float gx;
+                        if (SM == 1) gx = gI;
+                        else if (SM == 2) gx = 0.5f * gI * ts_rcp_approx(I);
+                        else if (SM == 3) gx = 2.0f * gI * x;
+                        else gx = gI * sigma * I * ts_rcp_approx(x);
+                        // B5 interpolation
+                        const float wz = wgt * z, base = cg + zgd;
+                        const float go0 = wz * (d0 - base), go1 = wz * (d1 - base), go2 = wz * (d2 - base);
+                        const float b0 = -l[0] * q4.x, b1 = -l[1] * q4.y, b2 = -l[2] * q4.z;      // b_k = -lhat_k rho_k
+                        const float gw0 = b0 * go0, gw1 = b1 * go1, gw2 = b2 * go2;               // dL/dw_k
+                        // B6 (i): G = sum_k (w_k go_k) grad_p b_k,  grad_p b_k = -rho_k m_k
+                        const float t0 = q5.x * go0 * q4.x, t1 = q5.y * go1 * q4.y, t2 = q5.z * go2 * q4.z;
+                        const float Gx = -(t0 * r0.z + t1 * r1.x + t2 * r1.z), Gy = -(t0 * r0.w + t1 * r1.y + t2 * r1.w);
+                        float q0x = -b0 * Gx, q0y = -b0 * Gy, q1x = -b1 * Gx, q1y = -b1 * Gy, q2x = -b2 * Gx, q2y = -b2 * Gy;
+                        // B6 (ii): x = -lhat_{k*}; edge k* runs from a = q_{k*+1} to b = q_{k*+2};
+                        // t = b_{k*+2} + b_{k*} tau_{k*}
+                        if (l[0] >= l[1] && l[0] >= l[2]) {
+                            const float t = b2 + b0 * q5.w, mgx = r0.z * gx, mgy = r0.w * gx;
+                            q1x += (1.0f - t) * mgx, q1y += (1.0f - t) * mgy, q2x += t * mgx, q2y += t * mgy;
+                        } else if (l[1] >= l[2]) {
+                            const float t = b0 + b1 * q6.x, mgx = r1.x * gx, mgy = r1.y * gx;
+                            q2x += (1.0f - t) * mgx, q2y += (1.0f - t) * mgy, q0x += t * mgx, q0y += t * mgy;
+                        } else {
+                            const float t = b1 + b2 * q6.y, mgx = r1.z * gx, mgy = r1.w * gx;
+                            q0x += (1.0f - t) * mgx, q0y += (1.0f - t) * mgy, q1x += t * mgx, q1y += t * mgy;
+                        }
+                        // B6 (iii): through the inradius
+                        const float xg = x * gx;
+                        q0x += xg * q6.z, q0y += xg * q6.w, q1x += xg * q7.x, q1y += xg * q7.y;
+                        q2x += xg * q7.z, q2y += xg * q7.w;
+                        if (POSE) {
+                            // B7 + B9 per vertex, with Q = (xn, yn, 1)/w:  Z g_C = (a, b, c),
+                            // a = fx gu, b = fy gv, c = -(xn a + yn b) - w gw;  rho += w (a,b,c);  theta += Q x g_C
+                            const float4 n0 = R[10], n1 = R[11];
+                            {
+                                const float a = fx * q0x, b = fy * q0y, c = -(n0.x * a + n0.y * b) - q5.x * gw0;
+                                tau[0] += q5.x * a, tau[1] += q5.x * b, tau[2] += q5.x * c;
+                                tau[3] += n0.y * c - b, tau[4] += a - n0.x * c, tau[5] += n0.x * b - n0.y * a;
+                            }
+                            {
+                                const float a = fx * q1x, b = fy * q1y, c = -(n0.z * a + n0.w * b) - q5.y * gw1;
+                                tau[0] += q5.y * a, tau[1] += q5.y * b, tau[2] += q5.y * c;
+                                tau[3] += n0.w * c - b, tau[4] += a - n0.z * c, tau[5] += n0.z * b - n0.w * a;
+                            }
+                            {
+                                const float a = fx * q2x, b = fy * q2y, c = -(n1.x * a + n1.y * b) - q5.z * gw2;
+                                tau[0] += q5.z * a, tau[1] += q5.z * b, tau[2] += q5.z * c;
+                                tau[3] += n1.y * c - b, tau[4] += a - n1.x * c, tau[5] += n1.x * b - n1.y * a;
+                            }
+                        } else {
+                            acc[0] = q0x, acc[1] = q0y, acc[2] = gw0, acc[3] = q1x, acc[4] = q1y, acc[5] = gw1;
+                            acc[6] = q2x, acc[7] = q2y, acc[8] = gw2;
+                        }
+                    }
+                }
+                if (!POSE) {
+                    // reduce across the warp, then one lane issues the atomics
+                    const bool single = (hm & (hm - 1)) == 0;
+                    const int src = __ffs(hm) - 1;
+                    if (!single) {
+                        if (GEOM) {
+#pragma unroll
+                            for (int jj = 0; jj < 9; ++jj) acc[jj] = warp_sum(acc[jj]);
+                        }
                         if (ATTR) {
-                            // B1 colours, B4 opacity (one value per face; /3 applied when written)
-                            const float w0 = lam0 * wgt, w1 = lam1 * wgt, w2 = lam2 * wgt;
-                            acc[9] = w0 * gC0, acc[10] = w0 * gC1, acc[11] = w0 * gC2;
-                            acc[12] = w1 * gC0, acc[13] = w1 * gC1, acc[14] = w1 * gC2;
-                            acc[15] = w2 * gC0, acc[16] = w2 * gC1, acc[17] = w2 * gC2;
-                            acc[18] = I * ga;
-                        }
-                        if (GEOM || POSE) {
-                            const float4 q4 = R[6], q5 = R[7], q6 = R[8], q7 = R[9];   // record rows R4..R7
-                            // B4 window: gx = dL/dx
-                            const float gI = r2.w * ga;
-                            float gx;
-                            if (SM == 1) gx = gI;
-                            else if (SM == 2) gx = 0.5f * gI * __fdividef(1.0f, I);
-                            else if (SM == 3) gx = 2.0f * gI * x;
-                            else gx = gI * sigma * I * __fdividef(1.0f, x);
-                            // B5 interpolation
-                            const float wz = wgt * z, base = cg + zgd;
-                            const float go0 = wz * (d0 - base), go1 = wz * (d1 - base), go2 = wz * (d2 - base);
-                            const float b0 = -l[0] * q4.x, b1 = -l[1] * q4.y, b2 = -l[2] * q4.z;      // b_k = -lhat_k rho_k
-                            const float gw0 = b0 * go0, gw1 = b1 * go1, gw2 = b2 * go2;               // dL/dw_k
-                            // B6 (i): G = sum_k (w_k go_k) grad_p b_k,  grad_p b_k = -rho_k m_k
-                            const float t0 = q5.x * go0 * q4.x, t1 = q5.y * go1 * q4.y, t2 = q5.z * go2 * q4.z;
-                            const float Gx = -(t0 * r0.z + t1 * r1.x + t2 * r1.z), Gy = -(t0 * r0.w + t1 * r1.y + t2 * r1.w);
-                            float q0x = -b0 * Gx, q0y = -b0 * Gy, q1x = -b1 * Gx, q1y = -b1 * Gy, q2x = -b2 * Gx, q2y = -b2 * Gy;
-                            // B6 (ii): x = -lhat_{k*}; edge k* runs from a = q_{k*+1} to b = q_{k*+2};
-                            // t = b_{k*+2} + b_{k*} tau_{k*}
-                            if (l[0] >= l[1] && l[0] >= l[2]) {
-                                const float t = b2 + b0 * q5.w, mgx = r0.z * gx, mgy = r0.w * gx;
-                                q1x += (1.0f - t) * mgx, q1y += (1.0f - t) * mgy, q2x += t * mgx, q2y += t * mgy;
-                            } else if (l[1] >= l[2]) {
-                                const float t = b0 + b1 * q6.x, mgx = r1.x * gx, mgy = r1.y * gx;
-                                q2x += (1.0f - t) * mgx, q2y += (1.0f - t) * mgy, q0x += t * mgx, q0y += t * mgy;
-                            } else {
-                                const float t = b1 + b2 * q6.y, mgx = r1.z * gx, mgy = r1.w * gx;
-                                q0x += (1.0f - t) * mgx, q0y += (1.0f - t) * mgy, q1x += t * mgx, q1y += t * mgy;
-                            }
-                            // B6 (iii): through the inradius
-                            const float xg = x * gx;
-                            q0x += xg * q6.z, q0y += xg * q6.w, q1x += xg * q7.x, q1y += xg * q7.y;
-                            q2x += xg * q7.z, q2y += xg * q7.w;
-                            if (POSE) {
-                                // B7 + B9 per vertex, with Q = (xn, yn, 1)/w:  Z g_C = (a, b, c),
-                                // a = fx gu, b = fy gv, c = -(xn a + yn b) - w gw;  rho += w (a,b,c);  theta += Q x g_C
-                                const float4 n0 = R[10], n1 = R[11];
-                                {
-                                    const float a = fx * q0x, b = fy * q0y, c = -(n0.x * a + n0.y * b) - q5.x * gw0;
-                                    tau[0] += q5.x * a, tau[1] += q5.x * b, tau[2] += q5.x * c;
-                                    tau[3] += n0.y * c - b, tau[4] += a - n0.x * c, tau[5] += n0.x * b - n0.y * a;
-                                }
-                                {
-                                    const float a = fx * q1x, b = fy * q1y, c = -(n0.z * a + n0.w * b) - q5.y * gw1;
-                                    tau[0] += q5.y * a, tau[1] += q5.y * b, tau[2] += q5.y * c;
-                                    tau[3] += n0.w * c - b, tau[4] += a - n0.z * c, tau[5] += n0.z * b - n0.w * a;
-                                }
-                                {
-                                    const float a = fx * q2x, b = fy * q2y, c = -(n1.x * a + n1.y * b) - q5.z * gw2;
-                                    tau[0] += q5.z * a, tau[1] += q5.z * b, tau[2] += q5.z * c;
-                                    tau[3] += n1.y * c - b, tau[4] += a - n1.x * c, tau[5] += n1.x * b - n1.y * a;
-                                }
-                            } else {
-                                acc[0] = q0x, acc[1] = q0y, acc[2] = gw0, acc[3] = q1x, acc[4] = q1y, acc[5] = gw1;
-                                acc[6] = q2x, acc[7] = q2y, acc[8] = gw2;
-                            }
+#pragma unroll
+                            for (int jj = 9; jj < 19; ++jj) acc[jj] = warp_sum(acc[jj]);
                         }
                     }
-                    if (!POSE) {
-                        // reduce across the warp, then lane j issues the atomic of term j
-                        const bool single = (hm & (hm - 1)) == 0;
-                        const int src = __ffs(hm) - 1;
-                        if (!single) {
-                            if (GEOM) {
+                    if (lane == src) {
+                        if (GEOM) {
+                            float* gs = f.gscr + 9 * (size_t)sm.slot[e];
 #pragma unroll
-                                for (int j = 0; j < 9; ++j) acc[j] = warp_sum(acc[j]);
-                            }
-                            if (ATTR) {
-#pragma unroll
-                                for (int j = 9; j < 19; ++j) acc[j] = warp_sum(acc[j]);
-                            }
+                            for (int jj = 0; jj < 9; ++jj) atomicAdd(gs + jj, acc[jj]);
                         }
-                        if (lane == src) {
-                            if (GEOM) {
-                                float* gs = f.gscr + 9 * (size_t)sm.slot[e];
+                        if (ATTR) {
+                            const uint32_t m = sm.face[e];
+                            uint32_t v[3];
 #pragma unroll
-                                for (int j = 0; j < 9; ++j) atomicAdd(gs + j, acc[j]);
+                            for (int k = 0; k < 3; ++k) v[k] = sc.faces ? (uint32_t)__ldg(sc.faces + 3 * (size_t)m + k) : 3u * m + k;
+                            if (grad_color) {
+#pragma unroll
+                                for (int k = 0; k < 3; ++k)
+#pragma unroll
+                                    for (int ch = 0; ch < 3; ++ch) atomicAdd(grad_color + 3 * (size_t)v[k] + ch, acc[9 + 3 * k + ch]);
                             }
-                            if (ATTR) {
-                                const uint32_t m = sm.face[e];
-                                uint32_t v[3];
+                            if (grad_opacity) {
+                                const float go = acc[18] * (1.0f / 3.0f);
 #pragma unroll
-                                for (int k = 0; k < 3; ++k) v[k] = sc.faces ? (uint32_t)__ldg(sc.faces + 3 * (size_t)m + k) : 3u * m + k;
-                                if (grad_color) {
-#pragma unroll
-                                    for (int k = 0; k < 3; ++k)
-#pragma unroll
-                                        for (int ch = 0; ch < 3; ++ch) atomicAdd(grad_color + 3 * (size_t)v[k] + ch, acc[9 + 3 * k + ch]);
-                                }
-                                if (grad_opacity) {
-                                    const float go = acc[18] * (1.0f / 3.0f);
-#pragma unroll
-                                    for (int k = 0; k < 3; ++k) atomicAdd(grad_opacity + v[k], go);
-                                }
+                                for (int k = 0; k < 3; ++k) atomicAdd(grad_opacity + v[k], go);
                             }
                         }
                     }
                 }
             }
         }
-        hi = lo;
-    }
-    if (POSE) {
-        // per-thread -> per-warp (shuffles) -> per-CTA (shared memory, fixed order) -> per-tile partial
+        if (POSE) {
+            // per-thread -> per-job partial (fixed shuffle tree; the final reduction runs over jobs in index order)
 #pragma unroll
-        for (int j = 0; j < 6; ++j) {
-            const float s = warp_sum(tau[j]);
-            if (lane == 0) sm.red[warp][j] = s;
-        }
-        __syncthreads();
-        if (tid < 6) {
-            float s = 0.f;
+            for (int jj = 0; jj < 6; ++jj) tau[jj] = warp_sum(tau[jj]);
+            if (lane < 6) {
+                float v = tau[0];
 #pragma unroll
-            for (int w = 0; w < 8; ++w) s += sm.red[w][tid];
-            f.pose_partials[6 * (size_t)tile + tid] = s;
+                for (int jj = 1; jj < 6; ++jj) v = (lane == jj) ? tau[jj] : v;
+                // partials are indexed by (tile, block), not by ticket: the sum order does not depend on scheduling
+                f.pose_partials[6 * ((size_t)job.tile * TS_BLOCKS_PER_TILE + job.blk) + lane] = v;
+            }
+            (void)this_job;
         }
     }
+    ts_job_finish(f, 1, lane);
 }
 
 }  // namespace
@@ -356,34 +325,52 @@ proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __re
 }
 
 // a7: fixed-order tree reduction of the partials
-__global__ void __launch_bounds__(256) pose_reduce_kernel(const float* __restrict__ partials, uint32_t n, float* __restrict__ out) {
-    __shared__ float sm[256][6];
-    const int tid = threadIdx.x;
+__global__ void __launch_bounds__(1024) pose_reduce_kernel(const float* __restrict__ partials, uint32_t n, float* __restrict__ out) {
+    __shared__ float sm[32][6];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     float a[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    for (uint32_t i = tid; i < n; i += 256)
-#pragma unroll
-        for (int j = 0; j < 6; ++j) a[j] += partials[6 * (size_t)i + j];
-#pragma unroll
-    for (int j = 0; j < 6; ++j) sm[tid][j] = a[j];
-    __syncthreads();
-    for (int s = 128; s > 0; s >>= 1) {
-        if (tid < s)
-#pragma unroll
-            for (int j = 0; j < 6; ++j) sm[tid][j] += sm[tid + s][j];
-        __syncthreads();
+    const float2* p2 = reinterpret_cast<const float2*>(partials);
+    for (uint32_t i = tid; i < n; i += 1024) {
+        const float2 v0 = p2[3 * (size_t)i], v1 = p2[3 * (size_t)i + 1], v2 = p2[3 * (size_t)i + 2];
+        a[0] += v0.x, a[1] += v0.y, a[2] += v1.x, a[3] += v1.y, a[4] += v2.x, a[5] += v2.y;
     }
-    if (tid < 6) out[tid] = sm[0][tid];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) a[j] += __shfl_xor_sync(0xffffffffu, a[j], d);
+        if (lane == 0) sm[warp][j] = a[j];
+    }
+    __syncthreads();
+    if (tid < 6) {
+        float s = 0.f;
+#pragma unroll
+        for (int w = 0; w < 32; ++w) s += sm[w][tid];
+        out[tid] = s;
+    }
+}
+
+template <int SM, bool ATTR, bool GEOM, bool POSE>
+void launch_one(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, const float* gC, const float* gD, const float* gA,
+                float* gcol, float* gopa, cudaStream_t st) {
+    const TsFrameDev& f = fr->d;
+    const size_t smem = sizeof(BwdWarpSmem) * TS_JOB_WARPS;
+    static bool attr_set = false;                      // one-time opt-in above 48 KB of dynamic shared memory
+    if (!attr_set) {
+        cudaFuncSetAttribute(render_bwd_kernel<SM, ATTR, GEOM, POSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        attr_set = true;
+    }
+    const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 3, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
+    render_bwd_kernel<SM, ATTR, GEOM, POSE><<<grid, TS_JOB_WARPS * 32, smem, st>>>(f, sc, fr->prm.sigma, fr->prm.alpha_min,
+                                                                                   fr->cam.fx, fr->cam.fy, gC, gD, gA, gcol, gopa);
 }
 
 template <int SM>
-void launch_bwd_sm(const ts_frame* fr, const ts_scene& sc, const float* gC, const float* gD, const float* gA,
+void launch_bwd_sm(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, const float* gC, const float* gD, const float* gA,
                    float* gcol, float* gopa, bool attr, bool geom, bool pose_only, cudaStream_t st) {
-    const TsFrameDev& f = fr->d;
-    const float sg = fr->prm.sigma, am = fr->prm.alpha_min, fx = fr->cam.fx, fy = fr->cam.fy;
-    if (pose_only) render_bwd_kernel<SM, false, false, true><<<f.NT, 256, 0, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa);
-    else if (attr && geom) render_bwd_kernel<SM, true, true, false><<<f.NT, 256, 0, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa);
-    else if (geom) render_bwd_kernel<SM, false, true, false><<<f.NT, 256, 0, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa);
-    else render_bwd_kernel<SM, true, false, false><<<f.NT, 256, 0, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa);
+    if (pose_only) launch_one<SM, false, false, true>(ctx, fr, sc, gC, gD, gA, gcol, gopa, st);
+    else if (attr && geom) launch_one<SM, true, true, false>(ctx, fr, sc, gC, gD, gA, gcol, gopa, st);
+    else if (geom) launch_one<SM, false, true, false>(ctx, fr, sc, gC, gD, gA, gcol, gopa, st);
+    else launch_one<SM, true, false, false>(ctx, fr, sc, gC, gD, gA, gcol, gopa, st);
 }
 
 }  // namespace
@@ -398,14 +385,14 @@ int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
     float* gcol = (mask & TS_GRAD_COLOR) ? grad_color : nullptr;
     float* gopa = (mask & TS_GRAD_OPACITY) ? grad_opacity : nullptr;
     switch (ts_sigma_mode(fr->prm.sigma)) {
-        case 1: launch_bwd_sm<1>(fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
-        case 2: launch_bwd_sm<2>(fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
-        case 3: launch_bwd_sm<3>(fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
-        default: launch_bwd_sm<0>(fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
+        case 1: launch_bwd_sm<1>(ctx, fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
+        case 2: launch_bwd_sm<2>(ctx, fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
+        case 3: launch_bwd_sm<3>(ctx, fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
+        default: launch_bwd_sm<0>(ctx, fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
     }
     fr->pose_src = 0;
     if (pose_only) {
-        fr->pose_src = 1, fr->n_pose_partials = (uint32_t)fr->d.NT;
+        fr->pose_src = 1, fr->n_pose_partials = (uint32_t)fr->d.NT * TS_BLOCKS_PER_TILE;
     } else if (geom) {
         const int grid = (int)min((uint32_t)(ctx->num_sms * 4), fr->d.n_partials_cap);
         const int want_pose = (mask & TS_GRAD_POSE) ? 1 : 0;
@@ -422,7 +409,7 @@ int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
 
 int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame* fr, float* out, cudaStream_t st) {
     if (fr->pose_src == 0) return TS_ERR_STATE;
-    pose_reduce_kernel<<<1, 256, 0, st>>>(fr->d.pose_partials, fr->n_pose_partials, out);
+    pose_reduce_kernel<<<1, 1024, 0, st>>>(fr->d.pose_partials, fr->n_pose_partials, out);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

@@ -1,49 +1,166 @@
 // ts_sort.cu -- a2: bin + sort ("faces are sorted in depth order") as an MSD-first radix sort of
 // the (tile, depth) key, shaped for P ~ 1e5..1e6 pairs where a global LSD sort is pure launch latency:
-//   bin_setup_kernel : the most-significant digit IS the tile id, and its histogram and exclusive scan already
-//       exist (tile_count -> tile_ranges / tile_cursor, made by the project kernel), so the MSD pass is one
-//       scatter: every visible face writes (depth_key << 32 | face, slot) into the segment of each tile it
-//       touches (cursor atomics; faces that touch many tiles are spread over the warp).  The same pass builds
-//       the face's 160 B render record once (F7), instead of once per (tile, face) pair inside the renderers.
+//   bin_setup_kernel : the most-significant digit IS the tile id and its histogram already exists (tile_count,
+//       made by the project kernel).  Every CTA scans the NT counts into shared memory by itself (13 KB of L2
+//       reads: cheaper than a scan kernel or a last-CTA tail; CTA 0 also publishes tile_ranges, the frame
+//       counters and the heaviest-first tile order of the render work queues), then the MSD pass is one scatter:
+//       every visible face writes (depth_key, face, slot, rect) into the segment of each tile it touches (cursor
+//       atomics; faces that touch many tiles are spread over the warp).  The same pass builds the face's 160 B
+//       render record once (F7: unit normals, inradius, incentre, mean opacity), instead of once per (tile, face)
+//       pair inside the renderers.
 //   tile_sort_kernel : one CTA per tile sorts its segment by the remaining 60 key bits (depth, then face index:
-//       the result is exactly the stable sort of (tile << 32 | depth) with faces emitted in index order, F6) in
-//       shared memory -- rank sort for short lists, bitonic network above -- and writes the sorted (slot, face)
-//       list the renderers walk plus the sorted 64-bit keys.  Segments longer than TS_SORT_SMEM run the same
-//       network in global memory (slow, correct, rare).
+//       exactly the stable sort of (tile << 32 | depth) with faces emitted in index order, F6) in shared memory --
+//       rank sort for short lists, a compare-exchange network above -- and writes the sorted
+//       (slot, face, rect) list the renderers walk plus the sorted 64-bit keys.  Segments longer than
+//       TS_SORT_SMEM run the same network in global memory (slow, correct, rare).  It also re-zeroes the counters.
 // Integer only; bit-exact against the oracle's std::stable_sort.
 #include "ts_raster.cuh"
 
 namespace {
 
+// exclusive scan of tile_count[0..NT) by one CTA.  offs (shared or global) receives the offsets; returns the total
+// and the longest list.  Every thread owns a contiguous run of tiles.
+__device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* offs, uint32_t* s_tmp /*[2*warps+2]*/,
+                                               uint32_t& total, uint32_t& gmax) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
+    const int per = (f.NT + (int)blockDim.x - 1) / (int)blockDim.x;
+    const int t0 = min(f.NT, tid * per), t1 = min(f.NT, t0 + per);
+    uint32_t sum = 0, mx = 0;
+#pragma unroll 4
+    for (int t = t0; t < t1; ++t) {
+        const uint32_t c = __ldcg(f.tile_count + t);
+        sum += c, mx = max(mx, c);
+    }
+    uint32_t incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+    }
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if (lane == 31) s_tmp[warp] = incl;
+    if (lane == 0) s_tmp[nwarp + warp] = mx;
+    __syncthreads();
+    uint32_t woff = 0;
+    total = 0, gmax = 0;
+    for (int w = 0; w < nwarp; ++w) {
+        const uint32_t c = s_tmp[w];
+        if (w < warp) woff += c;
+        total += c;
+        gmax = max(gmax, s_tmp[nwarp + w]);
+    }
+    uint32_t run = woff + incl - sum;
+    for (int t = t0; t < t1; ++t) {
+        offs[t] = run;
+        run += __ldcg(f.tile_count + t);
+    }
+    __syncthreads();
+}
+
+// CTA 0 only: tile_ranges, frame counters, and the tile order (descending log2 bucket of the list length) that
+// the persistent render kernels pull work in
+__device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_t* offs, uint32_t nv, uint32_t total,
+                                              uint32_t gmax, uint32_t fl, uint32_t* s_hist /*[34]*/) {
+    const int tid = threadIdx.x;
+    if (tid < 34) s_hist[tid] = 0;
+    __syncthreads();
+    for (int t = tid; t < f.NT; t += blockDim.x) {
+        const uint32_t c = __ldcg(f.tile_count + t);
+        f.tile_ranges[t] = (fl || c == 0u) ? make_uint2(0u, 0u) : make_uint2(offs[t], offs[t] + c);   // empty tile = (0,0)
+        atomicAdd(&s_hist[32 - __clz(c)], 1u);                 // bucket 0 = empty, b = floor(log2 c) + 1
+    }
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t run = 0;
+        for (int b = 32; b >= 0; --b) {                        // heaviest bucket first
+            const uint32_t c = s_hist[b];
+            s_hist[b] = run;
+            run += c;
+        }
+        volatile TsCtrl* ctrl = f.ctrl;
+        ctrl->n_visible = nv, ctrl->n_pairs = total, ctrl->flags = fl, ctrl->max_list = gmax;
+    }
+    __syncthreads();
+    for (int t = tid; t < f.NT; t += blockDim.x) {
+        const uint32_t c = __ldcg(f.tile_count + t);
+        f.tile_order[atomicAdd(&s_hist[32 - __clz(c)], 1u)] = (uint32_t)t;
+    }
+}
+
+// fallback for NT > TS_SCAN_LOCAL_MAX: one CTA scans into global memory
+__global__ void __launch_bounds__(1024) tile_scan_kernel(TsFrameDev f) {
+    __shared__ uint32_t s_tmp[66];
+    __shared__ uint32_t s_hist[34];
+    uint32_t total, gmax;
+    cta_scan_tiles(f, f.tile_offset, s_tmp, total, gmax);
+    const uint32_t nv = *(volatile uint32_t*)&f.ctrl->vis_counter;
+    uint32_t fl = 0;
+    if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
+    if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
+    publish_tiles(f, f.tile_offset, nv, total, gmax, fl, s_hist);
+}
+
+template <bool LOCAL, bool SOUP>
 __global__ void __launch_bounds__(TS_BIN_THREADS)
-bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
+bin_setup_kernel(TsFrameDev f, TsCamDev cam, const float* __restrict__ opacity, const int32_t* __restrict__ faces) {
+    __shared__ uint32_t s_offs[LOCAL ? TS_SCAN_LOCAL_MAX : 1];
+    __shared__ uint32_t s_tmp[2 * (TS_BIN_THREADS / 32) + 2];
+    __shared__ uint32_t s_hist[34];
     const int lane = threadIdx.x & 31;
-    const uint32_t nvis = min(ts_eff_visible(f), f.vis_cap);
+    uint32_t nv, fl;
+    const uint32_t* offs;
+    if (LOCAL) {
+        uint32_t total, gmax;
+        cta_scan_tiles(f, s_offs, s_tmp, total, gmax);
+        nv = *(volatile uint32_t*)&f.ctrl->vis_counter;
+        fl = 0;
+        if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
+        if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
+        if (blockIdx.x == 0) publish_tiles(f, s_offs, nv, total, gmax, fl, s_hist);
+        offs = s_offs;
+    } else {
+        const volatile TsCtrl* ctrl = f.ctrl;
+        nv = ctrl->n_visible, fl = ctrl->flags;
+        offs = f.tile_offset;
+    }
+    const uint32_t nvis = fl ? 0u : nv;
     const uint32_t n_round = (nvis + TS_BIN_THREADS - 1) / TS_BIN_THREADS * TS_BIN_THREADS;
     for (uint32_t slot = blockIdx.x * TS_BIN_THREADS + threadIdx.x; slot < n_round; slot += gridDim.x * TS_BIN_THREADS) {
         const bool live = slot < nvis;
         int tx0 = 0, ty0 = 0, ntx = 0, nty = 0;
-        unsigned long long key = 0;
+        uint4 pa = make_uint4(0u, 0u, slot, 0u);
+        uint32_t pb = 0;
         if (live) {
-            const float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
+            float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
             const float4 s0 = s4[0], s1 = s4[1], s2 = s4[2], s3 = s4[3];
+            const uint32_t m = __float_as_uint(s3.x);
+            float ob;                                            // mean vertex opacity
+            if (SOUP) {
+                ob = (__ldg(opacity + 3 * (size_t)m) + __ldg(opacity + 3 * (size_t)m + 1) + __ldg(opacity + 3 * (size_t)m + 2)) *
+                     (1.0f / 3.0f);
+            } else {
+                ob = (__ldg(opacity + __ldg(faces + 3 * (size_t)m)) + __ldg(opacity + __ldg(faces + 3 * (size_t)m + 1)) +
+                      __ldg(opacity + __ldg(faces + 3 * (size_t)m + 2))) * (1.0f / 3.0f);
+            }
             float4 rec[TS_REC_F4];
-            ts_build_record(s0, s1, s2, cam, rec);
+            ts_build_record(s0, s1, s2, ob, cam, rec);
             float4* out = f.rec + TS_REC_F4 * (size_t)slot;
 #pragma unroll
             for (int i = 0; i < TS_REC_F4; ++i) out[i] = rec[i];
+            s4[2] = make_float4(s2.x, ob, s2.z, s2.w);
             const int rlo = __float_as_int(s2.z), rhi = __float_as_int(s2.w);
             const int x0 = (int)(short)(rlo & 0xffff), y0 = rlo >> 16, x1 = (int)(short)(rhi & 0xffff), y1 = rhi >> 16;
             tx0 = x0 >> 4, ty0 = y0 >> 4, ntx = (x1 >> 4) - tx0 + 1, nty = (y1 >> 4) - ty0 + 1;
-            key = ((unsigned long long)__float_as_uint(s3.y) << 32) | __float_as_uint(s3.x);
+            pa = make_uint4(__float_as_uint(s3.y), m, slot, (uint32_t)rlo);
+            pb = (uint32_t)rhi;
         }
         const int nt = ntx * nty;
         // narrow faces (the common case): the owning lane scatters its <= 4 pairs itself
         if (nt <= 4) {
             for (int i = 0; i < nt; ++i) {
-                const int ty = ty0 + i / ntx, tx = tx0 + i % ntx;
-                const uint32_t pos = atomicAdd(f.tile_cursor + ty * f.tiles_x + tx, 1u);
-                if (pos < f.pair_cap) f.pkey[pos] = key, f.pslot[pos] = slot;
+                const int t = (ty0 + i / ntx) * f.tiles_x + tx0 + i % ntx;
+                const uint32_t pos = offs[t] + atomicAdd(f.tile_cursor + t, 1u);
+                if (pos < f.pair_cap) f.pair_a[pos] = pa, f.pair_b[pos] = pb;
             }
         }
         // wide faces: the whole warp scatters one face's tiles together
@@ -53,12 +170,14 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
             wide &= wide - 1;
             const int btx0 = __shfl_sync(0xffffffffu, tx0, src), bty0 = __shfl_sync(0xffffffffu, ty0, src);
             const int bntx = __shfl_sync(0xffffffffu, ntx, src), bnt = __shfl_sync(0xffffffffu, nt, src);
-            const unsigned long long bkey = __shfl_sync(0xffffffffu, key, src);
-            const uint32_t bslot = __shfl_sync(0xffffffffu, slot, src);
+            uint4 ba;
+            ba.x = __shfl_sync(0xffffffffu, pa.x, src), ba.y = __shfl_sync(0xffffffffu, pa.y, src);
+            ba.z = __shfl_sync(0xffffffffu, pa.z, src), ba.w = __shfl_sync(0xffffffffu, pa.w, src);
+            const uint32_t bb = __shfl_sync(0xffffffffu, pb, src);
             for (int i = lane; i < bnt; i += 32) {
-                const int ty = bty0 + i / bntx, tx = btx0 + i % bntx;
-                const uint32_t pos = atomicAdd(f.tile_cursor + ty * f.tiles_x + tx, 1u);
-                if (pos < f.pair_cap) f.pkey[pos] = bkey, f.pslot[pos] = bslot;
+                const int t = (bty0 + i / bntx) * f.tiles_x + btx0 + i % bntx;
+                const uint32_t pos = offs[t] + atomicAdd(f.tile_cursor + t, 1u);
+                if (pos < f.pair_cap) f.pair_a[pos] = ba, f.pair_b[pos] = bb;
             }
         }
     }
@@ -103,48 +222,59 @@ __device__ __forceinline__ void cta_sort_network(KP k, VP v, uint32_t n) {
     }
 }
 
-__global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f) {
+__device__ __forceinline__ void emit_sorted(const TsFrameDev& f, uint32_t base, uint32_t rank, uint32_t src,
+                                            unsigned long long thi) {
+    const uint4 a = f.pair_a[base + src];
+    f.sorted[base + rank] = make_uint4(a.z, a.y, a.w, f.pair_b[base + src]);     // (slot, face, rect_lo, rect_hi)
+    f.skey[base + rank] = thi | a.x;
+}
+
+__global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f, unsigned long long* __restrict__ gkeys,
+                                                                    uint32_t* __restrict__ gidx) {
     __shared__ unsigned long long sk[TS_SORT_SMEM];
     __shared__ uint32_t sv[TS_SORT_SMEM];
-    const uint32_t tile = blockIdx.x;
+    const uint32_t tile = blockIdx.x, tid = threadIdx.x;
     const uint2 range = f.tile_ranges[tile];
+    // this kernel is the last reader of the project / binning counters: leave them at zero for the next frame
+    if (tid == 0) {
+        f.tile_count[tile] = 0u, f.tile_cursor[tile] = 0u;
+        if (tile == 0) f.ctrl->vis_counter = 0u;
+    }
     const uint32_t n = range.y - range.x;
     if (n == 0) return;
     const unsigned long long thi = (unsigned long long)tile << 32;
-    unsigned long long* gk = f.pkey + range.x;
-    uint32_t* gv = f.pslot + range.x;
-    if (n <= TS_SORT_THREADS) {
-        // rank sort: keys are unique (the face index is part of the key), so ranks are a permutation
-        unsigned long long mine = 0;
-        uint32_t mv = 0;
-        if (threadIdx.x < n) mine = gk[threadIdx.x], mv = gv[threadIdx.x], sk[threadIdx.x] = mine;
-        __syncthreads();
-        if (threadIdx.x < n) {
-            uint32_t rank = 0;
-            for (uint32_t j = 0; j < n; ++j) rank += (sk[j] < mine) ? 1u : 0u;
-            f.sorted[range.x + rank] = make_uint2(mv, (uint32_t)mine);
-            f.skey[range.x + rank] = thi | (mine >> 32);
-        }
-        return;
-    }
     if (n <= TS_SORT_SMEM) {
-        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) sk[i] = gk[i], sv[i] = gv[i];
-        __syncthreads();
-        cta_sort_network(sk, sv, n);
-        for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
-            const unsigned long long kk = sk[i];
-            f.sorted[range.x + i] = make_uint2(sv[i], (uint32_t)kk);
-            f.skey[range.x + i] = thi | (kk >> 32);
+        for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
+            const uint4 a = f.pair_a[range.x + i];
+            sk[i] = ((unsigned long long)a.x << 32) | a.y;
+            sv[i] = i;
         }
+        __syncthreads();
+        if (n <= 2 * TS_SORT_THREADS) {
+            // rank sort: keys are unique (the face index is part of the key), so ranks are a permutation
+            for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
+                const unsigned long long mine = sk[i];
+                uint32_t rank = 0;
+                for (uint32_t j = 0; j < n; ++j) rank += (sk[j] < mine) ? 1u : 0u;
+                emit_sorted(f, range.x, rank, i, thi);
+            }
+            return;
+        }
+        cta_sort_network(sk, sv, n);
+        for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) emit_sorted(f, range.x, i, sv[i], thi);
         return;
     }
-    // oversize segment: same network, in place in global memory (volatile: exchanged across threads between barriers)
-    cta_sort_network((volatile unsigned long long*)gk, (volatile uint32_t*)gv, n);
-    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
-        const unsigned long long kk = gk[i];
-        f.sorted[range.x + i] = make_uint2(gv[i], (uint32_t)kk);
-        f.skey[range.x + i] = thi | (kk >> 32);
+    // oversize segment: same network in global scratch (volatile: exchanged across threads between barriers)
+    unsigned long long* gk = gkeys + range.x;
+    uint32_t* gv = gidx + range.x;
+    for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
+        const uint4 a = f.pair_a[range.x + i];
+        gk[i] = ((unsigned long long)a.x << 32) | a.y;
+        gv[i] = i;
     }
+    __syncthreads();
+    cta_sort_network((volatile unsigned long long*)gk, (volatile uint32_t*)gv, n);
+    for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) emit_sorted(f, range.x, i, gv[i], thi);
 }
 
 }  // namespace
@@ -152,9 +282,17 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
 int32_t ts_launch_sort(const ts_ctx* ctx, ts_frame* fr, cudaStream_t stream) {
     const TsFrameDev& f = fr->d;
     const uint32_t grid_bin = (uint32_t)min((uint64_t)(f.vis_cap + TS_BIN_THREADS - 1) / TS_BIN_THREADS,
-                                            (uint64_t)ctx->num_sms * 16u);
-    bin_setup_kernel<<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam);
-    tile_sort_kernel<<<f.NT, TS_SORT_THREADS, 0, stream>>>(f);
+                                            (uint64_t)ctx->num_sms * 4u);
+    const bool soup = fr->scene.faces == nullptr;
+    if (f.NT <= TS_SCAN_LOCAL_MAX) {
+        if (soup) bin_setup_kernel<true, true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, nullptr);
+        else bin_setup_kernel<true, false><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, fr->scene.faces);
+    } else {
+        tile_scan_kernel<<<1, 1024, 0, stream>>>(f);
+        if (soup) bin_setup_kernel<false, true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, nullptr);
+        else bin_setup_kernel<false, false><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, fr->scene.faces);
+    }
+    tile_sort_kernel<<<f.NT, TS_SORT_THREADS, 0, stream>>>(f, f.big_key, f.big_idx);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

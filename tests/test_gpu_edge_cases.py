@@ -148,7 +148,7 @@ def test_determinism(ctx, oracle_mod):
     for _ in range(2):
         g = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
         C, D, A = g.forward()
-        keys, vals = g.view(ts.VIEW_KEYS), g.view(ts.VIEW_VALS).reshape(-1, 2)[:, 1]   # slots are allocation-ordered
+        keys, vals = g.view(ts.VIEW_KEYS), g.view(ts.VIEW_VALS).reshape(-1, 4)[:, 1]   # slots are allocation-ordered
         gp, gc, go, tau = g.backward(np.ones_like(C), np.ones_like(D), None, ts.GRAD_ALL)
         outs.append((C, D, A, keys, vals, gp, tau))
         # same frame reused (second project/sort/render on the same workspace) must reproduce itself too

@@ -56,7 +56,7 @@ def check_project_and_sort(o, g, M):
     assert np.array_equal(scatter_per_face(M, vf, vis[:, 14].view(np.uint32)), pr.tiles_touched)
     assert np.array_equal(vis[:, :9].view(np.uint32), pr.scr[vf].view(np.uint32))   # (u,v,w) bit for bit
     assert np.array_equal(g.view(ts.VIEW_KEYS).view(np.uint64), b.keys)
-    sv = g.view(ts.VIEW_VALS).reshape(-1, 2).astype(np.int64)                  # sorted (slot, face)
+    sv = g.view(ts.VIEW_VALS).reshape(-1, 4).astype(np.int64)                  # sorted (slot, face, rect_lo, rect_hi)
     assert np.array_equal(sv[:, 1], b.vals.astype(np.int64))
     assert np.array_equal(vf[sv[:, 0]], sv[:, 1])
     assert np.array_equal(g.view(ts.VIEW_TILE_RANGES).reshape(-1, 2).view(np.uint32), b.ranges)
