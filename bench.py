@@ -4,7 +4,7 @@
 
 A step = ONE tracking iteration on BASELINE.json configs[2] (Replica-shaped, 1200x680, 500k faces, seed 2):
 ts_project -> ts_bin_sort -> ts_render_fwd -> ts_l1_loss_grad -> ts_render_bwd(pose-only) ->
-ts_pose_jacobian_reduce -> ts_pose_step, i.e. every row a1..a8 of DESIGN.md section 2, on synthetic data.
+ts_pose_reduce_step (= ts_pose_jacobian_reduce + ts_pose_step in one launch), i.e. every row a1..a8 of DESIGN.md section 2, on synthetic data.
 L2 is flushed between timed steps (the 18 MB map would otherwise stay L2-resident across iterations); the extra
 "tracking_iters_per_s" figure is the 100-iteration block of one frame WITHOUT flushes (the real tracking loop).
 
@@ -146,7 +146,7 @@ class Tracker:
         ts.ts_render_fwd(self.ctx, self.scene, self.frame, self.Chat, self.Dhat, None)
         torch.cuda.synchronize()
 
-    launches_per_iter = 1 + 2 + 1 + 1 + 1 + 1 + 1   # project, bin+sort, fwd, loss, bwd, reduce, step
+    launches_per_iter = 1 + 2 + 1 + 1 + 1 + 1   # project, bin + sort, fwd, loss, bwd, reduce+step
 
     def forward(self):
         ts = self.ts
@@ -159,8 +159,7 @@ class Tracker:
         ts.ts_l1_loss_grad(self.ctx, self.W, self.H, self.C, self.D, self.Chat, self.Dhat, self.sc.params.lambda_dep,
                            self.gC, self.gD, self.loss)
         ts.ts_render_bwd(self.ctx, self.scene, self.frame, self.gC, self.gD, None, None, None, None, ts.GRAD_POSE)
-        ts.ts_pose_jacobian_reduce(self.ctx, self.frame, self.tau)
-        ts.ts_pose_step(self.ctx, self.T, self.tau, self.state, self.lr)
+        ts.ts_pose_reduce_step(self.ctx, self.frame, self.tau, self.T, self.state, self.lr)
 
     def iteration(self):
         self.forward()
@@ -180,8 +179,7 @@ class Tracker:
                                                     self.sc.params.lambda_dep, self.gC, self.gD, self.loss)),
                 ("render_bwd", lambda: ts.ts_render_bwd(self.ctx, self.scene, self.frame, self.gC, self.gD, None, None,
                                                         None, None, ts.GRAD_POSE)),
-                ("pose_reduce", lambda: ts.ts_pose_jacobian_reduce(self.ctx, self.frame, self.tau)),
-                ("pose_step", lambda: ts.ts_pose_step(self.ctx, self.T, self.tau, self.state, self.lr))]
+                ("pose_reduce", lambda: ts.ts_pose_reduce_step(self.ctx, self.frame, self.tau, self.T, self.state, self.lr))]
 
 
 def cpu_baseline(sc, budget_iters=3):

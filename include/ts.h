@@ -120,6 +120,11 @@ int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const
 int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev, const float* lr6,
                      float beta1, float beta2, float eps, void* stream);
 
+/* a7 + a8 in one launch: as ts_pose_jacobian_reduce, then the thread that wrote dL/dtau takes the ts_pose_step on
+ * T_cw_dev / state_dev (same arguments).  dL_dtau_dev still receives the gradient. */
+int32_t ts_pose_reduce_step(ts_ctx* ctx, ts_frame* frame, float* dL_dtau_dev, float* T_cw_dev, float* state_dev,
+                            const float* lr6, float beta1, float beta2, float eps, void* stream);
+
 /* ---- read-only debug accessors (bit-exact tests) ---------------------------------------------------------- */
 enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slot order (slots are NOT in face order):
                                     f32 (u,v,w)x3, f32 mean opacity, i16 x0,y0,x1,y1, u32 face, u32 depth_key,

@@ -42,7 +42,7 @@ bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pa
     L.sorted = take(16ull * pair_cap);
     L.n_contrib = take(4ull * W * H);
     L.t_last = take(4ull * W * H);
-    L.pose_partials = take(24ull * L.n_partials_cap);
+    L.pose_partials = take(24ull * (L.n_partials_cap + 32u));
     L.total = o;
     return true;
 }
@@ -213,7 +213,13 @@ int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float
 
 int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, void* stream) {
     if (!ctx || !fr || !dL_dtau_dev) return TS_ERR_INVALID_ARG;
-    return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, (cudaStream_t)stream);
+    return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, nullptr, nullptr, nullptr, 0.f, 0.f, 0.f, (cudaStream_t)stream);
+}
+
+int32_t ts_pose_reduce_step(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, float* T_cw_dev, float* state_dev,
+                            const float* lr6, float beta1, float beta2, float eps, void* stream) {
+    if (!ctx || !fr || !dL_dtau_dev || !T_cw_dev || !state_dev || !lr6) return TS_ERR_INVALID_ARG;
+    return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, T_cw_dev, state_dev, lr6, beta1, beta2, eps, (cudaStream_t)stream);
 }
 
 int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev_ptr, size_t* count, void* stream) {

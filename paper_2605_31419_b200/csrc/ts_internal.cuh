@@ -28,7 +28,8 @@ struct TsCtrl {
     uint32_t vis_counter;    // slot allocator of the project kernel (zeroed by the sort kernel)
     uint32_t job_ticket[2];  // work queues of the forward / backward render kernels (zero at rest)
     uint32_t job_done[2];    // warps finished, per render kernel (zero at rest)
-    uint32_t pad[3];
+    uint32_t reduce_done;    // pose-reduction CTAs finished (zero at rest)
+    uint32_t pad[2];
     unsigned long long counters[8];   // debug counters (TS_PARAM_COUNTERS)
 };
 
@@ -53,7 +54,7 @@ struct TsFrameDev {
     uint4* sorted;                    // [pair_cap] sorted: (slot, face, rect_lo, rect_hi)
     uint32_t* n_contrib;              // [H*W]
     float* t_last;                    // [H*W] transmittance in front of the last contributing face
-    float* pose_partials;             // [n_partials_cap][6]
+    float* pose_partials;             // [n_partials_cap][6], then [32][6] block partials of the final reduction
     uint32_t n_partials_cap;
 };
 
@@ -102,4 +103,5 @@ int32_t ts_launch_sort(const ts_ctx*, ts_frame*, cudaStream_t);
 int32_t ts_launch_render_fwd(const ts_ctx*, ts_frame*, const ts_scene*, float*, float*, float*, cudaStream_t);
 int32_t ts_launch_render_bwd(const ts_ctx*, ts_frame*, const ts_scene*, const float*, const float*, const float*,
                              float*, float*, float*, uint32_t, cudaStream_t);
-int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame*, float*, cudaStream_t);
+int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame*, float* out, float* T_cw, float* state, const float* lr6, float beta1,
+                              float beta2, float eps, cudaStream_t);

@@ -134,7 +134,7 @@ __host__ __device__ inline int ts_sigma_mode(float sigma) {
 // ~2e-7), and for sigma < 1 dI/dx = sigma x^(sigma-1) amplifies that beyond the gradient tolerance.  There -- for
 // well under 1 % of the visited lanes -- x and lhat_k are recomputed from the raw screen vertices with the
 // compensated 2x2 determinant (N6), which is accurate to a few ulp relative, like the oracle's.
-#define TS_REFINE_BAND 4e-3f
+#define TS_REFINE_BAND 1e-3f
 
 static __device__ __noinline__ float3 ts_refine_lhat(const float4* __restrict__ s4, float px, float py) {
     const float4 s0 = __ldg(s4), s1 = __ldg(s4 + 1);

@@ -14,6 +14,7 @@
 //       [g_C ; Q x g_C], tree-reduced per CTA into fixed-order partials.
 //   pose_reduce_kernel: fixed-order final reduction of the partials to dL/dtau[6].
 #include "ts_jobs.cuh"
+#include "ts_pose.cuh"
 
 namespace {
 
@@ -324,14 +325,24 @@ proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __re
     }
 }
 
-// a7: fixed-order tree reduction of the partials
-__global__ void __launch_bounds__(1024) pose_reduce_kernel(const float* __restrict__ partials, uint32_t n, float* __restrict__ out) {
-    __shared__ float sm[32][6];
+// a7: fixed-order tree reduction of the partials.  CTA g sums a fixed contiguous slice of the partials (fixed
+// per-thread order, fixed shuffle / shared-memory tree) into block partial g; the last CTA to finish adds the block
+// partials in index order and writes dL/dtau -- the result does not depend on scheduling.  Optionally the same
+// thread then takes the Adam / Exp step on the pose (a8), which saves a launch in the tracking loop.
+constexpr int PR_THREADS = 256, PR_BLOCKS = 32;
+
+__global__ void __launch_bounds__(PR_THREADS)
+pose_reduce_kernel(TsFrameDev f, uint32_t n, float* __restrict__ out, float* __restrict__ T_cw, float* __restrict__ state,
+                   TsLr6 lr, float beta1, float beta2, float eps) {
+    __shared__ float sm[PR_THREADS / 32][6];
+    __shared__ uint32_t s_last;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t per = (n + PR_BLOCKS - 1) / PR_BLOCKS;
+    const uint32_t i0 = min(n, blockIdx.x * per), i1 = min(n, i0 + per);
     float a[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    const float2* p2 = reinterpret_cast<const float2*>(partials);
-    for (uint32_t i = tid; i < n; i += 1024) {
-        const float2 v0 = p2[3 * (size_t)i], v1 = p2[3 * (size_t)i + 1], v2 = p2[3 * (size_t)i + 2];
+    const float2* p2 = reinterpret_cast<const float2*>(f.pose_partials);
+    for (uint32_t i = i0 + tid; i < i1; i += PR_THREADS) {
+        const float2 v0 = __ldcg(p2 + 3 * (size_t)i), v1 = __ldcg(p2 + 3 * (size_t)i + 1), v2 = __ldcg(p2 + 3 * (size_t)i + 2);
         a[0] += v0.x, a[1] += v0.y, a[2] += v1.x, a[3] += v1.y, a[4] += v2.x, a[5] += v2.y;
     }
 #pragma unroll
@@ -341,11 +352,31 @@ __global__ void __launch_bounds__(1024) pose_reduce_kernel(const float* __restri
         if (lane == 0) sm[warp][j] = a[j];
     }
     __syncthreads();
+    float* blockp = f.pose_partials + 6 * (size_t)f.n_partials_cap;      // [PR_BLOCKS][6] behind the partials
     if (tid < 6) {
         float s = 0.f;
 #pragma unroll
-        for (int w = 0; w < 32; ++w) s += sm[w][tid];
+        for (int w = 0; w < PR_THREADS / 32; ++w) s += sm[w][tid];
+        __stcg(blockp + 6 * blockIdx.x + tid, s);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        s_last = (atomicAdd(&f.ctrl->reduce_done, 1u) == gridDim.x - 1) ? 1u : 0u;
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    if (tid < 6) {
+        float s = 0.f;
+        for (int g = 0; g < (int)gridDim.x; ++g) s += __ldcg(blockp + 6 * g + tid);
         out[tid] = s;
+        sm[0][tid] = s;
+    }
+    __syncthreads();
+    if (tid == 0) {
+        f.ctrl->reduce_done = 0u;
+        if (T_cw) ts_pose_step_dev(T_cw, &sm[0][0], state, lr, beta1, beta2, eps);
     }
 }
 
@@ -407,9 +438,12 @@ int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
     return TS_OK;
 }
 
-int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame* fr, float* out, cudaStream_t st) {
+int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame* fr, float* out, float* T_cw, float* state, const float* lr6,
+                              float beta1, float beta2, float eps, cudaStream_t st) {
     if (fr->pose_src == 0) return TS_ERR_STATE;
-    pose_reduce_kernel<<<1, 1024, 0, st>>>(fr->d.pose_partials, fr->n_pose_partials, out);
+    TsLr6 lr;
+    for (int i = 0; i < 6; ++i) lr.v[i] = lr6 ? lr6[i] : 0.0f;
+    pose_reduce_kernel<<<PR_BLOCKS, PR_THREADS, 0, st>>>(fr->d, fr->n_pose_partials, out, T_cw, state, lr, beta1, beta2, eps);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

@@ -18,17 +18,20 @@
 
 namespace {
 
-// exclusive scan of tile_count[0..NT) by one CTA.  offs (shared or global) receives the offsets; returns the total
-// and the longest list.  Every thread owns a contiguous run of tiles.
+// exclusive scan of tile_count[0..NT) by one CTA, in place in `offs` (shared memory, or global for the fallback).
+// Pass 1 copies the counts with coalesced loads (every binning CTA does this at the same time: strided loads would
+// multiply the L2 requests on the few slices that hold the 13 KB of counts); pass 2 gives every thread a contiguous
+// run of tiles (stride `per` words: conflict-free for odd `per`).  Returns the total and the longest list.
 __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* offs, uint32_t* s_tmp /*[2*warps+2]*/,
                                                uint32_t& total, uint32_t& gmax) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
-    const int per = (f.NT + (int)blockDim.x - 1) / (int)blockDim.x;
+    for (int t = tid; t < f.NT; t += blockDim.x) offs[t] = __ldcg(f.tile_count + t);
+    __syncthreads();
+    const int per = ((f.NT + (int)blockDim.x - 1) / (int)blockDim.x) | 1;
     const int t0 = min(f.NT, tid * per), t1 = min(f.NT, t0 + per);
     uint32_t sum = 0, mx = 0;
-#pragma unroll 4
     for (int t = t0; t < t1; ++t) {
-        const uint32_t c = __ldcg(f.tile_count + t);
+        const uint32_t c = offs[t];
         sum += c, mx = max(mx, c);
     }
     uint32_t incl = sum;
@@ -51,8 +54,9 @@ __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* of
     }
     uint32_t run = woff + incl - sum;
     for (int t = t0; t < t1; ++t) {
+        const uint32_t c = offs[t];
         offs[t] = run;
-        run += __ldcg(f.tile_count + t);
+        run += c;
     }
     __syncthreads();
 }
@@ -243,6 +247,33 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
     const uint32_t n = range.y - range.x;
     if (n == 0) return;
     const unsigned long long thi = (unsigned long long)tile << 32;
+    if (n <= 2 * TS_SORT_THREADS) {
+        // rank sort, pair data kept in registers: keys are unique (the face index is part of the key), so the
+        // ranks are a permutation
+        uint4 a[2];
+        uint32_t bb[2];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const uint32_t i = tid + k * TS_SORT_THREADS;
+            if (i < n) {
+                a[k] = f.pair_a[range.x + i], bb[k] = f.pair_b[range.x + i];
+                sk[i] = ((unsigned long long)a[k].x << 32) | a[k].y;
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            const uint32_t i = tid + k * TS_SORT_THREADS;
+            if (i < n) {
+                const unsigned long long mine = ((unsigned long long)a[k].x << 32) | a[k].y;
+                uint32_t rank = 0;
+                for (uint32_t j = 0; j < n; ++j) rank += (sk[j] < mine) ? 1u : 0u;
+                f.sorted[range.x + rank] = make_uint4(a[k].z, a[k].y, a[k].w, bb[k]);   // (slot, face, rect_lo, rect_hi)
+                f.skey[range.x + rank] = thi | a[k].x;
+            }
+        }
+        return;
+    }
     if (n <= TS_SORT_SMEM) {
         for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
             const uint4 a = f.pair_a[range.x + i];
@@ -250,16 +281,6 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
             sv[i] = i;
         }
         __syncthreads();
-        if (n <= 2 * TS_SORT_THREADS) {
-            // rank sort: keys are unique (the face index is part of the key), so ranks are a permutation
-            for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
-                const unsigned long long mine = sk[i];
-                uint32_t rank = 0;
-                for (uint32_t j = 0; j < n; ++j) rank += (sk[j] < mine) ? 1u : 0u;
-                emit_sorted(f, range.x, rank, i, thi);
-            }
-            return;
-        }
         cta_sort_network(sk, sv, n);
         for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) emit_sorted(f, range.x, i, sv[i], thi);
         return;
@@ -282,7 +303,7 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
 int32_t ts_launch_sort(const ts_ctx* ctx, ts_frame* fr, cudaStream_t stream) {
     const TsFrameDev& f = fr->d;
     const uint32_t grid_bin = (uint32_t)min((uint64_t)(f.vis_cap + TS_BIN_THREADS - 1) / TS_BIN_THREADS,
-                                            (uint64_t)ctx->num_sms * 4u);
+                                            (uint64_t)ctx->num_sms * 2u);
     const bool soup = fr->scene.faces == nullptr;
     if (f.NT <= TS_SCAN_LOCAL_MAX) {
         if (soup) bin_setup_kernel<true, true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, nullptr);

@@ -25,7 +25,7 @@ _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.
 
 EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_bwd",
-           "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_pose_step", "ts_frame_view"]
+           "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view"]
 
 
 class TsError(RuntimeError):
@@ -71,6 +71,8 @@ def _load():
                                     C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_pose_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_float), C.c_float,
                                  C.c_float, C.c_float, C.c_void_p]
+    lib.ts_pose_reduce_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_float),
+                                        C.c_float, C.c_float, C.c_float, C.c_void_p]
     lib.ts_frame_status.argtypes = [C.c_void_p, C.c_void_p, C.POINTER(C.c_uint32), C.POINTER(C.c_uint32),
                                     C.POINTER(C.c_uint64), C.c_void_p]
     lib.ts_frame_view.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t),
@@ -185,6 +187,12 @@ def ts_l1_loss_grad(ctx, W, H, Cimg, Dimg, Chat, Dhat, lambda_dep, gC, gD, loss=
 def ts_pose_step(ctx, T_cw, dL_dtau, state, lr6, beta1=0.9, beta2=0.999, eps=1e-8, stream=None):
     lr = (C.c_float * 6)(*[float(x) for x in lr6])
     _check(lib.ts_pose_step(ctx.h, _ptr(T_cw), _ptr(dL_dtau), _ptr(state), lr, beta1, beta2, eps, _stream(stream)))
+
+
+def ts_pose_reduce_step(ctx, frame, dL_dtau, T_cw, state, lr6, beta1=0.9, beta2=0.999, eps=1e-8, stream=None):
+    lr = (C.c_float * 6)(*[float(x) for x in lr6])
+    _check(lib.ts_pose_reduce_step(ctx.h, frame.h, _ptr(dL_dtau), _ptr(T_cw), _ptr(state), lr, beta1, beta2, eps,
+                                   _stream(stream)))
 
 
 def ts_frame_status(ctx, frame, stream=None, check=True):

@@ -173,3 +173,30 @@ def test_pose_step_matches_oracle(ctx, oracle_mod):
         ts.ts_pose_step(ctx, Td, dev(gvec), sd, lr)
         assert np.allclose(Td.cpu().numpy().reshape(3, 4), T, atol=2e-6)
         assert np.allclose(sd.cpu().numpy(), state, rtol=1e-5, atol=1e-7)
+
+
+def test_pose_reduce_step_equals_separate_calls(ctx, oracle_mod):
+    """ts_pose_reduce_step (a7 + a8 fused) gives the same gradient and the same updated pose as the two calls."""
+    from gpu_util import dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(1)
+    o, g = both(ctx, oracle_mod, sc)
+    C, D, A = g.forward()
+    rng = np.random.default_rng(11)
+    gC, gD = dev(rng.normal(size=C.shape).astype(np.float32)), dev(rng.normal(size=D.shape).astype(np.float32))
+    lr = [1e-3] * 3 + [3e-3] * 3
+    res = []
+    for fused in (False, True):
+        T, st, tau = g.T.clone(), torch.zeros(13, device="cuda"), torch.zeros(6, device="cuda")
+        ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, None, None, None, ts.GRAD_POSE)
+        if fused:
+            ts.ts_pose_reduce_step(ctx, g.frame, tau, T, st, lr)
+        else:
+            ts.ts_pose_jacobian_reduce(ctx, g.frame, tau)
+            ts.ts_pose_step(ctx, T, tau, st, lr)
+        torch.cuda.synchronize()
+        res.append((tau.cpu().numpy(), T.cpu().numpy(), st.cpu().numpy()))
+    for a, b in zip(*res):
+        assert np.array_equal(a, b)
+    assert np.abs(res[0][0]).max() > 0
+    g.close()
