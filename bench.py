@@ -302,20 +302,33 @@ def main():
     frame_ms = a.elapsed_time(b)
     loss_after = None
 
-    # per-stage device times (eager launches, events between the calls; flush between steps)
+    # per-stage device times: every stage captured into its own CUDA graph (so that host launch overhead does not
+    # leak into the numbers), events between the graph launches; flush between steps
+    tr.reset()
+    stage_graphs = []
+    with torch.cuda.stream(stream):
+        for name, fn in tr.stages():
+            if args.no_graph:
+                stage_graphs.append((name, fn))
+            else:
+                gr = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gr, stream=stream):
+                    fn()
+                stage_graphs.append((name, gr.replay))
     tr.reset()
     stage_ms = {}
     with torch.cuda.stream(stream):
         for it in range(args.steps):
             flush.fill_(1)
-            for name, fn in tr.stages():
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record(stream)
+            evs = [torch.cuda.Event(enable_timing=True) for _ in range(len(stage_graphs) + 1)]
+            evs[0].record(stream)
+            for i, (name, fn) in enumerate(stage_graphs):
                 fn()
-                e1.record(stream)
-                stage_ms.setdefault(name, []).append((e0, e1))
+                evs[i + 1].record(stream)
+            for i, (name, fn) in enumerate(stage_graphs):
+                stage_ms.setdefault(name, []).append((evs[i], evs[i + 1]))
     stream.synchronize()
-    stage_ms = {k: float(np.mean([a.elapsed_time(b) for a, b in v])) for k, v in stage_ms.items()}
+    stage_ms = {k: float(np.median([a.elapsed_time(b) for a, b in v])) for k, v in stage_ms.items()}
     clocks = clk.stop()
 
     # e2e: same iteration through the C ABI with HOST buffers: the frame's target RGB-D (pinned) and the pose go

@@ -42,7 +42,7 @@ l1_loss_grad_kernel(size_t n, const float* __restrict__ C, const float* __restri
 
 __global__ void pose_step_kernel(float* __restrict__ T, const float* __restrict__ g, float* __restrict__ state, TsLr6 lr,
                                  float beta1, float beta2, float eps) {
-    if (threadIdx.x == 0) ts_pose_step_dev(T, g, state, lr, beta1, beta2, eps);
+    ts_pose_step_warp(T, g, state, lr, beta1, beta2, eps);   // launched with exactly one warp
 }
 
 }  // namespace

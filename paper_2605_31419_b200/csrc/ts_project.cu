@@ -58,7 +58,8 @@ __device__ __forceinline__ void project_face(const float* p, const float* T, con
 template <bool SOUP>
 __global__ void __launch_bounds__(TS_PROJ_THREADS)
 project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __restrict__ faces,
-               const float* __restrict__ Tcw, TsCamDev cam, float eps_area, int pos_aligned) {
+               const float* __restrict__ opacity, const float* __restrict__ Tcw, TsCamDev cam, float eps_area,
+               int pos_aligned) {
     __shared__ __align__(16) float sp[TS_PROJ_THREADS * 9];
     __shared__ float sT[12];
     __shared__ uint32_t s_w[TS_PROJ_THREADS / 32];
@@ -119,11 +120,19 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
         const uint32_t slot = s_base + s_w[warp] + __popc(bal & ((1u << lane) - 1u));
         if (slot < f.vis_cap) {
             const uint32_t m = (uint32_t)(face0 + tid);
+            float ob;                                            // mean vertex opacity
+            if (SOUP) {
+                ob = (__ldg(opacity + 3 * (int64_t)m) + __ldg(opacity + 3 * (int64_t)m + 1) +
+                      __ldg(opacity + 3 * (int64_t)m + 2)) * (1.0f / 3.0f);
+            } else {
+                ob = (__ldg(opacity + __ldg(faces + 3 * (int64_t)m)) + __ldg(opacity + __ldg(faces + 3 * (int64_t)m + 1)) +
+                      __ldg(opacity + __ldg(faces + 3 * (int64_t)m + 2))) * (1.0f / 3.0f);
+            }
             const int rlo = (o.x0 & 0xffff) | (o.y0 << 16), rhi = (o.x1 & 0xffff) | (o.y1 << 16);
             float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
             s4[0] = make_float4(o.u[0], o.v[0], o.w[0], o.u[1]);
             s4[1] = make_float4(o.v[1], o.w[1], o.u[2], o.v[2]);
-            s4[2] = make_float4(o.w[2], 0.0f, __int_as_float(rlo), __int_as_float(rhi));   // .y = mean opacity, set by the binning kernel
+            s4[2] = make_float4(o.w[2], ob, __int_as_float(rlo), __int_as_float(rhi));
             s4[3] = make_float4(__uint_as_float(m), __uint_as_float(o.key), __uint_as_float(o.tiles), 0.0f);
             for (int ty = o.y0 >> 4; ty <= (o.y1 >> 4); ++ty)
                 for (int tx = o.x0 >> 4; tx <= (o.x1 >> 4); ++tx) atomicAdd(f.tile_count + ty * f.tiles_x + tx, 1u);
@@ -140,11 +149,11 @@ int32_t ts_launch_project(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, c
     const int aligned = ((reinterpret_cast<uintptr_t>(sc->pos) & 15u) == 0) ? 1 : 0;
     const uint32_t grid = (uint32_t)((f.M + TS_PROJ_THREADS - 1) / TS_PROJ_THREADS);
     if (sc->faces == nullptr)
-        project_kernel<true><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, nullptr, fr->T_cw, fr->cam, fr->prm.eps_area,
-                                                                   aligned);
+        project_kernel<true><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, nullptr, sc->opacity, fr->T_cw, fr->cam,
+                                                                   fr->prm.eps_area, aligned);
     else
-        project_kernel<false><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, sc->faces, fr->T_cw, fr->cam,
-                                                                    fr->prm.eps_area, aligned);
+        project_kernel<false><<<grid, TS_PROJ_THREADS, 0, stream>>>(f, sc->pos, sc->faces, sc->opacity, fr->T_cw,
+                                                                    fr->cam, fr->prm.eps_area, aligned);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

@@ -341,9 +341,17 @@ pose_reduce_kernel(TsFrameDev f, uint32_t n, float* __restrict__ out, float* __r
     const uint32_t i0 = min(n, blockIdx.x * per), i1 = min(n, i0 + per);
     float a[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     const float2* p2 = reinterpret_cast<const float2*>(f.pose_partials);
-    for (uint32_t i = i0 + tid; i < i1; i += PR_THREADS) {
-        const float2 v0 = __ldcg(p2 + 3 * (size_t)i), v1 = __ldcg(p2 + 3 * (size_t)i + 1), v2 = __ldcg(p2 + 3 * (size_t)i + 2);
-        a[0] += v0.x, a[1] += v0.y, a[2] += v1.x, a[3] += v1.y, a[4] += v2.x, a[5] += v2.y;
+    for (uint32_t ib = i0; ib < i1; ib += 4 * PR_THREADS) {              // 12 independent loads in flight per thread
+        float2 v[4][3];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const uint32_t i = ib + k * PR_THREADS + tid;
+#pragma unroll
+            for (int q = 0; q < 3; ++q) v[k][q] = i < i1 ? __ldcg(p2 + 3 * (size_t)i + q) : make_float2(0.f, 0.f);
+        }
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+            a[0] += v[k][0].x, a[1] += v[k][0].y, a[2] += v[k][1].x, a[3] += v[k][1].y, a[4] += v[k][2].x, a[5] += v[k][2].y;
     }
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
@@ -367,17 +375,18 @@ pose_reduce_kernel(TsFrameDev f, uint32_t n, float* __restrict__ out, float* __r
     __syncthreads();
     if (!s_last) return;
     __threadfence();
+    __shared__ float sb[PR_BLOCKS * 6];
+    if (tid < (int)gridDim.x * 6) sb[tid] = __ldcg(blockp + tid);       // all block partials in one round trip
+    __syncthreads();
     if (tid < 6) {
         float s = 0.f;
-        for (int g = 0; g < (int)gridDim.x; ++g) s += __ldcg(blockp + 6 * g + tid);
+        for (int g = 0; g < (int)gridDim.x; ++g) s += sb[6 * g + tid];
         out[tid] = s;
         sm[0][tid] = s;
     }
     __syncthreads();
-    if (tid == 0) {
-        f.ctrl->reduce_done = 0u;
-        if (T_cw) ts_pose_step_dev(T_cw, &sm[0][0], state, lr, beta1, beta2, eps);
-    }
+    if (tid == 0) f.ctrl->reduce_done = 0u;
+    if (T_cw && tid < 32) ts_pose_step_warp(T_cw, &sm[0][0], state, lr, beta1, beta2, eps);
 }
 
 template <int SM, bool ATTR, bool GEOM, bool POSE>

@@ -25,7 +25,19 @@ namespace {
 __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* offs, uint32_t* s_tmp /*[2*warps+2]*/,
                                                uint32_t& total, uint32_t& gmax) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
-    for (int t = tid; t < f.NT; t += blockDim.x) offs[t] = __ldcg(f.tile_count + t);
+    for (int base = 0; base < f.NT; base += 8 * (int)blockDim.x) {      // 8 independent loads in flight per thread
+        uint32_t c[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int t = base + k * (int)blockDim.x + tid;
+            c[k] = t < f.NT ? __ldcg(f.tile_count + t) : 0u;
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            const int t = base + k * (int)blockDim.x + tid;
+            if (t < f.NT) offs[t] = c[k];
+        }
+    }
     __syncthreads();
     const int per = ((f.NT + (int)blockDim.x - 1) / (int)blockDim.x) | 1;
     const int t0 = min(f.NT, tid * per), t1 = min(f.NT, t0 + per);
@@ -62,15 +74,15 @@ __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* of
 }
 
 // CTA 0 only: tile_ranges, frame counters, and the tile order (descending log2 bucket of the list length) that
-// the persistent render kernels pull work in
+// the persistent render kernels pull work in.  Counts are recovered from the offsets (no second trip to memory).
 __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_t* offs, uint32_t nv, uint32_t total,
                                               uint32_t gmax, uint32_t fl, uint32_t* s_hist /*[34]*/) {
     const int tid = threadIdx.x;
     if (tid < 34) s_hist[tid] = 0;
     __syncthreads();
     for (int t = tid; t < f.NT; t += blockDim.x) {
-        const uint32_t c = __ldcg(f.tile_count + t);
-        f.tile_ranges[t] = (fl || c == 0u) ? make_uint2(0u, 0u) : make_uint2(offs[t], offs[t] + c);   // empty tile = (0,0)
+        const uint32_t o = offs[t], c = (t + 1 < f.NT ? offs[t + 1] : total) - o;
+        f.tile_ranges[t] = (fl || c == 0u) ? make_uint2(0u, 0u) : make_uint2(o, o + c);   // empty tile = (0,0)
         atomicAdd(&s_hist[32 - __clz(c)], 1u);                 // bucket 0 = empty, b = floor(log2 c) + 1
     }
     __syncthreads();
@@ -86,7 +98,7 @@ __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_
     }
     __syncthreads();
     for (int t = tid; t < f.NT; t += blockDim.x) {
-        const uint32_t c = __ldcg(f.tile_count + t);
+        const uint32_t c = (t + 1 < f.NT ? offs[t + 1] : total) - offs[t];
         f.tile_order[atomicAdd(&s_hist[32 - __clz(c)], 1u)] = (uint32_t)t;
     }
 }
@@ -104,23 +116,33 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(TsFrameDev f) {
     publish_tiles(f, f.tile_offset, nv, total, gmax, fl, s_hist);
 }
 
-template <bool LOCAL, bool SOUP>
+template <bool LOCAL>
 __global__ void __launch_bounds__(TS_BIN_THREADS)
-bin_setup_kernel(TsFrameDev f, TsCamDev cam, const float* __restrict__ opacity, const int32_t* __restrict__ faces) {
+bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
     __shared__ uint32_t s_offs[LOCAL ? TS_SCAN_LOCAL_MAX : 1];
     __shared__ uint32_t s_tmp[2 * (TS_BIN_THREADS / 32) + 2];
     __shared__ uint32_t s_hist[34];
     const int lane = threadIdx.x & 31;
+    // This kernel is one wave of dependent round trips, so they are kept few: the raw records of this thread's
+    // first slot are requested before anything else (speculatively: slot < n_visible is not known yet) and fly
+    // while the CTA scans the tile counts.
+    uint32_t slot = blockIdx.x * TS_BIN_THREADS + threadIdx.x;
+    float4 s0, s1, s2, s3;
+    s0 = s1 = s2 = s3 = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (slot < f.vis_cap) {
+        const float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
+        s0 = __ldcg(s4), s1 = __ldcg(s4 + 1), s2 = __ldcg(s4 + 2), s3 = __ldcg(s4 + 3);
+    }
     uint32_t nv, fl;
     const uint32_t* offs;
     if (LOCAL) {
         uint32_t total, gmax;
+        nv = __ldcg(&f.ctrl->vis_counter);
         cta_scan_tiles(f, s_offs, s_tmp, total, gmax);
-        nv = *(volatile uint32_t*)&f.ctrl->vis_counter;
         fl = 0;
         if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
         if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
-        if (blockIdx.x == 0) publish_tiles(f, s_offs, nv, total, gmax, fl, s_hist);
+        if (blockIdx.x == gridDim.x - 1) publish_tiles(f, s_offs, nv, total, gmax, fl, s_hist);   // the last CTA has the fewest slots
         offs = s_offs;
     } else {
         const volatile TsCtrl* ctrl = f.ctrl;
@@ -129,60 +151,82 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam, const float* __restrict__ opacity, 
     }
     const uint32_t nvis = fl ? 0u : nv;
     const uint32_t n_round = (nvis + TS_BIN_THREADS - 1) / TS_BIN_THREADS * TS_BIN_THREADS;
-    for (uint32_t slot = blockIdx.x * TS_BIN_THREADS + threadIdx.x; slot < n_round; slot += gridDim.x * TS_BIN_THREADS) {
+    while (slot < n_round) {
         const bool live = slot < nvis;
         int tx0 = 0, ty0 = 0, ntx = 0, nty = 0;
         uint4 pa = make_uint4(0u, 0u, slot, 0u);
         uint32_t pb = 0;
         if (live) {
-            float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
-            const float4 s0 = s4[0], s1 = s4[1], s2 = s4[2], s3 = s4[3];
-            const uint32_t m = __float_as_uint(s3.x);
-            float ob;                                            // mean vertex opacity
-            if (SOUP) {
-                ob = (__ldg(opacity + 3 * (size_t)m) + __ldg(opacity + 3 * (size_t)m + 1) + __ldg(opacity + 3 * (size_t)m + 2)) *
-                     (1.0f / 3.0f);
-            } else {
-                ob = (__ldg(opacity + __ldg(faces + 3 * (size_t)m)) + __ldg(opacity + __ldg(faces + 3 * (size_t)m + 1)) +
-                      __ldg(opacity + __ldg(faces + 3 * (size_t)m + 2))) * (1.0f / 3.0f);
-            }
             float4 rec[TS_REC_F4];
-            ts_build_record(s0, s1, s2, ob, cam, rec);
+            ts_build_record(s0, s1, s2, s2.y, cam, rec);
             float4* out = f.rec + TS_REC_F4 * (size_t)slot;
 #pragma unroll
             for (int i = 0; i < TS_REC_F4; ++i) out[i] = rec[i];
-            s4[2] = make_float4(s2.x, ob, s2.z, s2.w);
             const int rlo = __float_as_int(s2.z), rhi = __float_as_int(s2.w);
             const int x0 = (int)(short)(rlo & 0xffff), y0 = rlo >> 16, x1 = (int)(short)(rhi & 0xffff), y1 = rhi >> 16;
             tx0 = x0 >> 4, ty0 = y0 >> 4, ntx = (x1 >> 4) - tx0 + 1, nty = (y1 >> 4) - ty0 + 1;
-            pa = make_uint4(__float_as_uint(s3.y), m, slot, (uint32_t)rlo);
+            pa = make_uint4(__float_as_uint(s3.y), __float_as_uint(s3.x), slot, (uint32_t)rlo);
             pb = (uint32_t)rhi;
         }
         const int nt = ntx * nty;
-        // narrow faces (the common case): the owning lane scatters its <= 4 pairs itself
-        if (nt <= 4) {
-            for (int i = 0; i < nt; ++i) {
-                const int t = (ty0 + i / ntx) * f.tiles_x + tx0 + i % ntx;
-                const uint32_t pos = offs[t] + atomicAdd(f.tile_cursor + t, 1u);
-                if (pos < f.pair_cap) f.pair_a[pos] = pa, f.pair_b[pos] = pb;
+        // narrow faces (the common case): the owning lane scatters its <= 4 pairs itself; the cursor atomics are
+        // issued together so that they cost one round trip, not four
+        {
+            int tt[4];
+            uint32_t pos[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                tt[i] = (ty0 + i / max(ntx, 1)) * f.tiles_x + tx0 + i % max(ntx, 1);
+                pos[i] = 0;
+                if (nt <= 4 && i < nt) pos[i] = atomicAdd(f.tile_cursor + tt[i], 1u);
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                if (nt <= 4 && i < nt) {
+                    const uint32_t q = offs[tt[i]] + pos[i];
+                    if (q < f.pair_cap) f.pair_a[q] = pa, f.pair_b[q] = pb;
+                }
             }
         }
-        // wide faces: the whole warp scatters one face's tiles together
-        uint32_t wide = __ballot_sync(0xffffffffu, nt > 4);
-        while (wide) {
-            const int src = __ffs(wide) - 1;
-            wide &= wide - 1;
-            const int btx0 = __shfl_sync(0xffffffffu, tx0, src), bty0 = __shfl_sync(0xffffffffu, ty0, src);
-            const int bntx = __shfl_sync(0xffffffffu, ntx, src), bnt = __shfl_sync(0xffffffffu, nt, src);
-            uint4 ba;
-            ba.x = __shfl_sync(0xffffffffu, pa.x, src), ba.y = __shfl_sync(0xffffffffu, pa.y, src);
-            ba.z = __shfl_sync(0xffffffffu, pa.z, src), ba.w = __shfl_sync(0xffffffffu, pa.w, src);
-            const uint32_t bb = __shfl_sync(0xffffffffu, pb, src);
-            for (int i = lane; i < bnt; i += 32) {
-                const int t = (bty0 + i / bntx) * f.tiles_x + btx0 + i % bntx;
-                const uint32_t pos = offs[t] + atomicAdd(f.tile_cursor + t, 1u);
-                if (pos < f.pair_cap) f.pair_a[pos] = ba, f.pair_b[pos] = bb;
+        // wide faces: their (face, tile) pairs are flattened over the warp, 32 pairs per round trip
+        const uint32_t wnt = nt > 4 ? (uint32_t)nt : 0u;
+        if (__any_sync(0xffffffffu, wnt != 0u)) {
+            uint32_t incl = wnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
             }
+            const uint32_t W = __shfl_sync(0xffffffffu, incl, 31);
+            for (uint32_t p0 = 0; p0 < W; p0 += 32) {
+                const uint32_t p = p0 + lane;
+                int lo = 0, hi = 31;                            // owner = first lane whose inclusive prefix exceeds p
+#pragma unroll
+                for (int it = 0; it < 5; ++it) {
+                    const int mid = (lo + hi) >> 1;
+                    const uint32_t v = __shfl_sync(0xffffffffu, incl, mid);
+                    if (v <= p) lo = mid + 1; else hi = mid;
+                }
+                const int own = lo & 31;
+                const uint32_t o_incl = __shfl_sync(0xffffffffu, incl, own), o_nt = __shfl_sync(0xffffffffu, wnt, own);
+                const int btx0 = __shfl_sync(0xffffffffu, tx0, own), bty0 = __shfl_sync(0xffffffffu, ty0, own);
+                const int bntx = __shfl_sync(0xffffffffu, ntx, own);
+                uint4 ba;
+                ba.x = __shfl_sync(0xffffffffu, pa.x, own), ba.y = __shfl_sync(0xffffffffu, pa.y, own);
+                ba.z = __shfl_sync(0xffffffffu, pa.z, own), ba.w = __shfl_sync(0xffffffffu, pa.w, own);
+                const uint32_t bb = __shfl_sync(0xffffffffu, pb, own);
+                if (p < W) {
+                    const int i = (int)(p - (o_incl - o_nt));
+                    const int t = (bty0 + i / bntx) * f.tiles_x + btx0 + i % bntx;
+                    const uint32_t q = offs[t] + atomicAdd(f.tile_cursor + t, 1u);
+                    if (q < f.pair_cap) f.pair_a[q] = ba, f.pair_b[q] = bb;
+                }
+            }
+        }
+        slot += gridDim.x * TS_BIN_THREADS;
+        if (slot < nvis) {
+            const float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
+            s0 = __ldcg(s4), s1 = __ldcg(s4 + 1), s2 = __ldcg(s4 + 2), s3 = __ldcg(s4 + 3);
         }
     }
 }
@@ -303,15 +347,12 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
 int32_t ts_launch_sort(const ts_ctx* ctx, ts_frame* fr, cudaStream_t stream) {
     const TsFrameDev& f = fr->d;
     const uint32_t grid_bin = (uint32_t)min((uint64_t)(f.vis_cap + TS_BIN_THREADS - 1) / TS_BIN_THREADS,
-                                            (uint64_t)ctx->num_sms * 2u);
-    const bool soup = fr->scene.faces == nullptr;
+                                            (uint64_t)ctx->num_sms * 4u);
     if (f.NT <= TS_SCAN_LOCAL_MAX) {
-        if (soup) bin_setup_kernel<true, true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, nullptr);
-        else bin_setup_kernel<true, false><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, fr->scene.faces);
+        bin_setup_kernel<true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam);
     } else {
         tile_scan_kernel<<<1, 1024, 0, stream>>>(f);
-        if (soup) bin_setup_kernel<false, true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, nullptr);
-        else bin_setup_kernel<false, false><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->scene.opacity, fr->scene.faces);
+        bin_setup_kernel<false><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam);
     }
     tile_sort_kernel<<<f.NT, TS_SORT_THREADS, 0, stream>>>(f, f.big_key, f.big_idx);
     TS_CUDA_CHECK_LAUNCH();
