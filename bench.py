@@ -3,7 +3,8 @@
 "fwd+bwd render Mpix/s @1200x680, 500k tris; tracking iters/s; % of roofline").
 
 A step = ONE tracking iteration on BASELINE.json configs[2] (Replica-shaped, 1200x680, 500k faces, seed 2):
-ts_project -> ts_bin_sort -> ts_render_fwd -> ts_l1_loss_grad -> ts_render_bwd(pose-only) ->
+ts_project -> ts_bin_sort -> ts_render_fwd_l1 (= ts_render_fwd + ts_l1_loss_grad in one launch; C, D, A are still
+written) -> ts_render_bwd(pose-only) ->
 ts_pose_reduce_step (= ts_pose_jacobian_reduce + ts_pose_step in one launch), i.e. every row a1..a8 of DESIGN.md section 2, on synthetic data.
 L2 is flushed between timed steps (the 18 MB map would otherwise stay L2-resident across iterations); the extra
 "tracking_iters_per_s" figure is the 100-iteration block of one frame WITHOUT flushes (the real tracking loop).
@@ -146,18 +147,17 @@ class Tracker:
         ts.ts_render_fwd(self.ctx, self.scene, self.frame, self.Chat, self.Dhat, None)
         torch.cuda.synchronize()
 
-    launches_per_iter = 1 + 2 + 1 + 1 + 1 + 1   # project, bin + sort, fwd, loss, bwd, reduce+step
+    launches_per_iter = 1 + 2 + 1 + 1 + 1   # project, bin + sort, fwd+loss, bwd, reduce+step
 
     def forward(self):
         ts = self.ts
         ts.ts_project(self.ctx, self.scene, self.cam, self.prm, self.T, self.frame)
         ts.ts_bin_sort(self.ctx, self.frame)
-        ts.ts_render_fwd(self.ctx, self.scene, self.frame, self.C, self.D, self.A)
+        ts.ts_render_fwd_l1(self.ctx, self.scene, self.frame, self.C, self.D, self.A, self.Chat, self.Dhat,
+                            self.sc.params.lambda_dep, self.gC, self.gD, self.loss)
 
     def backward(self):
         ts = self.ts
-        ts.ts_l1_loss_grad(self.ctx, self.W, self.H, self.C, self.D, self.Chat, self.Dhat, self.sc.params.lambda_dep,
-                           self.gC, self.gD, self.loss)
         ts.ts_render_bwd(self.ctx, self.scene, self.frame, self.gC, self.gD, None, None, None, None, ts.GRAD_POSE)
         ts.ts_pose_reduce_step(self.ctx, self.frame, self.tau, self.T, self.state, self.lr)
 
@@ -174,9 +174,8 @@ class Tracker:
         ts = self.ts
         return [("project", lambda: ts.ts_project(self.ctx, self.scene, self.cam, self.prm, self.T, self.frame)),
                 ("bin_sort", lambda: ts.ts_bin_sort(self.ctx, self.frame)),
-                ("render_fwd", lambda: ts.ts_render_fwd(self.ctx, self.scene, self.frame, self.C, self.D, self.A)),
-                ("loss", lambda: ts.ts_l1_loss_grad(self.ctx, self.W, self.H, self.C, self.D, self.Chat, self.Dhat,
-                                                    self.sc.params.lambda_dep, self.gC, self.gD, self.loss)),
+                ("render_fwd", lambda: ts.ts_render_fwd_l1(self.ctx, self.scene, self.frame, self.C, self.D, self.A, self.Chat,
+                                                           self.Dhat, self.sc.params.lambda_dep, self.gC, self.gD, self.loss)),
                 ("render_bwd", lambda: ts.ts_render_bwd(self.ctx, self.scene, self.frame, self.gC, self.gD, None, None,
                                                         None, None, ts.GRAD_POSE)),
                 ("pose_reduce", lambda: ts.ts_pose_reduce_step(self.ctx, self.frame, self.tau, self.T, self.state, self.lr))]

@@ -115,6 +115,12 @@ int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* frame, float* dL_dtau_dev
  * cotangent images gC[3][H][W], gD[H][W] and, if loss_dev != NULL, adds L to *loss_dev (caller zeroes). */
 int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* D, const float* Chat,
                         const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev, void* stream);
+/* a3 + a4 in one launch: ts_render_fwd, with the L1 colour + depth loss of ts_l1_loss_grad evaluated on every pixel
+ * while its value is still in registers: writes gC, gD (and adds L to *loss_dev if not NULL) exactly as
+ * ts_l1_loss_grad would.  out_color / out_depth / out_alpha may be NULL (a tracking loop never reads them). */
+int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
+                         float* out_alpha, const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD,
+                         float* loss_dev, void* stream);
 /* a8: one Adam step on tau, then T_cw <- Exp(-delta) o T_cw, all on the device.
  * state_dev[13] = m[6], v[6], step; lr[6] passed by value (rho then theta). */
 int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev, const float* lr6,

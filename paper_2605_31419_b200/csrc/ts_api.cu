@@ -192,7 +192,20 @@ int32_t ts_render_fwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_
     if (!ctx || !sc || !fr || !sc->color) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
-    const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, (cudaStream_t)stream);
+    const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, nullptr, nullptr, 0.f, nullptr, nullptr,
+                                           nullptr, (cudaStream_t)stream);
+    fr->have_fwd = (s == TS_OK);
+    return s;
+}
+
+int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth, float* out_alpha,
+                         const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
+                         void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !Chat || !Dhat || !gC || !gD) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if (!fr->have_sort) return TS_ERR_STATE;
+    const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev,
+                                           (cudaStream_t)stream);
     fr->have_fwd = (s == TS_OK);
     return s;
 }

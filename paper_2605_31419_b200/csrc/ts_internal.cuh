@@ -8,7 +8,7 @@
 
 #define TS_TILE 16
 #define TS_PROJ_THREADS 256          // faces per project CTA
-#define TS_BIN_THREADS 256           // visible slots per bin/setup CTA iteration
+#define TS_BIN_THREADS 1024          // visible slots per bin/setup CTA iteration (one CTA per SM: one tile scan per SM)
 #define TS_SCAN_LOCAL_MAX 4096       // up to this many tiles every binning CTA scans the tile counts itself (smem)
 #define TS_SORT_THREADS 128
 #define TS_SORT_SMEM 2048            // tile lists up to this length are sorted in shared memory
@@ -100,7 +100,8 @@ __device__ __forceinline__ uint32_t ts_eff_visible(const TsFrameDev& f) {
 // launchers (one per .cu)
 int32_t ts_launch_project(const ts_ctx*, ts_frame*, const ts_scene*, cudaStream_t);
 int32_t ts_launch_sort(const ts_ctx*, ts_frame*, cudaStream_t);
-int32_t ts_launch_render_fwd(const ts_ctx*, ts_frame*, const ts_scene*, float*, float*, float*, cudaStream_t);
+int32_t ts_launch_render_fwd(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
+                             const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, cudaStream_t);
 int32_t ts_launch_render_bwd(const ts_ctx*, ts_frame*, const ts_scene*, const float*, const float*, const float*,
                              float*, float*, float*, uint32_t, cudaStream_t);
 int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame*, float* out, float* T_cw, float* state, const float* lr6, float beta1,

@@ -36,6 +36,11 @@ __device__ __forceinline__ float ts_sqrt_approx(float x) {
     asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
+__device__ __forceinline__ float ts_rsqrt_approx(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
 __device__ __forceinline__ float ts_rcp_approx(float x) {
     float y;
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -53,21 +58,25 @@ __device__ __forceinline__ void ts_face_geom(const float4 s0, const float4 s1, c
     const float S = __fmaf_rn(a, b, -__fmul_rn(c, d));
     g.sgn = S > 0.0f ? 1.0f : -1.0f;
     g.absS = fabsf(S);
+    // The record only has to be the same for the forward and the backward kernel (it is: both read it), not
+    // correctly rounded: lengths and reciprocals use the MUFU approximations (<= 2 ulp), which keeps this
+    // latency-bound set-up chain short.  Decisions next to an edge never depend on it (ts_refine_lhat).
     float sum = 0.0f;
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         const int ia = (k + 1) % 3, ib = (k + 2) % 3;
         const float ex = __fsub_rn(g.qx[ib], g.qx[ia]), ey = __fsub_rn(g.qy[ib], g.qy[ia]);
-        g.ell[k] = __fsqrt_rn(__fmaf_rn(ex, ex, __fmul_rn(ey, ey)));
-        g.inv_ell[k] = __frcp_rn(g.ell[k]);
+        const float l2 = __fmaf_rn(ex, ex, __fmul_rn(ey, ey));
+        g.inv_ell[k] = ts_rsqrt_approx(l2);
+        g.ell[k] = __fmul_rn(l2, g.inv_ell[k]);
         g.nx[k] = __fmul_rn(__fmul_rn(g.sgn, ey), g.inv_ell[k]);
         g.ny[k] = -__fmul_rn(__fmul_rn(g.sgn, ex), g.inv_ell[k]);
         sum = __fadd_rn(sum, g.ell[k]);
     }
     g.sumell = sum;
-    g.inv_sumell = __frcp_rn(sum);
+    g.inv_sumell = ts_rcp_approx(sum);
     g.r = __fmul_rn(g.absS, g.inv_sumell);
-    g.inv_r = __fdiv_rn(sum, g.absS);
+    g.inv_r = __fmul_rn(sum, ts_rcp_approx(g.absS));
     // reference point: incentre = sum(ell_k q_k) / sum(ell) (ell_k is the edge opposite vertex k), float-rounded
     g.refx = __fmul_rn(__fmaf_rn(g.ell[0], g.qx[0], __fmaf_rn(g.ell[1], g.qx[1], __fmul_rn(g.ell[2], g.qx[2]))), g.inv_sumell);
     g.refy = __fmul_rn(__fmaf_rn(g.ell[0], g.qy[0], __fmaf_rn(g.ell[1], g.qy[1], __fmul_rn(g.ell[2], g.qy[2]))), g.inv_sumell);
@@ -93,7 +102,7 @@ __device__ __forceinline__ void ts_build_record(const float4 s0, const float4 s1
     // stored as drr_j = -(1/r) dr/dq_j so that gq_j += (x * gx) * drr_j  (B6 iii)
     float drrx[3], drry[3], tau[3], xn[3], yn[3];
     const float rs = g.r * g.inv_sumell;
-    const float ifx = 1.0f / cam.fx, ify = 1.0f / cam.fy;
+    const float ifx = ts_rcp_approx(cam.fx), ify = ts_rcp_approx(cam.fy);
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
         const int i1 = (j + 1) % 3, i2 = (j + 2) % 3;

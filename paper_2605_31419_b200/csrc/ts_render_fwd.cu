@@ -16,10 +16,21 @@ struct FwdWarpSmem {
     uint32_t pos[32];                 // 1 + position of the entry in the tile list
 };
 
-template <int SM, bool COUNT>
+// optional fused a4: L1 colour + depth loss against a target frame, evaluated on the pixel values while they are
+// still in registers (Eq. 8-10 without D-SSIM; same arithmetic as l1_loss_grad_kernel in ts_helpers.cu)
+struct FwdLoss {
+    const float* Chat;
+    const float* Dhat;
+    float* gC;
+    float* gD;
+    float* loss;
+    float wc, wd;
+};
+
+template <int SM, bool COUNT, bool LOSS>
 __global__ void __launch_bounds__(TS_JOB_WARPS * 32)
 render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float t_min, float* __restrict__ out_color,
-                  float* __restrict__ out_depth, float* __restrict__ out_alpha) {
+                  float* __restrict__ out_depth, float* __restrict__ out_alpha, FwdLoss L) {
     __shared__ FwdWarpSmem smem[TS_JOB_WARPS];
     const int lane = threadIdx.x & 31;
     FwdWarpSmem& sm = smem[threadIdx.x >> 5];
@@ -27,6 +38,7 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
     const uint32_t lt = (1u << lane) - 1u;
     const size_t hw = (size_t)f.W * f.H;
     unsigned long long n_rect = 0, n_hit = 0, n_visit = 0;
+    float loss_acc = 0.0f;
 
     uint32_t j = ts_job_take(f, 0, lane);
     while (j < n_jobs) {
@@ -97,9 +109,31 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
             if (out_alpha) out_alpha[p] = 1.0f - T;
             f.n_contrib[p] = last;
             f.t_last[p] = Tlast;
+            if (LOSS) {
+                const float c[3] = {C0, C1, C2};
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) {
+                    const float d = c[ch] - __ldg(L.Chat + ch * hw + p);
+                    L.gC[ch * hw + p] = d > 0.f ? L.wc : (d < 0.f ? -L.wc : 0.f);
+                    loss_acc += L.wc * fabsf(d);
+                }
+                const float dh = __ldg(L.Dhat + p);
+                float g = 0.f;
+                if (dh > 0.f) {
+                    const float d = D - dh;
+                    g = d > 0.f ? L.wd : (d < 0.f ? -L.wd : 0.f);
+                    loss_acc += L.wd * fabsf(d);
+                }
+                L.gD[p] = g;
+            }
         }
     }
     ts_job_finish(f, 0, lane);
+    if (LOSS && L.loss) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) loss_acc += __shfl_xor_sync(0xffffffffu, loss_acc, d);
+        if (lane == 0) atomicAdd(L.loss, loss_acc);       // one atomic per persistent warp
+    }
     if (COUNT) {
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) {
@@ -115,25 +149,35 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
 }
 
 template <int SM>
-void launch_sm(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, float* oc, float* od, float* oa, cudaStream_t st) {
+void launch_sm(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, float* oc, float* od, float* oa, const FwdLoss* L,
+               cudaStream_t st) {
     const TsFrameDev& f = fr->d;
     const bool count = (fr->prm.flags & TS_PARAM_COUNTERS) != 0;
     const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 4, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
-    if (count)
-        render_fwd_kernel<SM, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, fr->prm.sigma, fr->prm.alpha_min, fr->prm.t_min, oc, od, oa);
-    else
-        render_fwd_kernel<SM, false><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, fr->prm.sigma, fr->prm.alpha_min, fr->prm.t_min, oc, od, oa);
+    const float sg = fr->prm.sigma, am = fr->prm.alpha_min, tm = fr->prm.t_min;
+    const FwdLoss none = {nullptr, nullptr, nullptr, nullptr, nullptr, 0.f, 0.f};
+    if (L) render_fwd_kernel<SM, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, *L);
+    else if (count) render_fwd_kernel<SM, true, false><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, none);
+    else render_fwd_kernel<SM, false, false><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, none);
 }
 
 }  // namespace
 
 int32_t ts_launch_render_fwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
+                             const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss,
                              cudaStream_t st) {
+    FwdLoss L;
+    const FwdLoss* Lp = nullptr;
+    if (gC) {
+        const double n = (double)fr->d.W * (double)fr->d.H;
+        L = FwdLoss{Chat, Dhat, gC, gD, loss, (float)(1.0 / (3.0 * n)), (float)((double)lambda_dep / n)};
+        Lp = &L;
+    }
     switch (ts_sigma_mode(fr->prm.sigma)) {
-        case 1: launch_sm<1>(ctx, fr, *sc, oc, od, oa, st); break;
-        case 2: launch_sm<2>(ctx, fr, *sc, oc, od, oa, st); break;
-        case 3: launch_sm<3>(ctx, fr, *sc, oc, od, oa, st); break;
-        default: launch_sm<0>(ctx, fr, *sc, oc, od, oa, st); break;
+        case 1: launch_sm<1>(ctx, fr, *sc, oc, od, oa, Lp, st); break;
+        case 2: launch_sm<2>(ctx, fr, *sc, oc, od, oa, Lp, st); break;
+        case 3: launch_sm<3>(ctx, fr, *sc, oc, od, oa, Lp, st); break;
+        default: launch_sm<0>(ctx, fr, *sc, oc, od, oa, Lp, st); break;
     }
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;

@@ -56,14 +56,21 @@ __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* of
     if (lane == 31) s_tmp[warp] = incl;
     if (lane == 0) s_tmp[nwarp + warp] = mx;
     __syncthreads();
-    uint32_t woff = 0;
-    total = 0, gmax = 0;
-    for (int w = 0; w < nwarp; ++w) {
-        const uint32_t c = s_tmp[w];
-        if (w < warp) woff += c;
-        total += c;
-        gmax = max(gmax, s_tmp[nwarp + w]);
+    if (warp == 0) {                                            // warp totals -> exclusive warp offsets, total, max
+        const uint32_t c = lane < nwarp ? s_tmp[lane] : 0u;
+        uint32_t m2 = lane < nwarp ? s_tmp[nwarp + lane] : 0u, in2 = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, in2, d);
+            if (lane >= d) in2 += t;
+        }
+        m2 = __reduce_max_sync(0xffffffffu, m2);
+        if (lane < nwarp) s_tmp[lane] = in2 - c;
+        if (lane == 31) s_tmp[2 * nwarp] = in2, s_tmp[2 * nwarp + 1] = m2;
     }
+    __syncthreads();
+    const uint32_t woff = s_tmp[warp];
+    total = s_tmp[2 * nwarp], gmax = s_tmp[2 * nwarp + 1];
     uint32_t run = woff + incl - sum;
     for (int t = t0; t < t1; ++t) {
         const uint32_t c = offs[t];
@@ -83,7 +90,11 @@ __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_
     for (int t = tid; t < f.NT; t += blockDim.x) {
         const uint32_t o = offs[t], c = (t + 1 < f.NT ? offs[t + 1] : total) - o;
         f.tile_ranges[t] = (fl || c == 0u) ? make_uint2(0u, 0u) : make_uint2(o, o + c);   // empty tile = (0,0)
-        atomicAdd(&s_hist[32 - __clz(c)], 1u);                 // bucket 0 = empty, b = floor(log2 c) + 1
+        // bucket 0 = empty, b = floor(log2 c) + 1; only ~10 buckets are in use, so the histogram is aggregated per
+        // warp (match) before it touches shared memory: one atomic per (warp, bucket), not 32-way conflicts
+        const int b = 32 - __clz(c);
+        const uint32_t peers = __match_any_sync(__activemask(), b);
+        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&s_hist[b], (uint32_t)__popc(peers));
     }
     __syncthreads();
     if (tid == 0) {
@@ -99,7 +110,13 @@ __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_
     __syncthreads();
     for (int t = tid; t < f.NT; t += blockDim.x) {
         const uint32_t c = (t + 1 < f.NT ? offs[t + 1] : total) - offs[t];
-        f.tile_order[atomicAdd(&s_hist[32 - __clz(c)], 1u)] = (uint32_t)t;
+        const int b = 32 - __clz(c);
+        const uint32_t act = __activemask(), peers = __match_any_sync(act, b);
+        const int leader = __ffs(peers) - 1, lane = threadIdx.x & 31;
+        uint32_t base = 0;
+        if (lane == leader) base = atomicAdd(&s_hist[b], (uint32_t)__popc(peers));
+        base = __shfl_sync(act, base, leader);
+        f.tile_order[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)t;
     }
 }
 
@@ -126,7 +143,8 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
     // This kernel is one wave of dependent round trips, so they are kept few: the raw records of this thread's
     // first slot are requested before anything else (speculatively: slot < n_visible is not known yet) and fly
     // while the CTA scans the tile counts.
-    uint32_t slot = blockIdx.x * TS_BIN_THREADS + threadIdx.x;
+    // slots are dealt to the grid warp by warp, so that the n_visible live ones spread over all SMs
+    uint32_t slot = ((threadIdx.x >> 5) * gridDim.x + blockIdx.x) * 32u + (threadIdx.x & 31);
     float4 s0, s1, s2, s3;
     s0 = s1 = s2 = s3 = make_float4(0.f, 0.f, 0.f, 0.f);
     if (slot < f.vis_cap) {
@@ -347,7 +365,7 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
 int32_t ts_launch_sort(const ts_ctx* ctx, ts_frame* fr, cudaStream_t stream) {
     const TsFrameDev& f = fr->d;
     const uint32_t grid_bin = (uint32_t)min((uint64_t)(f.vis_cap + TS_BIN_THREADS - 1) / TS_BIN_THREADS,
-                                            (uint64_t)ctx->num_sms * 4u);
+                                            (uint64_t)ctx->num_sms);
     if (f.NT <= TS_SCAN_LOCAL_MAX) {
         bin_setup_kernel<true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam);
     } else {

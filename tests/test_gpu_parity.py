@@ -200,3 +200,29 @@ def test_pose_reduce_step_equals_separate_calls(ctx, oracle_mod):
         assert np.array_equal(a, b)
     assert np.abs(res[0][0]).max() > 0
     g.close()
+
+
+def test_render_fwd_l1_equals_separate_calls(ctx, oracle_mod):
+    """ts_render_fwd_l1 (a3 + a4 fused) writes the same images and cotangents as ts_render_fwd + ts_l1_loss_grad."""
+    from gpu_util import dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(2)
+    o, g = both(ctx, oracle_mod, sc)
+    C, D, A = g.forward()
+    rng = np.random.default_rng(5)
+    Chat = dev(np.clip(C + rng.normal(0, 0.05, C.shape), 0, 1).astype(np.float32))
+    Dhat = dev((D * (rng.uniform(size=D.shape) > 0.2) * rng.uniform(0.9, 1.1, D.shape)).astype(np.float32))
+    gC1, gD1, L1 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
+    ts.ts_l1_loss_grad(ctx, g.W, g.H, g.C, g.D, Chat, Dhat, 0.05, gC1, gD1, L1)
+    C2, D2, A2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.empty_like(g.A)
+    gC2, gD2, L2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
+    ts.ts_render_fwd_l1(ctx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, 0.05, gC2, gD2, L2)
+    torch.cuda.synchronize()
+    assert torch.equal(C2, g.C) and torch.equal(D2, g.D) and torch.equal(A2, g.A)
+    assert torch.equal(gC1, gC2) and torch.equal(gD1, gD2)
+    assert abs(L1.item() - L2.item()) <= 1e-5 * abs(L1.item()) and L1.item() > 0
+    # outputs are optional in the fused call
+    ts.ts_render_fwd_l1(ctx, g.scene, g.frame, None, None, None, Chat, Dhat, 0.05, gC2, gD2, None)
+    torch.cuda.synchronize()
+    assert torch.equal(gC1, gC2) and torch.equal(gD1, gD2)
+    g.close()
