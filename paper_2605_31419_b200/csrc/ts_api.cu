@@ -29,7 +29,7 @@ bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pa
     L.tile_count = take(4ull * L.NT);
     L.tile_cursor = take(4ull * L.NT);
     L.tile_offset = take(4ull * L.NT);
-    L.tile_order = take(4ull * L.NT);
+    L.tile_order = take(16ull * L.NT);
     L.tile_ranges = take(8ull * L.NT);
     L.scr = take(16ull * TS_SCR_F4 * vis_cap);
     L.rec = take(16ull * TS_REC_F4 * vis_cap);
@@ -107,7 +107,7 @@ int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_
     d.tile_count = reinterpret_cast<uint32_t*>(b + L.tile_count);
     d.tile_cursor = reinterpret_cast<uint32_t*>(b + L.tile_cursor);
     d.tile_offset = reinterpret_cast<uint32_t*>(b + L.tile_offset);
-    d.tile_order = reinterpret_cast<uint32_t*>(b + L.tile_order);
+    d.tile_order = reinterpret_cast<uint4*>(b + L.tile_order);
     d.tile_ranges = reinterpret_cast<uint2*>(b + L.tile_ranges);
     d.scr = reinterpret_cast<float4*>(b + L.scr);
     d.rec = reinterpret_cast<float4*>(b + L.rec);

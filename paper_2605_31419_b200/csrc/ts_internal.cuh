@@ -41,7 +41,7 @@ struct TsFrameDev {
     uint32_t* tile_count;             // [NT] pairs per tile, counted by the project kernel (zeroed by the sort kernel)
     uint32_t* tile_cursor;            // [NT] write cursor of the binning pass, relative to the tile's begin (zero at rest)
     uint32_t* tile_offset;            // [NT] exclusive scan of tile_count (only used when NT > TS_SCAN_LOCAL_MAX)
-    uint32_t* tile_order;             // [NT] tiles by descending list length (render work queues)
+    uint4* tile_order;                // [NT] job headers (tile, begin, end, x0 | y0 << 16), tiles by descending list length
     uint2* tile_ranges;               // [NT] (begin, end) into the pair arrays
     float4* scr;                      // [vis_cap][4]: (u0,v0,w0,u1) (v1,w1,u2,v2) (w2,obar,rect_lo,rect_hi) (face,key,tiles,0)
     float4* rec;                      // [vis_cap][10]: per-face render record, see ts_raster.cuh

@@ -41,13 +41,14 @@ __device__ __forceinline__ void ts_job_finish(const TsFrameDev& f, int which, in
 }
 
 __device__ __forceinline__ void ts_job_decode(const TsFrameDev& f, uint32_t j, int lane, TsJob& job) {
-    job.tile = (int)__ldg(f.tile_order + (j >> 3));
+    const uint4 h = __ldg(f.tile_order + (j >> 3));         // (tile, begin, end, x0 | y0 << 16): one load per job
+    job.tile = (int)h.x;
     job.blk = (int)(j & 7u);
-    job.tx0 = (job.tile % f.tiles_x) * TS_TILE, job.ty0 = (job.tile / f.tiles_x) * TS_TILE;
+    job.tx0 = (int)(h.w & 0xffffu), job.ty0 = (int)(h.w >> 16);
     job.px = job.tx0 + ((job.blk & 1) << 3) + (lane & 7);
     job.py = job.ty0 + ((job.blk >> 1) << 2) + (lane >> 3);
     job.inside = job.px < f.W && job.py < f.H;
-    job.range = f.tile_ranges[job.tile];
+    job.range = make_uint2(h.y, h.z);
 }
 
 // lane mask of a sorted-list entry (slot, face, rect_lo, rect_hi) for this job's block
@@ -56,6 +57,22 @@ __device__ __forceinline__ uint32_t ts_entry_mask(const TsJob& job, const uint4 
     const int rx0 = max((int)(short)(rlo & 0xffff) - job.tx0, 0), ry0 = max((rlo >> 16) - job.ty0, 0);
     const int rx1 = min((int)(short)(rhi & 0xffff) - job.tx0, 15), ry1 = min((rhi >> 16) - job.ty0, 15);
     return ts_lane_mask(job.blk, rx0, ry0, rx1, ry1);
+}
+
+// Exact block cull: the entry's rect overlaps the block, but does the TRIANGLE?  For each edge the normalised edge
+// function is evaluated at the corner of (rect n block) where it is smallest; if that minimum is already above the
+// refinement band, every pixel of the block has x < -band for this face: no hit, and no refinement either, so
+// dropping the entry cannot change any result.  r0..r2 = record rows R0-R2.
+__device__ __forceinline__ bool ts_block_misses(const TsJob& job, const uint4 ent, const float4 r0, const float4 r1,
+                                                const float4 r2) {
+    const int rlo = (int)ent.z, rhi = (int)ent.w;
+    const int bx = job.tx0 + ((job.blk & 1) << 3), by = job.ty0 + ((job.blk >> 1) << 2);
+    const float x0 = (float)max((int)(short)(rlo & 0xffff), bx) - r0.x, x1 = (float)min((int)(short)(rhi & 0xffff), bx + 7) - r0.x;
+    const float y0 = (float)max(rlo >> 16, by) - r0.y, y1 = (float)min(rhi >> 16, by + 3) - r0.y;
+    const float l0 = fmaf(r0.z, r0.z > 0.f ? x0 : x1, fmaf(r0.w, r0.w > 0.f ? y0 : y1, r2.x));
+    const float l1 = fmaf(r1.x, r1.x > 0.f ? x0 : x1, fmaf(r1.y, r1.y > 0.f ? y0 : y1, r2.y));
+    const float l2 = fmaf(r1.z, r1.z > 0.f ? x0 : x1, fmaf(r1.w, r1.w > 0.f ? y0 : y1, r2.z));
+    return fmaxf(l0, fmaxf(l1, l2)) > 4.0f * TS_REFINE_BAND;
 }
 
 // the nine vertex-colour floats of a face

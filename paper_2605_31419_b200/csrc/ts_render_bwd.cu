@@ -23,7 +23,6 @@ struct BwdWarpSmem {
     uint32_t lm[32];
     uint32_t slot[32];
     uint32_t face[32];
-    uint32_t pos[32];                 // position of the entry in the tile list (0-based)
 };
 
 __device__ __forceinline__ float warp_sum(float v) {
@@ -73,31 +72,34 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
             const uint32_t n = hi - lo;
             uint4 cur = make_uint4(0u, 0u, 0u, 0u);
             if ((uint32_t)lane < n) cur = f.sorted[job.range.x + lo + lane];
-            const uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
-            const uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);
+            uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
             hi = lo;
-            if (ov == 0u) continue;
+            if (!__any_sync(0xffffffffu, lmask != 0u)) continue;
             __syncwarp();
             if (lmask) {
-                const int idx = __popc(ov & lt);
+                // staged at the lane's own index (no compaction); the walk follows the set bits of `ov` backwards
                 const float4* rp = f.rec + TS_REC_F4 * (size_t)cur.x;
                 float4 r[TS_REC_F4];
 #pragma unroll
                 for (int i = 0; i < (POSE ? 10 : 8); ++i) r[i] = __ldg(rp + i);
                 float col[9];
                 ts_load_colors(sc, cur.y, col);
-                float4* d = sm.r[idx];
+                if (ts_block_misses(job, cur, r[0], r[1], r[2])) lmask = 0u;
+                float4* d = sm.r[lane];
                 d[0] = r[0], d[1] = r[1], d[2] = r[2];
                 d[3] = make_float4(r[3].x, r[3].y, r[3].z, col[0]);
                 d[4] = make_float4(col[1], col[2], col[3], col[4]);
                 d[5] = make_float4(col[5], col[6], col[7], col[8]);
                 d[6] = r[4], d[7] = r[5], d[8] = r[6], d[9] = r[7];
                 if (POSE) d[10] = r[8], d[11] = r[9];
-                sm.lm[idx] = lmask, sm.slot[idx] = cur.x, sm.face[idx] = cur.y, sm.pos[idx] = lo + (uint32_t)lane;
+                sm.lm[lane] = lmask, sm.slot[lane] = cur.x, sm.face[lane] = cur.y;
             }
             __syncwarp();
-            for (int e = __popc(ov) - 1; e >= 0; --e) {
-                const bool in_rect = sm.pos[e] < ncon && ((sm.lm[e] >> lane) & 1u);
+            uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);
+            while (ov) {
+                const int e = 31 - __clz(ov);
+                ov &= ~(1u << e);
+                const bool in_rect = lo + (uint32_t)e < ncon && ((sm.lm[e] >> lane) & 1u);
                 if (!__any_sync(0xffffffffu, in_rect)) continue;
                 const float4* R = sm.r[e];
                 const float4 r0 = R[0], r1 = R[1], r2 = R[2];

@@ -13,7 +13,6 @@ struct FwdWarpSmem {
     float4 r[32][6];                  // R0 R1 R2 | kap0 kap1 kap2 c00 | c01 c02 c10 c11 | c12 c20 c21 c22
     uint32_t lm[32];                  // lane mask of the entry for this block
     uint32_t slot[32];
-    uint32_t pos[32];                 // 1 + position of the entry in the tile list
 };
 
 // optional fused a4: L1 colour + depth loss against a target frame, evaluated on the pixel values while they are
@@ -56,25 +55,29 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
             const uint32_t n = min(32u, job.range.y - c0);
             const uint4 cur = ent;
             if (c0 + 32 + lane < job.range.y) ent = f.sorted[c0 + 32 + lane];    // prefetch the next chunk
-            const uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
-            const uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);
-            if (ov == 0u) continue;
+            uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
+            if (!__any_sync(0xffffffffu, lmask != 0u)) continue;
             __syncwarp();                                   // previous chunk's reads are done
             if (lmask) {
-                const int idx = __popc(ov & lt);
+                // records are staged at the lane's own index (no compaction: nothing has to stay in registers
+                // across the ballot); the walk below follows the set bits of `ov` in list order
                 const float4* rp = f.rec + TS_REC_F4 * (size_t)cur.x;
                 const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2), r3 = __ldg(rp + 3);
                 float col[9];
                 ts_load_colors(sc, cur.y, col);
-                sm.r[idx][0] = r0, sm.r[idx][1] = r1, sm.r[idx][2] = r2;
-                sm.r[idx][3] = make_float4(r3.x, r3.y, r3.z, col[0]);
-                sm.r[idx][4] = make_float4(col[1], col[2], col[3], col[4]);
-                sm.r[idx][5] = make_float4(col[5], col[6], col[7], col[8]);
-                sm.lm[idx] = lmask, sm.slot[idx] = cur.x, sm.pos[idx] = (c0 - job.range.x) + (uint32_t)lane + 1u;
+                if (ts_block_misses(job, cur, r0, r1, r2)) lmask = 0u;
+                sm.r[lane][0] = r0, sm.r[lane][1] = r1, sm.r[lane][2] = r2;
+                sm.r[lane][3] = make_float4(r3.x, r3.y, r3.z, col[0]);
+                sm.r[lane][4] = make_float4(col[1], col[2], col[3], col[4]);
+                sm.r[lane][5] = make_float4(col[5], col[6], col[7], col[8]);
+                sm.lm[lane] = lmask, sm.slot[lane] = cur.x;
             }
             __syncwarp();
-            const int nov = __popc(ov);
-            for (int e = 0; e < nov; ++e) {
+            uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);
+            const uint32_t pos0 = (c0 - job.range.x) + 1u;
+            while (ov) {
+                const int e = __ffs(ov) - 1;
+                ov &= ov - 1;
                 const bool in_rect = !done && ((sm.lm[e] >> lane) & 1u);
                 if (COUNT) n_visit += 1, n_rect += in_rect ? 1 : 0;
                 if (!__any_sync(0xffffffffu, in_rect)) continue;
@@ -96,7 +99,7 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                     D += wz;
                     Tlast = T;
                     T = __fmul_rn(T, __fsub_rn(1.0f, alpha));
-                    last = sm.pos[e];
+                    last = pos0 + (uint32_t)e;
                     if (T <= t_min) done = true;
                 }
                 if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }

@@ -116,7 +116,10 @@ __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_
         uint32_t base = 0;
         if (lane == leader) base = atomicAdd(&s_hist[b], (uint32_t)__popc(peers));
         base = __shfl_sync(act, base, leader);
-        f.tile_order[base + __popc(peers & ((1u << lane) - 1u))] = (uint32_t)t;
+        const uint32_t o = offs[t];
+        const uint32_t xy = (uint32_t)((t % f.tiles_x) * TS_TILE) | ((uint32_t)((t / f.tiles_x) * TS_TILE) << 16);
+        f.tile_order[base + __popc(peers & ((1u << lane) - 1u))] =
+            (fl || c == 0u) ? make_uint4((uint32_t)t, 0u, 0u, xy) : make_uint4((uint32_t)t, o, o + c, xy);
     }
 }
 
