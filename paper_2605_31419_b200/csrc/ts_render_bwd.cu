@@ -5,9 +5,11 @@
 //       T_n = T_{n+1}/(1-alpha_n), keeps ONE scalar "behind" accumulator R = R^c.gC + R^d gD + R^a gA (no division
 //       by T), and forms the per-hit gradients wrt the face's screen vertices (u,v,w) x 3, its vertex colours and
 //       its opacity.
-//       POSE-ONLY mode (tracking): every hit's nine screen terms are pushed straight through d(u,v,w)/dtau
-//       (Eq. 5-7) into six per-thread accumulators -- no shuffle, no atomic, no per-face
-//       buffer -- which are tree-reduced once per job into a per-job partial (fixed order: deterministic).
+//       POSE-ONLY mode (tracking): the per-pixel walk only does the sequential part of a hit (alpha, T_n, dL/dalpha)
+//       and queues it; whenever 32 hits are queued every lane finishes one of them (B4-B6, then the nine screen
+//       terms straight through d(u,v,w)/dtau, Eq. 5-7) into six per-thread accumulators --
+//       all 32 lanes busy instead of the ~8 that hit a given face, no shuffle, no atomic, no per-face buffer.
+//       The accumulators are tree-reduced once per job into a per-job partial (fixed order: deterministic).
 //       FULL mode (mapping): per face the terms are reduced across the warp with shuffles BEFORE any global
 //       atomic (one lane issues the RED.ADD.F32s).
 //   proj_bwd_kernel   : full mode only; per visible face, screen -> camera -> world (B7-B8) and the se(3) terms
@@ -23,6 +25,10 @@ struct BwdWarpSmem {
     uint32_t lm[32];
     uint32_t slot[32];
     uint32_t face[32];
+    // pose-only mode: queue of hits waiting for the packed second phase, and the block's cotangents
+    uint32_t q_code[64];              // entry index | pixel lane << 8
+    float q_ga[64], q_wgt[64], q_l0[64], q_l1[64], q_l2[64];
+    float4 pix[32];                   // (gC0, gC1, gC2, gD) of the lane's pixel
 };
 
 __device__ __forceinline__ float warp_sum(float v) {
@@ -31,10 +37,89 @@ __device__ __forceinline__ float warp_sum(float v) {
     return v;
 }
 
+// B4 (window) + B5 (interpolation) + B6 (screen-space vertex terms) of ONE hit.  R = the staged record
+// (rows as in BwdWarpSmem::r), l = lhat_k, x = -max l, I = x^sigma, ga = dL/dalpha, wgt = T alpha,
+// z, d_k = c_k.gC, cg = c.gC, zgd = z gD.  Outputs g[9] = dL/d(u0,v0,w0,u1,v1,w1,u2,v2,w2).
+template <int SM>
+__device__ __forceinline__ void ts_bwd_geom(const float4* R, const float l[3], float x, float I, float ga, float wgt,
+                                            float z, float d0, float d1, float d2, float cg, float zgd, float sigma,
+                                            float g[9]) {
+    const float4 r0 = R[0], r1 = R[1], r2 = R[2];
+    const float4 q4 = R[6], q5 = R[7], q6 = R[8], q7 = R[9];   // record rows R4..R7
+    // B4 window: gx = dL/dx
+    const float gI = r2.w * ga;
+    float gx;
+    if (SM == 1) gx = gI;
+    else if (SM == 2) gx = 0.5f * gI * ts_rcp_approx(I);
+    else if (SM == 3) gx = 2.0f * gI * x;
+    else gx = gI * sigma * I * ts_rcp_approx(x);
+    // B5 interpolation
+    const float wz = wgt * z, base = cg + zgd;
+    const float go0 = wz * (d0 - base), go1 = wz * (d1 - base), go2 = wz * (d2 - base);
+    const float b0 = -l[0] * q4.x, b1 = -l[1] * q4.y, b2 = -l[2] * q4.z;      // b_k = -lhat_k rho_k
+    g[2] = b0 * go0, g[5] = b1 * go1, g[8] = b2 * go2;                        // dL/dw_k
+    // B6 (i): G = sum_k (w_k go_k) grad_p b_k,  grad_p b_k = -rho_k m_k
+    const float t0 = q5.x * go0 * q4.x, t1 = q5.y * go1 * q4.y, t2 = q5.z * go2 * q4.z;
+    const float Gx = -(t0 * r0.z + t1 * r1.x + t2 * r1.z), Gy = -(t0 * r0.w + t1 * r1.y + t2 * r1.w);
+    float q0x = -b0 * Gx, q0y = -b0 * Gy, q1x = -b1 * Gx, q1y = -b1 * Gy, q2x = -b2 * Gx, q2y = -b2 * Gy;
+    // B6 (ii): x = -lhat_{k*}; edge k* runs from a = q_{k*+1} to b = q_{k*+2};  t = b_{k*+2} + b_{k*} tau_{k*}
+    if (l[0] >= l[1] && l[0] >= l[2]) {
+        const float t = b2 + b0 * q5.w, mgx = r0.z * gx, mgy = r0.w * gx;
+        q1x += (1.0f - t) * mgx, q1y += (1.0f - t) * mgy, q2x += t * mgx, q2y += t * mgy;
+    } else if (l[1] >= l[2]) {
+        const float t = b0 + b1 * q6.x, mgx = r1.x * gx, mgy = r1.y * gx;
+        q2x += (1.0f - t) * mgx, q2y += (1.0f - t) * mgy, q0x += t * mgx, q0y += t * mgy;
+    } else {
+        const float t = b1 + b2 * q6.y, mgx = r1.z * gx, mgy = r1.w * gx;
+        q0x += (1.0f - t) * mgx, q0y += (1.0f - t) * mgy, q1x += t * mgx, q1y += t * mgy;
+    }
+    // B6 (iii): through the inradius
+    const float xg = x * gx;
+    g[0] = q0x + xg * q6.z, g[1] = q0y + xg * q6.w, g[3] = q1x + xg * q7.x, g[4] = q1y + xg * q7.y;
+    g[6] = q2x + xg * q7.z, g[7] = q2y + xg * q7.w;
+}
+
+// Pose-only second phase, one QUEUED hit per lane (lanes hold hits of different pixels and faces): recompute the
+// interpolation terms from the queued lhat_k, run B4-B6 and push the nine screen terms through B7 + B9
+// (Eq. 5-7): with Q = (xn, yn, 1)/w,  Z g_C = (a, b, c),  a = fx gu, b = fy gv, c = -(xn a + yn b) - w gw;
+// rho += w (a,b,c);  theta += Q x g_C.
+template <int SM>
+__device__ __forceinline__ void ts_bwd_pose_hit(const float4* R, const float4 pg, float l0, float l1, float l2, float ga,
+                                                float wgt, float fx, float fy, float sigma, float tau[6]) {
+    const float4 r3 = R[3], r4 = R[4], r5 = R[5];
+    const float l[3] = {l0, l1, l2};
+    const float x = -fmaxf(l0, fmaxf(l1, l2));
+    const float I = ts_window_pow<SM>(x, sigma);
+    const float o0 = l0 * r3.x, o1 = l1 * r3.y, o2 = l2 * r3.z;
+    const float Om = (o0 + o1) + o2, z = ts_rcp_approx(Om);
+    const float d0 = r3.w * pg.x + r4.x * pg.y + r4.y * pg.z;
+    const float d1 = r4.z * pg.x + r4.w * pg.y + r5.x * pg.z;
+    const float d2 = r5.y * pg.x + r5.z * pg.y + r5.w * pg.z;
+    const float cg = (o0 * d0 + o1 * d1 + o2 * d2) * z;
+    float g[9];
+    ts_bwd_geom<SM>(R, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sigma, g);
+    const float4 q5 = R[7], n0 = R[10], n1 = R[11];
+    {
+        const float a = fx * g[0], b = fy * g[1], c = -(n0.x * a + n0.y * b) - q5.x * g[2];
+        tau[0] += q5.x * a, tau[1] += q5.x * b, tau[2] += q5.x * c;
+        tau[3] += n0.y * c - b, tau[4] += a - n0.x * c, tau[5] += n0.x * b - n0.y * a;
+    }
+    {
+        const float a = fx * g[3], b = fy * g[4], c = -(n0.z * a + n0.w * b) - q5.y * g[5];
+        tau[0] += q5.y * a, tau[1] += q5.y * b, tau[2] += q5.y * c;
+        tau[3] += n0.w * c - b, tau[4] += a - n0.z * c, tau[5] += n0.z * b - n0.w * a;
+    }
+    {
+        const float a = fx * g[6], b = fy * g[7], c = -(n1.x * a + n1.y * b) - q5.z * g[8];
+        tau[0] += q5.z * a, tau[1] += q5.z * b, tau[2] += q5.z * c;
+        tau[3] += n1.y * c - b, tau[4] += a - n1.x * c, tau[5] += n1.x * b - n1.y * a;
+    }
+}
+
 // ATTR: colour / opacity gradients (B1, B4).  GEOM: screen-space vertex gradients into gscr (B5-B6).
-// POSE: screen-space vertex gradients pushed through Eq. 5-7 into per-thread se(3) accumulators (pose-only).
+// POSE: pose-only; hits are queued by the per-pixel walk and finished 32 at a time (ts_bwd_pose_hit).
 template <int SM, bool ATTR, bool GEOM, bool POSE>
-__global__ void __launch_bounds__(TS_JOB_WARPS * 32)
+__global__ void __launch_bounds__(TS_JOB_WARPS * 32, 3)
 render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float fx, float fy,
                   const float* __restrict__ gCi, const float* __restrict__ gDi, const float* __restrict__ gAi,
                   float* __restrict__ grad_color, float* __restrict__ grad_opacity) {
@@ -49,8 +134,6 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
     while (j < n_jobs) {
         TsJob job;
         ts_job_decode(f, j, lane, job);
-        const uint32_t this_job = j;
-        j = ts_job_take(f, 1, lane);
         const float fpx = (float)job.px, fpy = (float)job.py;
         const size_t p = (size_t)job.py * f.W + job.px;
         uint32_t ncon = 0;
@@ -62,10 +145,13 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
             if (gDi) gD = gDi[p];
             if (gAi) gA = gAi[p];
         }
+        j = ts_job_take(f, 1, lane);       // next ticket: its round trip overlaps the pixel loads
         const uint32_t n_walk = min(__reduce_max_sync(0xffffffffu, ncon), job.range.y - job.range.x);
+        if (POSE) sm.pix[lane] = make_float4(gC0, gC1, gC2, gD);
         float Rs = 0.f;                    // R^c.gC + R^d gD + R^a gA behind the current face
         float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         bool first = true;
+        uint32_t qn = 0;                   // queued hits (warp-uniform); the queue always starts at index 0
 
         for (uint32_t hi = n_walk; hi > 0;) {
             const uint32_t lo = hi > 32u ? hi - 32u : 0u;
@@ -102,10 +188,13 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                 const bool in_rect = lo + (uint32_t)e < ncon && ((sm.lm[e] >> lane) & 1u);
                 if (!__any_sync(0xffffffffu, in_rect)) continue;
                 const float4* R = sm.r[e];
-                const float4 r0 = R[0], r1 = R[1], r2 = R[2];
-                const float4* s4 = f.scr + TS_SCR_F4 * (size_t)sm.slot[e];
                 float l[3], x, I, alpha;
-                const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
+                bool hit = false;
+                {
+                    const float4 r0 = R[0], r1 = R[1], r2 = R[2];
+                    const float4* s4 = f.scr + TS_SCR_F4 * (size_t)sm.slot[e];
+                    hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
+                }
                 const uint32_t hm = __ballot_sync(0xffffffffu, hit);
                 if (!hm) continue;
                 float acc[19];
@@ -121,85 +210,58 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                     Tcur = Tn, first = false;
                     const float o0 = l[0] * r3.x, o1 = l[1] * r3.y, o2 = l[2] * r3.z;
                     const float Om = (o0 + o1) + o2, z = ts_rcp_approx(Om);
-                    const float lam0 = o0 * z, lam1 = o1 * z, lam2 = o2 * z;
                     // d_k = c_k . gC
                     const float d0 = r3.w * gC0 + r4.x * gC1 + r4.y * gC2;
                     const float d1 = r4.z * gC0 + r4.w * gC1 + r5.x * gC2;
                     const float d2 = r5.y * gC0 + r5.z * gC1 + r5.w * gC2;
-                    const float cg = lam0 * d0 + lam1 * d1 + lam2 * d2;       // c . gC
+                    const float cg = (o0 * d0 + o1 * d1 + o2 * d2) * z;       // c . gC
                     const float zgd = z * gD;
                     const float S = cg + zgd + gA;
                     const float wgt = Tn * alpha;
                     const float ga = Tn * (S - Rs);                           // B2
                     Rs = alpha * S + one_m * Rs;                              // B3
-                    if (ATTR) {
-                        // B1 colours, B4 opacity (one value per face; /3 applied when written)
-                        const float w0 = lam0 * wgt, w1 = lam1 * wgt, w2 = lam2 * wgt;
-                        acc[9] = w0 * gC0, acc[10] = w0 * gC1, acc[11] = w0 * gC2;
-                        acc[12] = w1 * gC0, acc[13] = w1 * gC1, acc[14] = w1 * gC2;
-                        acc[15] = w2 * gC0, acc[16] = w2 * gC1, acc[17] = w2 * gC2;
-                        acc[18] = I * ga;
-                    }
-                    if (GEOM || POSE) {
-                        const float4 q4 = R[6], q5 = R[7], q6 = R[8], q7 = R[9];   // record rows R4..R7
-                        // B4 window: gx = dL/dx
-                        const float gI = r2.w * ga;
-                        float gx;
-                        if (SM == 1) gx = gI;
-                        else if (SM == 2) gx = 0.5f * gI * ts_rcp_approx(I);
-                        else if (SM == 3) gx = 2.0f * gI * x;
-                        else gx = gI * sigma * I * ts_rcp_approx(x);
-                        // B5 interpolation
-                        const float wz = wgt * z, base = cg + zgd;
-                        const float go0 = wz * (d0 - base), go1 = wz * (d1 - base), go2 = wz * (d2 - base);
-                        const float b0 = -l[0] * q4.x, b1 = -l[1] * q4.y, b2 = -l[2] * q4.z;      // b_k = -lhat_k rho_k
-                        const float gw0 = b0 * go0, gw1 = b1 * go1, gw2 = b2 * go2;               // dL/dw_k
-                        // B6 (i): G = sum_k (w_k go_k) grad_p b_k,  grad_p b_k = -rho_k m_k
-                        const float t0 = q5.x * go0 * q4.x, t1 = q5.y * go1 * q4.y, t2 = q5.z * go2 * q4.z;
-                        const float Gx = -(t0 * r0.z + t1 * r1.x + t2 * r1.z), Gy = -(t0 * r0.w + t1 * r1.y + t2 * r1.w);
-                        float q0x = -b0 * Gx, q0y = -b0 * Gy, q1x = -b1 * Gx, q1y = -b1 * Gy, q2x = -b2 * Gx, q2y = -b2 * Gy;
-                        // B6 (ii): x = -lhat_{k*}; edge k* runs from a = q_{k*+1} to b = q_{k*+2};
-                        // t = b_{k*+2} + b_{k*} tau_{k*}
-                        if (l[0] >= l[1] && l[0] >= l[2]) {
-                            const float t = b2 + b0 * q5.w, mgx = r0.z * gx, mgy = r0.w * gx;
-                            q1x += (1.0f - t) * mgx, q1y += (1.0f - t) * mgy, q2x += t * mgx, q2y += t * mgy;
-                        } else if (l[1] >= l[2]) {
-                            const float t = b0 + b1 * q6.x, mgx = r1.x * gx, mgy = r1.y * gx;
-                            q2x += (1.0f - t) * mgx, q2y += (1.0f - t) * mgy, q0x += t * mgx, q0y += t * mgy;
-                        } else {
-                            const float t = b1 + b2 * q6.y, mgx = r1.z * gx, mgy = r1.w * gx;
-                            q0x += (1.0f - t) * mgx, q0y += (1.0f - t) * mgy, q1x += t * mgx, q1y += t * mgy;
+                    if (POSE) {
+                        // the sequential part of this hit is done; the rest (B4-B9) waits in the queue
+                        const uint32_t qi = qn + (uint32_t)__popc(hm & lt);
+                        sm.q_code[qi] = (uint32_t)e | ((uint32_t)lane << 8);
+                        sm.q_ga[qi] = ga, sm.q_wgt[qi] = wgt, sm.q_l0[qi] = l[0], sm.q_l1[qi] = l[1], sm.q_l2[qi] = l[2];
+                    } else {
+                        if (ATTR) {
+                            // B1 colours, B4 opacity (one value per face; /3 applied when written)
+                            const float w0 = o0 * z * wgt, w1 = o1 * z * wgt, w2 = o2 * z * wgt;
+                            acc[9] = w0 * gC0, acc[10] = w0 * gC1, acc[11] = w0 * gC2;
+                            acc[12] = w1 * gC0, acc[13] = w1 * gC1, acc[14] = w1 * gC2;
+                            acc[15] = w2 * gC0, acc[16] = w2 * gC1, acc[17] = w2 * gC2;
+                            acc[18] = I * ga;
                         }
-                        // B6 (iii): through the inradius
-                        const float xg = x * gx;
-                        q0x += xg * q6.z, q0y += xg * q6.w, q1x += xg * q7.x, q1y += xg * q7.y;
-                        q2x += xg * q7.z, q2y += xg * q7.w;
-                        if (POSE) {
-                            // B7 + B9 per vertex, with Q = (xn, yn, 1)/w:  Z g_C = (a, b, c),
-                            // a = fx gu, b = fy gv, c = -(xn a + yn b) - w gw;  rho += w (a,b,c);  theta += Q x g_C
-                            const float4 n0 = R[10], n1 = R[11];
-                            {
-                                const float a = fx * q0x, b = fy * q0y, c = -(n0.x * a + n0.y * b) - q5.x * gw0;
-                                tau[0] += q5.x * a, tau[1] += q5.x * b, tau[2] += q5.x * c;
-                                tau[3] += n0.y * c - b, tau[4] += a - n0.x * c, tau[5] += n0.x * b - n0.y * a;
-                            }
-                            {
-                                const float a = fx * q1x, b = fy * q1y, c = -(n0.z * a + n0.w * b) - q5.y * gw1;
-                                tau[0] += q5.y * a, tau[1] += q5.y * b, tau[2] += q5.y * c;
-                                tau[3] += n0.w * c - b, tau[4] += a - n0.z * c, tau[5] += n0.z * b - n0.w * a;
-                            }
-                            {
-                                const float a = fx * q2x, b = fy * q2y, c = -(n1.x * a + n1.y * b) - q5.z * gw2;
-                                tau[0] += q5.z * a, tau[1] += q5.z * b, tau[2] += q5.z * c;
-                                tau[3] += n1.y * c - b, tau[4] += a - n1.x * c, tau[5] += n1.x * b - n1.y * a;
-                            }
-                        } else {
-                            acc[0] = q0x, acc[1] = q0y, acc[2] = gw0, acc[3] = q1x, acc[4] = q1y, acc[5] = gw1;
-                            acc[6] = q2x, acc[7] = q2y, acc[8] = gw2;
-                        }
+                        if (GEOM) ts_bwd_geom<SM>(R, l, x, I, ga, wgt, z, d0, d1, d2, cg, zgd, sigma, acc);
                     }
                 }
-                if (!POSE) {
+                if (POSE) {
+                    qn += (uint32_t)__popc(hm);
+                    if (qn >= 32u) {
+                        // a full group: every lane finishes one queued hit
+                        __syncwarp();
+                        const uint32_t code = sm.q_code[lane];
+                        const float qga = sm.q_ga[lane], qw = sm.q_wgt[lane], ql0 = sm.q_l0[lane], ql1 = sm.q_l1[lane], ql2 = sm.q_l2[lane];
+                        const uint32_t rest = qn - 32u;
+                        // move the remainder (< 32 entries) to the front
+                        uint32_t mc = 0;
+                        float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f, m4 = 0.f;
+                        if ((uint32_t)lane < rest) {
+                            mc = sm.q_code[32 + lane], m0 = sm.q_ga[32 + lane], m1 = sm.q_wgt[32 + lane];
+                            m2 = sm.q_l0[32 + lane], m3 = sm.q_l1[32 + lane], m4 = sm.q_l2[32 + lane];
+                        }
+                        __syncwarp();
+                        if ((uint32_t)lane < rest) {
+                            sm.q_code[lane] = mc, sm.q_ga[lane] = m0, sm.q_wgt[lane] = m1;
+                            sm.q_l0[lane] = m2, sm.q_l1[lane] = m3, sm.q_l2[lane] = m4;
+                        }
+                        qn = rest;
+                        ts_bwd_pose_hit<SM>(sm.r[code & 0xffu], sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
+                        __syncwarp();
+                    }
+                } else {
                     // reduce across the warp, then one lane issues the atomics
                     const bool single = (hm & (hm - 1)) == 0;
                     const int src = __ffs(hm) - 1;
@@ -239,6 +301,17 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                     }
                 }
             }
+            if (POSE && qn) {
+                // the staged records are about to be replaced: finish what is still queued (partial group)
+                __syncwarp();
+                if ((uint32_t)lane < qn) {
+                    const uint32_t code = sm.q_code[lane];
+                    ts_bwd_pose_hit<SM>(sm.r[code & 0xffu], sm.pix[code >> 8], sm.q_l0[lane], sm.q_l1[lane], sm.q_l2[lane],
+                                        sm.q_ga[lane], sm.q_wgt[lane], fx, fy, sigma, tau);
+                }
+                qn = 0;
+                __syncwarp();
+            }
         }
         if (POSE) {
             // per-thread -> per-job partial (fixed shuffle tree; the final reduction runs over jobs in index order)
@@ -251,7 +324,6 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                 // partials are indexed by (tile, block), not by ticket: the sum order does not depend on scheduling
                 f.pose_partials[6 * ((size_t)job.tile * TS_BLOCKS_PER_TILE + job.blk) + lane] = v;
             }
-            (void)this_job;
         }
     }
     ts_job_finish(f, 1, lane);

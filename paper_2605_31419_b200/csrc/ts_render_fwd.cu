@@ -43,7 +43,6 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
     while (j < n_jobs) {
         TsJob job;
         ts_job_decode(f, j, lane, job);
-        j = ts_job_take(f, 0, lane);                       // next ticket: its latency hides behind this job
         const float fpx = (float)job.px, fpy = (float)job.py;
         float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, D = 0.0f, Tlast = 1.0f;
         uint32_t last = 0;
@@ -51,6 +50,7 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
         bool warp_done = __all_sync(0xffffffffu, done);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
         if (job.range.x + lane < job.range.y) ent = f.sorted[job.range.x + lane];
+        j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
         for (uint32_t c0 = job.range.x; c0 < job.range.y && !warp_done; c0 += 32) {
             const uint32_t n = min(32u, job.range.y - c0);
             const uint4 cur = ent;
