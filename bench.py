@@ -69,17 +69,38 @@ class ClockSampler:
 
 
 def algorithmic_work(cnt, HW, NT, M, p_sort, mode="pose"):
-    """algorithmic bytes / FP32 flops per step from the measured counters."""
+    """algorithmic bytes / FP32 flops per step from the measured counters, per bench stage
+    (render_fwd = a3 + a4 fused: + 16 B/px of target read and 16 B/px of cotangents written)."""
     nv, P, nr, nh = cnt["n_visible"], cnt["n_pairs"], cnt["n_rect"], cnt["n_hit"]
     B = {"project": 36 * M + 4 * nv + 48 * nv,
          "bin_sort": 12 * nv + P * (12 + 8 + 24 * p_sort + 4) + 8 * NT,
-         "render_fwd": 84 * nv + 24 * HW,
-         "loss": 36 * HW,
+         "render_fwd": 84 * nv + 24 * HW + 32 * HW,
          "render_bwd": 84 * nv + 28 * HW + (24 * NT if mode == "pose" else 168 * nv) + (0 if mode == "pose" else 144 * nv),
          "pose_reduce": 24 * NT}
-    F = {"project": 130 * M, "bin_sort": 0, "render_fwd": 100 * P + 15 * nr + 40 * nh, "loss": 8 * HW,
+    F = {"project": 130 * M, "bin_sort": 0, "render_fwd": 100 * P + 15 * nr + 40 * nh + 8 * HW,
          "render_bwd": 100 * P + 15 * nr + (170 if mode == "pose" else 190) * nh + 60 * nv, "pose_reduce": 60 * nv}
     return B, F
+
+
+def load_traffic():
+    """dram bytes per launch of each stage's kernels from the committed ncu --set full capture (profiles/)."""
+    p = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    return json.load(open(p)) if os.path.exists(p) else {}
+
+
+def rank_seed(config, rank):
+    """Replicas / weak scaling: rank r tracks its own frame of the same scene family."""
+    return config + 100 * rank
+
+
+def max_over_ranks(dist, value, device):
+    """Max over ranks of a scalar (device-timed milliseconds): one all-reduce outside the timed region."""
+    import torch
+    if dist is None:
+        return float(value)
+    t = torch.tensor([float(value)], device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
 
 
 def run_reference(args):
@@ -223,7 +244,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peaks = load_peaks()
     # replicas / weak scaling: every rank tracks its own frame of the same scene family (seed offset by rank)
-    sc = scenes.make_config(args.config, seed=args.config + 100 * rank) if rank else scenes.make_config(args.config)
+    sc = scenes.make_config(args.config, seed=rank_seed(args.config, rank)) if rank else scenes.make_config(args.config)
     HW, M = sc.cam.width * sc.cam.height, sc.M
 
     # counters (debug instantiation, outside the timed region)
@@ -231,9 +252,9 @@ def main():
     trc.forward()
     fl, nvis, npairs = ts.ts_frame_status(trc.ctx, trc.frame)
     cn = ts.ts_frame_view(trc.ctx, trc.frame, ts.VIEW_COUNTERS).cpu().numpy()
-    # the target render in Tracker.__init__ also counted: two forwards ran with counters on
+    # the counting instantiation ran once, for the target render in Tracker.__init__ (the fused forward does not count)
     cnt = {"n_visible": int(nvis), "n_pairs": int(npairs), "n_warp_visits": int(cn[0]), "n_rect": int(cn[1]), "n_hit": int(cn[2]),
-           "note": "n_rect/n_hit/n_warp_visits summed over the target render and the start-pose render"}
+           "note": "n_rect / n_hit / n_warp_visits: one forward render (ground-truth pose); n_visible / n_pairs: start pose"}
     del trc
     torch.cuda.empty_cache()
 
@@ -277,10 +298,8 @@ def main():
     torch.cuda.synchronize()
     t_wall = time.perf_counter() - t_wall0
     total_ms = float(sum(ms))
+    total_ms = max_over_ranks(dist, total_ms, "cuda")
     if dist is not None:
-        t = torch.tensor([total_ms], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
         dist.barrier()
     ms_per_step = total_ms / args.steps
 
@@ -352,15 +371,11 @@ def main():
         if it >= args.warmup:
             e2e_ms.append((time.perf_counter() - t0) * 1e3)
     e2e_step = float(np.mean(e2e_ms))
-    if dist is not None:
-        t = torch.tensor([e2e_step], device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_step = float(t.item())
+    e2e_step = max_over_ranks(dist, e2e_step, "cuda")
 
     value = world * HW / (ms_per_step * 1e-3) / 1e6
     p_sort = (32 + max(0, (NT - 1).bit_length()) + 7) // 8
-    half = {k: (v // 2 if k in ("n_rect", "n_hit", "n_warp_visits") else v) for k, v in cnt.items() if k != "note"}
-    B, F = algorithmic_work(half, HW, NT, M, p_sort, "pose")
+    B, F = algorithmic_work(cnt, HW, NT, M, p_sort, "pose")
     p_fp32 = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12        # TFLOP/s, nominal
     t_hbm = sum(B.values()) / (peaks["hbm_gbs"] * 1e9)
     t_alu = sum(F.values()) / (p_fp32 * 1e12)
@@ -374,7 +389,7 @@ def main():
         roof = {"bound": "hbm", "kernel": dom, "achieved": B[dom] / dom_t / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "peak_source": peaks["src"]}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
+    roof["traffic"] = load_traffic().get(dom)
     roof["algorithmic_bytes"] = B[dom]
     roof["algorithmic_flops"] = F[dom]
     roof["launch_ms"] = stage_ms[dom]
