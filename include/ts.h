@@ -121,6 +121,14 @@ int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const
 int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
                          float* out_alpha, const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD,
                          float* loss_dev, void* stream);
+/* a3 + a4 + a5 (pose-only) in one launch, the tracking fast path: every 8x4-pixel block is rendered, its L1
+ * cotangents are formed in registers and its reverse walk runs at once; leaves the se(3) partial sums for
+ * ts_pose_jacobian_reduce / ts_pose_reduce_step exactly as ts_render_fwd_l1 + ts_render_bwd(TS_GRAD_POSE) would
+ * (same arithmetic, bit-identical result).  out_*, gC, gD and loss_dev may be NULL.  ts_render_bwd cannot follow
+ * this call (the per-pixel walk state is not written out). */
+int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
+                           float* out_alpha, const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD,
+                           float* loss_dev, void* stream);
 /* a8: one Adam step on tau, then T_cw <- Exp(-delta) o T_cw, all on the device.
  * state_dev[13] = m[6], v[6], step; lr[6] passed by value (rho then theta). */
 int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev, const float* lr6,

@@ -210,6 +210,17 @@ int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* o
     return s;
 }
 
+int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth, float* out_alpha,
+                           const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
+                           void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !Chat || !Dhat) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if (!fr->have_sort) return TS_ERR_STATE;
+    fr->have_fwd = 0;                                       // n_contrib / T_last are not written: no ts_render_bwd after this
+    return ts_launch_render_track(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev,
+                                  (cudaStream_t)stream);
+}
+
 int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
                       const float* dL_dalpha, float* grad_pos, float* grad_color, float* grad_opacity,
                       uint32_t grad_mask, void* stream) {

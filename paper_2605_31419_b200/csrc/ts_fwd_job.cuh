@@ -1,0 +1,86 @@
+// ts_fwd_job.cuh -- the forward walk of ONE job (one 8x4-pixel block, one warp): Eq. 2-4.
+// Shared by render_fwd_kernel (ts_render_fwd.cu) and the fused tracking kernel (ts_render_bwd.cu).
+#pragma once
+#include "ts_jobs.cuh"
+
+struct FwdWarpSmem {
+    float4 r[32][6];                  // R0 R1 R2 | kap0 kap1 kap2 c00 | c01 c02 c10 c11 | c12 c20 c21 c22
+    uint32_t lm[32];                  // lane mask of the entry for this block
+    uint32_t slot[32];
+};
+
+struct FwdPix {                       // what the walk leaves for this lane's pixel
+    float T, C0, C1, C2, D, Tlast;
+    uint32_t last;
+};
+
+// `ent` = the lane's entry of the first 32-entry chunk of the tile list (already requested by the caller, so that
+// its round trip overlaps the caller's ticket atomic).
+template <int SM, bool COUNT>
+__device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene& sc, const TsJob& job, int lane,
+                                            FwdWarpSmem& sm, float sigma, float alpha_min, float t_min, uint4 ent,
+                                            FwdPix& o, unsigned long long& n_visit, unsigned long long& n_rect,
+                                            unsigned long long& n_hit) {
+    const float fpx = (float)job.px, fpy = (float)job.py;
+    float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, D = 0.0f, Tlast = 1.0f;
+    uint32_t last = 0;
+    const uint32_t lt = (1u << lane) - 1u;
+    (void)lt;
+    bool done = !job.inside;
+    bool warp_done = __all_sync(0xffffffffu, done);
+    for (uint32_t c0 = job.range.x; c0 < job.range.y && !warp_done; c0 += 32) {
+        const uint32_t n = min(32u, job.range.y - c0);
+        const uint4 cur = ent;
+        if (c0 + 32 + lane < job.range.y) ent = f.sorted[c0 + 32 + lane];    // prefetch the next chunk
+        uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
+        if (!__any_sync(0xffffffffu, lmask != 0u)) continue;
+        __syncwarp();                                   // previous chunk's reads are done
+        if (lmask) {
+            // records are staged at the lane's own index (no compaction: nothing has to stay in registers
+            // across the ballot); the walk below follows the set bits of `ov` in list order
+            const float4* rp = f.rec + TS_REC_F4 * (size_t)cur.x;
+            const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2), r3 = __ldg(rp + 3);
+            float col[9];
+            ts_load_colors(sc, cur.y, col);
+            if (ts_block_misses(job, cur, r0, r1, r2)) lmask = 0u;
+            sm.r[lane][0] = r0, sm.r[lane][1] = r1, sm.r[lane][2] = r2;
+            sm.r[lane][3] = make_float4(r3.x, r3.y, r3.z, col[0]);
+            sm.r[lane][4] = make_float4(col[1], col[2], col[3], col[4]);
+            sm.r[lane][5] = make_float4(col[5], col[6], col[7], col[8]);
+            sm.lm[lane] = lmask, sm.slot[lane] = cur.x;
+        }
+        __syncwarp();
+        uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);
+        const uint32_t pos0 = (c0 - job.range.x) + 1u;
+        while (ov) {
+            const int e = __ffs(ov) - 1;
+            ov &= ov - 1;
+            const bool in_rect = !done && ((sm.lm[e] >> lane) & 1u);
+            if (COUNT) n_visit += 1, n_rect += in_rect ? 1 : 0;
+            if (!__any_sync(0xffffffffu, in_rect)) continue;
+            const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
+            const float4* s4 = f.scr + TS_SCR_F4 * (size_t)sm.slot[e];
+            float l[3], x, I, alpha;
+            const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
+            if (!__any_sync(0xffffffffu, hit)) continue;
+            if (hit) {
+                const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
+                if (COUNT) n_hit += 1;
+                const float o0 = l[0] * r3.x, o1 = l[1] * r3.y, o2 = l[2] * r3.z;   // omega_k = lhat_k kappa_k
+                const float Om = (o0 + o1) + o2;
+                const float z = ts_rcp_approx(Om);
+                const float wgt = T * alpha, wz = wgt * z;
+                C0 = fmaf(wz, fmaf(o0, r3.w, fmaf(o1, r4.z, o2 * r5.y)), C0);
+                C1 = fmaf(wz, fmaf(o0, r4.x, fmaf(o1, r4.w, o2 * r5.z)), C1);
+                C2 = fmaf(wz, fmaf(o0, r4.y, fmaf(o1, r5.x, o2 * r5.w)), C2);
+                D += wz;
+                Tlast = T;
+                T = __fmul_rn(T, __fsub_rn(1.0f, alpha));
+                last = pos0 + (uint32_t)e;
+                if (T <= t_min) done = true;
+            }
+            if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }
+        }
+    }
+    o.T = T, o.C0 = C0, o.C1 = C1, o.C2 = C2, o.D = D, o.Tlast = Tlast, o.last = last;
+}

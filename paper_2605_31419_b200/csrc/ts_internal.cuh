@@ -104,5 +104,7 @@ int32_t ts_launch_render_fwd(const ts_ctx*, ts_frame*, const ts_scene*, float* o
                              const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, cudaStream_t);
 int32_t ts_launch_render_bwd(const ts_ctx*, ts_frame*, const ts_scene*, const float*, const float*, const float*,
                              float*, float*, float*, uint32_t, cudaStream_t);
+int32_t ts_launch_render_track(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
+                               const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, cudaStream_t);
 int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame*, float* out, float* T_cw, float* state, const float* lr6, float beta1,
                               float beta2, float eps, cudaStream_t);

@@ -226,3 +226,42 @@ def test_render_fwd_l1_equals_separate_calls(ctx, oracle_mod):
     torch.cuda.synchronize()
     assert torch.equal(gC1, gC2) and torch.equal(gD1, gD2)
     g.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 2, 4])
+def test_render_track_l1_equals_separate_calls(ctx, oracle_mod, cfg):
+    """ts_render_track_l1 (a3 + a4 + a5 pose-only fused) == ts_render_fwd_l1 + ts_render_bwd(POSE), bit for bit, and
+    its pose gradient matches the oracle's."""
+    from gpu_util import dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(cfg)
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    tgt = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+    Chat, Dhat = dev(tgt.color), dev(tgt.depth)
+    lam = sc.params.lambda_dep
+    gC, gD, L1 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
+    ts.ts_render_fwd_l1(ctx, g.scene, g.frame, None, None, None, Chat, Dhat, lam, gC, gD, L1)
+    ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, None, None, None, ts.GRAD_POSE)
+    tau1 = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau1)
+    C2, D2, A2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.empty_like(g.A)
+    gC2, gD2, L2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
+    ts.ts_render_track_l1(ctx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, lam, gC2, gD2, L2)
+    tau2 = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau2)
+    torch.cuda.synchronize()
+    assert torch.equal(C2, g.C) and torch.equal(D2, g.D) and torch.equal(A2, g.A)
+    assert torch.equal(gC, gC2) and torch.equal(gD, gD2)
+    assert torch.equal(tau1, tau2) and tau1.abs().max().item() > 0
+    assert abs(L1.item() - L2.item()) <= 1e-5 * abs(L1.item())
+    # against the oracle: same loss cotangents on the unambiguous pixels, pose gradient to 1e-3
+    Lo, gCo, gDo = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, lam)
+    same = (gC.cpu().numpy() == gCo).all(axis=0) & (gD.cpu().numpy() == gDo) & ok
+    if same.mean() > 0.999:       # sign images agree (they can differ where |C - Chat| is within float rounding)
+        ref = o.backward(gC.cpu().numpy(), gD.cpu().numpy(), None, want=("pose",))
+        t2 = tau2.cpu().numpy()
+        assert np.abs(t2 - ref.dL_dtau).max() <= 2e-3 * np.abs(ref.dL_dtau).max(), (t2, ref.dL_dtau)
+    with pytest.raises(ts.TsError):
+        ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, None, None, None, ts.GRAD_POSE)   # no walk state after track
+    g.close()
