@@ -9,9 +9,9 @@
  *    workspace and repeats.
  *  - Ownership: every DEVICE buffer is owned by the caller (e.g. torch tensors' data_ptr()), including the
  *    frame workspace.  The library allocates no device memory after ts_create, never frees caller memory and
- *    keeps no caller pointer beyond the call, with one exception: a ts_frame remembers the scene and pose pointers
- *    given to ts_project until the next ts_project on it (ts_bin_sort reads scene->opacity, ts_render_bwd reads the
- *    pose), so they must stay valid and unchanged until the frame's backward pass has been enqueued.
+ *    keeps no caller pointer beyond the call, with one exception: a ts_frame remembers the pose pointer given to
+ *    ts_project until the next ts_project on it (the full-gradient ts_render_bwd reads the pose again), so it must
+ *    stay valid and unchanged until the frame's backward pass has been enqueued.
  *  - Streams: `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is enqueued
  *    on it.  No export synchronises except ts_frame_status and ts_frame_view.  All exports may be captured
  *    into a CUDA graph (launch geometry never depends on device-side counts).
@@ -77,7 +77,7 @@ int32_t ts_frame_status(ts_ctx* ctx, ts_frame* frame, uint32_t* flags, uint32_t*
  * depth key, and are counted into every 16x16 tile they touch; the per-tile counts are scanned into
  * tile_ranges[NT] = (begin,end).  float32 with a fixed operation order: cull set, rects, depth keys and tile
  * counts are bit-identical to the oracle (N1-N5).  One kernel, one pass over the map.
- * scene->color may be NULL here; scene->opacity must be valid. */
+ * scene->color may be NULL here; scene->opacity must be valid (the mean vertex opacity of PAPER.md:82 is taken here). */
 int32_t ts_project(ts_ctx* ctx, const ts_scene* scene, const ts_camera* cam, const ts_params* prm,
                    const float* T_cw_dev, ts_frame* frame, void* stream);
 
@@ -98,7 +98,7 @@ int32_t ts_render_fwd(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float
 /* a5+a6: reverse walk of the same lists (B1-B8), gradients of L given dL/dC, dL/dD, dL/dA
  * (same layouts as the outputs; any may be NULL = 0).  grad_mask selects TS_GRAD_*.  With TS_GRAD_POSE alone
  * ("pose-only", the tracking mode) no per-vertex buffer is touched: per-thread se(3) terms are tree-reduced
- * in-kernel to one 6-vector per tile.  Otherwise per-face screen-space gradients are warp-reduced, added with
+ * in-kernel to one 6-vector per 8x4-pixel block.  Otherwise per-face screen-space gradients are warp-reduced, added with
  * global float atomics and pushed through the projection (B7-B8) into grad_pos; colour / opacity gradients are
  * added to grad_color / grad_opacity.  Requires ts_render_fwd on the same frame. */
 int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, const float* dL_dcolor,

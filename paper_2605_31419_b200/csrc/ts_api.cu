@@ -162,7 +162,6 @@ int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const 
     fr->cam = TsCamDev{cam->width, cam->height, cam->fx, cam->fy, cam->cx, cam->cy, cam->znear};
     fr->prm = TsPrmDev{prm->sigma, prm->alpha_min, prm->t_min, prm->eps_area, prm->flags};
     fr->T_cw = T_cw_dev;
-    fr->scene = *sc;
     fr->have_sort = fr->have_fwd = 0;
     fr->pose_src = 0;
     if (fr->counters_dirty) {

@@ -72,7 +72,6 @@ struct ts_frame {
     TsCamDev cam;
     TsPrmDev prm;
     const float* T_cw;       // device pointer given to the last ts_project (read again by the projection backward)
-    ts_scene scene;          // scene given to the last ts_project (opacity is read by the binning kernel)
     int have_project, have_sort, have_fwd;
     int counters_dirty;      // ts_project ran but ts_bin_sort has not consumed (and re-zeroed) its counters yet
     uint32_t pose_src;       // 0 = none, 1 = per-tile partials (pose-only), 2 = per-block partials (projection backward)
