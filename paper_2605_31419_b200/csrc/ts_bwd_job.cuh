@@ -99,9 +99,97 @@ __device__ __forceinline__ void ts_bwd_pose_hit(const float4* R, const float4 pg
     }
 }
 
+// Full-gradient second phase, one QUEUED hit per lane: the 9 screen terms (GEOM) and / or the 9 colour terms + the
+// opacity term (ATTR) of the lane's hit; hits of the same face sit in consecutive lanes (they were queued by one
+// visit), so a segmented shuffle reduction adds them up per face BEFORE any global atomic, and the first lane of every
+// run issues the RED.ADD.F32s.  `active` = this lane holds a hit.
+template <int SM, bool ATTR, bool GEOM>
+__device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_scene& sc, BwdWarpSmem& sm, int lane,
+                                                  bool active, uint32_t code, float l0, float l1, float l2, float ga,
+                                                  float wgt, float sigma, float* __restrict__ grad_color,
+                                                  float* __restrict__ grad_opacity) {
+    const uint32_t e = code & 0xffu;
+    float acc[19];
+#pragma unroll
+    for (int j = 0; j < 19; ++j) acc[j] = 0.f;
+    if (active) {
+        const float4* R = sm.r[e];
+        const float4 pg = sm.pix[code >> 8];
+        const float4 r3 = R[3], r4 = R[4], r5 = R[5];
+        const float l[3] = {l0, l1, l2};
+        const float x = -fmaxf(l0, fmaxf(l1, l2));
+        const float I = ts_window_pow<SM>(x, sigma);
+        const float o0 = l0 * r3.x, o1 = l1 * r3.y, o2 = l2 * r3.z;
+        const float Om = (o0 + o1) + o2, z = ts_rcp_approx(Om);
+        if (ATTR) {
+            // B1 colours, B4 opacity (one value per face; /3 applied when written)
+            const float w0 = o0 * z * wgt, w1 = o1 * z * wgt, w2 = o2 * z * wgt;
+            acc[9] = w0 * pg.x, acc[10] = w0 * pg.y, acc[11] = w0 * pg.z;
+            acc[12] = w1 * pg.x, acc[13] = w1 * pg.y, acc[14] = w1 * pg.z;
+            acc[15] = w2 * pg.x, acc[16] = w2 * pg.y, acc[17] = w2 * pg.z;
+            acc[18] = I * ga;
+        }
+        if (GEOM) {
+            const float d0 = r3.w * pg.x + r4.x * pg.y + r4.y * pg.z;
+            const float d1 = r4.z * pg.x + r4.w * pg.y + r5.x * pg.z;
+            const float d2 = r5.y * pg.x + r5.z * pg.y + r5.w * pg.z;
+            const float cg = (o0 * d0 + o1 * d1 + o2 * d2) * z;
+            ts_bwd_geom<SM>(R, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sigma, acc);
+        }
+    }
+    // segmented reduction over runs of equal staged index (inactive lanes never match anybody)
+    const uint32_t key = active ? e : 0x100u + (uint32_t)lane;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t kd = __shfl_down_sync(0xffffffffu, key, d);
+        const bool same = (lane + d < 32) && kd == key;
+        if (GEOM) {
+#pragma unroll
+            for (int j = 0; j < 9; ++j) {
+                const float t = __shfl_down_sync(0xffffffffu, acc[j], d);
+                if (same) acc[j] += t;
+            }
+        }
+        if (ATTR) {
+#pragma unroll
+            for (int j = 9; j < 19; ++j) {
+                const float t = __shfl_down_sync(0xffffffffu, acc[j], d);
+                if (same) acc[j] += t;
+            }
+        }
+    }
+    const uint32_t kp = __shfl_up_sync(0xffffffffu, key, 1);
+    if (active && (lane == 0 || kp != key)) {                  // first lane of a run
+        if (GEOM) {
+            float* gs = f.gscr + 9 * (size_t)sm.slot[e];
+#pragma unroll
+            for (int j = 0; j < 9; ++j) atomicAdd(gs + j, acc[j]);
+        }
+        if (ATTR) {
+            const uint32_t m = sm.face[e];
+            uint32_t v[3];
+#pragma unroll
+            for (int k = 0; k < 3; ++k) v[k] = sc.faces ? (uint32_t)__ldg(sc.faces + 3 * (size_t)m + k) : 3u * m + k;
+            if (grad_color) {
+#pragma unroll
+                for (int k = 0; k < 3; ++k)
+#pragma unroll
+                    for (int ch = 0; ch < 3; ++ch) atomicAdd(grad_color + 3 * (size_t)v[k] + ch, acc[9 + 3 * k + ch]);
+            }
+            if (grad_opacity) {
+                const float go = acc[18] * (1.0f / 3.0f);
+#pragma unroll
+                for (int k = 0; k < 3; ++k) atomicAdd(grad_opacity + v[k], go);
+            }
+        }
+    }
+}
+
 // ncon / Tcur = the forward walk's n_contrib and T in front of the last contributing face for this lane's pixel;
-// gC*, gD, gA = the pixel's cotangents.  POSE: tau[6] += this lane's se(3) terms.  Otherwise atomics into
-// f.gscr / grad_color / grad_opacity.
+// gC*, gD, gA = the pixel's cotangents.  The per-pixel walk does the sequential part of every hit and queues it;
+// 32 queued hits at a time are finished with all lanes busy: POSE: tau[6] += the lane's se(3) terms
+// (ts_bwd_pose_hit); otherwise segmented per-face reduction + atomics into f.gscr / grad_color / grad_opacity
+// (ts_bwd_full_group).
 template <int SM, bool ATTR, bool GEOM, bool POSE>
 __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene& sc, const TsJob& job, int lane,
                                             BwdWarpSmem& sm, float sigma, float alpha_min, float fx, float fy,
@@ -111,7 +199,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
     const float fpx = (float)job.px, fpy = (float)job.py;
     const uint32_t lt = (1u << lane) - 1u;
     const uint32_t n_walk = min(__reduce_max_sync(0xffffffffu, ncon), job.range.y - job.range.x);
-    if (POSE) sm.pix[lane] = make_float4(gC0, gC1, gC2, gD);
+    sm.pix[lane] = make_float4(gC0, gC1, gC2, gD);
     float Rs = 0.f;                    // R^c.gC + R^d gD + R^a gA behind the current face
     bool first = true;
     uint32_t qn = 0;                   // queued hits (warp-uniform); the queue always starts at index 0
@@ -160,11 +248,6 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             }
             const uint32_t hm = __ballot_sync(0xffffffffu, hit);
             if (!hm) continue;
-            float acc[19];
-            if (!POSE) {
-#pragma unroll
-                for (int jj = 0; jj < 19; ++jj) acc[jj] = 0.f;
-            }
             if (hit) {
                 const float4 r3 = R[3], r4 = R[4], r5 = R[5];
                 // transmittance in front of this face
@@ -183,94 +266,52 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
                 const float wgt = Tn * alpha;
                 const float ga = Tn * (S - Rs);                           // B2
                 Rs = alpha * S + one_m * Rs;                              // B3
-                if (POSE) {
+                {
                     // the sequential part of this hit is done; the rest (B4-B9) waits in the queue
                     const uint32_t qi = qn + (uint32_t)__popc(hm & lt);
                     sm.q_code[qi] = (uint32_t)e | ((uint32_t)lane << 8);
                     sm.q_ga[qi] = ga, sm.q_wgt[qi] = wgt, sm.q_l0[qi] = l[0], sm.q_l1[qi] = l[1], sm.q_l2[qi] = l[2];
-                } else {
-                    if (ATTR) {
-                        // B1 colours, B4 opacity (one value per face; /3 applied when written)
-                        const float w0 = o0 * z * wgt, w1 = o1 * z * wgt, w2 = o2 * z * wgt;
-                        acc[9] = w0 * gC0, acc[10] = w0 * gC1, acc[11] = w0 * gC2;
-                        acc[12] = w1 * gC0, acc[13] = w1 * gC1, acc[14] = w1 * gC2;
-                        acc[15] = w2 * gC0, acc[16] = w2 * gC1, acc[17] = w2 * gC2;
-                        acc[18] = I * ga;
-                    }
-                    if (GEOM) ts_bwd_geom<SM>(R, l, x, I, ga, wgt, z, d0, d1, d2, cg, zgd, sigma, acc);
                 }
+                (void)x, (void)I;
             }
-            if (POSE) {
-                qn += (uint32_t)__popc(hm);
-                if (qn >= 32u) {
-                    // a full group: every lane finishes one queued hit
-                    __syncwarp();
-                    const uint32_t code = sm.q_code[lane];
-                    const float qga = sm.q_ga[lane], qw = sm.q_wgt[lane], ql0 = sm.q_l0[lane], ql1 = sm.q_l1[lane], ql2 = sm.q_l2[lane];
-                    const uint32_t rest = qn - 32u;
-                    // move the remainder (< 32 entries) to the front
-                    uint32_t mc = 0;
-                    float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f, m4 = 0.f;
-                    if ((uint32_t)lane < rest) {
-                        mc = sm.q_code[32 + lane], m0 = sm.q_ga[32 + lane], m1 = sm.q_wgt[32 + lane];
-                        m2 = sm.q_l0[32 + lane], m3 = sm.q_l1[32 + lane], m4 = sm.q_l2[32 + lane];
-                    }
-                    __syncwarp();
-                    if ((uint32_t)lane < rest) {
-                        sm.q_code[lane] = mc, sm.q_ga[lane] = m0, sm.q_wgt[lane] = m1;
-                        sm.q_l0[lane] = m2, sm.q_l1[lane] = m3, sm.q_l2[lane] = m4;
-                    }
-                    qn = rest;
+            qn += (uint32_t)__popc(hm);
+            if (qn >= 32u) {
+                // a full group: every lane finishes one queued hit
+                __syncwarp();
+                const uint32_t code = sm.q_code[lane];
+                const float qga = sm.q_ga[lane], qw = sm.q_wgt[lane], ql0 = sm.q_l0[lane], ql1 = sm.q_l1[lane], ql2 = sm.q_l2[lane];
+                const uint32_t rest = qn - 32u;
+                // move the remainder (< 32 entries) to the front
+                uint32_t mc = 0;
+                float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f, m4 = 0.f;
+                if ((uint32_t)lane < rest) {
+                    mc = sm.q_code[32 + lane], m0 = sm.q_ga[32 + lane], m1 = sm.q_wgt[32 + lane];
+                    m2 = sm.q_l0[32 + lane], m3 = sm.q_l1[32 + lane], m4 = sm.q_l2[32 + lane];
+                }
+                __syncwarp();
+                if ((uint32_t)lane < rest) {
+                    sm.q_code[lane] = mc, sm.q_ga[lane] = m0, sm.q_wgt[lane] = m1;
+                    sm.q_l0[lane] = m2, sm.q_l1[lane] = m3, sm.q_l2[lane] = m4;
+                }
+                qn = rest;
+                if (POSE)
                     ts_bwd_pose_hit<SM>(sm.r[code & 0xffu], sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
-                    __syncwarp();
-                }
-            } else {
-                // reduce across the warp, then one lane issues the atomics
-                const bool single = (hm & (hm - 1)) == 0;
-                const int src = __ffs(hm) - 1;
-                if (!single) {
-                    if (GEOM) {
-#pragma unroll
-                        for (int jj = 0; jj < 9; ++jj) acc[jj] = warp_sum(acc[jj]);
-                    }
-                    if (ATTR) {
-#pragma unroll
-                        for (int jj = 9; jj < 19; ++jj) acc[jj] = warp_sum(acc[jj]);
-                    }
-                }
-                if (lane == src) {
-                    if (GEOM) {
-                        float* gs = f.gscr + 9 * (size_t)sm.slot[e];
-#pragma unroll
-                        for (int jj = 0; jj < 9; ++jj) atomicAdd(gs + jj, acc[jj]);
-                    }
-                    if (ATTR) {
-                        const uint32_t m = sm.face[e];
-                        uint32_t v[3];
-#pragma unroll
-                        for (int k = 0; k < 3; ++k) v[k] = sc.faces ? (uint32_t)__ldg(sc.faces + 3 * (size_t)m + k) : 3u * m + k;
-                        if (grad_color) {
-#pragma unroll
-                            for (int k = 0; k < 3; ++k)
-#pragma unroll
-                                for (int ch = 0; ch < 3; ++ch) atomicAdd(grad_color + 3 * (size_t)v[k] + ch, acc[9 + 3 * k + ch]);
-                        }
-                        if (grad_opacity) {
-                            const float go = acc[18] * (1.0f / 3.0f);
-#pragma unroll
-                            for (int k = 0; k < 3; ++k) atomicAdd(grad_opacity + v[k], go);
-                        }
-                    }
-                }
+                else
+                    ts_bwd_full_group<SM, ATTR, GEOM>(f, sc, sm, lane, true, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
+                __syncwarp();
             }
         }
-        if (POSE && qn) {
+        if (qn) {
             // the staged records are about to be replaced: finish what is still queued (partial group)
             __syncwarp();
-            if ((uint32_t)lane < qn) {
-                const uint32_t code = sm.q_code[lane];
-                ts_bwd_pose_hit<SM>(sm.r[code & 0xffu], sm.pix[code >> 8], sm.q_l0[lane], sm.q_l1[lane], sm.q_l2[lane],
-                                    sm.q_ga[lane], sm.q_wgt[lane], fx, fy, sigma, tau);
+            const bool act = (uint32_t)lane < qn;
+            const uint32_t code = act ? sm.q_code[lane] : 0u;
+            const float qga = act ? sm.q_ga[lane] : 0.f, qw = act ? sm.q_wgt[lane] : 0.f;
+            const float ql0 = act ? sm.q_l0[lane] : 0.f, ql1 = act ? sm.q_l1[lane] : 0.f, ql2 = act ? sm.q_l2[lane] : 0.f;
+            if (POSE) {
+                if (act) ts_bwd_pose_hit<SM>(sm.r[code & 0xffu], sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
+            } else {
+                ts_bwd_full_group<SM, ATTR, GEOM>(f, sc, sm, lane, act, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
             }
             qn = 0;
             __syncwarp();
