@@ -243,8 +243,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             bool hit = false;
             {
                 const float4 r0 = R[0], r1 = R[1], r2 = R[2];
-                const float4* s4 = f.scr + TS_SCR_F4 * (size_t)sm.slot[e];
-                hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, s4, l, x, I, alpha);
+                hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, &sm.slot[e], l, x, I, alpha);
             }
             const uint32_t hm = __ballot_sync(0xffffffffu, hit);
             if (!hm) continue;
