@@ -31,6 +31,22 @@ __device__ __forceinline__ void project_face(const float* p, const float* T, con
     o.vis = false;
     o.tiles = 0;
     if (!(Z[0] > cam.znear) || !(Z[1] > cam.znear) || !(Z[2] > cam.znear)) return;   // F2 (NaN culls)
+    // Conservative frustum pre-cull (most of the map is outside the view): if all three vertices are more than two
+    // pixels beyond the same image border -- decided without a division, with a margin ~1000x the rounding error of
+    // these expressions -- the exact path below would find an empty pixel rect (F5) and cull the face as well, so
+    // skipping it cannot change any result.
+    {
+        const float ax = cam.cx + 2.0f, bx = cam.cx - (float)(cam.W + 1), ay = cam.cy + 2.0f, by = cam.cy - (float)(cam.H + 1);
+        bool l = true, r = true, t = true, b = true;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            l = l && (cam.fx * X[k] + ax * Z[k] < 0.0f);      // u_k < -2
+            r = r && (cam.fx * X[k] + bx * Z[k] > 0.0f);      // u_k > W + 1
+            t = t && (cam.fy * Y[k] + ay * Z[k] < 0.0f);      // v_k < -2
+            b = b && (cam.fy * Y[k] + by * Z[k] > 0.0f);      // v_k > H + 1
+        }
+        if (l || r || t || b) return;
+    }
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
         o.w[k] = __fdiv_rn(1.0f, Z[k]);                                               // N2
@@ -100,6 +116,17 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
     FaceOut o;
     o.vis = false, o.tiles = 0;
     if (tid < n_here) project_face(p, sT, cam, eps_area, o);
+    // mean vertex opacity of the survivors: requested now, so that its round trip overlaps the slot atomic
+    float ob = 0.0f;
+    if (o.vis) {
+        const int64_t m = face0 + tid;
+        if (SOUP) {
+            ob = (__ldg(opacity + 3 * m) + __ldg(opacity + 3 * m + 1) + __ldg(opacity + 3 * m + 2)) * (1.0f / 3.0f);
+        } else {
+            ob = (__ldg(opacity + __ldg(faces + 3 * m)) + __ldg(opacity + __ldg(faces + 3 * m + 1)) +
+                  __ldg(opacity + __ldg(faces + 3 * m + 2))) * (1.0f / 3.0f);
+        }
+    }
 
     // slot allocation: warp ballot -> CTA total -> one global atomic per CTA
     const uint32_t bal = __ballot_sync(0xffffffffu, o.vis);
@@ -120,14 +147,6 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
         const uint32_t slot = s_base + s_w[warp] + __popc(bal & ((1u << lane) - 1u));
         if (slot < f.vis_cap) {
             const uint32_t m = (uint32_t)(face0 + tid);
-            float ob;                                            // mean vertex opacity
-            if (SOUP) {
-                ob = (__ldg(opacity + 3 * (int64_t)m) + __ldg(opacity + 3 * (int64_t)m + 1) +
-                      __ldg(opacity + 3 * (int64_t)m + 2)) * (1.0f / 3.0f);
-            } else {
-                ob = (__ldg(opacity + __ldg(faces + 3 * (int64_t)m)) + __ldg(opacity + __ldg(faces + 3 * (int64_t)m + 1)) +
-                      __ldg(opacity + __ldg(faces + 3 * (int64_t)m + 2))) * (1.0f / 3.0f);
-            }
             const int rlo = (o.x0 & 0xffff) | (o.y0 << 16), rhi = (o.x1 & 0xffff) | (o.y1 << 16);
             float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
             s4[0] = make_float4(o.u[0], o.v[0], o.w[0], o.u[1]);

@@ -18,28 +18,37 @@
 
 namespace {
 
+// a CTA or a warp-aligned part of one, with its own barrier (0 = the CTA barrier, else a named barrier)
+struct TsGroup {
+    int tid, n, bar;
+    __device__ __forceinline__ void sync() const {
+        if (bar == 0) __syncthreads();
+        else asm volatile("bar.sync %0, %1;" ::"r"(bar), "r"(n) : "memory");
+    }
+};
+
 // exclusive scan of tile_count[0..NT) by one CTA, in place in `offs` (shared memory, or global for the fallback).
 // Pass 1 copies the counts with coalesced loads (every binning CTA does this at the same time: strided loads would
 // multiply the L2 requests on the few slices that hold the 13 KB of counts); pass 2 gives every thread a contiguous
 // run of tiles (stride `per` words: conflict-free for odd `per`).  Returns the total and the longest list.
 __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* offs, uint32_t* s_tmp /*[2*warps+2]*/,
-                                               uint32_t& total, uint32_t& gmax) {
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarp = blockDim.x >> 5;
-    for (int base = 0; base < f.NT; base += 8 * (int)blockDim.x) {      // 8 independent loads in flight per thread
+                                               uint32_t& total, uint32_t& gmax, const TsGroup g) {
+    const int tid = g.tid, lane = tid & 31, warp = tid >> 5, nwarp = g.n >> 5, nthr = g.n;
+    for (int base = 0; base < f.NT; base += 8 * nthr) {      // 8 independent loads in flight per thread
         uint32_t c[8];
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            const int t = base + k * (int)blockDim.x + tid;
+            const int t = base + k * nthr + tid;
             c[k] = t < f.NT ? __ldcg(f.tile_count + t) : 0u;
         }
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
-            const int t = base + k * (int)blockDim.x + tid;
+            const int t = base + k * nthr + tid;
             if (t < f.NT) offs[t] = c[k];
         }
     }
-    __syncthreads();
-    const int per = ((f.NT + (int)blockDim.x - 1) / (int)blockDim.x) | 1;
+    g.sync();
+    const int per = ((f.NT + nthr - 1) / nthr) | 1;
     const int t0 = min(f.NT, tid * per), t1 = min(f.NT, t0 + per);
     uint32_t sum = 0, mx = 0;
     for (int t = t0; t < t1; ++t) {
@@ -55,7 +64,7 @@ __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* of
     mx = __reduce_max_sync(0xffffffffu, mx);
     if (lane == 31) s_tmp[warp] = incl;
     if (lane == 0) s_tmp[nwarp + warp] = mx;
-    __syncthreads();
+    g.sync();
     if (warp == 0) {                                            // warp totals -> exclusive warp offsets, total, max
         const uint32_t c = lane < nwarp ? s_tmp[lane] : 0u;
         uint32_t m2 = lane < nwarp ? s_tmp[nwarp + lane] : 0u, in2 = c;
@@ -68,7 +77,7 @@ __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* of
         if (lane < nwarp) s_tmp[lane] = in2 - c;
         if (lane == 31) s_tmp[2 * nwarp] = in2, s_tmp[2 * nwarp + 1] = m2;
     }
-    __syncthreads();
+    g.sync();
     const uint32_t woff = s_tmp[warp];
     total = s_tmp[2 * nwarp], gmax = s_tmp[2 * nwarp + 1];
     uint32_t run = woff + incl - sum;
@@ -77,26 +86,26 @@ __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* of
         offs[t] = run;
         run += c;
     }
-    __syncthreads();
+    g.sync();
 }
 
 // CTA 0 only: tile_ranges, frame counters, and the tile order (descending log2 bucket of the list length) that
 // the persistent render kernels pull work in.  Counts are recovered from the offsets (no second trip to memory).
 __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_t* offs, uint32_t nv, uint32_t total,
-                                              uint32_t gmax, uint32_t fl, uint32_t* s_hist /*[34]*/) {
-    const int tid = threadIdx.x;
+                                              uint32_t gmax, uint32_t fl, uint32_t* s_hist /*[34]*/, const TsGroup g) {
+    const int tid = g.tid;
     if (tid < 34) s_hist[tid] = 0;
-    __syncthreads();
-    for (int t = tid; t < f.NT; t += blockDim.x) {
+    g.sync();
+    for (int t = tid; t < f.NT; t += g.n) {
         const uint32_t o = offs[t], c = (t + 1 < f.NT ? offs[t + 1] : total) - o;
         f.tile_ranges[t] = (fl || c == 0u) ? make_uint2(0u, 0u) : make_uint2(o, o + c);   // empty tile = (0,0)
         // bucket 0 = empty, b = floor(log2 c) + 1; only ~10 buckets are in use, so the histogram is aggregated per
         // warp (match) before it touches shared memory: one atomic per (warp, bucket), not 32-way conflicts
         const int b = 32 - __clz(c);
         const uint32_t peers = __match_any_sync(__activemask(), b);
-        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&s_hist[b], (uint32_t)__popc(peers));
+        if ((int)(tid & 31) == __ffs(peers) - 1) atomicAdd(&s_hist[b], (uint32_t)__popc(peers));
     }
-    __syncthreads();
+    g.sync();
     if (tid == 0) {
         uint32_t run = 0;
         for (int b = 32; b >= 0; --b) {                        // heaviest bucket first
@@ -107,12 +116,12 @@ __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_
         volatile TsCtrl* ctrl = f.ctrl;
         ctrl->n_visible = nv, ctrl->n_pairs = total, ctrl->flags = fl, ctrl->max_list = gmax;
     }
-    __syncthreads();
-    for (int t = tid; t < f.NT; t += blockDim.x) {
+    g.sync();
+    for (int t = tid; t < f.NT; t += g.n) {
         const uint32_t c = (t + 1 < f.NT ? offs[t + 1] : total) - offs[t];
         const int b = 32 - __clz(c);
         const uint32_t act = __activemask(), peers = __match_any_sync(act, b);
-        const int leader = __ffs(peers) - 1, lane = threadIdx.x & 31;
+        const int leader = __ffs(peers) - 1, lane = tid & 31;
         uint32_t base = 0;
         if (lane == leader) base = atomicAdd(&s_hist[b], (uint32_t)__popc(peers));
         base = __shfl_sync(act, base, leader);
@@ -128,13 +137,16 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(TsFrameDev f) {
     __shared__ uint32_t s_tmp[66];
     __shared__ uint32_t s_hist[34];
     uint32_t total, gmax;
-    cta_scan_tiles(f, f.tile_offset, s_tmp, total, gmax);
+    const TsGroup g{(int)threadIdx.x, (int)blockDim.x, 0};
+    cta_scan_tiles(f, f.tile_offset, s_tmp, total, gmax, g);
     const uint32_t nv = *(volatile uint32_t*)&f.ctrl->vis_counter;
     uint32_t fl = 0;
     if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
     if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
-    publish_tiles(f, f.tile_offset, nv, total, gmax, fl, s_hist);
+    publish_tiles(f, f.tile_offset, nv, total, gmax, fl, s_hist, g);
 }
+
+#define TS_BIN_SCAN_WARPS 8          // warps of a binning CTA that scan the tile counts while the others set faces up
 
 template <bool LOCAL>
 __global__ void __launch_bounds__(TS_BIN_THREADS)
@@ -142,38 +154,39 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
     __shared__ uint32_t s_offs[LOCAL ? TS_SCAN_LOCAL_MAX : 1];
     __shared__ uint32_t s_tmp[2 * (TS_BIN_THREADS / 32) + 2];
     __shared__ uint32_t s_hist[34];
-    const int lane = threadIdx.x & 31;
-    // This kernel is one wave of dependent round trips, so they are kept few: the raw records of this thread's
-    // first slot are requested before anything else (speculatively: slot < n_visible is not known yet) and fly
-    // while the CTA scans the tile counts.
-    // slots are dealt to the grid warp by warp, so that the n_visible live ones spread over all SMs
-    uint32_t slot = ((threadIdx.x >> 5) * gridDim.x + blockIdx.x) * 32u + (threadIdx.x & 31);
+    __shared__ uint32_t s_tot[2];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // This kernel is one wave of dependent round trips, so they are kept few and overlapped: the last
+    // TS_BIN_SCAN_WARPS warps scan the tile counts (the scatter needs the offsets) while the other warps fetch their
+    // first raw records (speculatively: n_visible arrives with them) and build the render records, which need no
+    // offset.  Slots are dealt to the grid warp by warp, so that the live ones spread over all SMs.
+    constexpr int SLOT_WARPS = LOCAL ? TS_BIN_THREADS / 32 - TS_BIN_SCAN_WARPS : TS_BIN_THREADS / 32;
+    const bool scanner = LOCAL && warp >= SLOT_WARPS;
+    const TsGroup sg{(int)threadIdx.x - SLOT_WARPS * 32, TS_BIN_SCAN_WARPS * 32, 1};
+    const uint32_t stride = gridDim.x * SLOT_WARPS * 32u;
+    uint32_t slot = ((uint32_t)warp * gridDim.x + blockIdx.x) * 32u + (uint32_t)lane;
     float4 s0, s1, s2, s3;
     s0 = s1 = s2 = s3 = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (slot < f.vis_cap) {
+    uint32_t nv = 0, fl = 0, total = 0, gmax = 0;
+    const uint32_t* offs = s_offs;
+    if (scanner) {
+        cta_scan_tiles(f, s_offs, s_tmp, total, gmax, sg);
+        if (sg.tid == 0) s_tot[0] = total, s_tot[1] = gmax;
+    } else if (slot < f.vis_cap) {
         const float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
         s0 = __ldcg(s4), s1 = __ldcg(s4 + 1), s2 = __ldcg(s4 + 2), s3 = __ldcg(s4 + 3);
     }
-    uint32_t nv, fl;
-    const uint32_t* offs;
     if (LOCAL) {
-        uint32_t total, gmax;
         nv = __ldcg(&f.ctrl->vis_counter);
-        cta_scan_tiles(f, s_offs, s_tmp, total, gmax);
-        fl = 0;
-        if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
-        if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
-        if (blockIdx.x == gridDim.x - 1) publish_tiles(f, s_offs, nv, total, gmax, fl, s_hist);   // the last CTA has the fewest slots
-        offs = s_offs;
     } else {
         const volatile TsCtrl* ctrl = f.ctrl;
         nv = ctrl->n_visible, fl = ctrl->flags;
         offs = f.tile_offset;
     }
-    const uint32_t nvis = fl ? 0u : nv;
-    const uint32_t n_round = (nvis + TS_BIN_THREADS - 1) / TS_BIN_THREADS * TS_BIN_THREADS;
-    while (slot < n_round) {
-        const bool live = slot < nvis;
+    const uint32_t nlive = min(nv, f.vis_cap);
+    bool synced = !LOCAL;
+    for (;; slot += stride) {
+        const bool live = !scanner && slot < nlive;
         int tx0 = 0, ty0 = 0, ntx = 0, nty = 0;
         uint4 pa = make_uint4(0u, 0u, slot, 0u);
         uint32_t pb = 0;
@@ -189,7 +202,23 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
             pa = make_uint4(__float_as_uint(s3.y), __float_as_uint(s3.x), slot, (uint32_t)rlo);
             pb = (uint32_t)rhi;
         }
-        const int nt = ntx * nty;
+        if (!synced) {
+            // the offsets are ready from here on; the scan warps of the last CTA (it has the fewest slots) go on to
+            // publish the tile ranges, the frame counters and the job headers, the others are done
+            __syncthreads();
+            synced = true;
+            total = s_tot[0], gmax = s_tot[1];
+            if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
+            if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
+            if (scanner) {
+                if (blockIdx.x == gridDim.x - 1) publish_tiles(f, s_offs, nv, total, gmax, fl, s_hist, sg);
+                return;
+            }
+        }
+        const uint32_t nvis = fl ? 0u : nlive;                 // an overflowed frame bins nothing
+        const uint32_t n_round = (nvis + 31u) & ~31u;
+        if (slot >= n_round) break;                            // warp-uniform
+        const int nt = (fl || !live) ? 0 : ntx * nty;
         // narrow faces (the common case): the owning lane scatters its <= 4 pairs itself; the cursor atomics are
         // issued together so that they cost one round trip, not four
         {
@@ -244,9 +273,8 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
                 }
             }
         }
-        slot += gridDim.x * TS_BIN_THREADS;
-        if (slot < nvis) {
-            const float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
+        if (slot + stride < nvis) {
+            const float4* s4 = f.scr + TS_SCR_F4 * (size_t)(slot + stride);
             s0 = __ldcg(s4), s1 = __ldcg(s4 + 1), s2 = __ldcg(s4 + 2), s3 = __ldcg(s4 + 3);
         }
     }
