@@ -162,15 +162,16 @@ def test_determinism(ctx, oracle_mod):
     assert np.allclose(outs[0][6], outs[1][6], rtol=1e-4, atol=1e-4 * np.abs(outs[0][6]).max())
 
 
-@pytest.mark.parametrize("cfg", [2, 4])
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
 def test_full_size_configs(ctx, oracle_mod, cfg):
-    """BASELINE.json sizes (500k faces tracking frame; 2M faces stress) through the tiled oracle, as bench.py runs them."""
+    """BASELINE.json sizes (100k / 500k faces tracking frames; one view of the 1M-face mapping step; 2M faces stress)
+    through the tiled oracle, in the launch configuration bench.py times."""
     from test_gpu_parity import both, check_backward, check_forward, check_project_and_sort
     from paper_2605_31419_b200 import ts
     sc = scenes.make_config(cfg)
     o, g = both(ctx, oracle_mod, sc, pair_capacity=2 * sc.M)
     check_project_and_sort(o, g, sc.M)
     f, ok = check_forward(o, g)
-    masks = [ts.GRAD_POSE] if cfg == 2 else [ts.GRAD_ALL]
+    masks = [ts.GRAD_POSE] if cfg in (1, 2) else [ts.GRAD_ALL]
     check_backward(o, g, ok, 40 + cfg, masks)
     g.close()

@@ -265,3 +265,34 @@ def test_render_track_l1_equals_separate_calls(ctx, oracle_mod, cfg):
     with pytest.raises(ts.TsError):
         ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, None, None, None, ts.GRAD_POSE)   # no walk state after track
     g.close()
+
+
+def test_mapping_step_accumulates_over_views(ctx, oracle_mod):
+    """Config-3 recipe at a small size: one mapping step = fwd+bwd over the keyframes, per-vertex gradients
+    ACCUMULATED (+=) over the views into the same buffers; compared with the sum of the oracle's."""
+    from gpu_util import GpuView, assert_grad_close, dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(3)
+    V = sc.pos.shape[0]
+    gp, gc, go = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+    ref_p, ref_c, ref_o = np.zeros((V, 3)), np.zeros((V, 3)), np.zeros(V)
+    rng = np.random.default_rng(33)
+    for view in range(len(sc.T_start)):
+        T = sc.T_start[view]
+        o = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, None, T, sc.cam, sc.params, "f32", amb_tol=5e-3)
+        g = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, T, sc.cam, sc.params)
+        f, ok = check_forward(o, g)
+        H, W = ok.shape
+        gC = (rng.normal(size=(3, H, W)) * ok[None]).astype(np.float32)
+        gD = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+        ref = o.backward(gC, gD, None)
+        ref_p += ref.grad_pos
+        ref_c += ref.grad_color
+        ref_o += ref.grad_opacity
+        ts.ts_render_bwd(ctx, g.scene, g.frame, dev(gC), dev(gD), None, gp, gc, go,
+                         ts.GRAD_POS | ts.GRAD_COLOR | ts.GRAD_OPACITY)
+        torch.cuda.synchronize()
+        g.close()
+    assert_grad_close("grad_pos", gp.cpu().numpy(), ref_p)
+    assert_grad_close("grad_color", gc.cpu().numpy(), ref_c)
+    assert_grad_close("grad_opacity", go.cpu().numpy(), ref_o)
