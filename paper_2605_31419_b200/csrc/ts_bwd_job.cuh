@@ -24,11 +24,11 @@ __device__ __forceinline__ float warp_sum(float v) {
 // (rows as in BwdWarpSmem::r), l = lhat_k, x = -max l, I = x^sigma, ga = dL/dalpha, wgt = T alpha,
 // z, d_k = c_k.gC, cg = c.gC, zgd = z gD.  Outputs g[9] = dL/d(u0,v0,w0,u1,v1,w1,u2,v2,w2).
 template <int SM>
-__device__ __forceinline__ void ts_bwd_geom(const float4* R, const float l[3], float x, float I, float ga, float wgt,
+__device__ __forceinline__ void ts_bwd_geom(const BwdWarpSmem& sm, uint32_t e, const float l[3], float x, float I, float ga, float wgt,
                                             float z, float d0, float d1, float d2, float cg, float zgd, float sigma,
                                             float g[9]) {
-    const float4 r0 = R[0], r1 = R[1], r2 = R[2];
-    const float4 q4 = R[6], q5 = R[7], q6 = R[8], q7 = R[9];   // record rows R4..R7
+    const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
+    const float4 q4 = sm.r[e][6], q5 = sm.r[e][7], q6 = sm.r[e][8], q7 = sm.r[e][9];   // record rows R4..R7
     // B4 window: gx = dL/dx
     const float gI = r2.w * ga;
     float gx;
@@ -67,9 +67,9 @@ __device__ __forceinline__ void ts_bwd_geom(const float4* R, const float l[3], f
 // (Eq. 5-7): with Q = (xn, yn, 1)/w,  Z g_C = (a, b, c),  a = fx gu, b = fy gv, c = -(xn a + yn b) - w gw;
 // rho += w (a,b,c);  theta += Q x g_C.
 template <int SM>
-__device__ __forceinline__ void ts_bwd_pose_hit(const float4* R, const float4 pg, float l0, float l1, float l2, float ga,
+__device__ __forceinline__ void ts_bwd_pose_hit(const BwdWarpSmem& sm, uint32_t e, const float4 pg, float l0, float l1, float l2, float ga,
                                                 float wgt, float fx, float fy, float sigma, float tau[6]) {
-    const float4 r3 = R[3], r4 = R[4], r5 = R[5];
+    const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
     const float l[3] = {l0, l1, l2};
     const float x = -fmaxf(l0, fmaxf(l1, l2));
     const float I = ts_window_pow<SM>(x, sigma);
@@ -80,8 +80,8 @@ __device__ __forceinline__ void ts_bwd_pose_hit(const float4* R, const float4 pg
     const float d2 = r5.y * pg.x + r5.z * pg.y + r5.w * pg.z;
     const float cg = (o0 * d0 + o1 * d1 + o2 * d2) * z;
     float g[9];
-    ts_bwd_geom<SM>(R, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sigma, g);
-    const float4 q5 = R[7], n0 = R[10], n1 = R[11];
+    ts_bwd_geom<SM>(sm, e, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sigma, g);
+    const float4 q5 = sm.r[e][7], n0 = sm.r[e][10], n1 = sm.r[e][11];
     {
         const float a = fx * g[0], b = fy * g[1], c = -(n0.x * a + n0.y * b) - q5.x * g[2];
         tau[0] += q5.x * a, tau[1] += q5.x * b, tau[2] += q5.x * c;
@@ -113,9 +113,8 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
 #pragma unroll
     for (int j = 0; j < 19; ++j) acc[j] = 0.f;
     if (active) {
-        const float4* R = sm.r[e];
         const float4 pg = sm.pix[code >> 8];
-        const float4 r3 = R[3], r4 = R[4], r5 = R[5];
+        const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
         const float l[3] = {l0, l1, l2};
         const float x = -fmaxf(l0, fmaxf(l1, l2));
         const float I = ts_window_pow<SM>(x, sigma);
@@ -134,7 +133,7 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
             const float d1 = r4.z * pg.x + r4.w * pg.y + r5.x * pg.z;
             const float d2 = r5.y * pg.x + r5.z * pg.y + r5.w * pg.z;
             const float cg = (o0 * d0 + o1 * d1 + o2 * d2) * z;
-            ts_bwd_geom<SM>(R, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sigma, acc);
+            ts_bwd_geom<SM>(sm, e, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sigma, acc);
         }
     }
     // segmented reduction over runs of equal staged index (inactive lanes never match anybody)
@@ -238,17 +237,16 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             ov &= ~(1u << e);
             const bool in_rect = lo + (uint32_t)e < ncon && ((sm.lm[e] >> lane) & 1u);
             if (!__any_sync(0xffffffffu, in_rect)) continue;
-            const float4* R = sm.r[e];
             float l[3], x, I, alpha;
             bool hit = false;
             {
-                const float4 r0 = R[0], r1 = R[1], r2 = R[2];
-                hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, &sm.slot[e], l, x, I, alpha);
+                const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
+                hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
             }
             const uint32_t hm = __ballot_sync(0xffffffffu, hit);
             if (!hm) continue;
             if (hit) {
-                const float4 r3 = R[3], r4 = R[4], r5 = R[5];
+                const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
                 // transmittance in front of this face
                 const float one_m = __fsub_rn(1.0f, alpha);
                 const float Tn = first ? Tcur : Tcur * ts_rcp_approx(one_m);
@@ -294,7 +292,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
                 }
                 qn = rest;
                 if (POSE)
-                    ts_bwd_pose_hit<SM>(sm.r[code & 0xffu], sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
+                    ts_bwd_pose_hit<SM>(sm, code & 0xffu, sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
                 else
                     ts_bwd_full_group<SM, ATTR, GEOM>(f, sc, sm, lane, true, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
                 __syncwarp();
@@ -308,7 +306,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             const float qga = act ? sm.q_ga[lane] : 0.f, qw = act ? sm.q_wgt[lane] : 0.f;
             const float ql0 = act ? sm.q_l0[lane] : 0.f, ql1 = act ? sm.q_l1[lane] : 0.f, ql2 = act ? sm.q_l2[lane] : 0.f;
             if (POSE) {
-                if (act) ts_bwd_pose_hit<SM>(sm.r[code & 0xffu], sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
+                if (act) ts_bwd_pose_hit<SM>(sm, code & 0xffu, sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
             } else {
                 ts_bwd_full_group<SM, ATTR, GEOM>(f, sc, sm, lane, act, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
             }

@@ -60,7 +60,7 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             if (!__any_sync(0xffffffffu, in_rect)) continue;
             const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
             float l[3], x, I, alpha;
-            const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, &sm.slot[e], l, x, I, alpha);
+            const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
             if (!__any_sync(0xffffffffu, hit)) continue;
             if (hit) {
                 const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];

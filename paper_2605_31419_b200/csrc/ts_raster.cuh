@@ -145,11 +145,9 @@ __host__ __device__ inline int ts_sigma_mode(float sigma) {
 // compensated 2x2 determinant (N6), which is accurate to a few ulp relative, like the oracle's.
 #define TS_REFINE_BAND 1e-3f
 
-// scr = the frame's raw screen records, slot_ptr = where the face's slot is kept (shared memory): the address is
-// formed here, on the rare path, not on every visit
-static __device__ __noinline__ float3 ts_refine_lhat(const float4* __restrict__ scr, const uint32_t* slot_ptr, float px,
-                                                     float py) {
-    const float4* s4 = scr + TS_SCR_F4 * (size_t)(*slot_ptr);
+// scr = the frame's raw screen records, slot = the face's slot: the record address is formed here, on the rare path
+static __device__ __noinline__ float3 ts_refine_lhat(const float4* __restrict__ scr, uint32_t slot, float px, float py) {
+    const float4* s4 = scr + TS_SCR_F4 * (size_t)slot;
     const float4 s0 = __ldg(s4), s1 = __ldg(s4 + 1);
     const float qx[3] = {s0.x, s0.w, s1.z}, qy[3] = {s0.y, s1.x, s1.w};
     const float a = __fsub_rn(qx[1], qx[0]), b = __fsub_rn(qy[2], qy[0]);
@@ -175,11 +173,11 @@ static __device__ __noinline__ float3 ts_refine_lhat(const float4* __restrict__ 
 }
 
 // F8.1-3.  Returns true if the face contributes at (px,py); l[] = lhat_k, x, I, alpha are outputs.
-// r0..r2 = record rows R0-R2; scr / slot_ptr locate the face's raw screen record (only read inside the refinement band).
+// r0..r2 = record rows R0-R2; scr / slot locate the face's raw screen record (only read inside the refinement band).
 template <int SM>
 __device__ __forceinline__ bool ts_eval_alpha(const float4 r0, const float4 r1, const float4 r2, float px, float py,
                                               float sigma, float alpha_min, const float4* __restrict__ scr,
-                                              const uint32_t* slot_ptr, float l[3],
+                                              uint32_t slot, float l[3],
                                               float& x, float& I, float& alpha) {
     const float dx = __fsub_rn(px, r0.x), dy = __fsub_rn(py, r0.y);
     l[0] = __fmaf_rn(r0.z, dx, __fmaf_rn(r0.w, dy, r2.x));
@@ -187,7 +185,7 @@ __device__ __forceinline__ bool ts_eval_alpha(const float4 r0, const float4 r1, 
     l[2] = __fmaf_rn(r1.z, dx, __fmaf_rn(r1.w, dy, r2.z));
     x = -fmaxf(l[0], fmaxf(l[1], l[2]));
     if (fabsf(x) < TS_REFINE_BAND) {
-        const float3 lr = ts_refine_lhat(scr, slot_ptr, px, py);
+        const float3 lr = ts_refine_lhat(scr, slot, px, py);
         l[0] = lr.x, l[1] = lr.y, l[2] = lr.z;
         x = -fmaxf(l[0], fmaxf(l[1], l[2]));
     }
