@@ -259,6 +259,50 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
     if (counters) counters[0] = n_visit, counters[1] = n_rect, counters[2] = n_hit, counters[3] = 0;
 }
 
+// ---------------------------------------------------------------------------------- per-face statistics
+// What the map-management layer of the paper reads off a render (not part of Eq. 1-4): for every face the number of
+// pixels it contributed to (the "rendered" flag of the covisibility IoU; the pixel coverage of the
+// blur-split test) and its projected area in px^2 (prune test area > eps_a).
+// Same walk as render_fwd (same hit rule, same termination); area = |S| / 2 with S of F4.
+template <class T>
+void face_stats(const T* color, const T* opacity, const int32_t* faces, int32_t M, const tso_camera* cam_,
+                const tso_params* prm, const uint8_t* visible, const int16_t* rect, const T* scr, const uint32_t* list,
+                int64_t n_list, const uint32_t* tile_ranges, uint32_t* face_pixels, T* proj_area) {
+    const Cam<T> cam(cam_);
+    const int W = cam.W, H = cam.H;
+    const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min;
+    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr);
+    Lists<T> LS{list, n_list, tile_ranges, (W + 15) / 16};
+    for (int m = 0; m < M; ++m) {
+        if (face_pixels) face_pixels[m] = 0;
+        if (proj_area) {
+            proj_area[m] = 0;
+            if (visible[m]) {
+                const T* q = scr + 9 * (int64_t)m;                   // (u,v,w) x 3
+                const T a = q[3] - q[0], b = q[7] - q[1], c = q[4] - q[1], d = q[6] - q[0];
+                const T S = std::fma(a, b, -(c * d));                // F4 / N3
+                proj_area[m] = (T)0.5 * std::fabs(S);
+            }
+        }
+    }
+    if (!face_pixels) return;
+    for (int y = 0; y < H; ++y)
+        for (int x = 0; x < W; ++x) {
+            int64_t b, e;
+            LS.span(x, y, b, e);
+            T Tr = 1;
+            for (int64_t i = b; i < e; ++i) {
+                const Face<T>& f = F[list[i]];
+                if (x < f.x0 || x > f.x1 || y < f.y0 || y > f.y1) continue;
+                Hit<T> h;
+                if (!eval(f, (T)x, (T)y, sigma, amin, (T)0, h, nullptr)) continue;
+                face_pixels[list[i]] += 1;
+                Tr = Tr * ((T)1 - h.alpha);
+                if (Tr <= tmin) break;
+            }
+        }
+}
+
 // ---------------------------------------------------------------------------------- B1..B6
 template <class T>
 void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t M, const tso_camera* cam_,
@@ -556,5 +600,18 @@ void tso_pose_step_f32(float* T_cw, const float* g, float* state, const float* l
 }
 
 void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out) { left_perturb<double>(T_cw, tau, out); }
+
+void tso_face_stats_f32(const float* color, const float* opacity, const int32_t* faces, int32_t M, const tso_camera* cam,
+                        const tso_params* prm, const uint8_t* visible, const int16_t* rect, const float* scr,
+                        const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, uint32_t* face_pixels,
+                        float* proj_area) {
+    face_stats<float>(color, opacity, faces, M, cam, prm, visible, rect, scr, list, n_list, tile_ranges, face_pixels, proj_area);
+}
+void tso_face_stats_f64(const double* color, const double* opacity, const int32_t* faces, int32_t M, const tso_camera* cam,
+                        const tso_params* prm, const uint8_t* visible, const int16_t* rect, const double* scr,
+                        const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, uint32_t* face_pixels,
+                        double* proj_area) {
+    face_stats<double>(color, opacity, faces, M, cam, prm, visible, rect, scr, list, n_list, tile_ranges, face_pixels, proj_area);
+}
 
 }  // extern "C"

@@ -109,6 +109,18 @@ double tso_l1_loss_f64(int32_t W, int32_t H, const double* C, const double* D, c
 void tso_pose_step_f32(float* T_cw, const float* dL_dtau, float* state, const float* lr, float beta1, float beta2,
                        float eps);
 
+/* Per-face statistics of a render (map management): face_pixels[M] = number of pixels the
+ * face contributed to (same walk, hit rule and termination as tso_render_fwd); proj_area[M] = |S|/2 in px^2 (F4),
+ * 0 for culled faces.  Either output may be NULL. */
+void tso_face_stats_f32(const float* color, const float* opacity, const int32_t* faces, int32_t M, const tso_camera* cam,
+                        const tso_params* prm, const uint8_t* visible, const int16_t* rect, const float* scr,
+                        const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, uint32_t* face_pixels,
+                        float* proj_area);
+void tso_face_stats_f64(const double* color, const double* opacity, const int32_t* faces, int32_t M, const tso_camera* cam,
+                        const tso_params* prm, const uint8_t* visible, const int16_t* rect, const double* scr,
+                        const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, uint32_t* face_pixels,
+                        double* proj_area);
+
 /* SE(3) exponential, tau = (rho, theta): out[12] = Exp(tau) o T (3x4 row-major). */
 void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out);
 

@@ -156,6 +156,17 @@ class Oracle:
             _p(o.depth), _p(o.alpha), _p(o.n_contrib), _p(o.ambig), _p(o.sig), _p(o.counters))
         return o
 
+    def face_stats(self, mode="tiled"):
+        """Per-face pixel counts and projected areas of this view."""
+        pr = self.project()
+        lst, ranges = self._lists(mode)
+        o = SimpleNamespace(face_pixels=np.zeros(self.M, np.uint32), proj_area=np.zeros(self.M, self.dt))
+        self._fn("tso_face_stats")(
+            _p(self.color), _p(self.opacity), _p(self.faces), C.c_int32(self.M), C.byref(self.cam), C.byref(self.prm),
+            _p(pr.visible), _p(pr.rect), _p(pr.scr), _p(lst), C.c_int64(lst.shape[0]), _p(ranges), _p(o.face_pixels),
+            _p(o.proj_area))
+        return o
+
     # ------------------------------------------------------------------ B1-B9
     def backward(self, gC=None, gD=None, gA=None, mode="tiled", want=("pos", "color", "opacity", "pose")):
         pr = self.project()
