@@ -129,6 +129,16 @@ int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, fl
 int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
                            float* out_alpha, const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD,
                            float* loss_dev, void* stream);
+/* Per-face statistics for the map-management layer (PAPER.md:137 covisibility of rendered faces,
+ * :169 prune by projected area, :175 blur-split by pixel coverage).
+ * ts_render_fwd_stats: as ts_render_fwd, and face_pixels[m] += number of pixels face m contributed to (caller zeroes;
+ * a face is "rendered" iff its count is non-zero).  out_* may be NULL.
+ * ts_face_area: proj_area[m] = |S|/2 in px^2 for every face that survived the last ts_project (other entries are
+ * left untouched: zero the array first). */
+int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
+                            float* out_alpha, uint32_t* face_pixels, void* stream);
+int32_t ts_face_area(ts_ctx* ctx, ts_frame* frame, float* proj_area, void* stream);
+
 /* a8: one Adam step on tau, then T_cw <- Exp(-delta) o T_cw, all on the device.
  * state_dev[13] = m[6], v[6], step; lr[6] passed by value (rho then theta). */
 int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev, const float* lr6,

@@ -192,7 +192,7 @@ int32_t ts_render_fwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, nullptr, nullptr, 0.f, nullptr, nullptr,
-                                           nullptr, (cudaStream_t)stream);
+                                           nullptr, nullptr, (cudaStream_t)stream);
     fr->have_fwd = (s == TS_OK);
     return s;
 }
@@ -204,9 +204,26 @@ int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* o
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev,
-                                           (cudaStream_t)stream);
+                                           nullptr, (cudaStream_t)stream);
     fr->have_fwd = (s == TS_OK);
     return s;
+}
+
+int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
+                            float* out_alpha, uint32_t* face_pixels, void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !face_pixels) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if (!fr->have_sort) return TS_ERR_STATE;
+    const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, nullptr, nullptr, 0.f, nullptr, nullptr,
+                                           nullptr, face_pixels, (cudaStream_t)stream);
+    fr->have_fwd = (s == TS_OK);
+    return s;
+}
+
+int32_t ts_face_area(ts_ctx* ctx, ts_frame* fr, float* proj_area, void* stream) {
+    if (!ctx || !fr || !proj_area) return TS_ERR_INVALID_ARG;
+    if (!fr->have_project) return TS_ERR_STATE;
+    return ts_launch_face_area(ctx, fr, proj_area, (cudaStream_t)stream);
 }
 
 int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth, float* out_alpha,

@@ -7,6 +7,7 @@ struct FwdWarpSmem {
     float4 r[32][6];                  // R0 R1 R2 | kap0 kap1 kap2 c00 | c01 c02 c10 c11 | c12 c20 c21 c22
     uint32_t lm[32];                  // lane mask of the entry for this block
     uint32_t slot[32];
+    uint32_t face[32];                // only written / read by the statistics instantiation
 };
 
 struct FwdPix {                       // what the walk leaves for this lane's pixel
@@ -16,11 +17,11 @@ struct FwdPix {                       // what the walk leaves for this lane's pi
 
 // `ent` = the lane's entry of the first 32-entry chunk of the tile list (already requested by the caller, so that
 // its round trip overlaps the caller's ticket atomic).
-template <int SM, bool COUNT>
+template <int SM, bool COUNT, bool STATS = false>
 __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene& sc, const TsJob& job, int lane,
                                             FwdWarpSmem& sm, float sigma, float alpha_min, float t_min, uint4 ent,
                                             FwdPix& o, unsigned long long& n_visit, unsigned long long& n_rect,
-                                            unsigned long long& n_hit) {
+                                            unsigned long long& n_hit, uint32_t* __restrict__ face_pixels = nullptr) {
     const float fpx = (float)job.px, fpy = (float)job.py;
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, D = 0.0f, Tlast = 1.0f;
     uint32_t last = 0;
@@ -48,6 +49,7 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             sm.r[lane][4] = make_float4(col[1], col[2], col[3], col[4]);
             sm.r[lane][5] = make_float4(col[5], col[6], col[7], col[8]);
             sm.lm[lane] = lmask, sm.slot[lane] = cur.x;
+            if (STATS) sm.face[lane] = cur.y;
         }
         __syncwarp();
         uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);
@@ -61,7 +63,10 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
             float l[3], x, I, alpha;
             const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
-            if (!__any_sync(0xffffffffu, hit)) continue;
+            const uint32_t hm = __ballot_sync(0xffffffffu, hit);
+            if (!hm) continue;
+            // statistics: the face contributed to popc(hm) pixels of this block (one RED per visit)
+            if (STATS && lane == __ffs(hm) - 1) atomicAdd(face_pixels + sm.face[e], (uint32_t)__popc(hm));
             if (hit) {
                 const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
                 if (COUNT) n_hit += 1;

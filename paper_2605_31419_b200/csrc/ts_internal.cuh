@@ -100,7 +100,9 @@ __device__ __forceinline__ uint32_t ts_eff_visible(const TsFrameDev& f) {
 int32_t ts_launch_project(const ts_ctx*, ts_frame*, const ts_scene*, cudaStream_t);
 int32_t ts_launch_sort(const ts_ctx*, ts_frame*, cudaStream_t);
 int32_t ts_launch_render_fwd(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
-                             const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, cudaStream_t);
+                             const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, uint32_t* face_pixels,
+                             cudaStream_t);
+int32_t ts_launch_face_area(const ts_ctx*, ts_frame*, float* area, cudaStream_t);
 int32_t ts_launch_render_bwd(const ts_ctx*, ts_frame*, const ts_scene*, const float*, const float*, const float*,
                              float*, float*, float*, uint32_t, cudaStream_t);
 int32_t ts_launch_render_track(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,

@@ -20,10 +20,10 @@ struct FwdLoss {
     float wc, wd;
 };
 
-template <int SM, bool COUNT, bool LOSS>
+template <int SM, bool COUNT, bool LOSS, bool STATS>
 __global__ void __launch_bounds__(TS_JOB_WARPS * 32)
 render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float t_min, float* __restrict__ out_color,
-                  float* __restrict__ out_depth, float* __restrict__ out_alpha, FwdLoss L) {
+                  float* __restrict__ out_depth, float* __restrict__ out_alpha, FwdLoss L, uint32_t* __restrict__ face_pixels) {
     __shared__ FwdWarpSmem smem[TS_JOB_WARPS];
     const int lane = threadIdx.x & 31;
     FwdWarpSmem& sm = smem[threadIdx.x >> 5];
@@ -40,7 +40,7 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
         if (job.range.x + lane < job.range.y) ent = f.sorted[job.range.x + lane];
         j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
         FwdPix o;
-        ts_fwd_walk<SM, COUNT>(f, sc, job, lane, sm, sigma, alpha_min, t_min, ent, o, n_visit, n_rect, n_hit);
+        ts_fwd_walk<SM, COUNT, STATS>(f, sc, job, lane, sm, sigma, alpha_min, t_min, ent, o, n_visit, n_rect, n_hit, face_pixels);
         const float T = o.T, C0 = o.C0, C1 = o.C1, C2 = o.C2, D = o.D, Tlast = o.Tlast;
         const uint32_t last = o.last;
         if (job.inside) {
@@ -91,22 +91,41 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
 
 template <int SM>
 void launch_sm(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, float* oc, float* od, float* oa, const FwdLoss* L,
-               cudaStream_t st) {
+               uint32_t* face_pixels, cudaStream_t st) {
     const TsFrameDev& f = fr->d;
     const bool count = (fr->prm.flags & TS_PARAM_COUNTERS) != 0;
     const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 4, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
     const float sg = fr->prm.sigma, am = fr->prm.alpha_min, tm = fr->prm.t_min;
     const FwdLoss none = {nullptr, nullptr, nullptr, nullptr, nullptr, 0.f, 0.f};
-    if (L) render_fwd_kernel<SM, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, *L);
-    else if (count) render_fwd_kernel<SM, true, false><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, none);
-    else render_fwd_kernel<SM, false, false><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, none);
+    if (face_pixels) render_fwd_kernel<SM, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, none, face_pixels);
+    else if (L) render_fwd_kernel<SM, false, true, false><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, *L, nullptr);
+    else if (count) render_fwd_kernel<SM, true, false, false><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, none, nullptr);
+    else render_fwd_kernel<SM, false, false, false><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, sc, sg, am, tm, oc, od, oa, none, nullptr);
+}
+
+// projected area of every visible face, |S| / 2 with S of F4 (same operation order as the projection: bit-exact)
+__global__ void __launch_bounds__(256) face_area_kernel(TsFrameDev f, float* __restrict__ area) {
+    const uint32_t nvis = min(ts_eff_visible(f), f.vis_cap);
+    for (uint32_t slot = blockIdx.x * blockDim.x + threadIdx.x; slot < nvis; slot += gridDim.x * blockDim.x) {
+        const float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
+        const float4 s0 = s4[0], s1 = s4[1], s3 = s4[3];
+        const float a = __fsub_rn(s0.w, s0.x), b = __fsub_rn(s1.w, s0.y), c = __fsub_rn(s1.x, s0.y), d = __fsub_rn(s1.z, s0.x);
+        const float S = __fmaf_rn(a, b, -__fmul_rn(c, d));
+        area[__float_as_uint(s3.x)] = 0.5f * fabsf(S);
+    }
 }
 
 }  // namespace
 
+int32_t ts_launch_face_area(const ts_ctx* ctx, ts_frame* fr, float* area, cudaStream_t st) {
+    face_area_kernel<<<ctx->num_sms * 4, 256, 0, st>>>(fr->d, area);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
+
 int32_t ts_launch_render_fwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
                              const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss,
-                             cudaStream_t st) {
+                             uint32_t* face_pixels, cudaStream_t st) {
     FwdLoss L;
     const FwdLoss* Lp = nullptr;
     if (gC) {
@@ -115,10 +134,10 @@ int32_t ts_launch_render_fwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
         Lp = &L;
     }
     switch (ts_sigma_mode(fr->prm.sigma)) {
-        case 1: launch_sm<1>(ctx, fr, *sc, oc, od, oa, Lp, st); break;
-        case 2: launch_sm<2>(ctx, fr, *sc, oc, od, oa, Lp, st); break;
-        case 3: launch_sm<3>(ctx, fr, *sc, oc, od, oa, Lp, st); break;
-        default: launch_sm<0>(ctx, fr, *sc, oc, od, oa, Lp, st); break;
+        case 1: launch_sm<1>(ctx, fr, *sc, oc, od, oa, Lp, face_pixels, st); break;
+        case 2: launch_sm<2>(ctx, fr, *sc, oc, od, oa, Lp, face_pixels, st); break;
+        case 3: launch_sm<3>(ctx, fr, *sc, oc, od, oa, Lp, face_pixels, st); break;
+        default: launch_sm<0>(ctx, fr, *sc, oc, od, oa, Lp, face_pixels, st); break;
     }
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;

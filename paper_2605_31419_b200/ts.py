@@ -24,7 +24,7 @@ _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.
                 VIEW_TILE_RANGES: torch.int32, VIEW_N_CONTRIB: torch.int32, VIEW_COUNTERS: torch.int64}
 
 EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
-           "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_bwd",
+           "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
            "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view"]
 
 
@@ -67,6 +67,9 @@ def _load():
     lib.ts_render_fwd_l1.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_render_track_l1.argtypes = lib.ts_render_fwd_l1.argtypes
+    lib.ts_render_fwd_stats.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                        C.c_void_p, C.c_void_p]
+    lib.ts_face_area.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_render_bwd.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
     lib.ts_pose_jacobian_reduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -182,6 +185,15 @@ def ts_render_track_l1(ctx, scene, frame, out_color, out_depth, out_alpha, Chat,
                        loss=None, stream=None):
     _check(lib.ts_render_track_l1(ctx.h, C.byref(scene.c), frame.h, _ptr(out_color), _ptr(out_depth), _ptr(out_alpha),
                                   _ptr(Chat), _ptr(Dhat), float(lambda_dep), _ptr(gC), _ptr(gD), _ptr(loss), _stream(stream)))
+
+
+def ts_render_fwd_stats(ctx, scene, frame, out_color, out_depth, out_alpha, face_pixels, stream=None):
+    _check(lib.ts_render_fwd_stats(ctx.h, C.byref(scene.c), frame.h, _ptr(out_color), _ptr(out_depth), _ptr(out_alpha),
+                                   _ptr(face_pixels, torch.int32), _stream(stream)))
+
+
+def ts_face_area(ctx, frame, proj_area, stream=None):
+    _check(lib.ts_face_area(ctx.h, frame.h, _ptr(proj_area), _stream(stream)))
 
 
 def ts_render_bwd(ctx, scene, frame, dL_dcolor, dL_ddepth, dL_dalpha, grad_pos, grad_color, grad_opacity, grad_mask,
