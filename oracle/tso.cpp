@@ -259,6 +259,63 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
     if (counters) counters[0] = n_visit, counters[1] = n_rect, counters[2] = n_hit, counters[3] = 0;
 }
 
+// ---------------------------------------------------------------------------------- D-SSIM (Eq. 8)
+// L_DSSIM(I, Ibar) = 1 - mean over channels and pixels of SSIM (Eq. 8; the paper only names the
+// term, reading S25 of DESIGN.md fixes it as in 3D Gaussian Splatting: 11x11 Gaussian window, sigma 1.5, zero
+// padding, C1 = 0.01^2, C2 = 0.03^2, per channel).  Written as the definition: window sums by direct double loops,
+// gradient by plain reverse mode of those loops (for every pixel p and every tap q of its window).
+// x = rendered image [3][H][W], y = reference.  Returns L; g (may be NULL) receives dL/dx.
+template <class T>
+double dssim(int32_t W, int32_t H, const T* x, const T* y, T* g) {
+    const int R = 5;
+    double w1[11], wsum = 0;
+    for (int i = 0; i < 11; ++i) wsum += (w1[i] = std::exp(-(double)((i - R) * (i - R)) / (2.0 * 1.5 * 1.5)));
+    for (int i = 0; i < 11; ++i) w1[i] /= wsum;
+    const T C1 = (T)(0.01 * 0.01), C2 = (T)(0.03 * 0.03);
+    const int64_t HW = (int64_t)W * H;
+    const double N = 3.0 * (double)HW;
+    if (g) for (int64_t i = 0; i < 3 * HW; ++i) g[i] = 0;
+    double total = 0;
+    for (int c = 0; c < 3; ++c) {
+        const T* xc = x + c * HW;
+        const T* yc = y + c * HW;
+        T* gc = g ? g + c * HW : nullptr;
+        for (int py = 0; py < H; ++py)
+            for (int px = 0; px < W; ++px) {
+                T mu1 = 0, mu2 = 0, e11 = 0, e22 = 0, e12 = 0;
+                for (int dy = -R; dy <= R; ++dy)
+                    for (int dx = -R; dx <= R; ++dx) {
+                        const int qx = px + dx, qy = py + dy;
+                        if (qx < 0 || qx >= W || qy < 0 || qy >= H) continue;          // zero padding
+                        const T wgt = (T)(w1[dy + R] * w1[dx + R]);
+                        const T a = xc[(int64_t)qy * W + qx], b = yc[(int64_t)qy * W + qx];
+                        mu1 += wgt * a, mu2 += wgt * b, e11 += wgt * a * a, e22 += wgt * b * b, e12 += wgt * a * b;
+                    }
+                const T s11 = e11 - mu1 * mu1, s22 = e22 - mu2 * mu2, s12 = e12 - mu1 * mu2;
+                const T A1 = 2 * mu1 * mu2 + C1, A2 = 2 * s12 + C2, B1 = mu1 * mu1 + mu2 * mu2 + C1, B2 = s11 + s22 + C2;
+                const T ssim = (A1 * A2) / (B1 * B2);
+                total += (double)ssim;
+                if (!gc) continue;
+                // reverse mode: dL/dssim = -1/N; ssim depends on x through mu1, e11 (in s11) and e12 (in s12)
+                const T gs = (T)(-1.0 / N);
+                const T d_mu1_direct = (2 * mu2 * A2) / (B1 * B2) - (A1 * A2 * 2 * mu1) / (B1 * B1 * B2);
+                const T d_s11 = -(A1 * A2) / (B1 * B2 * B2);
+                const T d_s12 = (2 * A1) / (B1 * B2);
+                // s11 = e11 - mu1^2, s12 = e12 - mu1 mu2
+                const T d_mu1 = d_mu1_direct - 2 * mu1 * d_s11 - mu2 * d_s12;
+                for (int dy = -R; dy <= R; ++dy)
+                    for (int dx = -R; dx <= R; ++dx) {
+                        const int qx = px + dx, qy = py + dy;
+                        if (qx < 0 || qx >= W || qy < 0 || qy >= H) continue;
+                        const T wgt = (T)(w1[dy + R] * w1[dx + R]);
+                        const int64_t q = (int64_t)qy * W + qx;
+                        gc[q] += gs * wgt * (d_mu1 + d_s11 * 2 * xc[q] + d_s12 * yc[q]);
+                    }
+            }
+    }
+    return 1.0 - total / N;
+}
+
 // ---------------------------------------------------------------------------------- per-face statistics
 // What the map-management layer of the paper reads off a render (not part of Eq. 1-4): for every face the number of
 // pixels it contributed to (the "rendered" flag of the covisibility IoU; the pixel coverage of the
@@ -600,6 +657,9 @@ void tso_pose_step_f32(float* T_cw, const float* g, float* state, const float* l
 }
 
 void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out) { left_perturb<double>(T_cw, tau, out); }
+
+double tso_dssim_f32(int32_t W, int32_t H, const float* x, const float* y, float* g) { return dssim<float>(W, H, x, y, g); }
+double tso_dssim_f64(int32_t W, int32_t H, const double* x, const double* y, double* g) { return dssim<double>(W, H, x, y, g); }
 
 void tso_face_stats_f32(const float* color, const float* opacity, const int32_t* faces, int32_t M, const tso_camera* cam,
                         const tso_params* prm, const uint8_t* visible, const int16_t* rect, const float* scr,

@@ -109,6 +109,12 @@ double tso_l1_loss_f64(int32_t W, int32_t H, const double* C, const double* D, c
 void tso_pose_step_f32(float* T_cw, const float* dL_dtau, float* state, const float* lr, float beta1, float beta2,
                        float eps);
 
+/* D-SSIM term of Eq. 8: L = 1 - mean SSIM over 3 channels x H x W, 11x11 Gaussian window
+ * (sigma 1.5), zero padding, C1 = 0.01^2, C2 = 0.03^2 (reading S25).  x = rendered [3][H][W], y = reference.
+ * Returns L; g (may be NULL) receives dL/dx. */
+double tso_dssim_f32(int32_t W, int32_t H, const float* x, const float* y, float* g);
+double tso_dssim_f64(int32_t W, int32_t H, const double* x, const double* y, double* g);
+
 /* Per-face statistics of a render (map management): face_pixels[M] = number of pixels the
  * face contributed to (same walk, hit rule and termination as tso_render_fwd); proj_area[M] = |S|/2 in px^2 (F4),
  * 0 for culled faces.  Either output may be NULL. */

@@ -50,6 +50,8 @@ def lib():
         _lib.tso_bin_sort.restype = C.c_int64
         _lib.tso_l1_loss_f32.restype = C.c_double
         _lib.tso_l1_loss_f64.restype = C.c_double
+        _lib.tso_dssim_f32.restype = C.c_double
+        _lib.tso_dssim_f64.restype = C.c_double
     return _lib
 
 
@@ -194,6 +196,16 @@ class Oracle:
         L = self._fn("tso_l1_loss")(C.c_int32(self.W), C.c_int32(self.H), _p(Cimg), _p(Dimg), _p(Chat), _p(Dhat),
                                     C.c_double(lambda_dep), _p(gC), _p(gD))
         return L, gC, gD
+
+
+def dssim(x, y, prec="f64", grad=True):
+    """L_DSSIM = 1 - mean SSIM (Eq. 8) of x (rendered, [3,H,W]) against y; returns (L, dL/dx or None)."""
+    dt = np.float32 if prec == "f32" else np.float64
+    x, y = np.ascontiguousarray(x, dt), np.ascontiguousarray(y, dt)
+    assert x.shape == y.shape and x.ndim == 3 and x.shape[0] == 3
+    g = np.zeros_like(x) if grad else None
+    L = getattr(lib(), "tso_dssim_" + prec)(C.c_int32(x.shape[2]), C.c_int32(x.shape[1]), _p(x), _p(y), _p(g))
+    return L, g
 
 
 def left_perturb(T_cw, tau):
