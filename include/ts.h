@@ -115,6 +115,13 @@ int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* frame, float* dL_dtau_dev
  * cotangent images gC[3][H][W], gD[H][W] and, if loss_dev != NULL, adds L to *loss_dev (caller zeroes). */
 int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* D, const float* Chat,
                         const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev, void* stream);
+/* D-SSIM term of E_pho (Eq. 8; lambda = 0.2):
+ * L_DSSIM = 1 - mean SSIM(C, Chat) over 3 x H x W, 11x11 Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2,
+ * C2 = 0.03^2.  On entry gC[3][H][W] holds the cotangent of the L1 term (ts_l1_loss_grad); on exit
+ * gC = (1 - lambda) gC + lambda dL_DSSIM/dC, i.e. the cotangent of E_pho.  If loss_dev != NULL, lambda * L_DSSIM is
+ * added to *loss_dev.  scratch: 9 * H * W floats of caller memory. */
+int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* Chat, float lambda, float* gC,
+                           float* loss_dev, float* scratch, void* stream);
 /* a3 + a4 in one launch: ts_render_fwd, with the L1 colour + depth loss of ts_l1_loss_grad evaluated on every pixel
  * while its value is still in registers: writes gC, gD (and adds L to *loss_dev if not NULL) exactly as
  * ts_l1_loss_grad would.  out_color / out_depth / out_alpha may be NULL (a tracking loop never reads them). */

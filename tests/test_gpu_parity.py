@@ -326,3 +326,65 @@ def test_face_statistics_match_the_oracle(ctx, oracle_mod, cfg):
     torch.cuda.synchronize()
     assert torch.equal(C, C2)
     g.close()
+
+
+@pytest.mark.parametrize("W,H", [(64, 48), (50, 37), (131, 70)])
+def test_dssim_loss_and_gradient(ctx, oracle_mod, W, H):
+    """ts_dssim_loss_grad against the oracle's D-SSIM (Eq. 8): lambda * L and (1 - lambda) gC + lambda dL/dC."""
+    from gpu_util import assert_grad_close, dev
+    from paper_2605_31419_b200 import ts
+    rng = np.random.default_rng(W)
+    yy, xx = np.mgrid[0:H, 0:W]
+    base = 0.5 + 0.4 * np.sin(0.3 * xx + 0.2 * yy)[None] * np.array([1.0, 0.7, -0.5])[:, None, None]
+    x = np.clip(base + rng.normal(0, 0.05, (3, H, W)), 0, 1).astype(np.float32)
+    y = np.clip(base + rng.normal(0, 0.05, (3, H, W)), 0, 1).astype(np.float32)
+    lam = 0.2
+    g_l1 = rng.normal(size=(3, H, W)).astype(np.float32) / (3 * H * W)
+    L64, g64 = oracle_mod.dssim(x, y, "f64")
+    L32, g32 = oracle_mod.dssim(x, y, "f32")
+    gC, loss = dev(g_l1), torch.zeros(1, device="cuda")
+    ts.ts_dssim_loss_grad(ctx, W, H, dev(x), dev(y), lam, gC, loss)
+    torch.cuda.synchronize()
+    assert abs(loss.item() - lam * L64) <= 2e-5 * lam * L64
+    got = gC.cpu().numpy()
+    assert_grad_close("dssim grad vs f64 oracle", got, (1 - lam) * g_l1.astype(np.float64) + lam * g64)
+    assert_grad_close("dssim grad vs f32 oracle", got, (1 - lam) * g_l1 + lam * g32)
+    # lambda = 0 leaves the L1 cotangent untouched
+    gC0 = dev(g_l1)
+    ts.ts_dssim_loss_grad(ctx, W, H, dev(x), dev(y), 0.0, gC0, None)
+    torch.cuda.synchronize()
+    assert np.array_equal(gC0.cpu().numpy(), g_l1)
+
+
+def test_tracking_gradient_with_full_photometric_loss(ctx, oracle_mod):
+    """E_track = (1 - lambda) L1 + lambda L_DSSIM + lambda_dep E_dep (Eq. 8-10, lambda = 0.2,
+    lambda_dep = 0.05): ts_render_fwd -> ts_l1_loss_grad -> ts_dssim_loss_grad -> ts_render_bwd(pose-only) ->
+    ts_pose_jacobian_reduce against the same chain through the oracle."""
+    from gpu_util import dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(1)
+    lam, lam_dep = 0.2, sc.params.lambda_dep
+    tgt = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    # oracle chain (on the oracle's own forward images)
+    L1, gC, gD = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, lam_dep)
+    Ls, gS = oracle_mod.dssim(f.color, tgt.color, "f32")
+    gC_o = ((1 - lam) * gC + lam * gS) * ok[None]
+    ref = o.backward(gC_o.astype(np.float32), (gD * ok).astype(np.float32), None, want=("pose",))
+    # CUDA chain
+    H, W = g.H, g.W
+    gCd, gDd = torch.empty_like(g.C), torch.empty_like(g.D)
+    ts.ts_l1_loss_grad(ctx, W, H, g.C, g.D, dev(tgt.color), dev(tgt.depth), lam_dep, gCd, gDd, None)
+    ts.ts_dssim_loss_grad(ctx, W, H, g.C, dev(tgt.color), lam, gCd, None)
+    okd = dev(ok.astype(np.float32))
+    gCd *= okd[None]
+    gDd *= okd
+    ts.ts_render_bwd(ctx, g.scene, g.frame, gCd, gDd, None, None, None, None, ts.GRAD_POSE)
+    tau = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau)
+    torch.cuda.synchronize()
+    t = tau.cpu().numpy()
+    # the L1 sign image can flip where |C - Chat| is within float rounding between the two forwards: a looser bound
+    assert np.abs(t - ref.dL_dtau).max() <= 5e-3 * np.abs(ref.dL_dtau).max(), (t, ref.dL_dtau)
+    g.close()
