@@ -316,6 +316,48 @@ double dssim(int32_t W, int32_t H, const T* x, const T* y, T* g) {
     return 1.0 - total / N;
 }
 
+// ---------------------------------------------------------------------------------- E_equi (Eq. 14)
+// E_equi = 1/|F| sum_m 1/3 sum_n (cos theta_{m,n} - 0.5)^2, cos of the internal angle at vertex n = dot product of the
+// normalised edge vectors leaving it, in world space.  Faces with an edge shorter than 1e-12 are
+// skipped (no angle).  Returns E; grad_pos[V][3] (may be NULL) += weight * dE/dpos.
+template <class T>
+double equi(const T* pos, const int32_t* faces, int32_t M, double weight, T* grad_pos) {
+    double total = 0;
+    for (int m = 0; m < M; ++m) {
+        int64_t id[3];
+        for (int k = 0; k < 3; ++k) id[k] = vid(faces, m, k);
+        T P[3][3];
+        for (int k = 0; k < 3; ++k)
+            for (int a = 0; a < 3; ++a) P[k][a] = pos[3 * id[k] + a];
+        bool ok = true;
+        for (int k = 0; k < 3 && ok; ++k) {
+            T l2 = 0;
+            for (int a = 0; a < 3; ++a) l2 += (P[(k + 1) % 3][a] - P[k][a]) * (P[(k + 1) % 3][a] - P[k][a]);
+            ok = l2 > (T)1e-24;
+        }
+        if (!ok) continue;
+        for (int n = 0; n < 3; ++n) {
+            const int b = (n + 1) % 3, c = (n + 2) % 3;
+            T u[3], v[3], uu = 0, vv = 0, uv = 0;
+            for (int a = 0; a < 3; ++a) {
+                u[a] = P[b][a] - P[n][a], v[a] = P[c][a] - P[n][a];
+                uu += u[a] * u[a], vv += v[a] * v[a], uv += u[a] * v[a];
+            }
+            const T lu = std::sqrt(uu), lv = std::sqrt(vv), cs = uv / (lu * lv);
+            total += (double)((cs - (T)0.5) * (cs - (T)0.5));
+            if (!grad_pos) continue;
+            const T gcs = (T)(weight / (3.0 * (double)M)) * 2 * (cs - (T)0.5);     // dE/dcos
+            for (int a = 0; a < 3; ++a) {
+                const T du = v[a] / (lu * lv) - cs * u[a] / uu, dv = u[a] / (lu * lv) - cs * v[a] / vv;
+                grad_pos[3 * id[b] + a] += gcs * du;
+                grad_pos[3 * id[c] + a] += gcs * dv;
+                grad_pos[3 * id[n] + a] -= gcs * (du + dv);
+            }
+        }
+    }
+    return total / (3.0 * (double)M);
+}
+
 // ---------------------------------------------------------------------------------- per-face statistics
 // What the map-management layer of the paper reads off a render (not part of Eq. 1-4): for every face the number of
 // pixels it contributed to (the "rendered" flag of the covisibility IoU; the pixel coverage of the
@@ -657,6 +699,13 @@ void tso_pose_step_f32(float* T_cw, const float* g, float* state, const float* l
 }
 
 void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out) { left_perturb<double>(T_cw, tau, out); }
+
+double tso_equi_f32(const float* pos, const int32_t* faces, int32_t M, double weight, float* grad_pos) {
+    return equi<float>(pos, faces, M, weight, grad_pos);
+}
+double tso_equi_f64(const double* pos, const int32_t* faces, int32_t M, double weight, double* grad_pos) {
+    return equi<double>(pos, faces, M, weight, grad_pos);
+}
 
 double tso_dssim_f32(int32_t W, int32_t H, const float* x, const float* y, float* g) { return dssim<float>(W, H, x, y, g); }
 double tso_dssim_f64(int32_t W, int32_t H, const double* x, const double* y, double* g) { return dssim<double>(W, H, x, y, g); }

@@ -109,6 +109,11 @@ double tso_l1_loss_f64(int32_t W, int32_t H, const double* C, const double* D, c
 void tso_pose_step_f32(float* T_cw, const float* dL_dtau, float* state, const float* lr, float beta1, float beta2,
                        float eps);
 
+/* E_equi of Eq. 14: mean over faces and their three internal angles of (cos theta - 0.5)^2, world
+ * space.  faces may be NULL (soup).  Returns E; grad_pos[V][3] (may be NULL) += weight * dE/dpos. */
+double tso_equi_f32(const float* pos, const int32_t* faces, int32_t M, double weight, float* grad_pos);
+double tso_equi_f64(const double* pos, const int32_t* faces, int32_t M, double weight, double* grad_pos);
+
 /* D-SSIM term of Eq. 8: L = 1 - mean SSIM over 3 channels x H x W, 11x11 Gaussian window
  * (sigma 1.5), zero padding, C1 = 0.01^2, C2 = 0.03^2 (reading S25).  x = rendered [3][H][W], y = reference.
  * Returns L; g (may be NULL) receives dL/dx. */

@@ -51,6 +51,8 @@ def lib():
         _lib.tso_l1_loss_f32.restype = C.c_double
         _lib.tso_l1_loss_f64.restype = C.c_double
         _lib.tso_dssim_f32.restype = C.c_double
+        _lib.tso_equi_f32.restype = C.c_double
+        _lib.tso_equi_f64.restype = C.c_double
         _lib.tso_dssim_f64.restype = C.c_double
     return _lib
 
@@ -196,6 +198,17 @@ class Oracle:
         L = self._fn("tso_l1_loss")(C.c_int32(self.W), C.c_int32(self.H), _p(Cimg), _p(Dimg), _p(Chat), _p(Dhat),
                                     C.c_double(lambda_dep), _p(gC), _p(gD))
         return L, gC, gD
+
+
+def equi(pos, faces=None, weight=1.0, prec="f64", grad=True):
+    """E_equi (Eq. 14) of a face set; returns (E, weight * dE/dpos or None)."""
+    dt = np.float32 if prec == "f32" else np.float64
+    pos = np.ascontiguousarray(pos, dt).reshape(-1, 3)
+    faces = None if faces is None else np.ascontiguousarray(faces, np.int32).reshape(-1, 3)
+    M = pos.shape[0] // 3 if faces is None else faces.shape[0]
+    g = np.zeros_like(pos) if grad else None
+    E = getattr(lib(), "tso_equi_" + prec)(_p(pos), _p(faces), C.c_int32(M), C.c_double(weight), _p(g))
+    return E, g
 
 
 def dssim(x, y, prec="f64", grad=True):
