@@ -115,6 +115,10 @@ int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* frame, float* dL_dtau_dev
  * cotangent images gC[3][H][W], gD[H][W] and, if loss_dev != NULL, adds L to *loss_dev (caller zeroes). */
 int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* D, const float* Chat,
                         const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev, void* stream);
+/* E_equi of E_map (Eq. 14-15): mean over the faces and their three internal
+ * angles of (cos theta - 0.5)^2, in world space.  grad_pos[V][3] += weight * dE_equi/dpos (may be NULL);
+ * *loss_dev += weight * E_equi (may be NULL).  Only scene->pos, faces, V, M are read. */
+int32_t ts_equi_loss_grad(ts_ctx* ctx, const ts_scene* scene, float weight, float* grad_pos, float* loss_dev, void* stream);
 /* D-SSIM term of E_pho (Eq. 8; lambda = 0.2):
  * L_DSSIM = 1 - mean SSIM(C, Chat) over 3 x H x W, 11x11 Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2,
  * C2 = 0.03^2.  On entry gC[3][H][W] holds the cotangent of the L1 term (ts_l1_loss_grad); on exit

@@ -45,7 +45,86 @@ __global__ void pose_step_kernel(float* __restrict__ T, const float* __restrict_
     ts_pose_step_warp(T, g, state, lr, beta1, beta2, eps);   // launched with exactly one warp
 }
 
+// E_equi (Eq. 14): per face, world space.  One thread per face; the loss is block-reduced into one
+// atomic per CTA, the gradient goes to grad_pos with RED.ADD (a soup face owns its three vertices: no contention).
+template <bool SOUP>
+__global__ void __launch_bounds__(256)
+equi_loss_grad_kernel(int M, const float* __restrict__ pos, const int32_t* __restrict__ faces, float gscale, float lscale,
+                      float* __restrict__ grad_pos, float* __restrict__ loss) {
+    float acc = 0.f;
+    for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < M; m += gridDim.x * blockDim.x) {
+        size_t id[3];
+        float P[3][3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            id[k] = SOUP ? (size_t)3 * m + k : (size_t)__ldg(faces + 3 * (size_t)m + k);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) P[k][a] = __ldg(pos + 3 * id[k] + a);
+        }
+        bool ok = true;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            float l2 = 0.f;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) l2 += (P[(k + 1) % 3][a] - P[k][a]) * (P[(k + 1) % 3][a] - P[k][a]);
+            ok = ok && l2 > 1e-24f;
+        }
+        if (!ok) continue;                                       // an edge of zero length: no angle
+        float G[3][3] = {{0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}, {0.f, 0.f, 0.f}};
+#pragma unroll
+        for (int n = 0; n < 3; ++n) {
+            const int b = (n + 1) % 3, c = (n + 2) % 3;
+            float u[3], v[3], uu = 0.f, vv = 0.f, uv = 0.f;
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                u[a] = P[b][a] - P[n][a], v[a] = P[c][a] - P[n][a];
+                uu += u[a] * u[a], vv += v[a] * v[a], uv += u[a] * v[a];
+            }
+            const float ilu = rsqrtf(uu), ilv = rsqrtf(vv), iluv = ilu * ilv, cs = uv * iluv;
+            acc += (cs - 0.5f) * (cs - 0.5f);
+            const float gcs = gscale * 2.0f * (cs - 0.5f);        // dE/dcos
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const float du = v[a] * iluv - cs * u[a] * ilu * ilu, dv = u[a] * iluv - cs * v[a] * ilv * ilv;
+                G[b][a] += gcs * du, G[c][a] += gcs * dv, G[n][a] -= gcs * (du + dv);
+            }
+        }
+        if (grad_pos) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) atomicAdd(grad_pos + 3 * id[k] + a, G[k][a]);
+        }
+    }
+    if (loss) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+        __shared__ float s[8];
+        if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = acc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            float t = 0.f;
+            for (int w = 0; w < 8; ++w) t += s[w];
+            atomicAdd(loss, lscale * t);
+        }
+    }
+}
+
 }  // namespace
+
+extern "C" int32_t ts_equi_loss_grad(ts_ctx* ctx, const ts_scene* sc, float weight, float* grad_pos, float* loss_dev,
+                                     void* stream) {
+    if (!ctx || !sc || !sc->pos || sc->M <= 0 || (!grad_pos && !loss_dev)) return TS_ERR_INVALID_ARG;
+    if (sc->faces == nullptr && sc->V != 3 * sc->M) return TS_ERR_INVALID_ARG;
+    const float scale = (float)((double)weight / (3.0 * (double)sc->M));
+    const int grid = (int)(((size_t)sc->M + 255) / 256 < (size_t)ctx->num_sms * 8 ? ((size_t)sc->M + 255) / 256 : (size_t)ctx->num_sms * 8);
+    if (sc->faces == nullptr)
+        equi_loss_grad_kernel<true><<<grid, 256, 0, (cudaStream_t)stream>>>(sc->M, sc->pos, nullptr, scale, scale, grad_pos, loss_dev);
+    else
+        equi_loss_grad_kernel<false><<<grid, 256, 0, (cudaStream_t)stream>>>(sc->M, sc->pos, sc->faces, scale, scale, grad_pos, loss_dev);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
 
 extern "C" int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* D, const float* Chat,
                                    const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,

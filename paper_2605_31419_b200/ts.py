@@ -25,7 +25,7 @@ _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.
 
 EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
-           "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view"]
+           "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view"]
 
 
 class TsError(RuntimeError):
@@ -77,6 +77,7 @@ def _load():
                                     C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_dssim_loss_grad.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
                                        C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_equi_loss_grad.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_pose_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_float), C.c_float,
                                  C.c_float, C.c_float, C.c_void_p]
     lib.ts_pose_reduce_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_float),
@@ -218,6 +219,10 @@ def ts_dssim_loss_grad(ctx, W, H, Cimg, Chat, lam, gC, loss=None, scratch=None, 
         scratch = torch.empty(9 * int(W) * int(H), device=Cimg.device)
     _check(lib.ts_dssim_loss_grad(ctx.h, int(W), int(H), _ptr(Cimg), _ptr(Chat), float(lam), _ptr(gC), _ptr(loss),
                                   _ptr(scratch), _stream(stream)))
+
+
+def ts_equi_loss_grad(ctx, scene, weight, grad_pos, loss=None, stream=None):
+    _check(lib.ts_equi_loss_grad(ctx.h, C.byref(scene.c), float(weight), _ptr(grad_pos), _ptr(loss), _stream(stream)))
 
 
 def ts_pose_step(ctx, T_cw, dL_dtau, state, lr6, beta1=0.9, beta2=0.999, eps=1e-8, stream=None):

@@ -388,3 +388,26 @@ def test_tracking_gradient_with_full_photometric_loss(ctx, oracle_mod):
     # the L1 sign image can flip where |C - Chat| is within float rounding between the two forwards: a looser bound
     assert np.abs(t - ref.dL_dtau).max() <= 5e-3 * np.abs(ref.dL_dtau).max(), (t, ref.dL_dtau)
     g.close()
+
+
+@pytest.mark.parametrize("indexed", [False, True])
+def test_equi_regulariser(ctx, oracle_mod, indexed):
+    """ts_equi_loss_grad against the oracle's E_equi (Eq. 14): value and gradient, soup and shared vertices."""
+    from gpu_util import assert_grad_close, dev
+    from paper_2605_31419_b200 import ts
+    rng = np.random.default_rng(4)
+    if indexed:
+        pos = rng.normal(size=(500, 3)).astype(np.float32)
+        faces = rng.integers(0, 500, size=(3000, 3)).astype(np.int32)
+        faces = faces[(faces[:, 0] != faces[:, 1]) & (faces[:, 1] != faces[:, 2]) & (faces[:, 0] != faces[:, 2])]
+    else:
+        pos, faces = scenes.config0(n_faces=3000).pos, None
+    w = 0.37
+    E, g = oracle_mod.equi(pos, faces, weight=w, prec="f64")
+    scene = ts.Scene(dev(pos), dev(np.zeros_like(pos)), dev(np.zeros(pos.shape[0], np.float32)),
+                     None if faces is None else dev(faces, torch.int32))
+    gp, loss = torch.zeros(pos.shape[0], 3, device="cuda"), torch.zeros(1, device="cuda")
+    ts.ts_equi_loss_grad(ctx, scene, w, gp, loss)
+    torch.cuda.synchronize()
+    assert abs(loss.item() - w * E) <= 1e-5 * w * E
+    assert_grad_close("equi grad", gp.cpu().numpy(), g)
