@@ -7,7 +7,8 @@
 //   :82                      barycentric vertex colour, mean vertex opacity
 //   Eq. 4 front-to-back compositing in depth order    -> render_fwd()
 //   Eq. 5-7 analytic se(3) pose Jacobian              -> project_bwd()
-// Step names F1..F8 / B1..B9 and readings S1..S24 / N1..N5 refer to DESIGN.md section 3.
+//   Eq. 12 rendered normal map                        -> face_normal(), render_fwd/bwd(nrm)
+// Step names F1..F8 / B1..B9 and readings S1..S26 / N1..N5 refer to DESIGN.md section 3.
 // Build: g++ -std=c++17 -O2 -ffp-contract=off (no implicit FMA contraction; the float32
 // projection uses explicit std::fma where N1..N3 say so).
 #include "tso.h"
@@ -216,7 +217,8 @@ template <class T>
 void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t M, const tso_camera* cam_,
                 const tso_params* prm, const uint8_t* visible, const int16_t* rect, const T* scr,
                 const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, T* oc, T* od, T* oa,
-                uint32_t* n_contrib, uint8_t* ambig, uint64_t* sig, uint64_t* counters) {
+                uint32_t* n_contrib, uint8_t* ambig, uint64_t* sig, uint64_t* counters, const T* nrm = nullptr,
+                T* on = nullptr) {
     const Cam<T> cam(cam_);
     const int W = cam.W, H = cam.H;
     const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min, atol = (T)prm->amb_tol;
@@ -227,7 +229,7 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
         for (int x = 0; x < W; ++x) {
             int64_t b, e;
             LS.span(x, y, b, e);
-            T Tr = 1, C[3] = {0, 0, 0}, D = 0;
+            T Tr = 1, C[3] = {0, 0, 0}, D = 0, Nv[3] = {0, 0, 0};
             uint32_t last = 0;
             bool amb = false;
             uint64_t sg = 1469598103934665603ull;
@@ -242,6 +244,7 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 T wgt = Tr * h.alpha;                                          // Eq. 4
                 for (int c = 0; c < 3; ++c) C[c] += wgt * h.c[c];
                 D += wgt * h.z;                                                // S11
+                if (nrm) for (int c = 0; c < 3; ++c) Nv[c] += wgt * nrm[3 * (int64_t)list[i] + c];   // S26
                 Tr = Tr * ((T)1 - h.alpha);
                 last = (uint32_t)(i - b + 1);
                 sg = (sg ^ (uint64_t)(list[i] + 1)) * 1099511628211ull;
@@ -249,9 +252,10 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 if (Tr <= tmin) break;                                         // S12: include, then test
             }
             int64_t p = (int64_t)y * W + x;
-            for (int c = 0; c < 3; ++c) oc[(int64_t)c * W * H + p] = C[c];
-            od[p] = D;
-            oa[p] = (T)1 - Tr;
+            if (oc) for (int c = 0; c < 3; ++c) oc[(int64_t)c * W * H + p] = C[c];
+            if (od) od[p] = D;
+            if (oa) oa[p] = (T)1 - Tr;
+            if (on) for (int c = 0; c < 3; ++c) on[(int64_t)c * W * H + p] = Nv[c];
             if (n_contrib) n_contrib[p] = last;
             if (ambig) ambig[p] = amb ? 1 : 0;
             if (sig) sig[p] = sg;
@@ -407,7 +411,8 @@ template <class T>
 void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t M, const tso_camera* cam_,
                 const tso_params* prm, const uint8_t* visible, const int16_t* rect, const T* scr,
                 const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, const T* gCi, const T* gDi,
-                const T* gAi, T* grad_color, T* grad_opacity, T* g_scr) {
+                const T* gAi, T* grad_color, T* grad_opacity, T* g_scr, const T* nrm = nullptr, const T* gNi = nullptr,
+                T* g_nrm = nullptr) {
     const Cam<T> cam(cam_);
     const int W = cam.W, H = cam.H;
     const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min;
@@ -418,7 +423,8 @@ void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
     for (int y = 0; y < H; ++y)
         for (int x = 0; x < W; ++x) {
             int64_t p = (int64_t)y * W + x;
-            T gC[3] = {0, 0, 0}, gD = 0, gA = 0;
+            T gC[3] = {0, 0, 0}, gD = 0, gA = 0, gN[3] = {0, 0, 0};
+            if (nrm && gNi) for (int c = 0; c < 3; ++c) gN[c] = gNi[(int64_t)c * W * H + p];
             if (gCi) for (int c = 0; c < 3; ++c) gC[c] = gCi[(int64_t)c * W * H + p];
             if (gDi) gD = gDi[p];
             if (gAi) gA = gAi[p];
@@ -437,7 +443,7 @@ void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 if (Tr <= tmin) break;
             }
             // reverse walk; R* = what is composited BEHIND the current face with unit transmittance
-            T Rc[3] = {0, 0, 0}, Rd = 0, Ra = 0;
+            T Rc[3] = {0, 0, 0}, Rd = 0, Ra = 0, Rn[3] = {0, 0, 0};
             for (int64_t j = (int64_t)hits.size() - 1; j >= 0; --j) {
                 const uint32_t m = hits[j].m;
                 const Face<T>& f = F[m];
@@ -453,6 +459,13 @@ void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 T ga = 0;
                 for (int c = 0; c < 3; ++c) ga += (h.c[c] - Rc[c]) * gC[c];
                 ga += (h.z - Rd) * gD + ((T)1 - Ra) * gA;
+                if (nrm) {
+                    // S26: the face normal is a flat attribute composited like a colour
+                    const T* nm = nrm + 3 * (int64_t)m;
+                    for (int c = 0; c < 3; ++c) ga += (nm[c] - Rn[c]) * gN[c];
+                    for (int c = 0; c < 3; ++c) Rn[c] = h.alpha * nm[c] + ((T)1 - h.alpha) * Rn[c];
+                    if (g_nrm) for (int c = 0; c < 3; ++c) g_nrm[3 * (int64_t)m + c] += wgt * gN[c];
+                }
                 ga *= Tn;
                 // B3: push this face onto the "behind" accumulators
                 for (int c = 0; c < 3; ++c) Rc[c] = h.alpha * h.c[c] + ((T)1 - h.alpha) * Rc[c];
@@ -534,6 +547,80 @@ void project_bwd(const int32_t* faces, int32_t M, const T* Tcw, const tso_camera
         }
     }
     if (dL_dtau) for (int i = 0; i < 6; ++i) dL_dtau[i] = tau[i];
+}
+
+// ---------------------------------------------------------------------------------- face normals (Eq. 12)
+// The rendered normal map N(V, T_CW) "returned by the rasteriser" (Eq. 12) composites one normal
+// per face.  Reading S26 of DESIGN.md: n_m = unit normal of the face plane in CAMERA space, oriented towards the
+// camera (n . Q_0 < 0; the plane offset n . Q is the same for every point of the plane).  The edge vectors are taken
+// in world space and rotated (R (P_k - P_0) = Q_k - Q_0 exactly, without the cancellation of subtracting two camera-
+// space points).  nrm[M][3]; zero for culled faces.
+template <class T>
+void face_normal(const T* pos, const int32_t* faces, int32_t M, const T* Tcw, const uint8_t* visible, const T* Q,
+                 T* nrm) {
+    for (int m = 0; m < M; ++m) {
+        T* n = nrm + 3 * (int64_t)m;
+        n[0] = n[1] = n[2] = 0;
+        if (!visible[m]) continue;
+        const T* P0 = pos + 3 * (int64_t)vid(faces, m, 0);
+        const T* P1 = pos + 3 * (int64_t)vid(faces, m, 1);
+        const T* P2 = pos + 3 * (int64_t)vid(faces, m, 2);
+        T a[3], b[3];
+        for (int i = 0; i < 3; ++i) {
+            a[i] = 0, b[i] = 0;
+            for (int j = 0; j < 3; ++j) a[i] += Tcw[4 * i + j] * (P1[j] - P0[j]), b[i] += Tcw[4 * i + j] * (P2[j] - P0[j]);
+        }
+        const T mm[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+        const T len = std::sqrt(mm[0] * mm[0] + mm[1] * mm[1] + mm[2] * mm[2]);
+        const T* Q0 = Q + 9 * (int64_t)m;
+        const T off = mm[0] * Q0[0] + mm[1] * Q0[1] + mm[2] * Q0[2];
+        const T s = off < 0 ? (T)1 : (T)-1;                  // towards the camera
+        for (int i = 0; i < 3; ++i) n[i] = s * mm[i] / len;
+    }
+}
+
+// Reverse mode of face_normal: n = s m/|m|, m = a x b, a = R (P1 - P0), b = R (P2 - P0).
+//   g_m = s (g_n - n (n . g_n)) / |m|,  g_a = b x g_m,  g_b = g_m x a   (camera space)
+//   grad_pos: P1 += R^T g_a, P2 += R^T g_b, P0 -= R^T (g_a + g_b)
+//   pose (left perturbation, Eq. 5-7): a -> Exp(theta) a, so dL/dtheta += a x g_a + b x g_b; no translation term.
+// grad_pos (may be NULL) and dL_dtau[6] (may be NULL) are ACCUMULATED into.
+template <class T>
+void face_normal_bwd(const T* pos, const int32_t* faces, int32_t M, const T* Tcw, const uint8_t* visible, const T* Q,
+                     const T* g_nrm, T* grad_pos, T* dL_dtau) {
+    for (int m = 0; m < M; ++m) {
+        if (!visible[m]) continue;
+        const int64_t id0 = vid(faces, m, 0), id1 = vid(faces, m, 1), id2 = vid(faces, m, 2);
+        const T *P0 = pos + 3 * id0, *P1 = pos + 3 * id1, *P2 = pos + 3 * id2;
+        T a[3], b[3];
+        for (int i = 0; i < 3; ++i) {
+            a[i] = 0, b[i] = 0;
+            for (int j = 0; j < 3; ++j) a[i] += Tcw[4 * i + j] * (P1[j] - P0[j]), b[i] += Tcw[4 * i + j] * (P2[j] - P0[j]);
+        }
+        const T mm[3] = {a[1] * b[2] - a[2] * b[1], a[2] * b[0] - a[0] * b[2], a[0] * b[1] - a[1] * b[0]};
+        const T len = std::sqrt(mm[0] * mm[0] + mm[1] * mm[1] + mm[2] * mm[2]);
+        const T* Q0 = Q + 9 * (int64_t)m;
+        const T s = (mm[0] * Q0[0] + mm[1] * Q0[1] + mm[2] * Q0[2]) < 0 ? (T)1 : (T)-1;
+        T n[3];
+        for (int i = 0; i < 3; ++i) n[i] = s * mm[i] / len;
+        const T* gn = g_nrm + 3 * (int64_t)m;
+        const T ngn = n[0] * gn[0] + n[1] * gn[1] + n[2] * gn[2];
+        T gm[3];
+        for (int i = 0; i < 3; ++i) gm[i] = s * (gn[i] - n[i] * ngn) / len;
+        const T ga[3] = {b[1] * gm[2] - b[2] * gm[1], b[2] * gm[0] - b[0] * gm[2], b[0] * gm[1] - b[1] * gm[0]};
+        const T gb[3] = {gm[1] * a[2] - gm[2] * a[1], gm[2] * a[0] - gm[0] * a[2], gm[0] * a[1] - gm[1] * a[0]};
+        if (grad_pos) {
+            for (int j = 0; j < 3; ++j) {
+                const T wa = Tcw[j] * ga[0] + Tcw[4 + j] * ga[1] + Tcw[8 + j] * ga[2];
+                const T wb = Tcw[j] * gb[0] + Tcw[4 + j] * gb[1] + Tcw[8 + j] * gb[2];
+                grad_pos[3 * id1 + j] += wa, grad_pos[3 * id2 + j] += wb, grad_pos[3 * id0 + j] -= wa + wb;
+            }
+        }
+        if (dL_dtau) {
+            dL_dtau[3] += (a[1] * ga[2] - a[2] * ga[1]) + (b[1] * gb[2] - b[2] * gb[1]);
+            dL_dtau[4] += (a[2] * ga[0] - a[0] * ga[2]) + (b[2] * gb[0] - b[0] * gb[2]);
+            dL_dtau[5] += (a[0] * ga[1] - a[1] * ga[0]) + (b[0] * gb[1] - b[1] * gb[0]);
+        }
+    }
 }
 
 template <class T>
@@ -722,5 +809,30 @@ void tso_face_stats_f64(const double* color, const double* opacity, const int32_
                         double* proj_area) {
     face_stats<double>(color, opacity, faces, M, cam, prm, visible, rect, scr, list, n_list, tile_ranges, face_pixels, proj_area);
 }
+
+#define TSO_NRM_FWD(T, sfx)                                                                                            \
+    void tso_face_normal_##sfx(const T* pos, const int32_t* faces, int32_t M, const T* T_cw, const uint8_t* visible,  \
+                               const T* Q, T* nrm) {                                                                   \
+        face_normal<T>(pos, faces, M, T_cw, visible, Q, nrm);                                                          \
+    }                                                                                                                  \
+    void tso_face_normal_bwd_##sfx(const T* pos, const int32_t* faces, int32_t M, const T* T_cw,                       \
+                                   const uint8_t* visible, const T* Q, const T* g_nrm, T* grad_pos, T* dL_dtau) {      \
+        face_normal_bwd<T>(pos, faces, M, T_cw, visible, Q, g_nrm, grad_pos, dL_dtau);                                 \
+    }                                                                                                                  \
+    void tso_render_normal_fwd_##sfx(const T* color, const T* opacity, const int32_t* faces, int32_t M,                \
+                                     const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \
+                                     const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
+                                     const uint32_t* tile_ranges, const T* nrm, T* out_normal) {                       \
+        render_fwd<T>(TSO_FWD_ARGS, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nrm, out_normal);   \
+    }                                                                                                                  \
+    void tso_render_normal_bwd_##sfx(const T* color, const T* opacity, const int32_t* faces, int32_t M,                \
+                                     const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \
+                                     const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
+                                     const uint32_t* tile_ranges, const T* nrm, const T* dL_dnormal, T* grad_opacity,  \
+                                     T* g_scr, T* g_nrm) {                                                             \
+        render_bwd<T>(TSO_FWD_ARGS, nullptr, nullptr, nullptr, nullptr, grad_opacity, g_scr, nrm, dL_dnormal, g_nrm);  \
+    }
+TSO_NRM_FWD(float, f32)
+TSO_NRM_FWD(double, f64)
 
 }  // extern "C"

@@ -17,7 +17,8 @@
  * Pins (tests/test_oracle_*.py): closed forms for one triangle, hand-computed worked example,
  * ray-plane depth, two-layer compositing, invariants, brute == tiled, std::stable_sort,
  * central finite differences for every gradient incl. SE(3) perturbations, rigid-motion
- * identity.  Parity unpinned: none.
+ * identity; normal map: plane coefficients, Eq. 11 on the rendered depth, flat-colour equivalence,
+ * finite differences.  Parity unpinned: none.
  *
  * All pointers are HOST pointers owned by the caller.  T = float (_f32) or double (_f64).
  */
@@ -131,6 +132,30 @@ void tso_face_stats_f64(const double* color, const double* opacity, const int32_
                         const tso_params* prm, const uint8_t* visible, const int16_t* rect, const double* scr,
                         const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, uint32_t* face_pixels,
                         double* proj_area);
+
+/* Rendered normal map of Eq. 12, reading S26: N(p) = sum_n n_n alpha_n T_n with n_n the
+ * unit normal of the face plane in CAMERA space, oriented towards the camera (n . Q_0 < 0), not renormalised.
+ *   tso_face_normal      nrm[M][3] from the world edges rotated by R (zero for culled faces)
+ *   tso_render_normal_fwd  out_normal[3][H][W]; same walk, hit rule and termination as tso_render_fwd
+ *   tso_render_normal_bwd  dL_dnormal[3][H][W] -> grad_opacity[V] (+=, may be NULL), g_scr[M][9] (+=, the window path
+ *                          only: a flat attribute has no interpolation term) and g_nrm[M][3] (+=)
+ *   tso_face_normal_bwd  g_nrm -> grad_pos[V][3] (+=, may be NULL) and dL_dtau[6] (+=, may be NULL; rotation part only) */
+#define TSO_NRM_DECL(T, sfx)                                                                                           \
+    void tso_face_normal_##sfx(const T* pos, const int32_t* faces, int32_t M, const T* T_cw, const uint8_t* visible,  \
+                               const T* Q, T* nrm);                                                                    \
+    void tso_face_normal_bwd_##sfx(const T* pos, const int32_t* faces, int32_t M, const T* T_cw,                       \
+                                   const uint8_t* visible, const T* Q, const T* g_nrm, T* grad_pos, T* dL_dtau);       \
+    void tso_render_normal_fwd_##sfx(const T* color, const T* opacity, const int32_t* faces, int32_t M,                \
+                                     const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \
+                                     const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
+                                     const uint32_t* tile_ranges, const T* nrm, T* out_normal);                        \
+    void tso_render_normal_bwd_##sfx(const T* color, const T* opacity, const int32_t* faces, int32_t M,                \
+                                     const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \
+                                     const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
+                                     const uint32_t* tile_ranges, const T* nrm, const T* dL_dnormal, T* grad_opacity,  \
+                                     T* g_scr, T* g_nrm);
+TSO_NRM_DECL(float, f32)
+TSO_NRM_DECL(double, f64)
 
 /* SE(3) exponential, tau = (rho, theta): out[12] = Exp(tau) o T (3x4 row-major). */
 void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out);

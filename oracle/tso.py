@@ -191,6 +191,48 @@ class Oracle:
                                     _p(pr.visible), _p(pr.Q), _p(o.g_scr), _p(o.grad_pos), _p(o.dL_dtau))
         return o
 
+    # ------------------------------------------------------------------ normal map (Eq. 12, reading S26)
+    def face_normals(self):
+        """nrm[M,3]: camera-space unit normals towards the camera (zero for culled faces)."""
+        pr = self.project()
+        nrm = np.zeros((self.M, 3), self.dt)
+        self._fn("tso_face_normal")(_p(self.pos), _p(self.faces), C.c_int32(self.M), _p(self.T_cw), _p(pr.visible),
+                                    _p(pr.Q), _p(nrm))
+        return nrm
+
+    def normal_forward(self, mode="tiled"):
+        pr = self.project()
+        lst, ranges = self._lists(mode)
+        nrm = self.face_normals()
+        N = np.zeros((3, self.H, self.W), self.dt)
+        self._fn("tso_render_normal_fwd")(
+            _p(self.color), _p(self.opacity), _p(self.faces), C.c_int32(self.M), C.byref(self.cam), C.byref(self.prm),
+            _p(pr.visible), _p(pr.rect), _p(pr.scr), _p(lst), C.c_int64(lst.shape[0]), _p(ranges), _p(nrm), _p(N))
+        return N
+
+    def normal_backward(self, gN, mode="tiled", want=("pos", "opacity", "pose")):
+        """Gradient of sum(gN * N): grad_pos (window path through B7-B8 plus the normal's own dependence on the
+        vertices), grad_opacity, dL_dtau."""
+        pr = self.project()
+        lst, ranges = self._lists(mode)
+        nrm = self.face_normals()
+        gN = np.ascontiguousarray(gN, self.dt)
+        o = SimpleNamespace()
+        o.grad_opacity = np.zeros_like(self.opacity) if "opacity" in want else None
+        o.g_scr = np.zeros((self.M, 9), self.dt)
+        o.g_nrm = np.zeros((self.M, 3), self.dt)
+        self._fn("tso_render_normal_bwd")(
+            _p(self.color), _p(self.opacity), _p(self.faces), C.c_int32(self.M), C.byref(self.cam), C.byref(self.prm),
+            _p(pr.visible), _p(pr.rect), _p(pr.scr), _p(lst), C.c_int64(lst.shape[0]), _p(ranges), _p(nrm), _p(gN),
+            _p(o.grad_opacity), _p(o.g_scr), _p(o.g_nrm))
+        o.grad_pos = np.zeros_like(self.pos) if "pos" in want else None
+        o.dL_dtau = np.zeros(6, self.dt)
+        self._fn("tso_project_bwd")(_p(self.faces), C.c_int32(self.M), _p(self.T_cw), C.byref(self.cam),
+                                    _p(pr.visible), _p(pr.Q), _p(o.g_scr), _p(o.grad_pos), _p(o.dL_dtau))
+        self._fn("tso_face_normal_bwd")(_p(self.pos), _p(self.faces), C.c_int32(self.M), _p(self.T_cw),
+                                        _p(pr.visible), _p(pr.Q), _p(o.g_nrm), _p(o.grad_pos), _p(o.dL_dtau))
+        return o
+
     def l1_loss(self, Cimg, Dimg, Chat, Dhat, lambda_dep):
         cv = lambda a: np.ascontiguousarray(a, self.dt)
         Cimg, Dimg, Chat, Dhat = cv(Cimg), cv(Dimg), cv(Chat), cv(Dhat)
