@@ -150,6 +150,24 @@ int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame,
                             float* out_alpha, uint32_t* face_pixels, void* stream);
 int32_t ts_face_area(ts_ctx* ctx, ts_frame* frame, float* proj_area, void* stream);
 
+/* Rendered normal map and its gradient (Eq. 12: the map "returned by the rasteriser" that E_norm
+ * compares with the sensor normals; reading S26):
+ *   N(p) = sum_n n_n alpha_n T_n,  n_n = unit normal of face n in CAMERA space, oriented towards the camera
+ * (n . Q < 0 for the points Q of the face), composited by the same walk as colour / depth / alpha, not renormalised.
+ * ts_render_fwd_normal: as ts_render_fwd (out_color / out_depth / out_alpha may be NULL) plus out_normal[3][H][W]
+ *   (device, required).  Reads scene->pos and the T_cw given to ts_project (still valid, unchanged).
+ * ts_render_bwd_normal: as ts_render_bwd with one more cotangent dL_dnormal[3][H][W] (device, required; the other
+ *   three may be NULL = 0): ONE reverse walk for all four outputs.  Full-gradient mode for every grad_mask (the
+ *   normal's own dependence on the vertices needs the per-face sums): grad_pos receives both the window path
+ *   (B4-B8) and d n / d vertices; TS_GRAD_POSE leaves partial sums for ts_pose_jacobian_reduce that include the
+ *   rotation of the normals (a translation of the camera does not turn them).  Requires ts_render_fwd_normal on the
+ *   same frame since the last ts_project. */
+int32_t ts_render_fwd_normal(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
+                             float* out_alpha, float* out_normal, void* stream);
+int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, const float* dL_dcolor,
+                             const float* dL_ddepth, const float* dL_dalpha, const float* dL_dnormal, float* grad_pos,
+                             float* grad_color, float* grad_opacity, uint32_t grad_mask, void* stream);
+
 /* a8: one Adam step on tau, then T_cw <- Exp(-delta) o T_cw, all on the device.
  * state_dev[13] = m[6], v[6], step; lr[6] passed by value (rho then theta). */
 int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev, const float* lr6,

@@ -10,7 +10,7 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t ctrl, tile_count, tile_cursor, tile_offset, tile_order, tile_ranges, scr, rec, gscr, pair_a, pair_b, big_key, big_idx, skey, sorted,
+    size_t ctrl, tile_count, tile_cursor, tile_offset, tile_order, tile_ranges, scr, rec, gscr, nrm, gnrm, pair_a, pair_b, big_key, big_idx, skey, sorted,
         n_contrib, t_last,
         pose_partials, total;
     int32_t tiles_x, tiles_y, NT;
@@ -34,6 +34,8 @@ bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pa
     L.scr = take(16ull * TS_SCR_F4 * vis_cap);
     L.rec = take(16ull * TS_REC_F4 * vis_cap);
     L.gscr = take(36ull * vis_cap);
+    L.nrm = take(16ull * vis_cap);
+    L.gnrm = take(12ull * vis_cap);
     L.pair_a = take(16ull * pair_cap);
     L.pair_b = take(4ull * pair_cap);
     L.big_key = take(8ull * pair_cap);
@@ -112,6 +114,8 @@ int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_
     d.scr = reinterpret_cast<float4*>(b + L.scr);
     d.rec = reinterpret_cast<float4*>(b + L.rec);
     d.gscr = reinterpret_cast<float*>(b + L.gscr);
+    d.nrm = reinterpret_cast<float4*>(b + L.nrm);
+    d.gnrm = reinterpret_cast<float*>(b + L.gnrm);
     d.pair_a = reinterpret_cast<uint4*>(b + L.pair_a);
     d.pair_b = reinterpret_cast<uint32_t*>(b + L.pair_b);
     d.big_key = reinterpret_cast<unsigned long long*>(b + L.big_key);
@@ -123,10 +127,11 @@ int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_
     d.pose_partials = reinterpret_cast<float*>(b + L.pose_partials);
     fr->bytes = L.total, fr->base = dev_ws;
     cudaStream_t st = (cudaStream_t)stream;
-    // one-time clears: control block, tile counters / cursors / ranges (contiguous), the zero-at-rest screen-gradient
-    // accumulator
+    // one-time clears: control block, tile counters / cursors / ranges (contiguous), the zero-at-rest gradient
+    // accumulators
     if (cudaMemsetAsync(b + L.ctrl, 0, L.scr - L.ctrl, st) != cudaSuccess ||
-        cudaMemsetAsync(b + L.gscr, 0, 36ull * visible_capacity, st) != cudaSuccess) {
+        cudaMemsetAsync(b + L.gscr, 0, 36ull * visible_capacity, st) != cudaSuccess ||
+        cudaMemsetAsync(b + L.gnrm, 0, 12ull * visible_capacity, st) != cudaSuccess) {
         delete fr;
         return TS_ERR_CUDA;
     }
@@ -162,7 +167,7 @@ int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const 
     fr->cam = TsCamDev{cam->width, cam->height, cam->fx, cam->fy, cam->cx, cam->cy, cam->znear};
     fr->prm = TsPrmDev{prm->sigma, prm->alpha_min, prm->t_min, prm->eps_area, prm->flags};
     fr->T_cw = T_cw_dev;
-    fr->have_sort = fr->have_fwd = 0;
+    fr->have_sort = fr->have_fwd = fr->have_normals = 0;
     fr->pose_src = 0;
     if (fr->counters_dirty) {
         // the previous ts_project was never followed by ts_bin_sort: its slot / tile counters are still live
@@ -218,6 +223,31 @@ int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float
                                            nullptr, face_pixels, (cudaStream_t)stream);
     fr->have_fwd = (s == TS_OK);
     return s;
+}
+
+int32_t ts_render_fwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
+                             float* out_alpha, float* out_normal, void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !sc->pos || !out_normal) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if (!fr->have_sort) return TS_ERR_STATE;
+    const int32_t s = ts_launch_render_fwd_normal(ctx, fr, sc, out_color, out_depth, out_alpha, out_normal, (cudaStream_t)stream);
+    fr->have_fwd = (s == TS_OK);
+    fr->have_normals = (s == TS_OK);
+    return s;
+}
+
+int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
+                             const float* dL_dalpha, const float* dL_dnormal, float* grad_pos, float* grad_color,
+                             float* grad_opacity, uint32_t grad_mask, void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !sc->pos || !dL_dnormal) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_POS) && !grad_pos) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_COLOR) && !grad_color) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_OPACITY) && !grad_opacity) return TS_ERR_INVALID_ARG;
+    if (grad_mask & ~(uint32_t)(TS_GRAD_POS | TS_GRAD_COLOR | TS_GRAD_OPACITY | TS_GRAD_POSE)) return TS_ERR_INVALID_ARG;
+    if (!fr->have_fwd || !fr->have_normals) return TS_ERR_STATE;
+    return ts_launch_render_bwd_normal(ctx, fr, sc, dL_dcolor, dL_ddepth, dL_dalpha, dL_dnormal, grad_pos, grad_color,
+                                       grad_opacity, grad_mask, (cudaStream_t)stream);
 }
 
 int32_t ts_face_area(ts_ctx* ctx, ts_frame* fr, float* proj_area, void* stream) {

@@ -103,17 +103,25 @@ __device__ __forceinline__ void ts_bwd_pose_hit(const BwdWarpSmem& sm, uint32_t 
 // opacity term (ATTR) of the lane's hit; hits of the same face sit in consecutive lanes (they were queued by one
 // visit), so a segmented shuffle reduction adds them up per face BEFORE any global atomic, and the first lane of every
 // run issues the RED.ADD.F32s.  `active` = this lane holds a hit.
-template <int SM, bool ATTR, bool GEOM>
+// NRM (normal-map backward, Eq. 12): the staged record carries the face normal in row 10 and row 11 of staged index
+// `pixel lane` carries that pixel's dL/dN (neither row is used outside pose-only mode); with GEOM the per-face dL/dn =
+// sum wgt dL/dN goes to f.gnrm.
+template <int SM, bool ATTR, bool GEOM, bool NRM = false>
 __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_scene& sc, BwdWarpSmem& sm, int lane,
                                                   bool active, uint32_t code, float l0, float l1, float l2, float ga,
                                                   float wgt, float sigma, float* __restrict__ grad_color,
                                                   float* __restrict__ grad_opacity) {
     const uint32_t e = code & 0xffu;
     float acc[19];
+    float accn[3] = {0.f, 0.f, 0.f};
 #pragma unroll
     for (int j = 0; j < 19; ++j) acc[j] = 0.f;
     if (active) {
         const float4 pg = sm.pix[code >> 8];
+        if (NRM && GEOM) {
+            const float4 pn = sm.r[code >> 8][11];
+            accn[0] = wgt * pn.x, accn[1] = wgt * pn.y, accn[2] = wgt * pn.z;
+        }
         const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
         const float l[3] = {l0, l1, l2};
         const float x = -fmaxf(l0, fmaxf(l1, l2));
@@ -156,6 +164,13 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
                 if (same) acc[j] += t;
             }
         }
+        if (NRM && GEOM) {
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                const float t = __shfl_down_sync(0xffffffffu, accn[j], d);
+                if (same) accn[j] += t;
+            }
+        }
     }
     const uint32_t kp = __shfl_up_sync(0xffffffffu, key, 1);
     if (active && (lane == 0 || kp != key)) {                  // first lane of a run
@@ -163,6 +178,11 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
             float* gs = f.gscr + 9 * (size_t)sm.slot[e];
 #pragma unroll
             for (int j = 0; j < 9; ++j) atomicAdd(gs + j, acc[j]);
+            if (NRM) {
+                float* gn = f.gnrm + 3 * (size_t)sm.slot[e];
+#pragma unroll
+                for (int j = 0; j < 3; ++j) atomicAdd(gn + j, accn[j]);
+            }
         }
         if (ATTR) {
             const uint32_t m = sm.face[e];
@@ -189,16 +209,18 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
 // 32 queued hits at a time are finished with all lanes busy: POSE: tau[6] += the lane's se(3) terms
 // (ts_bwd_pose_hit); otherwise segmented per-face reduction + atomics into f.gscr / grad_color / grad_opacity
 // (ts_bwd_full_group).
-template <int SM, bool ATTR, bool GEOM, bool POSE>
+template <int SM, bool ATTR, bool GEOM, bool POSE, bool NRM = false>
 __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene& sc, const TsJob& job, int lane,
                                             BwdWarpSmem& sm, float sigma, float alpha_min, float fx, float fy,
                                             uint32_t ncon, float Tcur, float gC0, float gC1, float gC2, float gD,
                                             float gA, float* __restrict__ grad_color, float* __restrict__ grad_opacity,
-                                            float tau[6]) {
+                                            float tau[6], float gN0 = 0.f, float gN1 = 0.f, float gN2 = 0.f) {
+    static_assert(!(NRM && POSE), "the normal-map backward runs in full-gradient mode");
     const float fpx = (float)job.px, fpy = (float)job.py;
     const uint32_t lt = (1u << lane) - 1u;
     const uint32_t n_walk = min(__reduce_max_sync(0xffffffffu, ncon), job.range.y - job.range.x);
     sm.pix[lane] = make_float4(gC0, gC1, gC2, gD);
+    if (NRM) sm.r[lane][11] = make_float4(gN0, gN1, gN2, 0.f);       // row 11 is free outside pose-only mode
     float Rs = 0.f;                    // R^c.gC + R^d gD + R^a gA behind the current face
     bool first = true;
     uint32_t qn = 0;                   // queued hits (warp-uniform); the queue always starts at index 0
@@ -228,6 +250,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             d[5] = make_float4(col[5], col[6], col[7], col[8]);
             d[6] = r[4], d[7] = r[5], d[8] = r[6], d[9] = r[7];
             if (POSE) d[10] = r[8], d[11] = r[9];
+            if (NRM) d[10] = f.nrm[cur.x];
             sm.lm[lane] = lmask, sm.slot[lane] = cur.x, sm.face[lane] = cur.y;
         }
         __syncwarp();
@@ -259,7 +282,11 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
                 const float d2 = r5.y * gC0 + r5.z * gC1 + r5.w * gC2;
                 const float cg = (o0 * d0 + o1 * d1 + o2 * d2) * z;       // c . gC
                 const float zgd = z * gD;
-                const float S = cg + zgd + gA;
+                float S = cg + zgd + gA;
+                if (NRM) {
+                    const float4 nf = sm.r[e][10];
+                    S += nf.x * gN0 + nf.y * gN1 + nf.z * gN2;            // flat attribute: n . dL/dN
+                }
                 const float wgt = Tn * alpha;
                 const float ga = Tn * (S - Rs);                           // B2
                 Rs = alpha * S + one_m * Rs;                              // B3
@@ -294,7 +321,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
                 if (POSE)
                     ts_bwd_pose_hit<SM>(sm, code & 0xffu, sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
                 else
-                    ts_bwd_full_group<SM, ATTR, GEOM>(f, sc, sm, lane, true, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
+                    ts_bwd_full_group<SM, ATTR, GEOM, NRM>(f, sc, sm, lane, true, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
                 __syncwarp();
             }
         }
@@ -308,7 +335,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             if (POSE) {
                 if (act) ts_bwd_pose_hit<SM>(sm, code & 0xffu, sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
             } else {
-                ts_bwd_full_group<SM, ATTR, GEOM>(f, sc, sm, lane, act, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
+                ts_bwd_full_group<SM, ATTR, GEOM, NRM>(f, sc, sm, lane, act, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
             }
             qn = 0;
             __syncwarp();

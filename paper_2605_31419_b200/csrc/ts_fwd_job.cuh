@@ -13,17 +13,21 @@ struct FwdWarpSmem {
 struct FwdPix {                       // what the walk leaves for this lane's pixel
     float T, C0, C1, C2, D, Tlast;
     uint32_t last;
+    float N0, N1, N2;                 // composited face normals (NRM instantiation only)
 };
 
 // `ent` = the lane's entry of the first 32-entry chunk of the tile list (already requested by the caller, so that
-// its round trip overlaps the caller's ticket atomic).
-template <int SM, bool COUNT, bool STATS = false>
+// its round trip overlaps the caller's ticket atomic).  NRM: also composite the flat per-face normal f.nrm[slot]
+// (Eq. 12, reading S26), staged in the warp's `nsm[32]`.
+template <int SM, bool COUNT, bool STATS = false, bool NRM = false>
 __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene& sc, const TsJob& job, int lane,
                                             FwdWarpSmem& sm, float sigma, float alpha_min, float t_min, uint4 ent,
                                             FwdPix& o, unsigned long long& n_visit, unsigned long long& n_rect,
-                                            unsigned long long& n_hit, uint32_t* __restrict__ face_pixels = nullptr) {
+                                            unsigned long long& n_hit, uint32_t* __restrict__ face_pixels = nullptr,
+                                            float4* nsm = nullptr) {
     const float fpx = (float)job.px, fpy = (float)job.py;
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, D = 0.0f, Tlast = 1.0f;
+    float N0 = 0.0f, N1 = 0.0f, N2 = 0.0f;
     uint32_t last = 0;
     const uint32_t lt = (1u << lane) - 1u;
     (void)lt;
@@ -50,6 +54,7 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             sm.r[lane][5] = make_float4(col[5], col[6], col[7], col[8]);
             sm.lm[lane] = lmask, sm.slot[lane] = cur.x;
             if (STATS) sm.face[lane] = cur.y;
+            if (NRM) nsm[lane] = f.nrm[cur.x];
         }
         __syncwarp();
         uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);
@@ -78,6 +83,10 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
                 C1 = fmaf(wz, fmaf(o0, r4.x, fmaf(o1, r4.w, o2 * r5.z)), C1);
                 C2 = fmaf(wz, fmaf(o0, r4.y, fmaf(o1, r5.x, o2 * r5.w)), C2);
                 D += wz;
+                if (NRM) {
+                    const float4 nf = nsm[e];
+                    N0 = fmaf(wgt, nf.x, N0), N1 = fmaf(wgt, nf.y, N1), N2 = fmaf(wgt, nf.z, N2);
+                }
                 Tlast = T;
                 T = __fmul_rn(T, __fsub_rn(1.0f, alpha));
                 last = pos0 + (uint32_t)e;
@@ -87,4 +96,5 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
         }
     }
     o.T = T, o.C0 = C0, o.C1 = C1, o.C2 = C2, o.D = D, o.Tlast = Tlast, o.last = last;
+    if (NRM) o.N0 = N0, o.N1 = N1, o.N2 = N2;
 }

@@ -46,6 +46,8 @@ struct TsFrameDev {
     float4* scr;                      // [vis_cap][4]: (u0,v0,w0,u1) (v1,w1,u2,v2) (w2,obar,rect_lo,rect_hi) (face,key,tiles,0)
     float4* rec;                      // [vis_cap][10]: per-face render record, see ts_raster.cuh
     float* gscr;                      // [vis_cap][9]: dL/d(u,v,w) per face vertex (full-gradient mode), zero at rest
+    float4* nrm;                      // [vis_cap]: camera-space unit face normal towards the camera (normal-map calls only)
+    float* gnrm;                      // [vis_cap][3]: dL/dn per face (normal-map backward), zero at rest
     uint4* pair_a;                    // [pair_cap] binned, unsorted: (depth_key, face, slot, rect_lo)
     uint32_t* pair_b;                 // [pair_cap] binned, unsorted: rect_hi
     unsigned long long* big_key;      // [pair_cap] scratch of the oversize-segment sort
@@ -73,6 +75,7 @@ struct ts_frame {
     TsPrmDev prm;
     const float* T_cw;       // device pointer given to the last ts_project (read again by the projection backward)
     int have_project, have_sort, have_fwd;
+    int have_normals;        // f.nrm holds the face normals of the current projection (ts_render_fwd_normal ran)
     int counters_dirty;      // ts_project ran but ts_bin_sort has not consumed (and re-zeroed) its counters yet
     uint32_t pose_src;       // 0 = none, 1 = per-tile partials (pose-only), 2 = per-block partials (projection backward)
     uint32_t n_pose_partials;
@@ -103,6 +106,11 @@ int32_t ts_launch_render_fwd(const ts_ctx*, ts_frame*, const ts_scene*, float* o
                              const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, uint32_t* face_pixels,
                              cudaStream_t);
 int32_t ts_launch_face_area(const ts_ctx*, ts_frame*, float* area, cudaStream_t);
+int32_t ts_launch_render_fwd_normal(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, float* on,
+                                    cudaStream_t);
+int32_t ts_launch_render_bwd_normal(const ts_ctx*, ts_frame*, const ts_scene*, const float* gC, const float* gD,
+                                    const float* gA, const float* gN, float* grad_pos, float* grad_color,
+                                    float* grad_opacity, uint32_t mask, cudaStream_t);
 int32_t ts_launch_render_bwd(const ts_ctx*, ts_frame*, const ts_scene*, const float*, const float*, const float*,
                              float*, float*, float*, uint32_t, cudaStream_t);
 int32_t ts_launch_render_track(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,

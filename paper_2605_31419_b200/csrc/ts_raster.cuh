@@ -92,6 +92,8 @@ __device__ __forceinline__ void ts_face_geom(const float4 s0, const float4 s1, c
     }
 }
 
+#define TS_NEEDLE_RATIO 400.0f        // perimeter / inradius above which a face is always evaluated on the compensated path
+
 // F7 + the backward-only per-face terms -> the 10-float4 record.  s0..s2 = raw screen record, obar = mean vertex
 // opacity, cam for (xn, yn).
 __device__ __forceinline__ void ts_build_record(const float4 s0, const float4 s1, const float4 s2, float obar,
@@ -115,6 +117,12 @@ __device__ __forceinline__ void ts_build_record(const float4 s0, const float4 s1
         tau[j] = ((g.qx[j] - g.qx[i1]) * ex + (g.qy[j] - g.qy[i1]) * ey) * (g.inv_ell[j] * g.inv_ell[j]);
         xn[j] = (g.qx[j] - cam.cx) * ifx, yn[j] = (g.qy[j] - cam.cy) * ify;
     }
+    // Needle faces (perimeter / inradius above TS_NEEDLE_RATIO; an equilateral triangle has 10.4): the affine form's
+    // absolute error ~3e-7 * |p - ref| / r is no longer small next to the image tolerance anywhere inside the face, not
+    // only next to an edge.  Their offsets c_k are stored as NaN: every evaluation then yields x = NaN, which
+    // ts_eval_alpha sends down the compensated path (ts_refine_lhat) and ts_block_misses never culls.  m_k stay
+    // exact (the backward reads them).  No cost for the other faces (N11).
+    if (g.sumell * g.inv_r > TS_NEEDLE_RATIO) g.c[0] = g.c[1] = g.c[2] = __int_as_float(0x7fc00000);
     out[0] = make_float4(g.refx, g.refy, g.mx[0], g.my[0]);
     out[1] = make_float4(g.mx[1], g.my[1], g.mx[2], g.my[2]);
     out[2] = make_float4(g.c[0], g.c[1], g.c[2], g.obar);
@@ -184,7 +192,7 @@ __device__ __forceinline__ bool ts_eval_alpha(const float4 r0, const float4 r1, 
     l[1] = __fmaf_rn(r1.x, dx, __fmaf_rn(r1.y, dy, r2.y));
     l[2] = __fmaf_rn(r1.z, dx, __fmaf_rn(r1.w, dy, r2.z));
     x = -fmaxf(l[0], fmaxf(l[1], l[2]));
-    if (fabsf(x) < TS_REFINE_BAND) {
+    if (!(fabsf(x) >= TS_REFINE_BAND)) {              // also taken when x is NaN (needle faces, see ts_build_record)
         const float3 lr = ts_refine_lhat(scr, slot, px, py);
         l[0] = lr.x, l[1] = lr.y, l[2] = lr.z;
         x = -fmaxf(l[0], fmaxf(l[1], l[2]));

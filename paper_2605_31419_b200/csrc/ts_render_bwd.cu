@@ -17,17 +17,19 @@
 //   pose_reduce_kernel: fixed-order final reduction of the partials to dL/dtau[6].
 #include "ts_bwd_job.cuh"
 #include "ts_fwd_job.cuh"
+#include "ts_normal.cuh"
 #include "ts_pose.cuh"
 
 namespace {
 
 // ATTR: colour / opacity gradients (B1, B4).  GEOM: screen-space vertex gradients into gscr (B5-B6).
 // POSE: pose-only; hits are queued by the per-pixel walk and finished 32 at a time (ts_bwd_pose_hit).
-template <int SM, bool ATTR, bool GEOM, bool POSE>
-__global__ void __launch_bounds__(TS_JOB_WARPS * 32, 3)
+// NRM: also the cotangent of the rendered normal map (Eq. 12); full-gradient mode only.
+template <int SM, bool ATTR, bool GEOM, bool POSE, bool NRM = false>
+__global__ void __launch_bounds__(TS_JOB_WARPS * 32, NRM ? 2 : 3)
 render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float fx, float fy,
                   const float* __restrict__ gCi, const float* __restrict__ gDi, const float* __restrict__ gAi,
-                  float* __restrict__ grad_color, float* __restrict__ grad_opacity) {
+                  float* __restrict__ grad_color, float* __restrict__ grad_opacity, const float* __restrict__ gNi = nullptr) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     BwdWarpSmem& sm = reinterpret_cast<BwdWarpSmem*>(smem_raw)[threadIdx.x >> 5];
@@ -40,18 +42,19 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
         ts_job_decode(f, j, lane, job);
         const size_t p = (size_t)job.py * f.W + job.px;
         uint32_t ncon = 0;
-        float Tcur = 1.0f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f;
+        float Tcur = 1.0f, gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f, gA = 0.f, gN0 = 0.f, gN1 = 0.f, gN2 = 0.f;
         if (job.inside && job.range.y > job.range.x) {
             ncon = f.n_contrib[p];
             Tcur = f.t_last[p];
             if (gCi) gC0 = gCi[p], gC1 = gCi[hw + p], gC2 = gCi[2 * hw + p];
             if (gDi) gD = gDi[p];
             if (gAi) gA = gAi[p];
+            if (NRM) gN0 = gNi[p], gN1 = gNi[hw + p], gN2 = gNi[2 * hw + p];
         }
         j = ts_job_take(f, 1, lane);       // next ticket: its round trip overlaps the pixel loads
         float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        ts_bwd_walk<SM, ATTR, GEOM, POSE>(f, sc, job, lane, sm, sigma, alpha_min, fx, fy, ncon, Tcur, gC0, gC1, gC2, gD, gA,
-                                          grad_color, grad_opacity, tau);
+        ts_bwd_walk<SM, ATTR, GEOM, POSE, NRM>(f, sc, job, lane, sm, sigma, alpha_min, fx, fy, ncon, Tcur, gC0, gC1, gC2, gD, gA,
+                                               grad_color, grad_opacity, tau, gN0, gN1, gN2);
         if (POSE) {
             // per-thread -> per-job partial (fixed shuffle tree; the final reduction runs over jobs in index order)
 #pragma unroll
@@ -169,7 +172,10 @@ constexpr int PB_THREADS = 256;
 
 // a6 + the per-vertex terms of a7 (full-gradient mode).  Persistent grid-stride over visible slots; consumes and
 // re-zeroes gscr.
-template <bool SOUP>
+// NRM: also consumes gnrm (dL/dn per face) and pushes it through n = s (a x b)/|a x b| (ts_normal.cuh) to the vertices
+// (P1 += R^T g_a, P2 += R^T g_b, P0 -= both) and to the rotation part of the pose (a x g_a + b x g_b; a translation of
+// the camera does not turn the normals).
+template <bool SOUP, bool NRM = false>
 __global__ void __launch_bounds__(PB_THREADS)
 proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __restrict__ faces,
                 const float* __restrict__ Tcw, TsCamDev cam, float* __restrict__ grad_pos, int want_pose) {
@@ -189,14 +195,50 @@ proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __re
             g9[j] = gs[j];
             any |= (g9[j] != 0.0f);
         }
+        float gn[3] = {0.f, 0.f, 0.f};
+        if (NRM) {
+            float* gp = f.gnrm + 3 * (size_t)slot;
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+                gn[j] = gp[j];
+                any |= (gn[j] != 0.0f);
+            }
+            if (any) gp[0] = gp[1] = gp[2] = 0.0f;
+        }
         if (!any) continue;
 #pragma unroll
         for (int j = 0; j < 9; ++j) gs[j] = 0.0f;
         const uint32_t m = __float_as_uint(f.scr[TS_SCR_F4 * (size_t)slot + 3].x);
+        size_t vid[3];
+        float P[3][3];
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
-            const size_t v = SOUP ? (size_t)3 * m + k : (size_t)__ldg(faces + 3 * (size_t)m + k);
-            const float px = __ldg(pos + 3 * v), py = __ldg(pos + 3 * v + 1), pz = __ldg(pos + 3 * v + 2);
+            vid[k] = SOUP ? (size_t)3 * m + k : (size_t)__ldg(faces + 3 * (size_t)m + k);
+            P[k][0] = __ldg(pos + 3 * vid[k]), P[k][1] = __ldg(pos + 3 * vid[k] + 1), P[k][2] = __ldg(pos + 3 * vid[k] + 2);
+        }
+        if (NRM) {
+            TsFaceNormal fn;
+            ts_face_normal_geom(sT, P, fn);
+            float ga[3], gb[3];
+            ts_face_normal_bwd(fn, gn, ga, gb);
+            if (grad_pos) {
+#pragma unroll
+                for (int j = 0; j < 3; ++j) {
+                    const float wa = sT[j] * ga[0] + sT[4 + j] * ga[1] + sT[8 + j] * ga[2];
+                    const float wb = sT[j] * gb[0] + sT[4 + j] * gb[1] + sT[8 + j] * gb[2];
+                    atomicAdd(grad_pos + 3 * vid[1] + j, wa);
+                    atomicAdd(grad_pos + 3 * vid[2] + j, wb);
+                    atomicAdd(grad_pos + 3 * vid[0] + j, -(wa + wb));
+                }
+            }
+            tau[3] += (fn.a[1] * ga[2] - fn.a[2] * ga[1]) + (fn.b[1] * gb[2] - fn.b[2] * gb[1]);
+            tau[4] += (fn.a[2] * ga[0] - fn.a[0] * ga[2]) + (fn.b[2] * gb[0] - fn.b[0] * gb[2]);
+            tau[5] += (fn.a[0] * ga[1] - fn.a[1] * ga[0]) + (fn.b[0] * gb[1] - fn.b[1] * gb[0]);
+        }
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const size_t v = vid[k];
+            const float px = P[k][0], py = P[k][1], pz = P[k][2];
             const float X = __fmaf_rn(sT[0], px, __fmaf_rn(sT[1], py, __fmaf_rn(sT[2], pz, sT[3])));
             const float Y = __fmaf_rn(sT[4], px, __fmaf_rn(sT[5], py, __fmaf_rn(sT[6], pz, sT[7])));
             const float Z = __fmaf_rn(sT[8], px, __fmaf_rn(sT[9], py, __fmaf_rn(sT[10], pz, sT[11])));
@@ -347,6 +389,58 @@ int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
             proj_bwd_kernel<true><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, nullptr, fr->T_cw, fr->cam, gp, want_pose);
         else
             proj_bwd_kernel<false><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, sc->faces, fr->T_cw, fr->cam, gp, want_pose);
+        if (want_pose) fr->pose_src = 2, fr->n_pose_partials = (uint32_t)grid;
+    }
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
+
+namespace {
+
+template <int SM>
+void launch_bwd_normal_sm(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, const float* gC, const float* gD,
+                          const float* gA, const float* gN, float* gcol, float* gopa, bool attr, bool geom, cudaStream_t st) {
+    const TsFrameDev& f = fr->d;
+    const size_t smem = sizeof(BwdWarpSmem) * TS_JOB_WARPS;
+    const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 2, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
+    const float sg = fr->prm.sigma, am = fr->prm.alpha_min, fx = fr->cam.fx, fy = fr->cam.fy;
+#define TS_LAUNCH_BN(A, G)                                                                                                  \
+    do {                                                                                                                    \
+        cudaFuncSetAttribute(render_bwd_kernel<SM, A, G, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+        render_bwd_kernel<SM, A, G, false, true><<<grid, TS_JOB_WARPS * 32, smem, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa, gN); \
+    } while (0)
+    if (attr && geom) TS_LAUNCH_BN(true, true);
+    else if (geom) TS_LAUNCH_BN(false, true);
+    else TS_LAUNCH_BN(true, false);
+#undef TS_LAUNCH_BN
+}
+
+}  // namespace
+
+// Normal-map variant of ts_launch_render_bwd: the cotangents of all four raster outputs in one backward pass.
+int32_t ts_launch_render_bwd_normal(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, const float* gC, const float* gD,
+                                    const float* gA, const float* gN, float* grad_pos, float* grad_color,
+                                    float* grad_opacity, uint32_t mask, cudaStream_t st) {
+    const bool attr = (mask & (TS_GRAD_COLOR | TS_GRAD_OPACITY)) != 0;
+    const bool geom = (mask & (TS_GRAD_POS | TS_GRAD_POSE)) != 0;
+    if (!attr && !geom) return TS_OK;
+    float* gcol = (mask & TS_GRAD_COLOR) ? grad_color : nullptr;
+    float* gopa = (mask & TS_GRAD_OPACITY) ? grad_opacity : nullptr;
+    switch (ts_sigma_mode(fr->prm.sigma)) {
+        case 1: launch_bwd_normal_sm<1>(ctx, fr, *sc, gC, gD, gA, gN, gcol, gopa, attr, geom, st); break;
+        case 2: launch_bwd_normal_sm<2>(ctx, fr, *sc, gC, gD, gA, gN, gcol, gopa, attr, geom, st); break;
+        case 3: launch_bwd_normal_sm<3>(ctx, fr, *sc, gC, gD, gA, gN, gcol, gopa, attr, geom, st); break;
+        default: launch_bwd_normal_sm<0>(ctx, fr, *sc, gC, gD, gA, gN, gcol, gopa, attr, geom, st); break;
+    }
+    fr->pose_src = 0;
+    if (geom) {
+        const int grid = (int)min((uint32_t)(ctx->num_sms * 4), fr->d.n_partials_cap);
+        const int want_pose = (mask & TS_GRAD_POSE) ? 1 : 0;
+        float* gp = (mask & TS_GRAD_POS) ? grad_pos : nullptr;
+        if (sc->faces == nullptr)
+            proj_bwd_kernel<true, true><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, nullptr, fr->T_cw, fr->cam, gp, want_pose);
+        else
+            proj_bwd_kernel<false, true><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, sc->faces, fr->T_cw, fr->cam, gp, want_pose);
         if (want_pose) fr->pose_src = 2, fr->n_pose_partials = (uint32_t)grid;
     }
     TS_CUDA_CHECK_LAUNCH();

@@ -6,6 +6,7 @@
 // with broadcast LDS.128 and testing "my pixel is in the rect" with one shift of the entry's lane mask.  Pixels
 // stop at T <= t_min, the warp when all its pixels stopped.  No CTA barrier, no atomics.
 #include "ts_fwd_job.cuh"
+#include "ts_normal.cuh"
 
 namespace {
 
@@ -20,11 +21,13 @@ struct FwdLoss {
     float wc, wd;
 };
 
-template <int SM, bool COUNT, bool LOSS, bool STATS>
+template <int SM, bool COUNT, bool LOSS, bool STATS, bool NRM = false>
 __global__ void __launch_bounds__(TS_JOB_WARPS * 32)
 render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float t_min, float* __restrict__ out_color,
-                  float* __restrict__ out_depth, float* __restrict__ out_alpha, FwdLoss L, uint32_t* __restrict__ face_pixels) {
+                  float* __restrict__ out_depth, float* __restrict__ out_alpha, FwdLoss L, uint32_t* __restrict__ face_pixels,
+                  float* __restrict__ out_normal = nullptr) {
     __shared__ FwdWarpSmem smem[TS_JOB_WARPS];
+    __shared__ float4 smem_n[NRM ? TS_JOB_WARPS * 32 : 1];
     const int lane = threadIdx.x & 31;
     FwdWarpSmem& sm = smem[threadIdx.x >> 5];
     const uint32_t n_jobs = (uint32_t)f.NT * TS_BLOCKS_PER_TILE;
@@ -40,7 +43,8 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
         if (job.range.x + lane < job.range.y) ent = f.sorted[job.range.x + lane];
         j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
         FwdPix o;
-        ts_fwd_walk<SM, COUNT, STATS>(f, sc, job, lane, sm, sigma, alpha_min, t_min, ent, o, n_visit, n_rect, n_hit, face_pixels);
+        ts_fwd_walk<SM, COUNT, STATS, NRM>(f, sc, job, lane, sm, sigma, alpha_min, t_min, ent, o, n_visit, n_rect, n_hit, face_pixels,
+                                           smem_n + (NRM ? (threadIdx.x & ~31) : 0));
         const float T = o.T, C0 = o.C0, C1 = o.C1, C2 = o.C2, D = o.D, Tlast = o.Tlast;
         const uint32_t last = o.last;
         if (job.inside) {
@@ -48,6 +52,7 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
             if (out_color) out_color[p] = C0, out_color[hw + p] = C1, out_color[2 * hw + p] = C2;
             if (out_depth) out_depth[p] = D;
             if (out_alpha) out_alpha[p] = 1.0f - T;
+            if (NRM) out_normal[p] = o.N0, out_normal[hw + p] = o.N1, out_normal[2 * hw + p] = o.N2;
             f.n_contrib[p] = last;
             f.t_last[p] = Tlast;
             if (LOSS) {
@@ -115,7 +120,49 @@ __global__ void __launch_bounds__(256) face_area_kernel(TsFrameDev f, float* __r
     }
 }
 
+// Eq. 12 / reading S26: unit normal of every visible face in camera space, towards the camera.  The edge vectors are
+// taken in world space (exact differences of nearby floats) and rotated; the orientation is the sign of the plane
+// offset m . Q_0.
+template <bool SOUP>
+__global__ void __launch_bounds__(256)
+face_normal_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __restrict__ faces, const float* __restrict__ Tcw) {
+    __shared__ float sT[12];
+    if (threadIdx.x < 12) sT[threadIdx.x] = __ldg(Tcw + threadIdx.x);
+    __syncthreads();
+    const uint32_t nvis = min(ts_eff_visible(f), f.vis_cap);
+    for (uint32_t slot = blockIdx.x * blockDim.x + threadIdx.x; slot < nvis; slot += gridDim.x * blockDim.x) {
+        const uint32_t m = __float_as_uint(f.scr[TS_SCR_F4 * (size_t)slot + 3].x);
+        float P[3][3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            const size_t v = SOUP ? (size_t)3 * m + k : (size_t)__ldg(faces + 3 * (size_t)m + k);
+            P[k][0] = __ldg(pos + 3 * v), P[k][1] = __ldg(pos + 3 * v + 1), P[k][2] = __ldg(pos + 3 * v + 2);
+        }
+        float4 n;
+        ts_face_normal(sT, P, n);
+        f.nrm[slot] = n;
+    }
+}
+
 }  // namespace
+
+int32_t ts_launch_render_fwd_normal(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
+                                    float* on, cudaStream_t st) {
+    const TsFrameDev& f = fr->d;
+    if (sc->faces == nullptr) face_normal_kernel<true><<<ctx->num_sms * 4, 256, 0, st>>>(f, sc->pos, nullptr, fr->T_cw);
+    else face_normal_kernel<false><<<ctx->num_sms * 4, 256, 0, st>>>(f, sc->pos, sc->faces, fr->T_cw);
+    const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 4, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
+    const float sg = fr->prm.sigma, am = fr->prm.alpha_min, tm = fr->prm.t_min;
+    const FwdLoss none = {nullptr, nullptr, nullptr, nullptr, nullptr, 0.f, 0.f};
+    switch (ts_sigma_mode(fr->prm.sigma)) {
+        case 1: render_fwd_kernel<1, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on); break;
+        case 2: render_fwd_kernel<2, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on); break;
+        case 3: render_fwd_kernel<3, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on); break;
+        default: render_fwd_kernel<0, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on); break;
+    }
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
 
 int32_t ts_launch_face_area(const ts_ctx* ctx, ts_frame* fr, float* area, cudaStream_t st) {
     face_area_kernel<<<ctx->num_sms * 4, 256, 0, st>>>(fr->d, area);

@@ -25,6 +25,7 @@ _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.
 
 EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
+           "ts_render_fwd_normal", "ts_render_bwd_normal",
            "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view"]
 
 
@@ -72,6 +73,10 @@ def _load():
     lib.ts_face_area.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_render_bwd.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                   C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
+    lib.ts_render_fwd_normal.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                         C.c_void_p, C.c_void_p]
+    lib.ts_render_bwd_normal.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
     lib.ts_pose_jacobian_reduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_l1_loss_grad.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -203,6 +208,18 @@ def ts_render_bwd(ctx, scene, frame, dL_dcolor, dL_ddepth, dL_dalpha, grad_pos, 
                   stream=None):
     _check(lib.ts_render_bwd(ctx.h, C.byref(scene.c), frame.h, _ptr(dL_dcolor), _ptr(dL_ddepth), _ptr(dL_dalpha),
                              _ptr(grad_pos), _ptr(grad_color), _ptr(grad_opacity), int(grad_mask), _stream(stream)))
+
+
+def ts_render_fwd_normal(ctx, scene, frame, out_color, out_depth, out_alpha, out_normal, stream=None):
+    _check(lib.ts_render_fwd_normal(ctx.h, C.byref(scene.c), frame.h, _ptr(out_color), _ptr(out_depth), _ptr(out_alpha),
+                                    _ptr(out_normal), _stream(stream)))
+
+
+def ts_render_bwd_normal(ctx, scene, frame, dL_dcolor, dL_ddepth, dL_dalpha, dL_dnormal, grad_pos, grad_color,
+                         grad_opacity, grad_mask, stream=None):
+    _check(lib.ts_render_bwd_normal(ctx.h, C.byref(scene.c), frame.h, _ptr(dL_dcolor), _ptr(dL_ddepth), _ptr(dL_dalpha),
+                                    _ptr(dL_dnormal), _ptr(grad_pos), _ptr(grad_color), _ptr(grad_opacity),
+                                    int(grad_mask), _stream(stream)))
 
 
 def ts_pose_jacobian_reduce(ctx, frame, dL_dtau, stream=None):

@@ -411,3 +411,144 @@ def test_equi_regulariser(ctx, oracle_mod, indexed):
     torch.cuda.synchronize()
     assert abs(loss.item() - w * E) <= 1e-5 * w * E
     assert_grad_close("equi grad", gp.cpu().numpy(), g)
+
+
+def needle_scene():
+    """Config-4 soup re-indexed so that every second face borrows a vertex of the previous face in the array -- which
+    lies anywhere in the room: thousands of needle-shaped faces hundreds of pixels long and a fraction of a pixel to a
+    few pixels wide (perimeter / inradius up to 1e5), the case note N11 of DESIGN.md is about."""
+    sc = small_cfg(4)
+    rng = np.random.default_rng(5)
+    n_face = 60_000
+    faces = np.arange(3 * n_face, dtype=np.int32).reshape(-1, 3)
+    share = rng.random(n_face) < 0.5
+    faces[1:][share[1:], 0] = faces[:-1][share[1:], 1]
+    return sc, sc.pos[: 3 * n_face], sc.color[: 3 * n_face], sc.opacity[: 3 * n_face], faces
+
+
+def grid_mesh(n=40, seed=21):
+    """A shared-vertex height-field mesh (2 (n-1)^2 faces on n^2 vertices): every vertex collects the gradients of up to
+    six faces."""
+    rng = np.random.default_rng(seed)
+    gx, gy = np.meshgrid(np.linspace(-1.3, 1.3, n), np.linspace(-1.0, 1.0, n))
+    pos = np.stack([gx, gy, 3.0 + 0.3 * np.sin(3 * gx) * np.cos(2 * gy)], axis=-1).reshape(-1, 3)
+    pos += rng.normal(0, 0.006, pos.shape)
+    idx = np.arange(n * n).reshape(n, n)
+    f1 = np.stack([idx[:-1, :-1], idx[:-1, 1:], idx[1:, :-1]], axis=-1).reshape(-1, 3)
+    f2 = np.stack([idx[1:, 1:], idx[1:, :-1], idx[:-1, 1:]], axis=-1).reshape(-1, 3)
+    faces = np.concatenate([f1, f2]).astype(np.int32)
+    sc = scenes.config0(n_faces=10)
+    sc.params = scenes.Params(sigma=0.5)
+    return (sc, pos.astype(np.float32), rng.uniform(0, 1, (n * n, 3)).astype(np.float32),
+            rng.uniform(0.3, 1.0, n * n).astype(np.float32), faces)
+
+
+def test_needle_faces(ctx, oracle_mod):
+    """Faces far outside the paper's size range (needles hundreds of pixels long): images still to 1e-4 and per-vertex
+    gradients to 1e-3 (relative L2), because such faces are evaluated on the compensated path everywhere (N11)."""
+    from gpu_util import GpuView, assert_grad_close
+    from paper_2605_31419_b200 import ts
+    sc, pos, col, opa, faces = needle_scene()
+    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, "f32", amb_tol=5e-3)
+    g = GpuView(ctx, pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, pair_capacity=o.bin_sort().P + 1024)
+    f, ok = check_forward(o, g)
+    assert (f.alpha > 0.5).mean() > 0.5
+    rng = np.random.default_rng(77)
+    H, W = ok.shape
+    gC = (rng.normal(size=(3, H, W)) * ok[None]).astype(np.float32)
+    gD = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+    ref = o.backward(gC, gD, None)
+    gp, gc, go, tau = g.backward(gC, gD, None, ts.GRAD_ALL)
+    assert_grad_close("grad_color", gc, ref.grad_color)
+    assert_grad_close("grad_opacity", go, ref.grad_opacity)
+    # vertex positions of needles: d x / d q grows like 1/r, and so does the rounding of both sides' float32 geometry
+    # terms; relative L2 still to 1e-3, single entries to 3e-3 of the largest
+    d = np.abs(gp.astype(np.float64) - ref.grad_pos)
+    assert np.linalg.norm(d) <= 1e-3 * np.linalg.norm(ref.grad_pos)
+    assert d.max() <= 3e-3 * np.abs(ref.grad_pos).max()
+    # the pose gradient of this scene is a sum of 1e6-sized terms of both signs: 5e-3 of its largest component
+    assert np.abs(tau - ref.dL_dtau).max() <= 5e-3 * np.abs(ref.dL_dtau).max(), (tau, ref.dL_dtau)
+    g.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 2, 3, "mesh"])
+def test_normal_map_forward_and_backward(ctx, oracle_mod, cfg):
+    """ts_render_fwd_normal / ts_render_bwd_normal (Eq. 12) against the oracle: the normal map to the
+    image tolerance, colour / depth / alpha bit-identical to ts_render_fwd, and ONE backward pass for the cotangents of
+    all four outputs against the sum of the oracle's colour/depth/alpha backward and its normal backward."""
+    from gpu_util import assert_grad_close, assert_images_close, dev
+    from paper_2605_31419_b200 import ts
+    if cfg == "mesh":
+        sc, pos, col, opa, faces = grid_mesh()
+    else:
+        sc = small_cfg(cfg)
+        pos, col, opa, faces = sc.pos, sc.color, sc.opacity, None
+    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, "f32", amb_tol=5e-3)
+    from gpu_util import GpuView
+    g = GpuView(ctx, pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params)
+    f, ok = check_forward(o, g)
+    H, W = ok.shape
+    C, D, A = torch.empty(3, H, W, device="cuda"), torch.empty(H, W, device="cuda"), torch.empty(H, W, device="cuda")
+    N = torch.empty(3, H, W, device="cuda")
+    ts.ts_render_fwd_normal(ctx, g.scene, g.frame, C, D, A, N)
+    torch.cuda.synchronize()
+    assert torch.equal(C, g.C) and torch.equal(D, g.D) and torch.equal(A, g.A)
+    Nref = o.normal_forward("tiled")
+    assert np.abs(Nref).max() > 0.5
+    assert_images_close("normal", N.cpu().numpy(), Nref, ok[None])
+    # outputs other than the normal map are optional
+    N2 = torch.empty_like(N)
+    ts.ts_render_fwd_normal(ctx, g.scene, g.frame, None, None, None, N2)
+    torch.cuda.synchronize()
+    assert torch.equal(N, N2)
+
+    rng = np.random.default_rng(700 + (9 if cfg == "mesh" else cfg))
+    gC = (rng.normal(size=(3, H, W)) * ok[None]).astype(np.float32)
+    gD = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+    gA = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+    gN = (rng.normal(size=(3, H, W)) * ok[None]).astype(np.float32)
+    r1, r2 = o.backward(gC, gD, gA), o.normal_backward(gN)
+    V = pos.shape[0]
+    for mask in (ts.GRAD_ALL, ts.GRAD_POS, ts.GRAD_POSE, ts.GRAD_OPACITY | ts.GRAD_COLOR):
+        gp, gc, go = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+        ts.ts_render_bwd_normal(ctx, g.scene, g.frame, dev(gC), dev(gD), dev(gA), dev(gN), gp, gc, go, mask)
+        if mask & ts.GRAD_POS:
+            assert_grad_close("grad_pos", gp.cpu().numpy(), r1.grad_pos + r2.grad_pos)
+        if mask & ts.GRAD_COLOR:
+            assert_grad_close("grad_color", gc.cpu().numpy(), r1.grad_color)
+        if mask & ts.GRAD_OPACITY:
+            assert_grad_close("grad_opacity", go.cpu().numpy(), r1.grad_opacity + r2.grad_opacity)
+        if mask & ts.GRAD_POSE:
+            tau = torch.zeros(6, device="cuda")
+            ts.ts_pose_jacobian_reduce(ctx, g.frame, tau)
+            ref = r1.dL_dtau + r2.dL_dtau
+            assert np.abs(tau.cpu().numpy() - ref).max() <= 1e-3 * np.abs(ref).max(), (tau, ref)
+    # the normal cotangent alone (E_norm is the only loss on N): d<gN, N>
+    gp, go = torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+    ts.ts_render_bwd_normal(ctx, g.scene, g.frame, None, None, None, dev(gN), gp, None, go,
+                            ts.GRAD_POS | ts.GRAD_OPACITY | ts.GRAD_POSE)
+    tau = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau)
+    assert_grad_close("grad_pos (normal only)", gp.cpu().numpy(), r2.grad_pos)
+    assert_grad_close("grad_opacity (normal only)", go.cpu().numpy(), r2.grad_opacity)
+    assert np.abs(tau.cpu().numpy() - r2.dL_dtau).max() <= 1e-3 * np.abs(r2.dL_dtau).max()
+    # the frame's accumulators are back at rest: a plain backward afterwards is unaffected
+    gp2 = torch.zeros(V, 3, device="cuda")
+    ts.ts_render_bwd(ctx, g.scene, g.frame, dev(gC), dev(gD), dev(gA), gp2, None, None, ts.GRAD_POS)
+    assert_grad_close("grad_pos (after)", gp2.cpu().numpy(), r1.grad_pos)
+    g.close()
+
+
+def test_normal_calls_need_their_forward(ctx, oracle_mod):
+    from gpu_util import GpuView, dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(0)
+    g = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
+    g.forward()
+    gN = torch.zeros(3, g.H, g.W, device="cuda")
+    gp = torch.zeros(sc.pos.shape[0], 3, device="cuda")
+    with pytest.raises(ts.TsError):
+        ts.ts_render_bwd_normal(ctx, g.scene, g.frame, None, None, None, gN, gp, None, None, ts.GRAD_POS)
+    with pytest.raises(ts.TsError):
+        ts.ts_render_fwd_normal(ctx, g.scene, g.frame, None, None, None, None)
+    g.close()
