@@ -168,6 +168,13 @@ int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame
                              const float* dL_ddepth, const float* dL_dalpha, const float* dL_dnormal, float* grad_pos,
                              float* grad_color, float* grad_opacity, uint32_t grad_mask, void* stream);
 
+/* E_norm of E_map (Eq. 12 and 15; lambda_norm = 0.05): weight / (H W) * sum over the
+ * valid pixels (those with a sensor normal, Nbar_p != 0) of 1 - N_p . Nbar_p (reading S27).  N = the map of
+ * ts_render_fwd_normal, Nbar = sensor normals, both [3][H][W] device.  Writes gN[3][H][W] = the cotangent of N (input of
+ * ts_render_bwd_normal); adds the weighted loss to *loss_dev if not NULL. */
+int32_t ts_normal_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* N, const float* Nbar, float weight, float* gN,
+                            float* loss_dev, void* stream);
+
 /* a8: one Adam step on tau, then T_cw <- Exp(-delta) o T_cw, all on the device.
  * state_dev[13] = m[6], v[6], step; lr[6] passed by value (rho then theta). */
 int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev, const float* lr6,

@@ -643,6 +643,23 @@ double l1_loss(int32_t W, int32_t H, const T* C, const T* D, const T* Ch, const 
     return L;
 }
 
+// E_norm of Eq. 12: sum over the valid pixels of 1 - N_p . Nbar_p.  Reading S27 of DESIGN.md: a pixel
+// is valid where the sensor normal exists (Nbar_p != 0), and the sum is divided by H W like the other image terms.
+// N, Nbar, gN are [3][H][W]; gN receives weight * dE/dN; returns weight * E_norm.
+template <class T>
+double normal_loss(int32_t W, int32_t H, const T* N, const T* Nb, double weight, T* gN) {
+    const int64_t n = (int64_t)W * H;
+    const T w = (T)(weight / (double)n);
+    double L = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        const T b0 = Nb[i], b1 = Nb[n + i], b2 = Nb[2 * n + i];
+        const bool valid = b0 != 0 || b1 != 0 || b2 != 0;
+        if (valid) L += (double)w * (1.0 - ((double)N[i] * b0 + (double)N[n + i] * b1 + (double)N[2 * n + i] * b2));
+        gN[i] = valid ? -w * b0 : (T)0, gN[n + i] = valid ? -w * b1 : (T)0, gN[2 * n + i] = valid ? -w * b2 : (T)0;
+    }
+    return L;
+}
+
 // SE(3) exponential, tau = (rho, theta).  out = Exp(tau) o T.
 template <class T>
 void left_perturb(const T* Tcw, const T* tau, T* out) {
@@ -834,5 +851,12 @@ void tso_face_stats_f64(const double* color, const double* opacity, const int32_
     }
 TSO_NRM_FWD(float, f32)
 TSO_NRM_FWD(double, f64)
+
+double tso_normal_loss_f32(int32_t W, int32_t H, const float* N, const float* Nbar, double weight, float* gN) {
+    return normal_loss<float>(W, H, N, Nbar, weight, gN);
+}
+double tso_normal_loss_f64(int32_t W, int32_t H, const double* N, const double* Nbar, double weight, double* gN) {
+    return normal_loss<double>(W, H, N, Nbar, weight, gN);
+}
 
 }  // extern "C"

@@ -157,6 +157,11 @@ void tso_face_stats_f64(const double* color, const double* opacity, const int32_
 TSO_NRM_DECL(float, f32)
 TSO_NRM_DECL(double, f64)
 
+/* E_norm of Eq. 12: weight / (H W) * sum over valid pixels (Nbar_p != 0) of 1 - N_p . Nbar_p
+ * (reading S27).  N, Nbar, gN are [3][H][W]; gN receives the cotangent of N; returns the weighted loss. */
+double tso_normal_loss_f32(int32_t W, int32_t H, const float* N, const float* Nbar, double weight, float* gN);
+double tso_normal_loss_f64(int32_t W, int32_t H, const double* N, const double* Nbar, double weight, double* gN);
+
 /* SE(3) exponential, tau = (rho, theta): out[12] = Exp(tau) o T (3x4 row-major). */
 void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out);
 

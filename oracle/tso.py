@@ -54,6 +54,8 @@ def lib():
         _lib.tso_equi_f32.restype = C.c_double
         _lib.tso_equi_f64.restype = C.c_double
         _lib.tso_dssim_f64.restype = C.c_double
+        _lib.tso_normal_loss_f32.restype = C.c_double
+        _lib.tso_normal_loss_f64.restype = C.c_double
     return _lib
 
 
@@ -251,6 +253,17 @@ def equi(pos, faces=None, weight=1.0, prec="f64", grad=True):
     g = np.zeros_like(pos) if grad else None
     E = getattr(lib(), "tso_equi_" + prec)(_p(pos), _p(faces), C.c_int32(M), C.c_double(weight), _p(g))
     return E, g
+
+
+def normal_loss(N, Nbar, weight=1.0, prec="f64"):
+    """weight * E_norm (Eq. 12) of a rendered normal map N [3,H,W] against sensor normals Nbar; returns (L, dL/dN)."""
+    dt = np.float32 if prec == "f32" else np.float64
+    N, Nbar = np.ascontiguousarray(N, dt), np.ascontiguousarray(Nbar, dt)
+    assert N.shape == Nbar.shape and N.ndim == 3 and N.shape[0] == 3
+    g = np.zeros_like(N)
+    L = getattr(lib(), "tso_normal_loss_" + prec)(C.c_int32(N.shape[2]), C.c_int32(N.shape[1]), _p(N), _p(Nbar),
+                                                  C.c_double(weight), _p(g))
+    return L, g
 
 
 def dssim(x, y, prec="f64", grad=True):

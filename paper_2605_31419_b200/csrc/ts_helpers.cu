@@ -110,7 +110,42 @@ equi_loss_grad_kernel(int M, const float* __restrict__ pos, const int32_t* __res
     }
 }
 
+// E_norm (Eq. 12): w sum over valid pixels (Nbar != 0) of 1 - N . Nbar; gN = -w Nbar there, 0 elsewhere.
+__global__ void __launch_bounds__(256)
+normal_loss_grad_kernel(size_t n, const float* __restrict__ N, const float* __restrict__ Nb, float w, float* __restrict__ gN,
+                        float* __restrict__ loss) {
+    float acc = 0.f;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float b0 = Nb[i], b1 = Nb[n + i], b2 = Nb[2 * n + i];
+        const bool valid = b0 != 0.f || b1 != 0.f || b2 != 0.f;
+        if (valid) acc += w * (1.0f - (N[i] * b0 + N[n + i] * b1 + N[2 * n + i] * b2));
+        gN[i] = valid ? -w * b0 : 0.f, gN[n + i] = valid ? -w * b1 : 0.f, gN[2 * n + i] = valid ? -w * b2 : 0.f;
+    }
+    if (loss) {
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
+        __shared__ float s[8];
+        if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = acc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            float t = 0.f;
+            for (int k = 0; k < 8; ++k) t += s[k];
+            atomicAdd(loss, t);
+        }
+    }
+}
+
 }  // namespace
+
+extern "C" int32_t ts_normal_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* N, const float* Nbar, float weight,
+                                       float* gN, float* loss_dev, void* stream) {
+    if (!ctx || W <= 0 || H <= 0 || !N || !Nbar || !gN) return TS_ERR_INVALID_ARG;
+    const size_t n = (size_t)W * H;
+    const int grid = (int)((n + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n + 255) / 256 : (size_t)ctx->num_sms * 8);
+    normal_loss_grad_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(n, N, Nbar, (float)((double)weight / (double)n), gN, loss_dev);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
 
 extern "C" int32_t ts_equi_loss_grad(ts_ctx* ctx, const ts_scene* sc, float weight, float* grad_pos, float* loss_dev,
                                      void* stream) {

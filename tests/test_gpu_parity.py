@@ -552,3 +552,63 @@ def test_normal_calls_need_their_forward(ctx, oracle_mod):
     with pytest.raises(ts.TsError):
         ts.ts_render_fwd_normal(ctx, g.scene, g.frame, None, None, None, None)
     g.close()
+
+
+def test_mapping_objective_gradient(ctx, oracle_mod):
+    """One view of E_map = E_pho + lambda_dep E_dep + lambda_norm E_norm + lambda_equi E_equi (Eq. 15, PAPER.md:165-167;
+    weights of Table S4) at the config-3 recipe: ts_render_fwd_normal -> ts_l1_loss_grad ->
+    ts_dssim_loss_grad -> ts_normal_loss_grad -> ts_render_bwd_normal -> ts_equi_loss_grad, against the same chain
+    through the oracle.  The target colour / depth / sensor normals are rendered from the unperturbed scene."""
+    from gpu_util import assert_grad_close, dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(3)
+    lam, lam_dep, lam_norm, lam_equi = 0.2, 0.05, 0.05, 1.2
+    T = sc.T_start[0]
+    gt = oracle_mod.Oracle(sc.pos_target, sc.color_target, sc.opacity, None, T, sc.cam, sc.params, "f32")
+    tgt, Ngt = gt.forward("tiled"), gt.normal_forward("tiled")
+    seen = tgt.alpha > 0.2                                  # (150 k faces cover the small case only sparsely)
+    Nbar = np.where(seen[None], Ngt / np.maximum(np.linalg.norm(Ngt, axis=0), 1e-12)[None], 0.0).astype(np.float32)
+    assert seen.mean() > 0.15 and (~seen).sum() > 0         # there are pixels without a sensor normal as well
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    H, W, V = g.H, g.W, sc.pos.shape[0]
+    # oracle chain, on the oracle's own images
+    No = o.normal_forward("tiled")
+    L1, gC, gD = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, lam_dep)
+    Ls, gS = oracle_mod.dssim(f.color, tgt.color, "f32")
+    Ln, gN = oracle_mod.normal_loss(No, Nbar, lam_norm, "f32")
+    Le, gE = oracle_mod.equi(sc.pos, None, lam_equi, "f32")
+    gC_o = (((1 - lam) * gC + lam * gS) * ok[None]).astype(np.float32)
+    r1 = o.backward(gC_o, (gD * ok).astype(np.float32), None)
+    r2 = o.normal_backward((gN * ok[None]).astype(np.float32))
+    ref_pos = r1.grad_pos + r2.grad_pos + gE
+    ref_opa = r1.grad_opacity + r2.grad_opacity
+    # CUDA chain
+    C, D, A = torch.empty(3, H, W, device="cuda"), torch.empty(H, W, device="cuda"), torch.empty(H, W, device="cuda")
+    N = torch.empty(3, H, W, device="cuda")
+    gCd, gDd, gNd = torch.empty_like(C), torch.empty_like(D), torch.empty_like(N)
+    loss = torch.zeros(1, device="cuda")
+    gp, gc, go = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+    ts.ts_render_fwd_normal(ctx, g.scene, g.frame, C, D, A, N)
+    ts.ts_l1_loss_grad(ctx, W, H, C, D, dev(tgt.color), dev(tgt.depth), lam_dep, gCd, gDd, None)
+    ts.ts_dssim_loss_grad(ctx, W, H, C, dev(tgt.color), lam, gCd, None)
+    ts.ts_normal_loss_grad(ctx, W, H, N, dev(Nbar), lam_norm, gNd, loss)
+    okd = dev(ok.astype(np.float32))
+    gCd *= okd[None]
+    gDd *= okd
+    gNd *= okd[None]
+    ts.ts_render_bwd_normal(ctx, g.scene, g.frame, gCd, gDd, None, gNd, gp, gc, go, ts.GRAD_POS | ts.GRAD_COLOR | ts.GRAD_OPACITY)
+    ts.ts_equi_loss_grad(ctx, g.scene, lam_equi, gp, None)
+    torch.cuda.synchronize()
+    assert abs(float(loss.item()) - Ln) <= 1e-4 * abs(Ln) + 1e-7
+    # (the L1 sign image can flip where |C - Chat| is within float rounding between the two forwards: looser bound)
+    assert_grad_close("grad_pos", gp.cpu().numpy(), ref_pos, tol=5e-3)
+    assert_grad_close("grad_color", gc.cpu().numpy(), r1.grad_color, tol=5e-3)
+    assert_grad_close("grad_opacity", go.cpu().numpy(), ref_opa, tol=5e-3)
+    # and the normal term alone, whose cotangent does not depend on a sign image, to the gradient tolerance
+    gp2, go2 = torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+    ts.ts_render_bwd_normal(ctx, g.scene, g.frame, None, None, None, gNd, gp2, None, go2, ts.GRAD_POS | ts.GRAD_OPACITY)
+    torch.cuda.synchronize()
+    assert_grad_close("grad_pos (E_norm)", gp2.cpu().numpy(), r2.grad_pos)
+    assert_grad_close("grad_opacity (E_norm)", go2.cpu().numpy(), r2.grad_opacity)
+    g.close()

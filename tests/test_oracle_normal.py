@@ -174,3 +174,30 @@ def test_p21_finite_differences(oracle_mod, sigma):
         oracle_mod._p(o.pos), None, o.M, oracle_mod._p(o.T_cw), oracle_mod._p(pr.visible), oracle_mod._p(pr.Q),
         oracle_mod._p(g.g_nrm), None, oracle_mod._p(only_n))
     assert np.all(only_n[:3] == 0) and np.abs(only_n[3:]).max() > 0
+
+
+def test_p22_normal_loss_closed_forms(oracle_mod):
+    """E_norm (Eq. 12): 0 when the maps agree on unit normals, 2 when they are opposite, 1 when orthogonal or when
+    nothing was rendered; pixels without a sensor normal do not count; the gradient is -w Nbar / (H W) on valid pixels
+    (the loss is linear in N, so a finite difference is exact)."""
+    rng = np.random.default_rng(3)
+    H, W = 7, 9
+    nb = rng.normal(size=(3, H, W))
+    nb /= np.linalg.norm(nb, axis=0)
+    for prec in ("f64", "f32"):
+        tol = 1e-12 if prec == "f64" else 1e-6
+        assert abs(oracle_mod.normal_loss(nb, nb, 1.0, prec)[0]) < tol
+        assert abs(oracle_mod.normal_loss(-nb, nb, 1.0, prec)[0] - 2.0) < tol
+        assert abs(oracle_mod.normal_loss(np.zeros_like(nb), nb, 0.05, prec)[0] - 0.05) < tol
+        t = np.cross(nb, np.array([0.3, -0.5, 0.8])[:, None, None], axis=0)
+        assert abs(oracle_mod.normal_loss(t, nb, 1.0, prec)[0] - 1.0) < tol
+    holes = nb.copy()
+    holes[:, 2:4, 3:6] = 0.0                      # 6 pixels without a sensor normal
+    L, g = oracle_mod.normal_loss(-nb, holes, 3.0)
+    assert abs(L - 3.0 * 2.0 * (H * W - 6) / (H * W)) < 1e-12
+    assert np.all(g[:, 2:4, 3:6] == 0) and np.allclose(g, -3.0 * holes / (H * W), atol=1e-15)
+    N = rng.normal(size=(3, H, W))
+    dN = rng.normal(size=(3, H, W))
+    L0, g0 = oracle_mod.normal_loss(N, holes, 0.7)
+    L1, _ = oracle_mod.normal_loss(N + dN, holes, 0.7)
+    assert abs((L1 - L0) - (g0 * dN).sum()) < 1e-12
