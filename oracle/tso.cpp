@@ -114,14 +114,15 @@ struct Face {
     T nx[3], ny[3];         // outward unit normal of edge k (opposite vertex k)
     T ell[3], h[3];         // edge length, altitude of vertex k
     T r, absS, sumell, s;   // inradius = -phi(s), |S|, perimeter, sign of S
-    T obar;                 // face opacity = mean of vertex opacities (:82)
+    T obar;                 // face opacity = mean of vertex opacities (:82), or their minimum (ablation, :433)
+    int kmin;               // min mode: the vertex the opacity gradient goes to (lowest index among equal minima)
     T col[3][3];            // vertex colours
     int x0, y0, x1, y1;
 };
 
 template <class T>
 void face_setup(Face<T>& f, const T* scr9, const int16_t* rc, const T* color, const T* opacity, const int32_t* faces,
-                int m) {
+                int m, bool min_op) {
     for (int k = 0; k < 3; ++k) f.qx[k] = scr9[3 * k], f.qy[k] = scr9[3 * k + 1], f.w[k] = scr9[3 * k + 2];
     T S = signed_area(f.qx, f.qy);
     T s = S > 0 ? (T)1 : (T)-1;
@@ -145,6 +146,14 @@ void face_setup(Face<T>& f, const T* scr9, const int16_t* rc, const T* color, co
         for (int c = 0; c < 3; ++c) f.col[k][c] = color[3 * (int64_t)v + c];
     }
     f.obar = osum / (T)3;
+    f.kmin = -1;
+    if (min_op) {
+        // "the minimum operator ... routes gradients solely to the vertex with the lowest opacity"
+        f.kmin = 0;
+        for (int k = 1; k < 3; ++k)
+            if (opacity[vid(faces, m, k)] < opacity[vid(faces, m, f.kmin)]) f.kmin = k;
+        f.obar = opacity[vid(faces, m, f.kmin)];
+    }
     f.x0 = rc[0], f.y0 = rc[1], f.x1 = rc[2], f.y1 = rc[3];
 }
 
@@ -205,10 +214,10 @@ struct Lists {
 // set-up every visible face once (the per-face constants do not depend on the pixel)
 template <class T>
 std::vector<Face<T>> setup_all(const T* color, const T* opacity, const int32_t* faces, int32_t M,
-                               const uint8_t* visible, const int16_t* rect, const T* scr) {
+                               const uint8_t* visible, const int16_t* rect, const T* scr, bool min_op) {
     std::vector<Face<T>> F((size_t)M);
     for (int m = 0; m < M; ++m)
-        if (visible[m]) face_setup(F[m], scr + 9 * (int64_t)m, rect + 4 * (int64_t)m, color, opacity, faces, m);
+        if (visible[m]) face_setup(F[m], scr + 9 * (int64_t)m, rect + 4 * (int64_t)m, color, opacity, faces, m, min_op);
     return F;
 }
 
@@ -222,7 +231,7 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
     const Cam<T> cam(cam_);
     const int W = cam.W, H = cam.H;
     const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min, atol = (T)prm->amb_tol;
-    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr);
+    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr, prm->min_opacity != 0);
     Lists<T> LS{list, n_list, tile_ranges, (W + 15) / 16};
     uint64_t n_visit = 0, n_rect = 0, n_hit = 0;
     for (int y = 0; y < H; ++y)
@@ -374,7 +383,7 @@ void face_stats(const T* color, const T* opacity, const int32_t* faces, int32_t 
     const Cam<T> cam(cam_);
     const int W = cam.W, H = cam.H;
     const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min;
-    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr);
+    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr, prm->min_opacity != 0);
     Lists<T> LS{list, n_list, tile_ranges, (W + 15) / 16};
     for (int m = 0; m < M; ++m) {
         if (face_pixels) face_pixels[m] = 0;
@@ -416,7 +425,7 @@ void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
     const Cam<T> cam(cam_);
     const int W = cam.W, H = cam.H;
     const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min;
-    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr);
+    std::vector<Face<T>> F = setup_all(color, opacity, faces, M, visible, rect, scr, prm->min_opacity != 0);
     Lists<T> LS{list, n_list, tile_ranges, (W + 15) / 16};
     struct Rec { uint32_t m; T Tn; };
     std::vector<Rec> hits;
@@ -472,8 +481,11 @@ void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 Rd = h.alpha * h.z + ((T)1 - h.alpha) * Rd;
                 Ra = h.alpha + ((T)1 - h.alpha) * Ra;
                 // B4: opacity (mean -> 1/3 each, :82) and window
-                if (grad_opacity)
-                    for (int k = 0; k < 3; ++k) grad_opacity[vid(faces, m, k)] += (h.I / (T)3) * ga;
+                if (grad_opacity) {
+                    if (f.kmin >= 0) grad_opacity[vid(faces, m, f.kmin)] += h.I * ga;
+                    else
+                        for (int k = 0; k < 3; ++k) grad_opacity[vid(faces, m, k)] += (h.I / (T)3) * ga;
+                }
                 const T gI = f.obar * ga;
                 const T gx = gI * sigma * h.I / h.x;
                 // B5: interpolation

@@ -37,6 +37,8 @@ typedef struct {
 typedef struct {
     double sigma, alpha_min, t_min, eps_area;
     double amb_tol;                    /* relative margin for the "ambiguous decision" flag (0 = off) */
+    int32_t min_opacity;               /* 0: face opacity = mean of the vertex opacities (the paper's choice);
+                                          1: minimum ("+ min opacity" ablation, Table S3; Mesh Splatting) */
 } tso_params;
 
 /* F1-F6: project, cull, bounds, depth key.  faces may be NULL (soup: face m = (3m,3m+1,3m+2)).

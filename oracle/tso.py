@@ -35,7 +35,7 @@ class _Cam(C.Structure):
 
 class _Prm(C.Structure):
     _fields_ = [("sigma", C.c_double), ("alpha_min", C.c_double), ("t_min", C.c_double),
-                ("eps_area", C.c_double), ("amb_tol", C.c_double)]
+                ("eps_area", C.c_double), ("amb_tol", C.c_double), ("min_opacity", C.c_int32)]
 
 
 _lib = None
@@ -86,7 +86,7 @@ class Oracle:
         self.cam = _Cam(self.W, self.H, _q(prec, cam.fx), _q(prec, cam.fy), _q(prec, cam.cx), _q(prec, cam.cy),
                         _q(prec, cam.znear))
         self.prm = _Prm(_q(prec, params.sigma), _q(prec, params.alpha_min), _q(prec, params.t_min),
-                        _q(prec, params.eps_area), float(amb_tol))
+                        _q(prec, params.eps_area), float(amb_tol), int(bool(getattr(params, "min_opacity", False))))
         self.tiles_x, self.tiles_y = (self.W + 15) // 16, (self.H + 15) // 16
         self.NT = self.tiles_x * self.tiles_y
         self._proj = None

@@ -41,6 +41,7 @@ class Params:
     t_min: float = 1e-4
     eps_area: float = 1e-6
     lambda_dep: float = 0.05
+    min_opacity: bool = False   # face opacity = min instead of mean of the vertex opacities (ablation)
 
 
 @dataclass

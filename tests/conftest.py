@@ -26,8 +26,9 @@ class SimpleCam:
 
 
 class SimpleParams:
-    def __init__(self, sigma=1.0, alpha_min=0.0, t_min=0.0, eps_area=1e-6, lambda_dep=0.05):
+    def __init__(self, sigma=1.0, alpha_min=0.0, t_min=0.0, eps_area=1e-6, lambda_dep=0.05, min_opacity=False):
         self.sigma, self.alpha_min, self.t_min, self.eps_area, self.lambda_dep = sigma, alpha_min, t_min, eps_area, lambda_dep
+        self.min_opacity = min_opacity
 
 
 IDENT = np.concatenate([np.eye(3), np.zeros((3, 1))], axis=1)
