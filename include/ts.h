@@ -47,7 +47,10 @@ enum { TS_OK = 0, TS_ERR_INVALID_ARG = -1, TS_ERR_WORKSPACE = -2, TS_ERR_CAPACIT
 enum { TS_GRAD_POS = 1, TS_GRAD_COLOR = 2, TS_GRAD_OPACITY = 4, TS_GRAD_POSE = 8 };
 enum { TS_FLAG_OVERFLOW_PAIRS = 1, TS_FLAG_OVERFLOW_VISIBLE = 2 };
 /* ts_params.flags */
-enum { TS_PARAM_COUNTERS = 0x100 };   /* count visits / rect tests / hits into the frame's debug counters */
+enum { TS_PARAM_COUNTERS = 0x100,     /* count visits / rect tests / hits into the frame's debug counters */
+       TS_PARAM_MIN_OPACITY = 0x200 }; /* face opacity = MIN of its vertex opacities instead of their mean (
+                                          "+ min opacity" ablation, Table S3); its gradient goes to that
+                                          vertex alone (lowest index among equal minima) */
 
 const char* ts_strerror(int32_t status);
 

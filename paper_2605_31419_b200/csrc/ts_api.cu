@@ -166,6 +166,7 @@ int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const 
         return TS_ERR_INVALID_ARG;
     fr->cam = TsCamDev{cam->width, cam->height, cam->fx, cam->fy, cam->cx, cam->cy, cam->znear};
     fr->prm = TsPrmDev{prm->sigma, prm->alpha_min, prm->t_min, prm->eps_area, prm->flags};
+    fr->d.prm_flags = prm->flags;
     fr->T_cw = T_cw_dev;
     fr->have_sort = fr->have_fwd = fr->have_normals = 0;
     fr->pose_src = 0;

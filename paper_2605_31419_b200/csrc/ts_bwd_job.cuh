@@ -196,9 +196,19 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
                     for (int ch = 0; ch < 3; ++ch) atomicAdd(grad_color + 3 * (size_t)v[k] + ch, acc[9 + 3 * k + ch]);
             }
             if (grad_opacity) {
-                const float go = acc[18] * (1.0f / 3.0f);
+                if (f.prm_flags & TS_PARAM_MIN_OPACITY) {
+                    // min mode: the gradient goes to the vertex with the lowest opacity (lowest index among equals)
+                    const float p0 = __ldg(sc.opacity + v[0]), p1 = __ldg(sc.opacity + v[1]), p2 = __ldg(sc.opacity + v[2]);
+                    int km = 0;
+                    float pm = p0;
+                    if (p1 < pm) km = 1, pm = p1;
+                    if (p2 < pm) km = 2;
+                    atomicAdd(grad_opacity + (km == 0 ? v[0] : (km == 1 ? v[1] : v[2])), acc[18]);
+                } else {
+                    const float go = acc[18] * (1.0f / 3.0f);
 #pragma unroll
-                for (int k = 0; k < 3; ++k) atomicAdd(grad_opacity + v[k], go);
+                    for (int k = 0; k < 3; ++k) atomicAdd(grad_opacity + v[k], go);
+                }
             }
         }
     }

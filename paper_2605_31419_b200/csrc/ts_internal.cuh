@@ -37,6 +37,7 @@ struct TsCtrl {
 struct TsFrameDev {
     int32_t M, W, H, tiles_x, tiles_y, NT;
     uint32_t pair_cap, vis_cap;
+    uint32_t prm_flags;               // ts_params.flags of the last ts_project (host-side copy, travels with the launches)
     TsCtrl* ctrl;
     uint32_t* tile_count;             // [NT] pairs per tile, counted by the project kernel (zeroed by the sort kernel)
     uint32_t* tile_cursor;            // [NT] write cursor of the binning pass, relative to the tile's begin (zero at rest)

@@ -120,12 +120,14 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
     float ob = 0.0f;
     if (o.vis) {
         const int64_t m = face0 + tid;
+        float o0, o1, o2;
         if (SOUP) {
-            ob = (__ldg(opacity + 3 * m) + __ldg(opacity + 3 * m + 1) + __ldg(opacity + 3 * m + 2)) * (1.0f / 3.0f);
+            o0 = __ldg(opacity + 3 * m), o1 = __ldg(opacity + 3 * m + 1), o2 = __ldg(opacity + 3 * m + 2);
         } else {
-            ob = (__ldg(opacity + __ldg(faces + 3 * m)) + __ldg(opacity + __ldg(faces + 3 * m + 1)) +
-                  __ldg(opacity + __ldg(faces + 3 * m + 2))) * (1.0f / 3.0f);
+            o0 = __ldg(opacity + __ldg(faces + 3 * m)), o1 = __ldg(opacity + __ldg(faces + 3 * m + 1)),
+            o2 = __ldg(opacity + __ldg(faces + 3 * m + 2));
         }
+        ob = (f.prm_flags & TS_PARAM_MIN_OPACITY) ? fminf(o0, fminf(o1, o2)) : (o0 + o1 + o2) * (1.0f / 3.0f);
     }
 
     // slot allocation: warp ballot -> CTA total -> one global atomic per CTA

@@ -19,6 +19,7 @@ GRAD_POS, GRAD_COLOR, GRAD_OPACITY, GRAD_POSE = 1, 2, 4, 8
 GRAD_ALL = 15
 FLAG_OVERFLOW_PAIRS, FLAG_OVERFLOW_VISIBLE = 1, 2
 PARAM_COUNTERS = 0x100   # ts_params.flags: count visits / rect tests / hits (debug instantiation)
+PARAM_MIN_OPACITY = 0x200   # ts_params.flags: face opacity = min instead of mean of the vertex opacities (ablation)
 VIEW_VIS, VIEW_KEYS, VIEW_VALS, VIEW_TILE_RANGES, VIEW_N_CONTRIB, VIEW_COUNTERS = range(6)
 _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.int32,
                 VIEW_TILE_RANGES: torch.int32, VIEW_N_CONTRIB: torch.int32, VIEW_COUNTERS: torch.int64}
@@ -169,6 +170,8 @@ def make_camera(cam):
 
 
 def make_params(p, flags=0):
+    if getattr(p, "min_opacity", False):
+        flags |= PARAM_MIN_OPACITY
     return ts_params(p.sigma, p.alpha_min, p.t_min, p.eps_area, flags)
 
 

@@ -612,3 +612,29 @@ def test_mapping_objective_gradient(ctx, oracle_mod):
     assert_grad_close("grad_pos (E_norm)", gp2.cpu().numpy(), r2.grad_pos)
     assert_grad_close("grad_opacity (E_norm)", go2.cpu().numpy(), r2.grad_opacity)
     g.close()
+
+
+@pytest.mark.parametrize("indexed", [False, True])
+def test_min_opacity_variant(ctx, oracle_mod, indexed):
+    """TS_PARAM_MIN_OPACITY ("+ min opacity" ablation, PAPER.md:82 and Table S3): images and all gradients against the
+    oracle in the same mode; the opacity gradient lands on one vertex per face; and the mode does change the image."""
+    from gpu_util import GpuView
+    from paper_2605_31419_b200 import ts
+    if indexed:
+        sc, pos, col, opa, faces = grid_mesh(n=30, seed=4)
+    else:
+        sc = small_cfg(2)
+        pos, col, opa, faces = sc.pos, sc.color, sc.opacity, None
+    prm = scenes.Params(sigma=sc.params.sigma, alpha_min=sc.params.alpha_min, t_min=sc.params.t_min, min_opacity=True)
+    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, prm, "f32", amb_tol=5e-3)
+    g = GpuView(ctx, pos, col, opa, faces, sc.T_start[0], sc.cam, prm)
+    f, ok = check_forward(o, g)
+    ref = check_backward(o, g, ok, 91, [ts.GRAD_ALL, ts.GRAD_POSE])
+    if not indexed:
+        tri = opa.reshape(-1, 3)
+        not_min = (tri != tri.min(axis=1, keepdims=True)).reshape(-1)
+        assert np.all(ref.grad_opacity[not_min] == 0)
+    g2 = GpuView(ctx, pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params)
+    A_mean = g2.forward()[2]
+    assert np.abs(A_mean - g.A.cpu().numpy()).max() > 0.05
+    g.close(), g2.close()
