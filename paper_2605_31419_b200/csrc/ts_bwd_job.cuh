@@ -224,7 +224,8 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
                                             BwdWarpSmem& sm, float sigma, float alpha_min, float fx, float fy,
                                             uint32_t ncon, float Tcur, float gC0, float gC1, float gC2, float gD,
                                             float gA, float* __restrict__ grad_color, float* __restrict__ grad_opacity,
-                                            float tau[6], float gN0 = 0.f, float gN1 = 0.f, float gN2 = 0.f) {
+                                            float tau[6], float gN0 = 0.f, float gN1 = 0.f, float gN2 = 0.f,
+                                            uint32_t prestaged_lo = 0xffffffffu) {
     static_assert(!(NRM && POSE), "the normal-map backward runs in full-gradient mode");
     const float fpx = (float)job.px, fpy = (float)job.py;
     const uint32_t lt = (1u << lane) - 1u;
@@ -236,15 +237,22 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
     uint32_t qn = 0;                   // queued hits (warp-uniform); the queue always starts at index 0
 
     for (uint32_t hi = n_walk; hi > 0;) {
-        const uint32_t lo = hi > 32u ? hi - 32u : 0u;
+        const uint32_t lo = (hi - 1u) & ~31u;           // chunks are aligned like the forward walk's
         const uint32_t n = hi - lo;
         uint4 cur = make_uint4(0u, 0u, 0u, 0u);
-        if ((uint32_t)lane < n) cur = f.sorted[job.range.x + lo + lane];
-        uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
+        uint32_t lmask;
+        const bool prestaged = POSE && lo == prestaged_lo;
+        if (prestaged) {
+            // the forward walk of this job left exactly this chunk staged, rows 0-11, masks after the block cull
+            lmask = (uint32_t)lane < n ? sm.lm[lane] : 0u;
+        } else {
+            if ((uint32_t)lane < n) cur = f.sorted[job.range.x + lo + lane];
+            lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
+        }
         hi = lo;
         if (!__any_sync(0xffffffffu, lmask != 0u)) continue;
         __syncwarp();
-        if (lmask) {
+        if (lmask && !prestaged) {
             // staged at the lane's own index (no compaction); the walk follows the set bits of `ov` backwards
             const float4* rp = f.rec + TS_REC_F4 * (size_t)cur.x;
             float4 r[TS_REC_F4];

@@ -19,12 +19,17 @@ struct FwdPix {                       // what the walk leaves for this lane's pi
 // `ent` = the lane's entry of the first 32-entry chunk of the tile list (already requested by the caller, so that
 // its round trip overlaps the caller's ticket atomic).  NRM: also composite the flat per-face normal f.nrm[slot]
 // (Eq. 12, reading S26), staged in the warp's `nsm[32]`.
-template <int SM, bool COUNT, bool STATS = false, bool NRM = false>
+// FULLREC (fused tracking job): SMEM is the backward's BwdWarpSmem (rows 0-5 mean the same in both layouts); for the
+// LAST chunk of the tile list the lanes also stage record rows R4-R9 into rows 6-11 and every lane publishes its lane
+// mask, so that the pose-only backward walk of the same job -- which begins in that chunk unless every pixel
+// terminated earlier -- can start without loading anything again (ts_bwd_walk, `prestaged_lo`; *staged_lo = list
+// position of that chunk relative to the tile's begin, 0xffffffff if it was not staged).
+template <int SM, bool COUNT, bool STATS = false, bool NRM = false, bool FULLREC = false, class SMEM = FwdWarpSmem>
 __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene& sc, const TsJob& job, int lane,
-                                            FwdWarpSmem& sm, float sigma, float alpha_min, float t_min, uint4 ent,
+                                            SMEM& sm, float sigma, float alpha_min, float t_min, uint4 ent,
                                             FwdPix& o, unsigned long long& n_visit, unsigned long long& n_rect,
                                             unsigned long long& n_hit, uint32_t* __restrict__ face_pixels = nullptr,
-                                            float4* nsm = nullptr) {
+                                            float4* nsm = nullptr, uint32_t* staged_lo = nullptr) {
     const float fpx = (float)job.px, fpy = (float)job.py;
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, D = 0.0f, Tlast = 1.0f;
     float N0 = 0.0f, N1 = 0.0f, N2 = 0.0f;
@@ -55,6 +60,17 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             sm.lm[lane] = lmask, sm.slot[lane] = cur.x;
             if (STATS) sm.face[lane] = cur.y;
             if (NRM) nsm[lane] = f.nrm[cur.x];
+            if (FULLREC && lmask && c0 + 32u >= job.range.y) {   // (only the list's last chunk: that is where the backward begins)
+                // the rest of the record, in two batches to keep the live range short
+                const float4 a0 = __ldg(rp + 4), a1 = __ldg(rp + 5), a2 = __ldg(rp + 6);
+                sm.r[lane][6] = a0, sm.r[lane][7] = a1, sm.r[lane][8] = a2;
+                const float4 b0 = __ldg(rp + 7), b1 = __ldg(rp + 8), b2 = __ldg(rp + 9);
+                sm.r[lane][9] = b0, sm.r[lane][10] = b1, sm.r[lane][11] = b2;
+            }
+        }
+        if (FULLREC && c0 + 32u >= job.range.y) {
+            if (!lmask) sm.lm[lane] = 0u;               // lanes without an entry for this block
+            *staged_lo = c0 - job.range.x;
         }
         __syncwarp();
         uint32_t ov = __ballot_sync(0xffffffffu, lmask != 0u);

@@ -105,7 +105,11 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
         if (job.range.x + lane < job.range.y) ent = f.sorted[job.range.x + lane];
         j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
         FwdPix o;
-        ts_fwd_walk<SM, false>(f, sc, job, lane, sm.fwd, sigma, alpha_min, t_min, ent, o, dummy0, dummy1, dummy2);
+        // the chunk the forward walk staged last (with the whole record) is where the backward walk begins
+        uint32_t staged_lo = 0xffffffffu;
+        ts_fwd_walk<SM, false, false, false, true, BwdWarpSmem>(f, sc, job, lane, sm.bwd, sigma, alpha_min, t_min, ent, o, dummy0,
+                                                                dummy1, dummy2, nullptr, nullptr, &staged_lo);
+        if (f.prm_flags & 0x8000u) staged_lo = 0xffffffffu;   // TEMP A/B switch
         float gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f;
         if (job.inside) {
             const size_t p = (size_t)job.py * f.W + job.px;
@@ -130,7 +134,7 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
         __syncwarp();                                      // the forward walk's shared-memory slice is re-used
         float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         ts_bwd_walk<SM, false, false, true>(f, sc, job, lane, sm.bwd, sigma, alpha_min, fx, fy, o.last, o.Tlast, gC0, gC1,
-                                            gC2, gD, 0.0f, nullptr, nullptr, tau);
+                                            gC2, gD, 0.0f, nullptr, nullptr, tau, 0.f, 0.f, 0.f, staged_lo);
 #pragma unroll
         for (int jj = 0; jj < 6; ++jj) tau[jj] = warp_sum(tau[jj]);
         if (lane < 6) {
