@@ -80,14 +80,19 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             ov &= ov - 1;
             const bool in_rect = !done && ((sm.lm[e] >> lane) & 1u);
             if (COUNT) n_visit += 1, n_rect += in_rect ? 1 : 0;
-            if (!__any_sync(0xffffffffu, in_rect)) continue;
-            const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
+            // (no warp votes here: after the exact block cull nearly every visit has a lane inside the rect and a
+            // hit, so "skip if nobody ..." tests cost more than they save)
             float l[3], x, I, alpha;
-            const bool hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
-            const uint32_t hm = __ballot_sync(0xffffffffu, hit);
-            if (!hm) continue;
-            // statistics: the face contributed to popc(hm) pixels of this block (one RED per visit)
-            if (STATS && lane == __ffs(hm) - 1) atomicAdd(face_pixels + sm.face[e], (uint32_t)__popc(hm));
+            bool hit = false;
+            if (in_rect) {
+                const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
+                hit = ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
+            }
+            if (STATS) {
+                // statistics: the face contributed to popc(hm) pixels of this block (one RED per visit)
+                const uint32_t hm = __ballot_sync(0xffffffffu, hit);
+                if (hm && lane == __ffs(hm) - 1) atomicAdd(face_pixels + sm.face[e], (uint32_t)__popc(hm));
+            }
             if (hit) {
                 const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
                 if (COUNT) n_hit += 1;
@@ -108,8 +113,8 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
                 last = pos0 + (uint32_t)e;
                 if (T <= t_min) done = true;
             }
-            if (__all_sync(0xffffffffu, done)) { warp_done = true; break; }
         }
+        warp_done = __all_sync(0xffffffffu, done);      // once per chunk: pixels rarely all terminate inside one
     }
     o.T = T, o.C0 = C0, o.C1 = C1, o.C2 = C2, o.D = D, o.Tlast = Tlast, o.last = last;
     if (NRM) o.N0 = N0, o.N1 = N1, o.N2 = N2;
