@@ -8,9 +8,9 @@ struct BwdWarpSmem {
     uint32_t lm[32];
     uint32_t slot[32];
     uint32_t face[32];
-    // pose-only mode: queue of hits waiting for the packed second phase, and the block's cotangents
-    uint32_t q_code[64];              // entry index | pixel lane << 8
-    float q_ga[64], q_wgt[64], q_l0[64], q_l1[64], q_l2[64];
+    // ring of hits waiting for the packed second phase, and the block's cotangents
+    float4 q_a[64];                   // (dL/dalpha, T alpha, lhat_0, lhat_1)
+    float2 q_b[64];                   // (lhat_2, bits of: entry index | pixel lane << 8)
     float4 pix[32];                   // (gC0, gC1, gC2, gD) of the lane's pixel
 };
 
@@ -234,7 +234,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
     if (NRM) sm.r[lane][11] = make_float4(gN0, gN1, gN2, 0.f);       // row 11 is free outside pose-only mode
     float Rs = 0.f;                    // R^c.gC + R^d gD + R^a gA behind the current face
     bool first = true;
-    uint32_t qn = 0;                   // queued hits (warp-uniform); the queue always starts at index 0
+    uint32_t qn = 0, qh = 0;           // queued hits and the ring's head (warp-uniform)
 
     for (uint32_t hi = n_walk; hi > 0;) {
         const uint32_t lo = (hi - 1u) & ~31u;           // chunks are aligned like the forward walk's
@@ -310,9 +310,9 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
                 Rs = alpha * S + one_m * Rs;                              // B3
                 {
                     // the sequential part of this hit is done; the rest (B4-B9) waits in the queue
-                    const uint32_t qi = qn + (uint32_t)__popc(hm & lt);
-                    sm.q_code[qi] = (uint32_t)e | ((uint32_t)lane << 8);
-                    sm.q_ga[qi] = ga, sm.q_wgt[qi] = wgt, sm.q_l0[qi] = l[0], sm.q_l1[qi] = l[1], sm.q_l2[qi] = l[2];
+                    const uint32_t qi = (qh + qn + (uint32_t)__popc(hm & lt)) & 63u;
+                    sm.q_a[qi] = make_float4(ga, wgt, l[0], l[1]);
+                    sm.q_b[qi] = make_float2(l[2], __uint_as_float((uint32_t)e | ((uint32_t)lane << 8)));
                 }
                 (void)x, (void)I;
             }
@@ -320,22 +320,11 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             if (qn >= 32u) {
                 // a full group: every lane finishes one queued hit
                 __syncwarp();
-                const uint32_t code = sm.q_code[lane];
-                const float qga = sm.q_ga[lane], qw = sm.q_wgt[lane], ql0 = sm.q_l0[lane], ql1 = sm.q_l1[lane], ql2 = sm.q_l2[lane];
-                const uint32_t rest = qn - 32u;
-                // move the remainder (< 32 entries) to the front
-                uint32_t mc = 0;
-                float m0 = 0.f, m1 = 0.f, m2 = 0.f, m3 = 0.f, m4 = 0.f;
-                if ((uint32_t)lane < rest) {
-                    mc = sm.q_code[32 + lane], m0 = sm.q_ga[32 + lane], m1 = sm.q_wgt[32 + lane];
-                    m2 = sm.q_l0[32 + lane], m3 = sm.q_l1[32 + lane], m4 = sm.q_l2[32 + lane];
-                }
-                __syncwarp();
-                if ((uint32_t)lane < rest) {
-                    sm.q_code[lane] = mc, sm.q_ga[lane] = m0, sm.q_wgt[lane] = m1;
-                    sm.q_l0[lane] = m2, sm.q_l1[lane] = m3, sm.q_l2[lane] = m4;
-                }
-                qn = rest;
+                const float4 qa = sm.q_a[(qh + lane) & 63u];
+                const float2 qb = sm.q_b[(qh + lane) & 63u];
+                const uint32_t code = __float_as_uint(qb.y);
+                const float qga = qa.x, qw = qa.y, ql0 = qa.z, ql1 = qa.w, ql2 = qb.x;
+                qh = (qh + 32u) & 63u, qn -= 32u;       // the remainder (< 32 entries) stays where it is
                 if (POSE)
                     ts_bwd_pose_hit<SM>(sm, code & 0xffu, sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
                 else
@@ -347,15 +336,17 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             // the staged records are about to be replaced: finish what is still queued (partial group)
             __syncwarp();
             const bool act = (uint32_t)lane < qn;
-            const uint32_t code = act ? sm.q_code[lane] : 0u;
-            const float qga = act ? sm.q_ga[lane] : 0.f, qw = act ? sm.q_wgt[lane] : 0.f;
-            const float ql0 = act ? sm.q_l0[lane] : 0.f, ql1 = act ? sm.q_l1[lane] : 0.f, ql2 = act ? sm.q_l2[lane] : 0.f;
+            float4 qa = make_float4(0.f, 0.f, 0.f, 0.f);
+            float2 qb = make_float2(0.f, 0.f);
+            if (act) qa = sm.q_a[(qh + lane) & 63u], qb = sm.q_b[(qh + lane) & 63u];
+            const uint32_t code = __float_as_uint(qb.y);
+            const float qga = qa.x, qw = qa.y, ql0 = qa.z, ql1 = qa.w, ql2 = qb.x;
             if (POSE) {
                 if (act) ts_bwd_pose_hit<SM>(sm, code & 0xffu, sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
             } else {
                 ts_bwd_full_group<SM, ATTR, GEOM, NRM>(f, sc, sm, lane, act, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
             }
-            qn = 0;
+            qn = 0, qh = 0;
             __syncwarp();
         }
     }
