@@ -109,7 +109,6 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
         uint32_t staged_lo = 0xffffffffu;
         ts_fwd_walk<SM, false, false, false, true, BwdWarpSmem>(f, sc, job, lane, sm.bwd, sigma, alpha_min, t_min, ent, o, dummy0,
                                                                 dummy1, dummy2, nullptr, nullptr, &staged_lo);
-        if (f.prm_flags & 0x8000u) staged_lo = 0xffffffffu;   // TEMP A/B switch
         float gC0 = 0.f, gC1 = 0.f, gC2 = 0.f, gD = 0.f;
         if (job.inside) {
             const size_t p = (size_t)job.py * f.W + job.px;
