@@ -4,7 +4,8 @@
 #include "ts_jobs.cuh"
 
 struct BwdWarpSmem {
-    float4 r[32][12];                 // R0 R1 R2 | kap,c00 | colours | colours | R4 R5 R6 R7 | R8 R9
+    float4 r[32][13];                 // R0 R1 R2 | kap,c00 | colours | colours | R4 R5 R6 R7 | R8 R9 | pad: a 208 B
+                                      // stride spreads the lanes' rows over all banks (192 B put them on two bank quads)
     uint32_t lm[32];
     uint32_t slot[32];
     uint32_t face[32];

@@ -4,7 +4,7 @@
 #include "ts_jobs.cuh"
 
 struct FwdWarpSmem {
-    float4 r[32][6];                  // R0 R1 R2 | kap0 kap1 kap2 c00 | c01 c02 c10 c11 | c12 c20 c21 c22
+    float4 r[32][7];                  // R0 R1 R2 | kap0 kap1 kap2 c00 | c01 c02 c10 c11 | c12 c20 c21 c22 | pad (bank spread)
     uint32_t lm[32];                  // lane mask of the entry for this block
     uint32_t slot[32];
     uint32_t face[32];                // only written / read by the statistics instantiation
