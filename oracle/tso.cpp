@@ -672,6 +672,25 @@ double normal_loss(int32_t W, int32_t H, const T* N, const T* Nb, double weight,
     return L;
 }
 
+// Screen-space gradient statistic of the densification test (Table S4: "gradient threshold 0.001", "gradient percentile
+// 0.99"; the text does not define it).  Reading S28 of DESIGN.md: per face, the norm of the gradient
+// of L with respect to a rigid translation of the face in the image plane, ||sum_k (dL/du_k, dL/dv_k)||_2 -- the
+// triangle analogue of the view-space point gradient that Gaussian-splatting densification accumulates.
+// g_scr[M][9] as written by render_bwd; face_grad2d[M] += the norm, face_views[M] += 1 where the face has a gradient.
+template <class T>
+void screen_grad_stat(int32_t M, const uint8_t* visible, const T* g_scr, T* face_grad2d, uint32_t* face_views) {
+    for (int m = 0; m < M; ++m) {
+        if (!visible[m]) continue;
+        const T* g = g_scr + 9 * (int64_t)m;
+        bool any = false;
+        for (int j = 0; j < 9; ++j) any = any || g[j] != 0;
+        if (!any) continue;
+        const T sx = (g[0] + g[3]) + g[6], sy = (g[1] + g[4]) + g[7];
+        face_grad2d[m] += std::sqrt(sx * sx + sy * sy);
+        if (face_views) face_views[m] += 1;
+    }
+}
+
 // SE(3) exponential, tau = (rho, theta).  out = Exp(tau) o T.
 template <class T>
 void left_perturb(const T* Tcw, const T* tau, T* out) {
@@ -863,6 +882,13 @@ void tso_face_stats_f64(const double* color, const double* opacity, const int32_
     }
 TSO_NRM_FWD(float, f32)
 TSO_NRM_FWD(double, f64)
+
+void tso_screen_grad_stat_f32(int32_t M, const uint8_t* visible, const float* g_scr, float* face_grad2d, uint32_t* face_views) {
+    screen_grad_stat<float>(M, visible, g_scr, face_grad2d, face_views);
+}
+void tso_screen_grad_stat_f64(int32_t M, const uint8_t* visible, const double* g_scr, double* face_grad2d, uint32_t* face_views) {
+    screen_grad_stat<double>(M, visible, g_scr, face_grad2d, face_views);
+}
 
 double tso_normal_loss_f32(int32_t W, int32_t H, const float* N, const float* Nbar, double weight, float* gN) {
     return normal_loss<float>(W, H, N, Nbar, weight, gN);

@@ -164,6 +164,12 @@ TSO_NRM_DECL(double, f64)
 double tso_normal_loss_f32(int32_t W, int32_t H, const float* N, const float* Nbar, double weight, float* gN);
 double tso_normal_loss_f64(int32_t W, int32_t H, const double* N, const double* Nbar, double weight, double* gN);
 
+/* Screen-space gradient statistic of the densification test (reading S28): per face,
+ * ||sum_k (dL/du_k, dL/dv_k)||_2 from g_scr[M][9] of tso_render_bwd.  face_grad2d[M] += it, face_views[M] += 1 (may be
+ * NULL) for every visible face that received a gradient. */
+void tso_screen_grad_stat_f32(int32_t M, const uint8_t* visible, const float* g_scr, float* face_grad2d, uint32_t* face_views);
+void tso_screen_grad_stat_f64(int32_t M, const uint8_t* visible, const double* g_scr, double* face_grad2d, uint32_t* face_views);
+
 /* SE(3) exponential, tau = (rho, theta): out[12] = Exp(tau) o T (3x4 row-major). */
 void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out);
 

@@ -191,6 +191,10 @@ class Oracle:
         o.dL_dtau = np.zeros(6, self.dt)
         self._fn("tso_project_bwd")(_p(self.faces), C.c_int32(self.M), _p(self.T_cw), C.byref(self.cam),
                                     _p(pr.visible), _p(pr.Q), _p(o.g_scr), _p(o.grad_pos), _p(o.dL_dtau))
+        if "stat" in want:
+            o.face_grad2d, o.face_views = np.zeros(self.M, self.dt), np.zeros(self.M, np.uint32)
+            self._fn("tso_screen_grad_stat")(C.c_int32(self.M), _p(pr.visible), _p(o.g_scr), _p(o.face_grad2d),
+                                             _p(o.face_views))
         return o
 
     # ------------------------------------------------------------------ normal map (Eq. 12, reading S26)
