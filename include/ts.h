@@ -152,6 +152,16 @@ int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, 
 int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
                             float* out_alpha, uint32_t* face_pixels, void* stream);
 int32_t ts_face_area(ts_ctx* ctx, ts_frame* frame, float* proj_area, void* stream);
+/* ts_render_bwd plus the screen-space gradient statistic of the densification test (Table S4 "gradient threshold /
+ * percentile"; reading S28): for every face that received a gradient,
+ * face_grad2d[m] += || sum_k (dL/du_k, dL/dv_k) ||_2 (the gradient of L under a rigid translation of the face in the
+ * image plane, in 1/px) and face_views[m] += 1 (may be NULL); both [M], device, accumulated over calls (caller zeroes).
+ * grad_mask must contain TS_GRAD_POS or TS_GRAD_POSE (the statistic is a by-product of the per-face screen gradients;
+ * with TS_GRAD_POSE alone the full-gradient path runs, not the pose-only one). */
+int32_t ts_render_bwd_stats(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, const float* dL_dcolor,
+                            const float* dL_ddepth, const float* dL_dalpha, float* grad_pos, float* grad_color,
+                            float* grad_opacity, uint32_t grad_mask, float* face_grad2d, uint32_t* face_views,
+                            void* stream);
 
 /* Rendered normal map and its gradient (Eq. 12: the map "returned by the rasteriser" that E_norm
  * compares with the sensor normals; reading S26):

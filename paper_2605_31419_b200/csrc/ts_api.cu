@@ -282,6 +282,21 @@ int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float
                                 grad_mask, (cudaStream_t)stream);
 }
 
+int32_t ts_render_bwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
+                            const float* dL_dalpha, float* grad_pos, float* grad_color, float* grad_opacity,
+                            uint32_t grad_mask, float* face_grad2d, uint32_t* face_views, void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !sc->pos || !face_grad2d) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_POS) && !grad_pos) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_COLOR) && !grad_color) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_OPACITY) && !grad_opacity) return TS_ERR_INVALID_ARG;
+    if (grad_mask & ~(uint32_t)(TS_GRAD_POS | TS_GRAD_COLOR | TS_GRAD_OPACITY | TS_GRAD_POSE)) return TS_ERR_INVALID_ARG;
+    if (!(grad_mask & (TS_GRAD_POS | TS_GRAD_POSE))) return TS_ERR_INVALID_ARG;      // the statistic is a by-product of B5-B6
+    if (!fr->have_fwd) return TS_ERR_STATE;
+    return ts_launch_render_bwd(ctx, fr, sc, dL_dcolor, dL_ddepth, dL_dalpha, grad_pos, grad_color, grad_opacity, grad_mask,
+                                (cudaStream_t)stream, face_grad2d, face_views);
+}
+
 int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, void* stream) {
     if (!ctx || !fr || !dL_dtau_dev) return TS_ERR_INVALID_ARG;
     return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, nullptr, nullptr, nullptr, 0.f, 0.f, 0.f, (cudaStream_t)stream);

@@ -113,7 +113,8 @@ int32_t ts_launch_render_bwd_normal(const ts_ctx*, ts_frame*, const ts_scene*, c
                                     const float* gA, const float* gN, float* grad_pos, float* grad_color,
                                     float* grad_opacity, uint32_t mask, cudaStream_t);
 int32_t ts_launch_render_bwd(const ts_ctx*, ts_frame*, const ts_scene*, const float*, const float*, const float*,
-                             float*, float*, float*, uint32_t, cudaStream_t);
+                             float*, float*, float*, uint32_t, cudaStream_t, float* face_grad2d = nullptr,
+                             uint32_t* face_views = nullptr);
 int32_t ts_launch_render_track(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
                                const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, cudaStream_t);
 int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame*, float* out, float* T_cw, float* state, const float* lr6, float beta1,

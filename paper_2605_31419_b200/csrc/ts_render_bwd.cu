@@ -178,10 +178,13 @@ constexpr int PB_THREADS = 256;
 // NRM: also consumes gnrm (dL/dn per face) and pushes it through n = s (a x b)/|a x b| (ts_normal.cuh) to the vertices
 // (P1 += R^T g_a, P2 += R^T g_b, P0 -= both) and to the rotation part of the pose (a x g_a + b x g_b; a translation of
 // the camera does not turn the normals).
+// face_grad2d / face_views (may be NULL): the screen-space gradient statistic of the densification test (reading S28):
+// ||sum_k (dL/du_k, dL/dv_k)|| added per face, and a count of the views in which the face received a gradient.
 template <bool SOUP, bool NRM = false>
 __global__ void __launch_bounds__(PB_THREADS)
 proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __restrict__ faces,
-                const float* __restrict__ Tcw, TsCamDev cam, float* __restrict__ grad_pos, int want_pose) {
+                const float* __restrict__ Tcw, TsCamDev cam, float* __restrict__ grad_pos, int want_pose,
+                float* __restrict__ face_grad2d = nullptr, uint32_t* __restrict__ face_views = nullptr) {
     __shared__ float sT[12];
     __shared__ float red[PB_THREADS / 32][6];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -212,6 +215,16 @@ proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __re
 #pragma unroll
         for (int j = 0; j < 9; ++j) gs[j] = 0.0f;
         const uint32_t m = __float_as_uint(f.scr[TS_SCR_F4 * (size_t)slot + 3].x);
+        if (face_grad2d) {
+            bool any_scr = false;
+#pragma unroll
+            for (int j = 0; j < 9; ++j) any_scr |= (g9[j] != 0.0f);
+            if (any_scr) {
+                const float sx = (g9[0] + g9[3]) + g9[6], sy = (g9[1] + g9[4]) + g9[7];
+                face_grad2d[m] += sqrtf(sx * sx + sy * sy);          // one slot per face: no other writer
+                if (face_views) face_views[m] += 1u;
+            }
+        }
         size_t vid[3];
         float P[3][3];
 #pragma unroll
@@ -368,10 +381,10 @@ void launch_bwd_sm(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, co
 
 int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, const float* gC, const float* gD,
                              const float* gA, float* grad_pos, float* grad_color, float* grad_opacity, uint32_t mask,
-                             cudaStream_t st) {
+                             cudaStream_t st, float* face_grad2d, uint32_t* face_views) {
     const bool attr = (mask & (TS_GRAD_COLOR | TS_GRAD_OPACITY)) != 0;
     const bool geom = (mask & (TS_GRAD_POS | TS_GRAD_POSE)) != 0;
-    const bool pose_only = (mask == TS_GRAD_POSE);
+    const bool pose_only = (mask == TS_GRAD_POSE) && !face_grad2d;   // the statistic needs the per-face sums
     if (!attr && !geom) return TS_OK;
     float* gcol = (mask & TS_GRAD_COLOR) ? grad_color : nullptr;
     float* gopa = (mask & TS_GRAD_OPACITY) ? grad_opacity : nullptr;
@@ -389,9 +402,11 @@ int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
         const int want_pose = (mask & TS_GRAD_POSE) ? 1 : 0;
         float* gp = (mask & TS_GRAD_POS) ? grad_pos : nullptr;
         if (sc->faces == nullptr)
-            proj_bwd_kernel<true><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, nullptr, fr->T_cw, fr->cam, gp, want_pose);
+            proj_bwd_kernel<true><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, nullptr, fr->T_cw, fr->cam, gp, want_pose,
+                                                               face_grad2d, face_views);
         else
-            proj_bwd_kernel<false><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, sc->faces, fr->T_cw, fr->cam, gp, want_pose);
+            proj_bwd_kernel<false><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, sc->faces, fr->T_cw, fr->cam, gp, want_pose,
+                                                                face_grad2d, face_views);
         if (want_pose) fr->pose_src = 2, fr->n_pose_partials = (uint32_t)grid;
     }
     TS_CUDA_CHECK_LAUNCH();

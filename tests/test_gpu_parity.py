@@ -638,3 +638,40 @@ def test_min_opacity_variant(ctx, oracle_mod, indexed):
     A_mean = g2.forward()[2]
     assert np.abs(A_mean - g.A.cpu().numpy()).max() > 0.05
     g.close(), g2.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_screen_gradient_statistic(ctx, oracle_mod, cfg):
+    """ts_render_bwd_stats (densification statistic, reading S28) against the oracle's; gradients are the
+    same as ts_render_bwd's; accumulation over two calls; the pose still comes out with TS_GRAD_POSE alone."""
+    from gpu_util import assert_grad_close, dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(cfg)
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    rng = np.random.default_rng(55 + cfg)
+    H, W = ok.shape
+    gC = (rng.normal(size=(3, H, W)) * ok[None]).astype(np.float32)
+    gD = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+    ref = o.backward(gC, gD, None, want=("pos", "pose", "stat"))
+    V, M = sc.pos.shape[0], sc.M
+    gp = torch.zeros(V, 3, device="cuda")
+    st, views = torch.zeros(M, device="cuda"), torch.zeros(M, dtype=torch.int32, device="cuda")
+    ts.ts_render_bwd_stats(ctx, g.scene, g.frame, dev(gC), dev(gD), None, gp, None, None, ts.GRAD_POS, st, views)
+    torch.cuda.synchronize()
+    assert_grad_close("grad_pos", gp.cpu().numpy(), ref.grad_pos)
+    assert_grad_close("face_grad2d", st.cpu().numpy(), ref.face_grad2d)
+    # a face "received a gradient" iff any of its nine screen terms is non-zero: the same set up to faces whose only
+    # contributions sit on ambiguous pixels (zeroed cotangents on both sides)
+    assert (views.cpu().numpy().astype(np.int64) != ref.face_views).sum() <= 2 + 1e-3 * M
+    assert views.sum().item() > 0
+    # second call: accumulates; pose-only mask goes through the full-gradient path and still leaves dL/dtau
+    ts.ts_render_bwd_stats(ctx, g.scene, g.frame, dev(gC), dev(gD), None, None, None, None, ts.GRAD_POSE, st, None)
+    tau = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau)
+    torch.cuda.synchronize()
+    assert_grad_close("face_grad2d x2", st.cpu().numpy(), 2 * ref.face_grad2d)
+    assert np.abs(tau.cpu().numpy() - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max()
+    with pytest.raises(ts.TsError):
+        ts.ts_render_bwd_stats(ctx, g.scene, g.frame, dev(gC), None, None, None, None, None, ts.GRAD_COLOR, st, None)
+    g.close()
