@@ -360,6 +360,41 @@ def main():
     stage_ms = {k: float(np.median([a.elapsed_time(b) for a, b in v])) for k, v in stage_ms.items()}
     clocks = clk.stop()
 
+    # extra, informational: one MAPPING view of the same scene (BASELINE.json configs[3]'s step is 8 of these on 1 M
+    # faces): project + bin/sort + forward with L1 + full-gradient backward (positions, colours, opacities), one graph
+    V = tr.scene.V
+    gpos, gcol, gopa = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+    lam = sc.params.lambda_dep
+
+    def map_view():
+        ts.ts_project(tr.ctx, tr.scene, tr.cam, tr.prm, tr.T, tr.frame)
+        ts.ts_bin_sort(tr.ctx, tr.frame)
+        ts.ts_render_fwd_l1(tr.ctx, tr.scene, tr.frame, tr.C, tr.D, tr.A, tr.Chat, tr.Dhat, lam, tr.gC, tr.gD, tr.loss)
+        ts.ts_render_bwd(tr.ctx, tr.scene, tr.frame, tr.gC, tr.gD, None, gpos, gcol, gopa,
+                         ts.GRAD_POS | ts.GRAD_COLOR | ts.GRAD_OPACITY)
+
+    tr.reset()
+    with torch.cuda.stream(stream):
+        for _ in range(2):
+            map_view()
+        stream.synchronize()
+        mrun = map_view
+        if not args.no_graph:
+            mg = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(mg, stream=stream):
+                map_view()
+            mrun = mg.replay
+        mev = []
+        for _ in range(max(10, args.steps // 2)):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            mrun()
+            b.record(stream)
+            mev.append((a, b))
+    stream.synchronize()
+    map_ms = float(np.median([a.elapsed_time(b) for a, b in mev]))
+
     # e2e: same iteration through the C ABI with HOST buffers: the frame's target RGB-D (pinned) and the pose go
     # up, dL/dtau and the loss come back, every step, inside the timed region
     hC, hD = tr.Chat.cpu().pin_memory(), tr.Dhat.cpu().pin_memory()
@@ -419,6 +454,9 @@ def main():
            "step_roofline": {"t_hbm_us": t_hbm * 1e6, "t_alu_us": t_alu * 1e6, "t_roof_us": t_roof * 1e6,
                              "frac": t_roof / (ms_per_step * 1e-3), "algorithmic_bytes": sum(B[k] for k in STEP_ROWS),
                              "algorithmic_flops": sum(F[k] for k in STEP_ROWS), "hbm_peak_gbs": peaks["hbm_gbs"], "fp32_peak_tflops": p_fp32},
+           "mapping_view": {"ms": map_ms, "Mpix_per_s": HW / (map_ms * 1e-3) / 1e6,
+                            "what": "project + bin/sort + forward with L1 + backward wrt positions, colours, opacities of ONE "
+                                    "view of this scene, one CUDA graph, L2 flushed (informational; not the headline metric)"},
            "tracking_iters_per_s": world * 100.0 / (frame_ms * 1e-3), "frame_100_iters_ms": frame_ms,
            "stage_ms": stage_ms, "counters": cnt, "wall_s_timed_region": t_wall}
     if rank == 0:
