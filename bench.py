@@ -395,28 +395,60 @@ def main():
     stream.synchronize()
     map_ms = float(np.median([a.elapsed_time(b) for a, b in mev]))
 
-    # e2e: same iteration through the C ABI with HOST buffers: the frame's target RGB-D (pinned) and the pose go
-    # up, dL/dtau and the loss come back, every step, inside the timed region
+    # e2e: same iteration through the C ABI with HOST buffers: every step the frame's target RGB-D (pinned, 16 B/pixel)
+    # and the pose go up and dL/dtau and the loss come back, all inside the timed region.  The uploads run on a copy
+    # stream into one of two device buffers while the previous step computes (what a tracking front-end does with the
+    # next camera frame); the L2 flush of the protocol is part of every step here, on the compute stream.
     hC, hD = tr.Chat.cpu().pin_memory(), tr.Dhat.cpu().pin_memory()
     hT = tr.T0.cpu().pin_memory()
-    h_out = torch.empty(7).pin_memory()
+    n_e2e = args.warmup + args.steps
+    h_out = torch.empty(n_e2e, 7).pin_memory()
+    bufs = [(tr.Chat, tr.Dhat), (torch.empty_like(tr.Chat), torch.empty_like(tr.Dhat))]
+    runs = [run]
+    with torch.cuda.stream(stream):
+        tr.Chat, tr.Dhat = bufs[1]
+        if args.no_graph:
+            def run_b():
+                tr.Chat, tr.Dhat = bufs[1]
+                tr.iteration()
+                tr.Chat, tr.Dhat = bufs[0]
+            runs.append(run_b)
+        else:
+            g2 = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g2, stream=stream):
+                tr.iteration()
+            runs.append(g2.replay)
+        tr.Chat, tr.Dhat = bufs[0]
+    stream.synchronize()
     tr.reset()
-    e2e_ms = []
-    for it in range(args.warmup + args.steps):
-        flush.fill_(1)
-        torch.cuda.synchronize()
-        t0 = time.perf_counter()
-        with torch.cuda.stream(stream):
-            tr.Chat.copy_(hC, non_blocking=True)
-            tr.Dhat.copy_(hD, non_blocking=True)
-            tr.T.copy_(hT, non_blocking=True)
-            run()
-            h_out[:6].copy_(tr.tau, non_blocking=True)
-            h_out[6:].copy_(tr.loss, non_blocking=True)
-        stream.synchronize()
-        if it >= args.warmup:
-            e2e_ms.append((time.perf_counter() - t0) * 1e3)
-    e2e_step = float(np.mean(e2e_ms))
+    copy_stream = torch.cuda.Stream()
+    copied = [torch.cuda.Event() for _ in range(n_e2e)]
+    done = [torch.cuda.Event() for _ in range(n_e2e)]
+
+    def e2e_steps(i0, i1):
+        for i in range(i0, i1):
+            b = i & 1
+            with torch.cuda.stream(copy_stream):
+                if i >= 2:
+                    copy_stream.wait_event(done[i - 2])           # the buffer's previous user has finished
+                bufs[b][0].copy_(hC, non_blocking=True)
+                bufs[b][1].copy_(hD, non_blocking=True)
+                copied[i].record(copy_stream)
+            with torch.cuda.stream(stream):
+                flush.fill_(1)
+                tr.T.copy_(hT, non_blocking=True)
+                stream.wait_event(copied[i])
+                runs[b]()
+                h_out[i, :6].copy_(tr.tau, non_blocking=True)
+                h_out[i, 6:].copy_(tr.loss, non_blocking=True)
+                done[i].record(stream)
+
+    e2e_steps(0, args.warmup)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e2e_steps(args.warmup, n_e2e)
+    torch.cuda.synchronize()
+    e2e_step = (time.perf_counter() - t0) * 1e3 / args.steps
     e2e_step = max_over_ranks(dist, e2e_step, "cuda")
 
     value = world * HW / (ms_per_step * 1e-3) / 1e6
@@ -449,7 +481,10 @@ def main():
                       "cuda_graph": graph is not None},
            "clocks": clocks, "gpu_launches": Tracker.launches_per_iter * args.steps,
            "e2e": {"value": world * HW / (e2e_step * 1e-3) / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": 16 * HW + 48,
-                   "d2h_bytes_per_step": 28, "ms_per_step": e2e_step},
+                   "d2h_bytes_per_step": 28, "ms_per_step": e2e_step,
+                   "how": "K steps timed as a whole by the host clock; every step uploads its target RGB-D frame and pose from "
+                          "pinned memory (copy stream, two device buffers, overlapping the previous step's kernels), flushes L2, "
+                          "runs the iteration and reads dL/dtau + loss back"},
            "roofline": roof,
            "step_roofline": {"t_hbm_us": t_hbm * 1e6, "t_alu_us": t_alu * 1e6, "t_roof_us": t_roof * 1e6,
                              "frac": t_roof / (ms_per_step * 1e-3), "algorithmic_bytes": sum(B[k] for k in STEP_ROWS),
