@@ -369,9 +369,8 @@ def main():
     def map_view():
         ts.ts_project(tr.ctx, tr.scene, tr.cam, tr.prm, tr.T, tr.frame)
         ts.ts_bin_sort(tr.ctx, tr.frame)
-        ts.ts_render_fwd_l1(tr.ctx, tr.scene, tr.frame, tr.C, tr.D, tr.A, tr.Chat, tr.Dhat, lam, tr.gC, tr.gD, tr.loss)
-        ts.ts_render_bwd(tr.ctx, tr.scene, tr.frame, tr.gC, tr.gD, None, gpos, gcol, gopa,
-                         ts.GRAD_POS | ts.GRAD_COLOR | ts.GRAD_OPACITY)
+        ts.ts_render_map_l1(tr.ctx, tr.scene, tr.frame, tr.C, tr.D, tr.A, tr.Chat, tr.Dhat, lam, tr.gC, tr.gD, tr.loss,
+                            gpos, gcol, gopa, ts.GRAD_POS | ts.GRAD_COLOR | ts.GRAD_OPACITY)
 
     tr.reset()
     with torch.cuda.stream(stream):
@@ -490,8 +489,9 @@ def main():
                              "frac": t_roof / (ms_per_step * 1e-3), "algorithmic_bytes": sum(B[k] for k in STEP_ROWS),
                              "algorithmic_flops": sum(F[k] for k in STEP_ROWS), "hbm_peak_gbs": peaks["hbm_gbs"], "fp32_peak_tflops": p_fp32},
            "mapping_view": {"ms": map_ms, "Mpix_per_s": HW / (map_ms * 1e-3) / 1e6,
-                            "what": "project + bin/sort + forward with L1 + backward wrt positions, colours, opacities of ONE "
-                                    "view of this scene, one CUDA graph, L2 flushed (informational; not the headline metric)"},
+                            "what": "project + bin/sort + ts_render_map_l1 (forward, L1, backward wrt positions, colours, "
+                                    "opacities) of ONE view of this scene, one CUDA graph, L2 flushed (informational; not the "
+                                    "headline metric)"},
            "tracking_iters_per_s": world * 100.0 / (frame_ms * 1e-3), "frame_100_iters_ms": frame_ms,
            "stage_ms": stage_ms, "counters": cnt, "wall_s_timed_region": t_wall}
     if rank == 0:

@@ -143,6 +143,16 @@ int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, fl
 int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
                            float* out_alpha, const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD,
                            float* loss_dev, void* stream);
+/* The mapping counterpart of ts_render_track_l1: a3 + a4 + a5 (FULL-gradient) per 8x4-pixel block in one launch, then a6:
+ * every block is rendered, its L1 cotangents are formed in registers and its reverse walk runs at once, with the
+ * colour / opacity gradients and the per-face screen terms accumulated as by ts_render_bwd (grad_* are added to;
+ * TS_GRAD_POSE leaves partial sums for ts_pose_jacobian_reduce).  grad_mask must select at least one of TS_GRAD_POS /
+ * TS_GRAD_COLOR / TS_GRAD_OPACITY.  Same arithmetic as ts_render_fwd_l1 + ts_render_bwd; the sums differ from theirs
+ * only in the order of the float atomics.  out_*, gC, gD and loss_dev may be NULL.  ts_render_bwd cannot follow. */
+int32_t ts_render_map_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
+                         float* out_alpha, const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD,
+                         float* loss_dev, float* grad_pos, float* grad_color, float* grad_opacity, uint32_t grad_mask,
+                         void* stream);
 /* Per-face statistics for the map-management layer (PAPER.md:137 covisibility of rendered faces,
  * :169 prune by projected area, :175 blur-split by pixel coverage).
  * ts_render_fwd_stats: as ts_render_fwd, and face_pixels[m] += number of pixels face m contributed to (caller zeroes;

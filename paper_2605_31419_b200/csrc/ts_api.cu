@@ -268,6 +268,22 @@ int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float*
                                   (cudaStream_t)stream);
 }
 
+int32_t ts_render_map_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth, float* out_alpha,
+                         const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
+                         float* grad_pos, float* grad_color, float* grad_opacity, uint32_t grad_mask, void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !sc->pos || !Chat || !Dhat) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_POS) && !grad_pos) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_COLOR) && !grad_color) return TS_ERR_INVALID_ARG;
+    if ((grad_mask & TS_GRAD_OPACITY) && !grad_opacity) return TS_ERR_INVALID_ARG;
+    if (grad_mask & ~(uint32_t)(TS_GRAD_POS | TS_GRAD_COLOR | TS_GRAD_OPACITY | TS_GRAD_POSE)) return TS_ERR_INVALID_ARG;
+    if (!(grad_mask & (TS_GRAD_POS | TS_GRAD_COLOR | TS_GRAD_OPACITY))) return TS_ERR_INVALID_ARG;   // pose-only: ts_render_track_l1
+    if (!fr->have_sort) return TS_ERR_STATE;
+    fr->have_fwd = 0;                                       // n_contrib / T_last are not written
+    return ts_launch_render_map(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev, grad_pos,
+                                grad_color, grad_opacity, grad_mask, (cudaStream_t)stream);
+}
+
 int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
                       const float* dL_dalpha, float* grad_pos, float* grad_color, float* grad_opacity,
                       uint32_t grad_mask, void* stream) {

@@ -242,7 +242,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
         const uint32_t n = hi - lo;
         uint4 cur = make_uint4(0u, 0u, 0u, 0u);
         uint32_t lmask;
-        const bool prestaged = POSE && lo == prestaged_lo;
+        const bool prestaged = lo == prestaged_lo;
         if (prestaged) {
             // the forward walk of this job left exactly this chunk staged, rows 0-11, masks after the block cull
             lmask = (uint32_t)lane < n ? sm.lm[lane] : 0u;

@@ -66,6 +66,7 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
                 sm.r[lane][6] = a0, sm.r[lane][7] = a1, sm.r[lane][8] = a2;
                 const float4 b0 = __ldg(rp + 7), b1 = __ldg(rp + 8), b2 = __ldg(rp + 9);
                 sm.r[lane][9] = b0, sm.r[lane][10] = b1, sm.r[lane][11] = b2;
+                sm.face[lane] = cur.y;                  // (read by the full-gradient backward only)
             }
         }
         if (FULLREC && c0 + 32u >= job.range.y) {

@@ -117,5 +117,8 @@ int32_t ts_launch_render_bwd(const ts_ctx*, ts_frame*, const ts_scene*, const fl
                              uint32_t* face_views = nullptr);
 int32_t ts_launch_render_track(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
                                const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, cudaStream_t);
+int32_t ts_launch_render_map(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
+                             const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, float* grad_pos,
+                             float* grad_color, float* grad_opacity, uint32_t mask, cudaStream_t);
 int32_t ts_launch_pose_reduce(const ts_ctx*, ts_frame*, float* out, float* T_cw, float* state, const float* lr6, float beta1,
                               float beta2, float eps, cudaStream_t);

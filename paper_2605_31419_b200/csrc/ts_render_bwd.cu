@@ -83,12 +83,16 @@ union TrackWarpSmem {
     BwdWarpSmem bwd;
 };
 
-template <int SM>
+// POSE = true: the tracking job above.  POSE = false: the MAPPING job, the same forward walk and loss followed by the
+// full-gradient backward walk (ATTR: colours / opacities, GEOM: screen-space vertex terms into gscr, which
+// proj_bwd_kernel consumes afterwards).
+template <int SM, bool ATTR = false, bool GEOM = false, bool POSE = true>
 __global__ void __launch_bounds__(TS_JOB_WARPS * 32, 3)
 render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float t_min, float fx, float fy,
                     float* __restrict__ out_color, float* __restrict__ out_depth, float* __restrict__ out_alpha,
                     const float* __restrict__ Chat, const float* __restrict__ Dhat, float wc, float wd,
-                    float* __restrict__ gCo, float* __restrict__ gDo, float* __restrict__ loss) {
+                    float* __restrict__ gCo, float* __restrict__ gDo, float* __restrict__ loss,
+                    float* __restrict__ grad_color = nullptr, float* __restrict__ grad_opacity = nullptr) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     TrackWarpSmem& sm = reinterpret_cast<TrackWarpSmem*>(smem_raw)[threadIdx.x >> 5];
@@ -132,15 +136,17 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
         }
         __syncwarp();                                      // the forward walk's shared-memory slice is re-used
         float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-        ts_bwd_walk<SM, false, false, true>(f, sc, job, lane, sm.bwd, sigma, alpha_min, fx, fy, o.last, o.Tlast, gC0, gC1,
-                                            gC2, gD, 0.0f, nullptr, nullptr, tau, 0.f, 0.f, 0.f, staged_lo);
+        ts_bwd_walk<SM, ATTR, GEOM, POSE>(f, sc, job, lane, sm.bwd, sigma, alpha_min, fx, fy, o.last, o.Tlast, gC0, gC1,
+                                          gC2, gD, 0.0f, grad_color, grad_opacity, tau, 0.f, 0.f, 0.f, staged_lo);
+        if (POSE) {
 #pragma unroll
-        for (int jj = 0; jj < 6; ++jj) tau[jj] = warp_sum(tau[jj]);
-        if (lane < 6) {
-            float v = tau[0];
+            for (int jj = 0; jj < 6; ++jj) tau[jj] = warp_sum(tau[jj]);
+            if (lane < 6) {
+                float v = tau[0];
 #pragma unroll
-            for (int jj = 1; jj < 6; ++jj) v = (lane == jj) ? tau[jj] : v;
-            f.pose_partials[6 * ((size_t)job.tile * TS_BLOCKS_PER_TILE + job.blk) + lane] = v;
+                for (int jj = 1; jj < 6; ++jj) v = (lane == jj) ? tau[jj] : v;
+                f.pose_partials[6 * ((size_t)job.tile * TS_BLOCKS_PER_TILE + job.blk) + lane] = v;
+            }
         }
         __syncwarp();
     }
@@ -165,6 +171,28 @@ void launch_track(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, flo
     const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 3, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
     render_track_kernel<SM><<<grid, TS_JOB_WARPS * 32, smem, st>>>(f, sc, fr->prm.sigma, fr->prm.alpha_min, fr->prm.t_min,
                                                                   fr->cam.fx, fr->cam.fy, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss);
+}
+
+template <int SM, bool ATTR, bool GEOM>
+void launch_map(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, float* oc, float* od, float* oa, const float* Chat,
+                const float* Dhat, float wc, float wd, float* gC, float* gD, float* loss, float* gcol, float* gopa,
+                cudaStream_t st) {
+    const TsFrameDev& f = fr->d;
+    const size_t smem = sizeof(TrackWarpSmem) * TS_JOB_WARPS;
+    cudaFuncSetAttribute(render_track_kernel<SM, ATTR, GEOM, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 3, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
+    render_track_kernel<SM, ATTR, GEOM, false><<<grid, TS_JOB_WARPS * 32, smem, st>>>(
+        f, sc, fr->prm.sigma, fr->prm.alpha_min, fr->prm.t_min, fr->cam.fx, fr->cam.fy, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss,
+        gcol, gopa);
+}
+
+template <int SM>
+void launch_map_sm(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, float* oc, float* od, float* oa, const float* Chat,
+                   const float* Dhat, float wc, float wd, float* gC, float* gD, float* loss, float* gcol, float* gopa, bool attr,
+                   bool geom, cudaStream_t st) {
+    if (attr && geom) launch_map<SM, true, true>(ctx, fr, sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, st);
+    else if (geom) launch_map<SM, false, true>(ctx, fr, sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, st);
+    else launch_map<SM, true, false>(ctx, fr, sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, st);
 }
 
 }  // namespace
@@ -477,6 +505,37 @@ int32_t ts_launch_render_track(const ts_ctx* ctx, ts_frame* fr, const ts_scene* 
         default: launch_track<0>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, st); break;
     }
     fr->pose_src = 1, fr->n_pose_partials = (uint32_t)fr->d.NT * TS_BLOCKS_PER_TILE;
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
+
+// a3 + a4 + a5 (full-gradient) + a6 in two launches: the mapping counterpart of ts_launch_render_track.
+int32_t ts_launch_render_map(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
+                             const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss,
+                             float* grad_pos, float* grad_color, float* grad_opacity, uint32_t mask, cudaStream_t st) {
+    const bool attr = (mask & (TS_GRAD_COLOR | TS_GRAD_OPACITY)) != 0;
+    const bool geom = (mask & (TS_GRAD_POS | TS_GRAD_POSE)) != 0;
+    const double n = (double)fr->d.W * (double)fr->d.H;
+    const float wc = (float)(1.0 / (3.0 * n)), wd = (float)((double)lambda_dep / n);
+    float* gcol = (mask & TS_GRAD_COLOR) ? grad_color : nullptr;
+    float* gopa = (mask & TS_GRAD_OPACITY) ? grad_opacity : nullptr;
+    switch (ts_sigma_mode(fr->prm.sigma)) {
+        case 1: launch_map_sm<1>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, attr, geom, st); break;
+        case 2: launch_map_sm<2>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, attr, geom, st); break;
+        case 3: launch_map_sm<3>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, attr, geom, st); break;
+        default: launch_map_sm<0>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, attr, geom, st); break;
+    }
+    fr->pose_src = 0;
+    if (geom) {
+        const int grid = (int)min((uint32_t)(ctx->num_sms * 4), fr->d.n_partials_cap);
+        const int want_pose = (mask & TS_GRAD_POSE) ? 1 : 0;
+        float* gp = (mask & TS_GRAD_POS) ? grad_pos : nullptr;
+        if (sc->faces == nullptr)
+            proj_bwd_kernel<true><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, nullptr, fr->T_cw, fr->cam, gp, want_pose);
+        else
+            proj_bwd_kernel<false><<<grid, PB_THREADS, 0, st>>>(fr->d, sc->pos, sc->faces, fr->T_cw, fr->cam, gp, want_pose);
+        if (want_pose) fr->pose_src = 2, fr->n_pose_partials = (uint32_t)grid;
+    }
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

@@ -25,7 +25,7 @@ _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.
                 VIEW_TILE_RANGES: torch.int32, VIEW_N_CONTRIB: torch.int32, VIEW_COUNTERS: torch.int64}
 
 EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
-           "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
+           "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_map_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
            "ts_render_fwd_normal", "ts_render_bwd_normal", "ts_normal_loss_grad", "ts_render_bwd_stats",
            "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view"]
 
@@ -82,6 +82,9 @@ def _load():
                                         C.c_void_p, C.c_void_p]
     lib.ts_render_bwd_stats.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_render_map_l1.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                     C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                     C.c_void_p, C.c_void_p, C.c_uint32, C.c_void_p]
     lib.ts_pose_jacobian_reduce.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_l1_loss_grad.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -239,6 +242,13 @@ def ts_render_bwd_stats(ctx, scene, frame, dL_dcolor, dL_ddepth, dL_dalpha, grad
     _check(lib.ts_render_bwd_stats(ctx.h, C.byref(scene.c), frame.h, _ptr(dL_dcolor), _ptr(dL_ddepth), _ptr(dL_dalpha),
                                    _ptr(grad_pos), _ptr(grad_color), _ptr(grad_opacity), int(grad_mask),
                                    _ptr(face_grad2d), _ptr(face_views, torch.int32), _stream(stream)))
+
+
+def ts_render_map_l1(ctx, scene, frame, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss, grad_pos,
+                     grad_color, grad_opacity, grad_mask, stream=None):
+    _check(lib.ts_render_map_l1(ctx.h, C.byref(scene.c), frame.h, _ptr(out_color), _ptr(out_depth), _ptr(out_alpha),
+                                _ptr(Chat), _ptr(Dhat), float(lambda_dep), _ptr(gC), _ptr(gD), _ptr(loss), _ptr(grad_pos),
+                                _ptr(grad_color), _ptr(grad_opacity), int(grad_mask), _stream(stream)))
 
 
 def ts_pose_jacobian_reduce(ctx, frame, dL_dtau, stream=None):

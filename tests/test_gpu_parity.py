@@ -675,3 +675,54 @@ def test_screen_gradient_statistic(ctx, oracle_mod, cfg):
     with pytest.raises(ts.TsError):
         ts.ts_render_bwd_stats(ctx, g.scene, g.frame, dev(gC), None, None, None, None, None, ts.GRAD_COLOR, st, None)
     g.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 3, 4])
+def test_render_map_l1_equals_separate_calls(ctx, oracle_mod, cfg):
+    """ts_render_map_l1 (a3 + a4 + a5 full-gradient + a6 fused) against ts_render_fwd_l1 + ts_render_bwd: images, loss
+    cotangents bit for bit; per-vertex gradients and the pose to the order of the float atomics; every mask shape."""
+    from gpu_util import assert_grad_close, dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(cfg)
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    tgt_pos = sc.pos_target if sc.pos_target is not None else sc.pos
+    tgt_col = sc.color_target if sc.color_target is not None else sc.color
+    tgt = oracle_mod.Oracle(tgt_pos, tgt_col, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+    Chat, Dhat = dev(tgt.color), dev(tgt.depth)
+    lam, V = sc.params.lambda_dep, sc.pos.shape[0]
+    z3, z1 = (lambda: torch.zeros(V, 3, device="cuda")), (lambda: torch.zeros(V, device="cuda"))
+    gC, gD, L1 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
+    gp1, gc1, go1 = z3(), z3(), z1()
+    ts.ts_render_fwd_l1(ctx, g.scene, g.frame, None, None, None, Chat, Dhat, lam, gC, gD, L1)
+    ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, gp1, gc1, go1, ts.GRAD_ALL)
+    tau1 = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau1)
+    C2, D2, A2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.empty_like(g.A)
+    gC2, gD2, L2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
+    gp2, gc2, go2 = z3(), z3(), z1()
+    ts.ts_render_map_l1(ctx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, lam, gC2, gD2, L2, gp2, gc2, go2, ts.GRAD_ALL)
+    tau2 = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau2)
+    torch.cuda.synchronize()
+    assert torch.equal(C2, g.C) and torch.equal(D2, g.D) and torch.equal(A2, g.A)
+    assert torch.equal(gC, gC2) and torch.equal(gD, gD2)
+    assert abs(L1.item() - L2.item()) <= 1e-5 * abs(L1.item())
+    n = lambda t: t.cpu().numpy()
+    assert_grad_close("grad_pos", n(gp2), n(gp1), tol=2e-5)
+    assert_grad_close("grad_color", n(gc2), n(gc1), tol=2e-5)
+    assert_grad_close("grad_opacity", n(go2), n(go1), tol=2e-5)
+    assert np.abs(n(tau2) - n(tau1)).max() <= 1e-4 * np.abs(n(tau1)).max()
+    # partial masks; accumulation (+=) into the same buffers
+    ts.ts_render_map_l1(ctx, g.scene, g.frame, None, None, None, Chat, Dhat, lam, None, None, None, gp2, None, None, ts.GRAD_POS)
+    ts.ts_render_map_l1(ctx, g.scene, g.frame, None, None, None, Chat, Dhat, lam, None, None, None, None, gc2, go2,
+                        ts.GRAD_COLOR | ts.GRAD_OPACITY)
+    torch.cuda.synchronize()
+    assert_grad_close("grad_pos x2", n(gp2), 2 * n(gp1), tol=2e-5)
+    assert_grad_close("grad_color x2", n(gc2), 2 * n(gc1), tol=2e-5)
+    assert_grad_close("grad_opacity x2", n(go2), 2 * n(go1), tol=2e-5)
+    with pytest.raises(ts.TsError):
+        ts.ts_render_map_l1(ctx, g.scene, g.frame, None, None, None, Chat, Dhat, lam, None, None, None, None, None, None, ts.GRAD_POSE)
+    with pytest.raises(ts.TsError):
+        ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, gp1, None, None, ts.GRAD_POS)      # no walk state after map
+    g.close()
