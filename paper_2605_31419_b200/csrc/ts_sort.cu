@@ -287,10 +287,12 @@ __device__ __forceinline__ void cta_sort_network(KP k, VP v, uint32_t n) {
     uint32_t N = 1;
     while (N < n) N <<= 1;
     const uint32_t half = N >> 1;
-    for (uint32_t size = 2; size <= N; size <<= 1) {
+    // (all sizes and strides are powers of two: shifts and masks, no integer division)
+    uint32_t lg_hs = 0;
+    for (uint32_t size = 2; size <= N; size <<= 1, ++lg_hs) {
         const uint32_t hs = size >> 1;
         for (uint32_t t = threadIdx.x; t < half; t += blockDim.x) {
-            const uint32_t blk = t / hs, off = t - blk * hs;
+            const uint32_t blk = t >> lg_hs, off = t & (hs - 1u);
             const uint32_t lo = blk * size + off, hi = blk * size + size - 1 - off;
             if (hi < n) {
                 const unsigned long long a = k[lo], b = k[hi];
@@ -302,9 +304,11 @@ __device__ __forceinline__ void cta_sort_network(KP k, VP v, uint32_t n) {
             }
         }
         __syncthreads();
+        uint32_t lg_st = lg_hs;
         for (uint32_t stride = hs >> 1; stride > 0; stride >>= 1) {
+            --lg_st;
             for (uint32_t t = threadIdx.x; t < half; t += blockDim.x) {
-                const uint32_t lo = 2 * stride * (t / stride) + (t % stride), hi = lo + stride;
+                const uint32_t lo = ((t >> lg_st) << (lg_st + 1u)) + (t & (stride - 1u)), hi = lo + stride;
                 if (hi < n) {
                     const unsigned long long a = k[lo], b = k[hi];
                     if (b < a) {
