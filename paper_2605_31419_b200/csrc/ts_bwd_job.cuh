@@ -147,8 +147,15 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
     }
     // segmented reduction over runs of equal staged index (inactive lanes never match anybody)
     const uint32_t key = active ? e : 0x100u + (uint32_t)lane;
+    // only as many doubling steps as the longest run needs (runs average ~8 hits; a chunk-end group is short)
+    const uint32_t kp = __shfl_up_sync(0xffffffffu, key, 1);
+    const bool run_start = lane == 0 || kp != key;
+    const uint32_t starts = __ballot_sync(0xffffffffu, run_start);
+    const int my_start = 31 - __clz((int)(starts & (0xffffffffu >> (31 - lane))));
+    const uint32_t max_off = __reduce_max_sync(0xffffffffu, active ? (uint32_t)(lane - my_start) : 0u);
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
+        if ((uint32_t)d > max_off) break;
         const uint32_t kd = __shfl_down_sync(0xffffffffu, key, d);
         const bool same = (lane + d < 32) && kd == key;
         if (GEOM) {
@@ -173,8 +180,7 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
             }
         }
     }
-    const uint32_t kp = __shfl_up_sync(0xffffffffu, key, 1);
-    if (active && (lane == 0 || kp != key)) {                  // first lane of a run
+    if (active && run_start) {                                 // first lane of a run
         if (GEOM) {
             float* gs = f.gscr + 9 * (size_t)sm.slot[e];
 #pragma unroll
