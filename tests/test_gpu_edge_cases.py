@@ -224,3 +224,44 @@ def test_tracking_loop_converges(ctx, oracle_mod):
     assert losses[-1] < 0.25 * losses[0], losses
     assert e1[0] < 0.2 * e0[0] and e1[1] < 0.2 * e0[1], (e0, e1, losses)
     frame.release()
+
+
+def test_mapping_loop_descends(ctx, oracle_mod):
+    """A mapping loop in the shape of PAPER.md:139-167 on the config-3 recipe (perturbed vertices and colours, keyframes
+    rendered from the unperturbed scene): per step the per-vertex gradients of all views are accumulated by
+    ts_render_map_l1 and an Adam step (torch, on the same device buffers) is taken.  The loss must come down."""
+    from gpu_util import dev
+    from paper_2605_31419_b200 import ts
+    sc = scenes.config3(n_faces=150_000, n_views=2)
+    pos, col, opa = dev(sc.pos), dev(sc.color), dev(sc.opacity)
+    scene = ts.Scene(pos, col, opa)
+    tscene = ts.Scene(dev(sc.pos_target), dev(sc.color_target), dev(sc.opacity))
+    cam, prm = ts.make_camera(sc.cam), ts.make_params(sc.params)
+    H, W, V = sc.cam.height, sc.cam.width, sc.pos.shape[0]
+    frame = ts.Frame(ctx, scene.M, W, H, 4 * scene.M)
+    poses = [dev(T.reshape(-1)) for T in sc.T_gt]
+    targets = []
+    for T in poses:
+        Chat, Dhat = torch.zeros(3, H, W, device="cuda"), torch.zeros(H, W, device="cuda")
+        ts.ts_project(ctx, tscene, cam, prm, T, frame)
+        ts.ts_bin_sort(ctx, frame)
+        ts.ts_render_fwd(ctx, tscene, frame, Chat, Dhat, None)
+        targets.append((Chat, Dhat))
+    gp, gc, go = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+    pos.grad, col.grad, opa.grad = gp, gc, go
+    opt = torch.optim.Adam([{"params": [pos], "lr": 1e-4}, {"params": [col], "lr": 2e-3}, {"params": [opa], "lr": 1e-3}])
+    loss = torch.zeros(1, device="cuda")
+    history = []
+    for step in range(40):
+        gp.zero_(), gc.zero_(), go.zero_(), loss.zero_()
+        for T, (Chat, Dhat) in zip(poses, targets):
+            ts.ts_project(ctx, scene, cam, prm, T, frame)
+            ts.ts_bin_sort(ctx, frame)
+            ts.ts_render_map_l1(ctx, scene, frame, None, None, None, Chat, Dhat, sc.params.lambda_dep, None, None, loss,
+                                gp, gc, go, ts.GRAD_POS | ts.GRAD_COLOR | ts.GRAD_OPACITY)
+        history.append(loss.item())
+        opt.step()
+    print(f"mapping: loss {history[0]:.5f} -> {history[-1]:.5f} ({' '.join(f'{h:.4f}' for h in history[::5])})")
+    assert ts.ts_frame_status(ctx, frame)[0] == 0
+    assert history[-1] < 0.7 * history[0], history
+    frame.release()
