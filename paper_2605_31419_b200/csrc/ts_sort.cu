@@ -226,7 +226,9 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
             uint32_t pos[4];
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                tt[i] = (ty0 + i / max(ntx, 1)) * f.tiles_x + tx0 + i % max(ntx, 1);
+                // i < 4 pairs over ntx columns: row = i / ntx by comparisons (an integer division is a subroutine call)
+                const int row = (i >= ntx ? 1 : 0) + (i >= 2 * ntx ? 1 : 0) + (i >= 3 * ntx ? 1 : 0);
+                tt[i] = (ty0 + row) * f.tiles_x + tx0 + (i - row * ntx);
                 pos[i] = 0;
                 if (nt <= 4 && i < nt) pos[i] = atomicAdd(f.tile_cursor + tt[i], 1u);
             }
