@@ -1,6 +1,7 @@
 // ts_api.cu -- the C-ABI boundary (include/ts.h): context, frame workspace carving, status / debug views and
 // host-side argument validation for the five hot-path calls.  No device memory is allocated here: the frame lives
 // entirely inside caller-provided memory.
+#include <cstdlib>
 #include <new>
 
 #include "ts_internal.cuh"
@@ -74,6 +75,8 @@ int32_t ts_create(int32_t device, ts_ctx** out) {
     ts_ctx* c = new (std::nothrow) ts_ctx;
     if (!c) return TS_ERR_CUDA;
     c->device = device, c->num_sms = p.multiProcessorCount, c->max_smem_optin = (int)p.sharedMemPerBlockOptin;
+    const char* tl = getenv("TS_TRACK_LOG");
+    c->track_log = (tl && tl[0] == '1') ? 1 : 0;
     *out = c;
     return TS_OK;
 }

@@ -29,15 +29,18 @@ __device__ __forceinline__ uint32_t ts_job_take(const TsFrameDev& f, int which, 
     return __shfl_sync(0xffffffffu, j, 0);
 }
 
-__device__ __forceinline__ void ts_job_finish(const TsFrameDev& f, int which, int lane) {
+// total = persistent warps of the launch
+__device__ __forceinline__ void ts_job_finish_n(const TsFrameDev& f, int which, int lane, uint32_t total) {
     if (lane == 0) {
-        const uint32_t total = gridDim.x * TS_JOB_WARPS;
         if (atomicAdd(&f.ctrl->job_done[which], 1u) == total - 1u) {
             // every warp has taken its last ticket: re-arm for the next launch
             f.ctrl->job_ticket[which] = 0u;
             f.ctrl->job_done[which] = 0u;
         }
     }
+}
+__device__ __forceinline__ void ts_job_finish(const TsFrameDev& f, int which, int lane) {
+    ts_job_finish_n(f, which, lane, gridDim.x * TS_JOB_WARPS);
 }
 
 __device__ __forceinline__ void ts_job_decode(const TsFrameDev& f, uint32_t j, int lane, TsJob& job) {

@@ -163,11 +163,7 @@ void launch_track(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, flo
                   const float* Dhat, float wc, float wd, float* gC, float* gD, float* loss, cudaStream_t st) {
     const TsFrameDev& f = fr->d;
     const size_t smem = sizeof(TrackWarpSmem) * TS_JOB_WARPS;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(render_track_kernel<SM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_set = true;
-    }
+    cudaFuncSetAttribute(render_track_kernel<SM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);   // per device
     const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 3, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
     render_track_kernel<SM><<<grid, TS_JOB_WARPS * 32, smem, st>>>(f, sc, fr->prm.sigma, fr->prm.alpha_min, fr->prm.t_min,
                                                                   fr->cam.fx, fr->cam.fy, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss);
@@ -386,11 +382,8 @@ void launch_one(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, const
                 float* gcol, float* gopa, cudaStream_t st) {
     const TsFrameDev& f = fr->d;
     const size_t smem = sizeof(BwdWarpSmem) * TS_JOB_WARPS;
-    static bool attr_set = false;                      // one-time opt-in above 48 KB of dynamic shared memory
-    if (!attr_set) {
-        cudaFuncSetAttribute(render_bwd_kernel<SM, ATTR, GEOM, POSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        attr_set = true;
-    }
+    // opt-in above 48 KB of dynamic shared memory; the attribute is per device, so it is set at every launch
+    cudaFuncSetAttribute(render_bwd_kernel<SM, ATTR, GEOM, POSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 3, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
     render_bwd_kernel<SM, ATTR, GEOM, POSE><<<grid, TS_JOB_WARPS * 32, smem, st>>>(f, sc, fr->prm.sigma, fr->prm.alpha_min,
                                                                                    fr->cam.fx, fr->cam.fy, gC, gD, gA, gcol, gopa);
@@ -493,9 +486,9 @@ int32_t ts_launch_render_bwd_normal(const ts_ctx* ctx, ts_frame* fr, const ts_sc
     return TS_OK;
 }
 
-int32_t ts_launch_render_track(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
-                               const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss,
-                               cudaStream_t st) {
+int32_t ts_launch_render_track_v1(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
+                                  const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss,
+                                  cudaStream_t st) {
     const double n = (double)fr->d.W * (double)fr->d.H;
     const float wc = (float)(1.0 / (3.0 * n)), wd = (float)((double)lambda_dep / n);
     switch (ts_sigma_mode(fr->prm.sigma)) {
