@@ -20,6 +20,9 @@
 #include "ts_normal.cuh"
 #include "ts_pose.cuh"
 
+#include <cooperative_groups.h>
+namespace cg = cooperative_groups;
+
 namespace {
 
 // ATTR: colour / opacity gradients (B1, B4).  GEOM: screen-space vertex gradients into gscr (B5-B6).
@@ -313,20 +316,25 @@ proj_bwd_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __re
     }
 }
 
-// a7: fixed-order tree reduction of the partials.  CTA g sums a fixed contiguous slice of the partials (fixed
-// per-thread order, fixed shuffle / shared-memory tree) into block partial g; the last CTA to finish adds the block
-// partials in index order and writes dL/dtau -- the result does not depend on scheduling.  Optionally the same
-// thread then takes the Adam / Exp step on the pose (a8), which saves a launch in the tracking loop.
-constexpr int PR_THREADS = 256, PR_BLOCKS = 32;
+// a7: fixed-order tree reduction of the partials, in ONE round trip: a thread-block cluster of PR_BLOCKS CTAs, CTA g
+// sums a fixed contiguous slice of the partials (fixed per-thread order, fixed shuffle / shared-memory tree) and puts
+// its six sums into the shared memory of CTA 0 through distributed shared memory; after the cluster barrier the first
+// six threads of CTA 0 add the block sums in index order and write dL/dtau -- the result does not depend on
+// scheduling, and there is no global atomic, fence or second trip to L2.  Optionally one warp of CTA 0 then takes the
+// Adam / Exp step on the pose (a8), which saves a launch in the tracking loop.
+constexpr int PR_THREADS = 1024, PR_BLOCKS = 8;
 
-__global__ void __launch_bounds__(PR_THREADS)
+__global__ void __cluster_dims__(PR_BLOCKS, 1, 1) __launch_bounds__(PR_THREADS)
 pose_reduce_kernel(TsFrameDev f, uint32_t n, float* __restrict__ out, float* __restrict__ T_cw, float* __restrict__ state,
                    TsLr6 lr, float beta1, float beta2, float eps) {
     __shared__ float sm[PR_THREADS / 32][6];
-    __shared__ uint32_t s_last;
+    __shared__ float sb[PR_BLOCKS][6];                                   // CTA 0's copy receives the block sums
+    __shared__ float tot[6];
+    cg::cluster_group cluster = cg::this_cluster();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t rank = cluster.block_rank();
     const uint32_t per = (n + PR_BLOCKS - 1) / PR_BLOCKS;
-    const uint32_t i0 = min(n, blockIdx.x * per), i1 = min(n, i0 + per);
+    const uint32_t i0 = min(n, rank * per), i1 = min(n, i0 + per);
     float a[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
     const float2* p2 = reinterpret_cast<const float2*>(f.pose_partials);
     for (uint32_t ib = i0; ib < i1; ib += 4 * PR_THREADS) {              // 12 independent loads in flight per thread
@@ -348,33 +356,24 @@ pose_reduce_kernel(TsFrameDev f, uint32_t n, float* __restrict__ out, float* __r
         if (lane == 0) sm[warp][j] = a[j];
     }
     __syncthreads();
-    float* blockp = f.pose_partials + 6 * (size_t)f.n_partials_cap;      // [PR_BLOCKS][6] behind the partials
     if (tid < 6) {
         float s = 0.f;
 #pragma unroll
         for (int w = 0; w < PR_THREADS / 32; ++w) s += sm[w][tid];
-        __stcg(blockp + 6 * blockIdx.x + tid, s);
+        float* dst = cluster.map_shared_rank(&sb[0][0], 0);               // CTA 0's sb
+        dst[6 * rank + tid] = s;
     }
-    __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        s_last = (atomicAdd(&f.ctrl->reduce_done, 1u) == gridDim.x - 1) ? 1u : 0u;
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    __shared__ float sb[PR_BLOCKS * 6];
-    if (tid < (int)gridDim.x * 6) sb[tid] = __ldcg(blockp + tid);       // all block partials in one round trip
-    __syncthreads();
+    cluster.sync();
+    if (rank != 0) return;
     if (tid < 6) {
         float s = 0.f;
-        for (int g = 0; g < (int)gridDim.x; ++g) s += sb[6 * g + tid];
+#pragma unroll
+        for (int g = 0; g < PR_BLOCKS; ++g) s += sb[g][tid];
         out[tid] = s;
-        sm[0][tid] = s;
+        tot[tid] = s;
     }
     __syncthreads();
-    if (tid == 0) f.ctrl->reduce_done = 0u;
-    if (T_cw && tid < 32) ts_pose_step_warp(T_cw, &sm[0][0], state, lr, beta1, beta2, eps);
+    if (T_cw && tid < 32) ts_pose_step_warp(T_cw, tot, state, lr, beta1, beta2, eps);
 }
 
 template <int SM, bool ATTR, bool GEOM, bool POSE>

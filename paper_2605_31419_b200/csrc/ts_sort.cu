@@ -332,69 +332,119 @@ __device__ __forceinline__ void emit_sorted(const TsFrameDev& f, uint32_t base, 
     f.skey[base + rank] = thi | a.x;
 }
 
+// One CTA per position b of the job-header array tile_order (tiles by descending list length, written by the binning
+// kernel; every tile appears once).  A LONG list (more than TS_SORT_WARP_MAX pairs) is sorted by the CTA at its own
+// position: rank sort up to 2 x threads, compare-exchange network in shared memory up to TS_SORT_SMEM, the same
+// network in global scratch above.  SHORT lists (nine in ten at the paper's tracking workloads) are sorted four to a
+// CTA by the CTA at the first position of their group of four, ONE WARP per list -- keys in the warp's slice of
+// shared memory, rank sort with the pair data in registers, no CTA barrier; the other three CTAs of a short group
+// exit at once.  Two dependent loads (header, pairs) precede every sort, whatever its kind.
+#define TS_SORT_TILES (TS_SORT_THREADS / 32)
+#define TS_SORT_WARP_MAX 64
+
 __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f, unsigned long long* __restrict__ gkeys,
                                                                     uint32_t* __restrict__ gidx) {
     __shared__ unsigned long long sk[TS_SORT_SMEM];
     __shared__ uint32_t sv[TS_SORT_SMEM];
-    const uint32_t tile = blockIdx.x, tid = threadIdx.x;
-    const uint2 range = f.tile_ranges[tile];
+    const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, b = blockIdx.x;
+    const bool leader = (b % TS_SORT_TILES) == 0;
+    const uint4 hb = __ldcg(f.tile_order + b);              // (tile, begin, end, xy)
+    uint4 hw = make_uint4(0u, 0u, 0u, 0u);
+    if (leader && b + warp < (uint32_t)f.NT) hw = __ldcg(f.tile_order + b + warp);
     // this kernel is the last reader of the project / binning counters: leave them at zero for the next frame
     if (tid == 0) {
-        f.tile_count[tile] = 0u, f.tile_cursor[tile] = 0u;
-        if (tile == 0) f.ctrl->vis_counter = 0u;
+        f.tile_count[hb.x] = 0u, f.tile_cursor[hb.x] = 0u;
+        if (b == 0) f.ctrl->vis_counter = 0u;
     }
-    const uint32_t n = range.y - range.x;
-    if (n == 0) return;
-    const unsigned long long thi = (unsigned long long)tile << 32;
-    if (n <= 2 * TS_SORT_THREADS) {
-        // rank sort, pair data kept in registers: keys are unique (the face index is part of the key), so the
-        // ranks are a permutation
-        uint4 a[2];
-        uint32_t bb[2];
+    const uint32_t nb = hb.z - hb.y;
+    if (nb > TS_SORT_WARP_MAX) {
+        // ---- a long list: the whole CTA ------------------------------------------------------------------------
+        const uint2 range = make_uint2(hb.y, hb.z);
+        const uint32_t n = nb;
+        const unsigned long long thi = (unsigned long long)hb.x << 32;
+        if (n <= 2 * TS_SORT_THREADS) {
+            // rank sort, pair data kept in registers: keys are unique (the face index is part of the key), so the
+            // ranks are a permutation
+            uint4 a[2];
+            uint32_t bb[2];
 #pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const uint32_t i = tid + k * TS_SORT_THREADS;
-            if (i < n) {
-                a[k] = f.pair_a[range.x + i], bb[k] = f.pair_b[range.x + i];
-                sk[i] = ((unsigned long long)a[k].x << 32) | a[k].y;
+            for (int k = 0; k < 2; ++k) {
+                const uint32_t i = tid + k * TS_SORT_THREADS;
+                if (i < n) {
+                    a[k] = f.pair_a[range.x + i], bb[k] = f.pair_b[range.x + i];
+                    sk[i] = ((unsigned long long)a[k].x << 32) | a[k].y;
+                }
             }
-        }
-        __syncthreads();
+            __syncthreads();
 #pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            const uint32_t i = tid + k * TS_SORT_THREADS;
-            if (i < n) {
-                const unsigned long long mine = ((unsigned long long)a[k].x << 32) | a[k].y;
-                uint32_t rank = 0;
-                for (uint32_t j = 0; j < n; ++j) rank += (sk[j] < mine) ? 1u : 0u;
-                f.sorted[range.x + rank] = make_uint4(a[k].z, a[k].y, a[k].w, bb[k]);   // (slot, face, rect_lo, rect_hi)
-                f.skey[range.x + rank] = thi | a[k].x;
+            for (int k = 0; k < 2; ++k) {
+                const uint32_t i = tid + k * TS_SORT_THREADS;
+                if (i < n) {
+                    const unsigned long long mine = ((unsigned long long)a[k].x << 32) | a[k].y;
+                    uint32_t rank = 0;
+                    for (uint32_t j = 0; j < n; ++j) rank += (sk[j] < mine) ? 1u : 0u;
+                    f.sorted[range.x + rank] = make_uint4(a[k].z, a[k].y, a[k].w, bb[k]);   // (slot, face, rect_lo, rect_hi)
+                    f.skey[range.x + rank] = thi | a[k].x;
+                }
             }
+        } else if (n <= TS_SORT_SMEM) {
+            for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
+                const uint4 a = f.pair_a[range.x + i];
+                sk[i] = ((unsigned long long)a.x << 32) | a.y;
+                sv[i] = i;
+            }
+            __syncthreads();
+            cta_sort_network(sk, sv, n);
+            for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) emit_sorted(f, range.x, i, sv[i], thi);
+        } else {
+            // oversize segment: same network in global scratch (volatile: exchanged across threads between barriers)
+            unsigned long long* gk = gkeys + range.x;
+            uint32_t* gv = gidx + range.x;
+            for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
+                const uint4 a = f.pair_a[range.x + i];
+                gk[i] = ((unsigned long long)a.x << 32) | a.y;
+                gv[i] = i;
+            }
+            __syncthreads();
+            cta_sort_network((volatile unsigned long long*)gk, (volatile uint32_t*)gv, n);
+            for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) emit_sorted(f, range.x, i, gv[i], thi);
         }
-        return;
+        if (!leader) return;
+        __syncthreads();                                    // the shared arrays are re-used below
     }
-    if (n <= TS_SORT_SMEM) {
-        for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
-            const uint4 a = f.pair_a[range.x + i];
-            sk[i] = ((unsigned long long)a.x << 32) | a.y;
-            sv[i] = i;
+    if (!leader) return;
+    // ---- the group's short lists: one warp each ------------------------------------------------------------------
+    const uint32_t n = hw.z - hw.y;
+    if (n == 0 || n > TS_SORT_WARP_MAX) return;
+    unsigned long long* wk = sk + warp * TS_SORT_WARP_MAX;
+    const unsigned long long thi = (unsigned long long)hw.x << 32;
+    uint4 a[2];
+    uint32_t bb[2];
+    unsigned long long mine[2];
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const uint32_t i = lane + 32u * k;
+        mine[k] = ~0ull;
+        if (i < n) {
+            a[k] = f.pair_a[hw.y + i], bb[k] = f.pair_b[hw.y + i];
+            mine[k] = ((unsigned long long)a[k].x << 32) | a[k].y;             // (depth key, face): unique
+            wk[i] = mine[k];
         }
-        __syncthreads();
-        cta_sort_network(sk, sv, n);
-        for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) emit_sorted(f, range.x, i, sv[i], thi);
-        return;
     }
-    // oversize segment: same network in global scratch (volatile: exchanged across threads between barriers)
-    unsigned long long* gk = gkeys + range.x;
-    uint32_t* gv = gidx + range.x;
-    for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
-        const uint4 a = f.pair_a[range.x + i];
-        gk[i] = ((unsigned long long)a.x << 32) | a.y;
-        gv[i] = i;
+    __syncwarp();
+    uint32_t r0 = 0, r1 = 0;
+    for (uint32_t j = 0; j < n; ++j) {
+        const unsigned long long kj = wk[j];
+        r0 += (kj < mine[0]) ? 1u : 0u, r1 += (kj < mine[1]) ? 1u : 0u;
     }
-    __syncthreads();
-    cta_sort_network((volatile unsigned long long*)gk, (volatile uint32_t*)gv, n);
-    for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) emit_sorted(f, range.x, i, gv[i], thi);
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        const uint32_t i = lane + 32u * k, rank = k ? r1 : r0;
+        if (i < n) {
+            f.sorted[hw.y + rank] = make_uint4(a[k].z, a[k].y, a[k].w, bb[k]);
+            f.skey[hw.y + rank] = thi | a[k].x;
+        }
+    }
 }
 
 }  // namespace
