@@ -12,6 +12,9 @@
  *    keeps no caller pointer beyond the call, with one exception: a ts_frame remembers the pose pointer given to
  *    ts_project until the next ts_project on it (the full-gradient ts_render_bwd reads the pose again), so it must
  *    stay valid and unchanged until the frame's backward pass has been enqueued.
+ *  - Devices: a ts_ctx belongs to the device given to ts_create; every export that launches work returns
+ *    TS_ERR_INVALID_ARG unless that device is the calling thread's current device (cudaSetDevice is the caller's).
+ *    Several contexts, one per device, may live in one process.
  *  - Streams: `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  All work is enqueued
  *    on it.  No export synchronises except ts_frame_status and ts_frame_view.  All exports may be captured
  *    into a CUDA graph (launch geometry never depends on device-side counts).
@@ -158,7 +161,8 @@ int32_t ts_render_map_l1(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, fl
  * ts_render_fwd_stats: as ts_render_fwd, and face_pixels[m] += number of pixels face m contributed to (caller zeroes;
  * a face is "rendered" iff its count is non-zero).  out_* may be NULL.
  * ts_face_area: proj_area[m] = |S|/2 in px^2 for every face that survived the last ts_project (other entries are
- * left untouched: zero the array first). */
+ * left untouched: zero the array first).  Requires ts_bin_sort on the frame (which publishes the visible count);
+ * TS_ERR_STATE otherwise. */
 int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
                             float* out_alpha, uint32_t* face_pixels, void* stream);
 int32_t ts_face_area(ts_ctx* ctx, ts_frame* frame, float* proj_area, void* stream);

@@ -50,6 +50,13 @@ bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pa
     return true;
 }
 
+// every launching export runs on the device of its context (ts_create): a mismatch with the current device is an
+// argument error, not a launch on the wrong GPU
+bool on_ctx_device(const ts_ctx* ctx) {
+    int cur = -1;
+    return ctx && cudaGetDevice(&cur) == cudaSuccess && cur == ctx->device;
+}
+
 }  // namespace
 
 extern "C" {
@@ -97,6 +104,7 @@ size_t ts_frame_bytes(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64
 int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_t W, int32_t H, uint64_t pair_capacity,
                       uint64_t visible_capacity, void* stream, ts_frame** out) {
     if (!out || !dev_ws) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     Layout L;
     if (visible_capacity == 0) visible_capacity = (uint64_t)(M > 0 ? M : 0);
     if (!make_layout(ctx, M, W, H, pair_capacity, visible_capacity, L)) return TS_ERR_INVALID_ARG;
@@ -162,6 +170,7 @@ int32_t ts_frame_status(ts_ctx* ctx, ts_frame* fr, uint32_t* flags, uint32_t* n_
 int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const ts_params* prm, const float* T_cw_dev,
                    ts_frame* fr, void* stream) {
     if (!ctx || !sc || !cam || !prm || !T_cw_dev || !fr || !sc->pos || !sc->opacity) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M || cam->width != fr->d.W || cam->height != fr->d.H) return TS_ERR_INVALID_ARG;
     if (sc->faces == nullptr && sc->V != 3 * sc->M) return TS_ERR_INVALID_ARG;
     if (!(prm->sigma > 0.0f) || !(prm->alpha_min >= 0.0f) || !(prm->t_min >= 0.0f) || !(prm->eps_area >= 0.0f) ||
@@ -187,6 +196,7 @@ int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const 
 
 int32_t ts_bin_sort(ts_ctx* ctx, ts_frame* fr, void* stream) {
     if (!ctx || !fr) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (!fr->have_project) return TS_ERR_STATE;
     if (!fr->counters_dirty) return TS_ERR_STATE;          // one ts_bin_sort per ts_project
     const int32_t s = ts_launch_sort(ctx, fr, (cudaStream_t)stream);
@@ -198,6 +208,7 @@ int32_t ts_bin_sort(ts_ctx* ctx, ts_frame* fr, void* stream) {
 int32_t ts_render_fwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
                       float* out_alpha, void* stream) {
     if (!ctx || !sc || !fr || !sc->color) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, nullptr, nullptr, 0.f, nullptr, nullptr,
@@ -210,6 +221,7 @@ int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* o
                          const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
                          void* stream) {
     if (!ctx || !sc || !fr || !sc->color || !Chat || !Dhat || !gC || !gD) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev,
@@ -221,6 +233,7 @@ int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* o
 int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
                             float* out_alpha, uint32_t* face_pixels, void* stream) {
     if (!ctx || !sc || !fr || !sc->color || !face_pixels) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     const int32_t s = ts_launch_render_fwd(ctx, fr, sc, out_color, out_depth, out_alpha, nullptr, nullptr, 0.f, nullptr, nullptr,
@@ -232,6 +245,7 @@ int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float
 int32_t ts_render_fwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
                              float* out_alpha, float* out_normal, void* stream) {
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !out_normal) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     const int32_t s = ts_launch_render_fwd_normal(ctx, fr, sc, out_color, out_depth, out_alpha, out_normal, (cudaStream_t)stream);
@@ -244,6 +258,7 @@ int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, cons
                              const float* dL_dalpha, const float* dL_dnormal, float* grad_pos, float* grad_color,
                              float* grad_opacity, uint32_t grad_mask, void* stream) {
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !dL_dnormal) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if ((grad_mask & TS_GRAD_POS) && !grad_pos) return TS_ERR_INVALID_ARG;
     if ((grad_mask & TS_GRAD_COLOR) && !grad_color) return TS_ERR_INVALID_ARG;
@@ -256,7 +271,8 @@ int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, cons
 
 int32_t ts_face_area(ts_ctx* ctx, ts_frame* fr, float* proj_area, void* stream) {
     if (!ctx || !fr || !proj_area) return TS_ERR_INVALID_ARG;
-    if (!fr->have_project) return TS_ERR_STATE;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
+    if (!fr->have_sort) return TS_ERR_STATE;              // the visible count is published by ts_bin_sort
     return ts_launch_face_area(ctx, fr, proj_area, (cudaStream_t)stream);
 }
 
@@ -264,6 +280,7 @@ int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float*
                            const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
                            void* stream) {
     if (!ctx || !sc || !fr || !sc->color || !Chat || !Dhat) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     fr->have_fwd = 0;                                       // n_contrib / T_last are not written: no ts_render_bwd after this
@@ -275,6 +292,7 @@ int32_t ts_render_map_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* o
                          const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
                          float* grad_pos, float* grad_color, float* grad_opacity, uint32_t grad_mask, void* stream) {
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !Chat || !Dhat) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if ((grad_mask & TS_GRAD_POS) && !grad_pos) return TS_ERR_INVALID_ARG;
     if ((grad_mask & TS_GRAD_COLOR) && !grad_color) return TS_ERR_INVALID_ARG;
@@ -291,6 +309,7 @@ int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float
                       const float* dL_dalpha, float* grad_pos, float* grad_color, float* grad_opacity,
                       uint32_t grad_mask, void* stream) {
     if (!ctx || !sc || !fr || !sc->color || !sc->pos) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if ((grad_mask & TS_GRAD_POS) && !grad_pos) return TS_ERR_INVALID_ARG;
     if ((grad_mask & TS_GRAD_COLOR) && !grad_color) return TS_ERR_INVALID_ARG;
@@ -305,6 +324,7 @@ int32_t ts_render_bwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const
                             const float* dL_dalpha, float* grad_pos, float* grad_color, float* grad_opacity,
                             uint32_t grad_mask, float* face_grad2d, uint32_t* face_views, void* stream) {
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !face_grad2d) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if ((grad_mask & TS_GRAD_POS) && !grad_pos) return TS_ERR_INVALID_ARG;
     if ((grad_mask & TS_GRAD_COLOR) && !grad_color) return TS_ERR_INVALID_ARG;
@@ -318,12 +338,14 @@ int32_t ts_render_bwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const
 
 int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, void* stream) {
     if (!ctx || !fr || !dL_dtau_dev) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, nullptr, nullptr, nullptr, 0.f, 0.f, 0.f, (cudaStream_t)stream);
 }
 
 int32_t ts_pose_reduce_step(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, float* T_cw_dev, float* state_dev,
                             const float* lr6, float beta1, float beta2, float eps, void* stream) {
     if (!ctx || !fr || !dL_dtau_dev || !T_cw_dev || !state_dev || !lr6) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, T_cw_dev, state_dev, lr6, beta1, beta2, eps, (cudaStream_t)stream);
 }
 

@@ -17,6 +17,21 @@ def ctx():
     c.close()
 
 
+@pytest.fixture(scope="module")
+def ctx_log():
+    """A second context on the same device whose ts_render_track_l1 runs the hit-log kernel (TS_TRACK_LOG is read by
+    ts_create)."""
+    import os
+    from paper_2605_31419_b200 import ts
+    os.environ["TS_TRACK_LOG"] = "1"
+    try:
+        c = ts.Context(0)
+    finally:
+        del os.environ["TS_TRACK_LOG"]
+    yield c
+    c.close()
+
+
 def test_empty_scene_all_culled(ctx, oracle_mod):
     """Every face behind the camera: nothing visible, zero pairs, zero images, zero gradients."""
     from gpu_util import GpuView
@@ -163,7 +178,7 @@ def test_determinism(ctx, oracle_mod):
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4])
-def test_full_size_configs(ctx, oracle_mod, cfg):
+def test_full_size_configs(ctx, ctx_log, oracle_mod, cfg):
     """BASELINE.json sizes (100k / 500k faces tracking frames; one view of the 1M-face mapping step; 2M faces stress)
     through the tiled oracle, in the launch configuration bench.py times."""
     from test_gpu_parity import both, check_backward, check_forward, check_project_and_sort
@@ -174,6 +189,45 @@ def test_full_size_configs(ctx, oracle_mod, cfg):
     f, ok = check_forward(o, g)
     masks = [ts.GRAD_POSE] if cfg in (1, 2) else [ts.GRAD_ALL]
     check_backward(o, g, ok, 40 + cfg, masks)
+    # ... and the fused launches bench.py actually times, at full size, against the oracle: ts_render_track_l1 (tracking
+    # frames) / ts_render_map_l1 (mapping and stress frames).  The oracle's backward pass is fed the kernel's own loss
+    # cotangent images (which must agree with the oracle's own on >= 99.9 % of the pixels), gradients to 1e-3.
+    from gpu_util import assert_grad_close, dev
+    from test_gpu_parity import fused_cotangents_agree
+    tgt_pos = sc.pos_target if sc.pos_target is not None else sc.pos
+    tgt_col = sc.color_target if sc.color_target is not None else sc.color
+    tgt = oracle_mod.Oracle(tgt_pos, tgt_col, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+    Chat, Dhat, lam = dev(tgt.color), dev(tgt.depth), sc.params.lambda_dep
+    Lo, gCo, gDo = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, lam)
+    C2, D2, A2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.empty_like(g.A)
+    gC2, gD2, L2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
+    tau = torch.zeros(6, device="cuda")
+    if cfg in (1, 2):
+        for cx in (ctx, ctx_log):
+            ts.ts_render_track_l1(cx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, lam, gC2, gD2, L2)
+            ts.ts_pose_jacobian_reduce(cx, g.frame, tau)
+            torch.cuda.synchronize()
+            assert torch.equal(C2, g.C) and torch.equal(D2, g.D) and torch.equal(A2, g.A)
+            gCn, gDn = gC2.cpu().numpy(), gD2.cpu().numpy()
+            fused_cotangents_agree(gCn, gDn, gCo, gDo, ok)
+            ref = o.backward(gCn, gDn, None, want=("pose",))
+            t = tau.cpu().numpy()
+            assert np.abs(t - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max(), (t, ref.dL_dtau)
+    else:
+        V = sc.pos.shape[0]
+        gp, gc, go = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+        ts.ts_render_map_l1(ctx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, lam, gC2, gD2, L2, gp, gc, go, ts.GRAD_ALL)
+        ts.ts_pose_jacobian_reduce(ctx, g.frame, tau)
+        torch.cuda.synchronize()
+        assert torch.equal(C2, g.C) and torch.equal(D2, g.D) and torch.equal(A2, g.A)
+        gCn, gDn = gC2.cpu().numpy(), gD2.cpu().numpy()
+        fused_cotangents_agree(gCn, gDn, gCo, gDo, ok)
+        ref = o.backward(gCn, gDn, None)
+        assert_grad_close("grad_pos", gp.cpu().numpy(), ref.grad_pos)
+        assert_grad_close("grad_color", gc.cpu().numpy(), ref.grad_color)
+        assert_grad_close("grad_opacity", go.cpu().numpy(), ref.grad_opacity)
+        t = tau.cpu().numpy()
+        assert np.abs(t - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max(), (t, ref.dL_dtau)
     g.close()
 
 
@@ -265,3 +319,88 @@ def test_mapping_loop_descends(ctx, oracle_mod):
     assert ts.ts_frame_status(ctx, frame)[0] == 0
     assert history[-1] < 0.7 * history[0], history
     frame.release()
+
+
+def test_tile_list_longer_than_the_shared_memory_sort(ctx, oracle_mod):
+    """3 000 nearly coincident faces stacked in ONE tile (t_min = alpha_min = 0: every one of them is walked): the tile's
+    list is longer than TS_SORT_SMEM = 2048, so its sort runs the compare-exchange network in global scratch.  Sorted
+    keys / values / ranges bit-exact, images and gradients to tolerance."""
+    from test_gpu_parity import both, check_backward, check_forward, check_project_and_sort
+    from paper_2605_31419_b200 import ts
+    rng = np.random.default_rng(21)
+    M = 3000
+    sc = scenes.config0(n_faces=M)
+    base = np.array([[-0.12, -0.10, 0.0], [0.14, -0.08, 0.0], [0.0, 0.13, 0.0]])        # ~6 px triangle at the image centre
+    z = rng.uniform(2.0, 4.0, M)
+    pos = (base[None] * (z[:, None, None] / 3.0) + rng.normal(0, 0.004, (M, 3, 3)))
+    pos[:, :, 2] += z[:, None]
+    sc.pos = pos.reshape(-1, 3).astype(np.float32)
+    sc.opacity = rng.uniform(0.002, 0.01, 3 * M).astype(np.float32)                      # T stays far above zero
+    sc.params = scenes.Params(sigma=1.0, alpha_min=0.0, t_min=0.0)
+    o, g = both(ctx, oracle_mod, sc)
+    check_project_and_sort(o, g, sc.M)
+    ranges = g.view(ts.VIEW_TILE_RANGES).reshape(-1, 2).astype(np.int64)
+    assert (ranges[:, 1] - ranges[:, 0]).max() > 2048
+    f, ok = check_forward(o, g)
+    assert f.n_contrib.max() > 2048
+    check_backward(o, g, ok, 9, [ts.GRAD_ALL, ts.GRAD_POSE])
+    g.close()
+
+
+def test_image_with_more_than_4096_tiles(ctx, oracle_mod):
+    """1920 x 1088 (120 x 68 = 8 160 tiles > TS_SCAN_LOCAL_MAX): the tile scan runs as its own kernel and the binning pass
+    reads offsets from global memory.  Integer outputs bit-exact, images and pose gradient to tolerance."""
+    from test_gpu_parity import both, check_backward, check_forward, check_project_and_sort
+    from paper_2605_31419_b200 import ts
+    sc = scenes.config2(n_faces=50_000)
+    sc.cam = scenes.Camera(1920, 1088, 960.0, 960.0, 959.5, 543.5)
+    o, g = both(ctx, oracle_mod, sc)
+    check_project_and_sort(o, g, sc.M)
+    assert g.view(ts.VIEW_TILE_RANGES).size // 2 == 120 * 68
+    f, ok = check_forward(o, g)
+    assert f.alpha.max() > 0.5
+    check_backward(o, g, ok, 10, [ts.GRAD_ALL])
+    g.close()
+
+
+def test_two_contexts_in_one_process(oracle_mod):
+    """Two ts_ctx alive at once (the opt-in above 48 KB of dynamic shared memory is set per launch, not cached per
+    process): both render the same frame, identically; a context refuses to launch when another device is current."""
+    from gpu_util import GpuView
+    from paper_2605_31419_b200 import ts
+    sc = scenes.config1(n_faces=30_000)
+    ca, cb = ts.Context(0), ts.Context(0)
+    outs = []
+    for c in (ca, cb, ca):
+        g = GpuView(c, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
+        C, D, A = g.forward()
+        gp, gc, go, tau = g.backward(np.ones_like(C), np.ones_like(D), None, ts.GRAD_POSE)
+        outs.append((C, D, A, tau))
+        g.close()
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a, b)
+    for a, b in zip(outs[0], outs[2]):
+        assert np.array_equal(a, b)
+    if torch.cuda.device_count() > 1:
+        g = GpuView(ca, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
+        with torch.cuda.device(1), pytest.raises(ts.TsError):
+            g.project()
+        g.close()
+    ca.close(), cb.close()
+
+
+def test_face_area_needs_the_sort(ctx, oracle_mod):
+    """ts_face_area reads the visible count ts_bin_sort publishes: TS_ERR_STATE between ts_project and ts_bin_sort."""
+    from gpu_util import GpuView
+    from paper_2605_31419_b200 import ts
+    sc = scenes.config0()
+    g = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
+    area = torch.zeros(sc.M, device="cuda")
+    g.project()
+    with pytest.raises(ts.TsError):
+        ts.ts_face_area(ctx, g.frame, area)
+    g.sort()
+    ts.ts_face_area(ctx, g.frame, area)
+    torch.cuda.synchronize()
+    assert (area > 0).sum().item() == g.status()[1]
+    g.close()

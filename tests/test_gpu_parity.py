@@ -18,6 +18,21 @@ def ctx():
     c.close()
 
 
+@pytest.fixture(scope="module")
+def ctx_log():
+    """A second context on the same device whose ts_render_track_l1 runs the hit-log kernel (TS_TRACK_LOG is read by
+    ts_create)."""
+    import os
+    from paper_2605_31419_b200 import ts
+    os.environ["TS_TRACK_LOG"] = "1"
+    try:
+        c = ts.Context(0)
+    finally:
+        del os.environ["TS_TRACK_LOG"]
+    yield c
+    c.close()
+
+
 def small_cfg(i):
     """Sizes the oracle finishes in seconds that still span many tiles, several batches and ragged tails."""
     if i == 0:
@@ -35,7 +50,7 @@ def both(ctx, oracle_mod, sc, view=0, params=None, faces=None, T=None, **kw):
     from gpu_util import GpuView
     prm = params or sc.params
     T = sc.T_start[view] if T is None else T
-    o = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, faces, T, sc.cam, prm, "f32", amb_tol=5e-3)
+    o = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, faces, T, sc.cam, prm, "f32", amb_tol=5e-4)
     g = GpuView(ctx, sc.pos, sc.color, sc.opacity, faces, T, sc.cam, prm, **kw)
     return o, g
 
@@ -72,12 +87,19 @@ def test_project_and_sort_bit_exact(ctx, oracle_mod, cfg):
 
 def check_forward(o, g):
     from gpu_util import assert_images_close
+    from paper_2605_31419_b200 import ts
     f = o.forward("tiled")
     C, D, A = g.forward()
     ok = f.ambig == 0
-    # pixels where a hit's alpha is within 0.5 % of alpha_min (or T of t_min): the keep/skip decision may differ
-    # in the last float32 bit between the two sides; they are excluded, and must stay rare
-    assert (~ok).sum() <= 2 + 5e-3 * ok.size, "too many ambiguous pixels"
+    # pixels where a hit's alpha is within 0.05 % of alpha_min (or T of t_min): the keep/skip decision may differ
+    # in the last float32 bit between the two sides (reading N8); they are excluded, and must stay rare
+    # (measured: 0 - 22 pixels of 816 000 on the five configs)
+    n_amb = int((~ok).sum())
+    print(f"ambiguous pixels: {n_amb} of {ok.size}")
+    assert n_amb <= 2 + 5e-4 * ok.size, "too many ambiguous pixels"
+    # the walk's integer output: list position of the last contributing entry, equal on every unambiguous pixel
+    nc = g.view(ts.VIEW_N_CONTRIB).reshape(ok.shape)
+    assert np.array_equal(nc[ok], f.n_contrib[ok]), f"n_contrib differs on {(nc[ok] != f.n_contrib[ok]).sum()} pixels"
     assert_images_close("color", C, f.color, ok[None])
     assert_images_close("alpha", A, f.alpha, ok)
     assert_images_close("depth", D, f.depth, ok, scale=float(np.abs(f.depth).max()))
@@ -228,16 +250,31 @@ def test_render_fwd_l1_equals_separate_calls(ctx, oracle_mod):
     g.close()
 
 
-@pytest.mark.parametrize("cfg", [0, 2, 4])
-def test_render_track_l1_equals_separate_calls(ctx, oracle_mod, cfg):
-    """ts_render_track_l1 (a3 + a4 + a5 pose-only fused) == ts_render_fwd_l1 + ts_render_bwd(POSE), bit for bit, and
-    its pose gradient matches the oracle's."""
+def fused_cotangents_agree(gC, gD, gCo, gDo, ok):
+    """The L1 sign images of the CUDA path (from its own render) and of the oracle (from its own) may differ only where
+    abs(C - Chat) is within float rounding: they must agree on >= 99.9 % of the unambiguous pixels."""
+    same = (gC == gCo).all(axis=0) & (gD == gDo)
+    frac = same[ok].mean() if ok.any() else 1.0
+    print(f"L1 cotangent images agree on {100 * frac:.4f} % of the unambiguous pixels")
+    assert frac >= 0.999
+    return same
+
+
+@pytest.mark.parametrize("kernel", ["visit", "log"])
+@pytest.mark.parametrize("cfg", [0, 1, 2, 4])
+def test_render_track_l1_equals_separate_calls(ctx, ctx_log, oracle_mod, cfg, kernel):
+    """ts_render_track_l1 (a3 + a4 + a5 pose-only fused; both of its kernels: the visit form and the hit-log form) ==
+    ts_render_fwd_l1 + ts_render_bwd(POSE): images and loss cotangents bit for bit, the pose gradient bit for bit (visit
+    form, same arithmetic) or to rounding (hit log: the chain and the geometry sum in another order); and its pose
+    gradient matches the oracle's, fed with the same cotangent images, to 1e-3."""
     from gpu_util import dev
     from paper_2605_31419_b200 import ts
     sc = small_cfg(cfg)
     o, g = both(ctx, oracle_mod, sc)
     f, ok = check_forward(o, g)
-    tgt = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+    # a target that differs from the render: the ground-truth pose where the config has a start pose, else jittered vertices
+    tgt_pos = sc.pos_target if sc.pos_target is not None else sc.pos
+    tgt = oracle_mod.Oracle(tgt_pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
     Chat, Dhat = dev(tgt.color), dev(tgt.depth)
     lam = sc.params.lambda_dep
     gC, gD, L1 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
@@ -245,23 +282,30 @@ def test_render_track_l1_equals_separate_calls(ctx, oracle_mod, cfg):
     ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, None, None, None, ts.GRAD_POSE)
     tau1 = torch.zeros(6, device="cuda")
     ts.ts_pose_jacobian_reduce(ctx, g.frame, tau1)
+    cx = ctx if kernel == "visit" else ctx_log
     C2, D2, A2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.empty_like(g.A)
     gC2, gD2, L2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
-    ts.ts_render_track_l1(ctx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, lam, gC2, gD2, L2)
+    ts.ts_render_track_l1(cx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, lam, gC2, gD2, L2)
     tau2 = torch.zeros(6, device="cuda")
-    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau2)
+    ts.ts_pose_jacobian_reduce(cx, g.frame, tau2)
     torch.cuda.synchronize()
     assert torch.equal(C2, g.C) and torch.equal(D2, g.D) and torch.equal(A2, g.A)
     assert torch.equal(gC, gC2) and torch.equal(gD, gD2)
-    assert torch.equal(tau1, tau2) and tau1.abs().max().item() > 0
+    assert tau1.abs().max().item() > 0
+    if kernel == "visit":
+        assert torch.equal(tau1, tau2)
+    else:
+        assert (tau1 - tau2).abs().max().item() <= 1e-5 * tau1.abs().max().item()
     assert abs(L1.item() - L2.item()) <= 1e-5 * abs(L1.item())
-    # against the oracle: same loss cotangents on the unambiguous pixels, pose gradient to 1e-3
+    # against the oracle: its own loss cotangents agree with the kernel's on (nearly) every pixel, and its backward pass
+    # of the kernel's cotangent images gives the kernel's pose gradient to 1e-3
     Lo, gCo, gDo = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, lam)
-    same = (gC.cpu().numpy() == gCo).all(axis=0) & (gD.cpu().numpy() == gDo) & ok
-    if same.mean() > 0.999:       # sign images agree (they can differ where |C - Chat| is within float rounding)
-        ref = o.backward(gC.cpu().numpy(), gD.cpu().numpy(), None, want=("pose",))
-        t2 = tau2.cpu().numpy()
-        assert np.abs(t2 - ref.dL_dtau).max() <= 2e-3 * np.abs(ref.dL_dtau).max(), (t2, ref.dL_dtau)
+    gCn, gDn = gC2.cpu().numpy(), gD2.cpu().numpy()
+    fused_cotangents_agree(gCn, gDn, gCo, gDo, ok)
+    assert abs(L2.item() - Lo) <= 1e-4 * abs(Lo)
+    ref = o.backward(gCn, gDn, None, want=("pose",))
+    t2 = tau2.cpu().numpy()
+    assert np.abs(t2 - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max(), (t2, ref.dL_dtau)
     with pytest.raises(ts.TsError):
         ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, None, None, None, ts.GRAD_POSE)   # no walk state after track
     g.close()
@@ -279,7 +323,7 @@ def test_mapping_step_accumulates_over_views(ctx, oracle_mod):
     rng = np.random.default_rng(33)
     for view in range(len(sc.T_start)):
         T = sc.T_start[view]
-        o = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, None, T, sc.cam, sc.params, "f32", amb_tol=5e-3)
+        o = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, None, T, sc.cam, sc.params, "f32", amb_tol=5e-4)
         g = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, T, sc.cam, sc.params)
         f, ok = check_forward(o, g)
         H, W = ok.shape
@@ -385,7 +429,15 @@ def test_tracking_gradient_with_full_photometric_loss(ctx, oracle_mod):
     ts.ts_pose_jacobian_reduce(ctx, g.frame, tau)
     torch.cuda.synchronize()
     t = tau.cpu().numpy()
-    # the L1 sign image can flip where |C - Chat| is within float rounding between the two forwards: a looser bound
+    # the two cotangent images: equal L1 sign part on (nearly) every pixel (it can flip where |C - Chat| is within
+    # float rounding between the two forwards), D-SSIM part to the gradient tolerance
+    gCn, gDn = gCd.cpu().numpy(), gDd.cpu().numpy()
+    close = (np.abs(gCn - gC_o) <= 1e-3 * np.abs(gC_o).max()).all(axis=0) & (gDn == (gD * ok))
+    assert close[ok].mean() >= 0.999, close[ok].mean()
+    # the backward pass proper: both sides get the SAME cotangent images (the CUDA chain's), gradient to 1e-3
+    ref_same = o.backward(gCn, gDn, None, want=("pose",))
+    assert np.abs(t - ref_same.dL_dtau).max() <= 1e-3 * np.abs(ref_same.dL_dtau).max(), (t, ref_same.dL_dtau)
+    # and the whole chain end to end (each side on its own cotangents) stays within the few flipped pixels
     assert np.abs(t - ref.dL_dtau).max() <= 5e-3 * np.abs(ref.dL_dtau).max(), (t, ref.dL_dtau)
     g.close()
 
@@ -449,7 +501,7 @@ def test_needle_faces(ctx, oracle_mod):
     from gpu_util import GpuView, assert_grad_close
     from paper_2605_31419_b200 import ts
     sc, pos, col, opa, faces = needle_scene()
-    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, "f32", amb_tol=5e-3)
+    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, "f32", amb_tol=5e-4)
     g = GpuView(ctx, pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, pair_capacity=o.bin_sort().P + 1024)
     f, ok = check_forward(o, g)
     assert (f.alpha > 0.5).mean() > 0.5
@@ -461,13 +513,20 @@ def test_needle_faces(ctx, oracle_mod):
     gp, gc, go, tau = g.backward(gC, gD, None, ts.GRAD_ALL)
     assert_grad_close("grad_color", gc, ref.grad_color)
     assert_grad_close("grad_opacity", go, ref.grad_opacity)
-    # vertex positions of needles: d x / d q grows like 1/r, and so does the rounding of both sides' float32 geometry
-    # terms; relative L2 still to 1e-3, single entries to 3e-3 of the largest
+    # Vertex positions and pose of needles: d x / d q grows like 1/r, and so does the rounding of ANY float32 evaluation
+    # of the geometry terms.  The bound is therefore taken from the arithmetic itself (SURVEY.md pin P14: the float32
+    # oracle against the float64 oracle on the same inputs sets the achievable floor): relative L2 to 1e-3 as everywhere,
+    # single entries to max(1e-3, 2 x that floor).  (measured floor: ~1.5e-3 for grad_pos, ~2e-3 for the pose, whose
+    # components are sums of 1e6-sized terms of both signs)
+    o64 = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, "f64")
+    ref64 = o64.backward(gC.astype(np.float64), gD.astype(np.float64), None)
+    floor_pos = np.abs(ref.grad_pos - ref64.grad_pos).max() / np.abs(ref64.grad_pos).max()
+    floor_tau = np.abs(ref.dL_dtau - ref64.dL_dtau).max() / np.abs(ref64.dL_dtau).max()
+    print(f"needles: float32-vs-float64 oracle floor grad_pos {floor_pos:.2e}, pose {floor_tau:.2e}")
     d = np.abs(gp.astype(np.float64) - ref.grad_pos)
     assert np.linalg.norm(d) <= 1e-3 * np.linalg.norm(ref.grad_pos)
-    assert d.max() <= 3e-3 * np.abs(ref.grad_pos).max()
-    # the pose gradient of this scene is a sum of 1e6-sized terms of both signs: 5e-3 of its largest component
-    assert np.abs(tau - ref.dL_dtau).max() <= 5e-3 * np.abs(ref.dL_dtau).max(), (tau, ref.dL_dtau)
+    assert d.max() <= max(1e-3, 2 * floor_pos) * np.abs(ref.grad_pos).max()
+    assert np.abs(tau - ref.dL_dtau).max() <= max(1e-3, 2 * floor_tau) * np.abs(ref.dL_dtau).max(), (tau, ref.dL_dtau)
     g.close()
 
 
@@ -483,7 +542,7 @@ def test_normal_map_forward_and_backward(ctx, oracle_mod, cfg):
     else:
         sc = small_cfg(cfg)
         pos, col, opa, faces = sc.pos, sc.color, sc.opacity, None
-    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, "f32", amb_tol=5e-3)
+    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params, "f32", amb_tol=5e-4)
     from gpu_util import GpuView
     g = GpuView(ctx, pos, col, opa, faces, sc.T_start[0], sc.cam, sc.params)
     f, ok = check_forward(o, g)
@@ -601,10 +660,16 @@ def test_mapping_objective_gradient(ctx, oracle_mod):
     ts.ts_equi_loss_grad(ctx, g.scene, lam_equi, gp, None)
     torch.cuda.synchronize()
     assert abs(float(loss.item()) - Ln) <= 1e-4 * abs(Ln) + 1e-7
-    # (the L1 sign image can flip where |C - Chat| is within float rounding between the two forwards: looser bound)
-    assert_grad_close("grad_pos", gp.cpu().numpy(), ref_pos, tol=5e-3)
-    assert_grad_close("grad_color", gc.cpu().numpy(), r1.grad_color, tol=5e-3)
-    assert_grad_close("grad_opacity", go.cpu().numpy(), ref_opa, tol=5e-3)
+    # the backward pass proper: both sides get the SAME cotangent images (the CUDA chain's; its L1 sign image can differ
+    # from the oracle's where |C - Chat| is within float rounding between the two forwards), gradients to 1e-3
+    s1 = o.backward(gCd.cpu().numpy(), gDd.cpu().numpy(), None)
+    s2 = o.normal_backward(gNd.cpu().numpy())
+    assert_grad_close("grad_pos", gp.cpu().numpy(), s1.grad_pos + s2.grad_pos + gE)
+    assert_grad_close("grad_color", gc.cpu().numpy(), s1.grad_color)
+    assert_grad_close("grad_opacity", go.cpu().numpy(), s1.grad_opacity + s2.grad_opacity)
+    # and the whole chain end to end (each side on its own cotangents) stays within the few flipped pixels
+    assert np.linalg.norm(gp.cpu().numpy() - ref_pos) <= 5e-3 * np.linalg.norm(ref_pos)
+    assert np.linalg.norm(go.cpu().numpy() - ref_opa) <= 5e-3 * np.linalg.norm(ref_opa)
     # and the normal term alone, whose cotangent does not depend on a sign image, to the gradient tolerance
     gp2, go2 = torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
     ts.ts_render_bwd_normal(ctx, g.scene, g.frame, None, None, None, gNd, gp2, None, go2, ts.GRAD_POS | ts.GRAD_OPACITY)
@@ -626,7 +691,7 @@ def test_min_opacity_variant(ctx, oracle_mod, indexed):
         sc = small_cfg(2)
         pos, col, opa, faces = sc.pos, sc.color, sc.opacity, None
     prm = scenes.Params(sigma=sc.params.sigma, alpha_min=sc.params.alpha_min, t_min=sc.params.t_min, min_opacity=True)
-    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, prm, "f32", amb_tol=5e-3)
+    o = oracle_mod.Oracle(pos, col, opa, faces, sc.T_start[0], sc.cam, prm, "f32", amb_tol=5e-4)
     g = GpuView(ctx, pos, col, opa, faces, sc.T_start[0], sc.cam, prm)
     f, ok = check_forward(o, g)
     ref = check_backward(o, g, ok, 91, [ts.GRAD_ALL, ts.GRAD_POSE])
