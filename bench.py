@@ -2,16 +2,22 @@
 """bench.py -- fwd+bwd render throughput of the triangle-splatting rasteriser hot path (BASELINE.json metric:
 "fwd+bwd render Mpix/s @1200x680, 500k tris; tracking iters/s; % of roofline").
 
-A step = ONE tracking iteration on BASELINE.json configs[2] (Replica-shaped, 1200x680, 500k faces, seed 2):
-ts_project -> ts_bin_sort -> ts_render_track_l1 (= ts_render_fwd + ts_l1_loss_grad + ts_render_bwd(pose-only) in one
-launch; C, D, A and the cotangent images are still written) ->
-ts_pose_reduce_step (= ts_pose_jacobian_reduce + ts_pose_step in one launch), i.e. every row a1..a8 of DESIGN.md section 2, on synthetic data.
-L2 is flushed between timed steps (the 18 MB map would otherwise stay L2-resident across iterations); the extra
-"tracking_iters_per_s" figure is the 100-iteration block of one frame WITHOUT flushes (the real tracking loop).
+--config 2 (default; BASELINE.json configs[2], the workload the metric is quoted on) and --config 1: a step = ONE
+tracking iteration, every row a1..a8 of SURVEY.md section 8(a): ts_project -> ts_bin_sort -> ts_render_track_l1
+(= ts_render_fwd + ts_l1_loss_grad + ts_render_bwd(pose-only) in one launch; C, D, A and the cotangent images are still
+written) -> ts_pose_reduce_step (= ts_pose_jacobian_reduce + ts_pose_step in one launch), one CUDA graph.
+--config 3: a step = ONE mapping step: the 8 keyframes of the window, each ts_project -> ts_bin_sort -> ts_render_map_l1
+(forward + L1 + full-gradient backward + projection backward), gradients wrt all positions, colours and opacities
+accumulated over the views.  --config 4: one stress view, gradients wrt everything and the pose.
+L2 is flushed between timed steps (256 MiB write).  With --gpus N the script starts N ranks itself (torchrun, one per
+GPU): tracking = independent replicas (weak scaling, no collective); mapping = the views dealt to the ranks, the map
+replicated, ONE all-reduce of the gradient buffer per step (strong scaling).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1|2|3|4]
 """
 import argparse
+import glob
+import hashlib
 import json
 import os
 import subprocess
@@ -25,14 +31,15 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
 FP32_LANES_PER_SM = 128
+METRIC = "fwd+bwd render Mpix/s"
 
 
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         d = json.load(open(p))
-        return {"hbm_gbs": d["hbm_gbs"], "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "src": "measured"}
-    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+        return {"hbm_gbs": d["hbm_gbs"], "sm_max_mhz": d.get("sm_max_mhz", 1965.0), "src": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback (B200_PROFILING.md)"}
 
 
 class ClockSampler:
@@ -68,29 +75,65 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
-def algorithmic_work(cnt, HW, NT, M, p_sort, mode="pose"):
-    """algorithmic bytes / FP32 flops per step from the measured counters, per bench stage
-    (render_fwd = a3 + a4 fused: + 16 B/px of target read and 16 B/px of cotangents written)."""
+def algorithmic_work(cnt, HW, NT, M, p_sort, mode="pose", indexed=False):
+    """SURVEY.md section 8(d), "Algorithmic bytes and flops", verbatim, from the measured counters of ONE view.
+    mode "pose": pose-only backward (tracking); "full": all per-vertex gradients (+ a6)."""
     nv, P, nr, nh = cnt["n_visible"], cnt["n_pairs"], cnt["n_rect"], cnt["n_hit"]
-    B = {"project": 36 * M + 4 * nv + 48 * nv,
-         "bin_sort": 12 * nv + P * (12 + 8 + 24 * p_sort + 4) + 8 * NT,
-         "render_fwd": 84 * nv + 24 * HW + 32 * HW,
-         "render_bwd": 84 * nv + 28 * HW + (24 * NT if mode == "pose" else 168 * nv) + (0 if mode == "pose" else 144 * nv),
-         "pose_reduce": 24 * NT}
-    F = {"project": 130 * M, "bin_sort": 0, "render_fwd": 100 * P + 15 * nr + 40 * nh + 8 * HW,
-         "render_bwd": 100 * P + 15 * nr + (170 if mode == "pose" else 190) * nh + 60 * nv, "pose_reduce": 60 * nv}
-    B["render_track"] = B["render_fwd"] + B["render_bwd"]       # a3 + a4 + a5 in one launch: same rows, same work
-    F["render_track"] = F["render_fwd"] + F["render_bwd"]
+    full = mode == "full"
+    B = {"a1_project": 36 * M + (12 * M if indexed else 0) + 4 * M + 48 * nv,
+         "a2_bin_sort": 4 * M + 12 * nv + P * (12 + 8 + 24 * p_sort + 4) + 8 * NT,
+         "a3_forward": 84 * nv + 24 * HW,
+         "a4_loss": 36 * HW,
+         "a5_backward": 84 * nv + 28 * HW + (168 * nv if full else 24 * NT),
+         "a6_proj_bwd": 144 * nv if full else 0,
+         "a7_pose_reduce": 24 * NT}
+    F = {"a1_project": 130 * M, "a2_bin_sort": 0, "a3_forward": 100 * P + 15 * nr + 40 * nh, "a4_loss": 0,
+         "a5_backward": 100 * P + 15 * nr + (190 if full else 170) * nh, "a6_proj_bwd": 60 * nv if full else 0,
+         "a7_pose_reduce": 60 * nv}
     return B, F
 
 
-STEP_ROWS = ("project", "bin_sort", "render_fwd", "render_bwd", "pose_reduce")   # every row once
+# rows of SURVEY.md section 8(a) that each API call of the timed step covers
+STAGE_ROWS = {"project": ("a1_project",), "bin_sort": ("a2_bin_sort",),
+              "render_track": ("a3_forward", "a4_loss", "a5_backward"), "render_map": ("a3_forward", "a4_loss", "a5_backward", "a6_proj_bwd"),
+              "pose_reduce": ("a7_pose_reduce",), "render_fwd": ("a3_forward", "a4_loss"), "render_bwd": ("a5_backward",)}
 
 
-def load_traffic():
-    """dram bytes per launch of each stage's kernels from the committed ncu --set full capture (profiles/)."""
-    p = os.path.join(ROOT, "profiles", "r01_traffic.json")
-    return json.load(open(p)) if os.path.exists(p) else {}
+def src_sha16():
+    """Hash of the CUDA sources: the ncu traffic figures under profiles/ are stamped with it."""
+    h = hashlib.sha256()
+    for p in sorted(glob.glob(os.path.join(ROOT, "paper_2605_31419_b200", "csrc", "*.cu*"))):
+        h.update(os.path.basename(p).encode())
+        h.update(open(p, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def load_traffic(kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of a stage's kernels from the committed ncu --set full
+    capture (profiles/r02_traffic.json); null when the sources changed since that capture."""
+    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    if not os.path.exists(p):
+        return None, "no capture"
+    d = json.load(open(p))
+    if d.get("src_sha16") != src_sha16():
+        return None, f"stale: captured at sources {d.get('src_sha16')}, now {src_sha16()}"
+    return d.get("kernels", {}).get(kernel), f"ncu --set full, sources {d.get('src_sha16')}"
+
+
+def measure_fp32_peak(ts, ctx, torch, stream):
+    """Dependent-free FMA loop (ts_fp32_probe), timed with events: measured FP32 peak in TFLOP/s."""
+    scratch = torch.zeros(1, device="cuda")
+    best = 0.0
+    with torch.cuda.stream(stream):
+        ts.ts_fp32_probe(ctx, 2000, scratch, stream)
+        for _ in range(5):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            fl = ts.ts_fp32_probe(ctx, 20000, scratch, stream)
+            b.record(stream)
+            stream.synchronize()
+            best = max(best, fl / (a.elapsed_time(b) * 1e-3) / 1e12)
+    return best
 
 
 def rank_seed(config, rank):
@@ -108,42 +151,100 @@ def max_over_ranks(dist, value, device):
     return float(t.item())
 
 
+def config_dict(sc, mode):
+    """The `config` object: identical keys in both arms (ours and --impl reference)."""
+    return {"workload": sc.name, "faces": int(sc.M), "image": [int(sc.cam.width), int(sc.cam.height)],
+            "sigma": float(sc.params.sigma), "mode": mode}
+
+
+MODE = {1: "tracking iteration, pose-only gradients", 2: "tracking iteration, pose-only gradients",
+        3: "mapping step, 8 keyframes, gradients wrt positions, colours, opacities",
+        4: "stress view, gradients wrt positions, colours, opacities and the pose"}
+
+
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` starts the N ranks itself (one process per GPU, NCCL)."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")                    # the communicator log stays on (to a file: stdout is the JSON line)
+    logdir = os.path.join(ROOT, "gpurun_out") if os.path.isdir(os.path.join(ROOT, "gpurun_out")) else "/tmp"
+    env.setdefault("NCCL_DEBUG_FILE", os.path.join(logdir, "nccl_%h_%p.log"))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    sys.exit(subprocess.call(cmd, env=env))
+
+
+# ------------------------------------------------------------------------------------------------ reference arm
+
+def oracle_step_fn(sc, args):
+    """One bounded unit of the workload through the CPU oracle as it stands (float32, tiled, single thread)."""
+    from oracle import tso
+    if args.config in (1, 2):
+        tgt = tso.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+        st = {"T": sc.T_start[0].copy(), "state": np.zeros(13, np.float32)}
+        lr = [1e-3] * 3 + [3e-3] * 3
+
+        def step():
+            o = tso.Oracle(sc.pos, sc.color, sc.opacity, None, st["T"], sc.cam, sc.params, "f32")
+            f = o.forward("tiled")
+            L, gC, gD = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, sc.params.lambda_dep)
+            g = o.backward(gC, gD, None, want=("pose",))
+            st["T"], st["state"] = tso.pose_step_f32(st["T"], g.dL_dtau, st["state"], lr)
+        return step, 1, "one full tracking iteration (project, bin + sort, forward, L1, pose-only backward, pose step)"
+    tgt_pos = sc.pos_target if sc.pos_target is not None else sc.pos
+    tgt_col = sc.color_target if sc.color_target is not None else sc.color
+    T = sc.T_start[0]
+    tgt = tso.Oracle(tgt_pos, tgt_col, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
+
+    def step():
+        o = tso.Oracle(sc.pos, sc.color, sc.opacity, None, T, sc.cam, sc.params, "f32")
+        f = o.forward("tiled")
+        L, gC, gD = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, sc.params.lambda_dep)
+        o.backward(gC, gD, None)
+    n_views = len(sc.T_gt) if args.config == 3 else 1
+    return step, 1, f"ONE view of the step's {n_views} (project, bin + sort, forward, L1, full-gradient backward)"
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle, as it stands, on the same config / metric (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
-    from oracle import tso
     from paper_2605_31419_b200 import scenes
     sc = scenes.make_config(args.config)
     HW = sc.cam.width * sc.cam.height
-    tgt_o = tso.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
-    T = sc.T_start[0].copy()
-    state = np.zeros(13, np.float32)
-    lr = [1e-3] * 3 + [3e-3] * 3
-
-    def step(T, state):
-        o = tso.Oracle(sc.pos, sc.color, sc.opacity, None, T, sc.cam, sc.params, "f32")
-        f = o.forward("tiled")
-        L, gC, gD = o.l1_loss(f.color, f.depth, tgt_o.color, tgt_o.depth, sc.params.lambda_dep)
-        g = o.backward(gC, gD, None, want=("pose",))
-        return tso.pose_step_f32(T, g.dL_dtau, state, lr)
-
+    step, views, what = oracle_step_fn(sc, args)
     for _ in range(args.warmup):
-        T, state = step(T, state)
+        step()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        T, state = step(T, state)
+        step()
     dt = (time.perf_counter() - t0) / max(1, args.steps)
-    val = HW / dt / 1e6
+    val = views * HW / dt / 1e6
     cpu = {"value": val, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
-           "sample": f"{args.steps} full tracking iterations of {sc.name} (float32 tiled oracle, single thread)"}
-    print(json.dumps({"impl": "reference", "metric": "fwd+bwd render Mpix/s", "value": val, "unit": "Mpix/s",
-                      "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3,
-                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
-                      "data": "synthetic", "config": {"workload": sc.name, "faces": sc.M, "image": [sc.cam.width, sc.cam.height]},
-                      "cpu_baseline": cpu,
+           "sample": f"{args.steps} x {what} of {sc.name} (float32 tiled oracle, single thread)"}
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": val, "unit": "Mpix/s", "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True,
+                      "scaling": "weak" if args.config in (1, 2) else "strong", "vs_baseline": None, "dtype": "f32",
+                      "data": "synthetic", "config": config_dict(sc, MODE[args.config]), "cpu_baseline": cpu,
                       "e2e": {"value": val, "unit": "Mpix/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
+
+def cpu_baseline(sc, args, budget_iters=3):
+    """The oracle as it stands, single thread, on a bounded sample of the same workload."""
+    step, views, what = oracle_step_fn(sc, args)
+    t0 = time.perf_counter()
+    for _ in range(budget_iters):
+        step()
+    dt = (time.perf_counter() - t0) / budget_iters
+    return {"value": views * sc.cam.width * sc.cam.height / dt / 1e6, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
+            "sample": f"{budget_iters} x {what} of {sc.name}, float32 tiled oracle, 1 thread", "ms_per_unit": dt * 1e3}
+
+
+# ------------------------------------------------------------------------------------------------ tracking
 
 class Tracker:
     """Device state of one tracking problem + the call sequence of one iteration (argument marshalling only)."""
@@ -199,7 +300,7 @@ class Tracker:
 
     def stages(self):
         """The iteration split at its API calls; the last two entries time the unfused forward and backward, which
-        the fused ts_render_track_l1 replaces (reported for the roofline of the individual kernels)."""
+        the fused ts_render_track_l1 replaces (reported for the forward / backward split)."""
         ts = self.ts
         lam = self.sc.params.lambda_dep
         return [("project", lambda: ts.ts_project(self.ctx, self.scene, self.cam, self.prm, self.T, self.frame)),
@@ -213,91 +314,127 @@ class Tracker:
                                                         None, None, ts.GRAD_POSE))]
 
 
-def cpu_baseline(sc, budget_iters=3):
-    """The oracle as it stands, single thread, on the same frame (bounded: a few full iterations)."""
-    from oracle import tso
-    tgt = tso.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32").forward("tiled")
-    t0 = time.perf_counter()
-    for _ in range(budget_iters):
-        o = tso.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params, "f32")
-        f = o.forward("tiled")
-        L, gC, gD = o.l1_loss(f.color, f.depth, tgt.color, tgt.depth, sc.params.lambda_dep)
-        o.backward(gC, gD, None, want=("pose",))
-    dt = (time.perf_counter() - t0) / budget_iters
-    return {"value": sc.cam.width * sc.cam.height / dt / 1e6, "unit": "Mpix/s", "cores": 1, "kind": "oracle",
-            "sample": f"{budget_iters} full fwd+bwd tracking iterations of {sc.name}, float32 tiled oracle, 1 thread",
-            "ms_per_step": dt * 1e3}
+class Harness:
+    """Timing protocol shared by the tracking and the mapping benchmarks: L2 flush (256 MiB write) before every timed
+    step, CUDA events on the launching stream, per-stage graphs."""
+
+    def __init__(self, torch, args):
+        self.torch, self.args = torch, args
+        self.stream = torch.cuda.Stream()
+        self.flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+        self.sink = torch.zeros(1, dtype=torch.int64, device="cuda")
+
+    def flush(self, kind="write"):
+        if kind == "write":
+            self.flush_buf.fill_(1)
+        elif kind == "read":                                    # a read-only sweep: leaves clean lines behind
+            self.sink.copy_(self.flush_buf.view(self.torch.int64).sum().reshape(1))
+
+    def capture(self, fn, warm=3):
+        """fn captured into a CUDA graph (or fn itself with --no-graph)."""
+        torch = self.torch
+        with torch.cuda.stream(self.stream):
+            for _ in range(warm):
+                fn()
+            self.stream.synchronize()
+            if self.args.no_graph:
+                return fn, False
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=self.stream):
+                fn()
+        return g.replay, True
+
+    def timed(self, run, k, flush="write", post=None):
+        """k steps, each bracketed by events on the stream; returns the list of milliseconds."""
+        torch = self.torch
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+        with torch.cuda.stream(self.stream):
+            for a, b in ev:
+                self.flush(flush)
+                a.record(self.stream)
+                run()
+                if post is not None:
+                    post()
+                b.record(self.stream)
+        self.stream.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
+
+    def stage_times(self, stages, k):
+        """Every stage captured into its own CUDA graph (host launch overhead does not leak into the numbers; ~4 us
+        of graph launch are included in each), events between the graph launches, flush between steps; medians."""
+        torch = self.torch
+        runs = [(name, self.capture(fn, warm=0)[0]) for name, fn in stages]      # captured in call order: no eager run in between
+        acc = {}
+        with torch.cuda.stream(self.stream):
+            for _ in range(k):
+                self.flush("write")
+                evs = [torch.cuda.Event(enable_timing=True) for _ in range(len(runs) + 1)]
+                evs[0].record(self.stream)
+                for i, (name, fn) in enumerate(runs):
+                    fn()
+                    evs[i + 1].record(self.stream)
+                for i, (name, fn) in enumerate(runs):
+                    acc.setdefault(name, []).append((evs[i], evs[i + 1]))
+        self.stream.synchronize()
+        return {k_: float(np.median([a.elapsed_time(b) for a, b in v])) for k_, v in acc.items()}
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=50)
-    ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--impl", default="ours")
-    ap.add_argument("--config", type=int, default=2)
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-graph", action="store_true")
-    ap.add_argument("--skip-extras", action="store_true", help="only the timed region (for ncu launch lists)")
-    args = ap.parse_args()
-    args.warmup = max(args.warmup, 3)
-    if args.impl == "reference":
-        return run_reference(args)
+def roofline_objects(stage_ms, in_step, B, F, peaks, p_fp32, p_fp32_measured, ms_per_step, n_views_total=1):
+    """`roofline` (dominant kernel of the step, by stage time) and `step_roofline` (whole step)."""
+    bw = peaks["hbm_gbs"] * 1e9
+    sB = lambda st: sum(B[r] for r in STAGE_ROWS[st])
+    sF = lambda st: sum(F[r] for r in STAGE_ROWS[st])
+    dom = max((k for k in in_step if k in stage_ms), key=lambda k: stage_ms[k])
+    dom_t = stage_ms[dom] * 1e-3
+    if sF(dom) / (p_fp32 * 1e12) > sB(dom) / bw:
+        roof = {"bound": "alu", "kernel": dom, "achieved": sF(dom) / dom_t / 1e12, "peak": p_fp32, "unit": "TFLOP/s",
+                "peak_source": "nominal 148 SM x 128 FP32 lanes x 2 x sm_max_mhz (DESIGN.md section 8)",
+                "peak_measured_fma_loop": p_fp32_measured}
+    else:
+        roof = {"bound": "hbm", "kernel": dom, "achieved": sB(dom) / dom_t / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "peak_source": peaks["src"]}
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"], roof["traffic_source"] = load_traffic(dom)
+    roof["algorithmic_bytes"], roof["algorithmic_flops"], roof["launch_ms"] = sB(dom), sF(dom), stage_ms[dom]
+    rows = [r for st in in_step for r in STAGE_ROWS[st]]
+    Bt, Ft = n_views_total * sum(B[r] for r in rows), n_views_total * sum(F[r] for r in rows)
+    t_hbm, t_alu = Bt / bw, Ft / (p_fp32 * 1e12)
+    step = {"t_hbm_us": t_hbm * 1e6, "t_alu_us": t_alu * 1e6, "t_roof_us": max(t_hbm, t_alu) * 1e6,
+            "frac": max(t_hbm, t_alu) / (ms_per_step * 1e-3), "algorithmic_bytes": Bt, "algorithmic_flops": Ft,
+            "rows": {r: {"bytes": n_views_total * B[r], "flops": n_views_total * F[r]} for r in rows},
+            "hbm_peak_gbs": peaks["hbm_gbs"], "fp32_peak_tflops_nominal": p_fp32, "fp32_peak_tflops_measured": p_fp32_measured}
+    return roof, step
 
-    import torch
-    from paper_2605_31419_b200 import scenes, ts
-    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+def count_view(ts, torch, ctx, scene, cam, sc, T, frame):
+    """Device counters of one view (the counting instantiation of the forward kernel, outside any timed region)."""
+    prm = ts.make_params(sc.params, ts.PARAM_COUNTERS)
+    H, W = sc.cam.height, sc.cam.width
+    c0 = ts.ts_frame_view(ctx, frame, ts.VIEW_COUNTERS).cpu().numpy().astype(np.int64).copy()
+    ts.ts_project(ctx, scene, cam, prm, T, frame)
+    ts.ts_bin_sort(ctx, frame)
+    ts.ts_render_fwd(ctx, scene, frame, torch.empty(3, H, W, device="cuda"), torch.empty(H, W, device="cuda"), None)
+    fl, nvis, npairs = ts.ts_frame_status(ctx, frame)
+    c1 = ts.ts_frame_view(ctx, frame, ts.VIEW_COUNTERS).cpu().numpy().astype(np.int64)
+    d = c1 - c0
+    return {"n_visible": int(nvis), "n_pairs": int(npairs), "n_warp_visits": int(d[0]), "n_rect": int(d[1]), "n_hit": int(d[2])}
+
+
+def bench_tracking(args, torch, ts, scenes, dist, rank, world, local):
     peaks = load_peaks()
     # replicas / weak scaling: every rank tracks its own frame of the same scene family (seed offset by rank)
     sc = scenes.make_config(args.config, seed=rank_seed(args.config, rank)) if rank else scenes.make_config(args.config)
     HW, M = sc.cam.width * sc.cam.height, sc.M
-
-    # counters (debug instantiation, outside the timed region)
-    trc = Tracker(sc, local, count_flags=ts.PARAM_COUNTERS)
-    trc.forward()
-    fl, nvis, npairs = ts.ts_frame_status(trc.ctx, trc.frame)
-    cn = ts.ts_frame_view(trc.ctx, trc.frame, ts.VIEW_COUNTERS).cpu().numpy()
-    # the counting instantiation ran once, for the target render in Tracker.__init__ (the fused forward does not count)
-    cnt = {"n_visible": int(nvis), "n_pairs": int(npairs), "n_warp_visits": int(cn[0]), "n_rect": int(cn[1]), "n_hit": int(cn[2]),
-           "note": "n_rect / n_hit / n_warp_visits: one forward render (ground-truth pose); n_visible / n_pairs: start pose"}
-    del trc
-    torch.cuda.empty_cache()
-
+    NT = ((sc.cam.width + 15) // 16) * ((sc.cam.height + 15) // 16)
     tr = Tracker(sc, local)
-    NT = tr.frame_nt = ((sc.cam.width + 15) // 16) * ((sc.cam.height + 15) // 16)
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
-    stream = torch.cuda.Stream()
-    graph = None
-    with torch.cuda.stream(stream):
-        for _ in range(3):
-            tr.iteration()
-        stream.synchronize()
-        if not args.no_graph:
-            graph = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(graph, stream=stream):
-                tr.iteration()
-    run = (lambda: graph.replay()) if graph is not None else tr.iteration
-
-    def timed(k, do_flush=True):
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
-        with torch.cuda.stream(stream):
-            for a, b in ev:
-                if do_flush:
-                    flush.fill_(1)
-                a.record(stream)
-                run()
-                b.record(stream)
-        stream.synchronize()
-        return [a.elapsed_time(b) for a, b in ev]
+    cnt = count_view(ts, torch, tr.ctx, tr.scene, tr.cam, sc, tr.T, tr.frame)
+    cnt["note"] = "one forward render at the start pose (counting instantiation of the forward kernel)"
+    hz = Harness(torch, args)
+    stream = hz.stream
+    run, graphed = hz.capture(tr.iteration)
 
     tr.reset()
-    timed(args.warmup)
+    hz.timed(run, args.warmup)
     tr.reset()
     if dist is not None:
         dist.barrier()
@@ -305,20 +442,23 @@ def main():
     clk = ClockSampler(local)
     clk.start()
     t_wall0 = time.perf_counter()
-    ms = timed(args.steps)
+    ms = hz.timed(run, args.steps)
     torch.cuda.synchronize()
     t_wall = time.perf_counter() - t_wall0
-    total_ms = float(sum(ms))
-    total_ms = max_over_ranks(dist, total_ms, "cuda")
+    total_ms = max_over_ranks(dist, float(sum(ms)), "cuda")
     if dist is not None:
         dist.barrier()
     ms_per_step = total_ms / args.steps
 
     if args.skip_extras:
+        clk.stop()
         if rank == 0:
-            print(json.dumps({"metric": "fwd+bwd render Mpix/s", "value": world * HW / (ms_per_step * 1e-3) / 1e6,
-                              "unit": "Mpix/s", "ms_per_step": ms_per_step, "steps": args.steps, "partial": True}))
+            print(json.dumps({"metric": METRIC, "value": world * HW / (ms_per_step * 1e-3) / 1e6, "unit": "Mpix/s",
+                              "ms_per_step": ms_per_step, "steps": args.steps, "partial": True}))
         return
+    # the same protocol with a read-only flush (leaves clean instead of dirty lines in L2), for comparison
+    tr.reset()
+    ms_read = hz.timed(run, min(args.steps, 50), flush="read")
     # one frame = 100 tracking iterations back to back, no flush
     tr.reset()
     with torch.cuda.stream(stream):
@@ -329,70 +469,10 @@ def main():
         b.record(stream)
     stream.synchronize()
     frame_ms = a.elapsed_time(b)
-    loss_after = None
-
-    # per-stage device times: every stage captured into its own CUDA graph (so that host launch overhead does not
-    # leak into the numbers), events between the graph launches; flush between steps
     tr.reset()
-    stage_graphs = []
-    with torch.cuda.stream(stream):
-        for name, fn in tr.stages():
-            if args.no_graph:
-                stage_graphs.append((name, fn))
-            else:
-                gr = torch.cuda.CUDAGraph()
-                with torch.cuda.graph(gr, stream=stream):
-                    fn()
-                stage_graphs.append((name, gr.replay))
-    tr.reset()
-    stage_ms = {}
-    with torch.cuda.stream(stream):
-        for it in range(args.steps):
-            flush.fill_(1)
-            evs = [torch.cuda.Event(enable_timing=True) for _ in range(len(stage_graphs) + 1)]
-            evs[0].record(stream)
-            for i, (name, fn) in enumerate(stage_graphs):
-                fn()
-                evs[i + 1].record(stream)
-            for i, (name, fn) in enumerate(stage_graphs):
-                stage_ms.setdefault(name, []).append((evs[i], evs[i + 1]))
-    stream.synchronize()
-    stage_ms = {k: float(np.median([a.elapsed_time(b) for a, b in v])) for k, v in stage_ms.items()}
+    stage_ms = hz.stage_times(tr.stages(), args.steps)
     clocks = clk.stop()
-
-    # extra, informational: one MAPPING view of the same scene (BASELINE.json configs[3]'s step is 8 of these on 1 M
-    # faces): project + bin/sort + forward with L1 + full-gradient backward (positions, colours, opacities), one graph
-    V = tr.scene.V
-    gpos, gcol, gopa = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
-    lam = sc.params.lambda_dep
-
-    def map_view():
-        ts.ts_project(tr.ctx, tr.scene, tr.cam, tr.prm, tr.T, tr.frame)
-        ts.ts_bin_sort(tr.ctx, tr.frame)
-        ts.ts_render_map_l1(tr.ctx, tr.scene, tr.frame, tr.C, tr.D, tr.A, tr.Chat, tr.Dhat, lam, tr.gC, tr.gD, tr.loss,
-                            gpos, gcol, gopa, ts.GRAD_POS | ts.GRAD_COLOR | ts.GRAD_OPACITY)
-
-    tr.reset()
-    with torch.cuda.stream(stream):
-        for _ in range(2):
-            map_view()
-        stream.synchronize()
-        mrun = map_view
-        if not args.no_graph:
-            mg = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(mg, stream=stream):
-                map_view()
-            mrun = mg.replay
-        mev = []
-        for _ in range(max(10, args.steps // 2)):
-            flush.fill_(1)
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record(stream)
-            mrun()
-            b.record(stream)
-            mev.append((a, b))
-    stream.synchronize()
-    map_ms = float(np.median([a.elapsed_time(b) for a, b in mev]))
+    p_fp32_meas = measure_fp32_peak(ts, tr.ctx, torch, stream)
 
     # e2e: same iteration through the C ABI with HOST buffers: every step the frame's target RGB-D (pinned, 16 B/pixel)
     # and the pose go up and dL/dtau and the loss come back, all inside the timed region.  The uploads run on a copy
@@ -404,20 +484,9 @@ def main():
     h_out = torch.empty(n_e2e, 7).pin_memory()
     bufs = [(tr.Chat, tr.Dhat), (torch.empty_like(tr.Chat), torch.empty_like(tr.Dhat))]
     runs = [run]
-    with torch.cuda.stream(stream):
-        tr.Chat, tr.Dhat = bufs[1]
-        if args.no_graph:
-            def run_b():
-                tr.Chat, tr.Dhat = bufs[1]
-                tr.iteration()
-                tr.Chat, tr.Dhat = bufs[0]
-            runs.append(run_b)
-        else:
-            g2 = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g2, stream=stream):
-                tr.iteration()
-            runs.append(g2.replay)
-        tr.Chat, tr.Dhat = bufs[0]
+    tr.Chat, tr.Dhat = bufs[1]
+    runs.append(hz.capture(tr.iteration, warm=1)[0])
+    tr.Chat, tr.Dhat = bufs[0]
     stream.synchronize()
     tr.reset()
     copy_stream = torch.cuda.Stream()
@@ -426,18 +495,18 @@ def main():
 
     def e2e_steps(i0, i1):
         for i in range(i0, i1):
-            b = i & 1
+            bsel = i & 1
             with torch.cuda.stream(copy_stream):
                 if i >= 2:
                     copy_stream.wait_event(done[i - 2])           # the buffer's previous user has finished
-                bufs[b][0].copy_(hC, non_blocking=True)
-                bufs[b][1].copy_(hD, non_blocking=True)
+                bufs[bsel][0].copy_(hC, non_blocking=True)
+                bufs[bsel][1].copy_(hD, non_blocking=True)
                 copied[i].record(copy_stream)
             with torch.cuda.stream(stream):
-                flush.fill_(1)
+                hz.flush("write")
                 tr.T.copy_(hT, non_blocking=True)
                 stream.wait_event(copied[i])
-                runs[b]()
+                runs[bsel]()
                 h_out[i, :6].copy_(tr.tau, non_blocking=True)
                 h_out[i, 6:].copy_(tr.loss, non_blocking=True)
                 done[i].record(stream)
@@ -447,57 +516,241 @@ def main():
     t0 = time.perf_counter()
     e2e_steps(args.warmup, n_e2e)
     torch.cuda.synchronize()
-    e2e_step = (time.perf_counter() - t0) * 1e3 / args.steps
-    e2e_step = max_over_ranks(dist, e2e_step, "cuda")
+    e2e_step = max_over_ranks(dist, (time.perf_counter() - t0) * 1e3 / args.steps, "cuda")
 
     value = world * HW / (ms_per_step * 1e-3) / 1e6
     p_sort = (32 + max(0, (NT - 1).bit_length()) + 7) // 8
     B, F = algorithmic_work(cnt, HW, NT, M, p_sort, "pose")
     p_fp32 = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12        # TFLOP/s, nominal
-    t_hbm = sum(B[k] for k in STEP_ROWS) / (peaks["hbm_gbs"] * 1e9)
-    t_alu = sum(F[k] for k in STEP_ROWS) / (p_fp32 * 1e12)
-    t_roof = max(t_hbm, t_alu)
-    in_step = ("project", "bin_sort", "render_track", "pose_reduce")          # the launches of the timed iteration
-    dom = max((k for k in in_step if k in stage_ms), key=lambda k: stage_ms[k])
-    dom_t = stage_ms[dom] * 1e-3
-    if F[dom] / (p_fp32 * 1e12) > B[dom] / (peaks["hbm_gbs"] * 1e9):
-        roof = {"bound": "alu", "kernel": dom, "achieved": F[dom] / dom_t / 1e12, "peak": p_fp32, "unit": "TFLOP/s",
-                "peak_source": "nominal 148 SM x 128 FP32 lanes x 2 x sm_max_mhz (DESIGN.md section 8)"}
-    else:
-        roof = {"bound": "hbm", "kernel": dom, "achieved": B[dom] / dom_t / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                "peak_source": peaks["src"]}
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = load_traffic().get(dom)
-    roof["algorithmic_bytes"] = B[dom]
-    roof["algorithmic_flops"] = F[dom]
-    roof["launch_ms"] = stage_ms[dom]
-
-    out = {"metric": "fwd+bwd render Mpix/s", "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps,
-           "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
-           "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-           "config": {"workload": sc.name, "faces": M, "image": [sc.cam.width, sc.cam.height], "sigma": sc.params.sigma,
-                      "mode": "tracking iteration, pose-only gradients", "l2": "flushed between timed steps (256 MiB write)",
-                      "cuda_graph": graph is not None},
+    in_step = ("project", "bin_sort", "render_track", "pose_reduce")               # the launches of the timed iteration
+    roof, step_roof = roofline_objects(stage_ms, in_step, B, F, peaks, p_fp32, p_fp32_meas, ms_per_step)
+    fwd_ms = stage_ms["project"] + stage_ms["bin_sort"] + stage_ms["render_fwd"]
+    bwd_ms = stage_ms["render_bwd"] + stage_ms["pose_reduce"]
+    out = {"metric": METRIC, "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms_per_step, "ms_per_step_median": float(np.median(ms)),
+           "ms_per_step_min": float(np.min(ms)), "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config_dict(sc, MODE[args.config]),
+           "protocol": {"l2": "flushed before every timed step (256 MiB write)", "cuda_graph": graphed,
+                        "ms_per_step_read_flush": float(np.mean(ms_read)),
+                        "multi_gpu": "replicas: one independent tracker per rank, no data-path collective"},
            "clocks": clocks, "gpu_launches": Tracker.launches_per_iter * args.steps,
            "e2e": {"value": world * HW / (e2e_step * 1e-3) / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": 16 * HW + 48,
                    "d2h_bytes_per_step": 28, "ms_per_step": e2e_step,
                    "how": "K steps timed as a whole by the host clock; every step uploads its target RGB-D frame and pose from "
                           "pinned memory (copy stream, two device buffers, overlapping the previous step's kernels), flushes L2, "
                           "runs the iteration and reads dL/dtau + loss back"},
-           "roofline": roof,
-           "step_roofline": {"t_hbm_us": t_hbm * 1e6, "t_alu_us": t_alu * 1e6, "t_roof_us": t_roof * 1e6,
-                             "frac": t_roof / (ms_per_step * 1e-3), "algorithmic_bytes": sum(B[k] for k in STEP_ROWS),
-                             "algorithmic_flops": sum(F[k] for k in STEP_ROWS), "hbm_peak_gbs": peaks["hbm_gbs"], "fp32_peak_tflops": p_fp32},
-           "mapping_view": {"ms": map_ms, "Mpix_per_s": HW / (map_ms * 1e-3) / 1e6,
-                            "what": "project + bin/sort + ts_render_map_l1 (forward, L1, backward wrt positions, colours, "
-                                    "opacities) of ONE view of this scene, one CUDA graph, L2 flushed (informational; not the "
-                                    "headline metric)"},
+           "roofline": roof, "step_roofline": step_roof,
+           "fwd_Mpix_s": world * HW / (fwd_ms * 1e-3) / 1e6, "bwd_Mpix_s": world * HW / (bwd_ms * 1e-3) / 1e6,
+           "fwd_bwd_split": {"fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
+                             "what": "unfused stages, each its own CUDA graph (~4 us of graph launch in each): forward = "
+                                     "ts_project + ts_bin_sort + ts_render_fwd_l1, backward = ts_render_bwd(pose-only) + "
+                                     "ts_pose_reduce_step"},
            "tracking_iters_per_s": world * 100.0 / (frame_ms * 1e-3), "frame_100_iters_ms": frame_ms,
-           "stage_ms": stage_ms, "counters": cnt, "wall_s_timed_region": t_wall}
+           "stage_ms": stage_ms, "counters": cnt, "wall_s_timed_region": t_wall, "src_sha16": src_sha16()}
     if rank == 0:
-        if not args.no_cpu_baseline and world >= 1:
-            out["cpu_baseline"] = cpu_baseline(sc)
+        if not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(sc, args)
         print(json.dumps(out))
+
+
+# ------------------------------------------------------------------------------------------------ mapping
+
+class Mapper:
+    """Device state of one mapping problem (BASELINE.json configs[3] / [4]): replicated map, this rank's keyframes with
+    their target frames, one flat gradient buffer; the call sequence of one step (argument marshalling only)."""
+
+    def __init__(self, sc, device, views, want_pose):
+        import torch
+        from paper_2605_31419_b200 import dist_map, ts
+        self.torch, self.ts, self.sc, self.views, self.want_pose = torch, ts, sc, views, want_pose
+        self.ctx = ts.Context(device)
+        d = lambda a, dt=torch.float32: torch.as_tensor(np.ascontiguousarray(a), dtype=dt).cuda()
+        self.scene = ts.Scene(d(sc.pos), d(sc.color), d(sc.opacity))
+        self.cam, self.prm = ts.make_camera(sc.cam), ts.make_params(sc.params)
+        self.W, self.H = sc.cam.width, sc.cam.height
+        self.frame = ts.Frame(self.ctx, self.scene.M, self.W, self.H, pair_capacity=max(2 * self.scene.M, 1 << 16))
+        H, W = self.H, self.W
+        z = lambda *s: torch.zeros(*s, device="cuda")
+        self.C, self.D, self.A, self.gC, self.gD = z(3, H, W), z(H, W), z(H, W), z(3, H, W), z(H, W)
+        self.loss, self.tau = z(1), z(6)
+        self.bucket = dist_map.GradBucket(self.scene.V, "cuda")
+        self.mask = ts.GRAD_POS | ts.GRAD_COLOR | ts.GRAD_OPACITY | (ts.GRAD_POSE if want_pose else 0)
+        # target RGB-D frames: renders of the ground-truth scene from the keyframe poses (stand-in for dataset frames)
+        tpos = sc.pos_target if sc.pos_target is not None else sc.pos
+        tcol = sc.color_target if sc.color_target is not None else sc.color
+        tscene = ts.Scene(d(tpos), d(tcol), d(sc.opacity))
+        self.poses, self.targets = [], []
+        for v in views:
+            Tg = d(sc.T_gt[v].reshape(-1))
+            Chat, Dhat = z(3, H, W), z(H, W)
+            ts.ts_project(self.ctx, tscene, self.cam, self.prm, Tg, self.frame)
+            ts.ts_bin_sort(self.ctx, self.frame)
+            ts.ts_render_fwd(self.ctx, tscene, self.frame, Chat, Dhat, None)
+            self.poses.append(d(sc.T_start[v].reshape(-1)))
+            self.targets.append((Chat, Dhat))
+        del tscene
+        torch.cuda.synchronize()
+
+    def launches_per_step(self):
+        return len(self.views) * (1 + 2 + 2 + (1 if self.want_pose else 0)) + 1   # + the zeroing of the gradient buffer
+
+    def view(self, i):
+        ts = self.ts
+        Chat, Dhat = self.targets[i]
+        ts.ts_project(self.ctx, self.scene, self.cam, self.prm, self.poses[i], self.frame)
+        ts.ts_bin_sort(self.ctx, self.frame)
+        ts.ts_render_map_l1(self.ctx, self.scene, self.frame, self.C, self.D, self.A, Chat, Dhat, self.sc.params.lambda_dep,
+                            self.gC, self.gD, self.loss, self.bucket.grad_pos, self.bucket.grad_color,
+                            self.bucket.grad_opacity, self.mask)
+        if self.want_pose:
+            ts.ts_pose_jacobian_reduce(self.ctx, self.frame, self.tau)
+
+    def local_step(self):
+        """This rank's share of one mapping step: zero the gradient buffer, then every own view."""
+        self.bucket.zero_()
+        self.loss.zero_()
+        for i in range(len(self.views)):
+            self.view(i)
+
+    def stages(self):
+        ts = self.ts
+        Chat, Dhat = self.targets[0]
+        return [("project", lambda: ts.ts_project(self.ctx, self.scene, self.cam, self.prm, self.poses[0], self.frame)),
+                ("bin_sort", lambda: ts.ts_bin_sort(self.ctx, self.frame)),
+                ("render_map", lambda: ts.ts_render_map_l1(self.ctx, self.scene, self.frame, self.C, self.D, self.A, Chat, Dhat,
+                                                           self.sc.params.lambda_dep, self.gC, self.gD, self.loss,
+                                                           self.bucket.grad_pos, self.bucket.grad_color,
+                                                           self.bucket.grad_opacity, self.mask))]
+
+
+def bench_mapping(args, torch, ts, scenes, dist, rank, world, local):
+    from paper_2605_31419_b200 import dist_map
+    peaks = load_peaks()
+    sc = scenes.make_config(args.config)
+    n_views = len(sc.T_gt) if args.config == 3 else 1
+    want_pose = args.config == 4
+    if world > n_views:
+        raise SystemExit(f"--gpus {world} > {n_views} views of config {args.config}: nothing to shard")
+    HW, M = sc.cam.width * sc.cam.height, sc.M
+    NT = ((sc.cam.width + 15) // 16) * ((sc.cam.height + 15) // 16)
+    my_views = dist_map.shard_views(n_views, rank, world)
+    mp = Mapper(sc, local, my_views, want_pose)
+    # counters of every view of this rank (rank 0's are printed; the roofline uses view 0's x the number of views)
+    cnts = [count_view(ts, torch, mp.ctx, mp.scene, mp.cam, sc, mp.poses[i], mp.frame) for i in range(len(my_views))]
+    hz = Harness(torch, args)
+    stream = hz.stream
+    run, graphed = hz.capture(mp.local_step, warm=2)
+    # the step's one collective: sum of the gradient buffer over the ranks (NCCL), on the launching stream, after the
+    # rank's views; nothing to overlap it with inside ONE step (the optimiser needs the sum before the next one)
+    post = (lambda: mp.bucket.all_reduce(dist)) if world > 1 else None
+
+    hz.timed(run, args.warmup, post=post)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    clk = ClockSampler(local)
+    clk.start()
+    t_wall0 = time.perf_counter()
+    ms = hz.timed(run, args.steps, post=post)
+    torch.cuda.synchronize()
+    t_wall = time.perf_counter() - t_wall0
+    total_ms = max_over_ranks(dist, float(sum(ms)), "cuda")
+    if dist is not None:
+        dist.barrier()
+    ms_per_step = total_ms / args.steps
+    stage_ms = hz.stage_times(mp.stages(), max(10, args.steps // 2))
+    clocks = clk.stop()
+    p_fp32_meas = measure_fp32_peak(ts, mp.ctx, torch, stream)
+
+    # e2e: the step through the C ABI with HOST buffers: this rank's keyframe targets (pinned, 16 B/pixel each) and
+    # poses go up every step, the loss comes back; inside the timed region, host clock, device synchronised both sides
+    h_tg = [(c.cpu().pin_memory(), d_.cpu().pin_memory()) for c, d_ in mp.targets]
+    h_T = [p.cpu().pin_memory() for p in mp.poses]
+    h_loss = torch.empty(args.warmup + args.steps, 1).pin_memory()
+
+    def e2e_steps(i0, i1):
+        with torch.cuda.stream(stream):
+            for i in range(i0, i1):
+                hz.flush("write")
+                for (c, d_), (hc, hd), p, hp in zip(mp.targets, h_tg, mp.poses, h_T):
+                    c.copy_(hc, non_blocking=True), d_.copy_(hd, non_blocking=True), p.copy_(hp, non_blocking=True)
+                run()
+                if post is not None:
+                    post()
+                h_loss[i].copy_(mp.loss, non_blocking=True)
+
+    e2e_steps(0, args.warmup)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e2e_steps(args.warmup, args.warmup + args.steps)
+    torch.cuda.synchronize()
+    e2e_step = max_over_ranks(dist, (time.perf_counter() - t0) * 1e3 / args.steps, "cuda")
+
+    value = n_views * HW / (ms_per_step * 1e-3) / 1e6
+    p_sort = (32 + max(0, (NT - 1).bit_length()) + 7) // 8
+    B, F = algorithmic_work(cnts[0], HW, NT, M, p_sort, "full")
+    p_fp32 = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    in_step = ("project", "bin_sort", "render_map") + (("pose_reduce",) if want_pose else ())
+    if want_pose:
+        stage_ms.setdefault("pose_reduce", 0.0)
+    # the step roofline is the work of ALL views of the step against the whole-job time (max over ranks)
+    roof, step_roof = roofline_objects(stage_ms, [s for s in in_step if s in stage_ms and stage_ms[s] > 0], B, F, peaks, p_fp32,
+                                       p_fp32_meas, ms_per_step, n_views_total=n_views)
+    step_roof["note"] = ("bytes / flops of view 0 x the number of views; with N ranks the bound is that work at ONE GPU's "
+                         "peaks, so the fraction can exceed what one GPU could reach")
+    out = {"metric": METRIC, "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": ms_per_step, "ms_per_step_median": float(np.median(ms)),
+           "ms_per_step_min": float(np.min(ms)), "higher_is_better": True, "scaling": "strong",
+           "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config_dict(sc, MODE[args.config]),
+           "protocol": {"l2": "flushed before every timed step (256 MiB write)", "cuda_graph": graphed, "views": n_views,
+                        "views_of_rank_0": my_views,
+                        "multi_gpu": "views dealt round-robin to the ranks, replicated map, one all-reduce (sum) of the 7 V "
+                                     "float gradient buffer per step" if world > 1 else "single rank: no collective",
+                        "allreduce_bytes_per_step": 28 * mp.scene.V if world > 1 else 0},
+           "clocks": clocks, "gpu_launches": mp.launches_per_step() * args.steps,
+           "e2e": {"value": n_views * HW / (e2e_step * 1e-3) / 1e6, "unit": "Mpix/s",
+                   "h2d_bytes_per_step": len(my_views) * (16 * HW + 48), "d2h_bytes_per_step": 4, "ms_per_step": e2e_step,
+                   "how": "K steps timed as a whole by the host clock; every step uploads this rank's keyframe targets and "
+                          "poses from pinned memory, flushes L2, runs the step (and the all-reduce) and reads the loss back"},
+           "roofline": roof, "step_roofline": step_roof, "ms_per_view": ms_per_step / max(1, len(my_views)),
+           "stage_ms": stage_ms, "counters": cnts[0], "counters_all_views_of_rank_0": cnts,
+           "wall_s_timed_region": t_wall, "src_sha16": src_sha16()}
+    if rank == 0:
+        if not args.no_cpu_baseline:
+            out["cpu_baseline"] = cpu_baseline(sc, args, budget_iters=1 if args.config == 4 else 2)
+        print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--config", type=int, default=2, choices=(1, 2, 3, 4))
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-graph", action="store_true")
+    ap.add_argument("--skip-extras", action="store_true", help="only the timed region (for ncu launch lists)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return respawn_under_torchrun(args)
+
+    import torch
+    from paper_2605_31419_b200 import scenes, ts
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if args.config in (1, 2):
+        bench_tracking(args, torch, ts, scenes, dist, rank, world, local)
+    else:
+        bench_mapping(args, torch, ts, scenes, dist, rank, world, local)
     if dist is not None:
         dist.destroy_process_group()
 

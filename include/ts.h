@@ -212,6 +212,11 @@ int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, flo
 int32_t ts_pose_reduce_step(ts_ctx* ctx, ts_frame* frame, float* dL_dtau_dev, float* T_cw_dev, float* state_dev,
                             const float* lr6, float beta1, float beta2, float eps, void* stream);
 
+/* Measurement helper: enqueues a dependent-free FP32 FMA loop (`iters` rounds of eight
+ * independent chains per thread, 2 x 1024 threads per SM) and returns in *flops_out (HOST) the flops it performs; the
+ * caller times it with events on `stream` to get the measured FP32 peak.  scratch_dev: one float of device memory. */
+int32_t ts_fp32_probe(ts_ctx* ctx, int32_t iters, float* scratch_dev, uint64_t* flops_out, void* stream);
+
 /* ---- read-only debug accessors (bit-exact tests) ---------------------------------------------------------- */
 enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slot order (slots are NOT in face order):
                                     f32 (u,v,w)x3, f32 mean opacity, i16 x0,y0,x1,y1, u32 face, u32 depth_key,

@@ -182,3 +182,27 @@ extern "C" int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dt
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }
+
+// Measurement helper ("measure a dependent-free FMA loop and print both nominal and measured
+// peaks"): every thread runs `iters` rounds of eight independent FMA chains; 16 flops per thread and round.
+namespace {
+__global__ void __launch_bounds__(1024) fp32_probe_kernel(int iters, float a, float b, float* __restrict__ out) {
+    float x0 = threadIdx.x * 1e-3f, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f, x4 = x0 + 4.f, x5 = x0 + 5.f, x6 = x0 + 6.f, x7 = x0 + 7.f;
+#pragma unroll 4
+    for (int i = 0; i < iters; ++i) {
+        x0 = fmaf(x0, a, b), x1 = fmaf(x1, a, b), x2 = fmaf(x2, a, b), x3 = fmaf(x3, a, b);
+        x4 = fmaf(x4, a, b), x5 = fmaf(x5, a, b), x6 = fmaf(x6, a, b), x7 = fmaf(x7, a, b);
+    }
+    const float s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 123.456f) out[0] = s;                       // never true: keeps the chains alive
+}
+}  // namespace
+
+extern "C" int32_t ts_fp32_probe(ts_ctx* ctx, int32_t iters, float* scratch_dev, uint64_t* flops_out, void* stream) {
+    if (!ctx || iters <= 0 || !scratch_dev || !flops_out) return TS_ERR_INVALID_ARG;
+    const int grid = ctx->num_sms * 2;
+    fp32_probe_kernel<<<grid, 1024, 0, (cudaStream_t)stream>>>(iters, 0.999f, 1e-3f, scratch_dev);
+    *flops_out = (uint64_t)grid * 1024ull * 16ull * (uint64_t)iters;
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}

@@ -27,7 +27,8 @@ _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.
 EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_map_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
            "ts_render_fwd_normal", "ts_render_bwd_normal", "ts_normal_loss_grad", "ts_render_bwd_stats",
-           "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view"]
+           "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view",
+           "ts_fp32_probe"]
 
 
 class TsError(RuntimeError):
@@ -99,6 +100,7 @@ def _load():
                                     C.POINTER(C.c_uint64), C.c_void_p]
     lib.ts_frame_view.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t),
                                   C.c_void_p]
+    lib.ts_fp32_probe.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.POINTER(C.c_uint64), C.c_void_p]
     lib.ts_frame_release.argtypes = [C.c_void_p]
     lib.ts_destroy.argtypes = [C.c_void_p]
     lib.ts_create.argtypes = [C.c_int32, C.POINTER(C.c_void_p)]
@@ -280,6 +282,13 @@ def ts_pose_reduce_step(ctx, frame, dL_dtau, T_cw, state, lr6, beta1=0.9, beta2=
     lr = (C.c_float * 6)(*[float(x) for x in lr6])
     _check(lib.ts_pose_reduce_step(ctx.h, frame.h, _ptr(dL_dtau), _ptr(T_cw), _ptr(state), lr, beta1, beta2, eps,
                                    _stream(stream)))
+
+
+def ts_fp32_probe(ctx, iters, scratch, stream=None):
+    """Enqueues the dependent-free FMA loop; returns the flops it performs (time it with events)."""
+    fl = C.c_uint64()
+    _check(lib.ts_fp32_probe(ctx.h, int(iters), _ptr(scratch), C.byref(fl), _stream(stream)))
+    return int(fl.value)
 
 
 def ts_frame_status(ctx, frame, stream=None, check=True):
