@@ -129,7 +129,9 @@ int32_t ts_equi_loss_grad(ts_ctx* ctx, const ts_scene* scene, float weight, floa
  * L_DSSIM = 1 - mean SSIM(C, Chat) over 3 x H x W, 11x11 Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2,
  * C2 = 0.03^2.  On entry gC[3][H][W] holds the cotangent of the L1 term (ts_l1_loss_grad); on exit
  * gC = (1 - lambda) gC + lambda dL_DSSIM/dC, i.e. the cotangent of E_pho.  If loss_dev != NULL, lambda * L_DSSIM is
- * added to *loss_dev.  scratch: 9 * H * W floats of caller memory. */
+ * added to *loss_dev.  One launch; both separable passes run in shared memory on a tile + apron, so `scratch` is not
+ * used any more (pass NULL; the argument stays for ABI compatibility with round 1).  In a tracking iteration it sits
+ * between ts_render_fwd_l1 (which writes C and the L1 cotangents) and ts_render_bwd. */
 int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* Chat, float lambda, float* gC,
                            float* loss_dev, float* scratch, void* stream);
 /* a3 + a4 in one launch: ts_render_fwd, with the L1 colour + depth loss of ts_l1_loss_grad evaluated on every pixel

@@ -2,83 +2,170 @@
 // ts_l1_loss_grad.  L_DSSIM = 1 - mean SSIM over 3 channels x H x W with the 11x11 Gaussian
 // window (sigma 1.5), zero padding, C1 = 0.01^2, C2 = 0.03^2 (reading S25).
 //
-// Two HBM-bound passes over the image, each a separable 11-tap convolution through shared memory on 32x32 tiles
-// with a 5-pixel halo:
-//   dssim_fwd_kernel : window sums of x, y, x^2, y^2, xy -> SSIM map (summed into the loss) and the three maps
-//                      M0 = w (d_mu1 - 2 mu1 d_s11 - mu2 d_s12), M1 = w d_s11, M2 = w d_s12   (w = -lambda / 3HW)
-//   dssim_bwd_kernel : gC <- (1 - lambda) gC + conv(M0) + 2 x conv(M1) + y conv(M2)
-// (the window is symmetric, so the adjoint of the zero-padded convolution is the same convolution).
+// ONE launch, no scratch image: a CTA owns a 32x32 tile of one channel and does BOTH separable 11-tap convolutions in
+// shared memory.  The gradient at a pixel needs the maps M0..M2 on its 11x11 neighbourhood, and every M needs the
+// window sums of x, y, x^2, y^2, xy on ITS neighbourhood, so the CTA reads the images on the tile + a 10-pixel apron
+// (52 x 52), forms the window sums and
+//     M0 = w (d_mu1 - 2 mu1 d_s11 - mu2 d_s12),  M1 = w d_s11,  M2 = w d_s12        (w = -lambda / 3HW)
+// on the tile + a 5-pixel apron (42 x 42; zero outside the image, like the zero padding of the forward window), then
+//     gC <- (1 - lambda) gC + conv(M0) + 2 x conv(M1) + y conv(M2)
+// on the tile (the window is symmetric, so the adjoint of the zero-padded convolution is the same convolution).  The
+// apron costs 2.6x the reads of the tile (all L2 hits: the forward pass has just written C) and 1.7x the window sums;
+// it saves the 9 HW floats of the two-pass form and a launch.  SSIM itself is summed into the loss on the tile only.
 #include <cmath>
 
 #include "ts_internal.cuh"
 
 namespace {
 
-constexpr int DT = 32, DR = 5, DIN = DT + 2 * DR;   // tile, window radius, tile + halo
+constexpr int DT = 32, DR = 5;
+constexpr int DB = DT + 2 * DR;      // 42: tile + apron of the M maps
+constexpr int DA = DT + 4 * DR;      // 52: tile + apron of the images
 
 struct Gauss11 { float g[11]; };
 
+struct DssimSmem {
+    union {
+        struct { float sx[DA][DA + 1], sy[DA][DA + 1]; } in;    // images (steps 1-2)
+        float m[3][DB][DB + 1];                                  // M maps (steps 3-4)
+    } a;
+    union {
+        float hs[5][DA][DB];                                     // row sums of x, y, x^2, y^2, xy (steps 2-3)
+        float hm[3][DB][DT];                                     // row sums of the M maps (steps 4-5)
+    } b;
+    float red[8];
+};
+
 __global__ void __launch_bounds__(256)
-dssim_fwd_kernel(int W, int H, const float* __restrict__ X, const float* __restrict__ Y, Gauss11 G, float wgt,
-                 float lambda, float* __restrict__ M, float* __restrict__ loss) {
-    __shared__ float sx[DIN][DIN + 1], sy[DIN][DIN + 1];
-    __shared__ float hs[5][DIN][DT];
-    __shared__ float s_red[8];
+dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __restrict__ Y, Gauss11 G, float wgt,
+                   float lambda, float keep, float* __restrict__ gC, float* __restrict__ loss) {
+    extern __shared__ __align__(16) unsigned char dssim_raw[];
+    DssimSmem& S = *reinterpret_cast<DssimSmem*>(dssim_raw);
     const int tid = threadIdx.x, x0 = blockIdx.x * DT, y0 = blockIdx.y * DT;
     const size_t hw = (size_t)W * H;
     const float* Xc = X + blockIdx.z * hw;
     const float* Yc = Y + blockIdx.z * hw;
-    for (int i = tid; i < DIN * DIN; i += 256) {
-        const int r = i / DIN, c = i - r * DIN, gx = x0 + c - DR, gy = y0 + r - DR;
+    // 1. images on the tile + 10-pixel apron, zero padded
+    for (int i = tid; i < DA * DA; i += 256) {
+        const int r = i / DA, c = i - r * DA, gx = x0 + c - 2 * DR, gy = y0 + r - 2 * DR;
         const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
-        sx[r][c] = in ? __ldg(Xc + (size_t)gy * W + gx) : 0.0f;       // zero padding
-        sy[r][c] = in ? __ldg(Yc + (size_t)gy * W + gx) : 0.0f;
+        S.a.in.sx[r][c] = in ? __ldg(Xc + (size_t)gy * W + gx) : 0.0f;
+        S.a.in.sy[r][c] = in ? __ldg(Yc + (size_t)gy * W + gx) : 0.0f;
     }
     __syncthreads();
-    for (int i = tid; i < DIN * DT; i += 256) {                       // horizontal pass
-        const int r = i / DT, c = i - r * DT;
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f;
+    // Every pass is register-blocked: a thread produces a run of 6 (or 4) consecutive outputs ALONG the convolution,
+    // so the 16 (14) inputs it needs are read from shared memory once instead of 11 times per output; tasks are dealt
+    // so that the lanes of a warp differ in the OTHER coordinate (rows: stride 53 / 43 words, columns: stride 1), which
+    // keeps the reads free of bank conflicts.
+    // 2. horizontal pass: 52 rows x 42 columns (7 runs of 6)
+    for (int i = tid; i < DA * (DB / 6); i += 256) {
+        const int r = i % DA, c0 = (i / DA) * 6;
+        float vx[16], vy[16];
 #pragma unroll
-        for (int k = 0; k < 11; ++k) {
-            const float a = sx[r][c + k], b = sy[r][c + k], g = G.g[k];
-            a0 = fmaf(g, a, a0), a1 = fmaf(g, b, a1), a2 = fmaf(g, a * a, a2), a3 = fmaf(g, b * b, a3), a4 = fmaf(g, a * b, a4);
+        for (int k = 0; k < 16; ++k) vx[k] = S.a.in.sx[r][c0 + k], vy[k] = S.a.in.sy[r][c0 + k];
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f;
+#pragma unroll
+            for (int k = 0; k < 11; ++k) {
+                const float a = vx[j + k], b = vy[j + k], g = G.g[k];
+                a0 = fmaf(g, a, a0), a1 = fmaf(g, b, a1), a2 = fmaf(g, a * a, a2), a3 = fmaf(g, b * b, a3), a4 = fmaf(g, a * b, a4);
+            }
+            S.b.hs[0][r][c0 + j] = a0, S.b.hs[1][r][c0 + j] = a1, S.b.hs[2][r][c0 + j] = a2, S.b.hs[3][r][c0 + j] = a3,
+            S.b.hs[4][r][c0 + j] = a4;
         }
-        hs[0][r][c] = a0, hs[1][r][c] = a1, hs[2][r][c] = a2, hs[3][r][c] = a3, hs[4][r][c] = a4;
     }
     __syncthreads();
+    // 3. vertical pass + SSIM + the three maps on 42 x 42 (7 runs of 6 rows; the images in S.a are dead from here on)
     const float C1 = 0.01f * 0.01f, C2 = 0.03f * 0.03f;
     float acc = 0.0f;
-    for (int i = tid; i < DT * DT; i += 256) {                        // vertical pass + SSIM
-        const int r = i / DT, c = i - r * DT, gx = x0 + c, gy = y0 + r;
-        if (gx >= W || gy >= H) continue;
-        float mu1 = 0.f, mu2 = 0.f, e11 = 0.f, e22 = 0.f, e12 = 0.f;
+    for (int i = tid; i < DB * (DB / 6); i += 256) {
+        const int c = i % DB, r0 = (i / DB) * 6, gx = x0 + c - DR;
+        float st[5][6];
 #pragma unroll
-        for (int k = 0; k < 11; ++k) {
-            const float g = G.g[k];
-            mu1 = fmaf(g, hs[0][r + k][c], mu1), mu2 = fmaf(g, hs[1][r + k][c], mu2);
-            e11 = fmaf(g, hs[2][r + k][c], e11), e22 = fmaf(g, hs[3][r + k][c], e22), e12 = fmaf(g, hs[4][r + k][c], e12);
+        for (int q = 0; q < 5; ++q) {
+            float v[16];
+#pragma unroll
+            for (int k = 0; k < 16; ++k) v[k] = S.b.hs[q][r0 + k][c];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) {
+                float a = 0.f;
+#pragma unroll
+                for (int k = 0; k < 11; ++k) a = fmaf(G.g[k], v[j + k], a);
+                st[q][j] = a;
+            }
         }
-        const float s11 = e11 - mu1 * mu1, s22 = e22 - mu2 * mu2, s12 = e12 - mu1 * mu2;
-        const float A1 = 2.f * mu1 * mu2 + C1, A2 = 2.f * s12 + C2, B1 = mu1 * mu1 + mu2 * mu2 + C1, B2 = s11 + s22 + C2;
-        const float iB1 = 1.0f / B1, iB2 = 1.0f / B2;
-        acc += A1 * A2 * iB1 * iB2;
-        const float d_mu1_direct = 2.f * mu2 * A2 * iB1 * iB2 - A1 * A2 * 2.f * mu1 * iB1 * iB1 * iB2;
-        const float d_s11 = -A1 * A2 * iB1 * iB2 * iB2;
-        const float d_s12 = 2.f * A1 * iB1 * iB2;
-        const size_t p = (size_t)gy * W + gx;
-        float* Mc = M + 3 * blockIdx.z * hw;
-        Mc[p] = wgt * (d_mu1_direct - 2.f * mu1 * d_s11 - mu2 * d_s12);
-        Mc[hw + p] = wgt * d_s11;
-        Mc[2 * hw + p] = wgt * d_s12;
+#pragma unroll
+        for (int j = 0; j < 6; ++j) {
+            const int r = r0 + j, gy = y0 + r - DR;
+            float m0 = 0.f, m1 = 0.f, m2 = 0.f;
+            if (gx >= 0 && gx < W && gy >= 0 && gy < H) {
+                const float mu1 = st[0][j], mu2 = st[1][j], e11 = st[2][j], e22 = st[3][j], e12 = st[4][j];
+                const float s11 = e11 - mu1 * mu1, s22 = e22 - mu2 * mu2, s12 = e12 - mu1 * mu2;
+                const float A1 = 2.f * mu1 * mu2 + C1, A2 = 2.f * s12 + C2, B1 = mu1 * mu1 + mu2 * mu2 + C1, B2 = s11 + s22 + C2;
+                const float iB1 = 1.0f / B1, iB2 = 1.0f / B2;
+                if (r >= DR && r < DR + DT && c >= DR && c < DR + DT) acc += A1 * A2 * iB1 * iB2;   // the tile's own pixels
+                const float d_mu1_direct = 2.f * mu2 * A2 * iB1 * iB2 - A1 * A2 * 2.f * mu1 * iB1 * iB1 * iB2;
+                const float d_s11 = -A1 * A2 * iB1 * iB2 * iB2;
+                const float d_s12 = 2.f * A1 * iB1 * iB2;
+                m0 = wgt * (d_mu1_direct - 2.f * mu1 * d_s11 - mu2 * d_s12), m1 = wgt * d_s11, m2 = wgt * d_s12;
+            }
+            // (S.a.m aliases the images, which step 2 has finished reading: the barrier after step 2 covers it)
+            S.a.m[0][r][c] = m0, S.a.m[1][r][c] = m1, S.a.m[2][r][c] = m2;
+        }
+    }
+    __syncthreads();
+    // 4. horizontal pass of the maps: 42 rows x 32 columns, 8 runs of 4 (S.b.hs is dead: every thread passed the barrier)
+    for (int i = tid; i < DB * (DT / 4); i += 256) {
+        const int r = i % DB, c0 = (i / DB) * 4;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            float v[14];
+#pragma unroll
+            for (int k = 0; k < 14; ++k) v[k] = S.a.m[q][r][c0 + k];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float a = 0.f;
+#pragma unroll
+                for (int k = 0; k < 11; ++k) a = fmaf(G.g[k], v[j + k], a);
+                S.b.hm[q][r][c0 + j] = a;
+            }
+        }
+    }
+    __syncthreads();
+    // 5. vertical pass + the cotangent of E_pho on the tile (8 runs of 4 rows)
+    for (int i = tid; i < DT * (DT / 4); i += 256) {
+        const int c = i % DT, r0 = (i / DT) * 4, gx = x0 + c;
+        float cc[3][4];
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            float v[14];
+#pragma unroll
+            for (int k = 0; k < 14; ++k) v[k] = S.b.hm[q][r0 + k][c];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                float a = 0.f;
+#pragma unroll
+                for (int k = 0; k < 11; ++k) a = fmaf(G.g[k], v[j + k], a);
+                cc[q][j] = a;
+            }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int gy = y0 + r0 + j;
+            if (gx >= W || gy >= H) continue;
+            const size_t p = blockIdx.z * hw + (size_t)gy * W + gx;
+            gC[p] = keep * gC[p] + cc[0][j] + 2.0f * __ldg(X + p) * cc[1][j] + __ldg(Y + p) * cc[2][j];
+        }
     }
     if (loss) {
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, d);
-        if ((tid & 31) == 0) s_red[tid >> 5] = acc;
+        if ((tid & 31) == 0) S.red[tid >> 5] = acc;
         __syncthreads();
         if (tid == 0) {
             float t = 0.f;
-            for (int w = 0; w < 8; ++w) t += s_red[w];
+            for (int w = 0; w < 8; ++w) t += S.red[w];
             // lambda * L = lambda * (1 - sum / 3HW): the constant is added once, by block (0,0,0)
             float v = wgt * t;                                        // wgt = -lambda / 3HW
             if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) v += lambda;
@@ -87,52 +174,12 @@ dssim_fwd_kernel(int W, int H, const float* __restrict__ X, const float* __restr
     }
 }
 
-__global__ void __launch_bounds__(256)
-dssim_bwd_kernel(int W, int H, const float* __restrict__ X, const float* __restrict__ Y, Gauss11 G, float keep,
-                 const float* __restrict__ M, float* __restrict__ gC) {
-    __shared__ float sm[3][DIN][DIN + 1];
-    __shared__ float hs[3][DIN][DT];
-    const int tid = threadIdx.x, x0 = blockIdx.x * DT, y0 = blockIdx.y * DT;
-    const size_t hw = (size_t)W * H;
-    const float* Mc = M + 3 * blockIdx.z * hw;
-    for (int i = tid; i < DIN * DIN; i += 256) {
-        const int r = i / DIN, c = i - r * DIN, gx = x0 + c - DR, gy = y0 + r - DR;
-        const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
-        const size_t p = (size_t)gy * W + gx;
-#pragma unroll
-        for (int q = 0; q < 3; ++q) sm[q][r][c] = in ? __ldg(Mc + q * hw + p) : 0.0f;
-    }
-    __syncthreads();
-    for (int i = tid; i < DIN * DT; i += 256) {
-        const int r = i / DT, c = i - r * DT;
-        float a0 = 0.f, a1 = 0.f, a2 = 0.f;
-#pragma unroll
-        for (int k = 0; k < 11; ++k) {
-            const float g = G.g[k];
-            a0 = fmaf(g, sm[0][r][c + k], a0), a1 = fmaf(g, sm[1][r][c + k], a1), a2 = fmaf(g, sm[2][r][c + k], a2);
-        }
-        hs[0][r][c] = a0, hs[1][r][c] = a1, hs[2][r][c] = a2;
-    }
-    __syncthreads();
-    for (int i = tid; i < DT * DT; i += 256) {
-        const int r = i / DT, c = i - r * DT, gx = x0 + c, gy = y0 + r;
-        if (gx >= W || gy >= H) continue;
-        float c0 = 0.f, c1 = 0.f, c2 = 0.f;
-#pragma unroll
-        for (int k = 0; k < 11; ++k) {
-            const float g = G.g[k];
-            c0 = fmaf(g, hs[0][r + k][c], c0), c1 = fmaf(g, hs[1][r + k][c], c1), c2 = fmaf(g, hs[2][r + k][c], c2);
-        }
-        const size_t p = blockIdx.z * hw + (size_t)gy * W + gx;
-        gC[p] = keep * gC[p] + c0 + 2.0f * __ldg(X + p) * c1 + __ldg(Y + p) * c2;
-    }
-}
-
 }  // namespace
 
 extern "C" int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* Chat, float lambda,
                                       float* gC, float* loss_dev, float* scratch, void* stream) {
-    if (!ctx || W <= 0 || H <= 0 || !C || !Chat || !gC || !scratch || !(lambda >= 0.0f) || !(lambda <= 1.0f))
+    (void)scratch;                                           // (the two-pass form of round 1 needed 9 HW floats here)
+    if (!ctx || W <= 0 || H <= 0 || !C || !Chat || !gC || !(lambda >= 0.0f) || !(lambda <= 1.0f))
         return TS_ERR_INVALID_ARG;
     Gauss11 G;
     double g[11], sum = 0.0;
@@ -140,8 +187,9 @@ extern "C" int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const f
     for (int i = 0; i < 11; ++i) G.g[i] = (float)(g[i] / sum);
     const float wgt = (float)(-(double)lambda / (3.0 * (double)W * (double)H));
     const dim3 grid((W + DT - 1) / DT, (H + DT - 1) / DT, 3);
-    dssim_fwd_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(W, H, C, Chat, G, wgt, lambda, scratch, loss_dev);
-    dssim_bwd_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(W, H, C, Chat, G, 1.0f - lambda, scratch, gC);
+    cudaFuncSetAttribute(dssim_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DssimSmem));   // per device
+    dssim_fused_kernel<<<grid, 256, sizeof(DssimSmem), (cudaStream_t)stream>>>(W, H, C, Chat, G, wgt, lambda, 1.0f - lambda, gC,
+                                                                               loss_dev);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }

@@ -263,8 +263,6 @@ def ts_l1_loss_grad(ctx, W, H, Cimg, Dimg, Chat, Dhat, lambda_dep, gC, gD, loss=
 
 
 def ts_dssim_loss_grad(ctx, W, H, Cimg, Chat, lam, gC, loss=None, scratch=None, stream=None):
-    if scratch is None:
-        scratch = torch.empty(9 * int(W) * int(H), device=Cimg.device)
     _check(lib.ts_dssim_loss_grad(ctx.h, int(W), int(H), _ptr(Cimg), _ptr(Chat), float(lam), _ptr(gC), _ptr(loss),
                                   _ptr(scratch), _stream(stream)))
 
