@@ -8,7 +8,7 @@
 //   Eq. 4 front-to-back compositing in depth order    -> render_fwd()
 //   Eq. 5-7 analytic se(3) pose Jacobian              -> project_bwd()
 //   Eq. 12 rendered normal map                        -> face_normal(), render_fwd/bwd(nrm)
-// Step names F1..F8 / B1..B9 and readings S1..S26 / N1..N5 refer to DESIGN.md section 3.
+// Step names F1..F8 / B1..B9 and readings S1..S28 / N1..N11 refer to DESIGN.md section 2 (pins: section 3).
 // Build: g++ -std=c++17 -O2 -ffp-contract=off (no implicit FMA contraction; the float32
 // projection uses explicit std::fma where N1..N3 say so).
 #include "tso.h"

@@ -11,7 +11,11 @@ CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libts.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
-         "--fmad=true", "-Xptxas", "-v"]
+         "-Xptxas", "-v"]
+# The projection decides integers (cull set, pixel rects, depth keys, tile counts) that must equal the float32 oracle's
+# bit for bit: its translation unit is compiled WITHOUT implicit multiply-add contraction, so that a plain a * b + c
+# written there later cannot silently fuse; the fused operations of DESIGN.md N1-N3 are spelled __fmaf_rn.
+FMAD = {"ts_project.cu": "--fmad=false"}
 
 
 def sources():
@@ -32,7 +36,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     logs = []
     for src in sources():
         obj = os.path.join(CSRC, os.path.basename(src)[:-3] + ".o")
-        r = subprocess.run([NVCC, *FLAGS, "-c", src, "-o", obj], capture_output=True, text=True)
+        fmad = FMAD.get(os.path.basename(src), "--fmad=true")
+        r = subprocess.run([NVCC, *FLAGS, fmad, "-c", src, "-o", obj], capture_output=True, text=True)
         logs.append(r.stderr)
         if r.returncode != 0:
             sys.stderr.write(r.stdout + r.stderr)
