@@ -227,7 +227,7 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 const tso_params* prm, const uint8_t* visible, const int16_t* rect, const T* scr,
                 const uint32_t* list, int64_t n_list, const uint32_t* tile_ranges, T* oc, T* od, T* oa,
                 uint32_t* n_contrib, uint8_t* ambig, uint64_t* sig, uint64_t* counters, const T* nrm = nullptr,
-                T* on = nullptr) {
+                T* on = nullptr, T* on_top = nullptr) {
     const Cam<T> cam(cam_);
     const int W = cam.W, H = cam.H;
     const T sigma = (T)prm->sigma, amin = (T)prm->alpha_min, tmin = (T)prm->t_min, atol = (T)prm->amb_tol;
@@ -238,7 +238,7 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
         for (int x = 0; x < W; ++x) {
             int64_t b, e;
             LS.span(x, y, b, e);
-            T Tr = 1, C[3] = {0, 0, 0}, D = 0, Nv[3] = {0, 0, 0};
+            T Tr = 1, C[3] = {0, 0, 0}, D = 0, Nv[3] = {0, 0, 0}, Nt[3] = {0, 0, 0}, a_top = 0;
             uint32_t last = 0;
             bool amb = false;
             uint64_t sg = 1469598103934665603ull;
@@ -254,6 +254,10 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 for (int c = 0; c < 3; ++c) C[c] += wgt * h.c[c];
                 D += wgt * h.z;                                                // S11
                 if (nrm) for (int c = 0; c < 3; ++c) Nv[c] += wgt * nrm[3 * (int64_t)list[i] + c];   // S26
+                if (nrm && h.alpha > a_top) {                                  // S29: the first hit of the largest alpha
+                    a_top = h.alpha;
+                    for (int c = 0; c < 3; ++c) Nt[c] = nrm[3 * (int64_t)list[i] + c];
+                }
                 Tr = Tr * ((T)1 - h.alpha);
                 last = (uint32_t)(i - b + 1);
                 sg = (sg ^ (uint64_t)(list[i] + 1)) * 1099511628211ull;
@@ -265,6 +269,7 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
             if (od) od[p] = D;
             if (oa) oa[p] = (T)1 - Tr;
             if (on) for (int c = 0; c < 3; ++c) on[(int64_t)c * W * H + p] = Nv[c];
+            if (on_top) for (int c = 0; c < 3; ++c) on_top[(int64_t)c * W * H + p] = Nt[c];
             if (n_contrib) n_contrib[p] = last;
             if (ambig) ambig[p] = amb ? 1 : 0;
             if (sig) sig[p] = sg;
@@ -725,6 +730,22 @@ void left_perturb(const T* Tcw, const T* tau, T* out) {
 }  // namespace
 
 // ====================================================================================== C ABI
+// Normalised depth (E_dep of Eq. 9 / 13 compares a rendered depth with the sensor depth, and
+// D = sum z alpha T under-reads wherever A < 1): Dn = D / A where A > eps, else 0.  Backward of a cotangent gDn:
+// gD += gDn / A,  gA += -gDn D / A^2  (nothing where A <= eps).
+template <class T>
+void depth_normalise(int64_t n, const T* D, const T* A, T eps, T* Dn) {
+    for (int64_t i = 0; i < n; ++i) Dn[i] = A[i] > eps ? D[i] / A[i] : (T)0;
+}
+template <class T>
+void depth_normalise_bwd(int64_t n, const T* D, const T* A, T eps, const T* gDn, T* gD, T* gA) {
+    for (int64_t i = 0; i < n; ++i) {
+        if (!(A[i] > eps)) continue;
+        gD[i] += gDn[i] / A[i];
+        gA[i] += -gDn[i] * D[i] / (A[i] * A[i]);
+    }
+}
+
 extern "C" {
 
 int64_t tso_project_f32(const float* pos, const int32_t* faces, int32_t, int32_t M, const float* T_cw,
@@ -833,6 +854,15 @@ void tso_pose_step_f32(float* T_cw, const float* g, float* state, const float* l
     for (int i = 0; i < 12; ++i) T_cw[i] = T4[i];
 }
 
+void tso_depth_normalise_f32(int64_t n, const float* D, const float* A, float eps, float* Dn) { depth_normalise<float>(n, D, A, eps, Dn); }
+void tso_depth_normalise_f64(int64_t n, const double* D, const double* A, double eps, double* Dn) { depth_normalise<double>(n, D, A, eps, Dn); }
+void tso_depth_normalise_bwd_f32(int64_t n, const float* D, const float* A, float eps, const float* gDn, float* gD, float* gA) {
+    depth_normalise_bwd<float>(n, D, A, eps, gDn, gD, gA);
+}
+void tso_depth_normalise_bwd_f64(int64_t n, const double* D, const double* A, double eps, const double* gDn, double* gD, double* gA) {
+    depth_normalise_bwd<double>(n, D, A, eps, gDn, gD, gA);
+}
+
 void tso_left_perturb_f64(const double* T_cw, const double* tau, double* out) { left_perturb<double>(T_cw, tau, out); }
 
 double tso_equi_f32(const float* pos, const int32_t* faces, int32_t M, double weight, float* grad_pos) {
@@ -872,6 +902,13 @@ void tso_face_stats_f64(const double* color, const double* opacity, const int32_
                                      const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
                                      const uint32_t* tile_ranges, const T* nrm, T* out_normal) {                       \
         render_fwd<T>(TSO_FWD_ARGS, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nrm, out_normal);   \
+    }                                                                                                                  \
+    void tso_render_normal_top_##sfx(const T* color, const T* opacity, const int32_t* faces, int32_t M,                \
+                                     const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \
+                                     const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
+                                     const uint32_t* tile_ranges, const T* nrm, T* out_normal_top) {                   \
+        render_fwd<T>(TSO_FWD_ARGS, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nrm, nullptr,       \
+                      out_normal_top);                                                                                 \
     }                                                                                                                  \
     void tso_render_normal_bwd_##sfx(const T* color, const T* opacity, const int32_t* faces, int32_t M,                \
                                      const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \

@@ -151,6 +151,10 @@ void tso_face_stats_f64(const double* color, const double* opacity, const int32_
                                      const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \
                                      const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
                                      const uint32_t* tile_ranges, const T* nrm, T* out_normal);                        \
+    void tso_render_normal_top_##sfx(const T* color, const T* opacity, const int32_t* faces, int32_t M,                \
+                                     const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \
+                                     const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
+                                     const uint32_t* tile_ranges, const T* nrm, T* out_normal_top);                    \
     void tso_render_normal_bwd_##sfx(const T* color, const T* opacity, const int32_t* faces, int32_t M,                \
                                      const tso_camera* cam, const tso_params* prm, const uint8_t* visible,             \
                                      const int16_t* rect, const T* scr, const uint32_t* list, int64_t n_list,          \
@@ -158,6 +162,17 @@ void tso_face_stats_f64(const double* color, const double* opacity, const int32_
                                      T* g_scr, T* g_nrm);
 TSO_NRM_DECL(float, f32)
 TSO_NRM_DECL(double, f64)
+
+/* tso_render_normal_top (above): the "normal direction of the triangle with highest opacity along each ray" of Fig. 3
+ * (PAPER.md:145), reading S29: among the hits the walk composites (same hit rule and termination), the face
+ * normal of the FIRST hit with the largest alpha = face opacity x window; zero where nothing is hit.  Forward only.
+ *
+ * Normalised depth D / A: Dn = D / A where A > eps, else 0; backward of a cotangent gDn:
+ * gD += gDn / A, gA += -gDn D / A^2.  n = H W elements. */
+void tso_depth_normalise_f32(int64_t n, const float* D, const float* A, float eps, float* Dn);
+void tso_depth_normalise_f64(int64_t n, const double* D, const double* A, double eps, double* Dn);
+void tso_depth_normalise_bwd_f32(int64_t n, const float* D, const float* A, float eps, const float* gDn, float* gD, float* gA);
+void tso_depth_normalise_bwd_f64(int64_t n, const double* D, const double* A, double eps, const double* gDn, double* gD, double* gA);
 
 /* E_norm of Eq. 12: weight / (H W) * sum over valid pixels (Nbar_p != 0) of 1 - N_p . Nbar_p
  * (reading S27).  N, Nbar, gN are [3][H][W]; gN receives the cotangent of N; returns the weighted loss. */

@@ -216,6 +216,17 @@ class Oracle:
             _p(pr.visible), _p(pr.rect), _p(pr.scr), _p(lst), C.c_int64(lst.shape[0]), _p(ranges), _p(nrm), _p(N))
         return N
 
+    def normal_top(self, mode="tiled"):
+        """Normal of the highest-opacity hit along each ray (Fig. 3 right, reading S29)."""
+        pr = self.project()
+        lst, ranges = self._lists(mode)
+        nrm = self.face_normals()
+        N = np.zeros((3, self.H, self.W), self.dt)
+        self._fn("tso_render_normal_top")(
+            _p(self.color), _p(self.opacity), _p(self.faces), C.c_int32(self.M), C.byref(self.cam), C.byref(self.prm),
+            _p(pr.visible), _p(pr.rect), _p(pr.scr), _p(lst), C.c_int64(lst.shape[0]), _p(ranges), _p(nrm), _p(N))
+        return N
+
     def normal_backward(self, gN, mode="tiled", want=("pos", "opacity", "pose")):
         """Gradient of sum(gN * N): grad_pos (window path through B7-B8 plus the normal's own dependence on the
         vertices), grad_opacity, dL_dtau."""
@@ -278,6 +289,24 @@ def dssim(x, y, prec="f64", grad=True):
     g = np.zeros_like(x) if grad else None
     L = getattr(lib(), "tso_dssim_" + prec)(C.c_int32(x.shape[2]), C.c_int32(x.shape[1]), _p(x), _p(y), _p(g))
     return L, g
+
+
+def depth_normalise(D, A, eps=1e-6, prec="f64"):
+    dt = np.float32 if prec == "f32" else np.float64
+    D, A = np.ascontiguousarray(D, dt), np.ascontiguousarray(A, dt)
+    out = np.zeros_like(D)
+    ce = C.c_float(eps) if prec == "f32" else C.c_double(eps)
+    getattr(lib(), "tso_depth_normalise_" + prec)(C.c_int64(D.size), _p(D), _p(A), ce, _p(out))
+    return out
+
+
+def depth_normalise_bwd(D, A, gDn, eps=1e-6, prec="f64"):
+    dt = np.float32 if prec == "f32" else np.float64
+    D, A, gDn = (np.ascontiguousarray(x, dt) for x in (D, A, gDn))
+    gD, gA = np.zeros_like(D), np.zeros_like(D)
+    ce = C.c_float(eps) if prec == "f32" else C.c_double(eps)
+    getattr(lib(), "tso_depth_normalise_bwd_" + prec)(C.c_int64(D.size), _p(D), _p(A), ce, _p(gDn), _p(gD), _p(gA))
+    return gD, gA
 
 
 def left_perturb(T_cw, tau):
