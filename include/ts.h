@@ -197,6 +197,21 @@ int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame
                              const float* dL_ddepth, const float* dL_dalpha, const float* dL_dnormal, float* grad_pos,
                              float* grad_color, float* grad_opacity, uint32_t grad_mask, void* stream);
 
+/* The "normal direction of the triangle with highest opacity along each ray" of Fig. 3 (
+ * DESIGN.md reading S29): as ts_render_fwd_normal, plus out_normal_top[3][H][W] (device, required) = the camera-space
+ * unit normal of the FIRST hit with the largest alpha (face opacity x window) among the hits the walk composites; zero
+ * where nothing is hit.  Forward only (a visualisation: piecewise constant, no gradient).  out_normal may be NULL. */
+int32_t ts_render_fwd_normal_top(ts_ctx* ctx, const ts_scene* scene, ts_frame* frame, float* out_color, float* out_depth,
+                                 float* out_alpha, float* out_normal, float* out_normal_top, void* stream);
+
+/* Normalised depth (E_dep compares a rendered depth with the sensor
+ * depth, and D = sum z alpha T under-reads wherever A < 1).  ts_depth_normalise: Dn = D / A where A > eps, else 0.
+ * ts_depth_normalise_bwd: given the cotangent gDn of Dn, gD += gDn / A and gA += -gDn D / A^2 (where A > eps); gD, gA are
+ * then the dL_ddepth / dL_dalpha of ts_render_bwd (they accumulate: the caller initialises them).  [H][W] device arrays. */
+int32_t ts_depth_normalise(ts_ctx* ctx, int32_t W, int32_t H, const float* D, const float* A, float eps, float* Dn, void* stream);
+int32_t ts_depth_normalise_bwd(ts_ctx* ctx, int32_t W, int32_t H, const float* D, const float* A, float eps, const float* gDn,
+                               float* gD, float* gA, void* stream);
+
 /* E_norm of E_map (Eq. 12 and 15; lambda_norm = 0.05): weight / (H W) * sum over the
  * valid pixels (those with a sensor normal, Nbar_p != 0) of 1 - N_p . Nbar_p (reading S27).  N = the map of
  * ts_render_fwd_normal, Nbar = sensor normals, both [3][H][W] device.  Writes gN[3][H][W] = the cotangent of N (input of

@@ -254,6 +254,19 @@ int32_t ts_render_fwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, floa
     return s;
 }
 
+int32_t ts_render_fwd_normal_top(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
+                                 float* out_alpha, float* out_normal, float* out_normal_top, void* stream) {
+    if (!ctx || !sc || !fr || !sc->color || !sc->pos || !out_normal_top) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
+    if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
+    if (!fr->have_sort) return TS_ERR_STATE;
+    const int32_t s = ts_launch_render_fwd_normal(ctx, fr, sc, out_color, out_depth, out_alpha, out_normal, (cudaStream_t)stream,
+                                                  out_normal_top);
+    fr->have_fwd = (s == TS_OK);
+    fr->have_normals = (s == TS_OK);
+    return s;
+}
+
 int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
                              const float* dL_dalpha, const float* dL_dnormal, float* grad_pos, float* grad_color,
                              float* grad_opacity, uint32_t grad_mask, void* stream) {

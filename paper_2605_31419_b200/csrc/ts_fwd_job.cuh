@@ -14,6 +14,7 @@ struct FwdPix {                       // what the walk leaves for this lane's pi
     float T, C0, C1, C2, D, Tlast;
     uint32_t last;
     float N0, N1, N2;                 // composited face normals (NRM instantiation only)
+    float Nt0, Nt1, Nt2;              // normal of the first hit with the largest alpha (NRM instantiation only; reading S29)
 };
 
 // `ent` = the lane's entry of the first 32-entry chunk of the tile list (already requested by the caller, so that
@@ -32,7 +33,7 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
                                             float4* nsm = nullptr, uint32_t* staged_lo = nullptr) {
     const float fpx = (float)job.px, fpy = (float)job.py;
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, D = 0.0f, Tlast = 1.0f;
-    float N0 = 0.0f, N1 = 0.0f, N2 = 0.0f;
+    float N0 = 0.0f, N1 = 0.0f, N2 = 0.0f, Nt0 = 0.0f, Nt1 = 0.0f, Nt2 = 0.0f, a_top = 0.0f;
     uint32_t last = 0;
     const uint32_t lt = (1u << lane) - 1u;
     (void)lt;
@@ -108,6 +109,7 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
                 if (NRM) {
                     const float4 nf = nsm[e];
                     N0 = fmaf(wgt, nf.x, N0), N1 = fmaf(wgt, nf.y, N1), N2 = fmaf(wgt, nf.z, N2);
+                    if (alpha > a_top) a_top = alpha, Nt0 = nf.x, Nt1 = nf.y, Nt2 = nf.z;     // Fig. 3 (right), reading S29
                 }
                 Tlast = T;
                 T = __fmul_rn(T, __fsub_rn(1.0f, alpha));
@@ -118,5 +120,5 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
         warp_done = __all_sync(0xffffffffu, done);      // once per chunk: pixels rarely all terminate inside one
     }
     o.T = T, o.C0 = C0, o.C1 = C1, o.C2 = C2, o.D = D, o.Tlast = Tlast, o.last = last;
-    if (NRM) o.N0 = N0, o.N1 = N1, o.N2 = N2;
+    if (NRM) o.N0 = N0, o.N1 = N1, o.N2 = N2, o.Nt0 = Nt0, o.Nt1 = Nt1, o.Nt2 = Nt2;
 }

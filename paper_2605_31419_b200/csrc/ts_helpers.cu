@@ -183,6 +183,49 @@ extern "C" int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dt
     return TS_OK;
 }
 
+// Normalised depth D / A (E_dep of Eq. 9 / 13 compares a rendered depth with the sensor depth, and
+// D = sum z alpha T under-reads wherever A < 1): elementwise, HBM-bound.
+namespace {
+__global__ void __launch_bounds__(256) depth_normalise_kernel(size_t n, const float* __restrict__ D, const float* __restrict__ A,
+                                                              float eps, float* __restrict__ Dn) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float a = A[i];
+        Dn[i] = a > eps ? __fdiv_rn(D[i], a) : 0.0f;
+    }
+}
+__global__ void __launch_bounds__(256) depth_normalise_bwd_kernel(size_t n, const float* __restrict__ D, const float* __restrict__ A,
+                                                                  float eps, const float* __restrict__ gDn, float* __restrict__ gD,
+                                                                  float* __restrict__ gA) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float a = A[i];
+        if (!(a > eps)) continue;
+        const float g = gDn[i], ia = __fdiv_rn(1.0f, a);
+        gD[i] += g * ia;
+        gA[i] += -g * D[i] * ia * ia;
+    }
+}
+}  // namespace
+
+extern "C" int32_t ts_depth_normalise(ts_ctx* ctx, int32_t W, int32_t H, const float* D, const float* A, float eps, float* Dn,
+                                      void* stream) {
+    if (!ctx || W <= 0 || H <= 0 || !D || !A || !Dn || !(eps >= 0.0f)) return TS_ERR_INVALID_ARG;
+    const size_t n = (size_t)W * H;
+    const int grid = (int)((n + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n + 255) / 256 : (size_t)ctx->num_sms * 8);
+    depth_normalise_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(n, D, A, eps, Dn);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
+
+extern "C" int32_t ts_depth_normalise_bwd(ts_ctx* ctx, int32_t W, int32_t H, const float* D, const float* A, float eps,
+                                          const float* gDn, float* gD, float* gA, void* stream) {
+    if (!ctx || W <= 0 || H <= 0 || !D || !A || !gDn || !gD || !gA || !(eps >= 0.0f)) return TS_ERR_INVALID_ARG;
+    const size_t n = (size_t)W * H;
+    const int grid = (int)((n + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n + 255) / 256 : (size_t)ctx->num_sms * 8);
+    depth_normalise_bwd_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(n, D, A, eps, gDn, gD, gA);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}
+
 // Measurement helper ("measure a dependent-free FMA loop and print both nominal and measured
 // peaks"): every thread runs `iters` rounds of eight independent FMA chains; 16 flops per thread and round.
 namespace {

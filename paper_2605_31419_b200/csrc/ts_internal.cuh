@@ -109,7 +109,7 @@ int32_t ts_launch_render_fwd(const ts_ctx*, ts_frame*, const ts_scene*, float* o
                              cudaStream_t);
 int32_t ts_launch_face_area(const ts_ctx*, ts_frame*, float* area, cudaStream_t);
 int32_t ts_launch_render_fwd_normal(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, float* on,
-                                    cudaStream_t);
+                                    cudaStream_t, float* on_top = nullptr);
 int32_t ts_launch_render_bwd_normal(const ts_ctx*, ts_frame*, const ts_scene*, const float* gC, const float* gD,
                                     const float* gA, const float* gN, float* grad_pos, float* grad_color,
                                     float* grad_opacity, uint32_t mask, cudaStream_t);

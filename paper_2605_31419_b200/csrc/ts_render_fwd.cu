@@ -25,7 +25,7 @@ template <int SM, bool COUNT, bool LOSS, bool STATS, bool NRM = false>
 __global__ void __launch_bounds__(TS_JOB_WARPS * 32)
 render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float t_min, float* __restrict__ out_color,
                   float* __restrict__ out_depth, float* __restrict__ out_alpha, FwdLoss L, uint32_t* __restrict__ face_pixels,
-                  float* __restrict__ out_normal = nullptr) {
+                  float* __restrict__ out_normal = nullptr, float* __restrict__ out_normal_top = nullptr) {
     __shared__ FwdWarpSmem smem[TS_JOB_WARPS];
     __shared__ float4 smem_n[NRM ? TS_JOB_WARPS * 32 : 1];
     const int lane = threadIdx.x & 31;
@@ -52,7 +52,8 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
             if (out_color) out_color[p] = C0, out_color[hw + p] = C1, out_color[2 * hw + p] = C2;
             if (out_depth) out_depth[p] = D;
             if (out_alpha) out_alpha[p] = 1.0f - T;
-            if (NRM) out_normal[p] = o.N0, out_normal[hw + p] = o.N1, out_normal[2 * hw + p] = o.N2;
+            if (NRM && out_normal) out_normal[p] = o.N0, out_normal[hw + p] = o.N1, out_normal[2 * hw + p] = o.N2;
+            if (NRM && out_normal_top) out_normal_top[p] = o.Nt0, out_normal_top[hw + p] = o.Nt1, out_normal_top[2 * hw + p] = o.Nt2;
             f.n_contrib[p] = last;
             f.t_last[p] = Tlast;
             if (LOSS) {
@@ -147,7 +148,7 @@ face_normal_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* _
 }  // namespace
 
 int32_t ts_launch_render_fwd_normal(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
-                                    float* on, cudaStream_t st) {
+                                    float* on, cudaStream_t st, float* on_top) {
     const TsFrameDev& f = fr->d;
     if (sc->faces == nullptr) face_normal_kernel<true><<<ctx->num_sms * 4, 256, 0, st>>>(f, sc->pos, nullptr, fr->T_cw);
     else face_normal_kernel<false><<<ctx->num_sms * 4, 256, 0, st>>>(f, sc->pos, sc->faces, fr->T_cw);
@@ -155,10 +156,10 @@ int32_t ts_launch_render_fwd_normal(const ts_ctx* ctx, ts_frame* fr, const ts_sc
     const float sg = fr->prm.sigma, am = fr->prm.alpha_min, tm = fr->prm.t_min;
     const FwdLoss none = {nullptr, nullptr, nullptr, nullptr, nullptr, 0.f, 0.f};
     switch (ts_sigma_mode(fr->prm.sigma)) {
-        case 1: render_fwd_kernel<1, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on); break;
-        case 2: render_fwd_kernel<2, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on); break;
-        case 3: render_fwd_kernel<3, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on); break;
-        default: render_fwd_kernel<0, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on); break;
+        case 1: render_fwd_kernel<1, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on, on_top); break;
+        case 2: render_fwd_kernel<2, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on, on_top); break;
+        case 3: render_fwd_kernel<3, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on, on_top); break;
+        default: render_fwd_kernel<0, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on, on_top); break;
     }
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;

@@ -28,7 +28,7 @@ EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_map_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
            "ts_render_fwd_normal", "ts_render_bwd_normal", "ts_normal_loss_grad", "ts_render_bwd_stats",
            "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view",
-           "ts_fp32_probe"]
+           "ts_fp32_probe", "ts_render_fwd_normal_top", "ts_depth_normalise", "ts_depth_normalise_bwd"]
 
 
 class TsError(RuntimeError):
@@ -100,6 +100,11 @@ def _load():
                                     C.POINTER(C.c_uint64), C.c_void_p]
     lib.ts_frame_view.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.POINTER(C.c_void_p), C.POINTER(C.c_size_t),
                                   C.c_void_p]
+    lib.ts_render_fwd_normal_top.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                             C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_depth_normalise.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p]
+    lib.ts_depth_normalise_bwd.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
+                                           C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_fp32_probe.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.POINTER(C.c_uint64), C.c_void_p]
     lib.ts_frame_release.argtypes = [C.c_void_p]
     lib.ts_destroy.argtypes = [C.c_void_p]
@@ -280,6 +285,20 @@ def ts_pose_reduce_step(ctx, frame, dL_dtau, T_cw, state, lr6, beta1=0.9, beta2=
     lr = (C.c_float * 6)(*[float(x) for x in lr6])
     _check(lib.ts_pose_reduce_step(ctx.h, frame.h, _ptr(dL_dtau), _ptr(T_cw), _ptr(state), lr, beta1, beta2, eps,
                                    _stream(stream)))
+
+
+def ts_render_fwd_normal_top(ctx, scene, frame, out_color, out_depth, out_alpha, out_normal, out_normal_top, stream=None):
+    _check(lib.ts_render_fwd_normal_top(ctx.h, C.byref(scene.c), frame.h, _ptr(out_color), _ptr(out_depth), _ptr(out_alpha),
+                                        _ptr(out_normal), _ptr(out_normal_top), _stream(stream)))
+
+
+def ts_depth_normalise(ctx, W, H, D, A, eps, Dn, stream=None):
+    _check(lib.ts_depth_normalise(ctx.h, int(W), int(H), _ptr(D), _ptr(A), float(eps), _ptr(Dn), _stream(stream)))
+
+
+def ts_depth_normalise_bwd(ctx, W, H, D, A, eps, gDn, gD, gA, stream=None):
+    _check(lib.ts_depth_normalise_bwd(ctx.h, int(W), int(H), _ptr(D), _ptr(A), float(eps), _ptr(gDn), _ptr(gD), _ptr(gA),
+                                      _stream(stream)))
 
 
 def ts_fp32_probe(ctx, iters, scratch, stream=None):

@@ -791,3 +791,58 @@ def test_render_map_l1_equals_separate_calls(ctx, oracle_mod, cfg):
     with pytest.raises(ts.TsError):
         ts.ts_render_bwd(ctx, g.scene, g.frame, gC, gD, None, gp1, None, None, ts.GRAD_POS)      # no walk state after map
     g.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 2, 3])
+def test_normalised_depth_and_top_normal(ctx, oracle_mod, cfg):
+    """NEXT-2 remainder: Dn = D / A with its backward pass through ts_render_bwd (gD, gA cotangents), and the normal of
+    the highest-opacity hit (Fig. 3, reading S29), against the oracle."""
+    from gpu_util import assert_grad_close, assert_images_close, dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(cfg)
+    o, g = both(ctx, oracle_mod, sc)
+    f, ok = check_forward(o, g)
+    H, W, V = g.H, g.W, sc.pos.shape[0]
+    eps = 1e-3
+    # forward: elementwise on the GPU's own images against the oracle routine on the same images (exact division), and
+    # against the oracle's own chain to the image tolerance where A is not tiny
+    Dn = torch.empty_like(g.D)
+    ts.ts_depth_normalise(ctx, W, H, g.D, g.A, eps, Dn)
+    torch.cuda.synchronize()
+    Dg, Ag = g.D.cpu().numpy(), g.A.cpu().numpy()
+    assert np.array_equal(Dn.cpu().numpy(), oracle_mod.depth_normalise(Dg, Ag, eps, "f32"))
+    ref_dn = oracle_mod.depth_normalise(f.depth, f.alpha, eps, "f32")
+    solid = ok & (f.alpha > 0.05) & (Ag > 0.05)
+    assert solid.mean() > 0.05
+    assert_images_close("normalised depth", Dn.cpu().numpy(), ref_dn, solid, scale=float(np.abs(ref_dn).max()), tol=2e-4)
+    # backward: cotangent of Dn -> (gD, gA) -> ts_render_bwd, against the oracle chain fed with the same cotangent
+    rng = np.random.default_rng(60 + cfg)
+    gDn = (rng.normal(size=(H, W)) * solid).astype(np.float32)
+    gD, gA = torch.zeros(H, W, device="cuda"), torch.zeros(H, W, device="cuda")
+    ts.ts_depth_normalise_bwd(ctx, W, H, g.D, g.A, eps, dev(gDn), gD, gA)
+    gDo, gAo = oracle_mod.depth_normalise_bwd(f.depth, f.alpha, gDn, eps, "f32")
+    torch.cuda.synchronize()
+    assert np.allclose(gD.cpu().numpy(), gDo, rtol=2e-4, atol=2e-4 * np.abs(gDo).max())
+    assert np.allclose(gA.cpu().numpy(), gAo, rtol=5e-4, atol=5e-4 * np.abs(gAo).max())
+    ref = o.backward(None, gDo, gAo)
+    gp, gc, go = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+    ts.ts_render_bwd(ctx, g.scene, g.frame, None, dev(gDo), dev(gAo), gp, gc, go, ts.GRAD_ALL)
+    tau = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau)
+    torch.cuda.synchronize()
+    assert_grad_close("grad_pos (D/A)", gp.cpu().numpy(), ref.grad_pos)
+    assert_grad_close("grad_opacity (D/A)", go.cpu().numpy(), ref.grad_opacity)
+    assert np.abs(tau.cpu().numpy() - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max()
+    # top normal: a flat per-face attribute picked by an argmax over alphas: equal wherever the argmax is not a
+    # near-tie between the two float32 implementations (pixels whose top alpha leads by less than 1e-4 are skipped)
+    N, Nt = torch.empty(3, H, W, device="cuda"), torch.empty(3, H, W, device="cuda")
+    ts.ts_render_fwd_normal_top(ctx, g.scene, g.frame, None, None, None, N, Nt)
+    torch.cuda.synchronize()
+    top_ref, N_ref = o.normal_top("tiled"), o.normal_forward("tiled")
+    assert_images_close("normal map", N.cpu().numpy(), N_ref, ok[None])
+    d = np.abs(Nt.cpu().numpy() - top_ref).max(axis=0)
+    bad = (d > 1e-5) & ok
+    print(f"top normal differs on {bad.sum()} of {ok.sum()} pixels (argmax near-ties)")
+    assert bad.sum() <= 2 + 2e-4 * ok.size
+    assert np.abs(np.linalg.norm(top_ref, axis=0)[f.n_contrib > 0] - 1.0).max() < 1e-5
+    g.close()
