@@ -684,6 +684,12 @@ def bench_mapping(args, torch, ts, scenes, dist, rank, world, local):
     if dist is not None:
         dist.barrier()
     ms_per_step = total_ms / args.steps
+    if args.skip_extras:
+        clk.stop()
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": n_views * HW / (ms_per_step * 1e-3) / 1e6, "unit": "Mpix/s",
+                              "ms_per_step": ms_per_step, "steps": args.steps, "partial": True}))
+        return
     stage_ms = hz.stage_times(mp.stages(), max(10, args.steps // 2))
     clocks = clk.stop()
     p_fp32_meas = measure_fp32_peak(ts, mp.ctx, torch, stream)
