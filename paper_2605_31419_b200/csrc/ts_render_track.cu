@@ -232,22 +232,13 @@ render_track_log_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min,
     const size_t hw = (size_t)f.W * f.H;
     float loss_acc = 0.0f;
 
-#ifdef TS_STATIC_JOBS
-    const uint32_t n_warps = gridDim.x * TS_JOB_WARPS;
-    uint32_t j = (threadIdx.x >> 5) * gridDim.x + blockIdx.x;
-#else
     uint32_t j = ts_job_take(f, 0, lane);
-#endif
     while (j < n_jobs) {
         TsJob job;
         ts_job_decode(f, j, lane, job);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
         if (job.range.x + lane < job.range.y) ent = f.sorted[job.range.x + lane];
-#ifdef TS_STATIC_JOBS
-        j += n_warps;
-#else
         j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
-#endif
         FwdPix o;
         uint32_t used, mylast;
         tl_fwd_walk<SM, CAP>(f, sc, job, lane, sm.log, sigma, alpha_min, t_min, ent, o, used, mylast);
@@ -294,9 +285,7 @@ render_track_log_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min,
         }
         __syncwarp();
     }
-#ifndef TS_STATIC_JOBS
     ts_job_finish(f, 0, lane);
-#endif
     if (loss) {
 #pragma unroll
         for (int d = 16; d > 0; d >>= 1) loss_acc += __shfl_xor_sync(TL_FULL, loss_acc, d);
