@@ -43,6 +43,40 @@ inline T signed_area(const T u[3], const T v[3]) {
 }
 
 // ---------------------------------------------------------------------------------- F1..F6
+// S31 (tight binning): does the triangle meet the box of pixel centres [bx0,bx1] x [by0,by1]?
+// For each edge k (from q_{k+1} to q_{k+2}) the un-normalised outward edge function
+//     E_k(p) = s (ey (px - ua) - ex (py - va)),   s = sign(S),
+// is taken at the corner of the box where it is smallest; the box is left out iff some E_k there exceeds
+// 2^-10 (|ex| + |ey|), i.e. every pixel of the box is at least ~1e-3 px OUTSIDE edge k: none of them can pass the hit
+// rule x > 0.  Conservative (the separating axes of the box itself are covered by the rect); fixed operation order, so
+// that two float32 implementations agree bit for bit.
+template <class T>
+bool tile_overlaps(const T* u, const T* v, int bx0, int by0, int bx1, int by1) {
+    const T a = u[1] - u[0], b = v[2] - v[0], c = v[1] - v[0], d = u[2] - u[0];
+    const T S = std::fma(a, b, -(c * d));
+    const T s = S > 0 ? (T)1 : (T)-1;
+    for (int k = 0; k < 3; ++k) {
+        const int ia = (k + 1) % 3, ib = (k + 2) % 3;
+        const T ex = u[ib] - u[ia], ey = v[ib] - v[ia];
+        const T sx = s * ey, sy = -(s * ex);
+        const T px = sx > 0 ? (T)bx0 : (T)bx1, py = sy > 0 ? (T)by0 : (T)by1;
+        const T dx = px - u[ia], dy = py - v[ia];
+        const T E = std::fma(sx, dx, sy * dy);
+        const T margin = (T)0.0009765625 * (std::fabs(ex) + std::fabs(ey));
+        if (E > margin) return false;
+    }
+    return true;
+}
+
+// tiles of the rect that the face is binned into: all of them, or (tight) those its triangle meets
+template <class T>
+bool tile_included(bool tight, const T* u, const T* v, const int16_t* rc, int tx, int ty) {
+    if (!tight) return true;
+    const int bx0 = std::max((int)rc[0], tx * 16), bx1 = std::min((int)rc[2], tx * 16 + 15);
+    const int by0 = std::max((int)rc[1], ty * 16), by1 = std::min((int)rc[3], ty * 16 + 15);
+    return tile_overlaps<T>(u, v, bx0, by0, bx1, by1);
+}
+
 template <class T>
 int64_t project(const T* pos, const int32_t* faces, int32_t M, const T* Tcw, const tso_camera* cam_,
                 const tso_params* prm, uint8_t* visible, int16_t* rect, uint32_t* depth_key,
@@ -97,7 +131,13 @@ int64_t project(const T* pos, const int32_t* faces, int32_t M, const T* Tcw, con
         rect[4 * m + 2] = (int16_t)x1, rect[4 * m + 3] = (int16_t)y1;
         depth_key[m] = bits;
         zbar[m] = zb;
-        tiles_touched[m] = (uint32_t)(((x1 >> 4) - (x0 >> 4) + 1) * ((y1 >> 4) - (y0 >> 4) + 1));
+        {
+            uint32_t nt = 0;
+            const int16_t* rc = rect + 4 * (int64_t)m;
+            for (int ty = y0 >> 4; ty <= (y1 >> 4); ++ty)
+                for (int tx = x0 >> 4; tx <= (x1 >> 4); ++tx) nt += tile_included<T>(prm->tight_binning != 0, u, v, rc, tx, ty) ? 1u : 0u;
+            tiles_touched[m] = nt;
+        }
         for (int k = 0; k < 3; ++k) {
             scr[9 * m + 3 * k + 0] = u[k], scr[9 * m + 3 * k + 1] = v[k], scr[9 * m + 3 * k + 2] = w[k];
             Q[9 * m + 3 * k + 0] = X[k], Q[9 * m + 3 * k + 1] = Y[k], Q[9 * m + 3 * k + 2] = Z[k];
@@ -746,6 +786,35 @@ void depth_normalise_bwd(int64_t n, const T* D, const T* A, T eps, const T* gDn,
     }
 }
 
+template <class T>
+int64_t bin_sort_impl(int32_t M, int32_t W, int32_t H, const uint8_t* visible, const int16_t* rect, const uint32_t* depth_key,
+                      const T* scr, int tight, uint64_t* keys, uint32_t* vals, uint32_t* ranges) {
+    const int tiles_x = (W + 15) / 16, tiles_y = (H + 15) / 16, NT = tiles_x * tiles_y;
+    struct KV { uint64_t k; uint32_t v; };
+    std::vector<KV> pairs;
+    for (int m = 0; m < M; ++m) {
+        if (!visible[m]) continue;
+        const int16_t* rc = rect + 4 * (int64_t)m;
+        T u[3] = {0, 0, 0}, v[3] = {0, 0, 0};
+        if (tight)
+            for (int k = 0; k < 3; ++k) u[k] = scr[9 * (int64_t)m + 3 * k], v[k] = scr[9 * (int64_t)m + 3 * k + 1];
+        for (int ty = rc[1] >> 4; ty <= (rc[3] >> 4); ++ty)
+            for (int tx = rc[0] >> 4; tx <= (rc[2] >> 4); ++tx)
+                if (tile_included<T>(tight != 0, u, v, rc, tx, ty))
+                    pairs.push_back({((uint64_t)(ty * tiles_x + tx) << 32) | depth_key[m], (uint32_t)m});
+    }
+    std::stable_sort(pairs.begin(), pairs.end(), [](const KV& a, const KV& b) { return a.k < b.k; });
+    for (int t = 0; t < 2 * NT; ++t) ranges[t] = 0;
+    const int64_t P = (int64_t)pairs.size();
+    for (int64_t i = 0; i < P; ++i) {
+        keys[i] = pairs[i].k, vals[i] = pairs[i].v;
+        uint32_t t = (uint32_t)(pairs[i].k >> 32);
+        if (i == 0 || (uint32_t)(pairs[i - 1].k >> 32) != t) ranges[2 * t] = (uint32_t)i;
+        ranges[2 * t + 1] = (uint32_t)(i + 1);
+    }
+    return P;
+}
+
 extern "C" {
 
 int64_t tso_project_f32(const float* pos, const int32_t* faces, int32_t, int32_t M, const float* T_cw,
@@ -763,26 +832,15 @@ int64_t tso_bin_sort(int32_t M, int32_t W, int32_t H, const uint8_t* visible, co
                      const uint32_t* depth_key, const uint32_t* tiles_touched, uint64_t* keys, uint32_t* vals,
                      uint32_t* ranges) {
     (void)tiles_touched;
-    const int tiles_x = (W + 15) / 16, tiles_y = (H + 15) / 16, NT = tiles_x * tiles_y;
-    struct KV { uint64_t k; uint32_t v; };
-    std::vector<KV> pairs;
-    for (int m = 0; m < M; ++m) {
-        if (!visible[m]) continue;
-        const int16_t* rc = rect + 4 * (int64_t)m;
-        for (int ty = rc[1] >> 4; ty <= (rc[3] >> 4); ++ty)
-            for (int tx = rc[0] >> 4; tx <= (rc[2] >> 4); ++tx)
-                pairs.push_back({((uint64_t)(ty * tiles_x + tx) << 32) | depth_key[m], (uint32_t)m});
-    }
-    std::stable_sort(pairs.begin(), pairs.end(), [](const KV& a, const KV& b) { return a.k < b.k; });
-    for (int t = 0; t < 2 * NT; ++t) ranges[t] = 0;
-    const int64_t P = (int64_t)pairs.size();
-    for (int64_t i = 0; i < P; ++i) {
-        keys[i] = pairs[i].k, vals[i] = pairs[i].v;
-        uint32_t t = (uint32_t)(pairs[i].k >> 32);
-        if (i == 0 || (uint32_t)(pairs[i - 1].k >> 32) != t) ranges[2 * t] = (uint32_t)i;
-        ranges[2 * t + 1] = (uint32_t)(i + 1);
-    }
-    return P;
+    return bin_sort_impl<float>(M, W, H, visible, rect, depth_key, nullptr, 0, keys, vals, ranges);
+}
+int64_t tso_bin_sort_tight_f32(int32_t M, int32_t W, int32_t H, const uint8_t* visible, const int16_t* rect,
+                               const uint32_t* depth_key, const float* scr, uint64_t* keys, uint32_t* vals, uint32_t* ranges) {
+    return bin_sort_impl<float>(M, W, H, visible, rect, depth_key, scr, 1, keys, vals, ranges);
+}
+int64_t tso_bin_sort_tight_f64(int32_t M, int32_t W, int32_t H, const uint8_t* visible, const int16_t* rect,
+                               const uint32_t* depth_key, const double* scr, uint64_t* keys, uint32_t* vals, uint32_t* ranges) {
+    return bin_sort_impl<double>(M, W, H, visible, rect, depth_key, scr, 1, keys, vals, ranges);
 }
 
 #define TSO_FWD_ARGS color, opacity, faces, M, cam, prm, visible, rect, scr, list, n_list, tile_ranges

@@ -39,6 +39,8 @@ typedef struct {
     double amb_tol;                    /* relative margin for the "ambiguous decision" flag (0 = off) */
     int32_t min_opacity;               /* 0: face opacity = mean of the vertex opacities (the paper's choice);
                                           1: minimum ("+ min opacity" ablation, Table S3; Mesh Splatting) */
+    int32_t tight_binning;             /* 0: a face is binned into every tile its pixel rect touches;
+                                          1: only into the tiles its TRIANGLE meets (reading S31, NEXT-4) */
 } tso_params;
 
 /* F1-F6: project, cull, bounds, depth key.  faces may be NULL (soup: face m = (3m,3m+1,3m+2)).
@@ -59,6 +61,13 @@ int64_t tso_project_f64(const double* pos, const int32_t* faces, int32_t V, int3
 int64_t tso_bin_sort(int32_t M, int32_t W, int32_t H, const uint8_t* visible, const int16_t* rect,
                      const uint32_t* depth_key, const uint32_t* tiles_touched, uint64_t* keys, uint32_t* vals,
                      uint32_t* ranges);
+
+/* tight binning (tso_params.tight_binning = 1): as tso_bin_sort, with the tiles chosen by the overlap rule S31 from the
+ * projected vertices scr[M][9] of tso_project (same precision as the project call that counted tiles_touched). */
+int64_t tso_bin_sort_tight_f32(int32_t M, int32_t W, int32_t H, const uint8_t* visible, const int16_t* rect,
+                               const uint32_t* depth_key, const float* scr, uint64_t* keys, uint32_t* vals, uint32_t* ranges);
+int64_t tso_bin_sort_tight_f64(int32_t M, int32_t W, int32_t H, const uint8_t* visible, const int16_t* rect,
+                               const uint32_t* depth_key, const double* scr, uint64_t* keys, uint32_t* vals, uint32_t* ranges);
 
 /* F7-F8 forward.  If tile_ranges == NULL: brute mode, `list` holds n_list visible face ids in global depth
  * order and every pixel walks all of it.  Else tiled mode: `list` = sorted vals, tile_ranges[NT][2].

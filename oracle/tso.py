@@ -35,7 +35,8 @@ class _Cam(C.Structure):
 
 class _Prm(C.Structure):
     _fields_ = [("sigma", C.c_double), ("alpha_min", C.c_double), ("t_min", C.c_double),
-                ("eps_area", C.c_double), ("amb_tol", C.c_double), ("min_opacity", C.c_int32)]
+                ("eps_area", C.c_double), ("amb_tol", C.c_double), ("min_opacity", C.c_int32),
+                ("tight_binning", C.c_int32)]
 
 
 _lib = None
@@ -48,6 +49,8 @@ def lib():
         _lib.tso_project_f32.restype = C.c_int64
         _lib.tso_project_f64.restype = C.c_int64
         _lib.tso_bin_sort.restype = C.c_int64
+        _lib.tso_bin_sort_tight_f32.restype = C.c_int64
+        _lib.tso_bin_sort_tight_f64.restype = C.c_int64
         _lib.tso_l1_loss_f32.restype = C.c_double
         _lib.tso_l1_loss_f64.restype = C.c_double
         _lib.tso_dssim_f32.restype = C.c_double
@@ -86,7 +89,8 @@ class Oracle:
         self.cam = _Cam(self.W, self.H, _q(prec, cam.fx), _q(prec, cam.fy), _q(prec, cam.cx), _q(prec, cam.cy),
                         _q(prec, cam.znear))
         self.prm = _Prm(_q(prec, params.sigma), _q(prec, params.alpha_min), _q(prec, params.t_min),
-                        _q(prec, params.eps_area), float(amb_tol), int(bool(getattr(params, "min_opacity", False))))
+                        _q(prec, params.eps_area), float(amb_tol), int(bool(getattr(params, "min_opacity", False))),
+                        int(bool(getattr(params, "tight_binning", False))))
         self.tiles_x, self.tiles_y = (self.W + 15) // 16, (self.H + 15) // 16
         self.NT = self.tiles_x * self.tiles_y
         self._proj = None
@@ -119,9 +123,13 @@ class Oracle:
             keys = np.zeros(max(P, 1), np.uint64)
             vals = np.zeros(max(P, 1), np.uint32)
             ranges = np.zeros((self.NT, 2), np.uint32)
-            Pn = lib().tso_bin_sort(C.c_int32(self.M), C.c_int32(self.W), C.c_int32(self.H), _p(pr.visible),
-                                    _p(pr.rect), _p(pr.depth_key), _p(pr.tiles_touched), _p(keys), _p(vals),
-                                    _p(ranges))
+            if self.prm.tight_binning:
+                Pn = self._fn("tso_bin_sort_tight")(C.c_int32(self.M), C.c_int32(self.W), C.c_int32(self.H), _p(pr.visible),
+                                                    _p(pr.rect), _p(pr.depth_key), _p(pr.scr), _p(keys), _p(vals), _p(ranges))
+            else:
+                Pn = lib().tso_bin_sort(C.c_int32(self.M), C.c_int32(self.W), C.c_int32(self.H), _p(pr.visible),
+                                        _p(pr.rect), _p(pr.depth_key), _p(pr.tiles_touched), _p(keys), _p(vals),
+                                        _p(ranges))
             assert Pn == P
             keys, vals = keys[:P], vals[:P]
             if self.prec == "f64" and P > 0:

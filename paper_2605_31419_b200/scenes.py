@@ -42,6 +42,7 @@ class Params:
     eps_area: float = 1e-6
     lambda_dep: float = 0.05
     min_opacity: bool = False   # face opacity = min instead of mean of the vertex opacities (ablation)
+    tight_binning: bool = False  # bin a face only into the tiles its triangle meets (reading S31)
 
 
 @dataclass

@@ -26,9 +26,10 @@ class SimpleCam:
 
 
 class SimpleParams:
-    def __init__(self, sigma=1.0, alpha_min=0.0, t_min=0.0, eps_area=1e-6, lambda_dep=0.05, min_opacity=False):
+    def __init__(self, sigma=1.0, alpha_min=0.0, t_min=0.0, eps_area=1e-6, lambda_dep=0.05, min_opacity=False,
+                 tight_binning=False):
         self.sigma, self.alpha_min, self.t_min, self.eps_area, self.lambda_dep = sigma, alpha_min, t_min, eps_area, lambda_dep
-        self.min_opacity = min_opacity
+        self.min_opacity, self.tight_binning = min_opacity, tight_binning
 
 
 IDENT = np.concatenate([np.eye(3), np.zeros((3, 1))], axis=1)
