@@ -51,9 +51,14 @@ enum { TS_GRAD_POS = 1, TS_GRAD_COLOR = 2, TS_GRAD_OPACITY = 4, TS_GRAD_POSE = 8
 enum { TS_FLAG_OVERFLOW_PAIRS = 1, TS_FLAG_OVERFLOW_VISIBLE = 2 };
 /* ts_params.flags */
 enum { TS_PARAM_COUNTERS = 0x100,     /* count visits / rect tests / hits into the frame's debug counters */
-       TS_PARAM_MIN_OPACITY = 0x200 }; /* face opacity = MIN of its vertex opacities instead of their mean (
+       TS_PARAM_MIN_OPACITY = 0x200,  /* face opacity = MIN of its vertex opacities instead of their mean (
                                           "+ min opacity" ablation, Table S3); its gradient goes to that
                                           vertex alone (lowest index among equal minima) */
+       TS_PARAM_TIGHT_BINNING = 0x400 }; /* a face is binned only into the tiles its TRIANGLE meets, not into every tile
+                                          its pixel rect touches (SURVEY.md NEXT-4 "tighter triangle-tile binning";
+                                          DESIGN.md reading S31): shorter lists, identical images and gradients; the
+                                          tile counts, sorted lists and ranges are then those of the oracle's
+                                          tight_binning mode, bit for bit */
 
 const char* ts_strerror(int32_t status);
 

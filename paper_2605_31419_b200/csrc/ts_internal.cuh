@@ -101,6 +101,37 @@ __device__ __forceinline__ uint32_t ts_eff_visible(const TsFrameDev& f) {
     return (c->flags != 0) ? 0u : c->n_visible;
 }
 
+// Tight binning (ts_params.flags & TS_PARAM_TIGHT_BINNING; reading S31): does the triangle with screen
+// vertices (u_k, v_k) meet the box of pixel centres [bx0,bx1] x [by0,by1]?  For each edge k (from q_{k+1} to q_{k+2})
+// the un-normalised outward edge function E_k(p) = s (ey (px - ua) - ex (py - va)) is taken at the corner of the box
+// where it is smallest; the box is left out iff some E_k there exceeds 2^-10 (|ex| + |ey|): every pixel of the box is
+// then at least ~1e-3 px outside edge k and cannot pass the hit rule.  Explicit round-to-nearest operations in a fixed
+// order: the decision is bit-identical to the float32 oracle's, and to itself in the projection and binning kernels.
+__device__ __forceinline__ bool ts_tile_overlaps(const float u[3], const float v[3], int bx0, int by0, int bx1, int by1) {
+    const float a = __fsub_rn(u[1], u[0]), b = __fsub_rn(v[2], v[0]), c = __fsub_rn(v[1], v[0]), d = __fsub_rn(u[2], u[0]);
+    const float S = __fmaf_rn(a, b, -__fmul_rn(c, d));
+    const float s = S > 0.0f ? 1.0f : -1.0f;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const int ia = (k + 1) % 3, ib = (k + 2) % 3;
+        const float ex = __fsub_rn(u[ib], u[ia]), ey = __fsub_rn(v[ib], v[ia]);
+        const float sx = __fmul_rn(s, ey), sy = -__fmul_rn(s, ex);
+        const float px = sx > 0.0f ? (float)bx0 : (float)bx1, py = sy > 0.0f ? (float)by0 : (float)by1;
+        const float dx = __fsub_rn(px, u[ia]), dy = __fsub_rn(py, v[ia]);
+        const float E = __fmaf_rn(sx, dx, __fmul_rn(sy, dy));
+        const float margin = __fmul_rn(0.0009765625f, __fadd_rn(fabsf(ex), fabsf(ey)));
+        if (E > margin) return false;
+    }
+    return true;
+}
+// is tile (tx, ty) of the face's rect [x0,x1] x [y0,y1] one the face is binned into?
+__device__ __forceinline__ bool ts_tile_included(bool tight, const float u[3], const float v[3], int x0, int y0, int x1, int y1,
+                                                 int tx, int ty) {
+    if (!tight) return true;
+    return ts_tile_overlaps(u, v, max(x0, tx * TS_TILE), max(y0, ty * TS_TILE), min(x1, tx * TS_TILE + TS_TILE - 1),
+                            min(y1, ty * TS_TILE + TS_TILE - 1));
+}
+
 // launchers (one per .cu)
 int32_t ts_launch_project(const ts_ctx*, ts_frame*, const ts_scene*, cudaStream_t);
 int32_t ts_launch_sort(const ts_ctx*, ts_frame*, cudaStream_t);

@@ -18,7 +18,7 @@ struct FaceOut {
 };
 
 // N1-N5.  p = 9 floats (three world vertices), T = row-major 3x4 pose.
-__device__ __forceinline__ void project_face(const float* p, const float* T, const TsCamDev& cam, float eps_area,
+__device__ __forceinline__ void project_face(const float* p, const float* T, const TsCamDev& cam, float eps_area, bool tight,
                                              FaceOut& o) {
     float X[3], Y[3], Z[3];
 #pragma unroll
@@ -68,6 +68,15 @@ __device__ __forceinline__ void project_face(const float* p, const float* T, con
     const float zb = __fmul_rn(__fadd_rn(__fadd_rn(Z[0], Z[1]), Z[2]), 1.0f / 3.0f);  // N5
     o.key = __float_as_uint(zb);
     o.tiles = (uint32_t)(((o.x1 >> 4) - (o.x0 >> 4) + 1) * ((o.y1 >> 4) - (o.y0 >> 4) + 1));
+    if (tight) {
+        // tiles_touched = the tiles the triangle meets (reading S31)
+        uint32_t nt = 0;
+        for (int ty = o.y0 >> 4; ty <= (o.y1 >> 4); ++ty)
+            for (int tx = o.x0 >> 4; tx <= (o.x1 >> 4); ++tx)
+                nt += ts_tile_overlaps(o.u, o.v, max(o.x0, tx * TS_TILE), max(o.y0, ty * TS_TILE), min(o.x1, tx * TS_TILE + TS_TILE - 1),
+                                       min(o.y1, ty * TS_TILE + TS_TILE - 1)) ? 1u : 0u;
+        o.tiles = nt;
+    }
     o.vis = true;
 }
 
@@ -115,7 +124,8 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
     }
     FaceOut o;
     o.vis = false, o.tiles = 0;
-    if (tid < n_here) project_face(p, sT, cam, eps_area, o);
+    const bool tight = (f.prm_flags & TS_PARAM_TIGHT_BINNING) != 0;
+    if (tid < n_here) project_face(p, sT, cam, eps_area, tight, o);
     // mean vertex opacity of the survivors: requested now, so that its round trip overlaps the slot atomic
     float ob = 0.0f;
     if (o.vis) {
@@ -156,7 +166,8 @@ project_kernel(TsFrameDev f, const float* __restrict__ pos, const int32_t* __res
             s4[2] = make_float4(o.w[2], ob, __int_as_float(rlo), __int_as_float(rhi));
             s4[3] = make_float4(__uint_as_float(m), __uint_as_float(o.key), __uint_as_float(o.tiles), 0.0f);
             for (int ty = o.y0 >> 4; ty <= (o.y1 >> 4); ++ty)
-                for (int tx = o.x0 >> 4; tx <= (o.x1 >> 4); ++tx) atomicAdd(f.tile_count + ty * f.tiles_x + tx, 1u);
+                for (int tx = o.x0 >> 4; tx <= (o.x1 >> 4); ++tx)
+                    if (ts_tile_included(tight, o.u, o.v, o.x0, o.y0, o.x1, o.y1, tx, ty)) atomicAdd(f.tile_count + ty * f.tiles_x + tx, 1u);
         }
     }
 

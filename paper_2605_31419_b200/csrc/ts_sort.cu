@@ -219,6 +219,10 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
         const uint32_t n_round = (nvis + 31u) & ~31u;
         if (slot >= n_round) break;                            // warp-uniform
         const int nt = (fl || !live) ? 0 : ntx * nty;
+        const bool tight = (f.prm_flags & TS_PARAM_TIGHT_BINNING) != 0;
+        const float fu[3] = {s0.x, s0.w, s1.z}, fv[3] = {s0.y, s1.x, s1.w};           // the face's screen vertices
+        const int frx0 = (int)(short)(__float_as_int(s2.z) & 0xffff), fry0 = __float_as_int(s2.z) >> 16;
+        const int frx1 = (int)(short)(__float_as_int(s2.w) & 0xffff), fry1 = __float_as_int(s2.w) >> 16;
         // narrow faces (the common case): the owning lane scatters its <= 4 pairs itself; the cursor atomics are
         // issued together so that they cost one round trip, not four
         {
@@ -229,12 +233,14 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
                 // i < 4 pairs over ntx columns: row = i / ntx by comparisons (an integer division is a subroutine call)
                 const int row = (i >= ntx ? 1 : 0) + (i >= 2 * ntx ? 1 : 0) + (i >= 3 * ntx ? 1 : 0);
                 tt[i] = (ty0 + row) * f.tiles_x + tx0 + (i - row * ntx);
-                pos[i] = 0;
-                if (nt <= 4 && i < nt) pos[i] = atomicAdd(f.tile_cursor + tt[i], 1u);
+                pos[i] = 0xffffffffu;
+                // (tight binning: only the tiles the triangle meets, by the rule the projection counted with)
+                if (nt <= 4 && i < nt && ts_tile_included(tight, fu, fv, frx0, fry0, frx1, fry1, tx0 + (i - row * ntx), ty0 + row))
+                    pos[i] = atomicAdd(f.tile_cursor + tt[i], 1u);
             }
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
-                if (nt <= 4 && i < nt) {
+                if (nt <= 4 && i < nt && pos[i] != 0xffffffffu) {
                     const uint32_t q = offs[tt[i]] + pos[i];
                     if (q < f.pair_cap) f.pair_a[q] = pa, f.pair_b[q] = pb;
                 }
@@ -267,11 +273,20 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
                 ba.x = __shfl_sync(0xffffffffu, pa.x, own), ba.y = __shfl_sync(0xffffffffu, pa.y, own);
                 ba.z = __shfl_sync(0xffffffffu, pa.z, own), ba.w = __shfl_sync(0xffffffffu, pa.w, own);
                 const uint32_t bb = __shfl_sync(0xffffffffu, pb, own);
+                float wu[3], wv[3];
+                if (tight) {                                    // (warp-uniform)
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) wu[k] = __shfl_sync(0xffffffffu, fu[k], own), wv[k] = __shfl_sync(0xffffffffu, fv[k], own);
+                }
                 if (p < W) {
                     const int i = (int)(p - (o_incl - o_nt));
-                    const int t = (bty0 + i / bntx) * f.tiles_x + btx0 + i % bntx;
-                    const uint32_t q = offs[t] + atomicAdd(f.tile_cursor + t, 1u);
-                    if (q < f.pair_cap) f.pair_a[q] = ba, f.pair_b[q] = bb;
+                    const int wty = bty0 + i / bntx, wtx = btx0 + i % bntx;
+                    const int t = wty * f.tiles_x + wtx;
+                    const int wx0 = (int)(short)(ba.w & 0xffffu), wy0 = (int)ba.w >> 16, wx1 = (int)(short)(bb & 0xffffu), wy1 = (int)bb >> 16;
+                    if (ts_tile_included(tight, wu, wv, wx0, wy0, wx1, wy1, wtx, wty)) {
+                        const uint32_t q = offs[t] + atomicAdd(f.tile_cursor + t, 1u);
+                        if (q < f.pair_cap) f.pair_a[q] = ba, f.pair_b[q] = bb;
+                    }
                 }
             }
         }

@@ -20,6 +20,7 @@ GRAD_ALL = 15
 FLAG_OVERFLOW_PAIRS, FLAG_OVERFLOW_VISIBLE = 1, 2
 PARAM_COUNTERS = 0x100   # ts_params.flags: count visits / rect tests / hits (debug instantiation)
 PARAM_MIN_OPACITY = 0x200   # ts_params.flags: face opacity = min instead of mean of the vertex opacities (ablation)
+PARAM_TIGHT_BINNING = 0x400  # ts_params.flags: bin a face only into the tiles its triangle meets (reading S31)
 VIEW_VIS, VIEW_KEYS, VIEW_VALS, VIEW_TILE_RANGES, VIEW_N_CONTRIB, VIEW_COUNTERS = range(6)
 _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.int32,
                 VIEW_TILE_RANGES: torch.int32, VIEW_N_CONTRIB: torch.int32, VIEW_COUNTERS: torch.int64}
@@ -184,6 +185,8 @@ def make_camera(cam):
 def make_params(p, flags=0):
     if getattr(p, "min_opacity", False):
         flags |= PARAM_MIN_OPACITY
+    if getattr(p, "tight_binning", False):
+        flags |= PARAM_TIGHT_BINNING
     return ts_params(p.sigma, p.alpha_min, p.t_min, p.eps_area, flags)
 
 

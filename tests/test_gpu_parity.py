@@ -846,3 +846,41 @@ def test_normalised_depth_and_top_normal(ctx, oracle_mod, cfg):
     assert bad.sum() <= 2 + 2e-4 * ok.size
     assert np.abs(np.linalg.norm(top_ref, axis=0)[f.n_contrib > 0] - 1.0).max() < 1e-5
     g.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 4])
+def test_tight_binning(ctx, oracle_mod, cfg):
+    """NEXT-4 remainder: TS_PARAM_TIGHT_BINNING (reading S31).  Tile counts, sorted keys / values and ranges bit-exact
+    against the oracle's tight mode; images bit-identical to the loose lists' (no dropped pair could contribute);
+    gradients to tolerance; fewer pairs."""
+    from gpu_util import GpuView
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(cfg)
+    prm = scenes.Params(**{**sc.params.__dict__, "tight_binning": True})
+    o, g = both(ctx, oracle_mod, sc, params=prm)
+    check_project_and_sort(o, g, sc.M)
+    f, ok = check_forward(o, g)
+    loose = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
+    Cl, Dl, Al = loose.forward()
+    assert np.array_equal(Cl, g.C.cpu().numpy()) and np.array_equal(Dl, g.D.cpu().numpy()) and np.array_equal(Al, g.A.cpu().numpy())
+    n_tight, n_loose = g.status()[2], loose.status()[2]
+    print(f"pairs: {n_loose} -> {n_tight} ({100.0 * (n_loose - n_tight) / max(1, n_loose):.1f} % dropped)")
+    assert n_tight < n_loose
+    check_backward(o, g, ok, 80 + cfg, [ts.GRAD_ALL, ts.GRAD_POSE])
+    loose.close()
+    g.close()
+
+
+def test_tight_binning_wide_faces(ctx, oracle_mod):
+    """Faces that span many tiles (the flattened scatter path of the binning kernel) under tight binning."""
+    sc = scenes.config0(n_faces=60)
+    rng = np.random.default_rng(3)
+    pos = sc.pos.reshape(-1, 3, 3).copy()
+    pos[:, :, :2] = (pos[:, :1, :2] + rng.normal(0, 0.9, (60, 3, 2)))            # ~50-pixel triangles
+    sc.pos = pos.reshape(-1, 3).astype(np.float32)
+    prm = scenes.Params(**{**sc.params.__dict__, "tight_binning": True})
+    o, g = both(ctx, oracle_mod, sc, params=prm)
+    check_project_and_sort(o, g, sc.M)
+    assert o.project().tiles_touched.max() > 4
+    check_forward(o, g)
+    g.close()
