@@ -252,6 +252,13 @@ struct Lists {
 };
 
 // set-up every visible face once (the per-face constants do not depend on the pixel)
+// S32: window smoothness of face m: the per-face array of tso_params (Triangle Splatting's learnable sigma)
+// if there is one, else the global constant the paper uses
+template <class T>
+inline T face_sigma(const tso_params* prm, uint32_t m) {
+    return prm->face_sigma ? ((const T*)prm->face_sigma)[m] : (T)prm->sigma;
+}
+
 template <class T>
 std::vector<Face<T>> setup_all(const T* color, const T* opacity, const int32_t* faces, int32_t M,
                                const uint8_t* visible, const int16_t* rect, const T* scr, bool min_op) {
@@ -288,7 +295,7 @@ void render_fwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 if (x < f.x0 || x > f.x1 || y < f.y0 || y > f.y1) continue;   // rect is part of the hit rule (S5)
                 ++n_rect;
                 Hit<T> h;
-                if (!eval(f, (T)x, (T)y, sigma, amin, atol, h, &amb)) continue;
+                if (!eval(f, (T)x, (T)y, face_sigma<T>(prm, list[i]), amin, atol, h, &amb)) continue;
                 ++n_hit;
                 T wgt = Tr * h.alpha;                                          // Eq. 4
                 for (int c = 0; c < 3; ++c) C[c] += wgt * h.c[c];
@@ -452,7 +459,7 @@ void face_stats(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 const Face<T>& f = F[list[i]];
                 if (x < f.x0 || x > f.x1 || y < f.y0 || y > f.y1) continue;
                 Hit<T> h;
-                if (!eval(f, (T)x, (T)y, sigma, amin, (T)0, h, nullptr)) continue;
+                if (!eval(f, (T)x, (T)y, face_sigma<T>(prm, list[i]), amin, (T)0, h, nullptr)) continue;
                 face_pixels[list[i]] += 1;
                 Tr = Tr * ((T)1 - h.alpha);
                 if (Tr <= tmin) break;
@@ -491,7 +498,7 @@ void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
             for (int64_t i = b; i < e; ++i) {
                 const Face<T>& f = F[list[i]];
                 if (x < f.x0 || x > f.x1 || y < f.y0 || y > f.y1) continue;
-                if (!eval(f, (T)x, (T)y, sigma, amin, (T)0, h, nullptr)) continue;
+                if (!eval(f, (T)x, (T)y, face_sigma<T>(prm, list[i]), amin, (T)0, h, nullptr)) continue;
                 hits.push_back({list[i], Tr});
                 Tr = Tr * ((T)1 - h.alpha);
                 if (Tr <= tmin) break;
@@ -502,7 +509,8 @@ void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                 const uint32_t m = hits[j].m;
                 const Face<T>& f = F[m];
                 const T Tn = hits[j].Tn;
-                eval(f, (T)x, (T)y, sigma, amin, (T)0, h, nullptr);
+                const T sigma_m = face_sigma<T>(prm, m);
+                eval(f, (T)x, (T)y, sigma_m, amin, (T)0, h, nullptr);
                 const T wgt = Tn * h.alpha;
                 // B1: vertex colours
                 if (grad_color)
@@ -532,7 +540,9 @@ void render_bwd(const T* color, const T* opacity, const int32_t* faces, int32_t 
                         for (int k = 0; k < 3; ++k) grad_opacity[vid(faces, m, k)] += (h.I / (T)3) * ga;
                 }
                 const T gI = f.obar * ga;
-                const T gx = gI * sigma * h.I / h.x;
+                const T gx = gI * sigma_m * h.I / h.x;
+                // S32: I = x^sigma, so dL/dsigma_m += dL/dI * I ln x
+                if (prm->grad_face_sigma) ((T*)prm->grad_face_sigma)[m] += gI * h.I * std::log(h.x);
                 // B5: interpolation
                 T gom[3], gb[3], gw[3];
                 for (int k = 0; k < 3; ++k) {

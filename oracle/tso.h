@@ -41,6 +41,10 @@ typedef struct {
                                           1: minimum ("+ min opacity" ablation, Table S3; Mesh Splatting) */
     int32_t tight_binning;             /* 0: a face is binned into every tile its pixel rect touches;
                                           1: only into the tiles its TRIANGLE meets (reading S31, NEXT-4) */
+    const void* face_sigma;            /* NULL: the global sigma above (the paper); else [M] per-face window
+                                          smoothness in the scalar type of the call (Triangle Splatting's learnable
+                                          sigma; reading S32) */
+    void* grad_face_sigma;             /* NULL or [M] (+=): dL/dsigma_m, accumulated by tso_render_bwd */
 } tso_params;
 
 /* F1-F6: project, cull, bounds, depth key.  faces may be NULL (soup: face m = (3m,3m+1,3m+2)).

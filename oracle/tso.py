@@ -36,7 +36,7 @@ class _Cam(C.Structure):
 class _Prm(C.Structure):
     _fields_ = [("sigma", C.c_double), ("alpha_min", C.c_double), ("t_min", C.c_double),
                 ("eps_area", C.c_double), ("amb_tol", C.c_double), ("min_opacity", C.c_int32),
-                ("tight_binning", C.c_int32)]
+                ("tight_binning", C.c_int32), ("face_sigma", C.c_void_p), ("grad_face_sigma", C.c_void_p)]
 
 
 _lib = None
@@ -74,7 +74,7 @@ def _q(prec, x):
 class Oracle:
     """One view of one scene.  prec = 'f32' (parity) or 'f64' (finite differences / accuracy reference)."""
 
-    def __init__(self, pos, color, opacity, faces, T_cw, cam, params, prec="f32", amb_tol=0.0):
+    def __init__(self, pos, color, opacity, faces, T_cw, cam, params, prec="f32", amb_tol=0.0, face_sigma=None):
         self.prec = prec
         self.dt = np.float32 if prec == "f32" else np.float64
         self.sfx = "_" + prec
@@ -90,7 +90,11 @@ class Oracle:
                         _q(prec, cam.znear))
         self.prm = _Prm(_q(prec, params.sigma), _q(prec, params.alpha_min), _q(prec, params.t_min),
                         _q(prec, params.eps_area), float(amb_tol), int(bool(getattr(params, "min_opacity", False))),
-                        int(bool(getattr(params, "tight_binning", False))))
+                        int(bool(getattr(params, "tight_binning", False))), None, None)
+        # per-face window smoothness (reading S32); its gradient is returned by backward() as grad_sigma
+        self.face_sigma = None if face_sigma is None else np.ascontiguousarray(face_sigma, self.dt)
+        if self.face_sigma is not None:
+            self.prm.face_sigma = self.face_sigma.ctypes.data
         self.tiles_x, self.tiles_y = (self.W + 15) // 16, (self.H + 15) // 16
         self.NT = self.tiles_x * self.tiles_y
         self._proj = None
@@ -191,10 +195,13 @@ class Oracle:
         o.grad_color = np.zeros_like(self.color) if "color" in want else None
         o.grad_opacity = np.zeros_like(self.opacity) if "opacity" in want else None
         o.g_scr = np.zeros((self.M, 9), self.dt)
+        o.grad_sigma = np.zeros(self.M, self.dt) if self.face_sigma is not None else None
+        self.prm.grad_face_sigma = None if o.grad_sigma is None else o.grad_sigma.ctypes.data
         self._fn("tso_render_bwd")(
             _p(self.color), _p(self.opacity), _p(self.faces), C.c_int32(self.M), C.byref(self.cam),
             C.byref(self.prm), _p(pr.visible), _p(pr.rect), _p(pr.scr), _p(lst), C.c_int64(lst.shape[0]),
             _p(ranges), _p(gC), _p(gD), _p(gA), _p(o.grad_color), _p(o.grad_opacity), _p(o.g_scr))
+        self.prm.grad_face_sigma = None
         o.grad_pos = np.zeros_like(self.pos) if "pos" in want else None
         o.dL_dtau = np.zeros(6, self.dt)
         self._fn("tso_project_bwd")(_p(self.faces), C.c_int32(self.M), _p(self.T_cw), C.byref(self.cam),
