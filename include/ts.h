@@ -75,6 +75,14 @@ size_t ts_frame_bytes(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64
 int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_t W, int32_t H,
                       uint64_t pair_capacity, uint64_t visible_capacity, void* stream, ts_frame** out);
 int32_t ts_frame_release(ts_frame* frame);   /* frees the host handle only */
+/* Per-face window smoothness (reading S32): Triangle Splatting [8] learns one sigma per
+ * triangle, this paper fixes one global constant.  sigma_dev[M] (device, > 0; NULL = back to the
+ * global ts_params.sigma) replaces it for every later ts_project / ts_bin_sort / render call on this frame (the
+ * exponent travels in the per-face record: calls before the next ts_bin_sort return TS_ERR_STATE); the renders then run
+ * the generic-exponent instantiation.  grad_sigma_dev[M] (device, may be NULL; accumulates, caller zeroes): the
+ * full-gradient ts_render_bwd / ts_render_map_l1 / ts_render_bwd_normal add dL/dsigma_m = sum_hits dL/dI I ln x.  Both
+ * pointers must stay valid until replaced.  Host call, no launch. */
+int32_t ts_frame_set_face_sigma(ts_ctx* ctx, ts_frame* frame, const float* sigma_dev, float* grad_sigma_dev);
 /* Synchronises `stream`, then reports the counters of the last ts_project/ts_bin_sort on this frame. */
 int32_t ts_frame_status(ts_ctx* ctx, ts_frame* frame, uint32_t* flags, uint32_t* n_visible, uint64_t* n_pairs,
                         void* stream);

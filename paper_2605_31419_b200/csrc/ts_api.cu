@@ -150,6 +150,15 @@ int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_
     return TS_OK;
 }
 
+int32_t ts_frame_set_face_sigma(ts_ctx* ctx, ts_frame* fr, const float* sigma_dev, float* grad_sigma_dev) {
+    if (!ctx || !fr) return TS_ERR_INVALID_ARG;
+    if (!sigma_dev && grad_sigma_dev) return TS_ERR_INVALID_ARG;
+    fr->face_sigma = sigma_dev, fr->grad_sigma = grad_sigma_dev;
+    // the exponent travels in the per-face record, which ts_bin_sort builds: the frame has to be projected and binned again
+    fr->have_sort = fr->have_fwd = fr->have_normals = 0;
+    return TS_OK;
+}
+
 int32_t ts_frame_release(ts_frame* frame) {
     delete frame;
     return TS_OK;
@@ -297,6 +306,10 @@ int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float*
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     fr->have_fwd = 0;                                       // n_contrib / T_last are not written: no ts_render_bwd after this
+    // (the hit-log variant evaluates its geometry phase with the launch's sigma: per-face sigma takes the visit form)
+    if (fr->face_sigma)
+        return ts_launch_render_track_v1(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev,
+                                         (cudaStream_t)stream);
     return ts_launch_render_track(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev,
                                   (cudaStream_t)stream);
 }

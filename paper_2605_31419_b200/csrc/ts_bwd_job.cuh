@@ -73,7 +73,8 @@ __device__ __forceinline__ void ts_bwd_pose_hit(const BwdWarpSmem& sm, uint32_t 
     const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
     const float l[3] = {l0, l1, l2};
     const float x = -fmaxf(l0, fmaxf(l1, l2));
-    const float I = ts_window_pow<SM>(x, sigma);
+    const float sg = SM == 0 ? sm.r[e][12].x : sigma;             // per-entry exponent in the generic instantiation (S32)
+    const float I = ts_window_pow<SM>(x, sg);
     const float o0 = l0 * r3.x, o1 = l1 * r3.y, o2 = l2 * r3.z;
     const float Om = (o0 + o1) + o2, z = ts_rcp_approx(Om);
     const float d0 = r3.w * pg.x + r4.x * pg.y + r4.y * pg.z;
@@ -81,7 +82,7 @@ __device__ __forceinline__ void ts_bwd_pose_hit(const BwdWarpSmem& sm, uint32_t 
     const float d2 = r5.y * pg.x + r5.z * pg.y + r5.w * pg.z;
     const float cg = (o0 * d0 + o1 * d1 + o2 * d2) * z;
     float g[9];
-    ts_bwd_geom<SM>(sm, e, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sigma, g);
+    ts_bwd_geom<SM>(sm, e, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sg, g);
     const float4 q5 = sm.r[e][7], n0 = sm.r[e][10], n1 = sm.r[e][11];
     {
         const float a = fx * g[0], b = fy * g[1], c = -(n0.x * a + n0.y * b) - q5.x * g[2];
@@ -111,10 +112,12 @@ template <int SM, bool ATTR, bool GEOM, bool NRM = false>
 __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_scene& sc, BwdWarpSmem& sm, int lane,
                                                   bool active, uint32_t code, float l0, float l1, float l2, float ga,
                                                   float wgt, float sigma, float* __restrict__ grad_color,
-                                                  float* __restrict__ grad_opacity) {
+                                                  float* __restrict__ grad_opacity, float* __restrict__ grad_sigma = nullptr) {
     const uint32_t e = code & 0xffu;
     float acc[19];
     float accn[3] = {0.f, 0.f, 0.f};
+    float accs = 0.f;                                              // dL/dsigma of the hit's face (generic instantiation, S32)
+    const bool want_sigma = SM == 0 && grad_sigma != nullptr;
 #pragma unroll
     for (int j = 0; j < 19; ++j) acc[j] = 0.f;
     if (active) {
@@ -126,7 +129,9 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
         const float4 r3 = sm.r[e][3], r4 = sm.r[e][4], r5 = sm.r[e][5];
         const float l[3] = {l0, l1, l2};
         const float x = -fmaxf(l0, fmaxf(l1, l2));
-        const float I = ts_window_pow<SM>(x, sigma);
+        const float sg = SM == 0 ? sm.r[e][12].x : sigma;
+        const float I = ts_window_pow<SM>(x, sg);
+        if (want_sigma) accs = ga * sm.r[e][2].w * I * __logf(x);     // I = x^sigma: dL/dsigma += dL/dI I ln x
         const float o0 = l0 * r3.x, o1 = l1 * r3.y, o2 = l2 * r3.z;
         const float Om = (o0 + o1) + o2, z = ts_rcp_approx(Om);
         if (ATTR) {
@@ -142,7 +147,7 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
             const float d1 = r4.z * pg.x + r4.w * pg.y + r5.x * pg.z;
             const float d2 = r5.y * pg.x + r5.z * pg.y + r5.w * pg.z;
             const float cg = (o0 * d0 + o1 * d1 + o2 * d2) * z;
-            ts_bwd_geom<SM>(sm, e, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sigma, acc);
+            ts_bwd_geom<SM>(sm, e, l, x, I, ga, wgt, z, d0, d1, d2, cg, z * pg.w, sg, acc);
         }
     }
     // segmented reduction over runs of equal staged index (inactive lanes never match anybody)
@@ -179,8 +184,13 @@ __device__ __forceinline__ void ts_bwd_full_group(const TsFrameDev& f, const ts_
                 if (same) accn[j] += t;
             }
         }
+        if (want_sigma) {
+            const float t = __shfl_down_sync(0xffffffffu, accs, d);
+            if (same) accs += t;
+        }
     }
     if (active && run_start) {                                 // first lane of a run
+        if (want_sigma) atomicAdd(grad_sigma + sm.face[e], accs);
         if (GEOM) {
             float* gs = f.gscr + 9 * (size_t)sm.slot[e];
 #pragma unroll
@@ -232,7 +242,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
                                             uint32_t ncon, float Tcur, float gC0, float gC1, float gC2, float gD,
                                             float gA, float* __restrict__ grad_color, float* __restrict__ grad_opacity,
                                             float tau[6], float gN0 = 0.f, float gN1 = 0.f, float gN2 = 0.f,
-                                            uint32_t prestaged_lo = 0xffffffffu) {
+                                            uint32_t prestaged_lo = 0xffffffffu, float* __restrict__ grad_sigma = nullptr) {
     static_assert(!(NRM && POSE), "the normal-map backward runs in full-gradient mode");
     const float fpx = (float)job.px, fpy = (float)job.py;
     const uint32_t lt = (1u << lane) - 1u;
@@ -276,6 +286,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             d[6] = r[4], d[7] = r[5], d[8] = r[6], d[9] = r[7];
             if (POSE) d[10] = r[8], d[11] = r[9];
             if (NRM) d[10] = f.nrm[cur.x];
+            if (SM == 0) d[12] = make_float4(r[3].w, 0.f, 0.f, 0.f);  // the entry's window exponent (S32)
             sm.lm[lane] = lmask, sm.slot[lane] = cur.x, sm.face[lane] = cur.y;
         }
         __syncwarp();
@@ -289,7 +300,8 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             bool hit = false;
             {
                 const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
-                hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
+                const float sg = SM == 0 ? sm.r[e][12].x : sigma;
+                hit = in_rect && ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sg, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
             }
             const uint32_t hm = __ballot_sync(0xffffffffu, hit);
             if (!hm) continue;
@@ -335,7 +347,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
                 if (POSE)
                     ts_bwd_pose_hit<SM>(sm, code & 0xffu, sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
                 else
-                    ts_bwd_full_group<SM, ATTR, GEOM, NRM>(f, sc, sm, lane, true, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
+                    ts_bwd_full_group<SM, ATTR, GEOM, NRM>(f, sc, sm, lane, true, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity, grad_sigma);
                 __syncwarp();
             }
         }
@@ -351,7 +363,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             if (POSE) {
                 if (act) ts_bwd_pose_hit<SM>(sm, code & 0xffu, sm.pix[code >> 8], ql0, ql1, ql2, qga, qw, fx, fy, sigma, tau);
             } else {
-                ts_bwd_full_group<SM, ATTR, GEOM, NRM>(f, sc, sm, lane, act, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity);
+                ts_bwd_full_group<SM, ATTR, GEOM, NRM>(f, sc, sm, lane, act, code, ql0, ql1, ql2, qga, qw, sigma, grad_color, grad_opacity, grad_sigma);
             }
             qn = 0, qh = 0;
             __syncwarp();

@@ -31,6 +31,8 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
                                             FwdPix& o, unsigned long long& n_visit, unsigned long long& n_rect,
                                             unsigned long long& n_hit, uint32_t* __restrict__ face_pixels = nullptr,
                                             float4* nsm = nullptr, uint32_t* staged_lo = nullptr) {
+    // generic-sigma instantiation (SM == 0): the exponent of entry e is staged in the slice's pad row (reading S32)
+    constexpr int SIGROW = FULLREC ? 12 : 6;
     const float fpx = (float)job.px, fpy = (float)job.py;
     float T = 1.0f, C0 = 0.0f, C1 = 0.0f, C2 = 0.0f, D = 0.0f, Tlast = 1.0f;
     float N0 = 0.0f, N1 = 0.0f, N2 = 0.0f, Nt0 = 0.0f, Nt1 = 0.0f, Nt2 = 0.0f, a_top = 0.0f;
@@ -58,6 +60,7 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             sm.r[lane][3] = make_float4(r3.x, r3.y, r3.z, col[0]);
             sm.r[lane][4] = make_float4(col[1], col[2], col[3], col[4]);
             sm.r[lane][5] = make_float4(col[5], col[6], col[7], col[8]);
+            if (SM == 0) sm.r[lane][SIGROW] = make_float4(r3.w, 0.f, 0.f, 0.f);
             sm.lm[lane] = lmask, sm.slot[lane] = cur.x;
             if (STATS) sm.face[lane] = cur.y;
             if (NRM) nsm[lane] = f.nrm[cur.x];
@@ -88,7 +91,8 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             bool hit = false;
             if (in_rect) {
                 const float4 r0 = sm.r[e][0], r1 = sm.r[e][1], r2 = sm.r[e][2];
-                hit = ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sigma, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
+                const float sg = SM == 0 ? sm.r[e][SIGROW].x : sigma;
+                hit = ts_eval_alpha<SM>(r0, r1, r2, fpx, fpy, sg, alpha_min, f.scr, sm.slot[e], l, x, I, alpha);
             }
             if (STATS) {
                 // statistics: the face contributed to popc(hm) pixels of this block (one RED per visit)

@@ -76,6 +76,8 @@ struct ts_frame {
     TsCamDev cam;
     TsPrmDev prm;
     const float* T_cw;       // device pointer given to the last ts_project (read again by the projection backward)
+    const float* face_sigma; // ts_frame_set_face_sigma: per-face window smoothness [M] (NULL = the global sigma of ts_params)
+    float* grad_sigma;       // ... and where the full-gradient backward adds dL/dsigma_m [M] (may be NULL)
     int have_project, have_sort, have_fwd;
     int have_normals;        // f.nrm holds the face normals of the current projection (ts_render_fwd_normal ran)
     int counters_dirty;      // ts_project ran but ts_bin_sort has not consumed (and re-zeroed) its counters yet

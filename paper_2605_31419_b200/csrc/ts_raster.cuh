@@ -15,7 +15,7 @@
 //   R0  refx  refy  m0x   m0y        R5  w0     w1     w2     tau0
 //   R1  m1x   m1y   m2x   m2y        R6  tau1   tau2   drr0x  drr0y
 //   R2  c0    c1    c2    obar       R7  drr1x  drr1y  drr2x  drr2y
-//   R3  kap0  kap1  kap2  rect_lo    R8  xn0    yn0    xn1    yn1
+//   R3  kap0  kap1  kap2  sigma_f    R8  xn0    yn0    xn1    yn1
 //   R4  rho0  rho1  rho2  rect_hi    R9  xn2    yn2    -      -
 // R0-R2 decide alpha (forward and backward), R3 interpolates, R4-R7 are the backward-only geometry terms
 // (tau_k = foot of vertex k on its opposite edge, drr_j = -(1/r) dr/dq_j), R8-R9 the normalised camera
@@ -146,6 +146,9 @@ __device__ __forceinline__ float ts_window_pow(float x, float sigma) {
 __host__ __device__ inline int ts_sigma_mode(float sigma) {
     return sigma == 1.0f ? 1 : (sigma == 0.5f ? 2 : (sigma == 2.0f ? 3 : 0));
 }
+// Per-face sigma (reading S32) runs through the generic instantiation (SM = 0), which takes the exponent of entry e from
+// the staged copy of record row R3's last float instead of the launch parameter.
+inline int ts_frame_sigma_mode(const ts_frame* fr) { return fr->face_sigma ? 0 : ts_sigma_mode(fr->prm.sigma); }
 
 // Near an edge (|x| below this band) the fast affine form above loses RELATIVE accuracy in x (its absolute error is
 // ~2e-7), and for sigma < 1 dI/dx = sigma x^(sigma-1) amplifies that beyond the gradient tolerance.  There -- for

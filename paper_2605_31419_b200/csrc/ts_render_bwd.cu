@@ -32,7 +32,8 @@ template <int SM, bool ATTR, bool GEOM, bool POSE, bool NRM = false>
 __global__ void __launch_bounds__(TS_JOB_WARPS * 32, NRM ? 2 : 3)
 render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float fx, float fy,
                   const float* __restrict__ gCi, const float* __restrict__ gDi, const float* __restrict__ gAi,
-                  float* __restrict__ grad_color, float* __restrict__ grad_opacity, const float* __restrict__ gNi = nullptr) {
+                  float* __restrict__ grad_color, float* __restrict__ grad_opacity, const float* __restrict__ gNi = nullptr,
+                  float* __restrict__ grad_sigma = nullptr) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     BwdWarpSmem& sm = reinterpret_cast<BwdWarpSmem*>(smem_raw)[threadIdx.x >> 5];
@@ -57,7 +58,7 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
         j = ts_job_take(f, 1, lane);       // next ticket: its round trip overlaps the pixel loads
         float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         ts_bwd_walk<SM, ATTR, GEOM, POSE, NRM>(f, sc, job, lane, sm, sigma, alpha_min, fx, fy, ncon, Tcur, gC0, gC1, gC2, gD, gA,
-                                               grad_color, grad_opacity, tau, gN0, gN1, gN2);
+                                               grad_color, grad_opacity, tau, gN0, gN1, gN2, 0xffffffffu, grad_sigma);
         if (POSE) {
             // per-thread -> per-job partial (fixed shuffle tree; the final reduction runs over jobs in index order)
 #pragma unroll
@@ -95,7 +96,8 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
                     float* __restrict__ out_color, float* __restrict__ out_depth, float* __restrict__ out_alpha,
                     const float* __restrict__ Chat, const float* __restrict__ Dhat, float wc, float wd,
                     float* __restrict__ gCo, float* __restrict__ gDo, float* __restrict__ loss,
-                    float* __restrict__ grad_color = nullptr, float* __restrict__ grad_opacity = nullptr) {
+                    float* __restrict__ grad_color = nullptr, float* __restrict__ grad_opacity = nullptr,
+                    float* __restrict__ grad_sigma = nullptr) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     TrackWarpSmem& sm = reinterpret_cast<TrackWarpSmem*>(smem_raw)[threadIdx.x >> 5];
@@ -140,7 +142,7 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
         __syncwarp();                                      // the forward walk's shared-memory slice is re-used
         float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         ts_bwd_walk<SM, ATTR, GEOM, POSE>(f, sc, job, lane, sm.bwd, sigma, alpha_min, fx, fy, o.last, o.Tlast, gC0, gC1,
-                                          gC2, gD, 0.0f, grad_color, grad_opacity, tau, 0.f, 0.f, 0.f, staged_lo);
+                                          gC2, gD, 0.0f, grad_color, grad_opacity, tau, 0.f, 0.f, 0.f, staged_lo, grad_sigma);
         if (POSE) {
 #pragma unroll
             for (int jj = 0; jj < 6; ++jj) tau[jj] = warp_sum(tau[jj]);
@@ -182,7 +184,7 @@ void launch_map(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, float
     const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 3, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
     render_track_kernel<SM, ATTR, GEOM, false><<<grid, TS_JOB_WARPS * 32, smem, st>>>(
         f, sc, fr->prm.sigma, fr->prm.alpha_min, fr->prm.t_min, fr->cam.fx, fr->cam.fy, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss,
-        gcol, gopa);
+        gcol, gopa, fr->grad_sigma);
 }
 
 template <int SM>
@@ -385,7 +387,8 @@ void launch_one(const ts_ctx* ctx, const ts_frame* fr, const ts_scene& sc, const
     cudaFuncSetAttribute(render_bwd_kernel<SM, ATTR, GEOM, POSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 3, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
     render_bwd_kernel<SM, ATTR, GEOM, POSE><<<grid, TS_JOB_WARPS * 32, smem, st>>>(f, sc, fr->prm.sigma, fr->prm.alpha_min,
-                                                                                   fr->cam.fx, fr->cam.fy, gC, gD, gA, gcol, gopa);
+                                                                                   fr->cam.fx, fr->cam.fy, gC, gD, gA, gcol, gopa,
+                                                                                   nullptr, fr->grad_sigma);
 }
 
 template <int SM>
@@ -408,7 +411,7 @@ int32_t ts_launch_render_bwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
     if (!attr && !geom) return TS_OK;
     float* gcol = (mask & TS_GRAD_COLOR) ? grad_color : nullptr;
     float* gopa = (mask & TS_GRAD_OPACITY) ? grad_opacity : nullptr;
-    switch (ts_sigma_mode(fr->prm.sigma)) {
+    switch (ts_frame_sigma_mode(fr)) {
         case 1: launch_bwd_sm<1>(ctx, fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
         case 2: launch_bwd_sm<2>(ctx, fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
         case 3: launch_bwd_sm<3>(ctx, fr, *sc, gC, gD, gA, gcol, gopa, attr, geom, pose_only, st); break;
@@ -445,7 +448,8 @@ void launch_bwd_normal_sm(const ts_ctx* ctx, const ts_frame* fr, const ts_scene&
 #define TS_LAUNCH_BN(A, G)                                                                                                  \
     do {                                                                                                                    \
         cudaFuncSetAttribute(render_bwd_kernel<SM, A, G, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-        render_bwd_kernel<SM, A, G, false, true><<<grid, TS_JOB_WARPS * 32, smem, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa, gN); \
+        render_bwd_kernel<SM, A, G, false, true><<<grid, TS_JOB_WARPS * 32, smem, st>>>(f, sc, sg, am, fx, fy, gC, gD, gA, gcol, gopa, gN, \
+                                                                                        fr->grad_sigma);                       \
     } while (0)
     if (attr && geom) TS_LAUNCH_BN(true, true);
     else if (geom) TS_LAUNCH_BN(false, true);
@@ -464,7 +468,7 @@ int32_t ts_launch_render_bwd_normal(const ts_ctx* ctx, ts_frame* fr, const ts_sc
     if (!attr && !geom) return TS_OK;
     float* gcol = (mask & TS_GRAD_COLOR) ? grad_color : nullptr;
     float* gopa = (mask & TS_GRAD_OPACITY) ? grad_opacity : nullptr;
-    switch (ts_sigma_mode(fr->prm.sigma)) {
+    switch (ts_frame_sigma_mode(fr)) {
         case 1: launch_bwd_normal_sm<1>(ctx, fr, *sc, gC, gD, gA, gN, gcol, gopa, attr, geom, st); break;
         case 2: launch_bwd_normal_sm<2>(ctx, fr, *sc, gC, gD, gA, gN, gcol, gopa, attr, geom, st); break;
         case 3: launch_bwd_normal_sm<3>(ctx, fr, *sc, gC, gD, gA, gN, gcol, gopa, attr, geom, st); break;
@@ -490,7 +494,7 @@ int32_t ts_launch_render_track_v1(const ts_ctx* ctx, ts_frame* fr, const ts_scen
                                   cudaStream_t st) {
     const double n = (double)fr->d.W * (double)fr->d.H;
     const float wc = (float)(1.0 / (3.0 * n)), wd = (float)((double)lambda_dep / n);
-    switch (ts_sigma_mode(fr->prm.sigma)) {
+    switch (ts_frame_sigma_mode(fr)) {
         case 1: launch_track<1>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, st); break;
         case 2: launch_track<2>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, st); break;
         case 3: launch_track<3>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, st); break;
@@ -511,7 +515,7 @@ int32_t ts_launch_render_map(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
     const float wc = (float)(1.0 / (3.0 * n)), wd = (float)((double)lambda_dep / n);
     float* gcol = (mask & TS_GRAD_COLOR) ? grad_color : nullptr;
     float* gopa = (mask & TS_GRAD_OPACITY) ? grad_opacity : nullptr;
-    switch (ts_sigma_mode(fr->prm.sigma)) {
+    switch (ts_frame_sigma_mode(fr)) {
         case 1: launch_map_sm<1>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, attr, geom, st); break;
         case 2: launch_map_sm<2>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, attr, geom, st); break;
         case 3: launch_map_sm<3>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, gcol, gopa, attr, geom, st); break;

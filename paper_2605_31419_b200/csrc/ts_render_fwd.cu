@@ -155,7 +155,7 @@ int32_t ts_launch_render_fwd_normal(const ts_ctx* ctx, ts_frame* fr, const ts_sc
     const uint32_t grid = (uint32_t)min((int64_t)ctx->num_sms * 4, ((int64_t)f.NT * TS_BLOCKS_PER_TILE + TS_JOB_WARPS - 1) / TS_JOB_WARPS);
     const float sg = fr->prm.sigma, am = fr->prm.alpha_min, tm = fr->prm.t_min;
     const FwdLoss none = {nullptr, nullptr, nullptr, nullptr, nullptr, 0.f, 0.f};
-    switch (ts_sigma_mode(fr->prm.sigma)) {
+    switch (ts_frame_sigma_mode(fr)) {
         case 1: render_fwd_kernel<1, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on, on_top); break;
         case 2: render_fwd_kernel<2, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on, on_top); break;
         case 3: render_fwd_kernel<3, false, false, false, true><<<grid, TS_JOB_WARPS * 32, 0, st>>>(f, *sc, sg, am, tm, oc, od, oa, none, nullptr, on, on_top); break;
@@ -181,7 +181,7 @@ int32_t ts_launch_render_fwd(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc
         L = FwdLoss{Chat, Dhat, gC, gD, loss, (float)(1.0 / (3.0 * n)), (float)((double)lambda_dep / n)};
         Lp = &L;
     }
-    switch (ts_sigma_mode(fr->prm.sigma)) {
+    switch (ts_frame_sigma_mode(fr)) {
         case 1: launch_sm<1>(ctx, fr, *sc, oc, od, oa, Lp, face_pixels, st); break;
         case 2: launch_sm<2>(ctx, fr, *sc, oc, od, oa, Lp, face_pixels, st); break;
         case 3: launch_sm<3>(ctx, fr, *sc, oc, od, oa, Lp, face_pixels, st); break;

@@ -316,7 +316,7 @@ int32_t ts_launch_render_track(const ts_ctx* ctx, ts_frame* fr, const ts_scene* 
     if (!ctx->track_log) return ts_launch_render_track_v1(ctx, fr, sc, oc, od, oa, Chat, Dhat, lambda_dep, gC, gD, loss, st);
     const double n = (double)fr->d.W * (double)fr->d.H;
     const float wc = (float)(1.0 / (3.0 * n)), wd = (float)((double)lambda_dep / n);
-    switch (ts_sigma_mode(fr->prm.sigma)) {
+    switch (ts_frame_sigma_mode(fr)) {
         case 1: launch_track_log<1>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, st); break;
         case 2: launch_track_log<2>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, st); break;
         case 3: launch_track_log<3>(ctx, fr, *sc, oc, od, oa, Chat, Dhat, wc, wd, gC, gD, loss, st); break;

@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(TsFrameDev f) {
 
 template <bool LOCAL>
 __global__ void __launch_bounds__(TS_BIN_THREADS)
-bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
+bin_setup_kernel(TsFrameDev f, TsCamDev cam, const float* __restrict__ face_sigma, float sigma_global) {
     __shared__ uint32_t s_offs[LOCAL ? TS_SCAN_LOCAL_MAX : 1];
     __shared__ uint32_t s_tmp[2 * (TS_BIN_THREADS / 32) + 2];
     __shared__ uint32_t s_hist[34];
@@ -193,6 +193,8 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam) {
         if (live) {
             float4 rec[TS_REC_F4];
             ts_build_record(s0, s1, s2, s2.y, cam, rec);
+            // row R3's last float: the face's window smoothness (reading S32; read by the generic-sigma kernels only)
+            rec[3].w = face_sigma ? __ldg(face_sigma + __float_as_uint(s3.x)) : sigma_global;
             float4* out = f.rec + TS_REC_F4 * (size_t)slot;
 #pragma unroll
             for (int i = 0; i < TS_REC_F4; ++i) out[i] = rec[i];
@@ -469,10 +471,10 @@ int32_t ts_launch_sort(const ts_ctx* ctx, ts_frame* fr, cudaStream_t stream) {
     const uint32_t grid_bin = (uint32_t)min((uint64_t)(f.vis_cap + TS_BIN_THREADS - 1) / TS_BIN_THREADS,
                                             (uint64_t)ctx->num_sms);
     if (f.NT <= TS_SCAN_LOCAL_MAX) {
-        bin_setup_kernel<true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam);
+        bin_setup_kernel<true><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->face_sigma, fr->prm.sigma);
     } else {
         tile_scan_kernel<<<1, 1024, 0, stream>>>(f);
-        bin_setup_kernel<false><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam);
+        bin_setup_kernel<false><<<grid_bin, TS_BIN_THREADS, 0, stream>>>(f, fr->cam, fr->face_sigma, fr->prm.sigma);
     }
     tile_sort_kernel<<<f.NT, TS_SORT_THREADS, 0, stream>>>(f, f.big_key, f.big_idx);
     TS_CUDA_CHECK_LAUNCH();

@@ -29,7 +29,7 @@ EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_map_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
            "ts_render_fwd_normal", "ts_render_bwd_normal", "ts_normal_loss_grad", "ts_render_bwd_stats",
            "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view",
-           "ts_fp32_probe", "ts_render_fwd_normal_top", "ts_depth_normalise", "ts_depth_normalise_bwd"]
+           "ts_fp32_probe", "ts_frame_set_face_sigma", "ts_render_fwd_normal_top", "ts_depth_normalise", "ts_depth_normalise_bwd"]
 
 
 class TsError(RuntimeError):
@@ -106,6 +106,7 @@ def _load():
     lib.ts_depth_normalise.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p]
     lib.ts_depth_normalise_bwd.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
                                            C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_frame_set_face_sigma.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_fp32_probe.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.POINTER(C.c_uint64), C.c_void_p]
     lib.ts_frame_release.argtypes = [C.c_void_p]
     lib.ts_destroy.argtypes = [C.c_void_p]
@@ -302,6 +303,13 @@ def ts_depth_normalise(ctx, W, H, D, A, eps, Dn, stream=None):
 def ts_depth_normalise_bwd(ctx, W, H, D, A, eps, gDn, gD, gA, stream=None):
     _check(lib.ts_depth_normalise_bwd(ctx.h, int(W), int(H), _ptr(D), _ptr(A), float(eps), _ptr(gDn), _ptr(gD), _ptr(gA),
                                       _stream(stream)))
+
+
+def ts_frame_set_face_sigma(ctx, frame, sigma, grad_sigma=None):
+    """Per-face window smoothness [M] (None = the global sigma again) and where dL/dsigma accumulates (may be None).
+    The frame keeps the tensors alive."""
+    frame._sigma_refs = (sigma, grad_sigma)
+    _check(lib.ts_frame_set_face_sigma(ctx.h, frame.h, _ptr(sigma), _ptr(grad_sigma)))
 
 
 def ts_fp32_probe(ctx, iters, scratch, stream=None):

@@ -884,3 +884,71 @@ def test_tight_binning_wide_faces(ctx, oracle_mod):
     assert o.project().tiles_touched.max() > 4
     check_forward(o, g)
     g.close()
+
+
+@pytest.mark.parametrize("cfg", [0, 2, 3])
+def test_per_face_sigma(ctx, oracle_mod, cfg):
+    """NEXT-4 remainder: per-face window smoothness (ts_frame_set_face_sigma, reading S32): images, all gradients incl.
+    dL/dsigma_m and the pose against the oracle; the fused launches; a constant array equals the global constant."""
+    from gpu_util import GpuView, assert_grad_close, assert_images_close, dev
+    from paper_2605_31419_b200 import ts
+    sc = small_cfg(cfg)
+    rng = np.random.default_rng(90 + cfg)
+    sig = rng.uniform(0.4, 2.0, sc.M).astype(np.float32)
+    o = oracle_mod.Oracle(sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params, "f32", amb_tol=5e-4, face_sigma=sig)
+    g = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
+    sig_d, gs_d = dev(sig), torch.zeros(sc.M, device="cuda")
+    ts.ts_frame_set_face_sigma(ctx, g.frame, sig_d, gs_d)
+    check_project_and_sort(o, g, sc.M)
+    f, ok = check_forward(o, g)
+    # the window really differs from the global-sigma render
+    plain = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
+    assert np.abs(plain.forward()[2] - g.A.cpu().numpy()).max() > 0.05
+    plain.close()
+    H, W = ok.shape
+    gC = (rng.normal(size=(3, H, W)) * ok[None]).astype(np.float32)
+    gD = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+    gA = (rng.normal(size=(H, W)) * ok).astype(np.float32)
+    ref = o.backward(gC, gD, gA)
+    gp, gc, go, tau = g.backward(gC, gD, gA, ts.GRAD_ALL)
+    torch.cuda.synchronize()
+    assert_grad_close("grad_pos", gp, ref.grad_pos)
+    assert_grad_close("grad_color", gc, ref.grad_color)
+    assert_grad_close("grad_opacity", go, ref.grad_opacity)
+    assert_grad_close("grad_sigma", gs_d.cpu().numpy(), ref.grad_sigma)
+    assert np.abs(tau - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max()
+    # pose-only mode and the fused tracking launch (both run the visit form with the generic exponent)
+    _, _, _, tau_p = g.backward(gC, gD, gA, ts.GRAD_POSE)
+    assert np.abs(tau_p - ref.dL_dtau).max() <= 1e-3 * np.abs(ref.dL_dtau).max()
+    tgt_pos = sc.pos_target if sc.pos_target is not None else sc.pos
+    tgt = oracle_mod.Oracle(tgt_pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params, "f32", face_sigma=sig).forward("tiled")
+    Chat, Dhat, lam = dev(tgt.color), dev(tgt.depth), sc.params.lambda_dep
+    C2, D2, A2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.empty_like(g.A)
+    gC2, gD2 = torch.empty_like(g.C), torch.empty_like(g.D)
+    ts.ts_render_track_l1(ctx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, lam, gC2, gD2, None)
+    tau2 = torch.zeros(6, device="cuda")
+    ts.ts_pose_jacobian_reduce(ctx, g.frame, tau2)
+    torch.cuda.synchronize()
+    assert torch.equal(C2, g.C) and torch.equal(A2, g.A)
+    ref2 = o.backward(gC2.cpu().numpy(), gD2.cpu().numpy(), None, want=("pose",))
+    assert np.abs(tau2.cpu().numpy() - ref2.dL_dtau).max() <= 1e-3 * np.abs(ref2.dL_dtau).max()
+    # the fused mapping launch accumulates dL/dsigma too
+    V = sc.pos.shape[0]
+    gs_d.zero_()
+    gp3, gc3, go3 = torch.zeros(V, 3, device="cuda"), torch.zeros(V, 3, device="cuda"), torch.zeros(V, device="cuda")
+    ts.ts_render_map_l1(ctx, g.scene, g.frame, None, None, None, Chat, Dhat, lam, gC2, gD2, None, gp3, gc3, go3, ts.GRAD_ALL)
+    torch.cuda.synchronize()
+    ref3 = o.backward(gC2.cpu().numpy(), gD2.cpu().numpy(), None)
+    assert_grad_close("grad_sigma (map)", gs_d.cpu().numpy(), ref3.grad_sigma)
+    assert_grad_close("grad_pos (map)", gp3.cpu().numpy(), ref3.grad_pos)
+    # a constant array is the global constant (generic exponent against the sqrt fast path: to rounding)
+    ts.ts_frame_set_face_sigma(ctx, g.frame, dev(np.full(sc.M, sc.params.sigma, np.float32)), None)
+    with pytest.raises(ts.TsError):
+        ts.ts_render_fwd(ctx, g.scene, g.frame, C2, D2, A2)            # the record is stale: project + bin again
+    g.projected = g.sorted = False
+    Cc, Dc, Ac = g.forward()
+    ts.ts_frame_set_face_sigma(ctx, g.frame, None, None)
+    g.projected = g.sorted = False
+    Cg, Dg, Ag = g.forward()
+    assert np.abs(Cc - Cg).max() <= 2e-5 and np.abs(Ac - Ag).max() <= 2e-5
+    g.close()
