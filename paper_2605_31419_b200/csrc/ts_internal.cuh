@@ -31,6 +31,7 @@ struct TsCtrl {
     uint32_t reduce_done;    // pose-reduction CTAs finished (zero at rest)
     uint32_t pad[2];
     unsigned long long counters[8];   // debug counters (TS_PARAM_COUNTERS)
+    uint32_t bucket_cursor[32];       // per list-length bucket: job headers published so far (zeroed by the sort kernel)
 };
 
 // Everything a kernel needs to know about a frame; passed by value.

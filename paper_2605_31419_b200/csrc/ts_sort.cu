@@ -29,31 +29,37 @@ struct TsGroup {
 
 // exclusive scan of tile_count[0..NT) by one CTA, in place in `offs` (shared memory, or global for the fallback).
 // Pass 1 copies the counts with coalesced loads (every binning CTA does this at the same time: strided loads would
-// multiply the L2 requests on the few slices that hold the 13 KB of counts); pass 2 gives every thread a contiguous
-// run of tiles (stride `per` words: conflict-free for odd `per`).  Returns the total and the longest list.
+// multiply the L2 requests on the few slices that hold the 13 KB of counts) unless the caller has done so already
+// (PRELOADED); pass 2 gives every thread a contiguous run of tiles (stride `per` words: conflict-free for odd
+// `per`) and, with `hist`, counts the tiles per list-length bucket (0 = empty, b = floor(log2 c) + 1; zeroed by the
+// caller).  Returns the total and the longest list.
+template <bool PRELOADED>
 __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* offs, uint32_t* s_tmp /*[2*warps+2]*/,
-                                               uint32_t& total, uint32_t& gmax, const TsGroup g) {
+                                               uint32_t& total, uint32_t& gmax, const TsGroup g, uint32_t* hist = nullptr) {
     const int tid = g.tid, lane = tid & 31, warp = tid >> 5, nwarp = g.n >> 5, nthr = g.n;
-    for (int base = 0; base < f.NT; base += 8 * nthr) {      // 8 independent loads in flight per thread
-        uint32_t c[8];
+    if (!PRELOADED) {
+        for (int base = 0; base < f.NT; base += 8 * nthr) {      // 8 independent loads in flight per thread
+            uint32_t c[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const int t = base + k * nthr + tid;
-            c[k] = t < f.NT ? __ldcg(f.tile_count + t) : 0u;
-        }
+            for (int k = 0; k < 8; ++k) {
+                const int t = base + k * nthr + tid;
+                c[k] = t < f.NT ? __ldcg(f.tile_count + t) : 0u;
+            }
 #pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const int t = base + k * nthr + tid;
-            if (t < f.NT) offs[t] = c[k];
+            for (int k = 0; k < 8; ++k) {
+                const int t = base + k * nthr + tid;
+                if (t < f.NT) offs[t] = c[k];
+            }
         }
+        g.sync();
     }
-    g.sync();
     const int per = ((f.NT + nthr - 1) / nthr) | 1;
     const int t0 = min(f.NT, tid * per), t1 = min(f.NT, t0 + per);
     uint32_t sum = 0, mx = 0;
     for (int t = t0; t < t1; ++t) {
         const uint32_t c = offs[t];
         sum += c, mx = max(mx, c);
+        if (hist) atomicAdd(&hist[32 - __clz(c)], 1u);
     }
     uint32_t incl = sum;
 #pragma unroll
@@ -89,7 +95,7 @@ __device__ __forceinline__ void cta_scan_tiles(const TsFrameDev& f, uint32_t* of
     g.sync();
 }
 
-// CTA 0 only: tile_ranges, frame counters, and the tile order (descending log2 bucket of the list length) that
+// One CTA (the fallback scan): tile_ranges, frame counters, and the tile order (descending log2 bucket of the list length) that
 // the persistent render kernels pull work in.  Counts are recovered from the offsets (no second trip to memory).
 __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_t* offs, uint32_t nv, uint32_t total,
                                               uint32_t gmax, uint32_t fl, uint32_t* s_hist /*[34]*/, const TsGroup g) {
@@ -132,13 +138,56 @@ __device__ __forceinline__ void publish_tiles(const TsFrameDev& f, const uint32_
     }
 }
 
+// One warp of every binning CTA: publishes the tile ranges and job headers of the CTA's slice of the tiles.  The
+// headers go into tile_order by descending list-length bucket: the bucket begins come from the CTA's own histogram
+// (every CTA has scanned all counts), the place inside a bucket from a cursor in global memory that all CTAs share
+// (the order inside a bucket is free).  CTA 0 also writes the frame counters.
+__device__ __forceinline__ void publish_slice(const TsFrameDev& f, const uint32_t* offs, uint32_t nv, uint32_t total,
+                                              uint32_t gmax, uint32_t fl, const uint32_t* hist) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t h = hist[31 - lane];                        // lane 0 = the heaviest bucket (lists < 2^31: b <= 31)
+    uint32_t incl = h;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+        if (lane >= d) incl += t;
+    }
+    const uint32_t start = incl - h;                            // begin of bucket 31 - lane
+    const int S = (f.NT + (int)gridDim.x - 1) / (int)gridDim.x;
+    const int t0 = min(f.NT, (int)blockIdx.x * S), t1 = min(f.NT, t0 + S);
+    for (int base = t0; base < t1; base += 32) {                // (warp-uniform)
+        const int t = base + lane;
+        const bool on = t < t1;
+        uint32_t o = 0, c = 0;
+        if (on) o = offs[t], c = (t + 1 < f.NT ? offs[t + 1] : total) - o;
+        const int b = on ? 32 - __clz(c) : 32;                  // 32 = the lanes past the slice
+        const uint32_t peers = __match_any_sync(0xffffffffu, b);
+        const int leader = __ffs(peers) - 1;
+        uint32_t at = 0;
+        if (on && lane == leader) at = atomicAdd(&f.ctrl->bucket_cursor[b], (uint32_t)__popc(peers));
+        at = __shfl_sync(0xffffffffu, at, leader);
+        const uint32_t bstart = __shfl_sync(0xffffffffu, start, (31 - b) & 31);
+        if (on) {
+            const bool empty = fl || c == 0u;
+            const uint32_t xy = (uint32_t)((t % f.tiles_x) * TS_TILE) | ((uint32_t)((t / f.tiles_x) * TS_TILE) << 16);
+            f.tile_ranges[t] = empty ? make_uint2(0u, 0u) : make_uint2(o, o + c);     // empty tile = (0,0)
+            f.tile_order[bstart + at + __popc(peers & ((1u << lane) - 1u))] =
+                empty ? make_uint4((uint32_t)t, 0u, 0u, xy) : make_uint4((uint32_t)t, o, o + c, xy);
+        }
+    }
+    if (blockIdx.x == 0 && lane == 0) {
+        volatile TsCtrl* ctrl = f.ctrl;
+        ctrl->n_visible = nv, ctrl->n_pairs = total, ctrl->flags = fl, ctrl->max_list = gmax;
+    }
+}
+
 // fallback for NT > TS_SCAN_LOCAL_MAX: one CTA scans into global memory
 __global__ void __launch_bounds__(1024) tile_scan_kernel(TsFrameDev f) {
     __shared__ uint32_t s_tmp[66];
     __shared__ uint32_t s_hist[34];
     uint32_t total, gmax;
     const TsGroup g{(int)threadIdx.x, (int)blockDim.x, 0};
-    cta_scan_tiles(f, f.tile_offset, s_tmp, total, gmax, g);
+    cta_scan_tiles<false>(f, f.tile_offset, s_tmp, total, gmax, g);
     const uint32_t nv = *(volatile uint32_t*)&f.ctrl->vis_counter;
     uint32_t fl = 0;
     if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
@@ -169,15 +218,32 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam, const float* __restrict__ face_sigm
     s0 = s1 = s2 = s3 = make_float4(0.f, 0.f, 0.f, 0.f);
     uint32_t nv = 0, fl = 0, total = 0, gmax = 0;
     const uint32_t* offs = s_offs;
-    if (scanner) {
-        cta_scan_tiles(f, s_offs, s_tmp, total, gmax, sg);
-        if (sg.tid == 0) s_tot[0] = total, s_tot[1] = gmax;
-    } else if (slot < f.vis_cap) {
+    if (!scanner && slot < f.vis_cap) {
         const float4* s4 = f.scr + TS_SCR_F4 * (size_t)slot;
         s0 = __ldcg(s4), s1 = __ldcg(s4 + 1), s2 = __ldcg(s4 + 2), s3 = __ldcg(s4 + 3);
     }
     if (LOCAL) {
+        // every thread of the CTA brings in its share of the tile counts (one round trip for all of them), then the
+        // scan warps take over
+        constexpr int PER = TS_SCAN_LOCAL_MAX / TS_BIN_THREADS;
+        uint32_t c[PER];
+#pragma unroll
+        for (int k = 0; k < PER; ++k) {
+            const int t = k * TS_BIN_THREADS + (int)threadIdx.x;
+            c[k] = t < f.NT ? __ldcg(f.tile_count + t) : 0u;
+        }
         nv = __ldcg(&f.ctrl->vis_counter);
+        if (threadIdx.x < 34) s_hist[threadIdx.x] = 0u;
+#pragma unroll
+        for (int k = 0; k < PER; ++k) {
+            const int t = k * TS_BIN_THREADS + (int)threadIdx.x;
+            if (t < f.NT) s_offs[t] = c[k];
+        }
+        __syncthreads();
+        if (scanner) {
+            cta_scan_tiles<true>(f, s_offs, s_tmp, total, gmax, sg, s_hist);
+            if (sg.tid == 0) s_tot[0] = total, s_tot[1] = gmax;
+        }
     } else {
         const volatile TsCtrl* ctrl = f.ctrl;
         nv = ctrl->n_visible, fl = ctrl->flags;
@@ -205,15 +271,15 @@ bin_setup_kernel(TsFrameDev f, TsCamDev cam, const float* __restrict__ face_sigm
             pb = (uint32_t)rhi;
         }
         if (!synced) {
-            // the offsets are ready from here on; the scan warps of the last CTA (it has the fewest slots) go on to
-            // publish the tile ranges, the frame counters and the job headers, the others are done
+            // the offsets are ready from here on; the first scan warp goes on to publish the CTA's share of the tile
+            // ranges and job headers (CTA 0: the frame counters too), the other scan warps are done
             __syncthreads();
             synced = true;
             total = s_tot[0], gmax = s_tot[1];
             if (total > f.pair_cap) fl |= TS_FLAG_OVERFLOW_PAIRS;
             if (nv > f.vis_cap) fl |= TS_FLAG_OVERFLOW_VISIBLE;
             if (scanner) {
-                if (blockIdx.x == gridDim.x - 1) publish_tiles(f, s_offs, nv, total, gmax, fl, s_hist, sg);
+                if (warp == SLOT_WARPS) publish_slice(f, s_offs, nv, total, gmax, fl, s_hist);
                 return;
             }
         }
@@ -373,6 +439,7 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
         f.tile_count[hb.x] = 0u, f.tile_cursor[hb.x] = 0u;
         if (b == 0) f.ctrl->vis_counter = 0u;
     }
+    if (b == 0 && tid < 32) f.ctrl->bucket_cursor[tid] = 0u;
     const uint32_t nb = hb.z - hb.y;
     if (nb > TS_SORT_WARP_MAX) {
         // ---- a long list: the whole CTA ------------------------------------------------------------------------
