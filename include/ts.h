@@ -67,7 +67,9 @@ int32_t ts_create(int32_t device, ts_ctx** out);
 int32_t ts_destroy(ts_ctx* ctx);
 
 /* Bytes of device workspace a frame needs for M faces, a WxH image, at most `pair_capacity` (tile, face)
- * pairs and at most `visible_capacity` faces surviving the cull (0 = M).  Returns 0 on invalid arguments. */
+ * pairs (< 2^28) and at most `visible_capacity` faces surviving the cull (0 = M; < 2^28).  About 208 B per pair
+ * (the sorted tile lists plus room for every pair in the lists of all eight 8x4 blocks of its tile), 290 B per
+ * visible face and 16 B per pixel.  Returns 0 on invalid arguments. */
 size_t ts_frame_bytes(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pair_capacity,
                       uint64_t visible_capacity);
 /* Carves `dev_ws` (device memory, >= ts_frame_bytes, 256-byte aligned) into the frame's arrays; allocates
@@ -254,7 +256,9 @@ enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slo
        TS_VIEW_KEYS = 1,         /* u64[n_pairs] sorted keys (tile << 32 | depth_key)                        */
        TS_VIEW_VALS = 2,         /* u32[n_pairs][4] sorted (slot, face, rect_lo, rect_hi) entries            */
        TS_VIEW_TILE_RANGES = 3,  /* u32[NT][2]                                                               */
-       TS_VIEW_N_CONTRIB = 4,    /* u32[H][W]                                                                */
+       TS_VIEW_N_CONTRIB = 4,    /* u32[H][W]: 1 + position in the TILE's sorted list of the pixel's last contributing
+                                    entry (0 = none); converted on demand from the renderers' per-block counts by a
+                                    small launch on `stream`; needs ts_bin_sort (TS_ERR_STATE otherwise)           */
        TS_VIEW_COUNTERS = 5 };   /* u64[8]: n_visit(warp-level), n_rect, n_hit, ... (TS_PARAM_COUNTERS only)  */
 /* Synchronises `stream`; returns the device pointer and element count of an internal array. */
 int32_t ts_frame_view(ts_ctx* ctx, ts_frame* frame, int32_t which, const void** dev_ptr, size_t* count,

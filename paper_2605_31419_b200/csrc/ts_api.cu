@@ -11,15 +11,15 @@ namespace {
 inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 struct Layout {
-    size_t ctrl, tile_count, tile_cursor, tile_offset, tile_order, tile_ranges, scr, rec, gscr, nrm, gnrm, pair_a, pair_b, big_key, big_idx, skey, sorted,
-        n_contrib, t_last,
+    size_t ctrl, tile_count, tile_cursor, tile_offset, tile_order, tile_ranges, scr, rec, gscr, nrm, gnrm, pair_a, pair_b, big_key, big_idx, skey, sorted, blist, job_order,
+        n_contrib, n_contrib_view, t_last,
         pose_partials, total;
     int32_t tiles_x, tiles_y, NT;
     uint32_t n_partials_cap;
 };
 
 bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pair_cap, uint64_t vis_cap, Layout& L) {
-    if (!ctx || M <= 0 || W <= 0 || H <= 0 || W > 32767 || H > 32767 || pair_cap == 0 || pair_cap >= (1ull << 30) ||
+    if (!ctx || M <= 0 || W <= 0 || H <= 0 || W > 32767 || H > 32767 || pair_cap == 0 || pair_cap >= (1ull << 28) ||
         vis_cap == 0 || vis_cap >= (1ull << 28) || (uint64_t)M >= (1ull << 28))
         return false;
     L.tiles_x = (W + TS_TILE - 1) / TS_TILE, L.tiles_y = (H + TS_TILE - 1) / TS_TILE, L.NT = L.tiles_x * L.tiles_y;
@@ -43,7 +43,10 @@ bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pa
     L.big_idx = take(4ull * pair_cap);
     L.skey = take(8ull * pair_cap);
     L.sorted = take(16ull * pair_cap);
+    L.blist = take(16ull * 8ull * pair_cap);
+    L.job_order = take(16ull * 8ull * L.NT);
     L.n_contrib = take(4ull * W * H);
+    L.n_contrib_view = take(4ull * W * H);
     L.t_last = take(4ull * W * H);
     L.pose_partials = take(24ull * (L.n_partials_cap + 32u));
     L.total = o;
@@ -133,7 +136,10 @@ int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_
     d.big_idx = reinterpret_cast<uint32_t*>(b + L.big_idx);
     d.skey = reinterpret_cast<unsigned long long*>(b + L.skey);
     d.sorted = reinterpret_cast<uint4*>(b + L.sorted);
+    d.blist = reinterpret_cast<uint4*>(b + L.blist);
+    d.job_order = reinterpret_cast<uint4*>(b + L.job_order);
     d.n_contrib = reinterpret_cast<uint32_t*>(b + L.n_contrib);
+    d.n_contrib_view = reinterpret_cast<uint32_t*>(b + L.n_contrib_view);
     d.t_last = reinterpret_cast<float*>(b + L.t_last);
     d.pose_partials = reinterpret_cast<float*>(b + L.pose_partials);
     fr->bytes = L.total, fr->base = dev_ws;
@@ -388,7 +394,16 @@ int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev
         case TS_VIEW_KEYS: *dev_ptr = d.skey, *count = np; break;
         case TS_VIEW_VALS: *dev_ptr = d.sorted, *count = 4 * np; break;
         case TS_VIEW_TILE_RANGES: *dev_ptr = d.tile_ranges, *count = 2 * (size_t)d.NT; break;
-        case TS_VIEW_N_CONTRIB: *dev_ptr = d.n_contrib, *count = (size_t)d.W * d.H; break;
+        case TS_VIEW_N_CONTRIB: {
+            // (the renderers keep block-list positions: converted to positions in the tile's list on demand)
+            if (!fr->have_sort) return TS_ERR_STATE;
+            if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
+            if (ts_launch_ncontrib_view(ctx, fr, (cudaStream_t)stream) != TS_OK ||
+                cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess)
+                return TS_ERR_CUDA;
+            *dev_ptr = d.n_contrib_view, *count = (size_t)d.W * d.H;
+            break;
+        }
         case TS_VIEW_COUNTERS: *dev_ptr = &d.ctrl->counters[0], *count = 8; break;
         default: return TS_ERR_INVALID_ARG;
     }

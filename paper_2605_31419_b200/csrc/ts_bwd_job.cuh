@@ -263,11 +263,10 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             // the forward walk of this job left exactly this chunk staged, rows 0-11, masks after the block cull
             lmask = (uint32_t)lane < n ? sm.lm[lane] : 0u;
         } else {
-            if ((uint32_t)lane < n) cur = f.sorted[job.range.x + lo + lane];
+            if ((uint32_t)lane < n) cur = f.blist[job.range.x + lo + lane];
             lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
         }
         hi = lo;
-        if (!__any_sync(0xffffffffu, lmask != 0u)) continue;
         __syncwarp();
         if (lmask && !prestaged) {
             // staged at the lane's own index (no compaction); the walk follows the set bits of `ov` backwards
@@ -277,7 +276,7 @@ __device__ __forceinline__ void ts_bwd_walk(const TsFrameDev& f, const ts_scene&
             for (int i = 0; i < (POSE ? 10 : 8); ++i) r[i] = __ldg(rp + i);
             float col[9];
             ts_load_colors(sc, cur.y, col);
-            if (ts_block_misses(job, cur, r[0], r[1], r[2])) lmask = 0u;
+            if (ts_job_block_misses(job, cur, r[0], r[1], r[2])) lmask = 0u;
             float4* d = sm.r[lane];
             d[0] = r[0], d[1] = r[1], d[2] = r[2];
             d[3] = make_float4(r[3].x, r[3].y, r[3].z, col[0]);

@@ -44,9 +44,8 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
     for (uint32_t c0 = job.range.x; c0 < job.range.y && !warp_done; c0 += 32) {
         const uint32_t n = min(32u, job.range.y - c0);
         const uint4 cur = ent;
-        if (c0 + 32 + lane < job.range.y) ent = f.sorted[c0 + 32 + lane];    // prefetch the next chunk
-        uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
-        if (!__any_sync(0xffffffffu, lmask != 0u)) continue;
+        if (c0 + 32 + lane < job.range.y) ent = f.blist[c0 + 32 + lane];     // prefetch the next chunk
+        uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;   // (never 0 for an entry of the block's list)
         __syncwarp();                                   // previous chunk's reads are done
         if (lmask) {
             // records are staged at the lane's own index (no compaction: nothing has to stay in registers
@@ -55,7 +54,7 @@ __device__ __forceinline__ void ts_fwd_walk(const TsFrameDev& f, const ts_scene&
             const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2), r3 = __ldg(rp + 3);
             float col[9];
             ts_load_colors(sc, cur.y, col);
-            if (ts_block_misses(job, cur, r0, r1, r2)) lmask = 0u;
+            if (ts_job_block_misses(job, cur, r0, r1, r2)) lmask = 0u;
             sm.r[lane][0] = r0, sm.r[lane][1] = r1, sm.r[lane][2] = r2;
             sm.r[lane][3] = make_float4(r3.x, r3.y, r3.z, col[0]);
             sm.r[lane][4] = make_float4(col[1], col[2], col[3], col[4]);

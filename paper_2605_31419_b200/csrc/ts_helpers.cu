@@ -249,3 +249,34 @@ extern "C" int32_t ts_fp32_probe(ts_ctx* ctx, int32_t iters, float* scratch_dev,
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }
+
+// TS_VIEW_N_CONTRIB: the renderers count a pixel's last contributing entry in its BLOCK's list (ts_jobs.cuh); the
+// view gives it as 1 + the entry's position in the TILE's sorted list, the oracle's n_contrib.
+namespace {
+__global__ void __launch_bounds__(256) ncontrib_view_kernel(TsFrameDev f) {
+    const uint32_t j = (blockIdx.x * 256u + threadIdx.x) >> 5, lane = threadIdx.x & 31u;
+    if (j >= (uint32_t)f.NT * 8u) return;
+    const uint4 h = f.job_order[j];
+    const int blk = (int)(h.x >> 28);
+    const int px = (int)(h.w & 0xffffu) + ((blk & 1) << 3) + (int)(lane & 7u), py = (int)(h.w >> 16) + ((blk >> 1) << 2) + (int)(lane >> 3);
+    if (px >= f.W || py >= f.H) return;
+    const size_t p = (size_t)py * f.W + px;
+    const uint32_t nb = h.z > h.y ? f.n_contrib[p] : 0u;
+    uint32_t pos = 0;
+    if (nb) {
+        // (a debug accessor: a linear search of the tile's list for the entry's slot, which is unique in it)
+        const uint32_t slot = f.blist[h.y + nb - 1u].x;
+        const uint2 tr = f.tile_ranges[h.x & 0x0fffffffu];
+        for (uint32_t i = tr.x; i < tr.y; ++i)
+            if (f.sorted[i].x == slot) { pos = i - tr.x + 1u; break; }
+    }
+    f.n_contrib_view[p] = pos;
+}
+}  // namespace
+
+int32_t ts_launch_ncontrib_view(const ts_ctx*, ts_frame* fr, cudaStream_t st) {
+    const uint32_t threads = (uint32_t)fr->d.NT * 8u * 32u;
+    ncontrib_view_kernel<<<(threads + 255u) / 256u, 256, 0, st>>>(fr->d);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}

@@ -43,7 +43,7 @@ struct TsFrameDev {
     uint32_t* tile_count;             // [NT] pairs per tile, counted by the project kernel (zeroed by the sort kernel)
     uint32_t* tile_cursor;            // [NT] write cursor of the binning pass, relative to the tile's begin (zero at rest)
     uint32_t* tile_offset;            // [NT] exclusive scan of tile_count (only used when NT > TS_SCAN_LOCAL_MAX)
-    uint4* tile_order;                // [NT] job headers (tile, begin, end, x0 | y0 << 16), tiles by descending list length
+    uint4* tile_order;                // [NT] tile headers (tile, begin, end, x0 | y0 << 16), tiles by descending list length
     uint2* tile_ranges;               // [NT] (begin, end) into the pair arrays
     float4* scr;                      // [vis_cap][4]: (u0,v0,w0,u1) (v1,w1,u2,v2) (w2,obar,rect_lo,rect_hi) (face,key,tiles,0)
     float4* rec;                      // [vis_cap][10]: per-face render record, see ts_raster.cuh
@@ -56,7 +56,14 @@ struct TsFrameDev {
     uint32_t* big_idx;                // [pair_cap] scratch of the oversize-segment sort
     unsigned long long* skey;         // [pair_cap] sorted: tile << 32 | depth_key
     uint4* sorted;                    // [pair_cap] sorted: (slot, face, rect_lo, rect_hi)
-    uint32_t* n_contrib;              // [H*W]
+    uint4* blist;                     // [8 * pair_cap] per-BLOCK lists, what the renderers walk: the entries (slot, face,
+                                      // rect_lo, rect_hi) of a tile's sorted list whose pixel rect overlaps the 8x4-pixel
+                                      // block, in list order; block k of a tile whose list is [b, e) owns
+                                      // [8 b + k (e - b), 8 b + (k + 1)(e - b))
+    uint4* job_order;                 // [8 * NT] job headers (tile | block << 28, begin, end into blist, x0 | y0 << 16);
+                                      // job 8 p + k = block k of the tile at position p of tile_order
+    uint32_t* n_contrib;              // [H*W] per pixel: 1 + the position IN ITS BLOCK'S LIST of the last contributing entry
+    uint32_t* n_contrib_view;         // [H*W] scratch of TS_VIEW_N_CONTRIB (positions in the tile's list)
     float* t_last;                    // [H*W] transmittance in front of the last contributing face
     float* pose_partials;             // [n_partials_cap][6], then [32][6] block partials of the final reduction
     uint32_t n_partials_cap;
@@ -142,6 +149,7 @@ int32_t ts_launch_render_fwd(const ts_ctx*, ts_frame*, const ts_scene*, float* o
                              const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, uint32_t* face_pixels,
                              cudaStream_t);
 int32_t ts_launch_face_area(const ts_ctx*, ts_frame*, float* area, cudaStream_t);
+int32_t ts_launch_ncontrib_view(const ts_ctx*, ts_frame*, cudaStream_t);
 int32_t ts_launch_render_fwd_normal(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, float* on,
                                     cudaStream_t, float* on_top = nullptr);
 int32_t ts_launch_render_bwd_normal(const ts_ctx*, ts_frame*, const ts_scene*, const float* gC, const float* gD,

@@ -1,8 +1,9 @@
 // ts_jobs.cuh -- work distribution of the compositing kernels.
 //
 // A JOB is one 8x4-pixel block of one 16x16 tile, owned by ONE WARP from start to finish: the warp reads the
-// tile's sorted list 32 entries at a time, keeps the entries whose pixel rect overlaps its block (one lane mask per
-// entry, one ballot per chunk), copies their records into its private slice of shared memory and walks them.
+// BLOCK's list (the entries of the tile's sorted list whose pixel rect overlaps the block, in list order; built once
+// per frame by the sort kernel) 32 entries at a time, drops those whose triangle misses the block (exact cull, one
+// entry per lane), copies the records of the others into its private slice of shared memory and walks them.
 // There is no CTA-wide barrier anywhere: warps never wait for each other, so a crowded block does not stall the
 // seven other blocks of its tile, and nobody idles while records are being fetched.
 //
@@ -44,38 +45,27 @@ __device__ __forceinline__ void ts_job_finish(const TsFrameDev& f, int which, in
 }
 
 __device__ __forceinline__ void ts_job_decode(const TsFrameDev& f, uint32_t j, int lane, TsJob& job) {
-    const uint4 h = __ldg(f.tile_order + (j >> 3));         // (tile, begin, end, x0 | y0 << 16): one load per job
-    job.tile = (int)h.x;
-    job.blk = (int)(j & 7u);
+    const uint4 h = __ldg(f.job_order + j);     // (tile | block << 28, begin, end, x0 | y0 << 16): one load per job
+    job.tile = (int)(h.x & 0x0fffffffu);
+    job.blk = (int)(h.x >> 28);
     job.tx0 = (int)(h.w & 0xffffu), job.ty0 = (int)(h.w >> 16);
     job.px = job.tx0 + ((job.blk & 1) << 3) + (lane & 7);
     job.py = job.ty0 + ((job.blk >> 1) << 2) + (lane >> 3);
     job.inside = job.px < f.W && job.py < f.H;
-    job.range = make_uint2(h.y, h.z);
+    job.range = make_uint2(h.y, h.z);           // the block's list in f.blist
 }
 
-// lane mask of a sorted-list entry (slot, face, rect_lo, rect_hi) for this job's block
+// lane mask of a list entry (slot, face, rect_lo, rect_hi) for this job's block
 __device__ __forceinline__ uint32_t ts_entry_mask(const TsJob& job, const uint4 ent) {
     const int rlo = (int)ent.z, rhi = (int)ent.w;
     const int rx0 = max((int)(short)(rlo & 0xffff) - job.tx0, 0), ry0 = max((rlo >> 16) - job.ty0, 0);
     const int rx1 = min((int)(short)(rhi & 0xffff) - job.tx0, 15), ry1 = min((rhi >> 16) - job.ty0, 15);
     return ts_lane_mask(job.blk, rx0, ry0, rx1, ry1);
 }
-
-// Exact block cull: the entry's rect overlaps the block, but does the TRIANGLE?  For each edge the normalised edge
-// function is evaluated at the corner of (rect n block) where it is smallest; if that minimum is already above the
-// refinement band, every pixel of the block has x < -band for this face: no hit, and no refinement either, so
-// dropping the entry cannot change any result.  r0..r2 = record rows R0-R2.
-__device__ __forceinline__ bool ts_block_misses(const TsJob& job, const uint4 ent, const float4 r0, const float4 r1,
-                                                const float4 r2) {
-    const int rlo = (int)ent.z, rhi = (int)ent.w;
-    const int bx = job.tx0 + ((job.blk & 1) << 3), by = job.ty0 + ((job.blk >> 1) << 2);
-    const float x0 = (float)max((int)(short)(rlo & 0xffff), bx) - r0.x, x1 = (float)min((int)(short)(rhi & 0xffff), bx + 7) - r0.x;
-    const float y0 = (float)max(rlo >> 16, by) - r0.y, y1 = (float)min(rhi >> 16, by + 3) - r0.y;
-    const float l0 = fmaf(r0.z, r0.z > 0.f ? x0 : x1, fmaf(r0.w, r0.w > 0.f ? y0 : y1, r2.x));
-    const float l1 = fmaf(r1.x, r1.x > 0.f ? x0 : x1, fmaf(r1.y, r1.y > 0.f ? y0 : y1, r2.y));
-    const float l2 = fmaf(r1.z, r1.z > 0.f ? x0 : x1, fmaf(r1.w, r1.w > 0.f ? y0 : y1, r2.z));
-    return fmaxf(l0, fmaxf(l1, l2)) > 4.0f * TS_REFINE_BAND;
+// the exact cull of ts_raster.cuh for this job's block
+__device__ __forceinline__ bool ts_job_block_misses(const TsJob& job, const uint4 ent, const float4 r0, const float4 r1,
+                                                    const float4 r2) {
+    return ts_block_misses(job.tx0 + ((job.blk & 1) << 3), job.ty0 + ((job.blk >> 1) << 2), (int)ent.z, (int)ent.w, r0, r1, r2);
 }
 
 // the nine vertex-colour floats of a face

@@ -225,3 +225,18 @@ __device__ __forceinline__ uint32_t ts_lane_mask(int w, int rx0, int ry0, int rx
     const uint32_t rows = (0xffffffffu >> (8 * (3 - cy1))) & (0xffffffffu << (8 * cy0));
     return (col * 0x01010101u) & rows;
 }
+
+// Exact block cull (run by the render kernels when they stage an entry of a block's list): the entry's rect
+// overlaps the block with origin (bx, by), but does the TRIANGLE?  For each edge the normalised edge function is
+// evaluated at the corner of (rect n block) where it is smallest; if that minimum is already above the refinement
+// band, every pixel of the block has x < -band for this face: no hit, and no refinement either, so dropping the
+// entry cannot change any result.  r0..r2 = record rows R0-R2; (rlo, rhi) = the entry's pixel rect.
+__device__ __forceinline__ bool ts_block_misses(int bx, int by, int rlo, int rhi, const float4 r0, const float4 r1,
+                                                const float4 r2) {
+    const float x0 = (float)max((int)(short)(rlo & 0xffff), bx) - r0.x, x1 = (float)min((int)(short)(rhi & 0xffff), bx + 7) - r0.x;
+    const float y0 = (float)max(rlo >> 16, by) - r0.y, y1 = (float)min(rhi >> 16, by + 3) - r0.y;
+    const float l0 = fmaf(r0.z, r0.z > 0.f ? x0 : x1, fmaf(r0.w, r0.w > 0.f ? y0 : y1, r2.x));
+    const float l1 = fmaf(r1.x, r1.x > 0.f ? x0 : x1, fmaf(r1.y, r1.y > 0.f ? y0 : y1, r2.y));
+    const float l2 = fmaf(r1.z, r1.z > 0.f ? x0 : x1, fmaf(r1.w, r1.w > 0.f ? y0 : y1, r2.z));
+    return fmaxf(l0, fmaxf(l1, l2)) > 4.0f * TS_REFINE_BAND;
+}

@@ -111,8 +111,10 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
         TsJob job;
         ts_job_decode(f, j, lane, job);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
-        if (job.range.x + lane < job.range.y) ent = f.sorted[job.range.x + lane];
-        j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
+        if (job.range.x + lane < job.range.y) ent = f.blist[job.range.x + lane];
+        // next ticket: requested now, read (the shuffle) at the end of this job, so that nobody waits for its round trip
+        uint32_t j_next = 0;
+        if (lane == 0) j_next = atomicAdd(&f.ctrl->job_ticket[0], 1u);
         FwdPix o;
         // the chunk the forward walk staged last (with the whole record) is where the backward walk begins
         uint32_t staged_lo = 0xffffffffu;
@@ -154,6 +156,7 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
             }
         }
         __syncwarp();
+        j = __shfl_sync(0xffffffffu, j_next, 0);
     }
     ts_job_finish(f, 0, lane);
     if (loss) {

@@ -55,7 +55,7 @@ __device__ __forceinline__ void tl_fwd_walk(const TsFrameDev& f, const ts_scene&
     for (uint32_t c0 = job.range.x; c0 < job.range.y && !warp_done; c0 += 32) {
         const uint32_t n = min(32u, job.range.y - c0);
         const uint4 cur = ent;
-        if (c0 + 32 + lane < job.range.y) ent = f.sorted[c0 + 32 + lane];    // prefetch the next chunk
+        if (c0 + 32 + lane < job.range.y) ent = f.blist[c0 + 32 + lane];     // prefetch the next chunk
         uint32_t lmask = (uint32_t)lane < n ? ts_entry_mask(job, cur) : 0u;
         if (!__any_sync(TL_FULL, lmask != 0u)) continue;
         __syncwarp();                                   // previous chunk's reads are done
@@ -64,7 +64,7 @@ __device__ __forceinline__ void tl_fwd_walk(const TsFrameDev& f, const ts_scene&
             const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2), r3 = __ldg(rp + 3);
             float col[9];
             ts_load_colors(sc, cur.y, col);
-            if (ts_block_misses(job, cur, r0, r1, r2)) lmask = 0u;
+            if (ts_job_block_misses(job, cur, r0, r1, r2)) lmask = 0u;
             st.r[lane][0] = r0, st.r[lane][1] = r1, st.r[lane][2] = r2;
             st.r[lane][3] = make_float4(r3.x, r3.y, r3.z, col[0]);
             st.r[lane][4] = make_float4(col[1], col[2], col[3], col[4]);
@@ -169,7 +169,7 @@ __device__ __forceinline__ void tl_chain(LogWarpSmem<CAP>& sm, uint32_t fi, floa
 }
 
 // geometry phase: one logged hit per lane, through B4-B7 + B9 (Eq. 5-7) into the lane's six accumulators.  The entry
-// (slot, face) is read again from the tile's sorted list, the record and the colours from global memory / L1, and
+// (slot, face) is read again from the block's list, the record and the colours from global memory / L1, and
 // lhat_k is formed again exactly as the forward walk formed it (ts_eval_alpha: same operations, same refinement rule).
 template <int SM, int CAP>
 __device__ __forceinline__ void tl_geometry(const LogWarpSmem<CAP>& sm, const TsFrameDev& f, const ts_scene& sc, const TsJob& job,
@@ -179,7 +179,7 @@ __device__ __forceinline__ void tl_geometry(const LogWarpSmem<CAP>& sm, const Ts
         if (fi >= used) continue;
         const float2 zc = sm.fz[fi];
         const uint32_t code = __float_as_uint(zc.y), pl = (code >> 8) & 31u;
-        const uint4 ent = __ldg(f.sorted + job.range.x + (code >> 13));          // (slot, face, rect_lo, rect_hi)
+        const uint4 ent = __ldg(f.blist + job.range.x + (code >> 13));           // (slot, face, rect_lo, rect_hi)
         const float4* rp = f.rec + TS_REC_F4 * (size_t)ent.x;
         const float4 r0 = __ldg(rp), r1 = __ldg(rp + 1), r2 = __ldg(rp + 2), r3 = __ldg(rp + 3);
         const float4 q4 = __ldg(rp + 4), q5 = __ldg(rp + 5), q6 = __ldg(rp + 6), q7 = __ldg(rp + 7), n0 = __ldg(rp + 8), n1 = __ldg(rp + 9);
@@ -237,7 +237,7 @@ render_track_log_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min,
         TsJob job;
         ts_job_decode(f, j, lane, job);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
-        if (job.range.x + lane < job.range.y) ent = f.sorted[job.range.x + lane];
+        if (job.range.x + lane < job.range.y) ent = f.blist[job.range.x + lane];
         j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
         FwdPix o;
         uint32_t used, mylast;

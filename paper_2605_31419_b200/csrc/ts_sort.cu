@@ -415,6 +415,79 @@ __device__ __forceinline__ void emit_sorted(const TsFrameDev& f, uint32_t base, 
     f.skey[base + rank] = thi | a.x;
 }
 
+// Per-block lists (what the render kernels walk).  Once a tile's list [h.y, h.z) is sorted, the group that sorted it
+// (one warp, NW = 1, or the whole CTA) goes through it in order and copies every entry to the end of the list of each
+// of the tile's eight 8x4 blocks its pixel rect overlaps (ordered compaction: ballots inside a warp, per-warp counts in
+// shared memory across the CTA; integer work only -- the exact triangle-vs-block cull stays with the render kernels,
+// which have the face records at hand).  Block k of the tile owns blist[8 h.y + k n ...) (n = the tile's list
+// length: no allocation, no overflow).  Then the eight job headers of the tile, at the tile's position `p` of
+// tile_order.  SRC_SMEM: the sorted entries are in shared memory (the rank sorts leave them there), otherwise they are
+// read back from f.sorted.
+template <int NW, bool SRC_SMEM>
+__device__ __forceinline__ void build_block_lists(const TsFrameDev& f, uint32_t p, const uint4 h, uint32_t gtid,
+                                                  uint32_t (*wcnt)[8][NW] /* shared [2][8][NW], NW > 1 only */,
+                                                  const uint4* se = nullptr) {
+    const uint32_t lane = gtid & 31u, w = gtid >> 5, lt = (1u << lane) - 1u;
+    const uint32_t n = h.z - h.y;
+    const int tx0 = (int)(h.w & 0xffffu), ty0 = (int)(h.w >> 16);
+    uint4* out = f.blist + 8 * (size_t)h.y;
+    uint32_t run[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) run[k] = 0u;
+    uint32_t par = 0;
+    for (uint32_t c = 0; c < n; c += 32u * NW, par ^= 1u) {          // (uniform over the group)
+        const uint32_t i = c + gtid;
+        uint4 ent = make_uint4(0u, 0u, 0u, 0u);
+        uint32_t bits = 0;
+        if (i < n) {
+            ent = SRC_SMEM ? se[i] : __ldcg(f.sorted + h.y + i);     // (f.sorted: written by this group a moment ago)
+            // columns / rows of blocks the rect reaches: x in [tx0 + 8 c, +7], y in [ty0 + 4 r, +3]
+            const int x0 = (int)(short)(ent.z & 0xffffu) - tx0, y0 = ((int)ent.z >> 16) - ty0;
+            const int x1 = (int)(short)(ent.w & 0xffffu) - tx0, y1 = ((int)ent.w >> 16) - ty0;
+            const uint32_t cols = (x0 <= 7 && x1 >= 0 ? 1u : 0u) | (x0 <= 15 && x1 >= 8 ? 2u : 0u);
+#pragma unroll
+            for (int r = 0; r < 4; ++r)
+                if (y0 <= 4 * r + 3 && y1 >= 4 * r) bits |= cols << (2 * r);
+        }
+        uint32_t bal[8], before[8], mine = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            bal[k] = __ballot_sync(0xffffffffu, (bits >> k) & 1u);
+            before[k] = 0u;
+            if ((int)lane == k) mine = (uint32_t)__popc(bal[k]);
+        }
+        if (NW > 1) {
+            if (lane < 8u) wcnt[par][lane][w] = mine;
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                uint32_t tot = 0;
+#pragma unroll
+                for (int ww = 0; ww < NW; ++ww) {
+                    const uint32_t cw = wcnt[par][k][ww];
+                    if ((uint32_t)ww < w) before[k] += cw;
+                    tot += cw;
+                }
+                bal[k] &= lt;
+                before[k] += run[k], run[k] += tot;
+            }
+        } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) before[k] = run[k], run[k] += (uint32_t)__popc(bal[k]), bal[k] &= lt;
+        }
+#pragma unroll
+        for (int k = 0; k < 8; ++k)
+            if ((bits >> k) & 1u) out[(uint32_t)k * n + before[k] + (uint32_t)__popc(bal[k])] = ent;
+    }
+    if (gtid < 8u) {
+        uint32_t cnt = run[0];
+#pragma unroll
+        for (int k = 1; k < 8; ++k) cnt = gtid == (uint32_t)k ? run[k] : cnt;
+        const uint32_t b0 = 8u * h.y + gtid * n;
+        f.job_order[8 * (size_t)p + gtid] = make_uint4(h.x | (gtid << 28), b0, b0 + cnt, h.w);
+    }
+}
+
 // One CTA per position b of the job-header array tile_order (tiles by descending list length, written by the binning
 // kernel; every tile appears once).  A LONG list (more than TS_SORT_WARP_MAX pairs) is sorted by the CTA at its own
 // position: rank sort up to 2 x threads, compare-exchange network in shared memory up to TS_SORT_SMEM, the same
@@ -429,6 +502,8 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
                                                                     uint32_t* __restrict__ gidx) {
     __shared__ unsigned long long sk[TS_SORT_SMEM];
     __shared__ uint32_t sv[TS_SORT_SMEM];
+    __shared__ uint32_t wcnt[2][8][TS_SORT_THREADS / 32];
+    __shared__ uint4 se[2 * TS_SORT_THREADS];               // the sorted entries (rank-sort paths)
     const uint32_t tid = threadIdx.x, lane = tid & 31u, warp = tid >> 5, b = blockIdx.x;
     const bool leader = (b % TS_SORT_TILES) == 0;
     const uint4 hb = __ldcg(f.tile_order + b);              // (tile, begin, end, xy)
@@ -467,10 +542,17 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
                     const unsigned long long mine = ((unsigned long long)a[k].x << 32) | a[k].y;
                     uint32_t rank = 0;
                     for (uint32_t j = 0; j < n; ++j) rank += (sk[j] < mine) ? 1u : 0u;
-                    f.sorted[range.x + rank] = make_uint4(a[k].z, a[k].y, a[k].w, bb[k]);   // (slot, face, rect_lo, rect_hi)
+                    const uint4 ent = make_uint4(a[k].z, a[k].y, a[k].w, bb[k]);            // (slot, face, rect_lo, rect_hi)
+                    f.sorted[range.x + rank] = ent;
                     f.skey[range.x + rank] = thi | a[k].x;
+                    se[rank] = ent;
                 }
             }
+            __syncthreads();
+            build_block_lists<TS_SORT_THREADS / 32, true>(f, b, hb, tid, wcnt, se);
+            if (!leader) return;
+            __syncthreads();
+            goto short_lists;
         } else if (n <= TS_SORT_SMEM) {
             for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) {
                 const uint4 a = f.pair_a[range.x + i];
@@ -493,14 +575,22 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
             cta_sort_network((volatile unsigned long long*)gk, (volatile uint32_t*)gv, n);
             for (uint32_t i = tid; i < n; i += TS_SORT_THREADS) emit_sorted(f, range.x, i, gv[i], thi);
         }
+        __syncthreads();                                    // the sorted list is complete (and visible to the CTA)
+        build_block_lists<TS_SORT_THREADS / 32, false>(f, b, hb, tid, wcnt);
         if (!leader) return;
         __syncthreads();                                    // the shared arrays are re-used below
     }
-    if (!leader) return;
+short_lists:
+    if (!leader || b + warp >= (uint32_t)f.NT) return;
     // ---- the group's short lists: one warp each ------------------------------------------------------------------
     const uint32_t n = hw.z - hw.y;
-    if (n == 0 || n > TS_SORT_WARP_MAX) return;
+    if (n > TS_SORT_WARP_MAX) return;                       // (sorted by the CTA at its own position)
+    if (n == 0) {                                           // an empty tile still has its eight (empty) jobs
+        if (lane < 8u) f.job_order[8 * (size_t)(b + warp) + lane] = make_uint4(hw.x | (lane << 28), 0u, 0u, hw.w);
+        return;
+    }
     unsigned long long* wk = sk + warp * TS_SORT_WARP_MAX;
+    uint4* we = se + warp * TS_SORT_WARP_MAX;
     const unsigned long long thi = (unsigned long long)hw.x << 32;
     uint4 a[2];
     uint32_t bb[2];
@@ -525,10 +615,14 @@ __global__ void __launch_bounds__(TS_SORT_THREADS) tile_sort_kernel(TsFrameDev f
     for (int k = 0; k < 2; ++k) {
         const uint32_t i = lane + 32u * k, rank = k ? r1 : r0;
         if (i < n) {
-            f.sorted[hw.y + rank] = make_uint4(a[k].z, a[k].y, a[k].w, bb[k]);
+            const uint4 ent = make_uint4(a[k].z, a[k].y, a[k].w, bb[k]);
+            f.sorted[hw.y + rank] = ent;
             f.skey[hw.y + rank] = thi | a[k].x;
+            we[rank] = ent;
         }
     }
+    __syncwarp();
+    build_block_lists<1, true>(f, b + warp, hw, lane, nullptr, we);
 }
 
 }  // namespace
