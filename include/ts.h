@@ -259,7 +259,13 @@ enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slo
        TS_VIEW_N_CONTRIB = 4,    /* u32[H][W]: 1 + position in the TILE's sorted list of the pixel's last contributing
                                     entry (0 = none); converted on demand from the renderers' per-block counts by a
                                     small launch on `stream`; needs ts_bin_sort (TS_ERR_STATE otherwise)           */
-       TS_VIEW_COUNTERS = 5 };   /* u64[8]: n_visit(warp-level), n_rect, n_hit, ... (TS_PARAM_COUNTERS only)  */
+       TS_VIEW_COUNTERS = 5,     /* u64[8]: n_visit(warp-level), n_rect, n_hit, ... (TS_PARAM_COUNTERS only)  */
+       TS_VIEW_JOBS = 6,         /* u32[8 NT][4] job headers of the render kernels, in ticket order: (tile | block << 28,
+                                    begin, end, x0 | y0 << 16); block b = 2 row + column of the tile's 2 x 4 blocks of
+                                    8x4 pixels; [begin, end) indexes TS_VIEW_BLOCK_LISTS in entries of four u32        */
+       TS_VIEW_BLOCK_LISTS = 7 };/* u32[8 n_pairs][4]: the per-block lists: for every job the entries (slot, face,
+                                    rect_lo, rect_hi) of its tile's sorted list whose pixel rect overlaps the block, in
+                                    list order (only the ranges named by the job headers are defined)                  */
 /* Synchronises `stream`; returns the device pointer and element count of an internal array. */
 int32_t ts_frame_view(ts_ctx* ctx, ts_frame* frame, int32_t which, const void** dev_ptr, size_t* count,
                       void* stream);

@@ -405,6 +405,14 @@ int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev
             break;
         }
         case TS_VIEW_COUNTERS: *dev_ptr = &d.ctrl->counters[0], *count = 8; break;
+        case TS_VIEW_JOBS:
+            if (!fr->have_sort) return TS_ERR_STATE;
+            *dev_ptr = d.job_order, *count = 4 * 8 * (size_t)d.NT;
+            break;
+        case TS_VIEW_BLOCK_LISTS:
+            if (!fr->have_sort) return TS_ERR_STATE;
+            *dev_ptr = d.blist, *count = 4 * 8 * np;
+            break;
         default: return TS_ERR_INVALID_ARG;
     }
     return TS_OK;

@@ -23,11 +23,18 @@ struct TsJob {
     bool inside;
 };
 
-// which = 0 forward, 1 backward
-__device__ __forceinline__ uint32_t ts_job_take(const TsFrameDev& f, int which, int lane) {
+// which = 0 forward, 1 backward.  The ticket is REQUESTED by lane 0 (ts_job_request) and READ later (ts_job_ticket, a
+// shuffle), so that its round trip to L2 overlaps whatever lies in between.  Inline PTX on purpose: nvcc turns
+// `if (lane == 0) atomicAdd(p, 1)` into a warp-aggregated atomic whose broadcast shuffle waits for the result on the
+// spot (5 % of the fused kernel's stall samples sat on that shuffle).
+__device__ __forceinline__ uint32_t ts_job_request(const TsFrameDev& f, int which, int lane) {
     uint32_t j = 0;
-    if (lane == 0) j = atomicAdd(&f.ctrl->job_ticket[which], 1u);
-    return __shfl_sync(0xffffffffu, j, 0);
+    if (lane == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(j) : "l"(&f.ctrl->job_ticket[which]) : "memory");
+    return j;
+}
+__device__ __forceinline__ uint32_t ts_job_ticket(uint32_t requested) { return __shfl_sync(0xffffffffu, requested, 0); }
+__device__ __forceinline__ uint32_t ts_job_take(const TsFrameDev& f, int which, int lane) {
+    return ts_job_ticket(ts_job_request(f, which, lane));
 }
 
 // total = persistent warps of the launch

@@ -55,7 +55,7 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
             if (gAi) gA = gAi[p];
             if (NRM) gN0 = gNi[p], gN1 = gNi[hw + p], gN2 = gNi[2 * hw + p];
         }
-        j = ts_job_take(f, 1, lane);       // next ticket: its round trip overlaps the pixel loads
+        const uint32_t j_next = ts_job_request(f, 1, lane);   // next ticket: read at the end of this job
         float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         ts_bwd_walk<SM, ATTR, GEOM, POSE, NRM>(f, sc, job, lane, sm, sigma, alpha_min, fx, fy, ncon, Tcur, gC0, gC1, gC2, gD, gA,
                                                grad_color, grad_opacity, tau, gN0, gN1, gN2, 0xffffffffu, grad_sigma);
@@ -71,6 +71,7 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                 f.pose_partials[6 * ((size_t)job.tile * TS_BLOCKS_PER_TILE + job.blk) + lane] = v;
             }
         }
+        j = ts_job_ticket(j_next);
     }
     ts_job_finish(f, 1, lane);
 }
@@ -112,9 +113,7 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
         ts_job_decode(f, j, lane, job);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
         if (job.range.x + lane < job.range.y) ent = f.blist[job.range.x + lane];
-        // next ticket: requested now, read (the shuffle) at the end of this job, so that nobody waits for its round trip
-        uint32_t j_next = 0;
-        if (lane == 0) j_next = atomicAdd(&f.ctrl->job_ticket[0], 1u);
+        const uint32_t j_next = ts_job_request(f, 0, lane);   // next ticket: read at the end of this job
         FwdPix o;
         // the chunk the forward walk staged last (with the whole record) is where the backward walk begins
         uint32_t staged_lo = 0xffffffffu;
@@ -156,7 +155,7 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
             }
         }
         __syncwarp();
-        j = __shfl_sync(0xffffffffu, j_next, 0);
+        j = ts_job_ticket(j_next);
     }
     ts_job_finish(f, 0, lane);
     if (loss) {

@@ -41,7 +41,7 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
         ts_job_decode(f, j, lane, job);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
         if (job.range.x + lane < job.range.y) ent = f.blist[job.range.x + lane];
-        j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
+        const uint32_t j_next = ts_job_request(f, 0, lane);   // next ticket: read at the end of this job
         FwdPix o;
         ts_fwd_walk<SM, COUNT, STATS, NRM>(f, sc, job, lane, sm, sigma, alpha_min, t_min, ent, o, n_visit, n_rect, n_hit, face_pixels,
                                            smem_n + (NRM ? (threadIdx.x & ~31) : 0));
@@ -74,6 +74,7 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                 L.gD[p] = g;
             }
         }
+        j = ts_job_ticket(j_next);
     }
     ts_job_finish(f, 0, lane);
     if (LOSS && L.loss) {

@@ -238,7 +238,7 @@ render_track_log_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min,
         ts_job_decode(f, j, lane, job);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
         if (job.range.x + lane < job.range.y) ent = f.blist[job.range.x + lane];
-        j = ts_job_take(f, 0, lane);                       // next ticket: its round trip overlaps the list fetch
+        const uint32_t j_next = ts_job_request(f, 0, lane);   // next ticket: read at the end of this job
         FwdPix o;
         uint32_t used, mylast;
         tl_fwd_walk<SM, CAP>(f, sc, job, lane, sm.log, sigma, alpha_min, t_min, ent, o, used, mylast);
@@ -284,6 +284,7 @@ render_track_log_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min,
             f.pose_partials[6 * ((size_t)job.tile * TS_BLOCKS_PER_TILE + job.blk) + lane] = v;
         }
         __syncwarp();
+        j = ts_job_ticket(j_next);
     }
     ts_job_finish(f, 0, lane);
     if (loss) {

@@ -75,6 +75,37 @@ def check_project_and_sort(o, g, M):
     assert np.array_equal(sv[:, 1], b.vals.astype(np.int64))
     assert np.array_equal(vf[sv[:, 0]], sv[:, 1])
     assert np.array_equal(g.view(ts.VIEW_TILE_RANGES).reshape(-1, 2).view(np.uint32), b.ranges)
+    check_block_lists(g, sv, b.ranges.astype(np.int64))
+
+
+def check_block_lists(g, sv, ranges):
+    """The per-block lists the render kernels walk (integer work: exact).  Every tile has eight jobs, one per 8x4
+    block; a job's list is the subsequence, in order, of its tile's sorted list whose pixel rect overlaps the block."""
+    from paper_2605_31419_b200 import ts
+    jobs = g.view(ts.VIEW_JOBS).reshape(-1, 4).view(np.uint32).astype(np.int64)
+    bl = g.view(ts.VIEW_BLOCK_LISTS).reshape(-1, 4).astype(np.int64)
+    NT = ranges.shape[0]
+    assert jobs.shape[0] == 8 * NT
+    tile, blk = jobs[:, 0] & 0x0fffffff, jobs[:, 0] >> 28
+    assert np.array_equal(np.sort(tile * 8 + blk), np.arange(8 * NT))             # every (tile, block) exactly once
+    assert np.array_equal(tile.reshape(-1, 8), np.repeat(tile[::8], 8).reshape(-1, 8))   # a tile's jobs are consecutive
+    n_tile = ranges[tile, 1] - ranges[tile, 0]
+    assert np.all(np.diff(np.floor(np.log2(np.maximum(n_tile[::8], 1)))) <= 0)          # longest lists first (by log2 bucket)
+    x0 = (sv[:, 2] & 0xffff).astype(np.int16).astype(np.int64)
+    y0 = sv[:, 2] >> 16
+    x1 = (sv[:, 3] & 0xffff).astype(np.int16).astype(np.int64)
+    y1 = sv[:, 3] >> 16
+    total = 0
+    for j in range(jobs.shape[0]):
+        tb, te = ranges[tile[j]]
+        bx, by = (jobs[j, 3] & 0xffff) + 8 * (blk[j] & 1), (jobs[j, 3] >> 16) + 4 * (blk[j] >> 1)
+        s = slice(tb, te)
+        keep = (x0[s] <= bx + 7) & (x1[s] >= bx) & (y0[s] <= by + 3) & (y1[s] >= by)
+        want = sv[s][keep]
+        got = bl[jobs[j, 1]:jobs[j, 2]]
+        assert got.shape == want.shape and np.array_equal(got, want), (j, tile[j], blk[j])
+        total += want.shape[0]
+    assert total >= sv.shape[0]                                                   # every pair is in at least one block
 
 
 @pytest.mark.parametrize("cfg", [0, 1, 2, 3, 4])
