@@ -324,6 +324,23 @@ def depth_normalise_bwd(D, A, gDn, eps=1e-6, prec="f64"):
     return gD, gA
 
 
+def unpack_rgbd(rgb_u8, depth_u16, depth_scale, prec="f64"):
+    """Sensor frame -> the targets of Eq. 8-9 (PAPER.md:74 "RGB-D frames are processed", :125-131; DESIGN.md reading
+    S33): rgb_u8 [H][W][3] interleaved 8-bit colour, depth_u16 [H][W] in 1/depth_scale metres (0 = no measurement).
+    Chat[c][y][x] = rgb[y][x][c] / 255, Dhat[y][x] = depth[y][x] / depth_scale; one correctly rounded division each
+    (plain numpy, no blocking)."""
+    dt = np.float32 if prec == "f32" else np.float64
+    rgb = np.asarray(rgb_u8)
+    dep = np.asarray(depth_u16)
+    assert rgb.dtype == np.uint8 and rgb.ndim == 3 and rgb.shape[2] == 3 and dep.dtype == np.uint16 and dep.shape == rgb.shape[:2]
+    H, W = dep.shape
+    Chat = np.empty((3, H, W), dt)
+    for c in range(3):
+        Chat[c] = rgb[:, :, c].astype(dt) / dt(255)
+    Dhat = dep.astype(dt) / dt(depth_scale)
+    return Chat, Dhat
+
+
 def left_perturb(T_cw, tau):
     T = np.ascontiguousarray(np.asarray(T_cw)[:3, :4], np.float64)
     tau = np.ascontiguousarray(tau, np.float64)
