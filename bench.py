@@ -32,6 +32,7 @@ sys.path.insert(0, ROOT)
 
 FP32_LANES_PER_SM = 128
 METRIC = "fwd+bwd render Mpix/s"
+DEPTH_SCALE = 5000.0        # depth units per metre of the 16-bit sensor frames the e2e leg uploads (TUM RGB-D's factor)
 
 
 def load_peaks():
@@ -139,6 +140,14 @@ def measure_fp32_peak(ts, ctx, torch, stream):
 def rank_seed(config, rank):
     """Replicas / weak scaling: rank r tracks its own frame of the same scene family."""
     return config + 100 * rank
+
+
+def quantise_frame(Chat, Dhat, torch):
+    """The float targets as a camera would deliver them (reading S33): pinned u8 [H, W, 3] and u16 [H, W] (held as the
+    int16 bit pattern) host tensors."""
+    rgb = (Chat.clamp(0, 1) * 255.0).round().to(torch.uint8).permute(1, 2, 0).contiguous().cpu()
+    dep = (Dhat.clamp(min=0) * DEPTH_SCALE).round().clamp(max=65535).to(torch.int32).cpu().numpy().astype(np.uint16)
+    return rgb.pin_memory(), torch.from_numpy(dep.view(np.int16)).pin_memory()
 
 
 def max_over_ranks(dist, value, device):
@@ -495,19 +504,31 @@ def bench_tracking(args, torch, ts, scenes, dist, rank, world, local):
     clocks = clk.stop()
     p_fp32_meas = measure_fp32_peak(ts, tr.ctx, torch, stream)
 
-    # e2e: same iteration through the C ABI with HOST buffers: every step the frame's target RGB-D (pinned, 16 B/pixel)
-    # and the pose go up and dL/dtau and the loss come back, all inside the timed region.  The uploads run on a copy
-    # stream into one of two device buffers while the previous step computes (what a tracking front-end does with the
-    # next camera frame); the L2 flush of the protocol is part of every step here, on the compute stream.
-    hC, hD = tr.Chat.cpu().pin_memory(), tr.Dhat.cpu().pin_memory()
+    # e2e: same iteration through the C ABI with HOST buffers: every step the frame's target RGB-D goes up in SENSOR
+    # format (8-bit interleaved colour + 16-bit depth, pinned, 5 B/pixel; reading S33) with the pose, is
+    # unpacked on the device (ts_unpack_rgbd), and dL/dtau and the loss come back, all inside the timed region.  The
+    # uploads run on a copy stream into one of two device staging buffers while the previous step computes (what a
+    # tracking front-end does with the next camera frame); the L2 flush of the protocol is part of every step here, on
+    # the compute stream.
+    h_rgb, h_dep = quantise_frame(tr.Chat, tr.Dhat, torch)
     hT = tr.T0.cpu().pin_memory()
     n_e2e = args.warmup + args.steps
-    h_out = torch.empty(n_e2e, 7).pin_memory()
-    bufs = [(tr.Chat, tr.Dhat), (torch.empty_like(tr.Chat), torch.empty_like(tr.Dhat))]
-    runs = [run]
-    tr.Chat, tr.Dhat = bufs[1]
-    runs.append(hz.capture(tr.iteration, warm=1)[0])
-    tr.Chat, tr.Dhat = bufs[0]
+    staging = [(torch.empty_like(h_rgb, device="cuda"), torch.empty_like(h_dep, device="cuda")) for _ in range(2)]
+    h_res = torch.empty(7).pin_memory()                           # dL/dtau and the loss of the last step
+
+    def e2e_body(b):
+        # everything a step enqueues on the compute stream, as ONE graph per staging buffer (the host then spends one
+        # launch per step instead of ten calls)
+        hz.flush("write")
+        tr.T.copy_(hT, non_blocking=True)
+        ts.ts_unpack_rgbd(tr.ctx, tr.W, tr.H, staging[b][0], staging[b][1], DEPTH_SCALE, tr.Chat, tr.Dhat, stream=stream)
+        tr.iteration()
+        h_res[:6].copy_(tr.tau, non_blocking=True)
+        h_res[6:].copy_(tr.loss, non_blocking=True)
+
+    for s_rgb, s_dep in staging:
+        s_rgb.copy_(h_rgb), s_dep.copy_(h_dep)
+    e2e_runs = [hz.capture(lambda b=b: e2e_body(b), warm=1)[0] for b in (0, 1)]
     stream.synchronize()
     tr.reset()
     copy_stream = torch.cuda.Stream()
@@ -516,20 +537,16 @@ def bench_tracking(args, torch, ts, scenes, dist, rank, world, local):
 
     def e2e_steps(i0, i1):
         for i in range(i0, i1):
-            bsel = i & 1
+            s_rgb, s_dep = staging[i & 1]
             with torch.cuda.stream(copy_stream):
                 if i >= 2:
                     copy_stream.wait_event(done[i - 2])           # the buffer's previous user has finished
-                bufs[bsel][0].copy_(hC, non_blocking=True)
-                bufs[bsel][1].copy_(hD, non_blocking=True)
+                s_rgb.copy_(h_rgb, non_blocking=True)
+                s_dep.copy_(h_dep, non_blocking=True)
                 copied[i].record(copy_stream)
             with torch.cuda.stream(stream):
-                hz.flush("write")
-                tr.T.copy_(hT, non_blocking=True)
                 stream.wait_event(copied[i])
-                runs[bsel]()
-                h_out[i, :6].copy_(tr.tau, non_blocking=True)
-                h_out[i, 6:].copy_(tr.loss, non_blocking=True)
+                e2e_runs[i & 1]()
                 done[i].record(stream)
 
     e2e_steps(0, args.warmup)
@@ -555,11 +572,12 @@ def bench_tracking(args, torch, ts, scenes, dist, rank, world, local):
                         "ms_per_step_read_flush": float(np.mean(ms_read)),
                         "multi_gpu": "replicas: one independent tracker per rank, no data-path collective"},
            "clocks": clocks, "gpu_launches": Tracker.launches_per_iter * args.steps,
-           "e2e": {"value": world * HW / (e2e_step * 1e-3) / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": 16 * HW + 48,
+           "e2e": {"value": world * HW / (e2e_step * 1e-3) / 1e6, "unit": "Mpix/s", "h2d_bytes_per_step": 5 * HW + 48,
                    "d2h_bytes_per_step": 28, "ms_per_step": e2e_step,
-                   "how": "K steps timed as a whole by the host clock; every step uploads its target RGB-D frame and pose from "
-                          "pinned memory (copy stream, two device buffers, overlapping the previous step's kernels), flushes L2, "
-                          "runs the iteration and reads dL/dtau + loss back"},
+                   "how": "K steps timed as a whole by the host clock; every step uploads its target RGB-D frame in sensor "
+                          "format (u8 colour + u16 depth) and the pose from pinned memory (copy stream, two device staging "
+                          "buffers, overlapping the previous step's kernels), flushes L2, unpacks the frame "
+                          "(ts_unpack_rgbd), runs the iteration and reads dL/dtau + loss back"},
            "roofline": roof, "step_roofline": step_roof,
            "fwd_Mpix_s": world * HW / (fwd_ms * 1e-3) / 1e6, "bwd_Mpix_s": world * HW / (bwd_ms * 1e-3) / 1e6,
            "fwd_bwd_split": {"fwd_ms": fwd_ms, "bwd_ms": bwd_ms,
@@ -721,22 +739,38 @@ def bench_mapping(args, torch, ts, scenes, dist, rank, world, local):
     clocks = clk.stop()
     p_fp32_meas = measure_fp32_peak(ts, mp.ctx, torch, stream)
 
-    # e2e: the step through the C ABI with HOST buffers: this rank's keyframe targets (pinned, 16 B/pixel each) and
-    # poses go up every step, the loss comes back; inside the timed region, host clock, device synchronised both sides
-    h_tg = [(c.cpu().pin_memory(), d_.cpu().pin_memory()) for c, d_ in mp.targets]
+    # e2e: the step through the C ABI with HOST buffers: this rank's keyframe targets in sensor format (pinned, u8
+    # colour + u16 depth, 5 B/pixel each; reading S33) and poses go up every step and are unpacked on the device, the
+    # loss comes back; inside the timed region, host clock, device synchronised both sides
+    h_tg = [quantise_frame(c, d_, torch) for c, d_ in mp.targets]
+    s_tg = [[(torch.empty_like(hr, device="cuda"), torch.empty_like(hd, device="cuda")) for hr, hd in h_tg] for _ in range(2)]
     h_T = [p.cpu().pin_memory() for p in mp.poses]
-    h_loss = torch.empty(args.warmup + args.steps, 1).pin_memory()
+    n_e2e = args.warmup + args.steps
+    h_loss = torch.empty(n_e2e, 1).pin_memory()
+    copy_stream = torch.cuda.Stream()
+    copied = [torch.cuda.Event() for _ in range(n_e2e)]
+    done = [torch.cuda.Event() for _ in range(n_e2e)]
 
     def e2e_steps(i0, i1):
-        with torch.cuda.stream(stream):
-            for i in range(i0, i1):
+        # the frames of step i go up on a copy stream into one of two sets of staging buffers while step i - 1 computes
+        for i in range(i0, i1):
+            with torch.cuda.stream(copy_stream):
+                if i >= 2:
+                    copy_stream.wait_event(done[i - 2])
+                for (sr, sd), (hr, hd) in zip(s_tg[i & 1], h_tg):
+                    sr.copy_(hr, non_blocking=True), sd.copy_(hd, non_blocking=True)
+                copied[i].record(copy_stream)
+            with torch.cuda.stream(stream):
                 hz.flush("write")
-                for (c, d_), (hc, hd), p, hp in zip(mp.targets, h_tg, mp.poses, h_T):
-                    c.copy_(hc, non_blocking=True), d_.copy_(hd, non_blocking=True), p.copy_(hp, non_blocking=True)
+                stream.wait_event(copied[i])
+                for (c, d_), (sr, sd), p, hp in zip(mp.targets, s_tg[i & 1], mp.poses, h_T):
+                    p.copy_(hp, non_blocking=True)
+                    ts.ts_unpack_rgbd(mp.ctx, mp.W, mp.H, sr, sd, DEPTH_SCALE, c, d_, stream=stream)
                 run()
                 if post is not None:
                     post()
                 h_loss[i].copy_(mp.loss, non_blocking=True)
+                done[i].record(stream)
 
     e2e_steps(0, args.warmup)
     torch.cuda.synchronize()
@@ -770,9 +804,11 @@ def bench_mapping(args, torch, ts, scenes, dist, rank, world, local):
                         "allreduce_bytes_per_step": 28 * mp.scene.V if world > 1 else 0},
            "clocks": clocks, "gpu_launches": mp.launches_per_step() * args.steps,
            "e2e": {"value": n_views * HW / (e2e_step * 1e-3) / 1e6, "unit": "Mpix/s",
-                   "h2d_bytes_per_step": len(my_views) * (16 * HW + 48), "d2h_bytes_per_step": 4, "ms_per_step": e2e_step,
-                   "how": "K steps timed as a whole by the host clock; every step uploads this rank's keyframe targets and "
-                          "poses from pinned memory, flushes L2, runs the step (and the all-reduce) and reads the loss back"},
+                   "h2d_bytes_per_step": len(my_views) * (5 * HW + 48), "d2h_bytes_per_step": 4, "ms_per_step": e2e_step,
+                   "how": "K steps timed as a whole by the host clock; every step uploads this rank's keyframe targets in sensor "
+                          "format (u8 colour + u16 depth; copy stream, two sets of device staging buffers, overlapping the "
+                          "previous step's kernels) and poses from pinned memory, flushes L2, unpacks the frames "
+                          "(ts_unpack_rgbd), runs the step (and the all-reduce) and reads the loss back"},
            "roofline": roof, "step_roofline": step_roof, "ms_per_view": ms_per_step / max(1, len(my_views)),
            "stage_ms": stage_ms, "counters": cnts[0], "counters_all_views_of_rank_0": cnts,
            "wall_s_timed_region": t_wall, "src_sha16": src_sha16()}

@@ -244,6 +244,15 @@ int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, flo
 int32_t ts_pose_reduce_step(ts_ctx* ctx, ts_frame* frame, float* dL_dtau_dev, float* T_cw_dev, float* state_dev,
                             const float* lr6, float beta1, float beta2, float eps, void* stream);
 
+/* Sensor frame -> the targets of a4 ("RGB-D frames are processed", Eq. 8-9 :125-131; DESIGN.md reading
+ * S33): rgb_dev u8[H][W][3] interleaved colour and depth_dev u16[H][W] in 1/depth_scale metres (0 = no measurement),
+ * both DEVICE memory (the caller uploads the 5 bytes per pixel of a camera frame instead of 16).
+ * Chat[c][y][x] = rgb[y][x][c] / 255 (f32[3][H][W]), Dhat[y][x] = depth[y][x] / depth_scale (f32[H][W]); one correctly
+ * rounded division each, bit-exact against the oracle's unpack_rgbd.  Either pair (rgb_dev, Chat) or (depth_dev, Dhat)
+ * may be NULL; depth_scale > 0.  Pointers of any alignment (4 / 8-byte aligned ones take the vector path). */
+int32_t ts_unpack_rgbd(ts_ctx* ctx, int32_t W, int32_t H, const uint8_t* rgb_dev, const uint16_t* depth_dev,
+                       float depth_scale, float* Chat, float* Dhat, void* stream);
+
 /* Measurement helper: enqueues a dependent-free FP32 FMA loop (`iters` rounds of eight
  * independent chains per thread, 2 x 1024 threads per SM) and returns in *flops_out (HOST) the flops it performs; the
  * caller times it with events on `stream` to get the measured FP32 peak.  scratch_dev: one float of device memory. */

@@ -280,3 +280,60 @@ int32_t ts_launch_ncontrib_view(const ts_ctx*, ts_frame* fr, cudaStream_t st) {
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }
+
+// Sensor frame -> targets of Eq. 8-9 (reading S33): 5 bytes read, 16 written per pixel; HBM-bound.  One thread
+// per four consecutive pixels (three 32-bit loads of colour and one 64-bit load of depth when the pointers allow it,
+// byte loads otherwise), float4 stores into the four planes.
+namespace {
+template <bool VEC>
+__global__ void __launch_bounds__(256) unpack_rgbd_kernel(size_t n, const uint8_t* __restrict__ rgb, const uint16_t* __restrict__ dep,
+                                                          float depth_scale, float* __restrict__ Chat, float* __restrict__ Dhat) {
+    const size_t n4 = (n + 3) / 4;
+    for (size_t q = blockIdx.x * (size_t)blockDim.x + threadIdx.x; q < n4; q += (size_t)gridDim.x * blockDim.x) {
+        const size_t p0 = 4 * q;
+        uint32_t c[12], d[4];
+        if (VEC && p0 + 4 <= n) {
+            if (rgb) {
+                const uint32_t* r32 = reinterpret_cast<const uint32_t*>(rgb + 3 * p0);
+                const uint32_t w0 = __ldg(r32), w1 = __ldg(r32 + 1), w2 = __ldg(r32 + 2);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) c[i] = (w0 >> (8 * i)) & 0xffu, c[4 + i] = (w1 >> (8 * i)) & 0xffu, c[8 + i] = (w2 >> (8 * i)) & 0xffu;
+            }
+            if (dep) {
+                const uint2 w = __ldg(reinterpret_cast<const uint2*>(dep + p0));
+                d[0] = w.x & 0xffffu, d[1] = w.x >> 16, d[2] = w.y & 0xffffu, d[3] = w.y >> 16;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const bool in = p0 + i < n;
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) c[3 * i + ch] = (rgb && in) ? rgb[3 * (p0 + i) + ch] : 0u;
+                d[i] = (dep && in) ? dep[p0 + i] : 0u;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+            if (p0 + i >= n) break;
+            if (rgb) {
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) Chat[ch * n + p0 + i] = __fdiv_rn((float)c[3 * i + ch], 255.0f);
+            }
+            if (dep) Dhat[p0 + i] = __fdiv_rn((float)d[i], depth_scale);
+        }
+    }
+}
+}  // namespace
+
+extern "C" int32_t ts_unpack_rgbd(ts_ctx* ctx, int32_t W, int32_t H, const uint8_t* rgb_dev, const uint16_t* depth_dev,
+                                  float depth_scale, float* Chat, float* Dhat, void* stream) {
+    if (!ctx || W <= 0 || H <= 0 || (!rgb_dev && !depth_dev) || (rgb_dev && !Chat) || (depth_dev && (!Dhat || !(depth_scale > 0.0f))))
+        return TS_ERR_INVALID_ARG;
+    const size_t n = (size_t)W * H, n4 = (n + 3) / 4;
+    const int grid = (int)((n4 + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n4 + 255) / 256 : (size_t)ctx->num_sms * 8);
+    const bool vec = (reinterpret_cast<uintptr_t>(rgb_dev) & 3u) == 0 && (reinterpret_cast<uintptr_t>(depth_dev) & 7u) == 0;
+    if (vec) unpack_rgbd_kernel<true><<<grid, 256, 0, (cudaStream_t)stream>>>(n, rgb_dev, depth_dev, depth_scale, Chat, Dhat);
+    else unpack_rgbd_kernel<false><<<grid, 256, 0, (cudaStream_t)stream>>>(n, rgb_dev, depth_dev, depth_scale, Chat, Dhat);
+    TS_CUDA_CHECK_LAUNCH();
+    return TS_OK;
+}

@@ -30,7 +30,7 @@ EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_map_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
            "ts_render_fwd_normal", "ts_render_bwd_normal", "ts_normal_loss_grad", "ts_render_bwd_stats",
            "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view",
-           "ts_fp32_probe", "ts_frame_set_face_sigma", "ts_render_fwd_normal_top", "ts_depth_normalise", "ts_depth_normalise_bwd"]
+           "ts_fp32_probe", "ts_frame_set_face_sigma", "ts_render_fwd_normal_top", "ts_depth_normalise", "ts_depth_normalise_bwd", "ts_unpack_rgbd"]
 
 
 class TsError(RuntimeError):
@@ -104,6 +104,8 @@ def _load():
                                   C.c_void_p]
     lib.ts_render_fwd_normal_top.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                              C.c_void_p, C.c_void_p, C.c_void_p]
+    lib.ts_unpack_rgbd.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p,
+                                   C.c_void_p]
     lib.ts_depth_normalise.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p, C.c_void_p]
     lib.ts_depth_normalise_bwd.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
                                            C.c_void_p, C.c_void_p, C.c_void_p]
@@ -295,6 +297,14 @@ def ts_pose_reduce_step(ctx, frame, dL_dtau, T_cw, state, lr6, beta1=0.9, beta2=
 def ts_render_fwd_normal_top(ctx, scene, frame, out_color, out_depth, out_alpha, out_normal, out_normal_top, stream=None):
     _check(lib.ts_render_fwd_normal_top(ctx.h, C.byref(scene.c), frame.h, _ptr(out_color), _ptr(out_depth), _ptr(out_alpha),
                                         _ptr(out_normal), _ptr(out_normal_top), _stream(stream)))
+
+
+def ts_unpack_rgbd(ctx, W, H, rgb, depth, depth_scale, Chat, Dhat, stream=None):
+    """rgb: uint8 [H, W, 3]; depth: uint16 (or its int16 bit pattern) [H, W]; both CUDA tensors, or None."""
+    if depth is not None and depth.dtype not in (torch.uint16, torch.int16):
+        raise TsError("depth must be a 16-bit integer tensor")
+    _check(lib.ts_unpack_rgbd(ctx.h, int(W), int(H), _ptr(rgb, torch.uint8), _ptr(depth, depth.dtype if depth is not None else None),
+                              float(depth_scale), _ptr(Chat), _ptr(Dhat), _stream(stream)))
 
 
 def ts_depth_normalise(ctx, W, H, D, A, eps, Dn, stream=None):

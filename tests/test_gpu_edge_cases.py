@@ -404,3 +404,36 @@ def test_face_area_needs_the_sort(ctx, oracle_mod):
     torch.cuda.synchronize()
     assert (area > 0).sum().item() == g.status()[1]
     g.close()
+
+
+@pytest.mark.parametrize("W,H", [(640, 480), (37, 23), (1, 1), (1203, 7)])
+def test_unpack_rgbd_is_bit_exact(ctx, oracle_mod, W, H):
+    """ts_unpack_rgbd against the oracle's unpack_rgbd (reading S33): bit-exact, ragged sizes, misaligned pointers (the
+    scalar path), either half absent."""
+    import torch
+    from paper_2605_31419_b200 import ts
+    rng = np.random.default_rng(5 + W)
+    rgb = rng.integers(0, 256, (H, W, 3), dtype=np.uint8)
+    dep = rng.integers(0, 65536, (H, W), dtype=np.uint16)
+    dep[rng.random((H, W)) < 0.1] = 0
+    for scale in (5000.0, 6553.5):
+        Cw, Dw = oracle_mod.unpack_rgbd(rgb, dep, scale, "f32")
+        for off in (0, 1):                                       # off = 1: pointers that are not 4 / 8-byte aligned
+            rbuf = torch.zeros(rgb.size + 8, dtype=torch.uint8, device="cuda")
+            dbuf = torch.zeros(dep.size + 8, dtype=torch.int16, device="cuda")
+            r = rbuf[off:off + rgb.size].view(H, W, 3)
+            d = dbuf[off:off + dep.size].view(H, W)
+            r.copy_(torch.from_numpy(rgb)), d.copy_(torch.from_numpy(dep.view(np.int16)))
+            C = torch.full((3, H, W), -1.0, device="cuda")
+            D = torch.full((H, W), -1.0, device="cuda")
+            ts.ts_unpack_rgbd(ctx, W, H, r, d, scale, C, D)
+            assert np.array_equal(C.cpu().numpy().view(np.uint32), Cw.view(np.uint32))
+            assert np.array_equal(D.cpu().numpy().view(np.uint32), Dw.view(np.uint32))
+    C.fill_(-1.0), D.fill_(-1.0)
+    ts.ts_unpack_rgbd(ctx, W, H, r, None, 1.0, C, None)
+    assert np.array_equal(C.cpu().numpy(), Cw) and float(D.min()) == -1.0
+    C.fill_(-1.0)
+    ts.ts_unpack_rgbd(ctx, W, H, None, d, 6553.5, None, D)
+    assert np.array_equal(D.cpu().numpy(), Dw) and float(C.max()) == -1.0
+    with pytest.raises(ts.TsError):
+        ts.ts_unpack_rgbd(ctx, W, H, None, None, 1.0, None, None)
