@@ -38,19 +38,33 @@ struct DssimSmem {
 
 __global__ void __launch_bounds__(256)
 dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __restrict__ Y, Gauss11 G, float wgt,
-                   float lambda, float keep, float* __restrict__ gC, float* __restrict__ loss) {
+                   float lambda, float keep, float* __restrict__ gC, float* __restrict__ loss, int vec2) {
     extern __shared__ __align__(16) unsigned char dssim_raw[];
     DssimSmem& S = *reinterpret_cast<DssimSmem*>(dssim_raw);
     const int tid = threadIdx.x, x0 = blockIdx.x * DT, y0 = blockIdx.y * DT;
     const size_t hw = (size_t)W * H;
     const float* Xc = X + blockIdx.z * hw;
     const float* Yc = Y + blockIdx.z * hw;
-    // 1. images on the tile + 10-pixel apron, zero padded
-    for (int i = tid; i < DA * DA; i += 256) {
-        const int r = i / DA, c = i - r * DA, gx = x0 + c - 2 * DR, gy = y0 + r - 2 * DR;
-        const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
-        S.a.in.sx[r][c] = in ? __ldg(Xc + (size_t)gy * W + gx) : 0.0f;
-        S.a.in.sy[r][c] = in ? __ldg(Yc + (size_t)gy * W + gx) : 0.0f;
+    // 1. images on the tile + 10-pixel apron, zero padded; two pixels per load where the row pitch allows it (the
+    //    apron starts at an even column: x0 - 10)
+    if (vec2) {                                              // (W even, images 8-byte aligned)
+        for (int i = tid; i < DA * (DA / 2); i += 256) {
+            const int r = i / (DA / 2), c = 2 * (i - r * (DA / 2)), gx = x0 + c - 2 * DR, gy = y0 + r - 2 * DR;
+            float2 vx = make_float2(0.f, 0.f), vy = make_float2(0.f, 0.f);
+            if (gx >= 0 && gx + 1 < W && gy >= 0 && gy < H) {            // (gx and W are even: both pixels in or both out)
+                vx = __ldg(reinterpret_cast<const float2*>(Xc + (size_t)gy * W + gx));
+                vy = __ldg(reinterpret_cast<const float2*>(Yc + (size_t)gy * W + gx));
+            }
+            S.a.in.sx[r][c] = vx.x, S.a.in.sx[r][c + 1] = vx.y;
+            S.a.in.sy[r][c] = vy.x, S.a.in.sy[r][c + 1] = vy.y;
+        }
+    } else {
+        for (int i = tid; i < DA * DA; i += 256) {
+            const int r = i / DA, c = i - r * DA, gx = x0 + c - 2 * DR, gy = y0 + r - 2 * DR;
+            const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
+            S.a.in.sx[r][c] = in ? __ldg(Xc + (size_t)gy * W + gx) : 0.0f;
+            S.a.in.sy[r][c] = in ? __ldg(Yc + (size_t)gy * W + gx) : 0.0f;
+        }
     }
     __syncthreads();
     // Every pass is register-blocked: a thread produces a run of 6 (or 4) consecutive outputs ALONG the convolution,
@@ -63,13 +77,17 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
         float vx[16], vy[16];
 #pragma unroll
         for (int k = 0; k < 16; ++k) vx[k] = S.a.in.sx[r][c0 + k], vy[k] = S.a.in.sy[r][c0 + k];
+        float vxx[16], vyy[16], vxy[16];                        // the products once per input, not once per tap
+#pragma unroll
+        for (int k = 0; k < 16; ++k) vxx[k] = vx[k] * vx[k], vyy[k] = vy[k] * vy[k], vxy[k] = vx[k] * vy[k];
 #pragma unroll
         for (int j = 0; j < 6; ++j) {
             float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f;
 #pragma unroll
             for (int k = 0; k < 11; ++k) {
-                const float a = vx[j + k], b = vy[j + k], g = G.g[k];
-                a0 = fmaf(g, a, a0), a1 = fmaf(g, b, a1), a2 = fmaf(g, a * a, a2), a3 = fmaf(g, b * b, a3), a4 = fmaf(g, a * b, a4);
+                const float g = G.g[k];
+                a0 = fmaf(g, vx[j + k], a0), a1 = fmaf(g, vy[j + k], a1), a2 = fmaf(g, vxx[j + k], a2), a3 = fmaf(g, vyy[j + k], a3),
+                a4 = fmaf(g, vxy[j + k], a4);
             }
             S.b.hs[0][r][c0 + j] = a0, S.b.hs[1][r][c0 + j] = a1, S.b.hs[2][r][c0 + j] = a2, S.b.hs[3][r][c0 + j] = a3,
             S.b.hs[4][r][c0 + j] = a4;
@@ -103,7 +121,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
                 const float mu1 = st[0][j], mu2 = st[1][j], e11 = st[2][j], e22 = st[3][j], e12 = st[4][j];
                 const float s11 = e11 - mu1 * mu1, s22 = e22 - mu2 * mu2, s12 = e12 - mu1 * mu2;
                 const float A1 = 2.f * mu1 * mu2 + C1, A2 = 2.f * s12 + C2, B1 = mu1 * mu1 + mu2 * mu2 + C1, B2 = s11 + s22 + C2;
-                const float iB1 = 1.0f / B1, iB2 = 1.0f / B2;
+                const float iB1 = __fdividef(1.0f, B1), iB2 = __fdividef(1.0f, B2);     // (B1 >= C1, B2 >= C2: MUFU.RCP is enough)
                 if (r >= DR && r < DR + DT && c >= DR && c < DR + DT) acc += A1 * A2 * iB1 * iB2;   // the tile's own pixels
                 const float d_mu1_direct = 2.f * mu2 * A2 * iB1 * iB2 - A1 * A2 * 2.f * mu1 * iB1 * iB1 * iB2;
                 const float d_s11 = -A1 * A2 * iB1 * iB2 * iB2;
@@ -188,8 +206,9 @@ extern "C" int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const f
     const float wgt = (float)(-(double)lambda / (3.0 * (double)W * (double)H));
     const dim3 grid((W + DT - 1) / DT, (H + DT - 1) / DT, 3);
     cudaFuncSetAttribute(dssim_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DssimSmem));   // per device
+    const int vec2 = (W & 1) == 0 && ((reinterpret_cast<uintptr_t>(C) | reinterpret_cast<uintptr_t>(Chat)) & 7u) == 0;
     dssim_fused_kernel<<<grid, 256, sizeof(DssimSmem), (cudaStream_t)stream>>>(W, H, C, Chat, G, wgt, lambda, 1.0f - lambda, gC,
-                                                                               loss_dev);
+                                                                               loss_dev, vec2);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }
