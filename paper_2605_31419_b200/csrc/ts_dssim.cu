@@ -19,6 +19,7 @@
 namespace {
 
 constexpr int DT = 32, DR = 5;
+constexpr int DN = 384;              // threads per CTA: every pass but the last fits one round of tasks (364, 294, 336, 256)
 constexpr int DB = DT + 2 * DR;      // 42: tile + apron of the M maps
 constexpr int DA = DT + 4 * DR;      // 52: tile + apron of the images
 
@@ -30,13 +31,13 @@ struct DssimSmem {
         float m[3][DB][DB + 1];                                  // M maps (steps 3-4)
     } a;
     union {
-        float hs[5][DA][DB];                                     // row sums of x, y, x^2, y^2, xy (steps 2-3)
-        float hm[3][DB][DT];                                     // row sums of the M maps (steps 4-5)
+        float hs[5][DA][DB + 1];                                 // row sums of x, y, x^2, y^2, xy (steps 2-3); odd row pitch:
+        float hm[3][DB][DT + 1];                                 // row sums of the M maps (steps 4-5)    lanes that differ in the row hit different banks
     } b;
-    float red[8];
+    float red[DN / 32];
 };
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(DN, 3)
 dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __restrict__ Y, Gauss11 G, float wgt,
                    float lambda, float keep, float* __restrict__ gC, float* __restrict__ loss, int vec2) {
     extern __shared__ __align__(16) unsigned char dssim_raw[];
@@ -48,7 +49,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
     // 1. images on the tile + 10-pixel apron, zero padded; two pixels per load where the row pitch allows it (the
     //    apron starts at an even column: x0 - 10)
     if (vec2) {                                              // (W even, images 8-byte aligned)
-        for (int i = tid; i < DA * (DA / 2); i += 256) {
+        for (int i = tid; i < DA * (DA / 2); i += DN) {
             const int r = i / (DA / 2), c = 2 * (i - r * (DA / 2)), gx = x0 + c - 2 * DR, gy = y0 + r - 2 * DR;
             float2 vx = make_float2(0.f, 0.f), vy = make_float2(0.f, 0.f);
             if (gx >= 0 && gx + 1 < W && gy >= 0 && gy < H) {            // (gx and W are even: both pixels in or both out)
@@ -59,7 +60,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
             S.a.in.sy[r][c] = vy.x, S.a.in.sy[r][c + 1] = vy.y;
         }
     } else {
-        for (int i = tid; i < DA * DA; i += 256) {
+        for (int i = tid; i < DA * DA; i += DN) {
             const int r = i / DA, c = i - r * DA, gx = x0 + c - 2 * DR, gy = y0 + r - 2 * DR;
             const bool in = gx >= 0 && gx < W && gy >= 0 && gy < H;
             S.a.in.sx[r][c] = in ? __ldg(Xc + (size_t)gy * W + gx) : 0.0f;
@@ -72,7 +73,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
     // so that the lanes of a warp differ in the OTHER coordinate (rows: stride 53 / 43 words, columns: stride 1), which
     // keeps the reads free of bank conflicts.
     // 2. horizontal pass: 52 rows x 42 columns (7 runs of 6)
-    for (int i = tid; i < DA * (DB / 6); i += 256) {
+    for (int i = tid; i < DA * (DB / 6); i += DN) {
         const int r = i % DA, c0 = (i / DA) * 6;
         float vx[16], vy[16];
 #pragma unroll
@@ -97,7 +98,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
     // 3. vertical pass + SSIM + the three maps on 42 x 42 (7 runs of 6 rows; the images in S.a are dead from here on)
     const float C1 = 0.01f * 0.01f, C2 = 0.03f * 0.03f;
     float acc = 0.0f;
-    for (int i = tid; i < DB * (DB / 6); i += 256) {
+    for (int i = tid; i < DB * (DB / 6); i += DN) {
         const int c = i % DB, r0 = (i / DB) * 6, gx = x0 + c - DR;
         float st[5][6];
 #pragma unroll
@@ -134,7 +135,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
     }
     __syncthreads();
     // 4. horizontal pass of the maps: 42 rows x 32 columns, 8 runs of 4 (S.b.hs is dead: every thread passed the barrier)
-    for (int i = tid; i < DB * (DT / 4); i += 256) {
+    for (int i = tid; i < DB * (DT / 4); i += DN) {
         const int r = i % DB, c0 = (i / DB) * 4;
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
@@ -152,7 +153,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
     }
     __syncthreads();
     // 5. vertical pass + the cotangent of E_pho on the tile (8 runs of 4 rows)
-    for (int i = tid; i < DT * (DT / 4); i += 256) {
+    for (int i = tid; i < DT * (DT / 4); i += DN) {
         const int c = i % DT, r0 = (i / DT) * 4, gx = x0 + c;
         float cc[3][4];
 #pragma unroll
@@ -183,7 +184,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
         __syncthreads();
         if (tid == 0) {
             float t = 0.f;
-            for (int w = 0; w < 8; ++w) t += S.red[w];
+            for (int w = 0; w < DN / 32; ++w) t += S.red[w];
             // lambda * L = lambda * (1 - sum / 3HW): the constant is added once, by block (0,0,0)
             float v = wgt * t;                                        // wgt = -lambda / 3HW
             if (blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) v += lambda;
@@ -207,7 +208,7 @@ extern "C" int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const f
     const dim3 grid((W + DT - 1) / DT, (H + DT - 1) / DT, 3);
     cudaFuncSetAttribute(dssim_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DssimSmem));   // per device
     const int vec2 = (W & 1) == 0 && ((reinterpret_cast<uintptr_t>(C) | reinterpret_cast<uintptr_t>(Chat)) & 7u) == 0;
-    dssim_fused_kernel<<<grid, 256, sizeof(DssimSmem), (cudaStream_t)stream>>>(W, H, C, Chat, G, wgt, lambda, 1.0f - lambda, gC,
+    dssim_fused_kernel<<<grid, DN, sizeof(DssimSmem), (cudaStream_t)stream>>>(W, H, C, Chat, G, wgt, lambda, 1.0f - lambda, gC,
                                                                                loss_dev, vec2);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
