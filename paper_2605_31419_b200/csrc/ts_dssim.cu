@@ -49,15 +49,26 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
     // 1. images on the tile + 10-pixel apron, zero padded; two pixels per load where the row pitch allows it (the
     //    apron starts at an even column: x0 - 10)
     if (vec2) {                                              // (W even, images 8-byte aligned)
-        for (int i = tid; i < DA * (DA / 2); i += DN) {
+        // all of a thread's loads are issued before its first store (one round trip, not one per iteration)
+        constexpr int N1 = (DA * (DA / 2) + DN - 1) / DN;
+        float2 vx[N1], vy[N1];
+#pragma unroll
+        for (int it = 0; it < N1; ++it) {
+            const int i = tid + it * DN;
             const int r = i / (DA / 2), c = 2 * (i - r * (DA / 2)), gx = x0 + c - 2 * DR, gy = y0 + r - 2 * DR;
-            float2 vx = make_float2(0.f, 0.f), vy = make_float2(0.f, 0.f);
-            if (gx >= 0 && gx + 1 < W && gy >= 0 && gy < H) {            // (gx and W are even: both pixels in or both out)
-                vx = __ldg(reinterpret_cast<const float2*>(Xc + (size_t)gy * W + gx));
-                vy = __ldg(reinterpret_cast<const float2*>(Yc + (size_t)gy * W + gx));
+            vx[it] = make_float2(0.f, 0.f), vy[it] = make_float2(0.f, 0.f);
+            if (i < DA * (DA / 2) && gx >= 0 && gx + 1 < W && gy >= 0 && gy < H) {   // (gx and W are even: both pixels in or both out)
+                vx[it] = __ldg(reinterpret_cast<const float2*>(Xc + (size_t)gy * W + gx));
+                vy[it] = __ldg(reinterpret_cast<const float2*>(Yc + (size_t)gy * W + gx));
             }
-            S.a.in.sx[r][c] = vx.x, S.a.in.sx[r][c + 1] = vx.y;
-            S.a.in.sy[r][c] = vy.x, S.a.in.sy[r][c + 1] = vy.y;
+        }
+#pragma unroll
+        for (int it = 0; it < N1; ++it) {
+            const int i = tid + it * DN;
+            if (i >= DA * (DA / 2)) break;
+            const int r = i / (DA / 2), c = 2 * (i - r * (DA / 2));
+            S.a.in.sx[r][c] = vx[it].x, S.a.in.sx[r][c + 1] = vx[it].y;
+            S.a.in.sy[r][c] = vy[it].x, S.a.in.sy[r][c + 1] = vy[it].y;
         }
     } else {
         for (int i = tid; i < DA * DA; i += DN) {
@@ -155,6 +166,17 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
     // 5. vertical pass + the cotangent of E_pho on the tile (8 runs of 4 rows)
     for (int i = tid; i < DT * (DT / 4); i += DN) {
         const int c = i % DT, r0 = (i / DT) * 4, gx = x0 + c;
+        // the pixel's cotangent and images are requested first: they arrive under the convolution
+        float g0[4], xv[4], yv[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int gy = y0 + r0 + j;
+            g0[j] = xv[j] = yv[j] = 0.f;
+            if (gx < W && gy < H) {
+                const size_t p = blockIdx.z * hw + (size_t)gy * W + gx;
+                g0[j] = gC[p], xv[j] = __ldg(X + p), yv[j] = __ldg(Y + p);
+            }
+        }
         float cc[3][4];
 #pragma unroll
         for (int q = 0; q < 3; ++q) {
@@ -174,7 +196,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
             const int gy = y0 + r0 + j;
             if (gx >= W || gy >= H) continue;
             const size_t p = blockIdx.z * hw + (size_t)gy * W + gx;
-            gC[p] = keep * gC[p] + cc[0][j] + 2.0f * __ldg(X + p) * cc[1][j] + __ldg(Y + p) * cc[2][j];
+            gC[p] = keep * g0[j] + cc[0][j] + 2.0f * xv[j] * cc[1][j] + yv[j] * cc[2][j];
         }
     }
     if (loss) {
