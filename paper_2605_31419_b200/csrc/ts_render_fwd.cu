@@ -1,10 +1,10 @@
 // ts_render_fwd.cu -- a3: front-to-back compositing (Eq. 2-4).
-// Persistent warps, one 8x4-pixel block of a 16x16 tile per job (ts_jobs.cuh), one pixel per lane.  The tile's
-// sorted list is read 32 entries at a time (one coalesced LDG.128 per lane: slot, face, rect); lanes whose entry
-// overlaps the block copy the pre-built face record (ts_raster.cuh; four LDG.128 + nine colour floats) into the
-// warp's private shared-memory slice, in list order; the warp then walks the staged entries, reading each record
-// with broadcast LDS.128 and testing "my pixel is in the rect" with one shift of the entry's lane mask.  Pixels
-// stop at T <= t_min, the warp when all its pixels stopped.  No CTA barrier, no atomics.
+// Persistent warps, one 8x4-pixel block of a 16x16 tile per job (ts_jobs.cuh), one pixel per lane.  The block's
+// list (built by the sort kernel) is read 32 entries at a time (one coalesced LDG.128 per lane: slot, face, rect);
+// lanes whose entry's triangle meets the block copy the pre-built face record (ts_raster.cuh; four LDG.128 + nine
+// colour floats) into the warp's private shared-memory slice, in list order; the warp then walks the staged entries,
+// reading each record with broadcast LDS.128 and testing "my pixel is in the rect" with one shift of the entry's
+// lane mask.  Pixels stop at T <= t_min, the warp when all its pixels stopped.  No CTA barrier, no atomics.
 #include "ts_fwd_job.cuh"
 #include "ts_normal.cuh"
 

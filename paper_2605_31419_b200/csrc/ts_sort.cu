@@ -2,8 +2,8 @@
 // the (tile, depth) key, shaped for P ~ 1e5..1e6 pairs where a global LSD sort is pure launch latency:
 //   bin_setup_kernel : the most-significant digit IS the tile id and its histogram already exists (tile_count,
 //       made by the project kernel).  Every CTA scans the NT counts into shared memory by itself (13 KB of L2
-//       reads: cheaper than a scan kernel or a last-CTA tail; CTA 0 also publishes tile_ranges, the frame
-//       counters and the heaviest-first tile order of the render work queues), then the MSD pass is one scatter:
+//       reads: cheaper than a scan kernel or a last-CTA tail; every CTA also publishes its slice of tile_ranges and
+//       of the heaviest-first tile order, CTA 0 the frame counters), then the MSD pass is one scatter:
 //       every visible face writes (depth_key, face, slot, rect) into the segment of each tile it touches (cursor
 //       atomics; faces that touch many tiles are spread over the warp).  The same pass builds the face's 160 B
 //       render record once (F7: unit normals, inradius, incentre, mean opacity), instead of once per (tile, face)
@@ -11,9 +11,12 @@
 //   tile_sort_kernel : one CTA per tile sorts its segment by the remaining 60 key bits (depth, then face index:
 //       exactly the stable sort of (tile << 32 | depth) with faces emitted in index order, F6) in shared memory --
 //       rank sort for short lists, a compare-exchange network above -- and writes the sorted
-//       (slot, face, rect) list the renderers walk plus the sorted 64-bit keys.  Segments longer than
-//       TS_SORT_SMEM run the same network in global memory (slow, correct, rare).  It also re-zeroes the counters.
-// Integer only; bit-exact against the oracle's std::stable_sort.
+//       (slot, face, rect) list plus the sorted 64-bit keys.  Segments longer than TS_SORT_SMEM run the same
+//       network in global memory (slow, correct, rare).  The group that sorted a tile then copies every entry into
+//       the list of each 8x4-pixel block its rect overlaps -- the PER-BLOCK lists the renderers walk -- and writes
+//       the tile's eight job headers (build_block_lists).  It also re-zeroes the counters.
+// Integer only; bit-exact against the oracle's std::stable_sort (the per-block lists: against their definition,
+// tests/test_gpu_parity.py check_block_lists).
 #include "ts_raster.cuh"
 
 namespace {
