@@ -46,7 +46,7 @@ typedef struct { float sigma, alpha_min, t_min, eps_area; uint32_t flags; } ts_p
 typedef struct { const float *pos, *color, *opacity; const int32_t *faces; int32_t V, M; } ts_scene; /* device ptrs */
 
 enum { TS_OK = 0, TS_ERR_INVALID_ARG = -1, TS_ERR_WORKSPACE = -2, TS_ERR_CAPACITY = -3, TS_ERR_CUDA = -4,
-       TS_ERR_STATE = -5 };
+       TS_ERR_STATE = -5, TS_ERR_STATIC_LIMIT = -6 /* ts_render_fwd_static: scene or image beyond TS_STATIC_MAX_* */ };
 enum { TS_GRAD_POS = 1, TS_GRAD_COLOR = 2, TS_GRAD_OPACITY = 4, TS_GRAD_POSE = 8 };
 enum { TS_FLAG_OVERFLOW_PAIRS = 1, TS_FLAG_OVERFLOW_VISIBLE = 2 };
 /* ts_params.flags */
@@ -257,6 +257,39 @@ int32_t ts_unpack_rgbd(ts_ctx* ctx, int32_t W, int32_t H, const uint8_t* rgb_dev
  * independent chains per thread, 2 x 1024 threads per SM) and returns in *flops_out (HOST) the flops it performs; the
  * caller times it with events on `stream` to get the measured FP32 peak.  scratch_dev: one float of device memory. */
 int32_t ts_fp32_probe(ts_ctx* ctx, int32_t iters, float* scratch_dev, uint64_t* flops_out, void* stream);
+
+/* ---- forward render without a caller workspace ------------------------------------------------------------ */
+
+/* Everything above needs a frame workspace that the caller allocates (ts_frame_bytes / ts_frame_bind).  A caller that
+ * may not allocate device memory while it runs -- a tracking thread that bans cudaMalloc / cudaFree after start-up because
+ * they can stall the whole device for an unbounded time, a plug-in inside a process whose device memory all belongs to the
+ * host application's arena, a preview path that must still work when HBM is full -- cannot make one.  This call is for
+ * them: ts_project + ts_bin_sort + ts_render_fwd (Eq. 1-4) on a workspace that is part of the library
+ * image, a static device array of TS_STATIC_WS_BYTES that every GPU which loads libts.so holds until the process exits.
+ *
+ * Limits (TS_ERR_STATIC_LIMIT beyond them, decided on the host before any launch): scene->M <= TS_STATIC_MAX_FACES and
+ * width * height <= TS_STATIC_MAX_PIXELS.  The (tile, face) pair capacity is whatever fits the rest of the array: at
+ * least 13 000 pairs at both maxima, more for smaller inputs.  A view with more pairs overflows like any frame: the
+ * images come out empty (zero, never out of bounds) and status_dev says so.
+ *
+ * Arguments as for ts_project (scene, cam, prm, T_cw_dev) and ts_render_fwd (out_color[3][H][W], out_depth[H][W],
+ * out_alpha[H][W]; device, any may be NULL).  status_dev: u32[3] DEVICE memory or NULL, receives (n_visible, n_pairs,
+ * flags) in stream order; flags != 0 (TS_FLAG_OVERFLOW_*) means the outputs are not a render.  All work is enqueued on
+ * `stream`; no synchronisation.  Calls no cudaMalloc / cudaFree / allocating routine (the frame handle is a few hundred
+ * bytes of host heap, freed before returning).  Forward only: the frame is gone when the call returns, ts_render_bwd has
+ * nothing to follow.
+ *
+ * Sharing: there is ONE array per GPU and every call uses all of it.  Contents left by an earlier call are harmless (each
+ * call clears what the kernels need at zero, in stream order), but two calls whose work overlaps on the GPU -- different
+ * streams without an event between them, or two threads -- race on it and both results are garbage.  Serialise them.
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress, once per device, cached); make that
+ * first call outside of any stream capture. */
+#define TS_STATIC_WS_BYTES (4u << 20)
+#define TS_STATIC_MAX_FACES 4096
+#define TS_STATIC_MAX_PIXELS 16384
+int32_t ts_render_fwd_static(ts_ctx* ctx, const ts_scene* scene, const ts_camera* cam, const ts_params* prm,
+                             const float* T_cw_dev, float* out_color, float* out_depth, float* out_alpha,
+                             uint32_t* status_dev, void* stream);
 
 /* ---- read-only debug accessors (bit-exact tests) ---------------------------------------------------------- */
 enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slot order (slots are NOT in face order):

@@ -72,6 +72,9 @@ const char* ts_strerror(int32_t s) {
         case TS_ERR_CAPACITY: return "pair / visible-face capacity exceeded";
         case TS_ERR_CUDA: return "CUDA error";
         case TS_ERR_STATE: return "call out of order for this frame";
+        case TS_ERR_STATIC_LIMIT:
+            return "too large for the built-in workspace of ts_render_fwd_static (more than TS_STATIC_MAX_FACES faces or "
+                   "TS_STATIC_MAX_PIXELS pixels): allocate a frame and use ts_project / ts_bin_sort / ts_render_fwd";
         default: return "unknown status";
     }
 }

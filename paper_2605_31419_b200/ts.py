@@ -14,7 +14,8 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libts.so")
 
-OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA, ERR_STATE = 0, -1, -2, -3, -4, -5
+OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA, ERR_STATE, ERR_STATIC_LIMIT = 0, -1, -2, -3, -4, -5, -6
+STATIC_WS_BYTES, STATIC_MAX_FACES, STATIC_MAX_PIXELS = 4 << 20, 4096, 16384   # ts_render_fwd_static (include/ts.h)
 GRAD_POS, GRAD_COLOR, GRAD_OPACITY, GRAD_POSE = 1, 2, 4, 8
 GRAD_ALL = 15
 FLAG_OVERFLOW_PAIRS, FLAG_OVERFLOW_VISIBLE = 1, 2
@@ -30,7 +31,8 @@ EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_map_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",
            "ts_render_fwd_normal", "ts_render_bwd_normal", "ts_normal_loss_grad", "ts_render_bwd_stats",
            "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view",
-           "ts_fp32_probe", "ts_frame_set_face_sigma", "ts_render_fwd_normal_top", "ts_depth_normalise", "ts_depth_normalise_bwd", "ts_unpack_rgbd"]
+           "ts_fp32_probe", "ts_frame_set_face_sigma", "ts_render_fwd_normal_top", "ts_depth_normalise", "ts_depth_normalise_bwd", "ts_unpack_rgbd",
+           "ts_render_fwd_static"]
 
 
 class TsError(RuntimeError):
@@ -111,6 +113,8 @@ def _load():
                                            C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_frame_set_face_sigma.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_fp32_probe.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.POINTER(C.c_uint64), C.c_void_p]
+    lib.ts_render_fwd_static.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.POINTER(ts_camera), C.POINTER(ts_params), C.c_void_p,
+                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_frame_release.argtypes = [C.c_void_p]
     lib.ts_destroy.argtypes = [C.c_void_p]
     lib.ts_create.argtypes = [C.c_int32, C.POINTER(C.c_void_p)]
@@ -314,6 +318,18 @@ def ts_depth_normalise(ctx, W, H, D, A, eps, Dn, stream=None):
 def ts_depth_normalise_bwd(ctx, W, H, D, A, eps, gDn, gD, gA, stream=None):
     _check(lib.ts_depth_normalise_bwd(ctx.h, int(W), int(H), _ptr(D), _ptr(A), float(eps), _ptr(gDn), _ptr(gD), _ptr(gA),
                                       _stream(stream)))
+
+
+def ts_render_fwd_static(ctx, scene, cam, prm, T_cw, out_color, out_depth, out_alpha, status=None, stream=None):
+    """Forward render of a small view with no Frame and no device allocation inside libts: for callers that must not
+    allocate while they run (a real-time tracking loop, a plug-in inside a process whose device memory belongs to the
+    host's arena, a preview when HBM is full).  The workspace is a 4 MiB static device array inside libts.so, shared by
+    every call on the device: calls that overlap on the GPU race, so keep them on one stream (or order them with
+    events).  Limits: scene.M <= STATIC_MAX_FACES, W * H <= STATIC_MAX_PIXELS (TsError "too large for the built-in
+    workspace" beyond).  status: int32 CUDA tensor of 3 (n_visible, n_pairs, flags; flags != 0 = pair overflow, the images
+    are empty) or None.  The output tensors are the caller's, as everywhere in this binding."""
+    _check(lib.ts_render_fwd_static(ctx.h, C.byref(scene.c), C.byref(cam), C.byref(prm), _ptr(T_cw), _ptr(out_color),
+                                    _ptr(out_depth), _ptr(out_alpha), _ptr(status, torch.int32), _stream(stream)))
 
 
 def ts_frame_set_face_sigma(ctx, frame, sigma, grad_sigma=None):
