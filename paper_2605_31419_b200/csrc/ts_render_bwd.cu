@@ -335,6 +335,10 @@ pose_reduce_kernel(TsFrameDev f, uint32_t n, float* __restrict__ out, float* __r
     __shared__ float sb[PR_BLOCKS][6];                                   // CTA 0's copy receives the block sums
     __shared__ float tot[6];
     cg::cluster_group cluster = cg::this_cluster();
+    // a CTA's shared memory may only be written from another CTA of the cluster once that CTA is known to have started:
+    // every thread arrives here and waits just before the remote store, after the load phase, where the barrier has long
+    // completed (it stays off the critical path)
+    cluster.barrier_arrive();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t rank = cluster.block_rank();
     const uint32_t per = (n + PR_BLOCKS - 1) / PR_BLOCKS;
@@ -360,6 +364,7 @@ pose_reduce_kernel(TsFrameDev f, uint32_t n, float* __restrict__ out, float* __r
         if (lane == 0) sm[warp][j] = a[j];
     }
     __syncthreads();
+    cluster.barrier_wait();                                               // all CTAs of the cluster are running
     if (tid < 6) {
         float s = 0.f;
 #pragma unroll
