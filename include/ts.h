@@ -300,7 +300,9 @@ enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slo
        TS_VIEW_TILE_RANGES = 3,  /* u32[NT][2]                                                               */
        TS_VIEW_N_CONTRIB = 4,    /* u32[H][W]: 1 + position in the TILE's sorted list of the pixel's last contributing
                                     entry (0 = none); converted on demand from the renderers' per-block counts by a
-                                    small launch on `stream`; needs ts_bin_sort (TS_ERR_STATE otherwise)           */
+                                    small launch on `stream`; needs a forward render (ts_render_fwd[_l1/_stats/_normal...])
+                                    since the last ts_bin_sort, TS_ERR_STATE otherwise: the fused ts_render_track_l1 /
+                                    ts_render_map_l1 do not write the counts                                           */
        TS_VIEW_COUNTERS = 5,     /* u64[8]: n_visit(warp-level), n_rect, n_hit, ... (TS_PARAM_COUNTERS only)  */
        TS_VIEW_JOBS = 6,         /* u32[8 NT][4] job headers of the render kernels, in ticket order: (tile | block << 28,
                                     begin, end, x0 | y0 << 16); block b = 2 row + column of the tile's 2 x 4 blocks of

@@ -53,13 +53,6 @@ bool make_layout(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64_t pa
     return true;
 }
 
-// every launching export runs on the device of its context (ts_create): a mismatch with the current device is an
-// argument error, not a launch on the wrong GPU
-bool on_ctx_device(const ts_ctx* ctx) {
-    int cur = -1;
-    return ctx && cudaGetDevice(&cur) == cudaSuccess && cur == ctx->device;
-}
-
 }  // namespace
 
 extern "C" {
@@ -399,7 +392,10 @@ int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev
         case TS_VIEW_TILE_RANGES: *dev_ptr = d.tile_ranges, *count = 2 * (size_t)d.NT; break;
         case TS_VIEW_N_CONTRIB: {
             // (the renderers keep block-list positions: converted to positions in the tile's list on demand)
-            if (!fr->have_sort) return TS_ERR_STATE;
+            // only a forward render on the CURRENT sort leaves counts that index its block lists: after ts_bin_sort alone,
+            // or after the fused ts_render_track_l1 / ts_render_map_l1 (which do not write them), the counts are those of
+            // an older sort
+            if (!fr->have_sort || !fr->have_fwd) return TS_ERR_STATE;
             if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
             if (ts_launch_ncontrib_view(ctx, fr, (cudaStream_t)stream) != TS_OK ||
                 cudaStreamSynchronize((cudaStream_t)stream) != cudaSuccess)

@@ -222,6 +222,7 @@ extern "C" int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const f
     (void)scratch;                                           // (the two-pass form of round 1 needed 9 HW floats here)
     if (!ctx || W <= 0 || H <= 0 || !C || !Chat || !gC || !(lambda >= 0.0f) || !(lambda <= 1.0f))
         return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     Gauss11 G;
     double g[11], sum = 0.0;
     for (int i = 0; i < 11; ++i) sum += (g[i] = exp(-(double)((i - 5) * (i - 5)) / (2.0 * 1.5 * 1.5)));

@@ -140,6 +140,7 @@ normal_loss_grad_kernel(size_t n, const float* __restrict__ N, const float* __re
 extern "C" int32_t ts_normal_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* N, const float* Nbar, float weight,
                                        float* gN, float* loss_dev, void* stream) {
     if (!ctx || W <= 0 || H <= 0 || !N || !Nbar || !gN) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H;
     const int grid = (int)((n + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n + 255) / 256 : (size_t)ctx->num_sms * 8);
     normal_loss_grad_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(n, N, Nbar, (float)((double)weight / (double)n), gN, loss_dev);
@@ -150,6 +151,7 @@ extern "C" int32_t ts_normal_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const 
 extern "C" int32_t ts_equi_loss_grad(ts_ctx* ctx, const ts_scene* sc, float weight, float* grad_pos, float* loss_dev,
                                      void* stream) {
     if (!ctx || !sc || !sc->pos || sc->M <= 0 || (!grad_pos && !loss_dev)) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->faces == nullptr && sc->V != 3 * sc->M) return TS_ERR_INVALID_ARG;
     const float scale = (float)((double)weight / (3.0 * (double)sc->M));
     const int grid = (int)(((size_t)sc->M + 255) / 256 < (size_t)ctx->num_sms * 8 ? ((size_t)sc->M + 255) / 256 : (size_t)ctx->num_sms * 8);
@@ -165,6 +167,7 @@ extern "C" int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const floa
                                    const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
                                    void* stream) {
     if (!ctx || W <= 0 || H <= 0 || !C || !D || !Chat || !Dhat || !gC || !gD) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H;
     const float wc = (float)(1.0 / (3.0 * (double)n)), wd = (float)((double)lambda_dep / (double)n);
     const int grid = (int)((n + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n + 255) / 256 : (size_t)ctx->num_sms * 8);
@@ -176,6 +179,7 @@ extern "C" int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const floa
 extern "C" int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev,
                                 const float* lr6, float beta1, float beta2, float eps, void* stream) {
     if (!ctx || !T_cw_dev || !dL_dtau_dev || !state_dev || !lr6) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     TsLr6 lr;
     for (int i = 0; i < 6; ++i) lr.v[i] = lr6[i];
     pose_step_kernel<<<1, 32, 0, (cudaStream_t)stream>>>(T_cw_dev, dL_dtau_dev, state_dev, lr, beta1, beta2, eps);
@@ -209,6 +213,7 @@ __global__ void __launch_bounds__(256) depth_normalise_bwd_kernel(size_t n, cons
 extern "C" int32_t ts_depth_normalise(ts_ctx* ctx, int32_t W, int32_t H, const float* D, const float* A, float eps, float* Dn,
                                       void* stream) {
     if (!ctx || W <= 0 || H <= 0 || !D || !A || !Dn || !(eps >= 0.0f)) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H;
     const int grid = (int)((n + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n + 255) / 256 : (size_t)ctx->num_sms * 8);
     depth_normalise_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(n, D, A, eps, Dn);
@@ -219,6 +224,7 @@ extern "C" int32_t ts_depth_normalise(ts_ctx* ctx, int32_t W, int32_t H, const f
 extern "C" int32_t ts_depth_normalise_bwd(ts_ctx* ctx, int32_t W, int32_t H, const float* D, const float* A, float eps,
                                           const float* gDn, float* gD, float* gA, void* stream) {
     if (!ctx || W <= 0 || H <= 0 || !D || !A || !gDn || !gD || !gA || !(eps >= 0.0f)) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H;
     const int grid = (int)((n + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n + 255) / 256 : (size_t)ctx->num_sms * 8);
     depth_normalise_bwd_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(n, D, A, eps, gDn, gD, gA);
@@ -243,6 +249,7 @@ __global__ void __launch_bounds__(1024) fp32_probe_kernel(int iters, float a, fl
 
 extern "C" int32_t ts_fp32_probe(ts_ctx* ctx, int32_t iters, float* scratch_dev, uint64_t* flops_out, void* stream) {
     if (!ctx || iters <= 0 || !scratch_dev || !flops_out) return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const int grid = ctx->num_sms * 2;
     fp32_probe_kernel<<<grid, 1024, 0, (cudaStream_t)stream>>>(iters, 0.999f, 1e-3f, scratch_dev);
     *flops_out = (uint64_t)grid * 1024ull * 16ull * (uint64_t)iters;
@@ -263,7 +270,7 @@ __global__ void __launch_bounds__(256) ncontrib_view_kernel(TsFrameDev f) {
     const size_t p = (size_t)py * f.W + px;
     const uint32_t nb = h.z > h.y ? f.n_contrib[p] : 0u;
     uint32_t pos = 0;
-    if (nb) {
+    if (nb && nb <= h.z - h.y) {                     // (a count beyond the job's list cannot come from this sort: reads as "none")
         // (a debug accessor: a linear search of the tile's list for the entry's slot, which is unique in it)
         const uint32_t slot = f.blist[h.y + nb - 1u].x;
         const uint2 tr = f.tile_ranges[h.x & 0x0fffffffu];
@@ -329,6 +336,7 @@ extern "C" int32_t ts_unpack_rgbd(ts_ctx* ctx, int32_t W, int32_t H, const uint8
                                   float depth_scale, float* Chat, float* Dhat, void* stream) {
     if (!ctx || W <= 0 || H <= 0 || (!rgb_dev && !depth_dev) || (rgb_dev && !Chat) || (depth_dev && (!Dhat || !(depth_scale > 0.0f))))
         return TS_ERR_INVALID_ARG;
+    if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H, n4 = (n + 3) / 4;
     const int grid = (int)((n4 + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n4 + 255) / 256 : (size_t)ctx->num_sms * 8);
     const bool vec = (reinterpret_cast<uintptr_t>(rgb_dev) & 3u) == 0 && (reinterpret_cast<uintptr_t>(depth_dev) & 7u) == 0;

@@ -95,6 +95,13 @@ struct ts_frame {
     void* base;
 };
 
+// every launching export runs on the device of its context (ts_create): a mismatch with the current device is an
+// argument error, not a launch on the wrong GPU
+inline bool on_ctx_device(const ts_ctx* ctx) {
+    int cur = -1;
+    return ctx && cudaGetDevice(&cur) == cudaSuccess && cur == ctx->device;
+}
+
 #define TS_CUDA_CHECK_LAUNCH()                              \
     do {                                                    \
         cudaError_t e__ = cudaGetLastError();               \

@@ -73,6 +73,35 @@ def test_ragged_face_counts(ctx, oracle_mod, M):
     g.close()
 
 
+def test_n_contrib_view_needs_a_forward_render_on_the_current_sort(ctx):
+    """The per-pixel counts index the block lists of the sort they were written under: after a new ts_bin_sort, or
+    after the fused tracking launch (which does not write them), the view is refused instead of walking the new lists
+    with old counts."""
+    from gpu_util import GpuView, dev
+    from paper_2605_31419_b200 import ts
+    sc = scenes.config0()
+    g = GpuView(ctx, sc.pos, sc.color, sc.opacity, None, sc.T_gt[0], sc.cam, sc.params)
+    g.sort()
+    with pytest.raises(ts.TsError, match="out of order"):
+        g.view(ts.VIEW_N_CONTRIB)
+    g.forward()
+    nc = g.view(ts.VIEW_N_CONTRIB)
+    assert nc.max() > 0
+    # the same frame projected from another pose and sorted again: the counts on the device are now stale
+    g.T = dev(np.asarray(sc.T_start[0], np.float32)[:3, :4].reshape(-1))
+    g.project().sort()
+    with pytest.raises(ts.TsError, match="out of order"):
+        g.view(ts.VIEW_N_CONTRIB)
+    H, W = sc.cam.height, sc.cam.width
+    ts.ts_render_track_l1(ctx, g.scene, g.frame, None, None, None, torch.zeros(3, H, W, device="cuda"),
+                          torch.zeros(H, W, device="cuda"), sc.params.lambda_dep)
+    with pytest.raises(ts.TsError, match="out of order"):
+        g.view(ts.VIEW_N_CONTRIB)
+    g.forward()
+    assert g.view(ts.VIEW_N_CONTRIB).shape == nc.shape
+    g.close()
+
+
 def test_capacity_overflow_is_reported_not_fatal(ctx, oracle_mod):
     from gpu_util import GpuView
     from paper_2605_31419_b200 import ts
@@ -387,6 +416,46 @@ def test_two_contexts_in_one_process(oracle_mod):
             g.project()
         g.close()
     ca.close(), cb.close()
+
+
+def test_helper_exports_refuse_a_context_of_another_device():
+    """include/ts.h: every export that launches work returns TS_ERR_INVALID_ARG unless the context's device is current.
+    The box has one GPU, so the mismatch is produced from the other side: a context whose recorded device ordinal (the
+    first field of the opaque handle) is changed to one that is not current.  Nothing may be launched: outputs stay."""
+    import ctypes
+    from paper_2605_31419_b200 import ts
+    c = ts.Context(0)
+    dev_field = ctypes.c_int.from_address(c.h.value)
+    assert dev_field.value == 0
+    dev_field.value = 5
+    W, H = 40, 24
+    z = lambda *s: torch.zeros(*s, device="cuda")
+    out3, out1, loss = torch.full((3, H, W), 9.0, device="cuda"), torch.full((H, W), 9.0, device="cuda"), z(1)
+    scene = ts.Scene(torch.rand(12, 3, device="cuda"), z(12, 3), z(12))
+    calls = [
+        lambda: ts.ts_l1_loss_grad(c, W, H, z(3, H, W), z(H, W), z(3, H, W), z(H, W), 0.05, out3, out1, loss),
+        lambda: ts.ts_dssim_loss_grad(c, W, H, z(3, H, W), z(3, H, W), 0.2, out3, loss),
+        lambda: ts.ts_normal_loss_grad(c, W, H, z(3, H, W), z(3, H, W), 0.05, out3, loss),
+        lambda: ts.ts_equi_loss_grad(c, scene, 1.0, None, loss),
+        lambda: ts.ts_pose_step(c, z(12), z(6), z(13), [1e-3] * 6),
+        lambda: ts.ts_depth_normalise(c, W, H, z(H, W), z(H, W), 1e-6, out1),
+        lambda: ts.ts_depth_normalise_bwd(c, W, H, z(H, W), z(H, W), 1e-6, z(H, W), out1, out1),
+        lambda: ts.ts_unpack_rgbd(c, W, H, torch.zeros(H, W, 3, dtype=torch.uint8, device="cuda"), None, 1000.0, out3, None),
+        lambda: ts.ts_fp32_probe(c, 4, z(1)),
+    ]
+    try:
+        for i, call in enumerate(calls):
+            with pytest.raises(ts.TsError, match="invalid argument"):
+                call()
+        torch.cuda.synchronize()
+        assert bool((out3 == 9.0).all()) and bool((out1 == 9.0).all()) and float(loss) == 0.0
+        dev_field.value = 0
+        for call in calls:                                   # the same calls go through on the right device
+            call()
+        torch.cuda.synchronize()
+    finally:
+        dev_field.value = 0
+        c.close()
 
 
 def test_face_area_needs_the_sort(ctx, oracle_mod):
