@@ -1,7 +1,6 @@
 // ts_api.cu -- the C-ABI boundary (include/ts.h): context, frame workspace carving, status / debug views and
 // host-side argument validation for the five hot-path calls.  No device memory is allocated here: the frame lives
 // entirely inside caller-provided memory.
-#include <cstdlib>
 #include <new>
 
 #include "ts_internal.cuh"
@@ -81,8 +80,6 @@ int32_t ts_create(int32_t device, ts_ctx** out) {
     ts_ctx* c = new (std::nothrow) ts_ctx;
     if (!c) return TS_ERR_CUDA;
     c->device = device, c->num_sms = p.multiProcessorCount, c->max_smem_optin = (int)p.sharedMemPerBlockOptin;
-    const char* tl = getenv("TS_TRACK_LOG");
-    c->track_log = (tl && tl[0] == '1') ? 1 : 0;
     *out = c;
     return TS_OK;
 }
@@ -308,10 +305,6 @@ int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float*
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;
     fr->have_fwd = 0;                                       // n_contrib / T_last are not written: no ts_render_bwd after this
-    // (the hit-log variant evaluates its geometry phase with the launch's sigma: per-face sigma takes the visit form)
-    if (fr->face_sigma)
-        return ts_launch_render_track_v1(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev,
-                                         (cudaStream_t)stream);
     return ts_launch_render_track(ctx, fr, sc, out_color, out_depth, out_alpha, Chat, Dhat, lambda_dep, gC, gD, loss_dev,
                                   (cudaStream_t)stream);
 }

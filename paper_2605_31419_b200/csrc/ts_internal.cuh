@@ -77,7 +77,6 @@ struct ts_ctx {
     int device;
     int num_sms;
     int max_smem_optin;
-    int track_log;           // TS_TRACK_LOG=1 in the environment at ts_create: ts_render_track_l1 runs the hit-log kernel
 };
 struct ts_frame {
     TsFrameDev d;
@@ -167,8 +166,6 @@ int32_t ts_launch_render_bwd(const ts_ctx*, ts_frame*, const ts_scene*, const fl
                              uint32_t* face_views = nullptr);
 int32_t ts_launch_render_track(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
                                const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, cudaStream_t);
-int32_t ts_launch_render_track_v1(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
-                                  const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, cudaStream_t);
 int32_t ts_launch_render_map(const ts_ctx*, ts_frame*, const ts_scene*, float* oc, float* od, float* oa, const float* Chat,
                              const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss, float* grad_pos,
                              float* grad_color, float* grad_opacity, uint32_t mask, cudaStream_t);

@@ -496,9 +496,9 @@ int32_t ts_launch_render_bwd_normal(const ts_ctx* ctx, ts_frame* fr, const ts_sc
     return TS_OK;
 }
 
-int32_t ts_launch_render_track_v1(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
-                                  const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss,
-                                  cudaStream_t st) {
+int32_t ts_launch_render_track(const ts_ctx* ctx, ts_frame* fr, const ts_scene* sc, float* oc, float* od, float* oa,
+                               const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss,
+                               cudaStream_t st) {
     const double n = (double)fr->d.W * (double)fr->d.H;
     const float wc = (float)(1.0 / (3.0 * n)), wd = (float)((double)lambda_dep / n);
     switch (ts_frame_sigma_mode(fr)) {

@@ -17,21 +17,6 @@ def ctx():
     c.close()
 
 
-@pytest.fixture(scope="module")
-def ctx_log():
-    """A second context on the same device whose ts_render_track_l1 runs the hit-log kernel (TS_TRACK_LOG is read by
-    ts_create)."""
-    import os
-    from paper_2605_31419_b200 import ts
-    os.environ["TS_TRACK_LOG"] = "1"
-    try:
-        c = ts.Context(0)
-    finally:
-        del os.environ["TS_TRACK_LOG"]
-    yield c
-    c.close()
-
-
 def test_empty_scene_all_culled(ctx, oracle_mod):
     """Every face behind the camera: nothing visible, zero pairs, zero images, zero gradients."""
     from gpu_util import GpuView
@@ -207,7 +192,7 @@ def test_determinism(ctx, oracle_mod):
 
 
 @pytest.mark.parametrize("cfg", [1, 2, 3, 4])
-def test_full_size_configs(ctx, ctx_log, oracle_mod, cfg):
+def test_full_size_configs(ctx, oracle_mod, cfg):
     """BASELINE.json sizes (100k / 500k faces tracking frames; one view of the 1M-face mapping step; 2M faces stress)
     through the tiled oracle, in the launch configuration bench.py times."""
     from test_gpu_parity import both, check_backward, check_forward, check_project_and_sort
@@ -232,7 +217,7 @@ def test_full_size_configs(ctx, ctx_log, oracle_mod, cfg):
     gC2, gD2, L2 = torch.empty_like(g.C), torch.empty_like(g.D), torch.zeros(1, device="cuda")
     tau = torch.zeros(6, device="cuda")
     if cfg in (1, 2):
-        for cx in (ctx, ctx_log):
+        for cx in (ctx,):
             ts.ts_render_track_l1(cx, g.scene, g.frame, C2, D2, A2, Chat, Dhat, lam, gC2, gD2, L2)
             ts.ts_pose_jacobian_reduce(cx, g.frame, tau)
             torch.cuda.synchronize()
