@@ -290,11 +290,12 @@ int32_t ts_launch_ncontrib_view(const ts_ctx*, ts_frame* fr, cudaStream_t st) {
 
 // Sensor frame -> targets of Eq. 8-9 (reading S33): 5 bytes read, 16 written per pixel; HBM-bound.  One thread
 // per four consecutive pixels (three 32-bit loads of colour and one 64-bit load of depth when the pointers allow it,
-// byte loads otherwise), float4 stores into the four planes.
+// byte loads otherwise); the four results of a plane go out as one float4 store when the planes are 16-byte aligned
+// and the pixel count is a multiple of four (ST4), as scalar stores otherwise.
 namespace {
 template <bool VEC>
 __global__ void __launch_bounds__(256) unpack_rgbd_kernel(size_t n, const uint8_t* __restrict__ rgb, const uint16_t* __restrict__ dep,
-                                                          float depth_scale, float* __restrict__ Chat, float* __restrict__ Dhat) {
+                                                          float depth_scale, float* __restrict__ Chat, float* __restrict__ Dhat, bool ST4) {
     const size_t n4 = (n + 3) / 4;
     for (size_t q = blockIdx.x * (size_t)blockDim.x + threadIdx.x; q < n4; q += (size_t)gridDim.x * blockDim.x) {
         const size_t p0 = 4 * q;
@@ -319,6 +320,19 @@ __global__ void __launch_bounds__(256) unpack_rgbd_kernel(size_t n, const uint8_
                 d[i] = (dep && in) ? dep[p0 + i] : 0u;
             }
         }
+        if (ST4) {                                           // (n % 4 == 0: every thread owns four whole pixels)
+            if (rgb) {
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch)
+                    *reinterpret_cast<float4*>(Chat + ch * n + p0) =
+                        make_float4(__fdiv_rn((float)c[ch], 255.0f), __fdiv_rn((float)c[3 + ch], 255.0f),
+                                    __fdiv_rn((float)c[6 + ch], 255.0f), __fdiv_rn((float)c[9 + ch], 255.0f));
+            }
+            if (dep)
+                *reinterpret_cast<float4*>(Dhat + p0) = make_float4(__fdiv_rn((float)d[0], depth_scale), __fdiv_rn((float)d[1], depth_scale),
+                                                                    __fdiv_rn((float)d[2], depth_scale), __fdiv_rn((float)d[3], depth_scale));
+            continue;
+        }
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
             if (p0 + i >= n) break;
@@ -340,8 +354,9 @@ extern "C" int32_t ts_unpack_rgbd(ts_ctx* ctx, int32_t W, int32_t H, const uint8
     const size_t n = (size_t)W * H, n4 = (n + 3) / 4;
     const int grid = (int)((n4 + 255) / 256 < (size_t)ctx->num_sms * 8 ? (n4 + 255) / 256 : (size_t)ctx->num_sms * 8);
     const bool vec = (reinterpret_cast<uintptr_t>(rgb_dev) & 3u) == 0 && (reinterpret_cast<uintptr_t>(depth_dev) & 7u) == 0;
-    if (vec) unpack_rgbd_kernel<true><<<grid, 256, 0, (cudaStream_t)stream>>>(n, rgb_dev, depth_dev, depth_scale, Chat, Dhat);
-    else unpack_rgbd_kernel<false><<<grid, 256, 0, (cudaStream_t)stream>>>(n, rgb_dev, depth_dev, depth_scale, Chat, Dhat);
+    const bool st4 = (n & 3u) == 0 && (reinterpret_cast<uintptr_t>(Chat) & 15u) == 0 && (reinterpret_cast<uintptr_t>(Dhat) & 15u) == 0;
+    if (vec) unpack_rgbd_kernel<true><<<grid, 256, 0, (cudaStream_t)stream>>>(n, rgb_dev, depth_dev, depth_scale, Chat, Dhat, st4);
+    else unpack_rgbd_kernel<false><<<grid, 256, 0, (cudaStream_t)stream>>>(n, rgb_dev, depth_dev, depth_scale, Chat, Dhat, st4);
     TS_CUDA_CHECK_LAUNCH();
     return TS_OK;
 }
