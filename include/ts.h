@@ -144,11 +144,10 @@ int32_t ts_equi_loss_grad(ts_ctx* ctx, const ts_scene* scene, float weight, floa
  * L_DSSIM = 1 - mean SSIM(C, Chat) over 3 x H x W, 11x11 Gaussian window (sigma 1.5), zero padding, C1 = 0.01^2,
  * C2 = 0.03^2.  On entry gC[3][H][W] holds the cotangent of the L1 term (ts_l1_loss_grad); on exit
  * gC = (1 - lambda) gC + lambda dL_DSSIM/dC, i.e. the cotangent of E_pho.  If loss_dev != NULL, lambda * L_DSSIM is
- * added to *loss_dev.  One launch; both separable passes run in shared memory on a tile + apron, so `scratch` is not
- * used any more (pass NULL; the argument stays for ABI compatibility with round 1).  In a tracking iteration it sits
- * between ts_render_fwd_l1 (which writes C and the L1 cotangents) and ts_render_bwd. */
+ * added to *loss_dev.  One launch; both separable passes run in shared memory on a tile + apron (no scratch image).  In a
+ * tracking iteration it sits between ts_render_fwd_l1 (which writes C and the L1 cotangents) and ts_render_bwd. */
 int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* Chat, float lambda, float* gC,
-                           float* loss_dev, float* scratch, void* stream);
+                           float* loss_dev, void* stream);
 /* a3 + a4 in one launch: ts_render_fwd, with the L1 colour + depth loss of ts_l1_loss_grad evaluated on every pixel
  * while its value is still in registers: writes gC, gD (and adds L to *loss_dev if not NULL) exactly as
  * ts_l1_loss_grad would.  out_color / out_depth / out_alpha may be NULL (a tracking loop never reads them). */
@@ -253,7 +252,7 @@ int32_t ts_pose_reduce_step(ts_ctx* ctx, ts_frame* frame, float* dL_dtau_dev, fl
 int32_t ts_unpack_rgbd(ts_ctx* ctx, int32_t W, int32_t H, const uint8_t* rgb_dev, const uint16_t* depth_dev,
                        float depth_scale, float* Chat, float* Dhat, void* stream);
 
-/* Measurement helper: enqueues a dependent-free FP32 FMA loop (`iters` rounds of eight
+/* NOT part of the rasteriser's API: a measurement helper for bench.py; it enqueues a dependent-free FP32 FMA loop (`iters` rounds of eight
  * independent chains per thread, 2 x 1024 threads per SM) and returns in *flops_out (HOST) the flops it performs; the
  * caller times it with events on `stream` to get the measured FP32 peak.  scratch_dev: one float of device memory. */
 int32_t ts_fp32_probe(ts_ctx* ctx, int32_t iters, float* scratch_dev, uint64_t* flops_out, void* stream);

@@ -94,7 +94,7 @@ def _load():
     lib.ts_l1_loss_grad.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_dssim_loss_grad.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_void_p,
-                                       C.c_void_p, C.c_void_p, C.c_void_p]
+                                       C.c_void_p, C.c_void_p]
     lib.ts_equi_loss_grad.argtypes = [C.c_void_p, C.POINTER(ts_scene), C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_pose_step.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_float), C.c_float,
                                  C.c_float, C.c_float, C.c_void_p]
@@ -278,9 +278,9 @@ def ts_l1_loss_grad(ctx, W, H, Cimg, Dimg, Chat, Dhat, lambda_dep, gC, gD, loss=
                                float(lambda_dep), _ptr(gC), _ptr(gD), _ptr(loss), _stream(stream)))
 
 
-def ts_dssim_loss_grad(ctx, W, H, Cimg, Chat, lam, gC, loss=None, scratch=None, stream=None):
+def ts_dssim_loss_grad(ctx, W, H, Cimg, Chat, lam, gC, loss=None, stream=None):
     _check(lib.ts_dssim_loss_grad(ctx.h, int(W), int(H), _ptr(Cimg), _ptr(Chat), float(lam), _ptr(gC), _ptr(loss),
-                                  _ptr(scratch), _stream(stream)))
+                                  _stream(stream)))
 
 
 def ts_equi_loss_grad(ctx, scene, weight, grad_pos, loss=None, stream=None):
