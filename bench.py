@@ -109,16 +109,23 @@ def src_sha16():
     return h.hexdigest()[:16]
 
 
-def load_traffic(kernel):
+TRAFFIC_FILE = "r03_traffic.json"
+
+
+def load_traffic(config, kernel):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of a stage's kernels from the committed ncu --set full
-    capture (profiles/r02_traffic.json); null when the sources changed since that capture."""
-    p = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    capture (profiles/r03_traffic.json, keyed by BASELINE config, then kernel): null when that (config, kernel) pair was
+    not captured or the sources changed since the capture."""
+    p = os.path.join(ROOT, "profiles", TRAFFIC_FILE)
     if not os.path.exists(p):
         return None, "no capture"
     d = json.load(open(p))
     if d.get("src_sha16") != src_sha16():
         return None, f"stale: captured at sources {d.get('src_sha16')}, now {src_sha16()}"
-    return d.get("kernels", {}).get(kernel), f"ncu --set full, sources {d.get('src_sha16')}"
+    v = d.get("configs", {}).get(str(config), {}).get(kernel)
+    if v is None:
+        return None, f"not captured at config {config}"
+    return v, f"ncu --set full at config {config}, sources {d.get('src_sha16')}"
 
 
 def measure_fp32_peak(ts, ctx, torch, stream):
@@ -401,7 +408,7 @@ class Harness:
         return {k_: float(np.median([a.elapsed_time(b) for a, b in v])) for k_, v in acc.items()}
 
 
-def roofline_objects(stage_ms, in_step, B, F, peaks, p_fp32, p_fp32_measured, ms_per_step, n_views_total=1):
+def roofline_objects(stage_ms, in_step, B, F, peaks, p_fp32, p_fp32_measured, ms_per_step, n_views_total=1, config=2):
     """`roofline` (dominant kernel of the step, by stage time) and `step_roofline` (whole step)."""
     bw = peaks["hbm_gbs"] * 1e9
     sB = lambda st: sum(B[r] for r in STAGE_ROWS[st])
@@ -416,7 +423,7 @@ def roofline_objects(stage_ms, in_step, B, F, peaks, p_fp32, p_fp32_measured, ms
         roof = {"bound": "hbm", "kernel": dom, "achieved": sB(dom) / dom_t / 1e9, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                 "peak_source": peaks["src"]}
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"], roof["traffic_source"] = load_traffic(dom)
+    roof["traffic"], roof["traffic_source"] = load_traffic(config, dom)
     roof["algorithmic_bytes"], roof["algorithmic_flops"], roof["launch_ms"] = sB(dom), sF(dom), stage_ms[dom]
     rows = [r for st in in_step for r in STAGE_ROWS[st]]
     Bt, Ft = n_views_total * sum(B[r] for r in rows), n_views_total * sum(F[r] for r in rows)
@@ -561,7 +568,7 @@ def bench_tracking(args, torch, ts, scenes, dist, rank, world, local):
     B, F = algorithmic_work(cnt, HW, NT, M, p_sort, "pose")
     p_fp32 = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12        # TFLOP/s, nominal
     in_step = ("project", "bin_sort", "render_track", "pose_reduce")               # the launches of the timed iteration
-    roof, step_roof = roofline_objects(stage_ms, in_step, B, F, peaks, p_fp32, p_fp32_meas, ms_per_step)
+    roof, step_roof = roofline_objects(stage_ms, in_step, B, F, peaks, p_fp32, p_fp32_meas, ms_per_step, config=args.config)
     fwd_ms = stage_ms["project"] + stage_ms["bin_sort"] + stage_ms["render_fwd"]
     bwd_ms = stage_ms["render_bwd"] + stage_ms["pose_reduce"]
     out = {"metric": METRIC, "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps,
@@ -691,7 +698,8 @@ class Mapper:
                 ("render_map", lambda: ts.ts_render_map_l1(self.ctx, self.scene, self.frame, self.C, self.D, self.A, Chat, Dhat,
                                                            self.sc.params.lambda_dep, self.gC, self.gD, self.loss,
                                                            self.bucket.grad_pos, self.bucket.grad_color,
-                                                           self.bucket.grad_opacity, self.mask))]
+                                                           self.bucket.grad_opacity, self.mask))] + (
+            [("pose_reduce", lambda: ts.ts_pose_jacobian_reduce(self.ctx, self.frame, self.tau))] if self.want_pose else [])
 
 
 def bench_mapping(args, torch, ts, scenes, dist, rank, world, local):
@@ -784,8 +792,6 @@ def bench_mapping(args, torch, ts, scenes, dist, rank, world, local):
     B, F = algorithmic_work(cnts[0], HW, NT, M, p_sort, "full")
     p_fp32 = 148 * FP32_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     in_step = ("project", "bin_sort", "render_map") + (("pose_reduce",) if want_pose else ())
-    if want_pose:
-        stage_ms.setdefault("pose_reduce", 0.0)
     # the step roofline is the work of ALL views of the step against the whole-job time (max over ranks)
     roof, step_roof = roofline_objects(stage_ms, [s for s in in_step if s in stage_ms and stage_ms[s] > 0], B, F, peaks, p_fp32,
                                        p_fp32_meas, ms_per_step, n_views_total=n_views)
