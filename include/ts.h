@@ -65,6 +65,10 @@ const char* ts_strerror(int32_t status);
 /* ---- lifecycle ------------------------------------------------------------------------------------------ */
 int32_t ts_create(int32_t device, ts_ctx** out);
 int32_t ts_destroy(ts_ctx* ctx);
+/* Tracing: with on != 0 every export of this context that enqueues work brackets itself with an NVTX
+ * range named after the call ("ts_project", "ts_bin_sort", ...), so a timeline / `ncu --nvtx` groups the kernels by API
+ * call.  Off by default; without a profiler attached an NVTX call is a no-op stub.  Host-side only, no launch. */
+int32_t ts_set_tracing(ts_ctx* ctx, int32_t on);
 
 /* Bytes of device workspace a frame needs for M faces, a WxH image, at most `pair_capacity` (tile, face)
  * pairs (< 2^28) and at most `visible_capacity` faces surviving the cull (0 = M; < 2^28).  About 208 B per pair

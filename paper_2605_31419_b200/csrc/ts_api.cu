@@ -79,8 +79,14 @@ int32_t ts_create(int32_t device, ts_ctx** out) {
     if (cudaGetDeviceProperties(&p, device) != cudaSuccess) return TS_ERR_CUDA;
     ts_ctx* c = new (std::nothrow) ts_ctx;
     if (!c) return TS_ERR_CUDA;
-    c->device = device, c->num_sms = p.multiProcessorCount, c->max_smem_optin = (int)p.sharedMemPerBlockOptin;
+    c->device = device, c->num_sms = p.multiProcessorCount, c->max_smem_optin = (int)p.sharedMemPerBlockOptin, c->tracing = 0;
     *out = c;
+    return TS_OK;
+}
+
+int32_t ts_set_tracing(ts_ctx* ctx, int32_t on) {
+    if (!ctx) return TS_ERR_INVALID_ARG;
+    ctx->tracing = on ? 1 : 0;
     return TS_OK;
 }
 
@@ -99,6 +105,7 @@ size_t ts_frame_bytes(const ts_ctx* ctx, int32_t M, int32_t W, int32_t H, uint64
 
 int32_t ts_frame_bind(ts_ctx* ctx, void* dev_ws, size_t bytes, int32_t M, int32_t W, int32_t H, uint64_t pair_capacity,
                       uint64_t visible_capacity, void* stream, ts_frame** out) {
+    TS_TRACE(ctx);
     if (!out || !dev_ws) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     Layout L;
@@ -164,6 +171,7 @@ int32_t ts_frame_release(ts_frame* frame) {
 }
 
 int32_t ts_frame_status(ts_ctx* ctx, ts_frame* fr, uint32_t* flags, uint32_t* n_visible, uint64_t* n_pairs, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !fr) return TS_ERR_INVALID_ARG;
     TsCtrl h;
     if (cudaMemcpyAsync(&h, fr->d.ctrl, sizeof(TsCtrl), cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess ||
@@ -177,6 +185,7 @@ int32_t ts_frame_status(ts_ctx* ctx, ts_frame* fr, uint32_t* flags, uint32_t* n_
 
 int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const ts_params* prm, const float* T_cw_dev,
                    ts_frame* fr, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !cam || !prm || !T_cw_dev || !fr || !sc->pos || !sc->opacity) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M || cam->width != fr->d.W || cam->height != fr->d.H) return TS_ERR_INVALID_ARG;
@@ -203,6 +212,7 @@ int32_t ts_project(ts_ctx* ctx, const ts_scene* sc, const ts_camera* cam, const 
 }
 
 int32_t ts_bin_sort(ts_ctx* ctx, ts_frame* fr, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !fr) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (!fr->have_project) return TS_ERR_STATE;
@@ -215,6 +225,7 @@ int32_t ts_bin_sort(ts_ctx* ctx, ts_frame* fr, void* stream) {
 
 int32_t ts_render_fwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
                       float* out_alpha, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -228,6 +239,7 @@ int32_t ts_render_fwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_
 int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth, float* out_alpha,
                          const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
                          void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !Chat || !Dhat || !gC || !gD) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -240,6 +252,7 @@ int32_t ts_render_fwd_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* o
 
 int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
                             float* out_alpha, uint32_t* face_pixels, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !face_pixels) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -252,6 +265,7 @@ int32_t ts_render_fwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float
 
 int32_t ts_render_fwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
                              float* out_alpha, float* out_normal, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !out_normal) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -264,6 +278,7 @@ int32_t ts_render_fwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, floa
 
 int32_t ts_render_fwd_normal_top(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth,
                                  float* out_alpha, float* out_normal, float* out_normal_top, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !out_normal_top) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -278,6 +293,7 @@ int32_t ts_render_fwd_normal_top(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, 
 int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
                              const float* dL_dalpha, const float* dL_dnormal, float* grad_pos, float* grad_color,
                              float* grad_opacity, uint32_t grad_mask, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !dL_dnormal) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -291,6 +307,7 @@ int32_t ts_render_bwd_normal(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, cons
 }
 
 int32_t ts_face_area(ts_ctx* ctx, ts_frame* fr, float* proj_area, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !fr || !proj_area) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (!fr->have_sort) return TS_ERR_STATE;              // the visible count is published by ts_bin_sort
@@ -300,6 +317,7 @@ int32_t ts_face_area(ts_ctx* ctx, ts_frame* fr, float* proj_area, void* stream) 
 int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth, float* out_alpha,
                            const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
                            void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !Chat || !Dhat) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -312,6 +330,7 @@ int32_t ts_render_track_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float*
 int32_t ts_render_map_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* out_color, float* out_depth, float* out_alpha,
                          const float* Chat, const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
                          float* grad_pos, float* grad_color, float* grad_opacity, uint32_t grad_mask, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !Chat || !Dhat) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -329,6 +348,7 @@ int32_t ts_render_map_l1(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, float* o
 int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
                       const float* dL_dalpha, float* grad_pos, float* grad_color, float* grad_opacity,
                       uint32_t grad_mask, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !sc->pos) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -344,6 +364,7 @@ int32_t ts_render_bwd(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float
 int32_t ts_render_bwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const float* dL_dcolor, const float* dL_ddepth,
                             const float* dL_dalpha, float* grad_pos, float* grad_color, float* grad_opacity,
                             uint32_t grad_mask, float* face_grad2d, uint32_t* face_views, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !fr || !sc->color || !sc->pos || !face_grad2d) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->M != fr->d.M) return TS_ERR_INVALID_ARG;
@@ -358,6 +379,7 @@ int32_t ts_render_bwd_stats(ts_ctx* ctx, const ts_scene* sc, ts_frame* fr, const
 }
 
 int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !fr || !dL_dtau_dev) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, nullptr, nullptr, nullptr, 0.f, 0.f, 0.f, (cudaStream_t)stream);
@@ -365,12 +387,14 @@ int32_t ts_pose_jacobian_reduce(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, v
 
 int32_t ts_pose_reduce_step(ts_ctx* ctx, ts_frame* fr, float* dL_dtau_dev, float* T_cw_dev, float* state_dev,
                             const float* lr6, float beta1, float beta2, float eps, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !fr || !dL_dtau_dev || !T_cw_dev || !state_dev || !lr6) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     return ts_launch_pose_reduce(ctx, fr, dL_dtau_dev, T_cw_dev, state_dev, lr6, beta1, beta2, eps, (cudaStream_t)stream);
 }
 
 int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev_ptr, size_t* count, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !fr || !dev_ptr || !count) return TS_ERR_INVALID_ARG;
     TsCtrl h;
     if (cudaMemcpyAsync(&h, fr->d.ctrl, sizeof(TsCtrl), cudaMemcpyDeviceToHost, (cudaStream_t)stream) != cudaSuccess ||

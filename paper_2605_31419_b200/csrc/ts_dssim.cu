@@ -219,6 +219,7 @@ dssim_fused_kernel(int W, int H, const float* __restrict__ X, const float* __res
 
 extern "C" int32_t ts_dssim_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* Chat, float lambda,
                                       float* gC, float* loss_dev, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || W <= 0 || H <= 0 || !C || !Chat || !gC || !(lambda >= 0.0f) || !(lambda <= 1.0f))
         return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;

@@ -139,6 +139,7 @@ normal_loss_grad_kernel(size_t n, const float* __restrict__ N, const float* __re
 
 extern "C" int32_t ts_normal_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* N, const float* Nbar, float weight,
                                        float* gN, float* loss_dev, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || W <= 0 || H <= 0 || !N || !Nbar || !gN) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H;
@@ -150,6 +151,7 @@ extern "C" int32_t ts_normal_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const 
 
 extern "C" int32_t ts_equi_loss_grad(ts_ctx* ctx, const ts_scene* sc, float weight, float* grad_pos, float* loss_dev,
                                      void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !sc || !sc->pos || sc->M <= 0 || (!grad_pos && !loss_dev)) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     if (sc->faces == nullptr && sc->V != 3 * sc->M) return TS_ERR_INVALID_ARG;
@@ -166,6 +168,7 @@ extern "C" int32_t ts_equi_loss_grad(ts_ctx* ctx, const ts_scene* sc, float weig
 extern "C" int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const float* C, const float* D, const float* Chat,
                                    const float* Dhat, float lambda_dep, float* gC, float* gD, float* loss_dev,
                                    void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || W <= 0 || H <= 0 || !C || !D || !Chat || !Dhat || !gC || !gD) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H;
@@ -178,6 +181,7 @@ extern "C" int32_t ts_l1_loss_grad(ts_ctx* ctx, int32_t W, int32_t H, const floa
 
 extern "C" int32_t ts_pose_step(ts_ctx* ctx, float* T_cw_dev, const float* dL_dtau_dev, float* state_dev,
                                 const float* lr6, float beta1, float beta2, float eps, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !T_cw_dev || !dL_dtau_dev || !state_dev || !lr6) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     TsLr6 lr;
@@ -212,6 +216,7 @@ __global__ void __launch_bounds__(256) depth_normalise_bwd_kernel(size_t n, cons
 
 extern "C" int32_t ts_depth_normalise(ts_ctx* ctx, int32_t W, int32_t H, const float* D, const float* A, float eps, float* Dn,
                                       void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || W <= 0 || H <= 0 || !D || !A || !Dn || !(eps >= 0.0f)) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H;
@@ -223,6 +228,7 @@ extern "C" int32_t ts_depth_normalise(ts_ctx* ctx, int32_t W, int32_t H, const f
 
 extern "C" int32_t ts_depth_normalise_bwd(ts_ctx* ctx, int32_t W, int32_t H, const float* D, const float* A, float eps,
                                           const float* gDn, float* gD, float* gA, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || W <= 0 || H <= 0 || !D || !A || !gDn || !gD || !gA || !(eps >= 0.0f)) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const size_t n = (size_t)W * H;
@@ -248,6 +254,7 @@ __global__ void __launch_bounds__(1024) fp32_probe_kernel(int iters, float a, fl
 }  // namespace
 
 extern "C" int32_t ts_fp32_probe(ts_ctx* ctx, int32_t iters, float* scratch_dev, uint64_t* flops_out, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || iters <= 0 || !scratch_dev || !flops_out) return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;
     const int grid = ctx->num_sms * 2;
@@ -348,6 +355,7 @@ __global__ void __launch_bounds__(256) unpack_rgbd_kernel(size_t n, const uint8_
 
 extern "C" int32_t ts_unpack_rgbd(ts_ctx* ctx, int32_t W, int32_t H, const uint8_t* rgb_dev, const uint16_t* depth_dev,
                                   float depth_scale, float* Chat, float* Dhat, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || W <= 0 || H <= 0 || (!rgb_dev && !depth_dev) || (rgb_dev && !Chat) || (depth_dev && (!Dhat || !(depth_scale > 0.0f))))
         return TS_ERR_INVALID_ARG;
     if (!on_ctx_device(ctx)) return TS_ERR_INVALID_ARG;

@@ -2,6 +2,7 @@
 // Shares nothing with oracle/ (the CPU oracle): no header, helper, table or constant generator.
 #pragma once
 #include <cuda_runtime.h>
+#include <nvtx3/nvToolsExt.h>
 #include <stdint.h>
 
 #include "../../include/ts.h"
@@ -77,6 +78,7 @@ struct ts_ctx {
     int device;
     int num_sms;
     int max_smem_optin;
+    int tracing;             // ts_set_tracing: every launching export brackets itself with an NVTX range named after it
 };
 struct ts_frame {
     TsFrameDev d;
@@ -100,6 +102,22 @@ inline bool on_ctx_device(const ts_ctx* ctx) {
     int cur = -1;
     return ctx && cudaGetDevice(&cur) == cudaSuccess && cur == ctx->device;
 }
+
+// NVTX range around one export (tracing): pushed on entry and popped on every return path when the
+// context has tracing on; nothing but a load and a branch otherwise.  The range covers the HOST side of the call (argument
+// checks and the enqueue); a profiler attributes the kernels launched inside it to the range.
+struct TsTraceRange {
+    bool on;
+    TsTraceRange(const ts_ctx* ctx, const char* name) : on(ctx && ctx->tracing) {
+        if (on) nvtxRangePushA(name);
+    }
+    ~TsTraceRange() {
+        if (on) nvtxRangePop();
+    }
+    TsTraceRange(const TsTraceRange&) = delete;
+    TsTraceRange& operator=(const TsTraceRange&) = delete;
+};
+#define TS_TRACE(ctx) TsTraceRange ts_trace_range__((ctx), __func__)
 
 #define TS_CUDA_CHECK_LAUNCH()                              \
     do {                                                    \

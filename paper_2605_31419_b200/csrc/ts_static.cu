@@ -69,6 +69,7 @@ uint64_t fitting_pair_capacity(const ts_ctx* ctx, int32_t M, int32_t W, int32_t 
 extern "C" int32_t ts_render_fwd_static(ts_ctx* ctx, const ts_scene* scene, const ts_camera* cam, const ts_params* prm,
                                         const float* T_cw_dev, float* out_color, float* out_depth, float* out_alpha,
                                         uint32_t* status_dev, void* stream) {
+    TS_TRACE(ctx);
     if (!ctx || !scene || !cam || !prm || !T_cw_dev || !scene->pos || !scene->color || !scene->opacity)
         return TS_ERR_INVALID_ARG;
     if (scene->M <= 0 || cam->width <= 0 || cam->height <= 0) return TS_ERR_INVALID_ARG;

@@ -32,7 +32,7 @@ EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame
            "ts_render_fwd_normal", "ts_render_bwd_normal", "ts_normal_loss_grad", "ts_render_bwd_stats",
            "ts_pose_jacobian_reduce", "ts_l1_loss_grad", "ts_dssim_loss_grad", "ts_equi_loss_grad", "ts_pose_step", "ts_pose_reduce_step", "ts_frame_view",
            "ts_fp32_probe", "ts_frame_set_face_sigma", "ts_render_fwd_normal_top", "ts_depth_normalise", "ts_depth_normalise_bwd", "ts_unpack_rgbd",
-           "ts_render_fwd_static"]
+           "ts_render_fwd_static", "ts_set_tracing"]
 
 
 class TsError(RuntimeError):
@@ -117,6 +117,7 @@ def _load():
                                          C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
     lib.ts_frame_release.argtypes = [C.c_void_p]
     lib.ts_destroy.argtypes = [C.c_void_p]
+    lib.ts_set_tracing.argtypes = [C.c_void_p, C.c_int32]
     lib.ts_create.argtypes = [C.c_int32, C.POINTER(C.c_void_p)]
     return lib
 
@@ -146,6 +147,10 @@ class Context:
         h = C.c_void_p()
         _check(lib.ts_create(int(device), C.byref(h)))
         self.h, self.device = h, int(device)
+
+    def set_tracing(self, on=True):
+        """NVTX range per ts_* call of this context (off by default)."""
+        _check(lib.ts_set_tracing(self.h, 1 if on else 0))
 
     def close(self):
         if self.h:

@@ -47,6 +47,9 @@ def test_argument_errors_without_gpu():
     assert ts.lib.ts_render_fwd(None, None, None, None, None, None, None) == ts.ERR_INVALID_ARG
     assert ts.lib.ts_render_bwd(None, None, None, None, None, None, None, None, None, 0, None) == ts.ERR_INVALID_ARG
     assert ts.lib.ts_pose_jacobian_reduce(None, None, None, None) == ts.ERR_INVALID_ARG
+    assert ts.lib.ts_set_tracing(None, 1) == ts.ERR_INVALID_ARG
+    assert ts.lib.ts_render_fwd_static(None, None, None, None, None, None, None, None, None, None) == ts.ERR_INVALID_ARG
+    assert b"built-in workspace" in ts.lib.ts_strerror(ts.ERR_STATIC_LIMIT)
 
 
 def test_no_cpu_fallback_and_no_oracle_in_product():

@@ -443,6 +443,29 @@ def test_helper_exports_refuse_a_context_of_another_device():
         c.close()
 
 
+def test_tracing_ranges_do_not_change_results():
+    """ts_set_tracing: with NVTX ranges on, every call still returns the same status and the same bits (the ranges are
+    host-side brackets; without a profiler attached they are stubs)."""
+    from gpu_util import GpuView
+    from paper_2605_31419_b200 import ts
+    sc = scenes.config0()
+    outs = []
+    for on in (False, True, False):
+        c = ts.Context(0)
+        c.set_tracing(on)
+        g = GpuView(c, sc.pos, sc.color, sc.opacity, None, sc.T_start[0], sc.cam, sc.params)
+        C, D, A = g.forward()
+        gp, gc, go, tau = g.backward(np.ones_like(C), np.ones_like(D), None, ts.GRAD_POSE)
+        with pytest.raises(ts.TsError):                      # an error return inside a range still pops it
+            ts.ts_render_bwd(c, g.scene, g.frame, None, None, None, None, None, None, 1 << 9)
+        outs.append((C, D, A, tau))
+        g.close()
+        c.close()
+    for o in outs[1:]:
+        for a, b in zip(outs[0], o):
+            assert np.array_equal(a, b)
+
+
 def test_face_area_needs_the_sort(ctx, oracle_mod):
     """ts_face_area reads the visible count ts_bin_sort publishes: TS_ERR_STATE between ts_project and ts_bin_sort."""
     from gpu_util import GpuView
