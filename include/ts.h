@@ -310,9 +310,13 @@ enum { TS_VIEW_VIS = 0,          /* u32[n_visible][16]: per visible face, in slo
        TS_VIEW_JOBS = 6,         /* u32[8 NT][4] job headers of the render kernels, in ticket order: (tile | block << 28,
                                     begin, end, x0 | y0 << 16); block b = 2 row + column of the tile's 2 x 4 blocks of
                                     8x4 pixels; [begin, end) indexes TS_VIEW_BLOCK_LISTS in entries of four u32        */
-       TS_VIEW_BLOCK_LISTS = 7 };/* u32[8 n_pairs][4]: the per-block lists: for every job the entries (slot, face,
+       TS_VIEW_BLOCK_LISTS = 7,  /* u32[8 n_pairs][4]: the per-block lists: for every job the entries (slot, face,
                                     rect_lo, rect_hi) of its tile's sorted list whose pixel rect overlaps the block, in
                                     list order (only the ranges named by the job headers are defined)                  */
+       TS_VIEW_TIMELINE = 8 };   /* u32[8 NT][4], profiling builds only (compiled with -DTS_JOB_TIMELINE by
+                                    paper_2605_31419_b200/timeline.py; TS_ERR_STATE in the normal library): per job of
+                                    the last ts_render_track_l1, in ticket order like TS_VIEW_JOBS: (%globaltimer at
+                                    start, at end [low 32 bits, ns], list length, persistent warp that ran it)         */
 /* Synchronises `stream`; returns the device pointer and element count of an internal array. */
 int32_t ts_frame_view(ts_ctx* ctx, ts_frame* frame, int32_t which, const void** dev_ptr, size_t* count,
                       void* stream);

@@ -29,6 +29,30 @@ def _stale():
     return any(os.path.getmtime(d) > os.path.getmtime(SO) for d in deps)
 
 
+def build_variant(name: str, defines) -> str:
+    """Another build of the same sources with extra -D flags (e.g. the job-timeline build of timeline.py): objects under
+    build/<name>/, library libts_<name>.so next to libts.so.  The product library is not touched."""
+    out_dir = os.path.join(HERE, "..", "build", name)
+    os.makedirs(out_dir, exist_ok=True)
+    so = os.path.join(HERE, f"libts_{name}.so")
+    objs = []
+    for src in sources():
+        obj = os.path.join(out_dir, os.path.basename(src)[:-3] + ".o")
+        fmad = FMAD.get(os.path.basename(src), "--fmad=true")
+        flags = [f for f in FLAGS if f not in ("-Xptxas", "-v")]
+        r = subprocess.run([NVCC, *flags, *[f"-D{d}" for d in defines], fmad, "-c", src, "-o", obj], capture_output=True, text=True)
+        if r.returncode != 0:
+            sys.stderr.write(r.stdout + r.stderr)
+            raise RuntimeError(f"nvcc failed on {src}")
+        objs.append(obj)
+    r = subprocess.run([NVCC, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", so, *objs, "-lcudart", "-ldl"],
+                       capture_output=True, text=True)
+    if r.returncode != 0:
+        sys.stderr.write(r.stdout + r.stderr)
+        raise RuntimeError("link failed")
+    return so
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return SO

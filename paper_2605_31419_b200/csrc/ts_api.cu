@@ -429,6 +429,14 @@ int32_t ts_frame_view(ts_ctx* ctx, ts_frame* fr, int32_t which, const void** dev
             if (!fr->have_sort) return TS_ERR_STATE;
             *dev_ptr = d.blist, *count = 4 * 8 * np;
             break;
+        case TS_VIEW_TIMELINE:
+#ifdef TS_JOB_TIMELINE
+            if (!fr->have_sort || (size_t)d.W * d.H < 32u * (size_t)d.NT) return TS_ERR_STATE;
+            *dev_ptr = d.n_contrib_view, *count = 4 * 8 * (size_t)d.NT;
+            break;
+#else
+            return TS_ERR_STATE;                             // not an instrumented build
+#endif
         default: return TS_ERR_INVALID_ARG;
     }
     return TS_OK;

@@ -37,6 +37,23 @@ __device__ __forceinline__ uint32_t ts_job_take(const TsFrameDev& f, int which, 
     return ts_job_ticket(ts_job_request(f, which, lane));
 }
 
+// When is the NEXT ticket taken?  Requesting it at the start of the current job hides the atomic's round trip, but it also
+// reserves a job for as long as the current one lasts: a warp on a 60 us job sits on a mid-list ticket all that time and
+// runs it afterwards, and at the end of the launch every warp still owes "this job + one reserved job" (measured at config
+// 2, profiles/r03_timeline_config2.md: first warp out of work at 71 us, last job finished at 85 us).  So the request is made
+// early only where the reservation is short and harmless -- the current job's list has at most TS_PREFETCH_MAX_LEN entries
+// and the ticket is not among the last TS_TAIL_ROUNDS x (persistent warps) -- and at the END of the job otherwise (a long
+// job does not notice one exposed round trip; in the tail, finishing order matters more than latency).  Warp-uniform.
+#ifndef TS_PREFETCH_MAX_LEN
+#define TS_PREFETCH_MAX_LEN 8u
+#endif
+#ifndef TS_TAIL_ROUNDS
+#define TS_TAIL_ROUNDS 4u
+#endif
+__device__ __forceinline__ bool ts_job_prefetch_next(uint32_t j, uint32_t n_jobs, uint32_t list_len, uint32_t total_warps) {
+    return list_len <= TS_PREFETCH_MAX_LEN && j + TS_TAIL_ROUNDS * total_warps < n_jobs;
+}
+
 // total = persistent warps of the launch
 __device__ __forceinline__ void ts_job_finish_n(const TsFrameDev& f, int which, int lane, uint32_t total) {
     if (lane == 0) {

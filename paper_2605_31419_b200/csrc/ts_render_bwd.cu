@@ -55,7 +55,8 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
             if (gAi) gA = gAi[p];
             if (NRM) gN0 = gNi[p], gN1 = gNi[hw + p], gN2 = gNi[2 * hw + p];
         }
-        const uint32_t j_next = ts_job_request(f, 1, lane);   // next ticket: read at the end of this job
+        const bool pre = ts_job_prefetch_next(j, n_jobs, job.range.y - job.range.x, gridDim.x * TS_JOB_WARPS);
+        const uint32_t j_next = pre ? ts_job_request(f, 1, lane) : 0u;   // next ticket: early (read at the end of this job) or late
         float tau[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         ts_bwd_walk<SM, ATTR, GEOM, POSE, NRM>(f, sc, job, lane, sm, sigma, alpha_min, fx, fy, ncon, Tcur, gC0, gC1, gC2, gD, gA,
                                                grad_color, grad_opacity, tau, gN0, gN1, gN2, 0xffffffffu, grad_sigma);
@@ -71,7 +72,7 @@ render_bwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                 f.pose_partials[6 * ((size_t)job.tile * TS_BLOCKS_PER_TILE + job.blk) + lane] = v;
             }
         }
-        j = ts_job_ticket(j_next);
+        j = pre ? ts_job_ticket(j_next) : ts_job_take(f, 1, lane);
     }
     ts_job_finish(f, 1, lane);
 }
@@ -109,11 +110,17 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
 
     uint32_t j = ts_job_take(f, 0, lane);
     while (j < n_jobs) {
+#ifdef TS_JOB_TIMELINE
+        // instrumented build only (paper_2605_31419_b200/timeline.py): when did this warp start and finish job j
+        unsigned long long tl_t0;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_t0));
+#endif
         TsJob job;
         ts_job_decode(f, j, lane, job);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
         if (job.range.x + lane < job.range.y) ent = f.blist[job.range.x + lane];
-        const uint32_t j_next = ts_job_request(f, 0, lane);   // next ticket: read at the end of this job
+        const bool pre = ts_job_prefetch_next(j, n_jobs, job.range.y - job.range.x, gridDim.x * TS_JOB_WARPS);
+        const uint32_t j_next = pre ? ts_job_request(f, 0, lane) : 0u;   // next ticket: early (read at the end of this job) or late
         FwdPix o;
         // the chunk the forward walk staged last (with the whole record) is where the backward walk begins
         uint32_t staged_lo = 0xffffffffu;
@@ -155,7 +162,18 @@ render_track_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, flo
             }
         }
         __syncwarp();
-        j = ts_job_ticket(j_next);
+#ifdef TS_JOB_TIMELINE
+        {
+            unsigned long long tl_t1;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(tl_t1));
+            // (start ns, end ns, list length, persistent warp) per ticket; TS_VIEW_TIMELINE; the array is the scratch of
+            // TS_VIEW_N_CONTRIB, which the fused kernels never touch
+            if (lane == 0)
+                reinterpret_cast<uint4*>(f.n_contrib_view)[j] = make_uint4((uint32_t)tl_t0, (uint32_t)tl_t1, job.range.y - job.range.x,
+                                                                           blockIdx.x * TS_JOB_WARPS + (threadIdx.x >> 5));
+        }
+#endif
+        j = pre ? ts_job_ticket(j_next) : ts_job_take(f, 0, lane);
     }
     ts_job_finish(f, 0, lane);
     if (loss) {

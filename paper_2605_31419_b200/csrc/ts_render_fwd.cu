@@ -41,7 +41,8 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
         ts_job_decode(f, j, lane, job);
         uint4 ent = make_uint4(0u, 0u, 0u, 0u);
         if (job.range.x + lane < job.range.y) ent = f.blist[job.range.x + lane];
-        const uint32_t j_next = ts_job_request(f, 0, lane);   // next ticket: read at the end of this job
+        const bool pre = ts_job_prefetch_next(j, n_jobs, job.range.y - job.range.x, gridDim.x * TS_JOB_WARPS);
+        const uint32_t j_next = pre ? ts_job_request(f, 0, lane) : 0u;   // next ticket: early (read at the end of this job) or late
         FwdPix o;
         ts_fwd_walk<SM, COUNT, STATS, NRM>(f, sc, job, lane, sm, sigma, alpha_min, t_min, ent, o, n_visit, n_rect, n_hit, face_pixels,
                                            smem_n + (NRM ? (threadIdx.x & ~31) : 0));
@@ -74,7 +75,7 @@ render_fwd_kernel(TsFrameDev f, ts_scene sc, float sigma, float alpha_min, float
                 L.gD[p] = g;
             }
         }
-        j = ts_job_ticket(j_next);
+        j = pre ? ts_job_ticket(j_next) : ts_job_take(f, 0, lane);
     }
     ts_job_finish(f, 0, lane);
     if (LOSS && L.loss) {

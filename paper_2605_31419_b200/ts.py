@@ -12,7 +12,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libts.so")
+# TS_LIBTS: path of another build of the same sources (the profiling build of timeline.py); unset = the product library
+_SO = os.environ.get("TS_LIBTS") or os.path.join(_HERE, "libts.so")
 
 OK, ERR_INVALID_ARG, ERR_WORKSPACE, ERR_CAPACITY, ERR_CUDA, ERR_STATE, ERR_STATIC_LIMIT = 0, -1, -2, -3, -4, -5, -6
 STATIC_WS_BYTES, STATIC_MAX_FACES, STATIC_MAX_PIXELS = 4 << 20, 4096, 16384   # ts_render_fwd_static (include/ts.h)
@@ -22,10 +23,10 @@ FLAG_OVERFLOW_PAIRS, FLAG_OVERFLOW_VISIBLE = 1, 2
 PARAM_COUNTERS = 0x100   # ts_params.flags: count visits / rect tests / hits (debug instantiation)
 PARAM_MIN_OPACITY = 0x200   # ts_params.flags: face opacity = min instead of mean of the vertex opacities (ablation)
 PARAM_TIGHT_BINNING = 0x400  # ts_params.flags: bin a face only into the tiles its triangle meets (reading S31)
-VIEW_VIS, VIEW_KEYS, VIEW_VALS, VIEW_TILE_RANGES, VIEW_N_CONTRIB, VIEW_COUNTERS, VIEW_JOBS, VIEW_BLOCK_LISTS = range(8)
+VIEW_VIS, VIEW_KEYS, VIEW_VALS, VIEW_TILE_RANGES, VIEW_N_CONTRIB, VIEW_COUNTERS, VIEW_JOBS, VIEW_BLOCK_LISTS, VIEW_TIMELINE = range(9)
 _VIEW_DTYPES = {VIEW_VIS: torch.int32, VIEW_KEYS: torch.int64, VIEW_VALS: torch.int32,
                 VIEW_TILE_RANGES: torch.int32, VIEW_N_CONTRIB: torch.int32, VIEW_COUNTERS: torch.int64,
-                VIEW_JOBS: torch.int32, VIEW_BLOCK_LISTS: torch.int32}
+                VIEW_JOBS: torch.int32, VIEW_BLOCK_LISTS: torch.int32, VIEW_TIMELINE: torch.int32}
 
 EXPORTS = ["ts_strerror", "ts_create", "ts_destroy", "ts_frame_bytes", "ts_frame_bind", "ts_frame_release",
            "ts_frame_status", "ts_project", "ts_bin_sort", "ts_render_fwd", "ts_render_fwd_l1", "ts_render_track_l1", "ts_render_map_l1", "ts_render_fwd_stats", "ts_face_area", "ts_render_bwd",

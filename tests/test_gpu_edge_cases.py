@@ -84,6 +84,8 @@ def test_n_contrib_view_needs_a_forward_render_on_the_current_sort(ctx):
         g.view(ts.VIEW_N_CONTRIB)
     g.forward()
     assert g.view(ts.VIEW_N_CONTRIB).shape == nc.shape
+    with pytest.raises(ts.TsError, match="out of order"):
+        g.view(ts.VIEW_TIMELINE)                     # only the profiling build (timeline.py) has job stamps
     g.close()
 
 
