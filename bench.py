@@ -794,7 +794,7 @@ def bench_mapping(args, torch, ts, scenes, dist, rank, world, local):
     in_step = ("project", "bin_sort", "render_map") + (("pose_reduce",) if want_pose else ())
     # the step roofline is the work of ALL views of the step against the whole-job time (max over ranks)
     roof, step_roof = roofline_objects(stage_ms, [s for s in in_step if s in stage_ms and stage_ms[s] > 0], B, F, peaks, p_fp32,
-                                       p_fp32_meas, ms_per_step, n_views_total=n_views)
+                                       p_fp32_meas, ms_per_step, n_views_total=n_views, config=args.config)
     step_roof["note"] = ("bytes / flops of view 0 x the number of views; with N ranks the bound is that work at ONE GPU's "
                          "peaks, so the fraction can exceed what one GPU could reach")
     out = {"metric": METRIC, "value": value, "unit": "Mpix/s", "n_gpus": world, "steps": args.steps,

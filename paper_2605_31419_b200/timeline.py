@@ -9,9 +9,12 @@ iterations of the BASELINE config on cuda:0, then one stamped launch, and writes
   <out>_warps.csv   one row per persistent warp: jobs run, first start, last end, busy time
   <out>.md          the figures the bound is made of: launch span, instant until which every warp is busy, drain, the
                     longest jobs, and span >= max(longest job, total busy time / number of warps).
-The stamps cost two timer reads and one 16-byte store per job (25 800 jobs at config 2): the stamped launch is within a
-few per cent of the product kernel; its time is reported, never used as a benchmark value.  Argument marshalling and
-bookkeeping only: nothing of the method is computed here.
+The stamps cost two timer reads and one 16-byte store per job (25 800 jobs at config 2) and the stamped launch is slower
+than the product kernel (config 2: about 100 us against 89 us by CUDA events), so its time is reported and never used as
+a benchmark value: what the stamps show is how the work is DISTRIBUTED over the warps.  --define NAME=VALUE adds compile
+definitions to the profiling build, e.g. the ticket policy before round 3 (every warp requests its next ticket at the
+start of the current job):  --define TS_PREFETCH_MAX_LEN=0x40000000u --define TS_TAIL_ROUNDS=0u --tag prefetch_always.
+Argument marshalling and bookkeeping only: nothing of the method is computed here.
 """
 from __future__ import annotations
 
@@ -27,10 +30,12 @@ def main():
     ap.add_argument("--config", type=int, default=2, choices=[1, 2])
     ap.add_argument("--out", default="gpurun_out/timeline")
     ap.add_argument("--warmup", type=int, default=40)
+    ap.add_argument("--define", action="append", default=[], help="extra NAME=VALUE compile definition (repeatable)")
+    ap.add_argument("--tag", default="", help="suffix of the profiling build's name when --define is used")
     args = ap.parse_args()
 
     from paper_2605_31419_b200 import build
-    os.environ["TS_LIBTS"] = build.build_variant("timeline", ["TS_JOB_TIMELINE"])
+    os.environ["TS_LIBTS"] = build.build_variant("timeline" + ("_" + args.tag if args.tag else ""), ["TS_JOB_TIMELINE", *args.define])
     import torch
     from paper_2605_31419_b200 import scenes, ts
 
@@ -92,7 +97,8 @@ def main():
     order = np.argsort(-dur)[:20]
     with open(args.out + ".md", "w") as fh:
         fh.write(f"# Job timeline of render_track_kernel, config {args.config} ({sc.M} faces, {W}x{H})\n\n")
-        fh.write(f"Command: `python -m paper_2605_31419_b200.timeline --config {args.config} --out {args.out}` "
+        extra = "".join(f" --define {d}" for d in args.define) + (f" --tag {args.tag}" if args.tag else "")
+        fh.write(f"Command: `python -m paper_2605_31419_b200.timeline --config {args.config}{extra} --out {args.out}` "
                  f"(profiling build -DTS_JOB_TIMELINE; rows: `{os.path.basename(args.out)}_jobs.csv`, "
                  f"`{os.path.basename(args.out)}_warps.csv`).\n\n")
         fh.write("| quantity | value |\n|---|---|\n")
